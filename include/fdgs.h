@@ -1,0 +1,152 @@
+/* fdgs.h — C ABI of the B200-native time-sliced tile rasterizer for native 4D Gaussians.
+ *
+ * Method: "4D Gaussian Splatting: Modeling Dynamic Scenes with Native 4D Primitives"
+ * (arxiv 2412.20720).  Citations below are PAPER.md:L<line> of the extracted paper text.
+ *
+ * Everything behind these entry points is hand-written CUDA for sm_100a (no CPU fallback, no
+ * library kernels).  The library never allocates device memory, never throws across the ABI and
+ * never synchronises the stream unless a `_host` out-pointer is given.
+ *
+ * Conventions
+ *   - Every pointer is a DEVICE pointer unless its name ends in `_host`.  fdgs_view and
+ *     fdgs_config are small HOST structs passed by pointer and copied into kernel parameters.
+ *   - All arrays are contiguous fp32 unless stated; base pointers must be 16-byte aligned.
+ *   - The caller owns every buffer, including the workspace `ws` (e.g. a torch uint8 tensor),
+ *     which is the only state carried between calls.  Call order on one `ws` and one stream:
+ *         fdgs_preprocess -> fdgs_render_forward -> fdgs_render_backward
+ *     with the same scene, view, config and pair_capacity (they define the workspace layout).
+ *   - Return value: 0 = OK, <0 = error (fdgs_strerror).
+ */
+#ifndef FDGS_H
+#define FDGS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FDGS_OK 0
+#define FDGS_ERR_INVALID (-1)       /* NULL / misaligned pointer, N<0, sh_degree not in 0..3, n_time<1, W/H<=0 ... */
+#define FDGS_ERR_WORKSPACE (-2)     /* ws_bytes smaller than fdgs_workspace_bytes() says                            */
+#define FDGS_ERR_CUDA (-3)          /* CUDA runtime error (text via fdgs_strerror)                                  */
+#define FDGS_ERR_PAIR_OVERFLOW (-4) /* number of (tile, primitive) pairs D exceeded pair_capacity                   */
+
+#define FDGS_TILE 16 /* 16x16-pixel tiles (tile rasterizer of [23]) */
+
+/* A scene = N 4D Gaussians.  K = n_time * (sh_degree+1)^2. */
+typedef struct {
+  int32_t N;                  /* number of primitives, >= 0                                             */
+  int32_t sh_degree;          /* spatial SH degree L in 0..3                                            */
+  int32_t n_time;             /* Fourier orders n = 0..n_time-1 of the 4DSH (eq. 20), >= 1        */
+  const float *mean;          /* [N,4]  (mu_x, mu_y, mu_z, mu_t)                               L135     */
+  const float *log_scale;     /* [N,4]  S = diag(exp(.)), order (x,y,z,t)                      L128     */
+  const float *quat_l;        /* [N,4]  q_l = (a,b,c,d), need not be unit (normalised inside)  L128     */
+  const float *quat_r;        /* [N,4]  q_r = (p,q,r,s)                                        L128     */
+  const float *opacity_logit; /* [N]    alpha = sigmoid(.)                                              */
+  const float *sh;            /* [N,K,3] 4DSH coefficients, k = n*(L+1)^2 + l*l + l + m, channel last   */
+} fdgs_scene;
+
+/* One view: extrinsic E = [W | tau] and intrinsic K, query time t, 4DSH period T. */
+typedef struct {
+  float view[16];       /* world -> camera, row-major 4x4 [W tau; 0 0 0 1], +z forward             */
+  float fx, fy, cx, cy; /* pinhole intrinsics in pixels; pixel (i,j) is sampled at (i+0.5, j+0.5)  */
+  int32_t width, height;
+  float t;              /* query time                                                    L108-L113 */
+  float period_T;       /* period T of cos(2 pi n (t - mu_t) / T)                        L187      */
+  float bg[3];          /* background colour composited with the final transmittance               */
+} fdgs_view;
+
+/* Thresholds.  Only marginal_min is the paper's (L324); the rest are the settings of [23] that the
+ * paper adopts without stating (L324) — see DESIGN.md readings S7-S10. */
+typedef struct {
+  float marginal_min;      /* 0.05: cull if exp(-(t-mu_t)^2 / (2 Sigma_44)) < marginal_min; 0 disables (L265) */
+  float alpha_min;         /* 1/255: a splat with alpha < alpha_min is skipped at that pixel                  */
+  float alpha_max;         /* 0.99:  alpha is clamped to alpha_max                                            */
+  float transmittance_min; /* 1e-4:  stop before the splat that would take T below this                       */
+  float dilation;          /* 0.3 px^2 added to the diagonal of Sigma_2d                                      */
+  float cutoff_sigma;      /* 3.0:   support radius = cutoff_sigma * sqrt(lambda_max(Sigma_2d))               */
+  float znear;             /* 0.2:   cull if camera-space depth <= znear                                      */
+  float guard;             /* 1.3:   guard band for the clamped ratios inside the Jacobian J                  */
+} fdgs_config;
+
+/* Gradient buffers, same shapes as the fdgs_scene arrays.  fdgs_render_backward ACCUMULATES (+=)
+ * into them: zero them once per optimisation step and the views of a batch sum (L324 "batch size 4"). */
+typedef struct {
+  float *mean, *log_scale, *quat_l, *quat_r, *opacity_logit, *sh;
+  float *mean2d; /* [N,2] optional (NULL ok): dL/d(u,v), the densification signal (L197) */
+} fdgs_grads;
+
+/* Fills the defaults listed above.  Returns FDGS_ERR_INVALID if cfg is NULL. */
+int fdgs_default_config(fdgs_config *cfg_host);
+
+/* Size of the workspace for a scene of N primitives with K coefficients per channel rendered at
+ * W x H with room for pair_capacity (tile, primitive) pairs (1 <= pair_capacity < 2^30).  W x H is limited to
+ * (ceil(W/16)+1)*(ceil(H/16)+1) <= 50000 tiles (e.g. 3500 x 3500). */
+int fdgs_workspace_bytes(int32_t N, int32_t K, int32_t W, int32_t H, int64_t pair_capacity, size_t *bytes_host);
+
+/* Steps A1-A5: activation and 4D covariance Sigma = R S S^T R^T with R = L(q_l) R(q_r)
+ * (eq. 7-8); time slice mu_xyz|t, Sigma_xyz|t and marginal weight (eq. 9-10)
+ * with the p(t) < marginal_min filter (L324); EWA projection to a 2D conic (eq. 3-4);
+ * 4DSH colour (eq. 20); tiles touched and their exclusive prefix sum.
+ * If num_pairs_host / num_visible_host are non-NULL the stream is synchronised and D / the number
+ * of surviving primitives are returned (and FDGS_ERR_PAIR_OVERFLOW if D > pair_capacity). */
+int fdgs_preprocess(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws,
+                    size_t ws_bytes, int64_t pair_capacity, void *cuda_stream, int64_t *num_pairs_host,
+                    int32_t *num_visible_host);
+
+/* Steps A6-A9: order the (tile, primitive) pairs as a stable sort on the key (tile id << 32 | fp32
+ * depth bits) with ties in primitive-id order would (done two-level: survivors by depth, then pairs by
+ * tile id — DESIGN.md), per-tile ranges, front-to-back alpha compositing of
+ * p_i(t) p_i(u,v|t) alpha_i c_i (eq. 6).  Outputs: image [3,H,W], final_T [H,W] (transmittance
+ * left), n_contrib [H,W] (1 + position in the tile list of the last splat composited).
+ * If D exceeded pair_capacity nothing is drawn (image = bg) and the overflow is reported by
+ * fdgs_debug_export(FDGS_EXPORT_STATUS) or the next synchronising call. */
+int fdgs_render_forward(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws,
+                        size_t ws_bytes, int64_t pair_capacity, void *cuda_stream, float *image, float *final_T,
+                        uint32_t *n_contrib);
+
+/* Steps B1-B2: reverse-order gradient of the compositing, then the chain through projection, 4DSH,
+ * conditioning, Sigma = M M^T and the two quaternions to every parameter (exact derivative of the
+ * forward as stated; zero through active clamps).  Accumulates into grads. */
+int fdgs_render_backward(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws,
+                         size_t ws_bytes, int64_t pair_capacity, void *cuda_stream, const float *dL_dimage,
+                         const float *final_T, const uint32_t *n_contrib, const fdgs_grads *grads_host);
+
+/* Harness-side loss ("rendering loss"): L = mean |image - target| over 3HW values.
+ * Writes dL/dimage [3,H,W] and adds L to *loss (device float, caller zeroes it). */
+int fdgs_l1_loss(const float *image, const float *target, int64_t count, float *dL_dimage, float *loss,
+                 void *cuda_stream);
+
+/* One forward(+backward) pass over one view with HOST target / result buffers: copies target_host
+ * [3,H,W] to `target_dev`, runs preprocess + forward (+ L1 loss + backward if grads_host != NULL),
+ * copies the loss (1 float) — or, when grads_host == NULL, the image — back to the host and
+ * synchronises the stream.  target_host / result_host should be pinned. */
+int fdgs_step_host(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws,
+                   size_t ws_bytes, int64_t pair_capacity, void *cuda_stream, const float *target_host,
+                   float *target_dev, float *image, float *final_T, uint32_t *n_contrib, float *dL_dimage,
+                   float *loss_dev, fdgs_grads *grads_host, float *result_host);
+
+/* Parity hooks: copy one intermediate of the last calls on `ws` to dst (device memory).  Synchronises. */
+#define FDGS_EXPORT_STATUS 0        /* int64[4]: D, num_visible, overflow flag, pair_capacity               */
+#define FDGS_EXPORT_RECORDS 1       /* float[N,12]: u, v, conic A, B, C, opacity o, r, g, b, depth, radius, w */
+#define FDGS_EXPORT_RECTS 2         /* int32[N,4]: tx0, ty0, tx1, ty1 (all 0 for culled primitives)          */
+#define FDGS_EXPORT_TILES_TOUCHED 3 /* uint32[N]                                                             */
+#define FDGS_EXPORT_OFFSETS 4       /* uint32[num_visible] exclusive prefix sum of tiles_touched in depth order */
+#define FDGS_EXPORT_SORTED_KEYS 5   /* uint64[D]                                                             */
+#define FDGS_EXPORT_SORTED_VALS 6   /* uint32[D] primitive ids                                               */
+#define FDGS_EXPORT_RANGES 7        /* uint32[tiles,2]: [first, last+1) into the sorted arrays               */
+#define FDGS_EXPORT_SPLAT_GRADS 8   /* float[N,9]: dL/d(u, v, A, B, C, o, r, g, b) from the last backward    */
+#define FDGS_EXPORT_DEPTH_ORDER 9   /* uint32[num_visible]: ids of the survivors sorted by (depth bits, id)   */
+int fdgs_debug_export(const void *ws, size_t ws_bytes, int what, void *dst, size_t dst_bytes, void *cuda_stream);
+
+/* Number of kernel launches the library has issued so far in this process (bench.py's gpu_launches). */
+int64_t fdgs_launch_count(void);
+
+const char *fdgs_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FDGS_H */

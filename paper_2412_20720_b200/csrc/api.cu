@@ -1,0 +1,300 @@
+// api.cu — the C ABI of include/fdgs.h: argument validation, workspace carve-up, launch sequence.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+
+#include "common.cuh"
+
+namespace fdgs {
+
+static char g_cuda_err[256] = "no CUDA error recorded";
+
+static int cuda_fail(cudaError_t e, const char* where) {
+  snprintf(g_cuda_err, sizeof(g_cuda_err), "CUDA error in %s: %s", where, cudaGetErrorString(e));
+  return FDGS_ERR_CUDA;
+}
+#define FDGS_CUDA(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, where); } while (0)
+
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+static int num_sms() {
+  static int sms = 0;
+  if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); if (sms <= 0) sms = 148; }
+  return sms;
+}
+
+static int ceil_log2(long long v) { int b = 0; while ((1LL << b) < v) ++b; return b; }
+
+static int check_common(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, const void* ws) {
+  if (!sc || !v || !c || !ws) return FDGS_ERR_INVALID;
+  if (sc->N < 0 || sc->sh_degree < 0 || sc->sh_degree > 3 || sc->n_time < 1) return FDGS_ERR_INVALID;
+  if (v->width <= 0 || v->height <= 0 || !(v->fx > 0) || !(v->fy > 0) || !(v->period_T > 0)) return FDGS_ERR_INVALID;
+  if (sc->N > 0) {
+    if (!sc->mean || !sc->log_scale || !sc->quat_l || !sc->quat_r || !sc->opacity_logit || !sc->sh) return FDGS_ERR_INVALID;
+    if (!aligned16(sc->mean) || !aligned16(sc->log_scale) || !aligned16(sc->quat_l) || !aligned16(sc->quat_r) || !aligned16(sc->sh))
+      return FDGS_ERR_INVALID;
+  }
+  if (!aligned16(ws)) return FDGS_ERR_INVALID;
+  const long long tx = (v->width + TILE - 1) / TILE, ty = (v->height + TILE - 1) / TILE;
+  if ((tx + 1) * (ty + 1) > MAX_GRID_CELLS || tx > 65535 || ty > 65535) return FDGS_ERR_INVALID;
+  return FDGS_OK;
+}
+
+static void make_params(const fdgs_view* v, const fdgs_config* c, ViewParams& vp, CfgParams& cp) {
+  for (int r = 0; r < 3; ++r) { for (int q = 0; q < 3; ++q) vp.W[r][q] = v->view[4 * r + q]; vp.tau[r] = v->view[4 * r + 3]; }
+  for (int r = 0; r < 3; ++r) vp.cam[r] = -(vp.W[0][r] * vp.tau[0] + vp.W[1][r] * vp.tau[1] + vp.W[2][r] * vp.tau[2]);
+  vp.fx = v->fx; vp.fy = v->fy; vp.cx = v->cx; vp.cy = v->cy;
+  vp.width = v->width; vp.height = v->height;
+  vp.tiles_x = (v->width + TILE - 1) / TILE; vp.tiles_y = (v->height + TILE - 1) / TILE;
+  vp.t = v->t; vp.inv_T = 1.0f / v->period_T;
+  for (int k = 0; k < 3; ++k) vp.bg[k] = v->bg[k];
+  vp.limx = c->guard * v->width / (2.0f * v->fx); vp.limy = c->guard * v->height / (2.0f * v->fy);
+  cp.marginal_min = c->marginal_min; cp.alpha_min = c->alpha_min; cp.alpha_max = c->alpha_max;
+  cp.transmittance_min = c->transmittance_min; cp.dilation = c->dilation; cp.cutoff_sigma = c->cutoff_sigma;
+  cp.znear = c->znear; cp.guard = c->guard;
+  cp.log2_alpha_min = c->alpha_min > 0.f ? log2f(c->alpha_min) * (1.0f + 1e-6f) - 1e-6f : -INFINITY;
+}
+
+// ---- parity exports -----------------------------------------------------------------------------
+__global__ void export_records_kernel(const SplatRec* __restrict__ rec, const unsigned int* __restrict__ tiles_touched, const int N,
+                                      float* __restrict__ dst) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  float* o = dst + (size_t)12 * i;
+  if (tiles_touched[i] == 0) { for (int k = 0; k < 12; ++k) o[k] = __int_as_float(0x7fc00000); return; }
+  const SplatRec r = rec[i];
+  const float ik = 1.0f / 0.72134752044448170f;     // conic from its exp2-scaled Cholesky factor
+  o[0] = r.u; o[1] = r.v;
+  o[2] = r.ca * r.ca * ik; o[3] = r.ca * r.cb * ik; o[4] = (r.cb * r.cb + r.cc * r.cc) * ik;
+  o[5] = exp2f(r.lo); o[6] = r.r; o[7] = r.g; o[8] = r.b; o[9] = r.depth; o[10] = r.radius; o[11] = r.w;
+}
+__global__ void export_rects_kernel(const ushort4* __restrict__ rect, const int N, int4* __restrict__ dst) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < N) { const ushort4 r = rect[i]; dst[i] = make_int4(r.x, r.y, r.z, r.w); }
+}
+// the literal 64-bit key of every sorted pair: tile id << 32 | fp32 depth bits
+__global__ void export_keys_kernel(const unsigned int* __restrict__ tile_keys, const unsigned int* __restrict__ ids,
+                                   const SplatRec* __restrict__ rec, const unsigned int D, unsigned long long* __restrict__ dst) {
+  const unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < D) dst[i] = ((unsigned long long)tile_keys[i] << 32) | __float_as_uint(rec[ids[i]].depth);
+}
+
+}  // namespace fdgs
+
+using namespace fdgs;
+
+extern "C" {
+
+int fdgs_default_config(fdgs_config* c) {
+  if (!c) return FDGS_ERR_INVALID;
+  c->marginal_min = 0.05f; c->alpha_min = 1.0f / 255.0f; c->alpha_max = 0.99f; c->transmittance_min = 1e-4f;
+  c->dilation = 0.3f; c->cutoff_sigma = 3.0f; c->znear = 0.2f; c->guard = 1.3f;
+  return FDGS_OK;
+}
+
+int fdgs_workspace_bytes(int32_t N, int32_t K, int32_t W, int32_t H, int64_t pair_capacity, size_t* bytes_host) {
+  if (!bytes_host || N < 0 || K < 1 || W <= 0 || H <= 0 || pair_capacity < 1 || pair_capacity >= (1LL << 30)) return FDGS_ERR_INVALID;
+  *bytes_host = carve(nullptr, N, K, W, H, pair_capacity).bytes;
+  return FDGS_OK;
+}
+
+int fdgs_preprocess(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
+                    int64_t cap, void* stream, int64_t* num_pairs_host, int32_t* num_visible_host) {
+  int rc = check_common(sc, v, c, ws_ptr);
+  if (rc) return rc;
+  if (cap < 1 || cap >= (1LL << 30)) return FDGS_ERR_INVALID;
+  const int K = sc->n_time * (sc->sh_degree + 1) * (sc->sh_degree + 1);
+  const Workspace ws = carve(ws_ptr, sc->N, K, v->width, v->height, cap);
+  if (ws.bytes > ws_bytes) return FDGS_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  ViewParams vp; CfgParams cp;
+  make_params(v, c, vp, cp);
+  // header (tickets, counters), coverage difference grid and scan states start from zero
+  FDGS_CUDA(cudaMemsetAsync(ws_ptr, 0, ws.zero_bytes, st), "memset(header)");
+  WsHeader h; memset(&h, 0, sizeof(h));
+  h.N = sc->N; h.K = K; h.W = v->width; h.H = v->height; h.pair_capacity = cap; h.tiles = (long long)vp.tiles_x * vp.tiles_y;
+  FDGS_CUDA(cudaMemcpyAsync(&ws.hdr->N, &h.N, 6 * sizeof(long long), cudaMemcpyHostToDevice, st), "memcpy(header)");
+  launch_preprocess_fwd(*sc, vp, cp, ws, st);                       // A1-A4 (+ coverage grid)
+  launch_compact(ws, sc->N, st);                                    // survivors -> (depth bits, id)
+  const int l2_passes = (ceil_log2((long long)vp.tiles_x * vp.tiles_y) + RADIX_BITS - 1) / RADIX_BITS;
+  launch_tile_grid(ws, vp, cap, l2_passes > 0 ? l2_passes : 1, st); // A5/A8: list lengths -> ranges, D
+  FDGS_CUDA(cudaGetLastError(), "preprocess launches");
+  if (num_pairs_host || num_visible_host) {
+    FDGS_CUDA(cudaStreamSynchronize(st), "preprocess sync");
+    unsigned int hv[16];
+    FDGS_CUDA(cudaMemcpy(hv, ws.hdr, sizeof(hv), cudaMemcpyDeviceToHost), "read header");
+    const WsHeader* hh = reinterpret_cast<const WsHeader*>(hv);
+    if (num_pairs_host) *num_pairs_host = hh->pad[0];
+    if (num_visible_host) *num_visible_host = (int32_t)hh->num_visible;
+    if (hh->overflow) return FDGS_ERR_PAIR_OVERFLOW;
+  }
+  return FDGS_OK;
+}
+
+}  // extern "C"
+
+// A6-A9.  The depth order of the survivors (level 1) is kept in the workspace for the backward.
+static int forward_impl(const fdgs_scene* sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, int64_t cap,
+                        cudaStream_t st, float* image, float* final_T, uint32_t* n_contrib, int* l1_buf_out, int* l2_buf_out) {
+  // scan_ticket[1] and sort_ticket[0..7] are adjacent in the header: clear them together
+  FDGS_CUDA(cudaMemsetAsync(&ws.hdr->scan_ticket[1], 0, 9 * sizeof(unsigned int), st), "memset(tickets)");
+  FDGS_CUDA(cudaMemsetAsync(ws.scan_state[1], 0, 8 * (((size_t)(sc->N > 0 ? sc->N : 1) + SCAN_TILE - 1) / SCAN_TILE + 1), st), "memset(scan)");
+  const int sms = num_sms();
+  const int l1 = launch_sort_pairs(ws, ws.l1_keys, ws.l1_vals, &ws.hdr->num_visible, sc->N, 32, SORT_ITEMS_L1, 0, false, sms, st);
+  launch_offsets(ws, l1, sc->N, st);
+  launch_duplicate(ws, l1, sc->N, vp, st);
+  const int tile_bits = ceil_log2((long long)vp.tiles_x * vp.tiles_y);
+  const int l2 = launch_sort_pairs(ws, ws.l2_keys, ws.l2_vals, &ws.hdr->num_pairs, cap, tile_bits, SORT_ITEMS_L2, 4, true, sms, st);
+  launch_blend_fwd(ws, l2, vp, cp, image, final_T, n_contrib, st);
+  FDGS_CUDA(cudaGetLastError(), "forward launches");
+  *l1_buf_out = l1; *l2_buf_out = l2;
+  return FDGS_OK;
+}
+
+static void sort_bufs(const fdgs_scene* sc, const ViewParams& vp, int64_t cap, int* l1, int* l2) {
+  // result buffers are a function of the pass counts only
+  *l1 = sc->N > 0 ? (4 & 1) : 0;
+  const int tile_bits = ceil_log2((long long)vp.tiles_x * vp.tiles_y);
+  const int p2 = (tile_bits + RADIX_BITS - 1) / RADIX_BITS;
+  *l2 = (p2 > 0 && cap > 0) ? (p2 & 1) : 0;
+}
+
+extern "C" {
+
+int fdgs_render_forward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
+                        int64_t cap, void* stream, float* image, float* final_T, uint32_t* n_contrib) {
+  int rc = check_common(sc, v, c, ws_ptr);
+  if (rc) return rc;
+  if (!image || !final_T || !n_contrib || cap < 1 || cap >= (1LL << 30)) return FDGS_ERR_INVALID;
+  const int K = sc->n_time * (sc->sh_degree + 1) * (sc->sh_degree + 1);
+  const Workspace ws = carve(ws_ptr, sc->N, K, v->width, v->height, cap);
+  if (ws.bytes > ws_bytes) return FDGS_ERR_WORKSPACE;
+  ViewParams vp; CfgParams cp;
+  make_params(v, c, vp, cp);
+  int l1, l2;
+  return forward_impl(sc, vp, cp, ws, cap, (cudaStream_t)stream, image, final_T, n_contrib, &l1, &l2);
+}
+
+int fdgs_render_backward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
+                         int64_t cap, void* stream, const float* dL_dimage, const float* final_T, const uint32_t* n_contrib,
+                         const fdgs_grads* g) {
+  int rc = check_common(sc, v, c, ws_ptr);
+  if (rc) return rc;
+  if (!dL_dimage || !final_T || !n_contrib || !g || cap < 1 || cap >= (1LL << 30)) return FDGS_ERR_INVALID;
+  if (sc->N > 0 && (!g->mean || !g->log_scale || !g->quat_l || !g->quat_r || !g->opacity_logit || !g->sh)) return FDGS_ERR_INVALID;
+  if (sc->N > 0 && (!aligned16(g->mean) || !aligned16(g->log_scale) || !aligned16(g->quat_l) || !aligned16(g->quat_r))) return FDGS_ERR_INVALID;
+  const int K = sc->n_time * (sc->sh_degree + 1) * (sc->sh_degree + 1);
+  const Workspace ws = carve(ws_ptr, sc->N, K, v->width, v->height, cap);
+  if (ws.bytes > ws_bytes) return FDGS_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  ViewParams vp; CfgParams cp;
+  make_params(v, c, vp, cp);
+  int l1, l2;
+  sort_bufs(sc, vp, cap, &l1, &l2);
+  if (sc->N > 0) FDGS_CUDA(cudaMemsetAsync(ws.g9, 0, sizeof(float) * 9 * (size_t)sc->N, st), "memset(g9)");
+  launch_blend_bwd(ws, l2, vp, cp, dL_dimage, final_T, n_contrib, st);          // B1
+  launch_preprocess_bwd(*sc, vp, cp, ws, l1, *g, st);                           // B2
+  FDGS_CUDA(cudaGetLastError(), "backward launches");
+  return FDGS_OK;
+}
+
+int fdgs_l1_loss(const float* image, const float* target, int64_t count, float* dL_dimage, float* loss, void* stream) {
+  if (!image || !target || !dL_dimage || !loss || count <= 0) return FDGS_ERR_INVALID;
+  launch_l1_loss(image, target, count, dL_dimage, loss, (cudaStream_t)stream);
+  FDGS_CUDA(cudaGetLastError(), "l1 loss launch");
+  return FDGS_OK;
+}
+
+int fdgs_step_host(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws, size_t ws_bytes, int64_t cap,
+                   void* stream, const float* target_host, float* target_dev, float* image, float* final_T,
+                   uint32_t* n_contrib, float* dL_dimage, float* loss_dev, fdgs_grads* g, float* result_host) {
+  if (!v || !result_host) return FDGS_ERR_INVALID;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t count = (size_t)3 * v->width * v->height;
+  if (g) {
+    if (!target_host || !target_dev || !dL_dimage || !loss_dev) return FDGS_ERR_INVALID;
+    FDGS_CUDA(cudaMemcpyAsync(target_dev, target_host, count * sizeof(float), cudaMemcpyHostToDevice, st), "H2D target");
+    FDGS_CUDA(cudaMemsetAsync(loss_dev, 0, sizeof(float), st), "memset(loss)");
+  }
+  int rc = fdgs_preprocess(sc, v, c, ws, ws_bytes, cap, stream, nullptr, nullptr);
+  if (rc) return rc;
+  rc = fdgs_render_forward(sc, v, c, ws, ws_bytes, cap, stream, image, final_T, n_contrib);
+  if (rc) return rc;
+  if (g) {
+    rc = fdgs_l1_loss(image, target_dev, (int64_t)count, dL_dimage, loss_dev, stream);
+    if (rc) return rc;
+    rc = fdgs_render_backward(sc, v, c, ws, ws_bytes, cap, stream, dL_dimage, final_T, n_contrib, g);
+    if (rc) return rc;
+    FDGS_CUDA(cudaMemcpyAsync(result_host, loss_dev, sizeof(float), cudaMemcpyDeviceToHost, st), "D2H loss");
+  } else {
+    FDGS_CUDA(cudaMemcpyAsync(result_host, image, count * sizeof(float), cudaMemcpyDeviceToHost, st), "D2H image");
+  }
+  FDGS_CUDA(cudaStreamSynchronize(st), "step sync");
+  return FDGS_OK;
+}
+
+int64_t fdgs_launch_count(void) { return g_launches; }
+
+const char* fdgs_strerror(int code) {
+  switch (code) {
+    case FDGS_OK: return "ok";
+    case FDGS_ERR_INVALID: return "invalid argument";
+    case FDGS_ERR_WORKSPACE: return "workspace too small (see fdgs_workspace_bytes)";
+    case FDGS_ERR_CUDA: return g_cuda_err;
+    case FDGS_ERR_PAIR_OVERFLOW: return "number of (tile, primitive) pairs exceeds pair_capacity";
+    default: return "unknown error";
+  }
+}
+
+}  // extern "C"
+
+extern "C" int fdgs_debug_export(const void* ws_ptr, size_t ws_bytes, int what, void* dst, size_t dst_bytes, void* stream) {
+  if (!ws_ptr || !dst) return FDGS_ERR_INVALID;
+  cudaStream_t st = (cudaStream_t)stream;
+  FDGS_CUDA(cudaStreamSynchronize(st), "export sync");
+  WsHeader h;
+  FDGS_CUDA(cudaMemcpy(&h, ws_ptr, sizeof(h), cudaMemcpyDeviceToHost), "export header");
+  const Workspace ws = carve(const_cast<void*>(ws_ptr), h.N, h.K, h.W, h.H, h.pair_capacity);
+  if (ws.bytes > ws_bytes) return FDGS_ERR_WORKSPACE;
+  const long long N = h.N, D = h.num_pairs;
+  ViewParams vp; vp.tiles_x = (int)((h.W + TILE - 1) / TILE); vp.tiles_y = (int)((h.H + TILE - 1) / TILE);
+  fdgs_scene sc; sc.N = (int)N;
+  int l1, l2;
+  sort_bufs(&sc, vp, h.pair_capacity, &l1, &l2);
+  size_t need = 0;
+  const void* src = nullptr;
+  switch (what) {
+    case FDGS_EXPORT_STATUS: {
+      const long long status[4] = {(long long)h.pad[0], (long long)h.num_visible, (long long)h.overflow, h.pair_capacity};
+      if (dst_bytes < sizeof(status)) return FDGS_ERR_INVALID;
+      FDGS_CUDA(cudaMemcpy(dst, status, sizeof(status), cudaMemcpyHostToDevice), "export status");
+      return h.overflow ? FDGS_ERR_PAIR_OVERFLOW : FDGS_OK;
+    }
+    case FDGS_EXPORT_RECORDS:
+      if (dst_bytes < sizeof(float) * 12 * (size_t)N) return FDGS_ERR_INVALID;
+      if (N > 0) export_records_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(ws.rec, ws.tiles_touched, (int)N, (float*)dst);
+      break;
+    case FDGS_EXPORT_RECTS:
+      if (dst_bytes < sizeof(int) * 4 * (size_t)N) return FDGS_ERR_INVALID;
+      if (N > 0) export_rects_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(ws.rect, (int)N, (int4*)dst);
+      break;
+    case FDGS_EXPORT_TILES_TOUCHED: src = ws.tiles_touched; need = 4 * (size_t)N; break;
+    case FDGS_EXPORT_OFFSETS: src = ws.offsets; need = 4 * (size_t)h.num_visible; break;
+    case FDGS_EXPORT_DEPTH_ORDER: src = ws.l1_vals[l1]; need = 4 * (size_t)h.num_visible; break;
+    case FDGS_EXPORT_SORTED_KEYS:
+      if (dst_bytes < 8 * (size_t)D) return FDGS_ERR_INVALID;
+      if (D > 0) export_keys_kernel<<<(unsigned)((D + 255) / 256), 256, 0, st>>>(ws.l2_keys[l2], ws.l2_vals[l2], ws.rec, (unsigned)D, (unsigned long long*)dst);
+      break;
+    case FDGS_EXPORT_SORTED_VALS: src = ws.l2_vals[l2]; need = 4 * (size_t)D; break;
+    case FDGS_EXPORT_RANGES: src = ws.ranges; need = 8 * (size_t)h.tiles; break;
+    case FDGS_EXPORT_SPLAT_GRADS: src = ws.g9; need = 36 * (size_t)N; break;
+    default: return FDGS_ERR_INVALID;
+  }
+  if (src) {
+    if (dst_bytes < need) return FDGS_ERR_INVALID;
+    if (need) FDGS_CUDA(cudaMemcpyAsync(dst, src, need, cudaMemcpyDeviceToDevice, st), "export copy");
+  }
+  FDGS_CUDA(cudaGetLastError(), "export launch");
+  FDGS_CUDA(cudaStreamSynchronize(st), "export sync");
+  return FDGS_OK;
+}

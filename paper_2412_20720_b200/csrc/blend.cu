@@ -1,0 +1,207 @@
+// blend.cu — A9 (forward compositing) and B1 (its reverse-order gradient) for sm_100a.
+// One CTA per 16x16 tile, one pixel per thread; each warp covers an 8x4 pixel patch so that early
+// termination and alpha-skips stay coherent inside a warp.  Splat records are gathered by id into shared
+// memory in batches of 256 and converted once per (tile, splat) to tile-local form:
+//     e1 = k1 - ca*x - cb*y,  e2 = k2 - cc*y,  log2(alpha) = lo - e1^2 - e2^2      (x, y tile-local pixel centres)
+// i.e. 5 FFMA + 1 MUFU.EX2 per (pixel, splat) evaluation; tile-local coordinates keep |e| small so fp32
+// cancellation stays ~1e-7.
+#include "common.cuh"
+
+namespace fdgs {
+
+constexpr int BATCH = 256;
+
+struct TileSplat {   // 48 B in shared memory, read as three broadcast LDS.128
+  float nca, ncb, ncc, k1;   // -ca, -cb, -cc, ca*(u-ox) + cb*(v-oy)
+  float k2, lo, r, g;        // cc*(v-oy), log2(o)
+  float b, u, v, pad;        // (u, v) tile-local, for the backward
+};
+
+__device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+__device__ __forceinline__ void stage_splat(const SplatRec* __restrict__ rec, const unsigned int id, const float ox, const float oy,
+                                            float4* s0, float4* s1, float4* s2) {
+  const float4* src = reinterpret_cast<const float4*>(rec + id);
+  const float4 q0 = __ldg(src), q1 = __ldg(src + 1), q2 = __ldg(src + 2);
+  const float ul = q0.x - ox, vl = q0.y - oy;
+  *s0 = make_float4(-q0.z, -q0.w, -q1.x, fmaf(q0.z, ul, q0.w * vl));
+  *s1 = make_float4(q1.x * vl, q1.y, q1.z, q1.w);
+  *s2 = make_float4(q2.x, ul, vl, 0.f);
+}
+
+__global__ void __launch_bounds__(256) blend_fwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
+                                                        const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
+                                                        float* __restrict__ image, float* __restrict__ final_T,
+                                                        unsigned int* __restrict__ n_contrib) {
+  __shared__ float4 s0[BATCH], s1[BATCH], s2[BATCH];
+  const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int lx = ((warp & 1) << 3) + (lane & 7), ly = ((warp >> 1) << 2) + (lane >> 3);
+  const int px = tx * TILE + lx, py = ty * TILE + ly;
+  const bool inside = px < vp.width && py < vp.height;
+  const float x = lx + 0.5f, y = ly + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
+  const uint2 range = ranges[tile];
+  const int n = (int)(range.y - range.x);
+  float T = 1.f, Cr = 0.f, Cg = 0.f, Cb = 0.f;
+  unsigned int last = 0;
+  bool done = !inside;
+  for (int base = 0; base < n; base += BATCH) {
+    if (__syncthreads_and(done)) break;
+    const int m = min(BATCH, n - base);
+    if ((int)threadIdx.x < m) stage_splat(rec, vals[range.x + base + threadIdx.x], ox, oy, &s0[threadIdx.x], &s1[threadIdx.x], &s2[threadIdx.x]);
+    __syncthreads();
+    if (__all_sync(0xffffffffu, done)) continue;     // whole 8x4 patch saturated: skip the batch (warp-uniform)
+    for (int j = 0; j < m; ++j) {
+      const float4 a = s0[j], b = s1[j];
+      const float e1 = fmaf(a.x, x, fmaf(a.y, y, a.w));
+      const float e2 = fmaf(a.z, y, b.x);
+      const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
+      if (done || l2a < cp.log2_alpha_min) continue;                 // alpha < alpha_min: skipped
+      const float alpha = fminf(cp.alpha_max, ex2_approx(l2a));
+      if (alpha < cp.alpha_min) continue;
+      const float Tn = fmaf(-T, alpha, T);
+      if (Tn < cp.transmittance_min) { done = true; continue; }      // the terminating splat is not composited
+      const float wgt = alpha * T;
+      Cr = fmaf(b.z, wgt, Cr); Cg = fmaf(b.w, wgt, Cg); Cb = fmaf(s2[j].x, wgt, Cb);
+      T = Tn;
+      last = base + j + 1;
+    }
+  }
+  if (inside) {
+    const size_t hw = (size_t)vp.width * vp.height, pix = (size_t)py * vp.width + px;
+    image[pix] = fmaf(T, vp.bg[0], Cr); image[hw + pix] = fmaf(T, vp.bg[1], Cg); image[2 * hw + pix] = fmaf(T, vp.bg[2], Cb);
+    final_T[pix] = T; n_contrib[pix] = last;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Sum of 8 values over the 32 lanes with 9 shuffles (halving exchange), result k lands on lane 4k.
+__device__ __forceinline__ float warp_reduce8(float v[8], const int lane) {
+  const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const float keep = b4 ? v[i + 4] : v[i], send = b4 ? v[i] : v[i + 4];
+    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+  }
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    const float keep = b3 ? v[i + 2] : v[i], send = b3 ? v[i] : v[i + 2];
+    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+  }
+  {
+    const float keep = b2 ? v[1] : v[0], send = b2 ? v[0] : v[1];
+    v[0] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+  }
+  v[0] += __shfl_xor_sync(0xffffffffu, v[0], 2);
+  v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
+  return v[0];
+}
+
+// B1.  Walks each tile list back to front from the last contributor of the tile; per splat the nine
+// gradients are reduced over the warp by shuffles, then over the eight warps in shared memory, and one
+// thread per splat flushes nine global atomics per (tile, splat).
+__global__ void __launch_bounds__(256) blend_bwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
+                                                        const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
+                                                        const float* __restrict__ dL_dimage, const float* __restrict__ final_T,
+                                                        const unsigned int* __restrict__ n_contrib, float* __restrict__ g9) {
+  __shared__ float4 s0[BATCH], s1[BATCH], s2[BATCH];
+  __shared__ float s_acc[9][BATCH];
+  __shared__ unsigned int s_id[BATCH];
+  __shared__ int s_max;
+  const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int lx = ((warp & 1) << 3) + (lane & 7), ly = ((warp >> 1) << 2) + (lane >> 3);
+  const int px = tx * TILE + lx, py = ty * TILE + ly;
+  const bool inside = px < vp.width && py < vp.height;
+  const float x = lx + 0.5f, y = ly + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
+  const uint2 range = ranges[tile];
+  const size_t hw = (size_t)vp.width * vp.height, pix = (size_t)py * vp.width + px;
+  float T = 1.f, gr = 0.f, gg = 0.f, gb = 0.f;
+  int mine = 0;
+  if (inside) { T = final_T[pix]; mine = (int)n_contrib[pix]; gr = dL_dimage[pix]; gg = dL_dimage[hw + pix]; gb = dL_dimage[2 * hw + pix]; }
+  if (threadIdx.x == 0) s_max = 0;
+  __syncthreads();
+  int warp_max = mine;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) warp_max = max(warp_max, __shfl_xor_sync(0xffffffffu, warp_max, o));
+  if (lane == 0) atomicMax(&s_max, warp_max);
+  __syncthreads();
+  const int total = s_max;
+  // S = colour accumulated behind the current splat (starts as T_final * bg)
+  float Sr = T * vp.bg[0], Sg = T * vp.bg[1], Sb = T * vp.bg[2];
+  const float ln2 = 0.69314718055994531f;
+  for (int hi = total; hi > 0; hi -= BATCH) {           // batch covers list positions [lo_pos, hi)
+    const int lo_pos = max(0, hi - BATCH), m = hi - lo_pos;
+    __syncthreads();                                    // previous batch fully flushed
+    if ((int)threadIdx.x < m) {
+      const unsigned int id = vals[range.x + lo_pos + threadIdx.x];
+      s_id[threadIdx.x] = id;
+      stage_splat(rec, id, ox, oy, &s0[threadIdx.x], &s1[threadIdx.x], &s2[threadIdx.x]);
+    }
+#pragma unroll
+    for (int k = 0; k < 9; ++k) s_acc[k][threadIdx.x] = 0.f;
+    __syncthreads();
+    if (lo_pos < warp_max) {
+      for (int j = m - 1; j >= 0; --j) {
+        const float4 a = s0[j], b = s1[j], c = s2[j];
+        const float e1 = fmaf(a.x, x, fmaf(a.y, y, a.w));
+        const float e2 = fmaf(a.z, y, b.x);
+        const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
+        bool active = (lo_pos + j < mine) && !(l2a < cp.log2_alpha_min);
+        float alpha = 0.f, araw = 0.f;
+        if (active) { araw = ex2_approx(l2a); alpha = fminf(cp.alpha_max, araw); active = !(alpha < cp.alpha_min); }
+        if (!__any_sync(0xffffffffu, active)) continue;
+        float v[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, v_o = 0.f;
+        if (active) {
+          const float om = 1.f - alpha;
+          T = T / om;                                                  // T_k
+          const float wgt = alpha * T;
+          v[5] = wgt * gr; v[6] = wgt * gg; v[7] = wgt * gb;           // dL/dc
+          const float iom = 1.f / om;
+          const float dalpha = gr * fmaf(-Sr, iom, T * b.z) + gg * fmaf(-Sg, iom, T * b.w) + gb * fmaf(-Sb, iom, T * c.x);
+          Sr = fmaf(b.z, wgt, Sr); Sg = fmaf(b.w, wgt, Sg); Sb = fmaf(c.x, wgt, Sb);
+          if (!(araw > cp.alpha_max)) {                                // alpha clamp inactive
+            // alpha = o * G:  d alpha/d o = G = alpha / o;  d alpha / d power = alpha
+            v_o = dalpha * ex2_approx(l2a - b.y);
+            const float dpow = alpha * dalpha;
+            const float dx = c.y - x, dy = c.z - y;
+            // power = -(e1^2 + e2^2) ln2, e1 = ca dx + cb dy, e2 = cc dy, expressed through the conic (A, B, C):
+            //   d power/du = -(A dx + B dy), d power/dv = -(B dx + C dy), d/dA = -dx^2/2, d/dB = -dx dy, d/dC = -dy^2/2
+            const float ca = -a.x, cb = -a.y, cc = -a.z;
+            const float t1 = 2.f * ln2 * e1, t2 = 2.f * ln2 * e2;      // d(-power)/d e1, d e2
+            v[0] = -dpow * (t1 * ca);
+            v[1] = -dpow * fmaf(t1, cb, t2 * cc);
+            v[2] = dpow * -0.5f * dx * dx; v[3] = dpow * -dx * dy; v[4] = dpow * -0.5f * dy * dy;
+          }
+        }
+        const float red = warp_reduce8(v, lane);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v_o += __shfl_xor_sync(0xffffffffu, v_o, o);
+        if ((lane & 3) == 0) atomicAdd(&s_acc[lane >> 2][j], red);
+        if (lane == 1) atomicAdd(&s_acc[8][j], v_o);
+      }
+    }
+    __syncthreads();
+    if ((int)threadIdx.x < m) {
+      float* dst = g9 + (size_t)9 * s_id[threadIdx.x];
+      // s_acc rows: 0 u, 1 v, 2 A, 3 B, 4 C, 5 r, 6 g, 7 b, 8 o  ->  g9 order u, v, A, B, C, o, r, g, b
+      const int row_of[9] = {0, 1, 2, 3, 4, 8, 5, 6, 7};
+#pragma unroll
+      for (int k = 0; k < 9; ++k) { const float val = s_acc[row_of[k]][threadIdx.x]; if (val != 0.f) atomicAdd(dst + k, val); }
+    }
+  }
+}
+
+void launch_blend_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
+                      unsigned int* n_contrib, cudaStream_t st) {
+  blend_fwd_kernel<<<vp.tiles_x * vp.tiles_y, 256, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib);
+  ++g_launches;
+}
+
+void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* dL_dimage,
+                      const float* final_T, const unsigned int* n_contrib, cudaStream_t st) {
+  blend_bwd_kernel<<<vp.tiles_x * vp.tiles_y, 256, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9);
+  ++g_launches;
+}
+
+}  // namespace fdgs

@@ -1,0 +1,181 @@
+// radix_sort.cu — A7: hand-written stable LSD radix sort of (u32 key, u32 value) pairs for sm_100a.
+// One kernel per 8-bit digit ("onesweep"): each CTA ranks a tile of pairs in shared memory with warp-level
+// match_any multisplit (stable), publishes its digit counts, obtains the counts of all earlier tiles by
+// decoupled look-back, and scatters straight to the final position of the pass — keys and values are read
+// once and written once per pass.  Tiles take dynamic ids from a ticket, CTAs are persistent, and the number
+// of pairs is read from device memory, so the host never synchronises.
+#include "common.cuh"
+
+namespace fdgs {
+
+constexpr unsigned int LB_AGG = 1u << 30, LB_PRE = 2u << 30, LB_MASK = (1u << 30) - 1;
+
+// Global digit histograms of all passes in one read of the keys.
+__global__ void __launch_bounds__(256) sort_hist_kernel(const unsigned int* __restrict__ keys, const unsigned int* __restrict__ count_dev,
+                                                        const int passes, unsigned int* __restrict__ hist /*[passes][RADIX]*/) {
+  __shared__ unsigned int sh[4][RADIX];
+  for (int i = threadIdx.x; i < 4 * RADIX; i += blockDim.x) (&sh[0][0])[i] = 0;
+  __syncthreads();
+  const unsigned int n = *count_dev;
+  for (unsigned int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const unsigned int k = keys[i];
+    for (int p = 0; p < passes; ++p) atomicAdd(&sh[p][(k >> (RADIX_BITS * p)) & (RADIX - 1)], 1u);
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < passes * RADIX; i += blockDim.x) { const unsigned int v = (&sh[0][0])[i]; if (v) atomicAdd(hist + i, v); }
+}
+
+// exclusive scan of each pass's 256 bins (one warp per pass)
+__global__ void sort_hist_scan_kernel(unsigned int* hist, const int passes) {
+  const int p = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (p >= passes) return;
+  unsigned int v[8], s = 0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) { v[k] = hist[p * RADIX + lane * 8 + k]; s += v[k]; }
+  unsigned int incl = s;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const unsigned int n = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += n; }
+  unsigned int r = incl - s;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) { hist[p * RADIX + lane * 8 + k] = r; r += v[k]; }
+}
+
+template <int ITEMS>
+__global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const unsigned int* __restrict__ keys_in, const unsigned int* __restrict__ vals_in,
+                                                                unsigned int* __restrict__ keys_out, unsigned int* __restrict__ vals_out,
+                                                                const unsigned int* __restrict__ count_dev, unsigned int* ticket,
+                                                                const unsigned int* __restrict__ digit_base /*[RADIX] exclusive*/,
+                                                                volatile unsigned int* lookback, const int shift) {
+  constexpr int TILE_N = SORT_THREADS * ITEMS, WARPS = SORT_THREADS / 32;
+  __shared__ unsigned int warp_hist[WARPS][RADIX];   // per-warp digit counts -> exclusive offsets over warps
+  __shared__ unsigned int s_local[RADIX];            // first slot of each digit inside the sorted tile
+  __shared__ unsigned int s_global[RADIX];           // global position of that slot (minus the slot index)
+  __shared__ unsigned int s_keys[TILE_N], s_vals[TILE_N];
+  __shared__ unsigned int warp_sums[33], s_tile;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned int lt_mask = (1u << lane) - 1;
+  const unsigned int n = *count_dev;
+  const unsigned int num_tiles = (n + TILE_N - 1) / TILE_N;
+  while (true) {
+    if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
+#pragma unroll
+    for (int w = 0; w < WARPS; ++w) warp_hist[w][threadIdx.x] = 0;
+    __syncthreads();
+    const unsigned int tile = s_tile;
+    if (tile >= num_tiles) break;
+    // ---- load: warp w owns the contiguous chunk [w*32*ITEMS, (w+1)*32*ITEMS) of the tile, round r = 32 consecutive pairs
+    const unsigned int tile_base = tile * TILE_N, warp_base = tile_base + warp * 32 * ITEMS;
+    unsigned int key[ITEMS], val[ITEMS];
+    unsigned short rank[ITEMS];
+#pragma unroll
+    for (int r = 0; r < ITEMS; ++r) {
+      const unsigned int idx = warp_base + r * 32 + lane;
+      key[r] = idx < n ? keys_in[idx] : 0xffffffffu;
+      val[r] = idx < n ? vals_in[idx] : 0u;
+    }
+    // ---- stable rank inside the warp's chunk: match_any groups equal digits, the lowest lane of a group bumps the count
+#pragma unroll
+    for (int r = 0; r < ITEMS; ++r) {
+      const bool valid = warp_base + r * 32 + lane < n;
+      const unsigned int digit = valid ? ((key[r] >> shift) & (RADIX - 1)) : 0xffffffffu;
+      const unsigned int grp = __match_any_sync(0xffffffffu, digit);
+      const int leader = __ffs(grp) - 1;
+      unsigned int old = 0;
+      if (valid && lane == leader) { old = warp_hist[warp][digit]; warp_hist[warp][digit] = old + __popc(grp); }
+      old = __shfl_sync(0xffffffffu, old, leader);
+      rank[r] = (unsigned short)(old + __popc(grp & lt_mask));
+      __syncwarp();
+    }
+    __syncthreads();
+    // ---- thread d owns digit d: exclusive offsets over warps, tile count, look-back, local digit base
+    const int d = threadIdx.x;
+    unsigned int cnt = 0;
+#pragma unroll
+    for (int w = 0; w < WARPS; ++w) { const unsigned int c = warp_hist[w][d]; warp_hist[w][d] = cnt; cnt += c; }
+    volatile unsigned int* lb = lookback + (size_t)tile * RADIX + d;
+    *lb = (tile == 0 ? LB_PRE : LB_AGG) | cnt;
+    unsigned int excl_tiles = 0;
+    if (tile > 0) {
+      long long j = (long long)tile - 1;
+      while (true) {
+        unsigned int s;
+        do { s = lookback[(size_t)j * RADIX + d]; } while ((s >> 30) == 0);
+        excl_tiles += s & LB_MASK;
+        if ((s >> 30) == 2 || j == 0) break;
+        --j;
+      }
+      *lb = LB_PRE | (excl_tiles + cnt);
+    }
+    // block exclusive scan of cnt over the 256 digits
+    unsigned int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const unsigned int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
+    if (lane == 31) warp_sums[warp] = incl;
+    __syncthreads();
+    unsigned int wprefix = 0;
+#pragma unroll
+    for (int w = 0; w < WARPS; ++w) if (w < warp) wprefix += warp_sums[w];
+    const unsigned int local = wprefix + incl - cnt;
+    s_local[d] = local;
+    s_global[d] = digit_base[d] + excl_tiles - local;
+    __syncthreads();
+    // ---- scatter into the tile's sorted order in shared memory
+#pragma unroll
+    for (int r = 0; r < ITEMS; ++r) {
+      if (warp_base + r * 32 + lane < n) {
+        const unsigned int digit = (key[r] >> shift) & (RADIX - 1);
+        const unsigned int pos = s_local[digit] + warp_hist[warp][digit] + rank[r];
+        s_keys[pos] = key[r]; s_vals[pos] = val[r];
+      }
+    }
+    __syncthreads();
+    // ---- coalesced write-out: consecutive slots of one digit go to consecutive global positions
+    const unsigned int valid_n = min((unsigned int)TILE_N, n - tile_base);
+#pragma unroll
+    for (int r = 0; r < ITEMS; ++r) {
+      const unsigned int slot = r * SORT_THREADS + threadIdx.x;
+      if (slot < valid_n) {
+        const unsigned int k = s_keys[slot];
+        const unsigned int out = s_global[(k >> shift) & (RADIX - 1)] + slot;
+        keys_out[out] = k; vals_out[out] = s_vals[slot];
+      }
+    }
+    __syncthreads();
+  }
+}
+
+int launch_sort_pairs(const Workspace& ws, unsigned int* const keys[2], unsigned int* const vals[2],
+                      const unsigned int* count_dev, long long max_count, int bits, int items_per_thread, int ticket_base,
+                      bool hist_ready, int num_sms, cudaStream_t st) {
+  const int passes = (bits + RADIX_BITS - 1) / RADIX_BITS;
+  if (passes <= 0 || max_count <= 0) return 0;
+  unsigned int* hist = ws.sort_hist + (size_t)ticket_base * RADIX;
+  if (!hist_ready) {
+    cudaMemsetAsync(hist, 0, sizeof(unsigned int) * passes * RADIX, st);
+    const int hb = (int)((max_count + 256 * 16 - 1) / (256 * 16));
+    sort_hist_kernel<<<hb < 4 * num_sms ? hb : 4 * num_sms, 256, 0, st>>>(keys[0], count_dev, passes, hist);
+    sort_hist_scan_kernel<<<1, 32 * passes, 0, st>>>(hist, passes);
+    g_launches += 2;
+  }
+  const int tile_n = SORT_THREADS * items_per_thread;
+  const long long tiles = (max_count + tile_n - 1) / tile_n;
+  const size_t lb_bytes = sizeof(unsigned int) * RADIX * (size_t)tiles;
+  int cur = 0;
+  for (int p = 0; p < passes; ++p) {
+    cudaMemsetAsync(ws.sort_lookback, 0, lb_bytes, st);
+    const int grid = (int)(tiles < 4LL * num_sms ? tiles : 4LL * num_sms);
+    if (items_per_thread == SORT_ITEMS_L1)
+      onesweep_kernel<SORT_ITEMS_L1><<<grid, SORT_THREADS, 0, st>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], count_dev,
+                                                                   &ws.hdr->sort_ticket[ticket_base + p], hist + p * RADIX,
+                                                                   ws.sort_lookback, p * RADIX_BITS);
+    else
+      onesweep_kernel<SORT_ITEMS_L2><<<grid, SORT_THREADS, 0, st>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], count_dev,
+                                                                   &ws.hdr->sort_ticket[ticket_base + p], hist + p * RADIX,
+                                                                   ws.sort_lookback, p * RADIX_BITS);
+    ++g_launches;
+    cur ^= 1;
+  }
+  return cur;
+}
+
+}  // namespace fdgs

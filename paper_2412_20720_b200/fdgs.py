@@ -1,0 +1,269 @@
+"""Thin ctypes binding over the C-ABI library of include/fdgs.h — argument marshalling only.
+
+Every step of the path runs in the hand-written CUDA kernels of libfdgs.so; PyTorch is used for
+device memory and streams.  There is NO CPU fallback: the first call raises if the library has not
+been built (``python -m paper_2412_20720_b200.build``) or if no CUDA device is present.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfdgs.so")
+_lib = None
+
+OK, ERR_INVALID, ERR_WORKSPACE, ERR_CUDA, ERR_PAIR_OVERFLOW = 0, -1, -2, -3, -4
+(EXPORT_STATUS, EXPORT_RECORDS, EXPORT_RECTS, EXPORT_TILES_TOUCHED, EXPORT_OFFSETS, EXPORT_SORTED_KEYS,
+ EXPORT_SORTED_VALS, EXPORT_RANGES, EXPORT_SPLAT_GRADS, EXPORT_DEPTH_ORDER) = range(10)
+
+EXPORTED_SYMBOLS = ["fdgs_default_config", "fdgs_workspace_bytes", "fdgs_preprocess", "fdgs_render_forward",
+                    "fdgs_render_backward", "fdgs_l1_loss", "fdgs_step_host", "fdgs_debug_export",
+                    "fdgs_launch_count", "fdgs_strerror"]
+
+
+class CScene(C.Structure):
+    _fields_ = [("N", C.c_int32), ("sh_degree", C.c_int32), ("n_time", C.c_int32), ("mean", C.c_void_p),
+                ("log_scale", C.c_void_p), ("quat_l", C.c_void_p), ("quat_r", C.c_void_p),
+                ("opacity_logit", C.c_void_p), ("sh", C.c_void_p)]
+
+
+class CView(C.Structure):
+    _fields_ = [("view", C.c_float * 16), ("fx", C.c_float), ("fy", C.c_float), ("cx", C.c_float), ("cy", C.c_float),
+                ("width", C.c_int32), ("height", C.c_int32), ("t", C.c_float), ("period_T", C.c_float),
+                ("bg", C.c_float * 3)]
+
+
+class CConfig(C.Structure):
+    _fields_ = [(k, C.c_float) for k in ("marginal_min", "alpha_min", "alpha_max", "transmittance_min", "dilation",
+                                         "cutoff_sigma", "znear", "guard")]
+
+
+class CGrads(C.Structure):
+    _fields_ = [(k, C.c_void_p) for k in ("mean", "log_scale", "quat_l", "quat_r", "opacity_logit", "sh", "mean2d")]
+
+
+class FdgsError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        super().__init__(f"{where}: {strerror(code)} ({code})")
+
+
+def load():
+    """Loads libfdgs.so; raises loudly if it is missing (the product has no fallback path)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} not found: build the CUDA library first "
+                           "(python -m paper_2412_20720_b200.build); there is no CPU fallback")
+    lib = C.CDLL(LIB_PATH)
+    vp, sz, i64, i32 = C.c_void_p, C.c_size_t, C.c_int64, C.c_int32
+    lib.fdgs_default_config.argtypes = [C.POINTER(CConfig)]
+    lib.fdgs_workspace_bytes.argtypes = [i32, i32, i32, i32, i64, C.POINTER(sz)]
+    lib.fdgs_preprocess.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp,
+                                    C.POINTER(i64), C.POINTER(i32)]
+    lib.fdgs_render_forward.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, vp, vp, vp]
+    lib.fdgs_render_backward.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, vp, vp,
+                                         vp, C.POINTER(CGrads)]
+    lib.fdgs_l1_loss.argtypes = [vp, vp, i64, vp, vp, vp]
+    lib.fdgs_step_host.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, vp, vp, vp, vp,
+                                   vp, vp, vp, C.POINTER(CGrads), vp]
+    lib.fdgs_debug_export.argtypes = [vp, sz, C.c_int, vp, sz, vp]
+    lib.fdgs_launch_count.restype = i64
+    lib.fdgs_strerror.restype = C.c_char_p
+    lib.fdgs_strerror.argtypes = [C.c_int]
+    for name in EXPORTED_SYMBOLS:
+        if name not in ("fdgs_launch_count", "fdgs_strerror"):
+            getattr(lib, name).restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def strerror(code: int) -> str:
+    return load().fdgs_strerror(int(code)).decode()
+
+
+def launch_count() -> int:
+    return int(load().fdgs_launch_count())
+
+
+def default_config(**overrides) -> CConfig:
+    cfg = CConfig()
+    rc = load().fdgs_default_config(C.byref(cfg))
+    if rc:
+        raise FdgsError(rc, "fdgs_default_config")
+    for k, v in overrides.items():
+        if k == "full_support":
+            continue
+        setattr(cfg, k, float(v))
+    return cfg
+
+
+def make_view(view) -> CView:
+    """From a scenes.View (or anything with the same attributes)."""
+    import numpy as np
+    cv = CView()
+    flat = np.asarray(view.view, dtype=np.float32).reshape(16)
+    for i in range(16):
+        cv.view[i] = float(flat[i])
+    cv.fx, cv.fy, cv.cx, cv.cy = float(view.fx), float(view.fy), float(view.cx), float(view.cy)
+    cv.width, cv.height, cv.t, cv.period_T = int(view.width), int(view.height), float(view.t), float(view.period_T)
+    for i in range(3):
+        cv.bg[i] = float(view.bg[i])
+    return cv
+
+
+def _ptr(t) -> Optional[int]:
+    return None if t is None else t.data_ptr()
+
+
+def _stream() -> int:
+    import torch
+    return torch.cuda.current_stream().cuda_stream
+
+
+@dataclass
+class DeviceScene:
+    """The six parameter arrays resident in HBM (torch float32 CUDA tensors)."""
+    sh_degree: int
+    n_time: int
+    mean: "torch.Tensor"
+    log_scale: "torch.Tensor"
+    quat_l: "torch.Tensor"
+    quat_r: "torch.Tensor"
+    opacity_logit: "torch.Tensor"
+    sh: "torch.Tensor"
+
+    @property
+    def N(self):
+        return int(self.mean.shape[0])
+
+    @property
+    def K(self):
+        return self.n_time * (self.sh_degree + 1) ** 2
+
+    @classmethod
+    def from_scene(cls, scene, device="cuda:0"):
+        import torch
+        f = lambda a: torch.from_numpy(a.astype("float32", copy=False)).contiguous().to(device)
+        return cls(scene.sh_degree, scene.n_time, f(scene.mean), f(scene.log_scale), f(scene.quat_l), f(scene.quat_r),
+                   f(scene.opacity_logit), f(scene.sh))
+
+    def c_struct(self) -> CScene:
+        return CScene(self.N, self.sh_degree, self.n_time, _ptr(self.mean), _ptr(self.log_scale), _ptr(self.quat_l),
+                      _ptr(self.quat_r), _ptr(self.opacity_logit), _ptr(self.sh))
+
+    def zero_grads(self, with_mean2d=False):
+        import torch
+        g = {k: torch.zeros_like(getattr(self, k)) for k in ("mean", "log_scale", "quat_l", "quat_r", "opacity_logit", "sh")}
+        g["mean2d"] = torch.zeros((self.N, 2), device=self.mean.device) if with_mean2d else None
+        return g
+
+
+def grads_struct(g: dict) -> CGrads:
+    return CGrads(_ptr(g["mean"]), _ptr(g["log_scale"]), _ptr(g["quat_l"]), _ptr(g["quat_r"]), _ptr(g["opacity_logit"]),
+                  _ptr(g["sh"]), _ptr(g.get("mean2d")))
+
+
+def workspace_bytes(N, K, width, height, pair_capacity) -> int:
+    out = C.c_size_t(0)
+    rc = load().fdgs_workspace_bytes(int(N), int(K), int(width), int(height), int(pair_capacity), C.byref(out))
+    if rc:
+        raise FdgsError(rc, "fdgs_workspace_bytes")
+    return int(out.value)
+
+
+class Renderer:
+    """Owns the workspace and output buffers for one (scene size, resolution, pair capacity)."""
+
+    def __init__(self, dscene: DeviceScene, width: int, height: int, pair_capacity: int, cfg: Optional[CConfig] = None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("fdgs needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.lib = load()
+        self.ds, self.width, self.height, self.cap = dscene, int(width), int(height), int(pair_capacity)
+        self.cfg = cfg if cfg is not None else default_config()
+        dev = dscene.mean.device
+        self.ws_bytes = workspace_bytes(dscene.N, dscene.K, width, height, pair_capacity)
+        self.ws = torch.empty(self.ws_bytes, dtype=torch.uint8, device=dev)
+        self.image = torch.empty((3, height, width), dtype=torch.float32, device=dev)
+        self.final_T = torch.empty((height, width), dtype=torch.float32, device=dev)
+        self.n_contrib = torch.empty((height, width), dtype=torch.int32, device=dev)
+        self.dL_dimage = torch.empty((3, height, width), dtype=torch.float32, device=dev)
+        self.loss = torch.zeros(1, dtype=torch.float32, device=dev)
+        self.target_dev = torch.empty((3, height, width), dtype=torch.float32, device=dev)
+        self._cs = dscene.c_struct()
+
+    # -- the three calls of the boundary ---------------------------------------------------------
+    def preprocess(self, cview: CView, sync: bool = False):
+        npairs, nvis = C.c_int64(-1), C.c_int32(-1)
+        rc = self.lib.fdgs_preprocess(C.byref(self._cs), C.byref(cview), C.byref(self.cfg), self.ws.data_ptr(), self.ws_bytes,
+                                      self.cap, _stream(), C.byref(npairs) if sync else None, C.byref(nvis) if sync else None)
+        if rc:
+            raise FdgsError(rc, "fdgs_preprocess")
+        return (int(npairs.value), int(nvis.value)) if sync else None
+
+    def forward(self, cview: CView):
+        rc = self.lib.fdgs_render_forward(C.byref(self._cs), C.byref(cview), C.byref(self.cfg), self.ws.data_ptr(),
+                                          self.ws_bytes, self.cap, _stream(), self.image.data_ptr(), self.final_T.data_ptr(),
+                                          self.n_contrib.data_ptr())
+        if rc:
+            raise FdgsError(rc, "fdgs_render_forward")
+        return self.image
+
+    def backward(self, cview: CView, dL_dimage, grads: dict):
+        cg = grads_struct(grads)
+        rc = self.lib.fdgs_render_backward(C.byref(self._cs), C.byref(cview), C.byref(self.cfg), self.ws.data_ptr(),
+                                           self.ws_bytes, self.cap, _stream(), dL_dimage.data_ptr(), self.final_T.data_ptr(),
+                                           self.n_contrib.data_ptr(), C.byref(cg))
+        if rc:
+            raise FdgsError(rc, "fdgs_render_backward")
+
+    def l1_loss(self, target):
+        """loss += mean|image - target|; writes self.dL_dimage."""
+        rc = self.lib.fdgs_l1_loss(self.image.data_ptr(), target.data_ptr(), self.image.numel(), self.dL_dimage.data_ptr(),
+                                   self.loss.data_ptr(), _stream())
+        if rc:
+            raise FdgsError(rc, "fdgs_l1_loss")
+
+    def step_host(self, cview: CView, target_host, result_host, grads: Optional[dict]):
+        """One view end to end with HOST target / result buffers (fdgs_step_host)."""
+        cg = grads_struct(grads) if grads is not None else None
+        rc = self.lib.fdgs_step_host(C.byref(self._cs), C.byref(cview), C.byref(self.cfg), self.ws.data_ptr(), self.ws_bytes,
+                                     self.cap, _stream(), _ptr(target_host), self.target_dev.data_ptr(), self.image.data_ptr(),
+                                     self.final_T.data_ptr(), self.n_contrib.data_ptr(), self.dL_dimage.data_ptr(),
+                                     self.loss.data_ptr(), C.byref(cg) if cg is not None else None, result_host.data_ptr())
+        if rc:
+            raise FdgsError(rc, "fdgs_step_host")
+
+    # -- parity hooks -----------------------------------------------------------------------------
+    def export(self, what: int):
+        import torch
+        dev = self.ws.device
+        N, tiles = self.ds.N, ((self.width + 15) // 16) * ((self.height + 15) // 16)
+        status = torch.zeros(4, dtype=torch.int64, device=dev)
+        rc = self.lib.fdgs_debug_export(self.ws.data_ptr(), self.ws_bytes, EXPORT_STATUS, status.data_ptr(), 32, _stream())
+        if rc not in (OK, ERR_PAIR_OVERFLOW):
+            raise FdgsError(rc, "fdgs_debug_export(status)")
+        D, nvis, overflow = int(status[0]), int(status[1]), int(status[2])
+        if what == EXPORT_STATUS:
+            return dict(num_pairs=D, num_visible=nvis, overflow=overflow, pair_capacity=int(status[3]))
+        if overflow:
+            D = 0
+        shapes = {EXPORT_RECORDS: ((N, 12), torch.float32), EXPORT_RECTS: ((N, 4), torch.int32),
+                  EXPORT_TILES_TOUCHED: ((N,), torch.int32), EXPORT_OFFSETS: ((nvis,), torch.int32),
+                  EXPORT_SORTED_KEYS: ((D,), torch.int64), EXPORT_SORTED_VALS: ((D,), torch.int32),
+                  EXPORT_RANGES: ((tiles, 2), torch.int32), EXPORT_SPLAT_GRADS: ((N, 9), torch.float32),
+                  EXPORT_DEPTH_ORDER: ((nvis,), torch.int32)}
+        shape, dt = shapes[what]
+        out = torch.zeros(shape, dtype=dt, device=dev)
+        if out.numel() == 0:
+            return out
+        rc = self.lib.fdgs_debug_export(self.ws.data_ptr(), self.ws_bytes, what, out.data_ptr(), out.numel() * out.element_size(),
+                                        _stream())
+        if rc:
+            raise FdgsError(rc, f"fdgs_debug_export({what})")
+        return out

@@ -1,0 +1,114 @@
+"""GPU-side test helpers: run the CUDA path through the C-ABI binding and compare with the oracle
+following the protocol of DESIGN.md ("parity protocol").  Imports nothing from oracle/ itself; the
+oracle objects are passed in by the tests."""
+import numpy as np
+import torch
+
+from paper_2412_20720_b200 import fdgs
+
+FRAG_TOL = 1e-5      # north_star: footprint edge / cull threshold within 1e-5 relative -> flagged, counted, reported
+TIE_TOL = 1e-5       # adjacent depths within 1e-5 relative may swap
+MARGIN_TOL = 1e-4    # pixels whose alpha / transmittance test is within 1e-4 relative of its threshold
+
+
+def gpu_run(scene, view, cfg_overrides=None, pair_capacity=None, dL=None, with_mean2d=True):
+    """preprocess + forward (+ backward if dL is given) on cuda:0.  Returns a dict of numpy arrays."""
+    ds = fdgs.DeviceScene.from_scene(scene)
+    cfg = fdgs.default_config(**(cfg_overrides or {}))
+    cap = pair_capacity or max(1 << 16, 64 * max(scene.N, 1))
+    r = fdgs.Renderer(ds, view.width, view.height, cap, cfg)
+    cv = fdgs.make_view(view)
+    D, nvis = r.preprocess(cv, sync=True)
+    img = r.forward(cv)
+    torch.cuda.synchronize()
+    out = dict(num_pairs=D, num_visible=nvis, image=img.cpu().numpy().astype(np.float64),
+               final_T=r.final_T.cpu().numpy().astype(np.float64), n_contrib=r.n_contrib.cpu().numpy(),
+               records=r.export(fdgs.EXPORT_RECORDS).cpu().numpy().astype(np.float64),
+               rects=r.export(fdgs.EXPORT_RECTS).cpu().numpy(), ranges=r.export(fdgs.EXPORT_RANGES).cpu().numpy(),
+               sorted_vals=r.export(fdgs.EXPORT_SORTED_VALS).cpu().numpy(),
+               sorted_keys=r.export(fdgs.EXPORT_SORTED_KEYS).cpu().numpy(),
+               tiles_touched=r.export(fdgs.EXPORT_TILES_TOUCHED).cpu().numpy(), status=r.export(fdgs.EXPORT_STATUS))
+    if dL is not None:
+        g = ds.zero_grads(with_mean2d=with_mean2d)
+        r.backward(cv, torch.from_numpy(np.ascontiguousarray(dL, dtype=np.float32)).cuda(), g)
+        torch.cuda.synchronize()
+        out["grads"] = {k: (v.cpu().numpy().astype(np.float64) if v is not None else None) for k, v in g.items()}
+        out["g9"] = r.export(fdgs.EXPORT_SPLAT_GRADS).cpu().numpy().astype(np.float64)
+    out["renderer"], out["dscene"] = r, ds
+    return out
+
+
+def compare_prims(gpu, P, report):
+    """Cull decisions exact except fragile primitives; per-primitive values within the stage-wise tolerances."""
+    vis_o = P.status == 0
+    vis_g = gpu["tiles_touched"] > 0
+    fragile = P.fragility < FRAG_TOL
+    bad = (vis_o != vis_g) & ~fragile
+    report["cull_mismatch_fragile"] = int(((vis_o != vis_g) & fragile).sum())
+    assert bad.sum() == 0, f"{bad.sum()} non-fragile primitives with different cull decisions"
+    both = vis_o & vis_g
+    rec = gpu["records"][both]
+    rel = lambda a, b, absol=0.0: np.abs(a - b) / (np.abs(b) + absol)
+    if both.any():
+        scale_uv = np.maximum(np.abs(P.uv[both]), 1.0)
+        assert (np.abs(rec[:, 0:2] - P.uv[both]) / scale_uv).max() < 1e-5
+        assert rel(rec[:, 9], P.p_cam[both][:, 2]).max() < 1e-5
+        assert rel(rec[:, 11], P.w[both], 1e-6).max() < 1e-5
+        assert np.abs(rec[:, 6:9] - P.rgb[both]).max() < 2e-5
+        nrm = np.sqrt(P.conic[both][:, 0] * P.conic[both][:, 2])[:, None]        # conic error relative to sqrt(A C)
+        report["conic_max_rel"] = float((np.abs(rec[:, 2:5] - P.conic[both]) / nrm).max())
+        assert report["conic_max_rel"] < 1e-4
+        assert rel(rec[:, 10], P.radius[both]).max() < 1e-4
+        assert rel(rec[:, 5], P.opacity[both], 1e-7).max() < 1e-5
+        # rects must agree except for fragile footprints
+        rdiff = (gpu["rects"][both] != P.rect[both].astype(np.int64)).any(1)
+        assert (rdiff & ~fragile[both]).sum() == 0
+        report["rect_mismatch_fragile"] = int(rdiff.sum())
+    return fragile
+
+
+def compare_tile_lists(gpu, P, tile_off, tile_ids, fragile, report):
+    """Per tile: ordered id sequences bit-exact, except members that are fragile primitives and swaps of
+    adjacent near-tie depths; those are counted and reported.  Returns a bool mask of tiles that differ."""
+    ranges, vals = gpu["ranges"], gpu["sorted_vals"]
+    tiles = len(tile_off) - 1
+    bad_tiles = np.zeros(tiles, dtype=bool)
+    depth = P.p_cam[:, 2]
+    n_member, n_order = 0, 0
+    # the exported 64-bit keys must be sorted and consistent with (tile, depth bits of the GPU record)
+    keys = gpu["sorted_keys"].astype(np.uint64)
+    assert (np.diff(keys.astype(np.float64)) >= 0).all() if len(keys) > 1 else True
+    for t in range(tiles):
+        g = vals[ranges[t, 0]:ranges[t, 1]]
+        o = tile_ids[tile_off[t]:tile_off[t + 1]]
+        if len(g) == len(o) and np.array_equal(g, o):
+            continue
+        bad_tiles[t] = True
+        sg, so = set(g.tolist()), set(o.tolist())
+        for i in sg ^ so:
+            assert fragile[i], f"tile {t}: primitive {i} listed on one side only and not fragile"
+            n_member += 1
+        common = [i for i in g.tolist() if i in so]
+        ref = [i for i in o.tolist() if i in sg]
+        if common != ref:
+            d = depth[np.array(common)]
+            viol = d[:-1] > d[1:] * (1 + TIE_TOL) + 1e-12
+            assert not viol.any(), f"tile {t}: order differs beyond near-tie depths"
+            n_order += 1
+    report["tiles_differing"] = int(bad_tiles.sum())
+    report["membership_diffs_fragile"] = n_member
+    report["tiles_with_tie_swaps"] = n_order
+    return bad_tiles
+
+
+def flagged_pixels(bad_tiles, margin, width, height):
+    tx = (width + 15) // 16
+    flag = margin < MARGIN_TOL
+    ys, xs = np.mgrid[0:height, 0:width]
+    flag |= bad_tiles[(ys // 16) * tx + xs // 16]
+    return flag
+
+
+def rel_l2(a, b):
+    a, b = np.asarray(a, dtype=np.float64).ravel(), np.asarray(b, dtype=np.float64).ravel()
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))

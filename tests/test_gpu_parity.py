@@ -1,0 +1,113 @@
+"""GPU parity: the CUDA path (through the C ABI) against the float64 oracle, element by element on the
+same seeded inputs.  Tolerances are north_star's: per-tile lists bit-exact except flagged (fragile /
+near-tie) items which are counted and reported, image max-abs <= 1e-4, per-parameter gradient rel-L2 <= 1e-3."""
+import json
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from helpers import hand_scene, oracle_for
+from paper_2412_20720_b200 import scenes
+
+IMG_TOL = 1e-4
+GRAD_TOL = 1e-3
+PARAMS = ("mean", "log_scale", "quat_l", "quat_r", "opacity_logit", "sh")
+
+
+def _full_parity(scene, view_index=0, cfg=None, dL_mode="normal", check_grads=True, label=""):
+    import gpu_helpers as gh
+    view = scene.views[view_index]
+    o = oracle_for(scene, view_index, cfg=cfg)
+    P = o.prims()
+    img_o, fT_o, nc_o, margin = o.forward()
+    if dL_mode == "normal":
+        dL = scenes.upstream_normal(scene.seed, view.width, view.height).astype(np.float64)
+    else:   # L1 loss against a seeded target; the sign is taken from the ORACLE image and fed to both sides
+        tgt = scenes.target_image(scene.seed, view_index, view.width, view.height).astype(np.float64)
+        dL = np.sign(img_o - tgt) / img_o.size
+    gpu = gh.gpu_run(scene, view, cfg_overrides=cfg, dL=dL if check_grads else None)
+    rep = dict(label=label, N=scene.N, num_pairs_gpu=gpu["num_pairs"], num_visible_gpu=gpu["num_visible"])
+    fragile = gh.compare_prims(gpu, P, rep)
+    off, ids = o.tile_lists()
+    rep["num_pairs_oracle"] = int(off[-1])
+    bad_tiles = gh.compare_tile_lists(gpu, P, off, ids, fragile, rep)
+    flag = gh.flagged_pixels(bad_tiles, margin, view.width, view.height)
+    err = np.abs(gpu["image"] - img_o).max(0)
+    rep["flagged_pixels"] = int(flag.sum())
+    rep["image_max_abs"] = float(err[~flag].max()) if (~flag).any() else 0.0
+    rep["image_max_abs_flagged"] = float(err[flag].max()) if flag.any() else 0.0
+    assert rep["image_max_abs"] <= IMG_TOL, rep
+    assert flag.mean() < 0.02, rep
+    assert np.abs(gpu["final_T"] - fT_o)[~flag].max() <= IMG_TOL
+    assert (gpu["n_contrib"][~flag] == nc_o[~flag]).mean() > 0.999
+    if check_grads:
+        go = o.backward(dL)
+        keep = ~fragile
+        rep["g9_rel_l2"] = gh.rel_l2(gpu["g9"][keep], go["g9"][keep])
+        for k in PARAMS + ("mean2d",):
+            rep["grad_" + k] = gh.rel_l2(gpu["grads"][k][keep], go[k][keep])
+            assert rep["grad_" + k] <= GRAD_TOL, rep
+        culled = P.status != 0
+        for k in PARAMS:
+            assert np.abs(gpu["grads"][k][culled & keep]).max(initial=0.0) == 0.0
+    print("PARITY " + json.dumps(rep))
+    return rep, gpu, o
+
+
+def test_cfg1_tiny():
+    rep, gpu, o = _full_parity(scenes.tiny(), label="cfg1")
+    assert rep["num_pairs_gpu"] == rep["num_pairs_oracle"] or rep["membership_diffs_fragile"] > 0
+
+
+def test_cfg1_thresholds_off_and_marginal_off():
+    _full_parity(scenes.tiny(), cfg=dict(alpha_min=0.0, transmittance_min=0.0), label="cfg1 alpha_min=0")
+    _full_parity(scenes.tiny(), cfg=dict(marginal_min=0.0), label="cfg1 marginal_min=0")
+
+
+def test_fd_scene_translucent_large_splats():
+    _full_parity(scenes.fd_scene(100, 8), label="fd8")
+
+
+def test_cfg2_reduced_and_ragged():
+    # several tiles with a ragged right / bottom edge (250 x 190 is not a multiple of 16)
+    sc = scenes.single_object(N=20000, width=250, height=190)
+    _full_parity(sc, dL_mode="l1", label="cfg2 20k 250x190")
+
+
+def test_cfg2_full():
+    _full_parity(scenes.single_object(), dL_mode="l1", label="cfg2 100k 800x800")
+
+
+def test_cfg3_reduced_random_rotations():
+    # stress variant: fully random 4D rotations (large space-time tilt), 4 jittered views
+    sc = scenes.multiview_video(N=60000, width=338, height=254, n_views=2, quat_mode="random")
+    for vi in range(2):
+        _full_parity(sc, view_index=vi, dL_mode="l1", label=f"cfg3 60k random view{vi}")
+
+
+def test_cfg4_reduced_heavy_tails():
+    # driving-style corridor: camera inside the cloud, splats covering the whole screen
+    sc = scenes.driving(N=40000, width=480, height=320, n_views=1)
+    _full_parity(sc, dL_mode="l1", label="cfg4 40k 480x320")
+
+
+@pytest.mark.parametrize("L,n_time", [(0, 1), (2, 1), (1, 3), (3, 2)])
+def test_sh_degree_variants(L, n_time):
+    base = scenes.tiny()
+    K = n_time * (L + 1) ** 2
+    sh = 0.05 * scenes.normal(7, 40, base.N * K * 3).reshape(base.N, K, 3)
+    sh[:, 0, :] += 0.5
+    v = base.views[0]
+    view = scenes.View(v.view, v.fx, v.fy, v.cx, v.cy, v.width, v.height, 0.45, 0.8, (0.1, 0.3, 0.2))
+    sc = scenes.Scene("variant", L, n_time, base.mean, base.log_scale, base.quat_l, base.quat_r, base.opacity_logit,
+                      sh.astype(np.float32), [view], 7)
+    _full_parity(sc, label=f"L={L} n_time={n_time}")
+
+
+def test_cfg3_full_one_view():
+    """BASELINE.json's headline size in the launch configuration bench.py times: 1M Gaussians, 1352x1014."""
+    sc = scenes.multiview_video(n_views=1)
+    rep, gpu, o = _full_parity(sc, dL_mode="l1", label="cfg3 1M 1352x1014 view0")
+    assert rep["num_pairs_gpu"] > 1_000_000
