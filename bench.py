@@ -1,0 +1,265 @@
+#!/usr/bin/env python
+"""bench.py — BASELINE.json's metric on its headline config: forward+backward steps/s (and forward FPS) of the
+time-sliced tile rasterizer at 1M 4D Gaussians, 1352x1014, batch of 4 views (cfg3), seeded synthetic data.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+One JSON line on stdout (rank 0).  `value` = steps/s with everything resident in HBM; `e2e` = the same through
+fdgs_step_host with pinned HOST target images and the loss read back every view; `roofline` = the dominant kernel
+against the ALU issue roof derived in DESIGN.md; `cpu_baseline` = the float64 oracle on this box's host cores on a
+bounded sample (one of the four views).  --impl reference times that oracle as the reference arm.
+Multi-GPU: the path does not shard: N ranks render N independent replicas.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "fwd+bwd steps/s, 1M 4D Gaussians @1352x1014, batch of 4 views"
+WORKLOAD = "cfg3_video: N=1M, K=48 (L=3 x n_time=3), 1352x1014, fov 60, 4 jittered views at 4 seeded times, L1 loss"
+PAIR_CAPACITY = 16 * 1024 * 1024
+SM_COUNT, LANES_PER_SM, SM_MAX_HZ = 148, 128, 1.965e9
+ALU_PEAK_TLANE = SM_COUNT * LANES_PER_SM * SM_MAX_HZ / 1e12      # 37.2 T lane-instructions/s
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.proc = index, [], None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200"], stdout=subprocess.PIPE, text=True)
+            for line in self.proc.stdout:
+                self.rows.append([x.strip() for x in line.split(",")])
+        except Exception:
+            pass
+
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
+        self.join(timeout=2)
+        sm = sorted(int(r[0]) for r in self.rows if r and r[0].isdigit())
+        reasons = set()
+        for r in self.rows:
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if val == "Active":
+                    reasons.add(name)
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": int(self.rows[0][1]) if self.rows and self.rows[0][1].isdigit() else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_view_seconds(scene, view_index=0, repeats=1):
+    """The oracle as it stands: preprocess + forward + L1 gradient + backward of ONE view on the host cores."""
+    import numpy as np
+    import oracle
+    from paper_2412_20720_b200 import scenes
+    o = oracle.Oracle(**scene.arrays(), sh_degree=scene.sh_degree, n_time=scene.n_time)
+    v = scene.views[view_index]
+    tgt = scenes.target_image(scene.seed, view_index, v.width, v.height).astype(np.float64)
+    times = []
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        o.preprocess(v.view, (v.fx, v.fy, v.cx, v.cy), v.width, v.height, v.t, v.period_T, v.bg)
+        img = o.forward()[0]
+        o.backward(np.sign(img - tgt) / img.size)
+        times.append(time.perf_counter() - t0)
+    return times, oracle.num_threads()
+
+
+def run_reference(args):
+    """Reference arm = the float64 oracle (there is no upstream code).  Rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from paper_2412_20720_b200 import scenes
+    scene = scenes.multiview_video()
+    n_views = len(scene.views)
+    times, cores = oracle_view_seconds(scene, 0, repeats=args.warmup + args.steps)
+    timed = times[args.warmup:]
+    ms_step = 1e3 * n_views * sum(timed) / len(timed)          # a step = 4 views; each timed step samples one view
+    val = 1e3 / ms_step
+    sample = f"each step = view 0 of the {n_views} views (preprocess+forward+L1+backward), time scaled x{n_views}"
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": val, "unit": "steps/s", "n_gpus": args.gpus, "steps": args.steps,
+                      "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                      "dtype": "f64", "data": "synthetic", "config": {"workload": WORKLOAD},
+                      "cpu_baseline": {"value": val, "unit": "steps/s", "cores": cores, "kind": "oracle", "sample": sample},
+                      "e2e": {"value": val, "unit": "steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def run_fdgs(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2412_20720_b200 import build, fdgs, scenes
+    rank, world, local = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    build.build()
+    scene = scenes.multiview_video()
+    views = scene.views
+    n_views = len(views)
+    ds = fdgs.DeviceScene.from_scene(scene, device=dev)
+    r = fdgs.Renderer(ds, views[0].width, views[0].height, PAIR_CAPACITY)
+    cviews = [fdgs.make_view(v) for v in views]
+    tg_np = [scenes.target_image(scene.seed, i, views[0].width, views[0].height) for i in range(n_views)]
+    targets = [torch.from_numpy(t).to(dev) for t in tg_np]
+    targets_host = [torch.from_numpy(t).pin_memory() for t in tg_np]
+    loss_host = torch.zeros(n_views).pin_memory()
+    grads = ds.zero_grads()
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)     # > 126 MB L2
+
+    def zero_grads():
+        for g in grads.values():
+            if g is not None:
+                g.zero_()
+
+    def step_device():
+        zero_grads()
+        r.loss.zero_()
+        for cv, tg in zip(cviews, targets):
+            r.preprocess(cv)
+            r.forward(cv)
+            r.l1_loss(tg)
+            r.backward(cv, r.dL_dimage, grads)
+
+    def step_host():
+        zero_grads()
+        for i, cv in enumerate(cviews):
+            r.step_host(cv, targets_host[i], loss_host[i:i + 1], grads)
+
+    def forward_only(cv):
+        r.preprocess(cv)
+        r.forward(cv)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def timed(fn, steps, warmup):
+        """per-step CUDA events on the launching stream; L2 flushed (outside the events) between steps"""
+        for _ in range(warmup):
+            fn()
+        barrier()
+        evs = []
+        for _ in range(steps):
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            evs.append((e0, e1))
+        barrier()
+        ms = [a.elapsed_time(b) for a, b in evs]
+        tot = torch.tensor([sum(ms)], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(tot, op=dist.ReduceOp.MAX)
+        return float(tot[0]) / steps, ms
+
+    # ---- headline: fwd+bwd steps/s, inputs resident in HBM -------------------------------------------------
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+        time.sleep(0.3)
+    l0 = fdgs.launch_count()
+    ms_step, _ = timed(step_device, args.steps, args.warmup)
+    launches = (fdgs.launch_count() - l0) * args.steps // (args.steps + args.warmup)
+    clocks = sampler.stop() if sampler else None
+    status = r.export(fdgs.EXPORT_STATUS)
+    if status["overflow"]:
+        raise RuntimeError(f"pair capacity {PAIR_CAPACITY} exceeded: {status}")
+    loss_dev = float(r.loss[0])
+    # ---- end to end through the C ABI with host buffers ----------------------------------------------------
+    ms_e2e, _ = timed(step_host, max(3, args.steps // 2), 3)
+    # ---- forward-only FPS (one frame = preprocess + forward of one view) -----------------------------------
+    fps_ms = []
+    for cv in cviews:
+        m, _ = timed(lambda: forward_only(cv), 25, 5)
+        fps_ms.append(m)
+    ms_frame = sum(fps_ms) / len(fps_ms)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    # ---- per-stage times (events at the stage boundaries inside the library), one view at a time -----------
+    fdgs.set_stage_timing(True)
+    stage = {k: 0.0 for k in fdgs.STAGES}
+    work = {"walk": 0, "exp": 0, "comp": 0, "staged": 0, "walk_bwd": 0, "pairs": 0, "visible": 0}
+    reps = 5
+    for cv, tg in zip(cviews, targets):
+        for _ in range(reps):
+            flush.fill_(1)
+            r.preprocess(cv); r.forward(cv); r.l1_loss(tg); r.backward(cv, r.dL_dimage, grads)
+            for k, v in fdgs.stage_ms().items():
+                stage[k] += v / reps
+        w = r.blend_stats(cv)
+        st = r.export(fdgs.EXPORT_STATUS)
+        work["walk"] += w[0]; work["exp"] += w[1]; work["comp"] += w[2]; work["staged"] += w[3]
+        work["walk_bwd"] += int(r.n_contrib.sum()); work["pairs"] += st["num_pairs"]; work["visible"] += st["num_visible"]
+    fdgs.set_stage_timing(False)
+    # ---- roofline of the dominant kernel (algorithmic lane-instructions / measured time) ----
+    instr_fwd = 8 * work["walk"] + 3 * work["exp"] + 7 * work["comp"]
+    frac_exp = work["exp"] / max(work["walk"], 1)
+    instr_bwd = 8 * work["walk_bwd"] + 3 * frac_exp * work["walk_bwd"] + 50 * work["comp"]
+    dom = "blend_bwd" if stage["blend_bwd"] >= stage["blend_fwd"] else "blend_fwd"
+    instr = instr_bwd if dom == "blend_bwd" else instr_fwd
+    achieved = instr / n_views / (stage[dom] / n_views * 1e-3) / 1e12
+    roofline = {"kernel": dom + "_kernel", "bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TLANE, "unit": "Tlane-instr/s",
+                "frac": achieved / ALU_PEAK_TLANE, "traffic": None,
+                "peak_source": "derived: 148 SMs x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md unit counts and max clock)",
+                "algorithmic_lane_instr_per_launch": instr / n_views, "ms_per_launch": stage[dom] / n_views}
+    # ---- CPU baseline: the oracle on one of the four views ---------------------------------------------------
+    cpu = None
+    if not args.no_cpu_baseline:
+        t, cores = oracle_view_seconds(scene, 0, 1)
+        cpu = {"value": 1.0 / (n_views * t[0]), "unit": "steps/s", "cores": cores, "kind": "oracle",
+               "sample": f"view 0 of {n_views} (preprocess+forward+L1+backward at N=1M, 1352x1014) in {t[0]:.1f} s, scaled x{n_views}"}
+    img_bytes = 3 * views[0].width * views[0].height * 4
+    out = {"metric": METRIC, "value": world * 1e3 / ms_step, "unit": "steps/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "config": {"workload": WORKLOAD, "pair_capacity": PAIR_CAPACITY, "l2": "256 MB flush write between timed steps; parameters (644 MB) exceed L2",
+                      "multi_gpu": "replicas only"},
+           "forward_fps": world * 1e3 / ms_frame, "ms_per_frame": ms_frame,
+           "e2e": {"value": world * 1e3 / ms_e2e, "unit": "steps/s", "h2d_bytes_per_step": n_views * img_bytes, "d2h_bytes_per_step": n_views * 4,
+                   "ms_per_step": ms_e2e},
+           "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
+           "stage_ms_per_step": stage, "work_per_step": work, "loss": loss_dev,
+           "paper_context": "114 FPS forward on Plenoptic Video, hardware not named (PAPER.md Table 1, L347) - context only"}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="fdgs", choices=["fdgs", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "fdgs" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_fdgs(args)
+
+
+if __name__ == "__main__":
+    main()

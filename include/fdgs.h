@@ -141,6 +141,17 @@ int fdgs_step_host(const fdgs_scene *scene, const fdgs_view *view_host, const fd
 #define FDGS_EXPORT_DEPTH_ORDER 9   /* uint32[num_visible]: ids of the survivors sorted by (depth bits, id)   */
 int fdgs_debug_export(const void *ws, size_t ws_bytes, int what, void *dst, size_t dst_bytes, void *cuda_stream);
 
+/* Measurement hooks (bench.py).  fdgs_set_stage_timing(1) makes the three calls record CUDA events at
+ * their stage boundaries; fdgs_get_stage_ms waits for them and fills ms_host[8]: preprocess kernel, compaction +
+ * tile grid, depth sort, offsets + pair emission, tile sort, forward blend, backward blend, backward preprocess
+ * (-1 for a stage that has not run).  fdgs_debug_blend_stats re-walks the tile lists of the last forward on `ws`
+ * and writes uint64[4] to stats_dev: (pixel, splat) pairs walked, pairs reaching the exp2, pairs composited,
+ * splats staged — the algorithmic work of the blend kernels. */
+int fdgs_set_stage_timing(int enable);
+int fdgs_get_stage_ms(float *ms_host);
+int fdgs_debug_blend_stats(const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws, size_t ws_bytes, int32_t N,
+                           int32_t K, int64_t pair_capacity, void *cuda_stream, unsigned long long *stats_dev);
+
 /* Number of kernel launches the library has issued so far in this process (bench.py's gpu_launches). */
 int64_t fdgs_launch_count(void);
 

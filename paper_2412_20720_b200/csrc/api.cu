@@ -15,6 +15,13 @@ static int cuda_fail(cudaError_t e, const char* where) {
 }
 #define FDGS_CUDA(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, where); } while (0)
 
+// Optional per-stage timing (fdgs_set_stage_timing): CUDA events recorded on the caller's stream at the stage
+// boundaries; off by default so that the product path carries no event records.
+enum { EV_PRE0, EV_PRE1, EV_PRE2, EV_FWD0, EV_FWD1, EV_FWD2, EV_FWD3, EV_FWD4, EV_BWD0, EV_BWD1, EV_BWD2, EV_COUNT };
+static int g_timing = 0;
+static cudaEvent_t g_ev[EV_COUNT];
+static inline void mark(int which, cudaStream_t st) { if (g_timing) cudaEventRecord(g_ev[which], st); }
+
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 static int num_sms() {
@@ -114,10 +121,13 @@ int fdgs_preprocess(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config*
   WsHeader h; memset(&h, 0, sizeof(h));
   h.N = sc->N; h.K = K; h.W = v->width; h.H = v->height; h.pair_capacity = cap; h.tiles = (long long)vp.tiles_x * vp.tiles_y;
   FDGS_CUDA(cudaMemcpyAsync(&ws.hdr->N, &h.N, 6 * sizeof(long long), cudaMemcpyHostToDevice, st), "memcpy(header)");
+  mark(EV_PRE0, st);
   launch_preprocess_fwd(*sc, vp, cp, ws, st);                       // A1-A4 (+ coverage grid)
+  mark(EV_PRE1, st);
   launch_compact(ws, sc->N, st);                                    // survivors -> (depth bits, id)
   const int l2_passes = (ceil_log2((long long)vp.tiles_x * vp.tiles_y) + RADIX_BITS - 1) / RADIX_BITS;
   launch_tile_grid(ws, vp, cap, l2_passes > 0 ? l2_passes : 1, st); // A5/A8: list lengths -> ranges, D
+  mark(EV_PRE2, st);
   FDGS_CUDA(cudaGetLastError(), "preprocess launches");
   if (num_pairs_host || num_visible_host) {
     FDGS_CUDA(cudaStreamSynchronize(st), "preprocess sync");
@@ -140,12 +150,17 @@ static int forward_impl(const fdgs_scene* sc, const ViewParams& vp, const CfgPar
   FDGS_CUDA(cudaMemsetAsync(&ws.hdr->scan_ticket[1], 0, 9 * sizeof(unsigned int), st), "memset(tickets)");
   FDGS_CUDA(cudaMemsetAsync(ws.scan_state[1], 0, 8 * (((size_t)(sc->N > 0 ? sc->N : 1) + SCAN_TILE - 1) / SCAN_TILE + 1), st), "memset(scan)");
   const int sms = num_sms();
+  mark(EV_FWD0, st);
   const int l1 = launch_sort_pairs(ws, ws.l1_keys, ws.l1_vals, &ws.hdr->num_visible, sc->N, 32, SORT_ITEMS_L1, 0, false, sms, st);
+  mark(EV_FWD1, st);
   launch_offsets(ws, l1, sc->N, st);
   launch_duplicate(ws, l1, sc->N, vp, st);
+  mark(EV_FWD2, st);
   const int tile_bits = ceil_log2((long long)vp.tiles_x * vp.tiles_y);
   const int l2 = launch_sort_pairs(ws, ws.l2_keys, ws.l2_vals, &ws.hdr->num_pairs, cap, tile_bits, SORT_ITEMS_L2, 4, true, sms, st);
+  mark(EV_FWD3, st);
   launch_blend_fwd(ws, l2, vp, cp, image, final_T, n_contrib, st);
+  mark(EV_FWD4, st);
   FDGS_CUDA(cudaGetLastError(), "forward launches");
   *l1_buf_out = l1; *l2_buf_out = l2;
   return FDGS_OK;
@@ -192,8 +207,11 @@ int fdgs_render_backward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_co
   int l1, l2;
   sort_bufs(sc, vp, cap, &l1, &l2);
   if (sc->N > 0) FDGS_CUDA(cudaMemsetAsync(ws.g9, 0, sizeof(float) * 9 * (size_t)sc->N, st), "memset(g9)");
+  mark(EV_BWD0, st);
   launch_blend_bwd(ws, l2, vp, cp, dL_dimage, final_T, n_contrib, st);          // B1
+  mark(EV_BWD1, st);
   launch_preprocess_bwd(*sc, vp, cp, ws, l1, *g, st);                           // B2
+  mark(EV_BWD2, st);
   FDGS_CUDA(cudaGetLastError(), "backward launches");
   return FDGS_OK;
 }
@@ -234,6 +252,41 @@ int fdgs_step_host(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* 
 }
 
 int64_t fdgs_launch_count(void) { return g_launches; }
+
+int fdgs_set_stage_timing(int enable) {
+  if (enable && !g_timing) for (int i = 0; i < EV_COUNT; ++i) FDGS_CUDA(cudaEventCreate(&g_ev[i]), "event create");
+  if (!enable && g_timing) for (int i = 0; i < EV_COUNT; ++i) cudaEventDestroy(g_ev[i]);
+  g_timing = enable ? 1 : 0;
+  return FDGS_OK;
+}
+
+int fdgs_get_stage_ms(float* ms_host) {
+  if (!ms_host || !g_timing) return FDGS_ERR_INVALID;
+  const int pairs[8][2] = {{EV_PRE0, EV_PRE1}, {EV_PRE1, EV_PRE2}, {EV_FWD0, EV_FWD1}, {EV_FWD1, EV_FWD2},
+                           {EV_FWD2, EV_FWD3}, {EV_FWD3, EV_FWD4}, {EV_BWD0, EV_BWD1}, {EV_BWD1, EV_BWD2}};
+  for (int k = 0; k < 8; ++k) {
+    ms_host[k] = -1.f;
+    if (cudaEventSynchronize(g_ev[pairs[k][1]]) == cudaSuccess) cudaEventElapsedTime(&ms_host[k], g_ev[pairs[k][0]], g_ev[pairs[k][1]]);
+  }
+  cudaGetLastError();   // stages that never ran leave an error state behind: clear it
+  return FDGS_OK;
+}
+
+int fdgs_debug_blend_stats(const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes, int32_t N, int32_t K,
+                           int64_t cap, void* stream, unsigned long long* stats_dev) {
+  if (!v || !c || !ws_ptr || !stats_dev) return FDGS_ERR_INVALID;
+  const Workspace ws = carve(ws_ptr, N, K, v->width, v->height, cap);
+  if (ws.bytes > ws_bytes) return FDGS_ERR_WORKSPACE;
+  ViewParams vp; CfgParams cp;
+  make_params(v, c, vp, cp);
+  fdgs_scene sc; sc.N = N;
+  int l1, l2;
+  sort_bufs(&sc, vp, cap, &l1, &l2);
+  FDGS_CUDA(cudaMemsetAsync(stats_dev, 0, 4 * sizeof(unsigned long long), (cudaStream_t)stream), "memset(stats)");
+  launch_blend_stats(ws, l2, vp, cp, stats_dev, (cudaStream_t)stream);
+  FDGS_CUDA(cudaGetLastError(), "stats launch");
+  return FDGS_OK;
+}
 
 const char* fdgs_strerror(int code) {
   switch (code) {

@@ -29,10 +29,14 @@ __device__ __forceinline__ void stage_splat(const SplatRec* __restrict__ rec, co
   *s2 = make_float4(q2.x, ul, vl, 0.f);
 }
 
+// STATS = true: same walk, but counts the work instead of writing the image (fdgs_debug_blend_stats):
+//   stats[0] pairs walked (pixel x splat, until the pixel terminates), [1] pairs that reach the exp2,
+//   [2] pairs composited, [3] splats staged into shared memory (summed over tiles)
+template <bool STATS>
 __global__ void __launch_bounds__(256) blend_fwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
                                                         const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
                                                         float* __restrict__ image, float* __restrict__ final_T,
-                                                        unsigned int* __restrict__ n_contrib) {
+                                                        unsigned int* __restrict__ n_contrib, unsigned long long* stats) {
   __shared__ float4 s0[BATCH], s1[BATCH], s2[BATCH];
   const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -44,10 +48,12 @@ __global__ void __launch_bounds__(256) blend_fwd_kernel(const uint2* __restrict_
   const int n = (int)(range.y - range.x);
   float T = 1.f, Cr = 0.f, Cg = 0.f, Cb = 0.f;
   unsigned int last = 0;
+  unsigned int st_walk = 0, st_exp = 0, st_comp = 0, st_stage = 0;
   bool done = !inside;
   for (int base = 0; base < n; base += BATCH) {
     if (__syncthreads_and(done)) break;
     const int m = min(BATCH, n - base);
+    if (STATS && threadIdx.x == 0) st_stage += m;
     if ((int)threadIdx.x < m) stage_splat(rec, vals[range.x + base + threadIdx.x], ox, oy, &s0[threadIdx.x], &s1[threadIdx.x], &s2[threadIdx.x]);
     __syncthreads();
     if (__all_sync(0xffffffffu, done)) continue;     // whole 8x4 patch saturated: skip the batch (warp-uniform)
@@ -56,8 +62,10 @@ __global__ void __launch_bounds__(256) blend_fwd_kernel(const uint2* __restrict_
       const float e1 = fmaf(a.x, x, fmaf(a.y, y, a.w));
       const float e2 = fmaf(a.z, y, b.x);
       const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
+      if (STATS && !done) ++st_walk;
       if (done || l2a < cp.log2_alpha_min) continue;                 // alpha < alpha_min: skipped
       const float alpha = fminf(cp.alpha_max, ex2_approx(l2a));
+      if (STATS) ++st_exp;
       if (alpha < cp.alpha_min) continue;
       const float Tn = fmaf(-T, alpha, T);
       if (Tn < cp.transmittance_min) { done = true; continue; }      // the terminating splat is not composited
@@ -65,7 +73,18 @@ __global__ void __launch_bounds__(256) blend_fwd_kernel(const uint2* __restrict_
       Cr = fmaf(b.z, wgt, Cr); Cg = fmaf(b.w, wgt, Cg); Cb = fmaf(s2[j].x, wgt, Cb);
       T = Tn;
       last = base + j + 1;
+      if (STATS) ++st_comp;
     }
+  }
+  if (STATS) {
+    unsigned int v[4] = {st_walk, st_exp, st_comp, st_stage};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
+      if (lane == 0 && v[k]) atomicAdd(stats + k, (unsigned long long)v[k]);
+    }
+    return;
   }
   if (inside) {
     const size_t hw = (size_t)vp.width * vp.height, pix = (size_t)py * vp.width + px;
@@ -194,7 +213,12 @@ __global__ void __launch_bounds__(256) blend_bwd_kernel(const uint2* __restrict_
 
 void launch_blend_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
                       unsigned int* n_contrib, cudaStream_t st) {
-  blend_fwd_kernel<<<vp.tiles_x * vp.tiles_y, 256, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib);
+  blend_fwd_kernel<false><<<vp.tiles_x * vp.tiles_y, 256, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr);
+  ++g_launches;
+}
+
+void launch_blend_stats(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, unsigned long long* stats, cudaStream_t st) {
+  blend_fwd_kernel<true><<<vp.tiles_x * vp.tiles_y, 256, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, nullptr, nullptr, nullptr, stats);
   ++g_launches;
 }
 

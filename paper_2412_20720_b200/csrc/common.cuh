@@ -137,6 +137,7 @@ void launch_offsets(const Workspace& ws, int l1_buf, int N, cudaStream_t st);
 void launch_duplicate(const Workspace& ws, int l1_buf, int N, const ViewParams& vp, cudaStream_t st);
 void launch_blend_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
                       unsigned int* n_contrib, cudaStream_t st);
+void launch_blend_stats(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, unsigned long long* stats, cudaStream_t st);
 void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* dL_dimage,
                       const float* final_T, const unsigned int* n_contrib, cudaStream_t st);
 void launch_preprocess_bwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, int l1_buf,

@@ -55,17 +55,29 @@ __device__ __forceinline__ int geom_forward(const float4 mean, const float4 ls, 
   g.inv_nl = 1.0f / sqrtf(nl2); g.inv_nr = 1.0f / sqrtf(nr2);
 #pragma unroll
   for (int k = 0; k < 4; ++k) { g.s[k] = expf(lsv[k]); g.ql[k] = qlr[k] * g.inv_nl; g.qr[k] = qrr[k] * g.inv_nr; }
-  // eq. 8: R = L(q_l) R(q_r); eq. 7: Sigma = M M^T with M = R diag(s)
-  float Lm[4][4], Rm[4][4];
-  quat_left(g.ql, Lm); quat_right(g.qr, Rm);
+  // eq. 8: R = L(q_l) R(q_r); eq. 7: Sigma = M M^T with M = R diag(s).
+  // The 16 four-term dot products are taken in fp64 (~100 DFMA per primitive, nothing next to the HBM time):
+  // an entry of R that is small against its terms would otherwise carry ~1e-7 ABSOLUTE error, and the time
+  // row of R is multiplied by a scale s_t that is typically 30x the spatial ones, so Sigma_44 and the marginal
+  // weight would lose up to two digits for nearly time-orthogonal primitives.
+  {
+    double dl2 = 0.0, dr2 = 0.0, qld[4], qrd[4];
 #pragma unroll
-  for (int r = 0; r < 4; ++r)
+    for (int k = 0; k < 4; ++k) { dl2 = fma((double)qlr[k], (double)qlr[k], dl2); dr2 = fma((double)qrr[k], (double)qrr[k], dr2); }
+    const double il = rsqrt(dl2), ir = rsqrt(dr2);
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      float acc = Lm[r][0] * Rm[0][k];
-      acc = fmaf(Lm[r][1], Rm[1][k], acc); acc = fmaf(Lm[r][2], Rm[2][k], acc); acc = fmaf(Lm[r][3], Rm[3][k], acc);
-      g.R4[r][k] = acc; g.M[r][k] = acc * g.s[k];
-    }
+    for (int k = 0; k < 4; ++k) { qld[k] = qlr[k] * il; qrd[k] = qrr[k] * ir; }
+    const double a = qld[0], b = qld[1], c = qld[2], d = qld[3], p = qrd[0], q = qrd[1], r = qrd[2], t = qrd[3];
+    const double Ld[4][4] = {{a, -b, -c, -d}, {b, a, -d, c}, {c, d, a, -b}, {d, -c, b, a}};
+    const double Rd[4][4] = {{p, -q, -r, -t}, {q, p, t, -r}, {r, -t, p, q}, {t, r, -q, p}};
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const double acc = fma(Ld[i][0], Rd[0][k], fma(Ld[i][1], Rd[1][k], fma(Ld[i][2], Rd[2][k], Ld[i][3] * Rd[3][k])));
+        g.R4[i][k] = (float)acc; g.M[i][k] = (float)acc * g.s[k];
+      }
+  }
   // eq. 10: marginal weight, and the p(t) < marginal_min filter (L324)
   g.b = g.M[3][0] * g.M[3][0] + g.M[3][1] * g.M[3][1] + g.M[3][2] * g.M[3][2] + g.M[3][3] * g.M[3][3];
   g.dt = vp.t - mean.w;

@@ -21,7 +21,8 @@ OK, ERR_INVALID, ERR_WORKSPACE, ERR_CUDA, ERR_PAIR_OVERFLOW = 0, -1, -2, -3, -4
 
 EXPORTED_SYMBOLS = ["fdgs_default_config", "fdgs_workspace_bytes", "fdgs_preprocess", "fdgs_render_forward",
                     "fdgs_render_backward", "fdgs_l1_loss", "fdgs_step_host", "fdgs_debug_export",
-                    "fdgs_launch_count", "fdgs_strerror"]
+                    "fdgs_launch_count", "fdgs_strerror", "fdgs_set_stage_timing", "fdgs_get_stage_ms",
+                    "fdgs_debug_blend_stats"]
 
 
 class CScene(C.Structure):
@@ -72,6 +73,9 @@ def load():
     lib.fdgs_step_host.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, vp, vp, vp, vp,
                                    vp, vp, vp, C.POINTER(CGrads), vp]
     lib.fdgs_debug_export.argtypes = [vp, sz, C.c_int, vp, sz, vp]
+    lib.fdgs_set_stage_timing.argtypes = [C.c_int]
+    lib.fdgs_get_stage_ms.argtypes = [C.POINTER(C.c_float)]
+    lib.fdgs_debug_blend_stats.argtypes = [C.POINTER(CView), C.POINTER(CConfig), vp, sz, i32, i32, i64, vp, vp]
     lib.fdgs_launch_count.restype = i64
     lib.fdgs_strerror.restype = C.c_char_p
     lib.fdgs_strerror.argtypes = [C.c_int]
@@ -88,6 +92,24 @@ def strerror(code: int) -> str:
 
 def launch_count() -> int:
     return int(load().fdgs_launch_count())
+
+
+STAGES = ("preprocess", "compact+tile_grid", "sort_depth", "offsets+duplicate", "sort_tile", "blend_fwd", "blend_bwd",
+          "preprocess_bwd")
+
+
+def set_stage_timing(on: bool):
+    rc = load().fdgs_set_stage_timing(1 if on else 0)
+    if rc:
+        raise FdgsError(rc, "fdgs_set_stage_timing")
+
+
+def stage_ms() -> dict:
+    buf = (C.c_float * 8)()
+    rc = load().fdgs_get_stage_ms(buf)
+    if rc:
+        raise FdgsError(rc, "fdgs_get_stage_ms")
+    return {k: float(buf[i]) for i, k in enumerate(STAGES)}
 
 
 def default_config(**overrides) -> CConfig:
@@ -238,6 +260,17 @@ class Renderer:
                                      self.loss.data_ptr(), C.byref(cg) if cg is not None else None, result_host.data_ptr())
         if rc:
             raise FdgsError(rc, "fdgs_step_host")
+
+    # -- measurement hooks -----------------------------------------------------------------------
+    def blend_stats(self, cview: CView):
+        """(pairs walked, pairs reaching exp2, pairs composited, splats staged) of the last forward on this workspace."""
+        import torch
+        out = torch.zeros(4, dtype=torch.int64, device=self.ws.device)
+        rc = self.lib.fdgs_debug_blend_stats(C.byref(cview), C.byref(self.cfg), self.ws.data_ptr(), self.ws_bytes, self.ds.N,
+                                             self.ds.K, self.cap, _stream(), out.data_ptr())
+        if rc:
+            raise FdgsError(rc, "fdgs_debug_blend_stats")
+        return [int(x) for x in out.cpu()]
 
     # -- parity hooks -----------------------------------------------------------------------------
     def export(self, what: int):
