@@ -39,7 +39,7 @@ extern "C" {
 typedef struct {
   int32_t N;                  /* number of primitives, >= 0                                             */
   int32_t sh_degree;          /* spatial SH degree L in 0..3                                            */
-  int32_t n_time;             /* Fourier orders n = 0..n_time-1 of the 4DSH (eq. 20), >= 1        */
+  int32_t n_time;             /* Fourier orders n = 0..n_time-1 of the 4DSH (eq. 20), 1..8         */
   const float *mean;          /* [N,4]  (mu_x, mu_y, mu_z, mu_t)                               L135     */
   const float *log_scale;     /* [N,4]  S = diag(exp(.)), order (x,y,z,t)                      L128     */
   const float *quat_l;        /* [N,4]  q_l = (a,b,c,d), need not be unit (normalised inside)  L128     */

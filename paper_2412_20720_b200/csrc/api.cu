@@ -34,7 +34,7 @@ static int ceil_log2(long long v) { int b = 0; while ((1LL << b) < v) ++b; retur
 
 static int check_common(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, const void* ws) {
   if (!sc || !v || !c || !ws) return FDGS_ERR_INVALID;
-  if (sc->N < 0 || sc->sh_degree < 0 || sc->sh_degree > 3 || sc->n_time < 1) return FDGS_ERR_INVALID;
+  if (sc->N < 0 || sc->sh_degree < 0 || sc->sh_degree > 3 || sc->n_time < 1 || sc->n_time > 8) return FDGS_ERR_INVALID;
   if (v->width <= 0 || v->height <= 0 || !(v->fx > 0) || !(v->fy > 0) || !(v->period_T > 0)) return FDGS_ERR_INVALID;
   if (sc->N > 0) {
     if (!sc->mean || !sc->log_scale || !sc->quat_l || !sc->quat_r || !sc->opacity_logit || !sc->sh) return FDGS_ERR_INVALID;

@@ -29,6 +29,19 @@ __device__ __forceinline__ void stage_splat(const SplatRec* __restrict__ rec, co
   *s2 = make_float4(q2.x, ul, vl, 0.f);
 }
 
+// Conservative test "can this splat reach alpha >= alpha_min anywhere on the warp's 8x4 pixel patch?": in the whitened
+// coordinates (e1, e2) the patch is a parallelogram; its bounding box gives the lower bound
+//   min(e1^2 + e2^2) >= max(0,|e1(c)| - ca*hw - |cb|*hh)^2 + max(0,|e2(c)| - cc*hh)^2     (c = patch centre)
+// A splat is dropped only if even that bound (shrunk by a rounding slack) puts log2(alpha) below the skip threshold,
+// i.e. only pairs every pixel of the patch would skip anyway are removed: the result is bit-identical.
+__device__ __forceinline__ bool patch_hit(const float4 a, const float4 b, const float xm, const float ym, const float l2min) {
+  const float e1c = fmaf(a.x, xm, fmaf(a.y, ym, a.w)), e2c = fmaf(a.z, ym, b.x);
+  const float r1 = fmaf(-a.x, 3.5f, 1.5f * fabsf(a.y)), r2 = -a.z * 1.5f;      // half extents: 3.5 px in x, 1.5 px in y
+  const float m1 = fmaxf(0.f, fabsf(e1c) - r1), m2 = fmaxf(0.f, fabsf(e2c) - r2);
+  const float qmin = fmaf(m1, m1, m2 * m2);
+  return !(fmaf(qmin, 0.999f, -1e-3f) > b.y - l2min);
+}
+
 // STATS = true: same walk, but counts the work instead of writing the image (fdgs_debug_blend_stats):
 //   stats[0] pairs walked (pixel x splat, until the pixel terminates), [1] pairs that reach the exp2,
 //   [2] pairs composited, [3] splats staged into shared memory (summed over tiles)
@@ -44,6 +57,7 @@ __global__ void __launch_bounds__(256) blend_fwd_kernel(const uint2* __restrict_
   const int px = tx * TILE + lx, py = ty * TILE + ly;
   const bool inside = px < vp.width && py < vp.height;
   const float x = lx + 0.5f, y = ly + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
+  const float xm = (float)((warp & 1) << 3) + 4.0f, ym = (float)((warp >> 1) << 2) + 2.0f;   // patch centre (tile-local)
   const uint2 range = ranges[tile];
   const int n = (int)(range.y - range.x);
   float T = 1.f, Cr = 0.f, Cg = 0.f, Cb = 0.f;
@@ -57,23 +71,32 @@ __global__ void __launch_bounds__(256) blend_fwd_kernel(const uint2* __restrict_
     if ((int)threadIdx.x < m) stage_splat(rec, vals[range.x + base + threadIdx.x], ox, oy, &s0[threadIdx.x], &s1[threadIdx.x], &s2[threadIdx.x]);
     __syncthreads();
     if (__all_sync(0xffffffffu, done)) continue;     // whole 8x4 patch saturated: skip the batch (warp-uniform)
-    for (int j = 0; j < m; ++j) {
-      const float4 a = s0[j], b = s1[j];
-      const float e1 = fmaf(a.x, x, fmaf(a.y, y, a.w));
-      const float e2 = fmaf(a.z, y, b.x);
-      const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
-      if (STATS && !done) ++st_walk;
-      if (done || l2a < cp.log2_alpha_min) continue;                 // alpha < alpha_min: skipped
-      const float alpha = fminf(cp.alpha_max, ex2_approx(l2a));
-      if (STATS) ++st_exp;
-      if (alpha < cp.alpha_min) continue;
-      const float Tn = fmaf(-T, alpha, T);
-      if (Tn < cp.transmittance_min) { done = true; continue; }      // the terminating splat is not composited
-      const float wgt = alpha * T;
-      Cr = fmaf(b.z, wgt, Cr); Cg = fmaf(b.w, wgt, Cg); Cb = fmaf(s2[j].x, wgt, Cb);
-      T = Tn;
-      last = base + j + 1;
-      if (STATS) ++st_comp;
+    for (int jb = 0; jb < m; jb += 32) {
+      // lane l tests splat jb+l against the warp's patch; the ballot is the list of splats worth evaluating per pixel
+      unsigned int hits;
+      if (STATS) hits = jb + 32 <= m ? 0xffffffffu : ((1u << (m - jb)) - 1u);
+      else hits = __ballot_sync(0xffffffffu, jb + lane < m && patch_hit(s0[jb + lane], s1[jb + lane], xm, ym, cp.log2_alpha_min));
+      while (hits) {
+        const int j = jb + __ffs(hits) - 1;
+        hits &= hits - 1;
+        const float4 a = s0[j], b = s1[j];
+        const float e1 = fmaf(a.x, x, fmaf(a.y, y, a.w));
+        const float e2 = fmaf(a.z, y, b.x);
+        const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
+        if (STATS && !done) ++st_walk;
+        if (done || l2a < cp.log2_alpha_min) continue;                 // alpha < alpha_min: skipped
+        const float alpha = fminf(cp.alpha_max, ex2_approx(l2a));
+        if (STATS) ++st_exp;
+        if (alpha < cp.alpha_min) continue;
+        const float Tn = fmaf(-T, alpha, T);
+        if (Tn < cp.transmittance_min) { done = true; continue; }      // the terminating splat is not composited
+        const float wgt = alpha * T;
+        Cr = fmaf(b.z, wgt, Cr); Cg = fmaf(b.w, wgt, Cg); Cb = fmaf(s2[j].x, wgt, Cb);
+        T = Tn;
+        last = base + j + 1;
+        if (STATS) ++st_comp;
+      }
+      if (__all_sync(0xffffffffu, done)) break;
     }
   }
   if (STATS) {
@@ -133,6 +156,7 @@ __global__ void __launch_bounds__(256) blend_bwd_kernel(const uint2* __restrict_
   const int px = tx * TILE + lx, py = ty * TILE + ly;
   const bool inside = px < vp.width && py < vp.height;
   const float x = lx + 0.5f, y = ly + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
+  const float xm = (float)((warp & 1) << 3) + 4.0f, ym = (float)((warp >> 1) << 2) + 2.0f;
   const uint2 range = ranges[tile];
   const size_t hw = (size_t)vp.width * vp.height, pix = (size_t)py * vp.width + px;
   float T = 1.f, gr = 0.f, gg = 0.f, gb = 0.f;
@@ -161,7 +185,13 @@ __global__ void __launch_bounds__(256) blend_bwd_kernel(const uint2* __restrict_
     for (int k = 0; k < 9; ++k) s_acc[k][threadIdx.x] = 0.f;
     __syncthreads();
     if (lo_pos < warp_max) {
-      for (int j = m - 1; j >= 0; --j) {
+     for (int jb = ((m - 1) >> 5) << 5; jb >= 0; jb -= 32) {
+      unsigned int hits = __ballot_sync(0xffffffffu, jb + lane < m && lo_pos + jb + lane < warp_max &&
+                                                     patch_hit(s0[jb + lane], s1[jb + lane], xm, ym, cp.log2_alpha_min));
+      while (hits) {
+        const int bit = 31 - __clz(hits);
+        hits &= ~(1u << bit);
+        const int j = jb + bit;
         const float4 a = s0[j], b = s1[j], c = s2[j];
         const float e1 = fmaf(a.x, x, fmaf(a.y, y, a.w));
         const float e2 = fmaf(a.z, y, b.x);
@@ -199,6 +229,7 @@ __global__ void __launch_bounds__(256) blend_bwd_kernel(const uint2* __restrict_
         if ((lane & 3) == 0) atomicAdd(&s_acc[lane >> 2][j], red);
         if (lane == 1) atomicAdd(&s_acc[8][j], v_o);
       }
+     }
     }
     __syncthreads();
     if ((int)threadIdx.x < m) {

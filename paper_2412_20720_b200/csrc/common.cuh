@@ -74,6 +74,7 @@ struct Workspace {
   unsigned int* tiles_touched;       // [N]
   unsigned int* l1_keys[2];          // [N] fp32 depth bits of survivors (double buffer)
   unsigned int* l1_vals[2];          // [N] primitive ids of survivors; after the sort: depth order
+  unsigned int* vis_ids;             // [N] primitive ids of survivors in ascending id order (kept for the backward)
   unsigned int* offsets;             // [N] exclusive prefix sum of tiles_touched in depth order
   unsigned int* l2_keys[2];          // [cap] tile ids
   unsigned int* l2_vals[2];          // [cap] primitive ids
@@ -103,6 +104,7 @@ inline Workspace carve(void* base, long long N, long long K, long long W, long l
   w.tiles_touched = (unsigned int*)take(4 * Np);
   for (int i = 0; i < 2; ++i) w.l1_keys[i] = (unsigned int*)take(4 * Np);
   for (int i = 0; i < 2; ++i) w.l1_vals[i] = (unsigned int*)take(4 * Np);
+  w.vis_ids = (unsigned int*)take(4 * Np);
   w.offsets = (unsigned int*)take(4 * Np);
   for (int i = 0; i < 2; ++i) w.l2_keys[i] = (unsigned int*)take(4 * (size_t)cap);
   for (int i = 0; i < 2; ++i) w.l2_vals[i] = (unsigned int*)take(4 * (size_t)cap);

@@ -10,96 +10,172 @@ namespace fdgs {
 
 __device__ __forceinline__ float4 ldg4b(const float* p, long long i) { return __ldg(reinterpret_cast<const float4*>(p) + i); }
 
+// Per-k gradient of the real SH basis wrt (x,y,z) (polynomial extension), G[k*3 + c].
 template <int KD>
-__global__ void __launch_bounds__(128) preprocess_bwd_kernel(const fdgs_scene sc, const ViewParams vp, const CfgParams cp,
-                                                             const unsigned int* __restrict__ vis_list,
-                                                             const WsHeader* __restrict__ hdr, const float* __restrict__ g9,
-                                                             const fdgs_grads gr) {
-  const unsigned int slot = blockIdx.x * blockDim.x + threadIdx.x;
-  if (slot >= hdr->num_visible) return;
-  const int i = vis_list[slot];
-  const float4 mean = ldg4b(sc.mean, i), ls = ldg4b(sc.log_scale, i), qlr = ldg4b(sc.quat_l, i), qrr = ldg4b(sc.quat_r, i);
-  const float logit = __ldg(sc.opacity_logit + i);
-  Geom g;
-  if (geom_forward(mean, ls, qlr, qrr, logit, vp, cp, g) != G_VISIBLE) return;
-  const float* gp = g9 + (size_t)9 * i;
-  const float g_u = gp[0], g_v = gp[1], g_A = gp[2], g_B = gp[3], g_C = gp[4], g_o = gp[5];
-  const float g_c[3] = {gp[6], gp[7], gp[8]};
-  if (gr.mean2d) { gr.mean2d[2 * i] += g_u; gr.mean2d[2 * i + 1] += g_v; }
-  float d_muc[3] = {0.f, 0.f, 0.f}, d_dt = 0.f, d_b = 0.f;
+__device__ __forceinline__ void sh_grad_table(const float x, const float y, const float z, float* G) {
+#pragma unroll
+  for (int i = 0; i < 3 * KD; ++i) G[i] = 0.f;
+  if (KD > 1) { G[1 * 3 + 1] = -SH_C1; G[2 * 3 + 2] = SH_C1; G[3 * 3 + 0] = -SH_C1; }
+  if (KD > 4) {
+    G[4 * 3 + 0] = SH_C2 * y;  G[4 * 3 + 1] = SH_C2 * x;
+    G[5 * 3 + 1] = -SH_C2 * z; G[5 * 3 + 2] = -SH_C2 * y;
+    G[6 * 3 + 0] = -2.f * SH_C20 * x; G[6 * 3 + 1] = -2.f * SH_C20 * y; G[6 * 3 + 2] = 4.f * SH_C20 * z;
+    G[7 * 3 + 0] = -SH_C2 * z; G[7 * 3 + 2] = -SH_C2 * x;
+    G[8 * 3 + 0] = 2.f * SH_C22 * x; G[8 * 3 + 1] = -2.f * SH_C22 * y;
+  }
+  if (KD > 9) {
+    const float xx = x * x, yy = y * y, zz = z * z;
+    G[9 * 3 + 0] = -SH_C3 * 6.f * x * y;  G[9 * 3 + 1] = -SH_C3 * 3.f * (xx - yy);
+    G[10 * 3 + 0] = SH_C4 * y * z;        G[10 * 3 + 1] = SH_C4 * x * z;                      G[10 * 3 + 2] = SH_C4 * x * y;
+    G[11 * 3 + 0] = SH_C5 * 2.f * x * y;  G[11 * 3 + 1] = -SH_C5 * (4.f * zz - xx - 3.f * yy); G[11 * 3 + 2] = -SH_C5 * 8.f * y * z;
+    G[12 * 3 + 0] = -SH_C6 * 6.f * x * z; G[12 * 3 + 1] = -SH_C6 * 6.f * y * z;               G[12 * 3 + 2] = SH_C6 * (6.f * zz - 3.f * xx - 3.f * yy);
+    G[13 * 3 + 0] = -SH_C5 * (4.f * zz - 3.f * xx - yy); G[13 * 3 + 1] = SH_C5 * 2.f * x * y;  G[13 * 3 + 2] = -SH_C5 * 8.f * x * z;
+    G[14 * 3 + 0] = SH_C4 * x * z;        G[14 * 3 + 1] = -SH_C4 * y * z;                     G[14 * 3 + 2] = SH_C42 * (xx - yy);
+    G[15 * 3 + 0] = -SH_C3 * 3.f * (xx - yy); G[15 * 3 + 1] = SH_C3 * 6.f * x * y;
+  }
+}
 
-  // ---- (A4) colour -------------------------------------------------------------------------
-  {
-    float dir[3], inv_rho;
-    {
-      const float dx = g.muc[0] - vp.cam[0], dy = g.muc[1] - vp.cam[1], dz = g.muc[2] - vp.cam[2];
-      inv_rho = 1.0f / sqrtf(dx * dx + dy * dy + dz * dz);
-      dir[0] = dx * inv_rho; dir[1] = dy * inv_rho; dir[2] = dz * inv_rho;
-    }
-    float Y[KD], a[KD];
+constexpr int BWD_WARPS = 4;
+// per-survivor table in shared memory: Y[16] | gradY[48] | cos_n[8] | -omega_n sin_n [8] | masked dL/dc [3]; odd stride
+constexpr int TAB_Y = 0, TAB_G = 16, TAB_CN = 64, TAB_WS = 72, TAB_GC = 80, TAB_STRIDE = 85;
+
+// A warp owns 32 consecutive survivors (ascending primitive id).  Lane s runs the per-primitive chain of survivor s;
+// the colour block (12K B of coefficients read + 12K B of coefficient gradients read-modify-written) is walked by the
+// whole warp, one survivor at a time, with fully coalesced 128-bit accesses.
+template <int KD>
+__global__ void __launch_bounds__(32 * BWD_WARPS) preprocess_bwd_kernel(const fdgs_scene sc, const ViewParams vp, const CfgParams cp,
+                                                                        const unsigned int* __restrict__ vis_list,
+                                                                        const WsHeader* __restrict__ hdr, const float* __restrict__ g9,
+                                                                        const SplatRec* __restrict__ rec, const fdgs_grads gr) {
+  __shared__ float tab[BWD_WARPS][32][TAB_STRIDE];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned int n_vis = hdr->num_visible;
+  const unsigned int warp_slot = (blockIdx.x * BWD_WARPS + warp) * 32;
+  if (warp_slot >= n_vis) return;
+  const unsigned int slot = warp_slot + lane;
+  const bool have = slot < n_vis;
+  int i = 0;
+  Geom g;
+  bool live = false;
+  float g_u = 0.f, g_v = 0.f, g_A = 0.f, g_B = 0.f, g_C = 0.f, g_o = 0.f;
+  float dir[3] = {0.f, 0.f, 1.f}, inv_rho = 0.f;
+  float* my = tab[warp][lane];
+  if (have) {
+    i = vis_list[slot];
+    const float4 mean = ldg4b(sc.mean, i), ls = ldg4b(sc.log_scale, i), qlr = ldg4b(sc.quat_l, i), qrr = ldg4b(sc.quat_r, i);
+    live = geom_forward(mean, ls, qlr, qrr, __ldg(sc.opacity_logit + i), vp, cp, g) == G_VISIBLE;
+  }
+  if (live) {
+    const float* gp = g9 + (size_t)9 * i;
+    g_u = gp[0]; g_v = gp[1]; g_A = gp[2]; g_B = gp[3]; g_C = gp[4]; g_o = gp[5];
+    const float dx = g.muc[0] - vp.cam[0], dy = g.muc[1] - vp.cam[1], dz = g.muc[2] - vp.cam[2];
+    inv_rho = 1.0f / sqrtf(dx * dx + dy * dy + dz * dz);
+    dir[0] = dx * inv_rho; dir[1] = dy * inv_rho; dir[2] = dz * inv_rho;
+    float Y[KD], G[3 * KD];
     sh_basis<KD>(dir[0], dir[1], dir[2], Y);
+    sh_grad_table<KD>(dir[0], dir[1], dir[2], G);
 #pragma unroll
-    for (int k = 0; k < KD; ++k) a[k] = 0.f;
-    const float* coef = sc.sh + (size_t)i * sc.n_time * KD * 3;
-    float* dcoef = gr.sh + (size_t)i * sc.n_time * KD * 3;
+    for (int k = 0; k < KD; ++k) my[TAB_Y + k] = Y[k];
+#pragma unroll
+    for (int k = 0; k < 3 * KD; ++k) my[TAB_G + k] = G[k];
     const float dtT = g.dt * vp.inv_T;
-    // first pass: un-clamped colour (the clamp state decides which channels carry gradient)
-    float raw[3] = {0.5f, 0.5f, 0.5f};
     for (int n = 0; n < sc.n_time; ++n) {
-      const float cn = cospif(2.0f * (float)n * dtT);
-      const float* cf = coef + (size_t)n * KD * 3;
+      my[TAB_CN + n] = cospif(2.0f * (float)n * dtT);
+      my[TAB_WS + n] = -6.283185307179586f * (float)n * vp.inv_T * sinpif(2.0f * (float)n * dtT);
+    }
+    // the colour clamp at 0 was active iff the stored (clamped) colour is 0: those channels carry no gradient
+    const float4 q1 = __ldg(reinterpret_cast<const float4*>(rec + i) + 1);
+    const float cb = __ldg(reinterpret_cast<const float*>(rec + i) + 8);
+    my[TAB_GC + 0] = q1.z > 0.f ? gp[6] : 0.f; my[TAB_GC + 1] = q1.w > 0.f ? gp[7] : 0.f; my[TAB_GC + 2] = cb > 0.f ? gp[8] : 0.f;
+    if (gr.mean2d) { gr.mean2d[2 * i] += g_u; gr.mean2d[2 * i + 1] += g_v; }
+  }
+  __syncwarp();
+  // ---- (A4) colour: warp-cooperative walk over each survivor's coefficient block ------------------------
+  const int rec_len = sc.n_time * KD * 3;
+  const unsigned int live_mask = __ballot_sync(0xffffffffu, live);
+  float gdx = 0.f, gdy = 0.f, gdz = 0.f, e_dt = 0.f;
+  for (int s = 0; s < 32; ++s) {
+    if (!((live_mask >> s) & 1u)) continue;
+    const int id = __shfl_sync(0xffffffffu, i, s);
+    const float* t = tab[warp][s];
+    const float* coef = sc.sh + (size_t)id * rec_len;
+    float* dcoef = gr.sh + (size_t)id * rec_len;
+    float ax = 0.f, ay = 0.f, az = 0.f, ad = 0.f;
+    if ((rec_len & 3) == 0) {
+      for (int j = lane; j < (rec_len >> 2); j += 32) {
+        const float4 c4 = __ldg(reinterpret_cast<const float4*>(coef) + j);
+        float4 d4 = reinterpret_cast<float4*>(dcoef)[j];
+        const float cv[4] = {c4.x, c4.y, c4.z, c4.w};
+        float dv[4] = {d4.x, d4.y, d4.z, d4.w};
 #pragma unroll
-      for (int k = 0; k < KD; ++k) {
-        const float yk = cn * Y[k];
-        raw[0] = fmaf(__ldg(cf + 3 * k), yk, raw[0]); raw[1] = fmaf(__ldg(cf + 3 * k + 1), yk, raw[1]); raw[2] = fmaf(__ldg(cf + 3 * k + 2), yk, raw[2]);
+        for (int q = 0; q < 4; ++q) {
+          const int e = 4 * j + q, n = e / (3 * KD), rem = e - n * 3 * KD, k = rem / 3, ch = rem - 3 * k;
+          const float yk = t[TAB_Y + k], cn = t[TAB_CN + n], gc = t[TAB_GC + ch];
+          dv[q] = fmaf(gc * cn, yk, dv[q]);
+          const float sv = cv[q] * gc, sc_n = sv * cn;
+          ad = fmaf(sv * t[TAB_WS + n], yk, ad);
+          ax = fmaf(sc_n, t[TAB_G + 3 * k], ax); ay = fmaf(sc_n, t[TAB_G + 3 * k + 1], ay); az = fmaf(sc_n, t[TAB_G + 3 * k + 2], az);
+        }
+        reinterpret_cast<float4*>(dcoef)[j] = make_float4(dv[0], dv[1], dv[2], dv[3]);
+      }
+    } else {
+      for (int e = lane; e < rec_len; e += 32) {
+        const int n = e / (3 * KD), rem = e - n * 3 * KD, k = rem / 3, ch = rem - 3 * k;
+        const float yk = t[TAB_Y + k], cn = t[TAB_CN + n], gc = t[TAB_GC + ch];
+        dcoef[e] = fmaf(gc * cn, yk, dcoef[e]);
+        const float sv = __ldg(coef + e) * gc, sc_n = sv * cn;
+        ad = fmaf(sv * t[TAB_WS + n], yk, ad);
+        ax = fmaf(sc_n, t[TAB_G + 3 * k], ax); ay = fmaf(sc_n, t[TAB_G + 3 * k + 1], ay); az = fmaf(sc_n, t[TAB_G + 3 * k + 2], az);
       }
     }
-    const float gc0 = raw[0] > 0.f ? g_c[0] : 0.f, gc1 = raw[1] > 0.f ? g_c[1] : 0.f, gc2 = raw[2] > 0.f ? g_c[2] : 0.f;
-    float e_dt = 0.f;
-    for (int n = 0; n < sc.n_time; ++n) {
-      const float cn = cospif(2.0f * (float)n * dtT), sn = sinpif(2.0f * (float)n * dtT);
-      const float om = 6.283185307179586f * (float)n * vp.inv_T;
-      const float* cf = coef + (size_t)n * KD * 3;
-      float* dcf = dcoef + (size_t)n * KD * 3;
 #pragma unroll
-      for (int k = 0; k < KD; ++k) {
-        const float yk = cn * Y[k];
-        const float s = gc0 * __ldg(cf + 3 * k) + gc1 * __ldg(cf + 3 * k + 1) + gc2 * __ldg(cf + 3 * k + 2);
-        dcf[3 * k] += gc0 * yk; dcf[3 * k + 1] += gc1 * yk; dcf[3 * k + 2] += gc2 * yk;
-        a[k] = fmaf(cn, s, a[k]);
-        e_dt = fmaf(-om * sn * Y[k], s, e_dt);
-      }
+    for (int o = 16; o > 0; o >>= 1) {
+      ax += __shfl_xor_sync(0xffffffffu, ax, o); ay += __shfl_xor_sync(0xffffffffu, ay, o);
+      az += __shfl_xor_sync(0xffffffffu, az, o); ad += __shfl_xor_sync(0xffffffffu, ad, o);
     }
-    d_dt += e_dt;
-    float gd[3];
-    sh_grad<KD>(dir[0], dir[1], dir[2], a, gd);
-    const float dd = gd[0] * dir[0] + gd[1] * dir[1] + gd[2] * dir[2];
-#pragma unroll
-    for (int r = 0; r < 3; ++r) d_muc[r] += (gd[r] - dir[r] * dd) * inv_rho;
+    if (lane == s) { gdx = ax; gdy = ay; gdz = az; e_dt = ad; }
+  }
+  if (!live) return;
+  float d_muc[3] = {0.f, 0.f, 0.f}, d_dt = e_dt, d_b = 0.f;
+  {
+    const float dd = gdx * dir[0] + gdy * dir[1] + gdz * dir[2];
+    d_muc[0] = (gdx - dir[0] * dd) * inv_rho; d_muc[1] = (gdy - dir[1] * dd) * inv_rho; d_muc[2] = (gdz - dir[2] * dd) * inv_rho;
   }
 
   // ---- conic -> Sigma_2d -> B -> (T, N) ------------------------------------------------------
-  const float idet = 1.0f / g.det;
-  const float A = g.c2 * idet, B = -g.b2 * idet, C = g.a2 * idet;
-  // G2 = -Q G_Q Q,  G_Q = [[g_A, g_B/2],[g_B/2, g_C]]
-  const float h = 0.5f * g_B;
-  const float qg00 = A * g_A + B * h, qg01 = A * h + B * g_C, qg10 = B * g_A + C * h, qg11 = B * h + C * g_C;
-  const float G2_00 = -(qg00 * A + qg01 * B), G2_01 = -(qg00 * B + qg01 * C), G2_11 = -(qg10 * B + qg11 * C);
-  float dBm[2][4], dT[2][3], dNm[3][4];
+  // G2 = -Q G_Q Q with G_Q = [[g_A, g_B/2],[g_B/2, g_C]], dB = 2 G2 B, dT = dB N^T, dN = T^T dB.
+  // For elongated splats Q is nearly singular and these products cancel by the squared axis ratio, so this block
+  // (about 100 DFMA per survivor) is carried in fp64 from the fp32 factor B.
+  float dT[2][3], dNm[3][4];
+  {
+    double Bd[2][4], n0 = 0.0, n1 = 0.0, d01 = 0.0, minors = 0.0;
 #pragma unroll
-  for (int k = 0; k < 4; ++k) {
-    dBm[0][k] = 2.f * (G2_00 * g.Bm[0][k] + G2_01 * g.Bm[1][k]);
-    dBm[1][k] = 2.f * (G2_01 * g.Bm[0][k] + G2_11 * g.Bm[1][k]);
-  }
+    for (int k = 0; k < 4; ++k) { Bd[0][k] = g.Bm[0][k]; Bd[1][k] = g.Bm[1][k]; n0 = fma(Bd[0][k], Bd[0][k], n0); n1 = fma(Bd[1][k], Bd[1][k], n1); d01 = fma(Bd[0][k], Bd[1][k], d01); }
 #pragma unroll
-  for (int r = 0; r < 2; ++r)
+    for (int p = 0; p < 4; ++p)
+#pragma unroll
+      for (int q = p + 1; q < 4; ++q) { const double m = Bd[0][p] * Bd[1][q] - Bd[0][q] * Bd[1][p]; minors = fma(m, m, minors); }
+    const double dil = cp.dilation, det = fma(dil, dil + n0 + n1, minors), idet = 1.0 / det;
+    const double A = (n1 + dil) * idet, B = -d01 * idet, C = (n0 + dil) * idet;
+    const double h = 0.5 * (double)g_B, gA = g_A, gC = g_C;
+    const double qg00 = A * gA + B * h, qg01 = A * h + B * gC, qg10 = B * gA + C * h, qg11 = B * h + C * gC;
+    const double G2_00 = -(qg00 * A + qg01 * B), G2_01 = -(qg00 * B + qg01 * C), G2_11 = -(qg10 * B + qg11 * C);
+    double dB[2][4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      dB[0][k] = 2.0 * (G2_00 * Bd[0][k] + G2_01 * Bd[1][k]);
+      dB[1][k] = 2.0 * (G2_01 * Bd[0][k] + G2_11 * Bd[1][k]);
+    }
+#pragma unroll
+    for (int r = 0; r < 2; ++r)
+#pragma unroll
+      for (int q = 0; q < 3; ++q)
+        dT[r][q] = (float)(dB[r][0] * g.Nm[q][0] + dB[r][1] * g.Nm[q][1] + dB[r][2] * g.Nm[q][2] + dB[r][3] * g.Nm[q][3]);
 #pragma unroll
     for (int q = 0; q < 3; ++q)
-      dT[r][q] = dBm[r][0] * g.Nm[q][0] + dBm[r][1] * g.Nm[q][1] + dBm[r][2] * g.Nm[q][2] + dBm[r][3] * g.Nm[q][3];
 #pragma unroll
-  for (int q = 0; q < 3; ++q)
-#pragma unroll
-    for (int k = 0; k < 4; ++k) dNm[q][k] = g.T[0][q] * dBm[0][k] + g.T[1][q] * dBm[1][k];
+      for (int k = 0; k < 4; ++k) dNm[q][k] = (float)(g.T[0][q] * dB[0][k] + g.T[1][q] * dB[1][k]);
+  }
 
   // ---- T = J W, J(p), pinhole --------------------------------------------------------------
   {
@@ -221,9 +297,10 @@ void launch_preprocess_bwd(const fdgs_scene& sc, const ViewParams& vp, const Cfg
                            const fdgs_grads& gr, cudaStream_t st) {
   if (sc.N <= 0) return;
   // the survivor count lives on the device: launch for all N slots, surplus threads exit at once
-  const int threads = 128, blocks = (sc.N + threads - 1) / threads;
+  const int threads = 32 * BWD_WARPS, blocks = (sc.N + threads - 1) / threads;
+  (void)l1_buf;
   const int KD = (sc.sh_degree + 1) * (sc.sh_degree + 1);
-#define FDGS_LAUNCH(KDV) preprocess_bwd_kernel<KDV><<<blocks, threads, 0, st>>>(sc, vp, cp, ws.l1_vals[l1_buf], ws.hdr, ws.g9, gr)
+#define FDGS_LAUNCH(KDV) preprocess_bwd_kernel<KDV><<<blocks, threads, 0, st>>>(sc, vp, cp, ws.vis_ids, ws.hdr, ws.g9, ws.rec, gr)
   if (KD == 1) FDGS_LAUNCH(1); else if (KD == 4) FDGS_LAUNCH(4); else if (KD == 9) FDGS_LAUNCH(9); else FDGS_LAUNCH(16);
 #undef FDGS_LAUNCH
   ++g_launches;

@@ -63,7 +63,7 @@ __device__ __forceinline__ unsigned int lookback_prefix(volatile unsigned long l
 __global__ void __launch_bounds__(SCAN_THREADS) compact_kernel(const unsigned int* __restrict__ tiles_touched,
                                                                const SplatRec* __restrict__ rec, const int N, WsHeader* hdr,
                                                                unsigned long long* state, unsigned int* __restrict__ keys,
-                                                               unsigned int* __restrict__ vals) {
+                                                               unsigned int* __restrict__ vals, unsigned int* __restrict__ vis_ids) {
   __shared__ unsigned int warp_sums[33], s_tile, s_prefix;
   if (threadIdx.x == 0) s_tile = atomicAdd(&hdr->scan_ticket[0], 1u);
   __syncthreads();
@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) compact_kernel(const unsigned in
   unsigned int pos = prefix + excl;
 #pragma unroll
   for (int k = 0; k < SCAN_ITEMS; ++k)
-    if (flags & (1u << k)) { keys[pos] = __float_as_uint(rec[base + k].depth); vals[pos] = (unsigned int)(base + k); ++pos; }
+    if (flags & (1u << k)) { keys[pos] = __float_as_uint(rec[base + k].depth); vals[pos] = (unsigned int)(base + k); vis_ids[pos] = (unsigned int)(base + k); ++pos; }
   if (tile == gridDim.x - 1 && threadIdx.x == 0) hdr->num_visible = prefix + total;
 }
 
@@ -209,7 +209,7 @@ __global__ void l1_loss_kernel(const float* __restrict__ image, const float* __r
 void launch_compact(const Workspace& ws, int N, cudaStream_t st) {
   if (N <= 0) return;
   const int blocks = (N + SCAN_TILE - 1) / SCAN_TILE;
-  compact_kernel<<<blocks, SCAN_THREADS, 0, st>>>(ws.tiles_touched, ws.rec, N, ws.hdr, ws.scan_state[0], ws.l1_keys[0], ws.l1_vals[0]);
+  compact_kernel<<<blocks, SCAN_THREADS, 0, st>>>(ws.tiles_touched, ws.rec, N, ws.hdr, ws.scan_state[0], ws.l1_keys[0], ws.l1_vals[0], ws.vis_ids);
   ++g_launches;
 }
 

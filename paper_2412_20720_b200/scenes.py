@@ -56,6 +56,13 @@ class View:
     period_T: float
     bg: tuple = (0.0, 0.0, 0.0)
 
+    def as_fp32(self) -> "View":
+        """The boundary takes fp32 scalars: a copy whose scalars are fp32-representable, so that the CUDA path and the
+        float64 oracle receive bit-identical inputs.  All generators below return such views."""
+        r = lambda x: float(np.float32(x))
+        return View(np.asarray(self.view, dtype=np.float32), r(self.fx), r(self.fy), r(self.cx), r(self.cy), self.width, self.height,
+                    r(self.t), r(self.period_T), tuple(r(b) for b in self.bg))
+
 
 @dataclass
 class Scene:
@@ -155,7 +162,7 @@ def tiny(seed: int = 0, N: int = 256) -> Scene:
     fx, fy, cx, cy = _pinhole(64, 64, 50.0)
     V = np.eye(4)
     V[2, 3] = 4.0      # camera at (0,0,-4) looking +z at the origin
-    view = View(_f32(V), fx, fy, cx, cy, 64, 64, 0.5, 1.0)
+    view = View(_f32(V), fx, fy, cx, cy, 64, 64, 0.5, 1.0).as_fp32()
     return Scene("cfg1_tiny", 1, 2, _f32(mean), _f32(ls), _f32(ql), _f32(qr), _f32(logit), _f32(sh), [view], seed)
 
 
@@ -174,7 +181,7 @@ def single_object(seed: int = 2, N: int = 100_000, width: int = 800, height: int
     el = np.deg2rad(-30 + 60 * uniform(seed, 51, 1)[0])
     cam = 4.0 * np.array([np.cos(el) * np.sin(az), np.sin(el), -np.cos(el) * np.cos(az)])
     t = float(uniform(seed, 52, 1)[0])
-    view = View(_f32(_look_at(cam, np.zeros(3))), fx, fy, cx, cy, width, height, t, 1.0)
+    view = View(_f32(_look_at(cam, np.zeros(3))), fx, fy, cx, cy, width, height, t, 1.0).as_fp32()
     return Scene("cfg2_object", 3, 3, _f32(mean), _f32(ls), _f32(ql), _f32(qr), _f32(logit), _f32(sh), [view], seed)
 
 
@@ -202,7 +209,7 @@ def multiview_video(seed: int = 3, N: int = 1_000_000, width: int = 1352, height
         V[:3, :3] = _axis_angle(axis, ang)
         V[:3, 3] = trans
         t = 10.0 * float(uniform(seed, 90 + k, 1)[0])
-        views.append(View(_f32(V), fx, fy, cx, cy, width, height, t, 10.0))
+        views.append(View(_f32(V), fx, fy, cx, cy, width, height, t, 10.0).as_fp32())
     return Scene("cfg3_video", 3, 3, _f32(mean), _f32(ls), _f32(ql), _f32(qr), _f32(logit), _f32(sh), views, seed)
 
 
@@ -222,7 +229,7 @@ def driving(seed: int = 4, N: int = 3_000_000, width: int = 1920, height: int = 
         t = 20.0 * float(uniform(seed, 90 + k, 1)[0])
         V = np.eye(4)
         V[2, 3] = -(10.0 + 4.0 * t)     # camera at (0,0,10+4t) looking +z
-        views.append(View(_f32(V), fx, fy, cx, cy, width, height, t, 20.0))
+        views.append(View(_f32(V), fx, fy, cx, cy, width, height, t, 20.0).as_fp32())
     return Scene("cfg4_driving", 3, 2, _f32(mean), _f32(ls), _f32(ql), _f32(qr), _f32(logit), _f32(sh), views, seed)
 
 
@@ -230,7 +237,7 @@ def sweep(seed: int = 3, N: int = 1_000_000, width: int = 1352, height: int = 10
     """cfg5: cfg3 distributions, fixed base camera, n_frames query times evenly spaced over [0,10]."""
     mean, ls, ql, qr, logit, sh = _video_params(seed, N)
     fx, fy, cx, cy = _pinhole(width, height, 60.0)
-    views = [View(_f32(np.eye(4)), fx, fy, cx, cy, width, height, 10.0 * k / max(1, n_frames - 1), 10.0)
+    views = [View(_f32(np.eye(4)), fx, fy, cx, cy, width, height, 10.0 * k / max(1, n_frames - 1), 10.0).as_fp32()
              for k in range(n_frames)]
     return Scene("cfg5_sweep", 3, 3, _f32(mean), _f32(ls), _f32(ql), _f32(qr), _f32(logit), _f32(sh), views, seed)
 
@@ -260,5 +267,5 @@ def fd_scene(seed: int, N: int = 8) -> Scene:
     V = np.eye(4)
     V[:3, :3] = _axis_angle(np.array([0.3, 1.0, 0.2]), 0.2)
     V[:3, 3] = np.array([0.1, -0.05, 4.0])
-    view = View(_f32(V), fx, fy, cx, cy, 64, 64, 0.5, 1.0, (0.1, 0.2, 0.3))
+    view = View(_f32(V), fx, fy, cx, cy, 64, 64, 0.5, 1.0, (0.1, 0.2, 0.3)).as_fp32()
     return Scene("fd", 1, 2, _f32(mean), _f32(ls), _f32(ql), _f32(qr), _f32(logit), _f32(sh), [view], seed)

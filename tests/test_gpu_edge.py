@@ -12,7 +12,7 @@ from paper_2412_20720_b200 import scenes
 def _f32(sc):
     for k in ("mean", "log_scale", "quat_l", "quat_r", "opacity_logit", "sh"):
         setattr(sc, k, np.ascontiguousarray(getattr(sc, k), dtype=np.float32))
-    sc.views[0].view = np.asarray(sc.views[0].view, dtype=np.float32)
+    sc.views[0] = sc.views[0].as_fp32()
     return sc
 
 
