@@ -139,17 +139,31 @@ __device__ __forceinline__ float warp_reduce8(float v[8], const int lane) {
   return v[0];
 }
 
-// B1.  Walks each tile list back to front from the last contributor of the tile; per splat the nine
-// gradients are reduced over the warp by shuffles, then over the eight warps in shared memory, and one
-// thread per splat flushes nine global atomics per (tile, splat).
+// B1.  Walks each tile list back to front from the last contributor of the tile.  Per (pixel, splat) the lane
+// produces two scalars, wgt = alpha T (for dL/dc) and dpow = alpha dL/dalpha (for everything that flows through the
+// exponent), and nine products of them with per-pixel quantities:
+//     dpow * {dx, dy, dx^2, dx dy, dy^2, 1}   and   wgt * dL/dpixel{r,g,b}        (dx = u - px, dy = v - py)
+// which are reduced over the warp by shuffles, then over the eight warps in shared memory; one thread per splat
+// turns the nine sums into dL/d(u, v, A, B, C, o, r, g, b) and flushes nine global atomics per (tile, splat):
+//     dL/du = -(A Sx + B Sy), dL/dv = -(B Sx + C Sy), dL/dA = -Sxx/2, dL/dB = -Sxy, dL/dC = -Syy/2, dL/do = S1 / o.
+// The colour behind the current splat enters only through its dot product with dL/dpixel, so one scalar s is carried:
+//     dL/dalpha_k = T_k (g.c_k) - s_k / (1 - alpha_k),   s_{k-1} = s_k + (g.c_k) alpha_k T_k,   s_last = T_final (g.bg).
+constexpr int ACC_STRIDE = BATCH + 1;   // odd stride: the eight lanes that hold the warp sums hit eight different banks
+
+struct BwdShared {
+  float4 s0[BATCH], s1[BATCH], s2[BATCH];
+  float acc[9 * ACC_STRIDE];
+  unsigned int id[BATCH];
+  int max_contrib;
+};
+
+__device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
 __global__ void __launch_bounds__(256) blend_bwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
                                                         const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
                                                         const float* __restrict__ dL_dimage, const float* __restrict__ final_T,
                                                         const unsigned int* __restrict__ n_contrib, float* __restrict__ g9) {
-  __shared__ float4 s0[BATCH], s1[BATCH], s2[BATCH];
-  __shared__ float s_acc[9][BATCH];
-  __shared__ unsigned int s_id[BATCH];
-  __shared__ int s_max;
+  __shared__ BwdShared sm;
   const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int lx = ((warp & 1) << 3) + (lane & 7), ly = ((warp >> 1) << 2) + (lane >> 3);
@@ -162,37 +176,39 @@ __global__ void __launch_bounds__(256) blend_bwd_kernel(const uint2* __restrict_
   float T = 1.f, gr = 0.f, gg = 0.f, gb = 0.f;
   int mine = 0;
   if (inside) { T = final_T[pix]; mine = (int)n_contrib[pix]; gr = dL_dimage[pix]; gg = dL_dimage[hw + pix]; gb = dL_dimage[2 * hw + pix]; }
-  if (threadIdx.x == 0) s_max = 0;
+  if (threadIdx.x == 0) sm.max_contrib = 0;
   __syncthreads();
   int warp_max = mine;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) warp_max = max(warp_max, __shfl_xor_sync(0xffffffffu, warp_max, o));
-  if (lane == 0) atomicMax(&s_max, warp_max);
+  if (lane == 0) atomicMax(&sm.max_contrib, warp_max);
   __syncthreads();
-  const int total = s_max;
-  // S = colour accumulated behind the current splat (starts as T_final * bg)
-  float Sr = T * vp.bg[0], Sg = T * vp.bg[1], Sb = T * vp.bg[2];
-  const float ln2 = 0.69314718055994531f;
+  const int total = sm.max_contrib;
+  float s = T * (gr * vp.bg[0] + gg * vp.bg[1] + gb * vp.bg[2]);
+  // warp_reduce8 leaves sum k on lane 4k; the ninth sum (butterfly, on every lane) is flushed by lane 1: one atomic
+  // instruction for all nine rows, nine different banks
+  const bool flusher = (lane & 3) == 0 || lane == 1;
+  float* const acc_lane = sm.acc + (lane == 1 ? 8 : lane >> 2) * ACC_STRIDE;
   for (int hi = total; hi > 0; hi -= BATCH) {           // batch covers list positions [lo_pos, hi)
     const int lo_pos = max(0, hi - BATCH), m = hi - lo_pos;
     __syncthreads();                                    // previous batch fully flushed
     if ((int)threadIdx.x < m) {
       const unsigned int id = vals[range.x + lo_pos + threadIdx.x];
-      s_id[threadIdx.x] = id;
-      stage_splat(rec, id, ox, oy, &s0[threadIdx.x], &s1[threadIdx.x], &s2[threadIdx.x]);
+      sm.id[threadIdx.x] = id;
+      stage_splat(rec, id, ox, oy, &sm.s0[threadIdx.x], &sm.s1[threadIdx.x], &sm.s2[threadIdx.x]);
     }
 #pragma unroll
-    for (int k = 0; k < 9; ++k) s_acc[k][threadIdx.x] = 0.f;
+    for (int k = 0; k < 9; ++k) sm.acc[k * ACC_STRIDE + threadIdx.x] = 0.f;
     __syncthreads();
     if (lo_pos < warp_max) {
      for (int jb = ((m - 1) >> 5) << 5; jb >= 0; jb -= 32) {
       unsigned int hits = __ballot_sync(0xffffffffu, jb + lane < m && lo_pos + jb + lane < warp_max &&
-                                                     patch_hit(s0[jb + lane], s1[jb + lane], xm, ym, cp.log2_alpha_min));
+                                                     patch_hit(sm.s0[jb + lane], sm.s1[jb + lane], xm, ym, cp.log2_alpha_min));
       while (hits) {
         const int bit = 31 - __clz(hits);
         hits &= ~(1u << bit);
         const int j = jb + bit;
-        const float4 a = s0[j], b = s1[j], c = s2[j];
+        const float4 a = sm.s0[j], b = sm.s1[j];
         const float e1 = fmaf(a.x, x, fmaf(a.y, y, a.w));
         const float e2 = fmaf(a.z, y, b.x);
         const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
@@ -200,44 +216,46 @@ __global__ void __launch_bounds__(256) blend_bwd_kernel(const uint2* __restrict_
         float alpha = 0.f, araw = 0.f;
         if (active) { araw = ex2_approx(l2a); alpha = fminf(cp.alpha_max, araw); active = !(alpha < cp.alpha_min); }
         if (!__any_sync(0xffffffffu, active)) continue;
-        float v[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, v_o = 0.f;
+        float v[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, v1 = 0.f;
         if (active) {
-          const float om = 1.f - alpha;
-          T = T / om;                                                  // T_k
+          const float4 c = sm.s2[j];
+          const float iom = rcp_approx(1.f - alpha);
+          T *= iom;                                                    // T_k
           const float wgt = alpha * T;
           v[5] = wgt * gr; v[6] = wgt * gg; v[7] = wgt * gb;           // dL/dc
-          const float iom = 1.f / om;
-          const float dalpha = gr * fmaf(-Sr, iom, T * b.z) + gg * fmaf(-Sg, iom, T * b.w) + gb * fmaf(-Sb, iom, T * c.x);
-          Sr = fmaf(b.z, wgt, Sr); Sg = fmaf(b.w, wgt, Sg); Sb = fmaf(c.x, wgt, Sb);
-          if (!(araw > cp.alpha_max)) {                                // alpha clamp inactive
-            // alpha = o * G:  d alpha/d o = G = alpha / o;  d alpha / d power = alpha
-            v_o = dalpha * ex2_approx(l2a - b.y);
-            const float dpow = alpha * dalpha;
-            const float dx = c.y - x, dy = c.z - y;
-            // power = -(e1^2 + e2^2) ln2, e1 = ca dx + cb dy, e2 = cc dy, expressed through the conic (A, B, C):
-            //   d power/du = -(A dx + B dy), d power/dv = -(B dx + C dy), d/dA = -dx^2/2, d/dB = -dx dy, d/dC = -dy^2/2
-            const float ca = -a.x, cb = -a.y, cc = -a.z;
-            const float t1 = 2.f * ln2 * e1, t2 = 2.f * ln2 * e2;      // d(-power)/d e1, d e2
-            v[0] = -dpow * (t1 * ca);
-            v[1] = -dpow * fmaf(t1, cb, t2 * cc);
-            v[2] = dpow * -0.5f * dx * dx; v[3] = dpow * -dx * dy; v[4] = dpow * -0.5f * dy * dy;
+          const float gc = fmaf(gr, b.z, fmaf(gg, b.w, gb * c.x));     // dL/dpixel . c_k
+          const float dalpha = fmaf(T, gc, -s * iom);
+          s = fmaf(gc, wgt, s);
+          if (!(araw > cp.alpha_max)) {                                // alpha clamp inactive: d alpha / d power = alpha
+            const float dpow = alpha * dalpha, dx = c.y - x, dy = c.z - y;
+            v1 = dpow;
+            v[0] = dpow * dx; v[1] = dpow * dy;
+            v[2] = v[0] * dx; v[3] = v[0] * dy; v[4] = v[1] * dy;
           }
         }
         const float red = warp_reduce8(v, lane);
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v_o += __shfl_xor_sync(0xffffffffu, v_o, o);
-        if ((lane & 3) == 0) atomicAdd(&s_acc[lane >> 2][j], red);
-        if (lane == 1) atomicAdd(&s_acc[8][j], v_o);
+        for (int o = 16; o > 0; o >>= 1) v1 += __shfl_xor_sync(0xffffffffu, v1, o);
+        if (flusher) atomicAdd(acc_lane + j, lane == 1 ? v1 : red);
       }
      }
     }
     __syncthreads();
     if ((int)threadIdx.x < m) {
-      float* dst = g9 + (size_t)9 * s_id[threadIdx.x];
-      // s_acc rows: 0 u, 1 v, 2 A, 3 B, 4 C, 5 r, 6 g, 7 b, 8 o  ->  g9 order u, v, A, B, C, o, r, g, b
-      const int row_of[9] = {0, 1, 2, 3, 4, 8, 5, 6, 7};
+      const int j = threadIdx.x;
+      const float Sx = sm.acc[j], Sy = sm.acc[ACC_STRIDE + j], Sxx = sm.acc[2 * ACC_STRIDE + j], Sxy = sm.acc[3 * ACC_STRIDE + j];
+      const float Syy = sm.acc[4 * ACC_STRIDE + j], S1 = sm.acc[8 * ACC_STRIDE + j];
+      const float4 a = sm.s0[j];
+      const float ik = 1.0f / 0.72134752044448170f;                    // conic (A, B, C) from its exp2-scaled factor
+      const float A = a.x * a.x * ik, B = a.x * a.y * ik, C = fmaf(a.y, a.y, a.z * a.z) * ik;
+      float out[9];
+      out[0] = -fmaf(A, Sx, B * Sy); out[1] = -fmaf(B, Sx, C * Sy);
+      out[2] = -0.5f * Sxx; out[3] = -Sxy; out[4] = -0.5f * Syy;
+      out[5] = S1 * exp2f(-sm.s1[j].y);
+      out[6] = sm.acc[5 * ACC_STRIDE + j]; out[7] = sm.acc[6 * ACC_STRIDE + j]; out[8] = sm.acc[7 * ACC_STRIDE + j];
+      float* dst = g9 + (size_t)9 * sm.id[j];
 #pragma unroll
-      for (int k = 0; k < 9; ++k) { const float val = s_acc[row_of[k]][threadIdx.x]; if (val != 0.f) atomicAdd(dst + k, val); }
+      for (int k = 0; k < 9; ++k) if (out[k] != 0.f) atomicAdd(dst + k, out[k]);
     }
   }
 }
