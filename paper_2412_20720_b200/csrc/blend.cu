@@ -1,24 +1,24 @@
 // blend.cu — A9 (forward compositing) and B1 (its reverse-order gradient) for sm_100a.
-// One CTA per 16x16 tile, one pixel per thread; each warp covers an 8x4 pixel patch so that early
-// termination and alpha-skips stay coherent inside a warp.  Splat records are gathered by id into shared
-// memory in batches of 256 and converted once per (tile, splat) to tile-local form:
+// One CTA per 16x16 tile.  A warp covers an 8-wide column strip of 4*PX rows; lane l owns PX pixels, one in each of the
+// strip's PX sub-patches of 8x4 pixels: (x0 + l%8, y0 + 4k + l/8), k < PX.  A sub-patch is the unit of culling (early
+// termination and alpha-skips stay coherent inside it); the strip is the unit of everything that costs once per
+// (warp, splat): the bit loop, the shared-memory loads of the splat and — in the backward — the warp reduction of the
+// per-splat gradient sums and their flush.  PX = 1 gives 8 warps per tile, PX = 2 four, PX = 4 two.
+// Splat records are gathered by id into shared memory in batches and converted once per (tile, splat) to tile-local form:
 //     e1 = k1 - ca*x - cb*y,  e2 = k2 - cc*y,  log2(alpha) = lo - e1^2 - e2^2      (x, y tile-local pixel centres)
 // i.e. 5 FFMA + 1 MUFU.EX2 per (pixel, splat) evaluation; tile-local coordinates keep |e| small so fp32
-// cancellation stays ~1e-7 (DESIGN.md "blend numerics").
+// cancellation stays ~1e-7 (DESIGN.md "fp32 numerics").
+#include <cstdlib>
+
 #include "common.cuh"
 
 namespace fdgs {
 
-constexpr int BATCH = 256;
-
-struct TileSplat {   // 48 B in shared memory, read as three broadcast LDS.128
-  float nca, ncb, ncc, k1;   // -ca, -cb, -cc, ca*(u-ox) + cb*(v-oy)
-  float k2, lo, r, g;        // cc*(v-oy), log2(o)
-  float b, u, v, pad;        // (u, v) tile-local, for the backward
-};
-
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
+// Shared-memory form of a splat: three float4, read as broadcast LDS.128
+//   s0 = (-ca, -cb, -cc, k1 = ca*(u-ox) + cb*(v-oy))   s1 = (k2 = cc*(v-oy), lo = log2(o), r, g)   s2 = (b, u-ox, v-oy, -)
 __device__ __forceinline__ void stage_splat(const SplatRec* __restrict__ rec, const unsigned int id, const float ox, const float oy,
                                             float4* s0, float4* s1, float4* s2) {
   const float4* src = reinterpret_cast<const float4*>(rec + id);
@@ -29,7 +29,7 @@ __device__ __forceinline__ void stage_splat(const SplatRec* __restrict__ rec, co
   *s2 = make_float4(q2.x, ul, vl, 0.f);
 }
 
-// Conservative test "can this splat reach alpha >= alpha_min anywhere on the warp's 8x4 pixel patch?": in the whitened
+// Conservative test "can this splat reach alpha >= alpha_min anywhere on an 8x4 pixel patch?": in the whitened
 // coordinates (e1, e2) the patch is a parallelogram; its bounding box gives the lower bound
 //   min(e1^2 + e2^2) >= max(0,|e1(c)| - ca*hw - |cb|*hh)^2 + max(0,|e2(c)| - cc*hh)^2     (c = patch centre)
 // A splat is dropped only if even that bound (shrunk by a rounding slack) puts log2(alpha) below the skip threshold,
@@ -42,61 +42,98 @@ __device__ __forceinline__ bool patch_hit(const float4 a, const float4 b, const 
   return !(fmaf(qmin, 0.999f, -1e-3f) > b.y - l2min);
 }
 
-// STATS = true: same walk, but counts the work instead of writing the image (fdgs_debug_blend_stats):
-//   stats[0] pairs walked (pixel x splat, until the pixel terminates), [1] pairs that reach the exp2,
-//   [2] pairs composited, [3] splats staged into shared memory (summed over tiles)
-template <bool STATS>
-__global__ void __launch_bounds__(256) blend_fwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
-                                                        const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
-                                                        float* __restrict__ image, float* __restrict__ final_T,
-                                                        unsigned int* __restrict__ n_contrib, unsigned long long* stats) {
-  __shared__ float4 s0[BATCH], s1[BATCH], s2[BATCH];
+// Pixel geometry of a lane: strip origin (sx0, sy0) inside the tile, lane offsets.
+template <int PX>
+struct Strip {
+  int lx, ly0;      // tile-local pixel column, row of sub-patch 0
+  float xm, ym0;    // centre of sub-patch 0 (tile-local)
+  __device__ __forceinline__ Strip(const int warp, const int lane) {
+    const int sx0 = (warp & 1) << 3, sy0 = (warp >> 1) * 4 * PX;
+    lx = sx0 + (lane & 7); ly0 = sy0 + (lane >> 3);
+    xm = (float)sx0 + 4.0f; ym0 = (float)sy0 + 2.0f;
+  }
+};
+
+// A9.  STATS = true: same walk without the patch culling, counting the work instead of writing the image
+// (fdgs_debug_blend_stats): stats[0] (pixel, splat) pairs walked until the pixel terminates, [1] pairs that reach the
+// exp2, [2] pairs composited, [3] splats staged into shared memory (summed over tiles).
+template <int PX, bool STATS>
+__global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
+                                                             const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
+                                                             float* __restrict__ image, float* __restrict__ final_T,
+                                                             unsigned int* __restrict__ n_contrib, unsigned long long* stats) {
+  constexpr int BATCH = 256 / PX;
+  __shared__ struct { float4 s0[BATCH], s1[BATCH], s2[BATCH]; } sm;
   const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int lx = ((warp & 1) << 3) + (lane & 7), ly = ((warp >> 1) << 2) + (lane >> 3);
-  const int px = tx * TILE + lx, py = ty * TILE + ly;
-  const bool inside = px < vp.width && py < vp.height;
-  const float x = lx + 0.5f, y = ly + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
-  const float xm = (float)((warp & 1) << 3) + 4.0f, ym = (float)((warp >> 1) << 2) + 2.0f;   // patch centre (tile-local)
+  const Strip<PX> sp(warp, lane);
+  const int px = tx * TILE + sp.lx;
+  const float x = sp.lx + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
+  float y[PX], T[PX], Cr[PX], Cg[PX], Cb[PX];
+  unsigned int last[PX];
+  bool done[PX], inside[PX];
+#pragma unroll
+  for (int k = 0; k < PX; ++k) {
+    const int ly = sp.ly0 + 4 * k;
+    inside[k] = px < vp.width && ty * TILE + ly < vp.height;
+    y[k] = ly + 0.5f; T[k] = 1.f; Cr[k] = Cg[k] = Cb[k] = 0.f; last[k] = 0; done[k] = !inside[k];
+  }
   const uint2 range = ranges[tile];
   const int n = (int)(range.y - range.x);
-  float T = 1.f, Cr = 0.f, Cg = 0.f, Cb = 0.f;
-  unsigned int last = 0;
   unsigned int st_walk = 0, st_exp = 0, st_comp = 0, st_stage = 0;
-  bool done = !inside;
   for (int base = 0; base < n; base += BATCH) {
-    if (__syncthreads_and(done)) break;
+    bool all_done = true;
+#pragma unroll
+    for (int k = 0; k < PX; ++k) all_done = all_done && done[k];
+    if (__syncthreads_and(all_done)) break;
     const int m = min(BATCH, n - base);
     if (STATS && threadIdx.x == 0) st_stage += m;
-    if ((int)threadIdx.x < m) stage_splat(rec, vals[range.x + base + threadIdx.x], ox, oy, &s0[threadIdx.x], &s1[threadIdx.x], &s2[threadIdx.x]);
+    if ((int)threadIdx.x < m) stage_splat(rec, vals[range.x + base + threadIdx.x], ox, oy, &sm.s0[threadIdx.x], &sm.s1[threadIdx.x], &sm.s2[threadIdx.x]);
     __syncthreads();
-    if (__all_sync(0xffffffffu, done)) continue;     // whole 8x4 patch saturated: skip the batch (warp-uniform)
+    unsigned int alive = 0;                           // sub-patches with an unsaturated pixel (warp-uniform)
+#pragma unroll
+    for (int k = 0; k < PX; ++k) if (!__all_sync(0xffffffffu, done[k])) alive |= 1u << k;
+    if (!alive) continue;
     for (int jb = 0; jb < m; jb += 32) {
-      // lane l tests splat jb+l against the warp's patch; the ballot is the list of splats worth evaluating per pixel
-      unsigned int hits;
-      if (STATS) hits = jb + 32 <= m ? 0xffffffffu : ((1u << (m - jb)) - 1u);
-      else hits = __ballot_sync(0xffffffffu, jb + lane < m && patch_hit(s0[jb + lane], s1[jb + lane], xm, ym, cp.log2_alpha_min));
-      while (hits) {
-        const int j = jb + __ffs(hits) - 1;
-        hits &= hits - 1;
-        const float4 a = s0[j], b = s1[j];
-        const float e1 = fmaf(a.x, x, fmaf(a.y, y, a.w));
-        const float e2 = fmaf(a.z, y, b.x);
-        const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
-        if (STATS && !done) ++st_walk;
-        if (done || l2a < cp.log2_alpha_min) continue;                 // alpha < alpha_min: skipped
-        const float alpha = fminf(cp.alpha_max, ex2_approx(l2a));
-        if (STATS) ++st_exp;
-        if (alpha < cp.alpha_min) continue;
-        const float Tn = fmaf(-T, alpha, T);
-        if (Tn < cp.transmittance_min) { done = true; continue; }      // the terminating splat is not composited
-        const float wgt = alpha * T;
-        Cr = fmaf(b.z, wgt, Cr); Cg = fmaf(b.w, wgt, Cg); Cb = fmaf(s2[j].x, wgt, Cb);
-        T = Tn;
-        last = base + j + 1;
-        if (STATS) ++st_comp;
+      // lane l tests splat jb+l against each live sub-patch; the ballots list the splats worth evaluating per pixel
+      unsigned int hk[PX], any = 0;
+      float4 ta, tb;
+      if (jb + lane < m) { ta = sm.s0[jb + lane]; tb = sm.s1[jb + lane]; }
+#pragma unroll
+      for (int k = 0; k < PX; ++k) {
+        if (STATS) hk[k] = jb + 32 <= m ? 0xffffffffu : ((1u << (m - jb)) - 1u);
+        else hk[k] = ((alive >> k) & 1u) ? __ballot_sync(0xffffffffu, jb + lane < m && patch_hit(ta, tb, sp.xm, sp.ym0 + 4.f * k, cp.log2_alpha_min)) : 0u;
+        any |= hk[k];
       }
-      if (__all_sync(0xffffffffu, done)) break;
+      while (any) {
+        const int bit = __ffs(any) - 1;
+        any &= any - 1;
+        const int j = jb + bit;
+        const float4 a = sm.s0[j], b = sm.s1[j];
+        const float e1x = fmaf(a.x, x, a.w);
+#pragma unroll
+        for (int k = 0; k < PX; ++k) {
+          if (!((hk[k] >> bit) & 1u)) continue;                          // warp-uniform
+          const float e1 = fmaf(a.y, y[k], e1x);
+          const float e2 = fmaf(a.z, y[k], b.x);
+          const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
+          if (STATS && !done[k]) ++st_walk;
+          if (done[k] || l2a < cp.log2_alpha_min) continue;              // alpha < alpha_min: skipped
+          const float alpha = fminf(cp.alpha_max, ex2_approx(l2a));
+          if (STATS) ++st_exp;
+          if (alpha < cp.alpha_min) continue;
+          const float Tn = fmaf(-T[k], alpha, T[k]);
+          if (Tn < cp.transmittance_min) { done[k] = true; continue; }   // the terminating splat is not composited
+          const float wgt = alpha * T[k];
+          Cr[k] = fmaf(b.z, wgt, Cr[k]); Cg[k] = fmaf(b.w, wgt, Cg[k]); Cb[k] = fmaf(sm.s2[j].x, wgt, Cb[k]);
+          T[k] = Tn;
+          last[k] = base + j + 1;
+          if (STATS) ++st_comp;
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < PX; ++k) if (((alive >> k) & 1u) && __all_sync(0xffffffffu, done[k])) alive &= ~(1u << k);
+      if (!alive) break;
     }
   }
   if (STATS) {
@@ -109,10 +146,13 @@ __global__ void __launch_bounds__(256) blend_fwd_kernel(const uint2* __restrict_
     }
     return;
   }
-  if (inside) {
-    const size_t hw = (size_t)vp.width * vp.height, pix = (size_t)py * vp.width + px;
-    image[pix] = fmaf(T, vp.bg[0], Cr); image[hw + pix] = fmaf(T, vp.bg[1], Cg); image[2 * hw + pix] = fmaf(T, vp.bg[2], Cb);
-    final_T[pix] = T; n_contrib[pix] = last;
+  const size_t hw = (size_t)vp.width * vp.height;
+#pragma unroll
+  for (int k = 0; k < PX; ++k) {
+    if (!inside[k]) continue;
+    const size_t pix = (size_t)(ty * TILE + sp.ly0 + 4 * k) * vp.width + px;
+    image[pix] = fmaf(T[k], vp.bg[0], Cr[k]); image[hw + pix] = fmaf(T[k], vp.bg[1], Cg[k]); image[2 * hw + pix] = fmaf(T[k], vp.bg[2], Cb[k]);
+    final_T[pix] = T[k]; n_contrib[pix] = last[k];
   }
 }
 
@@ -143,48 +183,49 @@ __device__ __forceinline__ float warp_reduce8(float v[8], const int lane) {
 // produces two scalars, wgt = alpha T (for dL/dc) and dpow = alpha dL/dalpha (for everything that flows through the
 // exponent), and nine products of them with per-pixel quantities:
 //     dpow * {dx, dy, dx^2, dx dy, dy^2, 1}   and   wgt * dL/dpixel{r,g,b}        (dx = u - px, dy = v - py)
-// which are reduced over the warp by shuffles, then over the eight warps in shared memory; one thread per splat
-// turns the nine sums into dL/d(u, v, A, B, C, o, r, g, b) and flushes nine global atomics per (tile, splat):
+// summed over the lane's PX pixels, reduced over the warp by shuffles, then over the warps in shared memory; one
+// thread per splat turns the nine sums into dL/d(u, v, A, B, C, o, r, g, b) and flushes nine global atomics per
+// (tile, splat):
 //     dL/du = -(A Sx + B Sy), dL/dv = -(B Sx + C Sy), dL/dA = -Sxx/2, dL/dB = -Sxy, dL/dC = -Syy/2, dL/do = S1 / o.
 // The colour behind the current splat enters only through its dot product with dL/dpixel, so one scalar s is carried:
 //     dL/dalpha_k = T_k (g.c_k) - s_k / (1 - alpha_k),   s_{k-1} = s_k + (g.c_k) alpha_k T_k,   s_last = T_final (g.bg).
-constexpr int ACC_STRIDE = BATCH + 1;   // odd stride: the eight lanes that hold the warp sums hit eight different banks
-
-struct BwdShared {
-  float4 s0[BATCH], s1[BATCH], s2[BATCH];
-  float acc[9 * ACC_STRIDE];
-  unsigned int id[BATCH];
-  int max_contrib;
-};
-
-__device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-
-__global__ void __launch_bounds__(256) blend_bwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
-                                                        const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
-                                                        const float* __restrict__ dL_dimage, const float* __restrict__ final_T,
-                                                        const unsigned int* __restrict__ n_contrib, float* __restrict__ g9) {
-  __shared__ BwdShared sm;
+template <int PX>
+__global__ void __launch_bounds__(256 / PX) blend_bwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
+                                                             const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
+                                                             const float* __restrict__ dL_dimage, const float* __restrict__ final_T,
+                                                             const unsigned int* __restrict__ n_contrib, float* __restrict__ g9) {
+  constexpr int BATCH = 256 / PX;
+  constexpr int ACC_STRIDE = BATCH + 1;   // odd stride: the nine lanes that hold the warp sums hit nine different banks
+  __shared__ struct { float4 s0[BATCH], s1[BATCH], s2[BATCH]; float acc[9 * ACC_STRIDE]; unsigned int id[BATCH]; int max_contrib; } sm;
   const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int lx = ((warp & 1) << 3) + (lane & 7), ly = ((warp >> 1) << 2) + (lane >> 3);
-  const int px = tx * TILE + lx, py = ty * TILE + ly;
-  const bool inside = px < vp.width && py < vp.height;
-  const float x = lx + 0.5f, y = ly + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
-  const float xm = (float)((warp & 1) << 3) + 4.0f, ym = (float)((warp >> 1) << 2) + 2.0f;
+  const Strip<PX> sp(warp, lane);
+  const int px = tx * TILE + sp.lx;
+  const float x = sp.lx + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
   const uint2 range = ranges[tile];
-  const size_t hw = (size_t)vp.width * vp.height, pix = (size_t)py * vp.width + px;
-  float T = 1.f, gr = 0.f, gg = 0.f, gb = 0.f;
-  int mine = 0;
-  if (inside) { T = final_T[pix]; mine = (int)n_contrib[pix]; gr = dL_dimage[pix]; gg = dL_dimage[hw + pix]; gb = dL_dimage[2 * hw + pix]; }
+  const size_t hw = (size_t)vp.width * vp.height;
+  float y[PX], T[PX], s[PX], gr[PX], gg[PX], gb[PX];
+  int mine[PX], wmax[PX];
+  int lane_max = 0;
+#pragma unroll
+  for (int k = 0; k < PX; ++k) {
+    const int ly = sp.ly0 + 4 * k, py = ty * TILE + ly;
+    y[k] = ly + 0.5f; T[k] = 1.f; mine[k] = 0; gr[k] = gg[k] = gb[k] = 0.f;
+    if (px < vp.width && py < vp.height) {
+      const size_t pix = (size_t)py * vp.width + px;
+      T[k] = final_T[pix]; mine[k] = (int)n_contrib[pix]; gr[k] = dL_dimage[pix]; gg[k] = dL_dimage[hw + pix]; gb[k] = dL_dimage[2 * hw + pix];
+    }
+    s[k] = T[k] * (gr[k] * vp.bg[0] + gg[k] * vp.bg[1] + gb[k] * vp.bg[2]);
+    int w = mine[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) w = max(w, __shfl_xor_sync(0xffffffffu, w, o));
+    wmax[k] = w; lane_max = max(lane_max, w);
+  }
   if (threadIdx.x == 0) sm.max_contrib = 0;
   __syncthreads();
-  int warp_max = mine;
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) warp_max = max(warp_max, __shfl_xor_sync(0xffffffffu, warp_max, o));
-  if (lane == 0) atomicMax(&sm.max_contrib, warp_max);
+  if (lane == 0) atomicMax(&sm.max_contrib, lane_max);
   __syncthreads();
   const int total = sm.max_contrib;
-  float s = T * (gr * vp.bg[0] + gg * vp.bg[1] + gb * vp.bg[2]);
   // warp_reduce8 leaves sum k on lane 4k; the ninth sum (butterfly, on every lane) is flushed by lane 1: one atomic
   // instruction for all nine rows, nine different banks
   const bool flusher = (lane & 3) == 0 || lane == 1;
@@ -200,37 +241,57 @@ __global__ void __launch_bounds__(256) blend_bwd_kernel(const uint2* __restrict_
 #pragma unroll
     for (int k = 0; k < 9; ++k) sm.acc[k * ACC_STRIDE + threadIdx.x] = 0.f;
     __syncthreads();
-    if (lo_pos < warp_max) {
+    if (lo_pos < lane_max) {
      for (int jb = ((m - 1) >> 5) << 5; jb >= 0; jb -= 32) {
-      unsigned int hits = __ballot_sync(0xffffffffu, jb + lane < m && lo_pos + jb + lane < warp_max &&
-                                                     patch_hit(sm.s0[jb + lane], sm.s1[jb + lane], xm, ym, cp.log2_alpha_min));
-      while (hits) {
-        const int bit = 31 - __clz(hits);
-        hits &= ~(1u << bit);
+      unsigned int hk[PX], any = 0;
+      float4 ta, tb;
+      if (jb + lane < m) { ta = sm.s0[jb + lane]; tb = sm.s1[jb + lane]; }
+#pragma unroll
+      for (int k = 0; k < PX; ++k) {
+        hk[k] = lo_pos + jb < wmax[k] ? __ballot_sync(0xffffffffu, jb + lane < m && lo_pos + jb + lane < wmax[k] &&
+                                                                    patch_hit(ta, tb, sp.xm, sp.ym0 + 4.f * k, cp.log2_alpha_min)) : 0u;
+        any |= hk[k];
+      }
+      while (any) {
+        const int bit = 31 - __clz(any);
+        any &= ~(1u << bit);
         const int j = jb + bit;
         const float4 a = sm.s0[j], b = sm.s1[j];
-        const float e1 = fmaf(a.x, x, fmaf(a.y, y, a.w));
-        const float e2 = fmaf(a.z, y, b.x);
-        const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
-        bool active = (lo_pos + j < mine) && !(l2a < cp.log2_alpha_min);
-        float alpha = 0.f, araw = 0.f;
-        if (active) { araw = ex2_approx(l2a); alpha = fminf(cp.alpha_max, araw); active = !(alpha < cp.alpha_min); }
-        if (!__any_sync(0xffffffffu, active)) continue;
+        const float e1x = fmaf(a.x, x, a.w);
+        float alpha[PX], araw[PX];
+        bool act[PX], some = false;
+#pragma unroll
+        for (int k = 0; k < PX; ++k) {
+          act[k] = false; alpha[k] = 0.f; araw[k] = 0.f;
+          if (!((hk[k] >> bit) & 1u)) continue;                          // warp-uniform
+          const float e1 = fmaf(a.y, y[k], e1x);
+          const float e2 = fmaf(a.z, y[k], b.x);
+          const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
+          if ((lo_pos + j < mine[k]) && !(l2a < cp.log2_alpha_min)) {
+            araw[k] = ex2_approx(l2a); alpha[k] = fminf(cp.alpha_max, araw[k]); act[k] = !(alpha[k] < cp.alpha_min);
+          }
+          some = some || act[k];
+        }
+        if (!__any_sync(0xffffffffu, some)) continue;
         float v[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, v1 = 0.f;
-        if (active) {
-          const float4 c = sm.s2[j];
-          const float iom = rcp_approx(1.f - alpha);
-          T *= iom;                                                    // T_k
-          const float wgt = alpha * T;
-          v[5] = wgt * gr; v[6] = wgt * gg; v[7] = wgt * gb;           // dL/dc
-          const float gc = fmaf(gr, b.z, fmaf(gg, b.w, gb * c.x));     // dL/dpixel . c_k
-          const float dalpha = fmaf(T, gc, -s * iom);
-          s = fmaf(gc, wgt, s);
-          if (!(araw > cp.alpha_max)) {                                // alpha clamp inactive: d alpha / d power = alpha
-            const float dpow = alpha * dalpha, dx = c.y - x, dy = c.z - y;
-            v1 = dpow;
-            v[0] = dpow * dx; v[1] = dpow * dy;
-            v[2] = v[0] * dx; v[3] = v[0] * dy; v[4] = v[1] * dy;
+        const float4 c = sm.s2[j];
+        const float dx = c.y - x;
+#pragma unroll
+        for (int k = 0; k < PX; ++k) {
+          if (!act[k]) continue;
+          const float iom = rcp_approx(1.f - alpha[k]);
+          T[k] *= iom;                                                 // T_k
+          const float wgt = alpha[k] * T[k];
+          v[5] = fmaf(wgt, gr[k], v[5]); v[6] = fmaf(wgt, gg[k], v[6]); v[7] = fmaf(wgt, gb[k], v[7]);   // dL/dc
+          const float gc = fmaf(gr[k], b.z, fmaf(gg[k], b.w, gb[k] * c.x));                               // dL/dpixel . c_k
+          const float dalpha = fmaf(T[k], gc, -s[k] * iom);
+          s[k] = fmaf(gc, wgt, s[k]);
+          if (!(araw[k] > cp.alpha_max)) {                             // alpha clamp inactive: d alpha / d power = alpha
+            const float dpow = alpha[k] * dalpha, dy = c.z - y[k];
+            const float mx = dpow * dx, my = dpow * dy;
+            v1 += dpow;
+            v[0] += mx; v[1] += my;
+            v[2] = fmaf(mx, dx, v[2]); v[3] = fmaf(mx, dy, v[3]); v[4] = fmaf(my, dy, v[4]);
           }
         }
         const float red = warp_reduce8(v, lane);
@@ -260,20 +321,34 @@ __global__ void __launch_bounds__(256) blend_bwd_kernel(const uint2* __restrict_
   }
 }
 
+// Pixels per lane of the two blend kernels.  2 is the measured optimum on cfg3; FDGS_BLEND_PX
+// overrides it for experiments (1, 2 or 4).
+static int blend_px() {
+  static int px = 0;
+  if (!px) { const char* e = getenv("FDGS_BLEND_PX"); px = e ? atoi(e) : 2; if (px != 1 && px != 2 && px != 4) px = 2; }
+  return px;
+}
+
 void launch_blend_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
                       unsigned int* n_contrib, cudaStream_t st) {
-  blend_fwd_kernel<false><<<vp.tiles_x * vp.tiles_y, 256, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr);
+  const int tiles = vp.tiles_x * vp.tiles_y;
+#define FDGS_FWD(PXV) blend_fwd_kernel<PXV, false><<<tiles, 256 / PXV, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr)
+  switch (blend_px()) { case 1: FDGS_FWD(1); break; case 4: FDGS_FWD(4); break; default: FDGS_FWD(2); }
+#undef FDGS_FWD
   ++g_launches;
 }
 
 void launch_blend_stats(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, unsigned long long* stats, cudaStream_t st) {
-  blend_fwd_kernel<true><<<vp.tiles_x * vp.tiles_y, 256, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, nullptr, nullptr, nullptr, stats);
+  blend_fwd_kernel<1, true><<<vp.tiles_x * vp.tiles_y, 256, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, nullptr, nullptr, nullptr, stats);
   ++g_launches;
 }
 
 void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* dL_dimage,
                       const float* final_T, const unsigned int* n_contrib, cudaStream_t st) {
-  blend_bwd_kernel<<<vp.tiles_x * vp.tiles_y, 256, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9);
+  const int tiles = vp.tiles_x * vp.tiles_y;
+#define FDGS_BWD(PXV) blend_bwd_kernel<PXV><<<tiles, 256 / PXV, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9)
+  switch (blend_px()) { case 1: FDGS_BWD(1); break; case 4: FDGS_BWD(4); break; default: FDGS_BWD(2); }
+#undef FDGS_BWD
   ++g_launches;
 }
 
