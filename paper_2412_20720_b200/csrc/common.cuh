@@ -82,6 +82,8 @@ struct Workspace {
   unsigned int* sort_lookback;       // [max sort tiles][RADIX]
   uint2* ranges;                     // [tiles] [first, last+1)
   float* g9;                         // [N,9] per-splat gradients of the blend backward
+  float4* aux;                       // [N] survivors: view direction (x, y, z) and (t - mu_t) / T, written by preprocess
+  float4* dcol;                      // [N] survivors: colour backward -> geometry backward: dL/d dir (x, y, z), dL/d Delta
   size_t lookback_bytes, zero_bytes; // zero_bytes: prefix of the workspace cleared by fdgs_preprocess
   size_t bytes;
 };
@@ -115,6 +117,8 @@ inline Workspace carve(void* base, long long N, long long K, long long W, long l
   w.sort_lookback = (unsigned int*)take(w.lookback_bytes);
   w.ranges = (uint2*)take(sizeof(uint2) * tiles);
   w.g9 = (float*)take(4 * 9 * Np);
+  w.aux = (float4*)take(16 * Np);
+  w.dcol = (float4*)take(16 * Np);
   (void)K;
   w.bytes = off;
   return w;

@@ -56,7 +56,7 @@ template <int KD>
 __global__ void __launch_bounds__(128) preprocess_fwd_kernel(const fdgs_scene sc, const ViewParams vp, const CfgParams cp,
                                                              SplatRec* __restrict__ rec, ushort4* __restrict__ rect,
                                                              unsigned int* __restrict__ tiles_touched,
-                                                             int* __restrict__ tile_diff) {
+                                                             int* __restrict__ tile_diff, float4* __restrict__ aux) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   bool visible = false;
   Geom g;
@@ -97,6 +97,7 @@ __global__ void __launch_bounds__(128) preprocess_fwd_kernel(const fdgs_scene sc
   float dir[3], inv_rho, raw[3];
   view_dir(g, vp, dir, inv_rho);
   colour_forward<KD>(sc.sh + (size_t)i * sc.n_time * KD * 3, sc.n_time, dir, g.dt * vp.inv_T, raw);
+  aux[i] = make_float4(dir[0], dir[1], dir[2], g.dt * vp.inv_T);     // kept for the colour backward
   // conic = Sigma_2d^-1 = [c2, -b2; -b2, a2] / det, stored as the exp2-scaled Cholesky factor (common.cuh)
   const float kk = 0.72134752044448170f;   // log2(e) / 2
   const float A = g.c2 / g.det, B = -g.b2 / g.det;
@@ -118,7 +119,7 @@ void launch_preprocess_fwd(const fdgs_scene& sc, const ViewParams& vp, const Cfg
   if (sc.N <= 0) return;
   const int threads = 128, blocks = (sc.N + threads - 1) / threads;
   const int KD = (sc.sh_degree + 1) * (sc.sh_degree + 1);
-#define FDGS_LAUNCH(KDV) preprocess_fwd_kernel<KDV><<<blocks, threads, 0, st>>>(sc, vp, cp, ws.rec, ws.rect, ws.tiles_touched, ws.tile_diff)
+#define FDGS_LAUNCH(KDV) preprocess_fwd_kernel<KDV><<<blocks, threads, 0, st>>>(sc, vp, cp, ws.rec, ws.rect, ws.tiles_touched, ws.tile_diff, ws.aux)
   if (KD == 1) FDGS_LAUNCH(1); else if (KD == 4) FDGS_LAUNCH(4); else if (KD == 9) FDGS_LAUNCH(9); else FDGS_LAUNCH(16);
 #undef FDGS_LAUNCH
   ++g_launches;

@@ -1,9 +1,9 @@
-// preprocess_bwd.cu — K8 (B2): VJP of A4, A3, A2, A1 for every surviving primitive (sm_100a).
-// Recomputes the forward chain from the raw parameters (nothing but the 9 per-splat gradients of the
-// blend backward is read from the workspace) and accumulates (+=) into the caller's gradient arrays.
-// One thread owns one primitive, so the read-modify-write needs no atomics.
-// The chain is differentiated in the same factor form the forward uses (geom.cuh): Sigma_2d = B B^T + dI,
-// B = T N, N = M3 - c m4^T / b, c = M3 m4, b = m4.m4, M = R diag(s), R = L(q_l) R(q_r).
+// preprocess_bwd.cu — K8 (B2): VJP of A4, A3, A2, A1 for every surviving primitive (sm_100a), as two kernels:
+//   colour_bwd_kernel  (A4)       HBM-bound, light in registers, many loads in flight;
+//   geom_bwd_kernel    (A3..A1)   register-heavy chain, ~300 B per survivor.
+// Nothing but the 9 per-splat gradients of the blend backward, the view direction / time offset kept by the forward
+// preprocess (ws.aux) and the hand-over vector ws.dcol is read from the workspace; gradients are accumulated (+=)
+// into the caller's arrays.
 #include "geom.cuh"
 
 namespace fdgs {
@@ -35,107 +35,138 @@ __device__ __forceinline__ void sh_grad_table(const float x, const float y, cons
   }
 }
 
-constexpr int BWD_WARPS = 4;
+constexpr int CB_WARPS = 4;
 // per-survivor table in shared memory: Y[16] | gradY[48] | cos_n[8] | -omega_n sin_n [8] | masked dL/dc [3]; odd stride
 constexpr int TAB_Y = 0, TAB_G = 16, TAB_CN = 64, TAB_WS = 72, TAB_GC = 80, TAB_STRIDE = 85;
 
-// A warp owns 32 consecutive survivors (ascending primitive id).  Lane s runs the per-primitive chain of survivor s;
-// the colour block (12K B of coefficients read + 12K B of coefficient gradients read-modify-written) is walked by the
-// whole warp, one survivor at a time, with fully coalesced 128-bit accesses.
+// One element of the 4DSH coefficient record (eq. 20): its own gradient and its share of dL/d dir, dL/d Delta.
 template <int KD>
-__global__ void __launch_bounds__(32 * BWD_WARPS) preprocess_bwd_kernel(const fdgs_scene sc, const ViewParams vp, const CfgParams cp,
-                                                                        const unsigned int* __restrict__ vis_list,
-                                                                        const WsHeader* __restrict__ hdr, const float* __restrict__ g9,
-                                                                        const SplatRec* __restrict__ rec, const fdgs_grads gr) {
-  __shared__ float tab[BWD_WARPS][32][TAB_STRIDE];
+__device__ __forceinline__ void colour_element(const float* __restrict__ t, const int e, const float coef, float& dcoef,
+                                               float& ax, float& ay, float& az, float& ad) {
+  const int n = e / (3 * KD), rem = e - n * 3 * KD, k = rem / 3, ch = rem - 3 * k;
+  const float yk = t[TAB_Y + k], cn = t[TAB_CN + n], gc = t[TAB_GC + ch];
+  dcoef = fmaf(gc * cn, yk, dcoef);
+  const float sv = coef * gc, sc_n = sv * cn;
+  ad = fmaf(sv * t[TAB_WS + n], yk, ad);
+  ax = fmaf(sc_n, t[TAB_G + 3 * k], ax); ay = fmaf(sc_n, t[TAB_G + 3 * k + 1], ay); az = fmaf(sc_n, t[TAB_G + 3 * k + 2], az);
+}
+
+// K8a (B2, colour part): VJP of A4.  HBM-bound: per survivor it reads the 12K-byte coefficient block and
+// read-modify-writes the 12K-byte gradient block.  A warp owns 32 consecutive survivors; lane s first builds survivor
+// s's table (SH basis, its gradient, the Fourier factors, the clamp-masked dL/dc); then groups of 4 lanes walk one
+// survivor each (8 survivors in flight per warp, 64 contiguous bytes per group and load instruction, three 128-bit
+// loads of coefficients and three of gradients issued before the first use), and a 2-level shuffle gives the
+// survivor's dL/d dir and dL/d Delta, handed to the geometry kernel through ws.dcol.
+template <int KD>
+__global__ void __launch_bounds__(32 * CB_WARPS) colour_bwd_kernel(const float* __restrict__ sh, const int n_time, const float inv_T,
+                                                                   const unsigned int* __restrict__ vis_list, const WsHeader* __restrict__ hdr,
+                                                                   const float* __restrict__ g9, const SplatRec* __restrict__ rec,
+                                                                   const float4* __restrict__ aux, float* __restrict__ dsh,
+                                                                   float4* __restrict__ dcol) {
+  __shared__ float tab[CB_WARPS][32][TAB_STRIDE];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned int n_vis = hdr->num_visible;
-  const unsigned int warp_slot = (blockIdx.x * BWD_WARPS + warp) * 32;
+  const unsigned int warp_slot = (blockIdx.x * CB_WARPS + warp) * 32;
   if (warp_slot >= n_vis) return;
   const unsigned int slot = warp_slot + lane;
   const bool have = slot < n_vis;
   int i = 0;
-  Geom g;
-  bool live = false;
-  float g_u = 0.f, g_v = 0.f, g_A = 0.f, g_B = 0.f, g_C = 0.f, g_o = 0.f;
-  float dir[3] = {0.f, 0.f, 1.f}, inv_rho = 0.f;
-  float* my = tab[warp][lane];
   if (have) {
     i = vis_list[slot];
-    const float4 mean = ldg4b(sc.mean, i), ls = ldg4b(sc.log_scale, i), qlr = ldg4b(sc.quat_l, i), qrr = ldg4b(sc.quat_r, i);
-    live = geom_forward(mean, ls, qlr, qrr, __ldg(sc.opacity_logit + i), vp, cp, g) == G_VISIBLE;
-  }
-  if (live) {
-    const float* gp = g9 + (size_t)9 * i;
-    g_u = gp[0]; g_v = gp[1]; g_A = gp[2]; g_B = gp[3]; g_C = gp[4]; g_o = gp[5];
-    const float dx = g.muc[0] - vp.cam[0], dy = g.muc[1] - vp.cam[1], dz = g.muc[2] - vp.cam[2];
-    inv_rho = 1.0f / sqrtf(dx * dx + dy * dy + dz * dz);
-    dir[0] = dx * inv_rho; dir[1] = dy * inv_rho; dir[2] = dz * inv_rho;
+    float* my = tab[warp][lane];
+    const float4 a = __ldg(aux + i);
     float Y[KD], G[3 * KD];
-    sh_basis<KD>(dir[0], dir[1], dir[2], Y);
-    sh_grad_table<KD>(dir[0], dir[1], dir[2], G);
+    sh_basis<KD>(a.x, a.y, a.z, Y);
+    sh_grad_table<KD>(a.x, a.y, a.z, G);
 #pragma unroll
     for (int k = 0; k < KD; ++k) my[TAB_Y + k] = Y[k];
 #pragma unroll
     for (int k = 0; k < 3 * KD; ++k) my[TAB_G + k] = G[k];
-    const float dtT = g.dt * vp.inv_T;
-    for (int n = 0; n < sc.n_time; ++n) {
-      my[TAB_CN + n] = cospif(2.0f * (float)n * dtT);
-      my[TAB_WS + n] = -6.283185307179586f * (float)n * vp.inv_T * sinpif(2.0f * (float)n * dtT);
+    for (int n = 0; n < n_time; ++n) {
+      my[TAB_CN + n] = cospif(2.0f * (float)n * a.w);
+      my[TAB_WS + n] = -6.283185307179586f * (float)n * inv_T * sinpif(2.0f * (float)n * a.w);
     }
     // the colour clamp at 0 was active iff the stored (clamped) colour is 0: those channels carry no gradient
+    const float* gp = g9 + (size_t)9 * i;
     const float4 q1 = __ldg(reinterpret_cast<const float4*>(rec + i) + 1);
     const float cb = __ldg(reinterpret_cast<const float*>(rec + i) + 8);
     my[TAB_GC + 0] = q1.z > 0.f ? gp[6] : 0.f; my[TAB_GC + 1] = q1.w > 0.f ? gp[7] : 0.f; my[TAB_GC + 2] = cb > 0.f ? gp[8] : 0.f;
-    if (gr.mean2d) { gr.mean2d[2 * i] += g_u; gr.mean2d[2 * i + 1] += g_v; }
   }
   __syncwarp();
-  // ---- (A4) colour: warp-cooperative walk over each survivor's coefficient block ------------------------
-  const int rec_len = sc.n_time * KD * 3;
-  const unsigned int live_mask = __ballot_sync(0xffffffffu, live);
-  float gdx = 0.f, gdy = 0.f, gdz = 0.f, e_dt = 0.f;
-  for (int s = 0; s < 32; ++s) {
-    if (!((live_mask >> s) & 1u)) continue;
+  const int rec_len = n_time * KD * 3, grp = lane >> 2, l = lane & 3;
+#pragma unroll 1
+  for (int b = 0; b < 4; ++b) {
+    const int s = 8 * b + grp;
     const int id = __shfl_sync(0xffffffffu, i, s);
-    const float* t = tab[warp][s];
-    const float* coef = sc.sh + (size_t)id * rec_len;
-    float* dcoef = gr.sh + (size_t)id * rec_len;
+    const bool valid = __shfl_sync(0xffffffffu, (int)have, s) != 0;
     float ax = 0.f, ay = 0.f, az = 0.f, ad = 0.f;
-    if ((rec_len & 3) == 0) {
-      for (int j = lane; j < (rec_len >> 2); j += 32) {
-        const float4 c4 = __ldg(reinterpret_cast<const float4*>(coef) + j);
-        float4 d4 = reinterpret_cast<float4*>(dcoef)[j];
-        const float cv[4] = {c4.x, c4.y, c4.z, c4.w};
-        float dv[4] = {d4.x, d4.y, d4.z, d4.w};
+    if (valid) {
+      const float* t = tab[warp][s];
+      const float* coef = sh + (size_t)id * rec_len;
+      float* dcoef = dsh + (size_t)id * rec_len;
+      if ((rec_len & 3) == 0) {
+        const int nv = rec_len >> 2;
+        const float4* c4p = reinterpret_cast<const float4*>(coef);
+        float4* d4p = reinterpret_cast<float4*>(dcoef);
+        for (int j0 = l; j0 < nv; j0 += 12) {       // three float4 per lane and trip: 6 loads in flight
+          float4 c4[3], d4[3];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const int e = 4 * j + q, n = e / (3 * KD), rem = e - n * 3 * KD, k = rem / 3, ch = rem - 3 * k;
-          const float yk = t[TAB_Y + k], cn = t[TAB_CN + n], gc = t[TAB_GC + ch];
-          dv[q] = fmaf(gc * cn, yk, dv[q]);
-          const float sv = cv[q] * gc, sc_n = sv * cn;
-          ad = fmaf(sv * t[TAB_WS + n], yk, ad);
-          ax = fmaf(sc_n, t[TAB_G + 3 * k], ax); ay = fmaf(sc_n, t[TAB_G + 3 * k + 1], ay); az = fmaf(sc_n, t[TAB_G + 3 * k + 2], az);
+          for (int r = 0; r < 3; ++r) if (j0 + 4 * r < nv) { c4[r] = __ldg(c4p + j0 + 4 * r); d4[r] = d4p[j0 + 4 * r]; }
+#pragma unroll
+          for (int r = 0; r < 3; ++r) {
+            const int j = j0 + 4 * r;
+            if (j < nv) {
+              colour_element<KD>(t, 4 * j, c4[r].x, d4[r].x, ax, ay, az, ad);
+              colour_element<KD>(t, 4 * j + 1, c4[r].y, d4[r].y, ax, ay, az, ad);
+              colour_element<KD>(t, 4 * j + 2, c4[r].z, d4[r].z, ax, ay, az, ad);
+              colour_element<KD>(t, 4 * j + 3, c4[r].w, d4[r].w, ax, ay, az, ad);
+              d4p[j] = d4[r];
+            }
+          }
         }
-        reinterpret_cast<float4*>(dcoef)[j] = make_float4(dv[0], dv[1], dv[2], dv[3]);
-      }
-    } else {
-      for (int e = lane; e < rec_len; e += 32) {
-        const int n = e / (3 * KD), rem = e - n * 3 * KD, k = rem / 3, ch = rem - 3 * k;
-        const float yk = t[TAB_Y + k], cn = t[TAB_CN + n], gc = t[TAB_GC + ch];
-        dcoef[e] = fmaf(gc * cn, yk, dcoef[e]);
-        const float sv = __ldg(coef + e) * gc, sc_n = sv * cn;
-        ad = fmaf(sv * t[TAB_WS + n], yk, ad);
-        ax = fmaf(sc_n, t[TAB_G + 3 * k], ax); ay = fmaf(sc_n, t[TAB_G + 3 * k + 1], ay); az = fmaf(sc_n, t[TAB_G + 3 * k + 2], az);
+      } else {
+        for (int e = l; e < rec_len; e += 4) {
+          float d = dcoef[e];
+          colour_element<KD>(t, e, __ldg(coef + e), d, ax, ay, az, ad);
+          dcoef[e] = d;
+        }
       }
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
+    for (int o = 1; o <= 2; o <<= 1) {
       ax += __shfl_xor_sync(0xffffffffu, ax, o); ay += __shfl_xor_sync(0xffffffffu, ay, o);
       az += __shfl_xor_sync(0xffffffffu, az, o); ad += __shfl_xor_sync(0xffffffffu, ad, o);
     }
-    if (lane == s) { gdx = ax; gdy = ay; gdz = az; e_dt = ad; }
+    if (valid && l == 0) dcol[id] = make_float4(ax, ay, az, ad);
   }
-  if (!live) return;
+}
+
+// K8b (B2, geometry part): VJP of A3, A2, A1 for every survivor.  Recomputes the forward chain from the raw parameters
+// and accumulates (+=) into the caller's gradient arrays.  One thread owns one primitive, so the read-modify-write
+// needs no atomics.  The chain is differentiated in the same factor form the forward uses (geom.cuh):
+// Sigma_2d = B B^T + dI, B = T N, N = M3 - c m4^T / b, c = M3 m4, b = m4.m4, M = R diag(s), R = L(q_l) R(q_r).
+__global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, const ViewParams vp, const CfgParams cp,
+                                                       const unsigned int* __restrict__ vis_list, const WsHeader* __restrict__ hdr,
+                                                       const float* __restrict__ g9, const float4* __restrict__ dcol, const fdgs_grads gr) {
+  const unsigned int slot = blockIdx.x * blockDim.x + threadIdx.x;
+  if (slot >= hdr->num_visible) return;
+  const int i = vis_list[slot];
+  Geom g;
+  {
+    const float4 mean = ldg4b(sc.mean, i), ls = ldg4b(sc.log_scale, i), qlr = ldg4b(sc.quat_l, i), qrr = ldg4b(sc.quat_r, i);
+    if (geom_forward(mean, ls, qlr, qrr, __ldg(sc.opacity_logit + i), vp, cp, g) != G_VISIBLE) return;
+  }
+  const float* gp = g9 + (size_t)9 * i;
+  const float g_u = gp[0], g_v = gp[1], g_A = gp[2], g_B = gp[3], g_C = gp[4], g_o = gp[5];
+  if (gr.mean2d) { gr.mean2d[2 * i] += g_u; gr.mean2d[2 * i + 1] += g_v; }
+  float dir[3], inv_rho;
+  {
+    const float dx = g.muc[0] - vp.cam[0], dy = g.muc[1] - vp.cam[1], dz = g.muc[2] - vp.cam[2];
+    inv_rho = 1.0f / sqrtf(dx * dx + dy * dy + dz * dz);
+    dir[0] = dx * inv_rho; dir[1] = dy * inv_rho; dir[2] = dz * inv_rho;
+  }
+  const float4 dc = __ldg(dcol + i);
+  const float gdx = dc.x, gdy = dc.y, gdz = dc.z, e_dt = dc.w;
   float d_muc[3] = {0.f, 0.f, 0.f}, d_dt = e_dt, d_b = 0.f;
   {
     const float dd = gdx * dir[0] + gdy * dir[1] + gdz * dir[2];
@@ -296,14 +327,17 @@ __global__ void __launch_bounds__(32 * BWD_WARPS) preprocess_bwd_kernel(const fd
 void launch_preprocess_bwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, int l1_buf,
                            const fdgs_grads& gr, cudaStream_t st) {
   if (sc.N <= 0) return;
-  // the survivor count lives on the device: launch for all N slots, surplus threads exit at once
-  const int threads = 32 * BWD_WARPS, blocks = (sc.N + threads - 1) / threads;
+  // the survivor count lives on the device: launch for all N slots, surplus warps / threads exit at once
   (void)l1_buf;
   const int KD = (sc.sh_degree + 1) * (sc.sh_degree + 1);
-#define FDGS_LAUNCH(KDV) preprocess_bwd_kernel<KDV><<<blocks, threads, 0, st>>>(sc, vp, cp, ws.vis_ids, ws.hdr, ws.g9, ws.rec, gr)
-  if (KD == 1) FDGS_LAUNCH(1); else if (KD == 4) FDGS_LAUNCH(4); else if (KD == 9) FDGS_LAUNCH(9); else FDGS_LAUNCH(16);
+  {
+    const int threads = 32 * CB_WARPS, blocks = (sc.N + threads - 1) / threads;
+#define FDGS_LAUNCH(KDV) colour_bwd_kernel<KDV><<<blocks, threads, 0, st>>>(sc.sh, sc.n_time, vp.inv_T, ws.vis_ids, ws.hdr, ws.g9, ws.rec, ws.aux, gr.sh, ws.dcol)
+    if (KD == 1) FDGS_LAUNCH(1); else if (KD == 4) FDGS_LAUNCH(4); else if (KD == 9) FDGS_LAUNCH(9); else FDGS_LAUNCH(16);
 #undef FDGS_LAUNCH
-  ++g_launches;
+  }
+  geom_bwd_kernel<<<(sc.N + 127) / 128, 128, 0, st>>>(sc, vp, cp, ws.vis_ids, ws.hdr, ws.g9, ws.dcol, gr);
+  g_launches += 2;
 }
 
 }  // namespace fdgs
