@@ -321,6 +321,187 @@ __global__ void __launch_bounds__(256 / PX) blend_bwd_kernel(const uint2* __rest
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// B1, transposed accumulation (PX = 2).  Same mathematics as blend_bwd_kernel, different bookkeeping: the pixel-parallel
+// walk only produces the two scalars (dpow, wgt) per pixel and parks them, one float4 per lane, in a per-warp buffer of
+// HB hits.  When the buffer is full the warp turns round: 4 lanes per buffered hit each sum 16 of the strip's 64 pixels
+// into the nine moment / colour sums (coordinates and dL/dpixel of a pixel are per-iteration constants / broadcast
+// loads), two shuffle levels join the four partial sums and three shared atomics per lane add them to the splat's
+// accumulators.  That replaces, per (warp, splat) hit, the 14-shuffle reduction, the nine products per pixel and the
+// per-hit atomic of the direct kernel by one STS.128 and ~1/8 of a 300-instruction flush.
+constexpr int HB = 8;      // hits buffered per warp
+constexpr int HROW = 36;   // float4 per buffered hit: 32 lanes + pad (144 words = 16 mod 32: quarter-warps hit 32 banks)
+
+struct Bwd2Shared {
+  float4 s0[128], s1[128], s2[128];
+  float acc[9 * 129];
+  unsigned int id[128];
+  int max_contrib;
+  int hitj[4][HB];
+  float4 hit[4][HB][HROW];
+  float4 pg[4][32][2];     // per warp, per lane: (gr0, gg0, gb0, gr1), (gg1, gb1, -, -)
+};
+
+__device__ __forceinline__ void bwd2_flush(Bwd2Shared& sm, const int warp, const int lane, const int n, const float sx0, const float sy0) {
+  __syncwarp();
+  const int h = lane >> 2, q = lane & 3;
+  float S[9] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};   // Sx, Sy, Sxx, Sxy, Syy, cr, cg, cb, S1
+  int j = 0;
+  if (h < n) {
+    j = sm.hitj[warp][h];
+    const float4 c = sm.s2[j];
+    const float ux = c.y - (sx0 + 0.5f) - (float)q, vy = c.z - (sy0 + 0.5f);
+    const float4* row = sm.hit[warp][h];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {            // pixel slot p = 4 i + q: column (p % 8), row (p / 8) of both sub-patches
+      const int p = 4 * i + q;
+      const float4 d = row[p];               // dpow0, wgt0, dpow1, wgt1
+      const float4 g0 = sm.pg[warp][p][0], g1 = sm.pg[warp][p][1];
+      const float dx = ux - (float)(4 * (i & 1)), dy0 = vy - (float)(i >> 1), dy1 = dy0 - 4.0f;
+      const float mx0 = d.x * dx, my0 = d.x * dy0, mx1 = d.z * dx, my1 = d.z * dy1;
+      S[0] += mx0; S[0] += mx1; S[1] += my0; S[1] += my1;
+      S[2] = fmaf(mx0, dx, S[2]); S[2] = fmaf(mx1, dx, S[2]);
+      S[3] = fmaf(mx0, dy0, S[3]); S[3] = fmaf(mx1, dy1, S[3]);
+      S[4] = fmaf(my0, dy0, S[4]); S[4] = fmaf(my1, dy1, S[4]);
+      S[5] = fmaf(d.y, g0.x, S[5]); S[6] = fmaf(d.y, g0.y, S[6]); S[7] = fmaf(d.y, g0.z, S[7]);
+      S[5] = fmaf(d.w, g0.w, S[5]); S[6] = fmaf(d.w, g1.x, S[6]); S[7] = fmaf(d.w, g1.y, S[7]);
+      S[8] += d.x; S[8] += d.z;
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < 9; ++k) { S[k] += __shfl_xor_sync(0xffffffffu, S[k], 1); S[k] += __shfl_xor_sync(0xffffffffu, S[k], 2); }
+  if (h < n) {                               // rows q, q + 4 (and 8 on q == 0) of the splat's accumulators
+    const float r0 = q == 0 ? S[0] : q == 1 ? S[1] : q == 2 ? S[2] : S[3];
+    const float r1 = q == 0 ? S[4] : q == 1 ? S[5] : q == 2 ? S[6] : S[7];
+    atomicAdd(&sm.acc[q * 129 + j], r0);
+    atomicAdd(&sm.acc[(q + 4) * 129 + j], r1);
+    if (q == 0) atomicAdd(&sm.acc[8 * 129 + j], S[8]);
+  }
+  __syncwarp();
+}
+
+__global__ void __launch_bounds__(128) blend_bwd2_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
+                                                         const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
+                                                         const float* __restrict__ dL_dimage, const float* __restrict__ final_T,
+                                                         const unsigned int* __restrict__ n_contrib, float* __restrict__ g9) {
+  constexpr int PX = 2, BATCH = 128, ACC_STRIDE = 129;
+  __shared__ Bwd2Shared sm;
+  const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const Strip<PX> sp(warp, lane);
+  const int px = tx * TILE + sp.lx;
+  const float x = sp.lx + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
+  const float sx0 = sp.xm - 4.0f, sy0 = sp.ym0 - 2.0f;          // strip origin (tile-local)
+  const uint2 range = ranges[tile];
+  const size_t hw = (size_t)vp.width * vp.height;
+  float y[PX], T[PX], s[PX], gr[PX], gg[PX], gb[PX];
+  int mine[PX], wmax[PX];
+  int lane_max = 0;
+#pragma unroll
+  for (int k = 0; k < PX; ++k) {
+    const int ly = sp.ly0 + 4 * k, py = ty * TILE + ly;
+    y[k] = ly + 0.5f; T[k] = 1.f; mine[k] = 0; gr[k] = gg[k] = gb[k] = 0.f;
+    if (px < vp.width && py < vp.height) {
+      const size_t pix = (size_t)py * vp.width + px;
+      T[k] = final_T[pix]; mine[k] = (int)n_contrib[pix]; gr[k] = dL_dimage[pix]; gg[k] = dL_dimage[hw + pix]; gb[k] = dL_dimage[2 * hw + pix];
+    }
+    s[k] = T[k] * (gr[k] * vp.bg[0] + gg[k] * vp.bg[1] + gb[k] * vp.bg[2]);
+    int w = mine[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) w = max(w, __shfl_xor_sync(0xffffffffu, w, o));
+    wmax[k] = w; lane_max = max(lane_max, w);
+  }
+  sm.pg[warp][lane][0] = make_float4(gr[0], gg[0], gb[0], gr[1]);
+  sm.pg[warp][lane][1] = make_float4(gg[1], gb[1], 0.f, 0.f);
+  if (threadIdx.x == 0) sm.max_contrib = 0;
+  __syncthreads();
+  if (lane == 0) atomicMax(&sm.max_contrib, lane_max);
+  __syncthreads();
+  const int total = sm.max_contrib;
+  for (int hi = total; hi > 0; hi -= BATCH) {           // batch covers list positions [lo_pos, hi)
+    const int lo_pos = max(0, hi - BATCH), m = hi - lo_pos;
+    __syncthreads();                                    // previous batch fully flushed
+    if ((int)threadIdx.x < m) {
+      const unsigned int id = vals[range.x + lo_pos + threadIdx.x];
+      sm.id[threadIdx.x] = id;
+      stage_splat(rec, id, ox, oy, &sm.s0[threadIdx.x], &sm.s1[threadIdx.x], &sm.s2[threadIdx.x]);
+    }
+#pragma unroll
+    for (int k = 0; k < 9; ++k) sm.acc[k * ACC_STRIDE + threadIdx.x] = 0.f;
+    __syncthreads();
+    if (lo_pos < lane_max) {
+     int nbuf = 0;                                      // buffered hits (warp-uniform)
+     for (int jb = ((m - 1) >> 5) << 5; jb >= 0; jb -= 32) {
+      unsigned int hk[PX], any = 0;
+      float4 ta, tb;
+      if (jb + lane < m) { ta = sm.s0[jb + lane]; tb = sm.s1[jb + lane]; }
+#pragma unroll
+      for (int k = 0; k < PX; ++k) {
+        hk[k] = lo_pos + jb < wmax[k] ? __ballot_sync(0xffffffffu, jb + lane < m && lo_pos + jb + lane < wmax[k] &&
+                                                                    patch_hit(ta, tb, sp.xm, sp.ym0 + 4.f * k, cp.log2_alpha_min)) : 0u;
+        any |= hk[k];
+      }
+      while (any) {
+        const int bit = 31 - __clz(any);
+        any &= ~(1u << bit);
+        const int j = jb + bit;
+        const float4 a = sm.s0[j], b = sm.s1[j];
+        const float e1x = fmaf(a.x, x, a.w);
+        float alpha[PX], araw[PX];                     // alpha == 0 <=> this pixel does not composite this splat
+#pragma unroll
+        for (int k = 0; k < PX; ++k) {
+          alpha[k] = 0.f; araw[k] = 0.f;
+          if (!((hk[k] >> bit) & 1u)) continue;                          // warp-uniform
+          const float e1 = fmaf(a.y, y[k], e1x);
+          const float e2 = fmaf(a.z, y[k], b.x);
+          const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
+          if ((lo_pos + j < mine[k]) && !(l2a < cp.log2_alpha_min)) {
+            araw[k] = ex2_approx(l2a);
+            const float al = fminf(cp.alpha_max, araw[k]);
+            alpha[k] = al < cp.alpha_min ? 0.f : al;
+          }
+        }
+        if (!__any_sync(0xffffffffu, alpha[0] > 0.f || alpha[1] > 0.f)) continue;
+        const float cb = sm.s2[j].x;
+        float dpow[PX], wgt[PX];
+#pragma unroll
+        for (int k = 0; k < PX; ++k) {                 // branch-free: alpha == 0 leaves T and s unchanged and yields zeros
+          const float iom = rcp_approx(1.f - alpha[k]);
+          const float Tk = alpha[k] > 0.f ? T[k] * iom : T[k];           // exact identity when alpha == 0
+          T[k] = Tk;
+          wgt[k] = alpha[k] * Tk;
+          const float gc = fmaf(gr[k], b.z, fmaf(gg[k], b.w, gb[k] * cb));   // dL/dpixel . c_k
+          const float dalpha = fmaf(Tk, gc, -s[k] * iom);
+          s[k] = fmaf(gc, wgt[k], s[k]);
+          dpow[k] = araw[k] > cp.alpha_max ? 0.f : alpha[k] * dalpha;      // alpha clamp active: no gradient through the exponent
+        }
+        sm.hit[warp][nbuf][lane] = make_float4(dpow[0], wgt[0], dpow[1], wgt[1]);
+        if (lane == 0) sm.hitj[warp][nbuf] = j;
+        if (++nbuf == HB) { bwd2_flush(sm, warp, lane, HB, sx0, sy0); nbuf = 0; }
+      }
+     }
+     if (nbuf) bwd2_flush(sm, warp, lane, nbuf, sx0, sy0);
+    }
+    __syncthreads();
+    if ((int)threadIdx.x < m) {
+      const int j = threadIdx.x;
+      const float Sx = sm.acc[j], Sy = sm.acc[ACC_STRIDE + j], Sxx = sm.acc[2 * ACC_STRIDE + j], Sxy = sm.acc[3 * ACC_STRIDE + j];
+      const float Syy = sm.acc[4 * ACC_STRIDE + j], S1 = sm.acc[8 * ACC_STRIDE + j];
+      const float4 a = sm.s0[j];
+      const float ik = 1.0f / 0.72134752044448170f;                    // conic (A, B, C) from its exp2-scaled factor
+      const float A = a.x * a.x * ik, B = a.x * a.y * ik, C = fmaf(a.y, a.y, a.z * a.z) * ik;
+      float out[9];
+      out[0] = -fmaf(A, Sx, B * Sy); out[1] = -fmaf(B, Sx, C * Sy);
+      out[2] = -0.5f * Sxx; out[3] = -Sxy; out[4] = -0.5f * Syy;
+      out[5] = S1 * exp2f(-sm.s1[j].y);
+      out[6] = sm.acc[5 * ACC_STRIDE + j]; out[7] = sm.acc[6 * ACC_STRIDE + j]; out[8] = sm.acc[7 * ACC_STRIDE + j];
+      float* dst = g9 + (size_t)9 * sm.id[j];
+#pragma unroll
+      for (int k = 0; k < 9; ++k) if (out[k] != 0.f) atomicAdd(dst + k, out[k]);
+    }
+  }
+}
+
 // Pixels per lane of the two blend kernels.  2 is the measured optimum on cfg3; FDGS_BLEND_PX
 // overrides it for experiments (1, 2 or 4).
 static int blend_px() {
@@ -347,7 +528,14 @@ void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, con
                       const float* final_T, const unsigned int* n_contrib, cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
 #define FDGS_BWD(PXV) blend_bwd_kernel<PXV><<<tiles, 256 / PXV, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9)
-  switch (blend_px()) { case 1: FDGS_BWD(1); break; case 4: FDGS_BWD(4); break; default: FDGS_BWD(2); }
+  static const bool direct = getenv("FDGS_BLEND_DIRECT") != nullptr;   // experiments: the shuffle-reduction kernel at PX = 2
+  switch (blend_px()) {
+    case 1: FDGS_BWD(1); break;
+    case 4: FDGS_BWD(4); break;
+    default:
+      if (direct) FDGS_BWD(2);
+      else blend_bwd2_kernel<<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9);
+  }
 #undef FDGS_BWD
   ++g_launches;
 }

@@ -124,6 +124,16 @@ inline Workspace carve(void* base, long long N, long long K, long long W, long l
   return w;
 }
 
+#ifdef __CUDACC__
+// Ask L2 for every 128-byte line of [p, p + bytes): the request costs no register and no scoreboard slot, so a thread
+// can have its whole record on the way while it is still doing arithmetic.
+__device__ __forceinline__ void prefetch_l2(const void* p, const int bytes) {
+  const char* c = reinterpret_cast<const char*>(reinterpret_cast<uintptr_t>(p) & ~(uintptr_t)127);
+  const char* end = reinterpret_cast<const char*>(p) + bytes;
+  for (; c < end; c += 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(c));
+}
+#endif
+
 // Launch counter (fdgs_launch_count) — bumped by every launcher.
 extern long long g_launches;
 

@@ -44,7 +44,8 @@ __device__ __forceinline__ void quat_right(const float q[4], float R[4][4]) {
 
 // Runs A1-A3 up to Sigma_2d.  Returns the status; fields are valid up to the point of the cull.
 __device__ __forceinline__ int geom_forward(const float4 mean, const float4 ls, const float4 ql_raw, const float4 qr_raw,
-                                            const float logit, const ViewParams& vp, const CfgParams& cp, Geom& g) {
+                                            const float logit, const ViewParams& vp, const CfgParams& cp, Geom& g,
+                                            const void* prefetch = nullptr, const int prefetch_bytes = 0) {
   const float qlr[4] = {ql_raw.x, ql_raw.y, ql_raw.z, ql_raw.w}, qrr[4] = {qr_raw.x, qr_raw.y, qr_raw.z, qr_raw.w};
   const float lsv[4] = {ls.x, ls.y, ls.z, ls.w};
   float nl2 = 0.f, nr2 = 0.f;
@@ -84,6 +85,8 @@ __device__ __forceinline__ int geom_forward(const float4 mean, const float4 ls, 
   g.w = expf(-0.5f * g.dt * g.dt / g.b);
   if (!isfinite(g.w) || !(g.b > 0.f) || !isfinite(g.b)) return G_CULL_NONFINITE;
   if (g.w < cp.marginal_min) return G_CULL_TIME;
+  // the primitive is alive at t: start fetching what only survivors read (its colour block) under the arithmetic below
+  if (prefetch) prefetch_l2(prefetch, prefetch_bytes);
   // eq. 9 in factor form
   const float inv_b = 1.0f / g.b;
   const float mu3[3] = {mean.x, mean.y, mean.z};

@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(128) preprocess_fwd_kernel(const fdgs_scene sc
   float radius = 0.f;
   if (i < sc.N) {
     const int st = geom_forward(ldg4(sc.mean, i), ldg4(sc.log_scale, i), ldg4(sc.quat_l, i), ldg4(sc.quat_r, i),
-                                __ldg(sc.opacity_logit + i), vp, cp, g);
+                                __ldg(sc.opacity_logit + i), vp, cp, g, sc.sh + (size_t)i * sc.n_time * KD * 3, sc.n_time * KD * 12);
     if (st == G_VISIBLE) {
       // support radius and tile rectangle (S9): real-valued r, floor/ceil
       const float mid = 0.5f * (g.a2 + g.c2), hd = 0.5f * (g.a2 - g.c2);

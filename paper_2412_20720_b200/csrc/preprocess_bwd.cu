@@ -73,6 +73,11 @@ __global__ void __launch_bounds__(32 * CB_WARPS) colour_bwd_kernel(const float* 
   int i = 0;
   if (have) {
     i = vis_list[slot];
+    if (lane < 8) {  // first batch of 8 survivors: both 12K-byte blocks on their way from HBM while the tables are built
+      const size_t off = (size_t)i * (n_time * KD * 3);
+      prefetch_l2(sh + off, n_time * KD * 12);
+      prefetch_l2(dsh + off, n_time * KD * 12);
+    }
     float* my = tab[warp][lane];
     const float4 a = __ldg(aux + i);
     float Y[KD], G[3 * KD];
@@ -97,6 +102,11 @@ __global__ void __launch_bounds__(32 * CB_WARPS) colour_bwd_kernel(const float* 
 #pragma unroll 1
   for (int b = 0; b < 4; ++b) {
     const int s = 8 * b + grp;
+    if (have && (lane >> 3) == b + 1) {     // next batch's blocks: requested one batch ahead (deeper would thrash L2)
+      const size_t off = (size_t)i * rec_len;
+      prefetch_l2(sh + off, 4 * rec_len);
+      prefetch_l2(dsh + off, 4 * rec_len);
+    }
     const int id = __shfl_sync(0xffffffffu, i, s);
     const bool valid = __shfl_sync(0xffffffffu, (int)have, s) != 0;
     float ax = 0.f, ay = 0.f, az = 0.f, ad = 0.f;

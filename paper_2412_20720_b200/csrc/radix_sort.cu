@@ -8,6 +8,7 @@
 
 namespace fdgs {
 
+constexpr int LB_WIN = 8;
 constexpr unsigned int LB_AGG = 1u << 30, LB_PRE = 2u << 30, LB_MASK = (1u << 30) - 1;
 
 // Global digit histograms of all passes in one read of the keys.
@@ -73,18 +74,25 @@ __global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const unsigned i
       key[r] = idx < n ? keys_in[idx] : 0xffffffffu;
       val[r] = idx < n ? vals_in[idx] : 0u;
     }
-    // ---- stable rank inside the warp's chunk: match_any groups equal digits, the lowest lane of a group bumps the count
+    // ---- stable rank inside the warp's chunk: match_any groups equal digits; the lowest lane of a group adds the group
+    // size to the warp's digit counter with one shared atomic that returns the count of earlier rounds.  The ITEMS
+    // match_any are independent of each other and the atomics of one warp retire in program order, so nothing in this
+    // loop waits on the previous round.
+    unsigned int grp[ITEMS];
 #pragma unroll
     for (int r = 0; r < ITEMS; ++r) {
       const bool valid = warp_base + r * 32 + lane < n;
       const unsigned int digit = valid ? ((key[r] >> shift) & (RADIX - 1)) : 0xffffffffu;
-      const unsigned int grp = __match_any_sync(0xffffffffu, digit);
-      const int leader = __ffs(grp) - 1;
+      grp[r] = __match_any_sync(0xffffffffu, digit);
+    }
+#pragma unroll
+    for (int r = 0; r < ITEMS; ++r) {
+      const bool valid = warp_base + r * 32 + lane < n;
+      const int leader = __ffs(grp[r]) - 1;
       unsigned int old = 0;
-      if (valid && lane == leader) { old = warp_hist[warp][digit]; warp_hist[warp][digit] = old + __popc(grp); }
+      if (valid && lane == leader) old = atomicAdd(&warp_hist[warp][(key[r] >> shift) & (RADIX - 1)], (unsigned int)__popc(grp[r]));
       old = __shfl_sync(0xffffffffu, old, leader);
-      rank[r] = (unsigned short)(old + __popc(grp & lt_mask));
-      __syncwarp();
+      rank[r] = (unsigned short)(old + __popc(grp[r] & lt_mask));
     }
     __syncthreads();
     // ---- thread d owns digit d: exclusive offsets over warps, tile count, look-back, local digit base
@@ -96,13 +104,21 @@ __global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const unsigned i
     *lb = (tile == 0 ? LB_PRE : LB_AGG) | cnt;
     unsigned int excl_tiles = 0;
     if (tile > 0) {
+      // windowed look-back: LB_WIN predecessors are read with independent loads, then consumed nearest first; the walk
+      // stops at the first inclusive prefix and re-polls from the first entry that is not published yet
       long long j = (long long)tile - 1;
-      while (true) {
-        unsigned int s;
-        do { s = lookback[(size_t)j * RADIX + d]; } while ((s >> 30) == 0);
-        excl_tiles += s & LB_MASK;
-        if ((s >> 30) == 2 || j == 0) break;
-        --j;
+      bool found = false;
+      while (!found) {
+        unsigned int sv[LB_WIN];
+#pragma unroll
+        for (int w = 0; w < LB_WIN; ++w) sv[w] = j - w >= 0 ? lookback[(size_t)(j - w) * RADIX + d] : (2u << 30);
+#pragma unroll
+        for (int w = 0; w < LB_WIN; ++w) {
+          if (found || (sv[w] >> 30) == 0) break;
+          excl_tiles += sv[w] & LB_MASK;
+          --j;
+          if ((sv[w] >> 30) == 2) found = true;
+        }
       }
       *lb = LB_PRE | (excl_tiles + cnt);
     }
