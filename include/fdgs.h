@@ -122,7 +122,9 @@ int fdgs_l1_loss(const float *image, const float *target, int64_t count, float *
 /* One forward(+backward) pass over one view with HOST target / result buffers: copies target_host
  * [3,H,W] to `target_dev`, runs preprocess + forward (+ L1 loss + backward if grads_host != NULL),
  * copies the loss (1 float) — or, when grads_host == NULL, the image — back to the host and
- * synchronises the stream.  target_host / result_host should be pinned. */
+ * synchronises the stream.  target_host / result_host should be pinned.  The host -> device copy of the target runs
+ * on a library-owned copy stream, forked from and joined to `cuda_stream` by events, so it overlaps preprocess and
+ * forward; `target_dev` must not be touched by other streams during the call. */
 int fdgs_step_host(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws,
                    size_t ws_bytes, int64_t pair_capacity, void *cuda_stream, const float *target_host,
                    float *target_dev, float *image, float *final_T, uint32_t *n_contrib, float *dL_dimage,

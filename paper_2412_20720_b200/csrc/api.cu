@@ -148,7 +148,7 @@ static int forward_impl(const fdgs_scene* sc, const ViewParams& vp, const CfgPar
                         cudaStream_t st, float* image, float* final_T, uint32_t* n_contrib, int* l1_buf_out, int* l2_buf_out) {
   // scan_ticket[1] and sort_ticket[0..7] are adjacent in the header: clear them together
   FDGS_CUDA(cudaMemsetAsync(&ws.hdr->scan_ticket[1], 0, 9 * sizeof(unsigned int), st), "memset(tickets)");
-  FDGS_CUDA(cudaMemsetAsync(ws.scan_state[1], 0, 8 * (((size_t)(sc->N > 0 ? sc->N : 1) + SCAN_TILE - 1) / SCAN_TILE + 1), st), "memset(scan)");
+  FDGS_CUDA(cudaMemsetAsync(ws.scan_state[1], 0, 8 * ((size_t)(sc->N > 0 ? sc->N : 1) / 256 + 2), st), "memset(scan)");
   const int sms = num_sms();
   mark(EV_FWD0, st);
   const int l1 = launch_sort_pairs(ws, ws.l1_keys, ws.l1_vals, &ws.hdr->num_visible, sc->N, 32, SORT_ITEMS_L1, 0, false, sms, st);
@@ -223,6 +223,10 @@ int fdgs_l1_loss(const float* image, const float* target, int64_t count, float* 
   return FDGS_OK;
 }
 
+// Copy stream of fdgs_step_host: the target image travels host -> device while preprocess and forward run.
+static cudaStream_t g_copy_stream = nullptr;
+static cudaEvent_t g_copy_fork = nullptr, g_copy_join = nullptr;
+
 int fdgs_step_host(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws, size_t ws_bytes, int64_t cap,
                    void* stream, const float* target_host, float* target_dev, float* image, float* final_T,
                    uint32_t* n_contrib, float* dL_dimage, float* loss_dev, fdgs_grads* g, float* result_host) {
@@ -231,7 +235,16 @@ int fdgs_step_host(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* 
   const size_t count = (size_t)3 * v->width * v->height;
   if (g) {
     if (!target_host || !target_dev || !dL_dimage || !loss_dev) return FDGS_ERR_INVALID;
-    FDGS_CUDA(cudaMemcpyAsync(target_dev, target_host, count * sizeof(float), cudaMemcpyHostToDevice, st), "H2D target");
+    if (!g_copy_stream) {
+      FDGS_CUDA(cudaStreamCreateWithFlags(&g_copy_stream, cudaStreamNonBlocking), "copy stream");
+      FDGS_CUDA(cudaEventCreateWithFlags(&g_copy_fork, cudaEventDisableTiming), "copy event");
+      FDGS_CUDA(cudaEventCreateWithFlags(&g_copy_join, cudaEventDisableTiming), "copy event");
+    }
+    // fork: the copy may start once everything queued on `st` so far (the previous user of target_dev) is done
+    FDGS_CUDA(cudaEventRecord(g_copy_fork, st), "fork");
+    FDGS_CUDA(cudaStreamWaitEvent(g_copy_stream, g_copy_fork, 0), "fork wait");
+    FDGS_CUDA(cudaMemcpyAsync(target_dev, target_host, count * sizeof(float), cudaMemcpyHostToDevice, g_copy_stream), "H2D target");
+    FDGS_CUDA(cudaEventRecord(g_copy_join, g_copy_stream), "join");
     FDGS_CUDA(cudaMemsetAsync(loss_dev, 0, sizeof(float), st), "memset(loss)");
   }
   int rc = fdgs_preprocess(sc, v, c, ws, ws_bytes, cap, stream, nullptr, nullptr);
@@ -239,6 +252,7 @@ int fdgs_step_host(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* 
   rc = fdgs_render_forward(sc, v, c, ws, ws_bytes, cap, stream, image, final_T, n_contrib);
   if (rc) return rc;
   if (g) {
+    FDGS_CUDA(cudaStreamWaitEvent(st, g_copy_join, 0), "join wait");
     rc = fdgs_l1_loss(image, target_dev, (int64_t)count, dL_dimage, loss_dev, stream);
     if (rc) return rc;
     rc = fdgs_render_backward(sc, v, c, ws, ws_bytes, cap, stream, dL_dimage, final_T, n_contrib, g);

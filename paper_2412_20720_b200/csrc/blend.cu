@@ -329,35 +329,38 @@ __global__ void __launch_bounds__(256 / PX) blend_bwd_kernel(const uint2* __rest
 // loads), two shuffle levels join the four partial sums and three shared atomics per lane add them to the splat's
 // accumulators.  That replaces, per (warp, splat) hit, the 14-shuffle reduction, the nine products per pixel and the
 // per-hit atomic of the direct kernel by one STS.128 and ~1/8 of a 300-instruction flush.
-constexpr int HB = 8;      // hits buffered per warp
 constexpr int HROW = 36;   // float4 per buffered hit: 32 lanes + pad (144 words = 16 mod 32: quarter-warps hit 32 banks)
 
+template <int HBUF>        // hits buffered per warp (4, 8 or 16; 8 measured best: 4 flushes too often, 16 costs occupancy)
 struct Bwd2Shared {
   float4 s0[128], s1[128], s2[128];
   float acc[9 * 129];
   unsigned int id[128];
   int max_contrib;
-  int hitj[4][HB];
-  float4 hit[4][HB][HROW];
+  int hitj[4][HBUF];
+  float4 hit[4][HBUF][HROW];
   float4 pg[4][32][2];     // per warp, per lane: (gr0, gg0, gb0, gr1), (gg1, gb1, -, -)
 };
 
-__device__ __forceinline__ void bwd2_flush(Bwd2Shared& sm, const int warp, const int lane, const int n, const float sx0, const float sy0) {
+template <int HBUF>
+__device__ __forceinline__ void bwd2_flush(Bwd2Shared<HBUF>& sm, const int warp, const int lane, const int n, const float sx0, const float sy0) {
+  constexpr int LPH = 32 / HBUF;             // lanes per buffered hit (4 or 8); each sums 64 / LPH pixels
   __syncwarp();
-  const int h = lane >> 2, q = lane & 3;
+  const int h = lane / LPH, q = lane % LPH;
   float S[9] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};   // Sx, Sy, Sxx, Sxy, Syy, cr, cg, cb, S1
   int j = 0;
   if (h < n) {
     j = sm.hitj[warp][h];
     const float4 c = sm.s2[j];
-    const float ux = c.y - (sx0 + 0.5f) - (float)q, vy = c.z - (sy0 + 0.5f);
+    const float ux = c.y - (sx0 + 0.5f) - (float)(q & 7), vy = c.z - (sy0 + 0.5f);
     const float4* row = sm.hit[warp][h];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {            // pixel slot p = 4 i + q: column (p % 8), row (p / 8) of both sub-patches
-      const int p = 4 * i + q;
+    for (int i = 0; i < 32 / LPH; ++i) {     // pixel slot p = LPH i + q: column (p % 8), row (p / 8) of both sub-patches
+      const int p = LPH * i + q;
       const float4 d = row[p];               // dpow0, wgt0, dpow1, wgt1
       const float4 g0 = sm.pg[warp][p][0], g1 = sm.pg[warp][p][1];
-      const float dx = ux - (float)(4 * (i & 1)), dy0 = vy - (float)(i >> 1), dy1 = dy0 - 4.0f;
+      const float dx = ux - (float)((LPH * i) & 7);
+      const float dy0 = vy - (float)((LPH * i) >> 3), dy1 = dy0 - 4.0f;
       const float mx0 = d.x * dx, my0 = d.x * dy0, mx1 = d.z * dx, my1 = d.z * dy1;
       S[0] += mx0; S[0] += mx1; S[1] += my0; S[1] += my1;
       S[2] = fmaf(mx0, dx, S[2]); S[2] = fmaf(mx1, dx, S[2]);
@@ -369,23 +372,38 @@ __device__ __forceinline__ void bwd2_flush(Bwd2Shared& sm, const int warp, const
     }
   }
 #pragma unroll
-  for (int k = 0; k < 9; ++k) { S[k] += __shfl_xor_sync(0xffffffffu, S[k], 1); S[k] += __shfl_xor_sync(0xffffffffu, S[k], 2); }
-  if (h < n) {                               // rows q, q + 4 (and 8 on q == 0) of the splat's accumulators
-    const float r0 = q == 0 ? S[0] : q == 1 ? S[1] : q == 2 ? S[2] : S[3];
-    const float r1 = q == 0 ? S[4] : q == 1 ? S[5] : q == 2 ? S[6] : S[7];
-    atomicAdd(&sm.acc[q * 129 + j], r0);
-    atomicAdd(&sm.acc[(q + 4) * 129 + j], r1);
+  for (int k = 0; k < 9; ++k)
+#pragma unroll
+    for (int o = 1; o < LPH; o <<= 1) S[k] += __shfl_xor_sync(0xffffffffu, S[k], o);
+  if (h < n) {                               // every lane of the hit holds all nine sums: lane q adds rows q, q + LPH, ...
+    if (LPH == 2) {
+      atomicAdd(&sm.acc[q * 129 + j], q ? S[1] : S[0]);
+      atomicAdd(&sm.acc[(q + 2) * 129 + j], q ? S[3] : S[2]);
+      atomicAdd(&sm.acc[(q + 4) * 129 + j], q ? S[5] : S[4]);
+      atomicAdd(&sm.acc[(q + 6) * 129 + j], q ? S[7] : S[6]);
+    } else if (LPH == 4) {
+      const float r0 = q == 0 ? S[0] : q == 1 ? S[1] : q == 2 ? S[2] : S[3];
+      const float r1 = q == 0 ? S[4] : q == 1 ? S[5] : q == 2 ? S[6] : S[7];
+      atomicAdd(&sm.acc[q * 129 + j], r0);
+      atomicAdd(&sm.acc[(q + 4) * 129 + j], r1);
+    } else {
+      float r0 = S[0];
+#pragma unroll
+      for (int k = 1; k < 8; ++k) r0 = q == k ? S[k] : r0;
+      atomicAdd(&sm.acc[q * 129 + j], r0);
+    }
     if (q == 0) atomicAdd(&sm.acc[8 * 129 + j], S[8]);
   }
   __syncwarp();
 }
 
-__global__ void __launch_bounds__(128) blend_bwd2_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
+template <int HBUF, int MINB>
+__global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
                                                          const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
                                                          const float* __restrict__ dL_dimage, const float* __restrict__ final_T,
                                                          const unsigned int* __restrict__ n_contrib, float* __restrict__ g9) {
   constexpr int PX = 2, BATCH = 128, ACC_STRIDE = 129;
-  __shared__ Bwd2Shared sm;
+  __shared__ Bwd2Shared<HBUF> sm;
   const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const Strip<PX> sp(warp, lane);
@@ -477,10 +495,10 @@ __global__ void __launch_bounds__(128) blend_bwd2_kernel(const uint2* __restrict
         }
         sm.hit[warp][nbuf][lane] = make_float4(dpow[0], wgt[0], dpow[1], wgt[1]);
         if (lane == 0) sm.hitj[warp][nbuf] = j;
-        if (++nbuf == HB) { bwd2_flush(sm, warp, lane, HB, sx0, sy0); nbuf = 0; }
+        if (++nbuf == HBUF) { bwd2_flush<HBUF>(sm, warp, lane, HBUF, sx0, sy0); nbuf = 0; }
       }
      }
-     if (nbuf) bwd2_flush(sm, warp, lane, nbuf, sx0, sy0);
+     if (nbuf) bwd2_flush<HBUF>(sm, warp, lane, nbuf, sx0, sy0);
     }
     __syncthreads();
     if ((int)threadIdx.x < m) {
@@ -534,7 +552,7 @@ void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, con
     case 4: FDGS_BWD(4); break;
     default:
       if (direct) FDGS_BWD(2);
-      else blend_bwd2_kernel<<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9);
+      else blend_bwd2_kernel<8, 6><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9);
   }
 #undef FDGS_BWD
   ++g_launches;

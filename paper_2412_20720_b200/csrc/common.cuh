@@ -78,7 +78,7 @@ struct Workspace {
   unsigned int* offsets;             // [N] exclusive prefix sum of tiles_touched in depth order
   unsigned int* l2_keys[2];          // [cap] tile ids
   unsigned int* l2_vals[2];          // [cap] primitive ids
-  unsigned int* sort_hist;           // [8][RADIX] global digit histograms -> exclusive bases
+  unsigned int* sort_hist;           // [8][RADIX] digit counts of the 4 depth passes (raw) and exclusive bases of the tile-id passes
   unsigned int* sort_lookback;       // [max sort tiles][RADIX]
   uint2* ranges;                     // [tiles] [first, last+1)
   float* g9;                         // [N,9] per-splat gradients of the blend backward
@@ -99,7 +99,8 @@ inline Workspace carve(void* base, long long N, long long K, long long W, long l
   const long long Np = N > 0 ? N : 1;
   w.hdr = (WsHeader*)take(sizeof(WsHeader));
   w.tile_diff = (int*)take(4 * (size_t)(tx + 1) * (ty + 1));
-  for (int i = 0; i < 2; ++i) w.scan_state[i] = (unsigned long long*)take(8 * ((Np + SCAN_TILE - 1) / SCAN_TILE + 1));
+  for (int i = 0; i < 2; ++i) w.scan_state[i] = (unsigned long long*)take(8 * (Np / 256 + 2));   // chained-scan tiles of >= 256 items
+  w.sort_hist = (unsigned int*)take(4 * 8 * RADIX);     // level-1 digit counts are accumulated by the compaction kernel
   w.zero_bytes = off;
   w.rec = (SplatRec*)take(sizeof(SplatRec) * Np);
   w.rect = (ushort4*)take(sizeof(ushort4) * Np);
@@ -110,7 +111,6 @@ inline Workspace carve(void* base, long long N, long long K, long long W, long l
   w.offsets = (unsigned int*)take(4 * Np);
   for (int i = 0; i < 2; ++i) w.l2_keys[i] = (unsigned int*)take(4 * (size_t)cap);
   for (int i = 0; i < 2; ++i) w.l2_vals[i] = (unsigned int*)take(4 * (size_t)cap);
-  w.sort_hist = (unsigned int*)take(4 * 8 * RADIX);
   const long long t1 = (Np + SORT_THREADS * SORT_ITEMS_L1 - 1) / (SORT_THREADS * SORT_ITEMS_L1);
   const long long t2 = (cap + SORT_THREADS * SORT_ITEMS_L2 - 1) / (SORT_THREADS * SORT_ITEMS_L2);
   w.lookback_bytes = 4 * (size_t)RADIX * ((t1 > t2 ? t1 : t2) + 1);
@@ -142,10 +142,11 @@ void launch_preprocess_fwd(const fdgs_scene& sc, const ViewParams& vp, const Cfg
 // compaction scan: survivors (tiles_touched > 0) in id order -> l1_keys[0] (depth bits), l1_vals[0] (ids), hdr->num_visible
 void launch_compact(const Workspace& ws, int N, cudaStream_t st);
 // Stable LSD radix sort of (key, val) u32 pairs on key bits [0, bits); the count is read on the device.
-// If hist_ready, ws.sort_hist[pass] already holds the exclusive digit bases.  Returns the result buffer (0/1).
+// ws.sort_hist[ticket_base + pass] holds the digit counts of the pass (bases_exclusive = false: every CTA scans them
+// itself) or their exclusive prefix (true).  Returns the result buffer (0/1).
 int launch_sort_pairs(const Workspace& ws, unsigned int* const keys[2], unsigned int* const vals[2],
                       const unsigned int* count_dev, long long max_count, int bits, int items_per_thread, int ticket_base,
-                      bool hist_ready, int num_sms, cudaStream_t st);
+                      bool bases_exclusive, int num_sms, cudaStream_t st);
 // 2D prefix of the coverage difference array -> ranges, D, overflow flag, level-2 digit bases
 void launch_tile_grid(const Workspace& ws, const ViewParams& vp, long long cap, int l2_passes, cudaStream_t st);
 // exclusive prefix sum of tiles_touched in depth order -> offsets

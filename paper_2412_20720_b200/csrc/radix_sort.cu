@@ -3,7 +3,9 @@
 // match_any multisplit (stable), publishes its digit counts, obtains the counts of all earlier tiles by
 // decoupled look-back, and scatters straight to the final position of the pass — keys and values are read
 // once and written once per pass.  Tiles take dynamic ids from a ticket, CTAs are persistent, and the number
-// of pairs is read from device memory, so the host never synchronises.
+// of pairs is read from device memory, so the host never synchronises.  The global digit counts come from the producer
+// of the keys (compaction kernel for the depth sort, tile-grid kernel for the tile-id sort): the keys are never read
+// just to be counted.
 #include "common.cuh"
 
 namespace fdgs {
@@ -11,42 +13,12 @@ namespace fdgs {
 constexpr int LB_WIN = 8;
 constexpr unsigned int LB_AGG = 1u << 30, LB_PRE = 2u << 30, LB_MASK = (1u << 30) - 1;
 
-// Global digit histograms of all passes in one read of the keys.
-__global__ void __launch_bounds__(256) sort_hist_kernel(const unsigned int* __restrict__ keys, const unsigned int* __restrict__ count_dev,
-                                                        const int passes, unsigned int* __restrict__ hist /*[passes][RADIX]*/) {
-  __shared__ unsigned int sh[4][RADIX];
-  for (int i = threadIdx.x; i < 4 * RADIX; i += blockDim.x) (&sh[0][0])[i] = 0;
-  __syncthreads();
-  const unsigned int n = *count_dev;
-  for (unsigned int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-    const unsigned int k = keys[i];
-    for (int p = 0; p < passes; ++p) atomicAdd(&sh[p][(k >> (RADIX_BITS * p)) & (RADIX - 1)], 1u);
-  }
-  __syncthreads();
-  for (int i = threadIdx.x; i < passes * RADIX; i += blockDim.x) { const unsigned int v = (&sh[0][0])[i]; if (v) atomicAdd(hist + i, v); }
-}
-
-// exclusive scan of each pass's 256 bins (one warp per pass)
-__global__ void sort_hist_scan_kernel(unsigned int* hist, const int passes) {
-  const int p = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  if (p >= passes) return;
-  unsigned int v[8], s = 0;
-#pragma unroll
-  for (int k = 0; k < 8; ++k) { v[k] = hist[p * RADIX + lane * 8 + k]; s += v[k]; }
-  unsigned int incl = s;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) { const unsigned int n = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += n; }
-  unsigned int r = incl - s;
-#pragma unroll
-  for (int k = 0; k < 8; ++k) { hist[p * RADIX + lane * 8 + k] = r; r += v[k]; }
-}
-
 template <int ITEMS>
 __global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const unsigned int* __restrict__ keys_in, const unsigned int* __restrict__ vals_in,
                                                                 unsigned int* __restrict__ keys_out, unsigned int* __restrict__ vals_out,
                                                                 const unsigned int* __restrict__ count_dev, unsigned int* ticket,
-                                                                const unsigned int* __restrict__ digit_base /*[RADIX] exclusive*/,
-                                                                volatile unsigned int* lookback, const int shift) {
+                                                                const unsigned int* __restrict__ digit_base /*[RADIX]*/,
+                                                                const bool bases_exclusive, volatile unsigned int* lookback, const int shift) {
   constexpr int TILE_N = SORT_THREADS * ITEMS, WARPS = SORT_THREADS / 32;
   __shared__ unsigned int warp_hist[WARPS][RADIX];   // per-warp digit counts -> exclusive offsets over warps
   __shared__ unsigned int s_local[RADIX];            // first slot of each digit inside the sorted tile
@@ -57,6 +29,20 @@ __global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const unsigned i
   const unsigned int lt_mask = (1u << lane) - 1;
   const unsigned int n = *count_dev;
   const unsigned int num_tiles = (n + TILE_N - 1) / TILE_N;
+  // global position of the first key of digit d = threadIdx.x: given, or the exclusive scan of the raw digit counts
+  unsigned int my_base = digit_base[threadIdx.x];
+  if (!bases_exclusive) {
+    unsigned int incl = my_base;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const unsigned int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
+    if (lane == 31) warp_sums[warp] = incl;
+    __syncthreads();
+    unsigned int wprefix = 0;
+#pragma unroll
+    for (int w = 0; w < WARPS; ++w) if (w < warp) wprefix += warp_sums[w];
+    my_base = wprefix + incl - my_base;
+    __syncthreads();
+  }
   while (true) {
     if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
 #pragma unroll
@@ -133,7 +119,7 @@ __global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const unsigned i
     for (int w = 0; w < WARPS; ++w) if (w < warp) wprefix += warp_sums[w];
     const unsigned int local = wprefix + incl - cnt;
     s_local[d] = local;
-    s_global[d] = digit_base[d] + excl_tiles - local;
+    s_global[d] = my_base + excl_tiles - local;
     __syncthreads();
     // ---- scatter into the tile's sorted order in shared memory
 #pragma unroll
@@ -162,17 +148,10 @@ __global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const unsigned i
 
 int launch_sort_pairs(const Workspace& ws, unsigned int* const keys[2], unsigned int* const vals[2],
                       const unsigned int* count_dev, long long max_count, int bits, int items_per_thread, int ticket_base,
-                      bool hist_ready, int num_sms, cudaStream_t st) {
+                      bool bases_exclusive, int num_sms, cudaStream_t st) {
   const int passes = (bits + RADIX_BITS - 1) / RADIX_BITS;
   if (passes <= 0 || max_count <= 0) return 0;
-  unsigned int* hist = ws.sort_hist + (size_t)ticket_base * RADIX;
-  if (!hist_ready) {
-    cudaMemsetAsync(hist, 0, sizeof(unsigned int) * passes * RADIX, st);
-    const int hb = (int)((max_count + 256 * 16 - 1) / (256 * 16));
-    sort_hist_kernel<<<hb < 4 * num_sms ? hb : 4 * num_sms, 256, 0, st>>>(keys[0], count_dev, passes, hist);
-    sort_hist_scan_kernel<<<1, 32 * passes, 0, st>>>(hist, passes);
-    g_launches += 2;
-  }
+  const unsigned int* hist = ws.sort_hist + (size_t)ticket_base * RADIX;
   const int tile_n = SORT_THREADS * items_per_thread;
   const long long tiles = (max_count + tile_n - 1) / tile_n;
   const size_t lb_bytes = sizeof(unsigned int) * RADIX * (size_t)tiles;
@@ -183,11 +162,11 @@ int launch_sort_pairs(const Workspace& ws, unsigned int* const keys[2], unsigned
     if (items_per_thread == SORT_ITEMS_L1)
       onesweep_kernel<SORT_ITEMS_L1><<<grid, SORT_THREADS, 0, st>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], count_dev,
                                                                    &ws.hdr->sort_ticket[ticket_base + p], hist + p * RADIX,
-                                                                   ws.sort_lookback, p * RADIX_BITS);
+                                                                   bases_exclusive, ws.sort_lookback, p * RADIX_BITS);
     else
       onesweep_kernel<SORT_ITEMS_L2><<<grid, SORT_THREADS, 0, st>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], count_dev,
                                                                    &ws.hdr->sort_ticket[ticket_base + p], hist + p * RADIX,
-                                                                   ws.sort_lookback, p * RADIX_BITS);
+                                                                   bases_exclusive, ws.sort_lookback, p * RADIX_BITS);
     ++g_launches;
     cur ^= 1;
   }

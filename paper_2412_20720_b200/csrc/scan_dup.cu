@@ -1,4 +1,4 @@
-// scan_dup.cu — A5/A6/A8 for sm_100a: compaction scan, tile-grid prefix (ranges, D), offsets scan, pair emission.
+// scan_dup.cu — A5/A6/A8 for sm_100a: compaction scan (+ depth digit counts), tile-grid prefix (ranges, D), offsets scan, pair emission.
 #include "common.cuh"
 
 namespace fdgs {
@@ -59,13 +59,17 @@ __device__ __forceinline__ unsigned int lookback_prefix(volatile unsigned long l
   return *s_bcast;
 }
 
-// Compaction: survivors (tiles_touched > 0) in primitive-id order -> (depth bits, id) pairs.
+// Compaction: survivors (tiles_touched > 0) in primitive-id order -> (depth bits, id) pairs, plus the digit counts of
+// the four 8-bit passes of the depth sort (the keys are in registers here: the sort never reads them just to count).
 __global__ void __launch_bounds__(SCAN_THREADS) compact_kernel(const unsigned int* __restrict__ tiles_touched,
                                                                const SplatRec* __restrict__ rec, const int N, WsHeader* hdr,
                                                                unsigned long long* state, unsigned int* __restrict__ keys,
-                                                               unsigned int* __restrict__ vals, unsigned int* __restrict__ vis_ids) {
-  __shared__ unsigned int warp_sums[33], s_tile, s_prefix;
+                                                               unsigned int* __restrict__ vals, unsigned int* __restrict__ vis_ids,
+                                                               unsigned int* __restrict__ sort_hist) {
+  __shared__ unsigned int warp_sums[33], s_tile, s_prefix, hist[4][RADIX];
   if (threadIdx.x == 0) s_tile = atomicAdd(&hdr->scan_ticket[0], 1u);
+#pragma unroll
+  for (int p = 0; p < 4; ++p) hist[p][threadIdx.x] = 0;     // SCAN_THREADS == RADIX
   __syncthreads();
   const unsigned int tile = s_tile;
   const long long base = (long long)tile * SCAN_TILE + (long long)threadIdx.x * SCAN_ITEMS;
@@ -79,8 +83,16 @@ __global__ void __launch_bounds__(SCAN_THREADS) compact_kernel(const unsigned in
   unsigned int pos = prefix + excl;
 #pragma unroll
   for (int k = 0; k < SCAN_ITEMS; ++k)
-    if (flags & (1u << k)) { keys[pos] = __float_as_uint(rec[base + k].depth); vals[pos] = (unsigned int)(base + k); vis_ids[pos] = (unsigned int)(base + k); ++pos; }
+    if (flags & (1u << k)) {
+      const unsigned int key = __float_as_uint(rec[base + k].depth);
+      keys[pos] = key; vals[pos] = (unsigned int)(base + k); vis_ids[pos] = (unsigned int)(base + k); ++pos;
+#pragma unroll
+      for (int p = 0; p < 4; ++p) atomicAdd(&hist[p][(key >> (RADIX_BITS * p)) & (RADIX - 1)], 1u);
+    }
   if (tile == gridDim.x - 1 && threadIdx.x == 0) hdr->num_visible = prefix + total;
+  __syncthreads();
+#pragma unroll
+  for (int p = 0; p < 4; ++p) { const unsigned int v = hist[p][threadIdx.x]; if (v) atomicAdd(sort_hist + p * RADIX + threadIdx.x, v); }
 }
 
 // offsets[j] = exclusive prefix of tiles_touched[sorted_ids[j]], j < num_visible (depth order)
@@ -209,7 +221,7 @@ __global__ void l1_loss_kernel(const float* __restrict__ image, const float* __r
 void launch_compact(const Workspace& ws, int N, cudaStream_t st) {
   if (N <= 0) return;
   const int blocks = (N + SCAN_TILE - 1) / SCAN_TILE;
-  compact_kernel<<<blocks, SCAN_THREADS, 0, st>>>(ws.tiles_touched, ws.rec, N, ws.hdr, ws.scan_state[0], ws.l1_keys[0], ws.l1_vals[0], ws.vis_ids);
+  compact_kernel<<<blocks, SCAN_THREADS, 0, st>>>(ws.tiles_touched, ws.rec, N, ws.hdr, ws.scan_state[0], ws.l1_keys[0], ws.l1_vals[0], ws.vis_ids, ws.sort_hist);
   ++g_launches;
 }
 
