@@ -25,7 +25,39 @@ METRIC = "fwd+bwd steps/s, 1M 4D Gaussians @1352x1014, batch of 4 views"
 WORKLOAD = "cfg3_video: N=1M, K=48 (L=3 x n_time=3), 1352x1014, fov 60, 4 jittered views at 4 seeded times, L1 loss"
 PAIR_CAPACITY = 16 * 1024 * 1024
 SM_COUNT, LANES_PER_SM, SM_MAX_HZ = 148, 128, 1.965e9
-ALU_PEAK_TLANE = SM_COUNT * LANES_PER_SM * SM_MAX_HZ / 1e12      # 37.2 T lane-instructions/s (DESIGN.md "roofline")
+ALU_PEAK_TLANE = SM_COUNT * LANES_PER_SM * SM_MAX_HZ / 1e12      # 37.2 T lane-instructions/s (DESIGN.md section 6)
+# DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/r1_blend_bwd2_ncu_full.md)
+BLEND_BWD_NCU_TRAFFIC_BYTES = 94.9e6
+
+
+def hbm_peak():
+    """Measured copy bandwidth of this pool's B200s (driver-written MEASURED_PEAKS.json), else the guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def stage_rooflines(stage, work, N, K, n_views):
+    """Every stage against its own roof: algorithmic bytes / CUDA-event time vs the HBM copy peak for
+    the memory-bound stages, algorithmic lane-instructions vs the ALU issue peak for the two blend kernels."""
+    peak, src = hbm_peak()
+    nv, D = work["visible"], work["pairs"]          # summed over the views of the step
+    byts = {"preprocess": n_views * 72 * N + nv * (12 * K + 76),
+            "compact+tile_grid": n_views * 4 * N + 16 * nv,
+            "sort_depth": 4 * 16 * nv,
+            "offsets+duplicate": 16 * nv + 8 * D,
+            "sort_tile": 2 * 16 * D,
+            "preprocess_bwd": nv * (36 + 68 + 12 * K + 2 * (12 * K + 68) + 64)}
+    out = {}
+    for k, b in byts.items():
+        gbs = b / (stage[k] * 1e-3) / 1e9
+        out[k] = {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "algorithmic_bytes": b}
+    out["peak_source_hbm"] = src
+    return out
+
+
 
 
 class ClockSampler(threading.Thread):
@@ -233,16 +265,25 @@ def run_fdgs(args):
     dom = "blend_bwd" if stage["blend_bwd"] >= stage["blend_fwd"] else "blend_fwd"
     instr = instr_bwd if dom == "blend_bwd" else instr_fwd
     achieved = instr / n_views / (stage[dom] / n_views * 1e-3) / 1e12
-    roofline = {"kernel": dom + "_kernel", "bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TLANE, "unit": "Tlane-instr/s",
-                "frac": achieved / ALU_PEAK_TLANE, "traffic": None,
+    roofline = {"kernel": "blend_bwd2_kernel" if dom == "blend_bwd" else "blend_fwd_kernel", "bound": "alu", "achieved": achieved,
+                "peak": ALU_PEAK_TLANE, "unit": "Tlane-instr/s", "frac": achieved / ALU_PEAK_TLANE,
+                "traffic": BLEND_BWD_NCU_TRAFFIC_BYTES if dom == "blend_bwd" else None,
                 "peak_source": "derived: 148 SMs x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md unit counts and max clock)",
                 "algorithmic_lane_instr_per_launch": instr / n_views, "ms_per_launch": stage[dom] / n_views}
+    per_stage = stage_rooflines(stage, work, ds.N, ds.K, n_views)
+    for name, ins in (("blend_fwd", instr_fwd), ("blend_bwd", instr_bwd)):
+        a = ins / (stage[name] * 1e-3) / 1e12
+        per_stage[name] = {"bound": "alu", "achieved": a, "peak": ALU_PEAK_TLANE, "unit": "Tlane-instr/s", "frac": a / ALU_PEAK_TLANE,
+                           "algorithmic_lane_instr": ins}
     # ---- CPU baseline: the oracle on one of the four views ---------------------------------------------------
     cpu = None
     if not args.no_cpu_baseline:
-        t, cores = oracle_view_seconds(scene, 0, 1)
-        cpu = {"value": 1.0 / (n_views * t[0]), "unit": "steps/s", "cores": cores, "kind": "oracle",
-               "sample": f"view 0 of {n_views} (preprocess+forward+L1+backward at N=1M, 1352x1014) in {t[0]:.1f} s, scaled x{n_views}"}
+        tot, cores = 0.0, 0
+        for vi in range(n_views):
+            t, cores = oracle_view_seconds(scene, vi, 1)
+            tot += t[0]
+        cpu = {"value": 1.0 / tot, "unit": "steps/s", "cores": cores, "kind": "oracle",
+               "sample": f"one full step: all {n_views} views (preprocess+forward+L1+backward at N=1M, 1352x1014) in {tot:.1f} s"}
     img_bytes = 3 * views[0].width * views[0].height * 4
     out = {"metric": METRIC, "value": whole_job_value(world, ms_step), "unit": "steps/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -252,7 +293,7 @@ def run_fdgs(args):
            "e2e": {"value": world * 1e3 / ms_e2e, "unit": "steps/s", "h2d_bytes_per_step": n_views * img_bytes, "d2h_bytes_per_step": n_views * 4,
                    "ms_per_step": ms_e2e},
            "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
-           "stage_ms_per_step": stage, "work_per_step": work, "loss": loss_dev,
+           "stage_ms_per_step": stage, "stage_rooflines": per_stage, "work_per_step": work, "loss": loss_dev,
            "paper_context": "114 FPS forward on Plenoptic Video, hardware not named (PAPER.md Table 1, L347) - context only"}
     print(json.dumps(out))
     if world > 1:
