@@ -5,7 +5,7 @@ time-sliced tile rasterizer at 1M 4D Gaussians, 1352x1014, batch of 4 views (cfg
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
 
 One JSON line on stdout (rank 0).  `value` = steps/s with everything resident in HBM; `e2e` = the same through
-fdgs_step_host with pinned HOST target images and the loss read back every view; `roofline` = the dominant kernel
+fdgs_step_batch with pinned HOST target images copied in and the per-view losses read back every step; `roofline` = the dominant kernel
 against the ALU issue roof derived in DESIGN.md; `cpu_baseline` = the float64 oracle on this box's host cores on a
 bounded sample (one of the four views).  --impl reference times that oracle as the reference arm.
 Multi-GPU: the path does not shard: N ranks render N independent replicas.
@@ -162,12 +162,15 @@ def run_fdgs(args):
     views = scene.views
     n_views = len(views)
     ds = fdgs.DeviceScene.from_scene(scene, device=dev)
-    r = fdgs.Renderer(ds, views[0].width, views[0].height, PAIR_CAPACITY)
+    bs = fdgs.BatchStep(ds, views[0].width, views[0].height, PAIR_CAPACITY, n_views)     # one workspace per view of the batch
+    r = bs.renderers[0]
     cviews = [fdgs.make_view(v) for v in views]
     tg_np = [scenes.target_image(scene.seed, i, views[0].width, views[0].height) for i in range(n_views)]
     targets = [torch.from_numpy(t).to(dev) for t in tg_np]
     targets_host = [torch.from_numpy(t).pin_memory() for t in tg_np]
     loss_host = torch.zeros(n_views).pin_memory()
+    for rr, tg in zip(bs.renderers, targets):
+        rr.target_dev.copy_(tg)
     grads = ds.zero_grads()
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)     # > 126 MB L2
 
@@ -176,19 +179,13 @@ def run_fdgs(args):
             if g is not None:
                 g.zero_()
 
-    def step_device():
+    def step_device():       # fdgs_step_batch, targets resident in HBM, nothing read back
         zero_grads()
-        r.loss.zero_()
-        for cv, tg in zip(cviews, targets):
-            r.preprocess(cv)
-            r.forward(cv)
-            r.l1_loss(tg)
-            r.backward(cv, r.dL_dimage, grads)
+        bs.step(cviews, grads)
 
-    def step_host():
+    def step_host():         # fdgs_step_batch with pinned HOST targets copied in and the four losses copied back (synchronises)
         zero_grads()
-        for i, cv in enumerate(cviews):
-            r.step_host(cv, targets_host[i], loss_host[i:i + 1], grads)
+        bs.step(cviews, grads, targets_host=targets_host, loss_host=loss_host)
 
     def forward_only(cv):
         r.preprocess(cv)
@@ -226,10 +223,11 @@ def run_fdgs(args):
     ms_step, _ = timed(step_device, args.steps, args.warmup)
     launches = (fdgs.launch_count() - l0) * args.steps // (args.steps + args.warmup)
     clocks = sampler.stop() if sampler else None
-    status = r.export(fdgs.EXPORT_STATUS)
-    if status["overflow"]:
-        raise RuntimeError(f"pair capacity {PAIR_CAPACITY} exceeded: {status}")
-    loss_dev = float(r.loss[0])
+    for rr in bs.renderers:
+        status = rr.export(fdgs.EXPORT_STATUS)
+        if status["overflow"]:
+            raise RuntimeError(f"pair capacity {PAIR_CAPACITY} exceeded: {status}")
+    loss_dev = float(bs.loss.sum())
     # ---- end to end through the C ABI with host buffers ----------------------------------------------------
     ms_e2e, _ = timed(step_host, max(3, args.steps // 2), 3)
     # ---- forward-only FPS (one frame = preprocess + forward of one view) -----------------------------------
@@ -288,7 +286,8 @@ def run_fdgs(args):
     out = {"metric": METRIC, "value": whole_job_value(world, ms_step), "unit": "steps/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
            "config": {"workload": WORKLOAD, "pair_capacity": PAIR_CAPACITY, "l2": "256 MB flush write between timed steps; parameters (644 MB) exceed L2",
-                      "multi_gpu": "replicas only"},
+                      "multi_gpu": "replicas only",
+                      "schedule": "fdgs_step_batch: the 4 views on 4 worker streams and workspaces, gradient accumulation chained"},
            "forward_fps": world * 1e3 / ms_frame, "ms_per_frame": ms_frame,
            "e2e": {"value": world * 1e3 / ms_e2e, "unit": "steps/s", "h2d_bytes_per_step": n_views * img_bytes, "d2h_bytes_per_step": n_views * 4,
                    "ms_per_step": ms_e2e},

@@ -130,6 +130,31 @@ int fdgs_step_host(const fdgs_scene *scene, const fdgs_view *view_host, const fd
                    float *target_dev, float *image, float *final_T, uint32_t *n_contrib, float *dL_dimage,
                    float *loss_dev, fdgs_grads *grads_host, float *result_host);
 
+/* One optimisation step over a batch of views ("batch size 4", batch sampling in time): for every view
+ * preprocess + forward + L1 loss against its target + backward, gradients of all views accumulated into `grads_host`
+ * (+=; the caller zeroes them).  The views run on library-owned worker streams forked from and joined to `cuda_stream`
+ * by events, each on its OWN workspace and buffers, so the latency-bound stages of one view (scans, sorts) overlap the
+ * blend kernels of the others; only the gradient accumulation into the shared arrays (second half of the backward) is
+ * chained view after view, because it is a non-atomic read-modify-write.  The accumulated result is the same as calling
+ * the three functions view by view, up to fp32 summation order of the blend atomics.
+ *   bufs_host[i].target_host  != NULL: [3,H,W] pinned host image, copied to target_dev inside the call;
+ *                             == NULL: target_dev already holds the target.
+ *   loss_dev [num_views] device floats: loss of each view (overwritten).
+ *   loss_host != NULL: the losses are copied back and `cuda_stream` is synchronised; NULL: fully asynchronous.
+ * 1 <= num_views <= FDGS_MAX_BATCH; workspaces must be distinct. */
+#define FDGS_MAX_BATCH 8
+typedef struct {
+  void *ws; size_t ws_bytes;     /* workspace of this view (fdgs_workspace_bytes)                      */
+  const float *target_host;      /* see above                                                          */
+  float *target_dev;             /* [3,H,W]                                                            */
+  float *image, *final_T;        /* [3,H,W], [H,W] outputs of the forward                              */
+  uint32_t *n_contrib;           /* [H,W]                                                              */
+  float *dL_dimage;              /* [3,H,W] scratch: dL/dimage of the L1 loss                          */
+} fdgs_view_buffers;
+int fdgs_step_batch(const fdgs_scene *scene, const fdgs_view *views_host, int32_t num_views, const fdgs_config *cfg_host,
+                    int64_t pair_capacity, const fdgs_view_buffers *bufs_host, void *cuda_stream, float *loss_dev,
+                    const fdgs_grads *grads_host, float *loss_host);
+
 /* Parity hooks: copy one intermediate of the last calls on `ws` to dst (device memory).  Synchronises. */
 #define FDGS_EXPORT_STATUS 0        /* int64[4]: D, num_visible, overflow flag, pair_capacity               */
 #define FDGS_EXPORT_RECORDS 1       /* float[N,12]: u, v, conic A, B, C, opacity o, r, g, b, depth, radius, w */

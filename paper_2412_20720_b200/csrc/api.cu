@@ -190,9 +190,13 @@ int fdgs_render_forward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_con
   return forward_impl(sc, vp, cp, ws, cap, (cudaStream_t)stream, image, final_T, n_contrib, &l1, &l2);
 }
 
-int fdgs_render_backward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
-                         int64_t cap, void* stream, const float* dL_dimage, const float* final_T, const uint32_t* n_contrib,
-                         const fdgs_grads* g) {
+}  // extern "C"
+
+// B1 + B2.  `before_b2` (optional): an event the stream waits for between the two — fdgs_step_batch uses it to order the
+// non-atomic gradient read-modify-writes of concurrent views while their blend kernels overlap.
+static int backward_impl(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes, int64_t cap,
+                         cudaStream_t st, const float* dL_dimage, const float* final_T, const uint32_t* n_contrib,
+                         const fdgs_grads* g, cudaEvent_t before_b2) {
   int rc = check_common(sc, v, c, ws_ptr);
   if (rc) return rc;
   if (!dL_dimage || !final_T || !n_contrib || !g || cap < 1 || cap >= (1LL << 30)) return FDGS_ERR_INVALID;
@@ -201,7 +205,6 @@ int fdgs_render_backward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_co
   const int K = sc->n_time * (sc->sh_degree + 1) * (sc->sh_degree + 1);
   const Workspace ws = carve(ws_ptr, sc->N, K, v->width, v->height, cap);
   if (ws.bytes > ws_bytes) return FDGS_ERR_WORKSPACE;
-  cudaStream_t st = (cudaStream_t)stream;
   ViewParams vp; CfgParams cp;
   make_params(v, c, vp, cp);
   int l1, l2;
@@ -210,10 +213,19 @@ int fdgs_render_backward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_co
   mark(EV_BWD0, st);
   launch_blend_bwd(ws, l2, vp, cp, dL_dimage, final_T, n_contrib, st);          // B1
   mark(EV_BWD1, st);
+  if (before_b2) FDGS_CUDA(cudaStreamWaitEvent(st, before_b2, 0), "wait before B2");
   launch_preprocess_bwd(*sc, vp, cp, ws, l1, *g, st);                           // B2
   mark(EV_BWD2, st);
   FDGS_CUDA(cudaGetLastError(), "backward launches");
   return FDGS_OK;
+}
+
+extern "C" {
+
+int fdgs_render_backward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
+                         int64_t cap, void* stream, const float* dL_dimage, const float* final_T, const uint32_t* n_contrib,
+                         const fdgs_grads* g) {
+  return backward_impl(sc, v, c, ws_ptr, ws_bytes, cap, (cudaStream_t)stream, dL_dimage, final_T, n_contrib, g, nullptr);
 }
 
 int fdgs_l1_loss(const float* image, const float* target, int64_t count, float* dL_dimage, float* loss, void* stream) {
@@ -262,6 +274,53 @@ int fdgs_step_host(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* 
     FDGS_CUDA(cudaMemcpyAsync(result_host, image, count * sizeof(float), cudaMemcpyDeviceToHost, st), "D2H image");
   }
   FDGS_CUDA(cudaStreamSynchronize(st), "step sync");
+  return FDGS_OK;
+}
+
+// Worker streams of fdgs_step_batch (one per view of the batch), created on first use.
+static cudaStream_t g_worker[FDGS_MAX_BATCH];
+static cudaEvent_t g_batch_fork = nullptr, g_b2_done[FDGS_MAX_BATCH];
+
+int fdgs_step_batch(const fdgs_scene* sc, const fdgs_view* views, int32_t num_views, const fdgs_config* c, int64_t cap,
+                    const fdgs_view_buffers* bufs, void* stream, float* loss_dev, const fdgs_grads* g, float* loss_host) {
+  if (!sc || !views || !c || !bufs || !loss_dev || !g || num_views < 1 || num_views > FDGS_MAX_BATCH) return FDGS_ERR_INVALID;
+  for (int i = 0; i < num_views; ++i) {
+    const fdgs_view_buffers& b = bufs[i];
+    if (!b.ws || !b.target_dev || !b.image || !b.final_T || !b.n_contrib || !b.dL_dimage) return FDGS_ERR_INVALID;
+    for (int k = 0; k < i; ++k) if (bufs[k].ws == b.ws) return FDGS_ERR_INVALID;      // one workspace per view
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!g_batch_fork) {
+    for (int i = 0; i < FDGS_MAX_BATCH; ++i) {
+      FDGS_CUDA(cudaStreamCreateWithFlags(&g_worker[i], cudaStreamNonBlocking), "worker stream");
+      FDGS_CUDA(cudaEventCreateWithFlags(&g_b2_done[i], cudaEventDisableTiming), "worker event");
+    }
+    FDGS_CUDA(cudaEventCreateWithFlags(&g_batch_fork, cudaEventDisableTiming), "fork event");
+  }
+  FDGS_CUDA(cudaEventRecord(g_batch_fork, st), "fork");
+  for (int i = 0; i < num_views; ++i) {
+    const fdgs_view_buffers& b = bufs[i];
+    cudaStream_t w = g_worker[i];
+    const size_t count = (size_t)3 * views[i].width * views[i].height;
+    FDGS_CUDA(cudaStreamWaitEvent(w, g_batch_fork, 0), "fork wait");
+    if (b.target_host) FDGS_CUDA(cudaMemcpyAsync(b.target_dev, b.target_host, count * sizeof(float), cudaMemcpyHostToDevice, w), "H2D target");
+    FDGS_CUDA(cudaMemsetAsync(loss_dev + i, 0, sizeof(float), w), "memset(loss)");
+    int rc = fdgs_preprocess(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, nullptr, nullptr);
+    if (rc) return rc;
+    rc = fdgs_render_forward(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, b.image, b.final_T, b.n_contrib);
+    if (rc) return rc;
+    rc = fdgs_l1_loss(b.image, b.target_dev, (int64_t)count, b.dL_dimage, loss_dev + i, w);
+    if (rc) return rc;
+    // blend backward of this view overlaps everything of the others; the gradient accumulation (B2) is chained
+    rc = backward_impl(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, b.dL_dimage, b.final_T, b.n_contrib, g, i > 0 ? g_b2_done[i - 1] : nullptr);
+    if (rc) return rc;
+    FDGS_CUDA(cudaEventRecord(g_b2_done[i], w), "record B2");
+  }
+  for (int i = 0; i < num_views; ++i) FDGS_CUDA(cudaStreamWaitEvent(st, g_b2_done[i], 0), "join");
+  if (loss_host) {
+    FDGS_CUDA(cudaMemcpyAsync(loss_host, loss_dev, sizeof(float) * num_views, cudaMemcpyDeviceToHost, st), "D2H loss");
+    FDGS_CUDA(cudaStreamSynchronize(st), "batch sync");
+  }
   return FDGS_OK;
 }
 

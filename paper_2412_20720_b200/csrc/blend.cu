@@ -80,6 +80,9 @@ __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __rest
   }
   const uint2 range = ranges[tile];
   const int n = (int)(range.y - range.x);
+  // thresholds pinned in registers (otherwise each use re-reads the constant bank: an issue slot per use in this loop)
+  float c_l2min = cp.log2_alpha_min, c_amax = cp.alpha_max, c_amin = cp.alpha_min, c_tmin = cp.transmittance_min;
+  asm volatile("" : "+f"(c_l2min), "+f"(c_amax), "+f"(c_amin), "+f"(c_tmin));
   unsigned int st_walk = 0, st_exp = 0, st_comp = 0, st_stage = 0;
   for (int base = 0; base < n; base += BATCH) {
     bool all_done = true;
@@ -102,7 +105,7 @@ __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __rest
 #pragma unroll
       for (int k = 0; k < PX; ++k) {
         if (STATS) hk[k] = jb + 32 <= m ? 0xffffffffu : ((1u << (m - jb)) - 1u);
-        else hk[k] = ((alive >> k) & 1u) ? __ballot_sync(0xffffffffu, jb + lane < m && patch_hit(ta, tb, sp.xm, sp.ym0 + 4.f * k, cp.log2_alpha_min)) : 0u;
+        else hk[k] = ((alive >> k) & 1u) ? __ballot_sync(0xffffffffu, jb + lane < m && patch_hit(ta, tb, sp.xm, sp.ym0 + 4.f * k, c_l2min)) : 0u;
         any |= hk[k];
       }
       while (any) {
@@ -118,12 +121,12 @@ __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __rest
           const float e2 = fmaf(a.z, y[k], b.x);
           const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
           if (STATS && !done[k]) ++st_walk;
-          if (done[k] || l2a < cp.log2_alpha_min) continue;              // alpha < alpha_min: skipped
-          const float alpha = fminf(cp.alpha_max, ex2_approx(l2a));
+          if (done[k] || l2a < c_l2min) continue;              // alpha < alpha_min: skipped
+          const float alpha = fminf(c_amax, ex2_approx(l2a));
           if (STATS) ++st_exp;
-          if (alpha < cp.alpha_min) continue;
+          if (alpha < c_amin) continue;
           const float Tn = fmaf(-T[k], alpha, T[k]);
-          if (Tn < cp.transmittance_min) { done[k] = true; continue; }   // the terminating splat is not composited
+          if (Tn < c_tmin) { done[k] = true; continue; }   // the terminating splat is not composited
           const float wgt = alpha * T[k];
           Cr[k] = fmaf(b.z, wgt, Cr[k]); Cg[k] = fmaf(b.w, wgt, Cg[k]); Cb[k] = fmaf(sm.s2[j].x, wgt, Cb[k]);
           T[k] = Tn;
@@ -436,6 +439,9 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
   if (lane == 0) atomicMax(&sm.max_contrib, lane_max);
   __syncthreads();
   const int total = sm.max_contrib;
+  // thresholds pinned in registers (otherwise each use re-reads the constant bank: an issue slot per use in this loop)
+  float c_l2min = cp.log2_alpha_min, c_amax = cp.alpha_max, c_amin = cp.alpha_min;
+  asm volatile("" : "+f"(c_l2min), "+f"(c_amax), "+f"(c_amin));
   for (int hi = total; hi > 0; hi -= BATCH) {           // batch covers list positions [lo_pos, hi)
     const int lo_pos = max(0, hi - BATCH), m = hi - lo_pos;
     __syncthreads();                                    // previous batch fully flushed
@@ -456,7 +462,7 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
 #pragma unroll
       for (int k = 0; k < PX; ++k) {
         hk[k] = lo_pos + jb < wmax[k] ? __ballot_sync(0xffffffffu, jb + lane < m && lo_pos + jb + lane < wmax[k] &&
-                                                                    patch_hit(ta, tb, sp.xm, sp.ym0 + 4.f * k, cp.log2_alpha_min)) : 0u;
+                                                                    patch_hit(ta, tb, sp.xm, sp.ym0 + 4.f * k, c_l2min)) : 0u;
         any |= hk[k];
       }
       while (any) {
@@ -473,10 +479,10 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
           const float e1 = fmaf(a.y, y[k], e1x);
           const float e2 = fmaf(a.z, y[k], b.x);
           const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
-          if ((lo_pos + j < mine[k]) && !(l2a < cp.log2_alpha_min)) {
+          if ((lo_pos + j < mine[k]) && !(l2a < c_l2min)) {
             araw[k] = ex2_approx(l2a);
-            const float al = fminf(cp.alpha_max, araw[k]);
-            alpha[k] = al < cp.alpha_min ? 0.f : al;
+            const float al = fminf(c_amax, araw[k]);
+            alpha[k] = al < c_amin ? 0.f : al;
           }
         }
         if (!__any_sync(0xffffffffu, alpha[0] > 0.f || alpha[1] > 0.f)) continue;
@@ -491,7 +497,7 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
           const float gc = fmaf(gr[k], b.z, fmaf(gg[k], b.w, gb[k] * cb));   // dL/dpixel . c_k
           const float dalpha = fmaf(Tk, gc, -s[k] * iom);
           s[k] = fmaf(gc, wgt[k], s[k]);
-          dpow[k] = araw[k] > cp.alpha_max ? 0.f : alpha[k] * dalpha;      // alpha clamp active: no gradient through the exponent
+          dpow[k] = araw[k] > c_amax ? 0.f : alpha[k] * dalpha;      // alpha clamp active: no gradient through the exponent
         }
         sm.hit[warp][nbuf][lane] = make_float4(dpow[0], wgt[0], dpow[1], wgt[1]);
         if (lane == 0) sm.hitj[warp][nbuf] = j;

@@ -22,7 +22,8 @@ OK, ERR_INVALID, ERR_WORKSPACE, ERR_CUDA, ERR_PAIR_OVERFLOW = 0, -1, -2, -3, -4
 EXPORTED_SYMBOLS = ["fdgs_default_config", "fdgs_workspace_bytes", "fdgs_preprocess", "fdgs_render_forward",
                     "fdgs_render_backward", "fdgs_l1_loss", "fdgs_step_host", "fdgs_debug_export",
                     "fdgs_launch_count", "fdgs_strerror", "fdgs_set_stage_timing", "fdgs_get_stage_ms",
-                    "fdgs_debug_blend_stats"]
+                    "fdgs_debug_blend_stats", "fdgs_step_batch"]
+MAX_BATCH = 8
 
 
 class CScene(C.Structure):
@@ -44,6 +45,11 @@ class CConfig(C.Structure):
 
 class CGrads(C.Structure):
     _fields_ = [(k, C.c_void_p) for k in ("mean", "log_scale", "quat_l", "quat_r", "opacity_logit", "sh", "mean2d")]
+
+
+class CViewBuffers(C.Structure):
+    _fields_ = [("ws", C.c_void_p), ("ws_bytes", C.c_size_t), ("target_host", C.c_void_p), ("target_dev", C.c_void_p),
+                ("image", C.c_void_p), ("final_T", C.c_void_p), ("n_contrib", C.c_void_p), ("dL_dimage", C.c_void_p)]
 
 
 class FdgsError(RuntimeError):
@@ -72,6 +78,8 @@ def load():
     lib.fdgs_l1_loss.argtypes = [vp, vp, i64, vp, vp, vp]
     lib.fdgs_step_host.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, vp, vp, vp, vp,
                                    vp, vp, vp, C.POINTER(CGrads), vp]
+    lib.fdgs_step_batch.argtypes = [C.POINTER(CScene), C.POINTER(CView), i32, C.POINTER(CConfig), i64, C.POINTER(CViewBuffers), vp, vp,
+                                    C.POINTER(CGrads), vp]
     lib.fdgs_debug_export.argtypes = [vp, sz, C.c_int, vp, sz, vp]
     lib.fdgs_set_stage_timing.argtypes = [C.c_int]
     lib.fdgs_get_stage_ms.argtypes = [C.POINTER(C.c_float)]
@@ -300,3 +308,35 @@ class Renderer:
         if rc:
             raise FdgsError(rc, f"fdgs_debug_export({what})")
         return out
+
+
+class BatchStep:
+    """One optimisation step over a batch of views through fdgs_step_batch: one Renderer (workspace + buffers) per view."""
+
+    def __init__(self, dscene: DeviceScene, width: int, height: int, pair_capacity: int, num_views: int, cfg: Optional[CConfig] = None):
+        import torch
+        if not 1 <= num_views <= MAX_BATCH:
+            raise ValueError(f"num_views must be in 1..{MAX_BATCH}")
+        self.lib = load()
+        self.ds, self.cap, self.num_views = dscene, int(pair_capacity), int(num_views)
+        self.renderers = [Renderer(dscene, width, height, pair_capacity, cfg) for _ in range(num_views)]
+        self.cfg = self.renderers[0].cfg
+        self.loss = torch.zeros(num_views, dtype=torch.float32, device=dscene.mean.device)
+        self._cs = dscene.c_struct()
+
+    def step(self, cviews, grads: dict, targets_host=None, loss_host=None):
+        """targets_host: list of pinned [3,H,W] host tensors (copied inside the call) or None if every renderer's
+        target_dev already holds its target.  loss_host: pinned float tensor [num_views] (copied back, synchronises)
+        or None (asynchronous)."""
+        n = self.num_views
+        views = (CView * n)(*cviews)
+        bufs = (CViewBuffers * n)()
+        for i, r in enumerate(self.renderers):
+            bufs[i] = CViewBuffers(r.ws.data_ptr(), r.ws_bytes, _ptr(targets_host[i]) if targets_host is not None else None,
+                                   r.target_dev.data_ptr(), r.image.data_ptr(), r.final_T.data_ptr(), r.n_contrib.data_ptr(),
+                                   r.dL_dimage.data_ptr())
+        cg = grads_struct(grads)
+        rc = self.lib.fdgs_step_batch(C.byref(self._cs), views, n, C.byref(self.cfg), self.cap, bufs, _stream(), self.loss.data_ptr(),
+                                      C.byref(cg), _ptr(loss_host))
+        if rc:
+            raise FdgsError(rc, "fdgs_step_batch")

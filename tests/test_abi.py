@@ -61,6 +61,7 @@ def test_struct_layouts_match_the_header():
     assert C.sizeof(fdgs.CView) == 64 + 16 + 8 + 8 + 12
     assert C.sizeof(fdgs.CConfig) == 32
     assert C.sizeof(fdgs.CGrads) == 56
+    assert C.sizeof(fdgs.CViewBuffers) == 64
 
 
 def test_product_fails_loudly_without_the_library(monkeypatch):

@@ -128,3 +128,17 @@ def test_cfg3_full_one_view():
     sc = scenes.multiview_video(n_views=1)
     rep, gpu, o = _full_parity(sc, dL_mode="l1", label="cfg3 1M 1352x1014 view0")
     assert rep["num_pairs_gpu"] > 1_000_000
+
+
+@pytest.mark.parametrize("env", [{"FDGS_BLEND_PX": "1"}, {"FDGS_BLEND_PX": "4"}, {"FDGS_BLEND_DIRECT": "1"}])
+def test_blend_kernel_variants_in_a_fresh_process(env):
+    """The PX = 1 / 4 strips and the direct (shuffle-reduction) backward are selected by environment variables read once
+    per process: run the ragged cfg2 parity case in a child process for each."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-m", "pytest", os.path.join(root, "tests", "test_gpu_parity.py"), "-m", "gpu", "-q", "-x",
+                        "-k", "cfg2_reduced_and_ragged or cfg1_tiny"], env=dict(os.environ, **env), capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+    assert "2 passed" in r.stdout
