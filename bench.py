@@ -236,6 +236,28 @@ def run_fdgs(args):
         m, _ = timed(lambda: forward_only(cv), 25, 5)
         fps_ms.append(m)
     ms_frame = sum(fps_ms) / len(fps_ms)
+    # ---- playback throughput: consecutive frames in flight on separate streams / workspaces (cfg5-style free-viewpoint
+    # video): the scans and sorts of frame k+1 overlap the blend of frame k -------------------------------
+    streams = [torch.cuda.Stream() for _ in range(n_views)]
+    n_frames = 40
+
+    def playback():
+        main = torch.cuda.current_stream()
+        ev = torch.cuda.Event()
+        ev.record(main)
+        for k in range(n_frames):
+            s_, rr = streams[k % n_views], bs.renderers[k % n_views]
+            s_.wait_event(ev)
+            with torch.cuda.stream(s_):
+                rr.preprocess(cviews[k % n_views])
+                rr.forward(cviews[k % n_views])
+        for s_ in streams:
+            e = torch.cuda.Event()
+            e.record(s_)
+            main.wait_event(e)
+
+    ms_playback, _ = timed(playback, 5, 3)
+    ms_frame_pipelined = ms_playback / n_frames
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -289,6 +311,7 @@ def run_fdgs(args):
                       "multi_gpu": "replicas only",
                       "schedule": "fdgs_step_batch: the 4 views on 4 worker streams and workspaces, gradient accumulation chained"},
            "forward_fps": world * 1e3 / ms_frame, "ms_per_frame": ms_frame,
+           "forward_fps_pipelined": world * 1e3 / ms_frame_pipelined, "ms_per_frame_pipelined": ms_frame_pipelined,
            "e2e": {"value": world * 1e3 / ms_e2e, "unit": "steps/s", "h2d_bytes_per_step": n_views * img_bytes, "d2h_bytes_per_step": n_views * 4,
                    "ms_per_step": ms_e2e},
            "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,

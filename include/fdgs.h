@@ -179,6 +179,12 @@ int fdgs_get_stage_ms(float *ms_host);
 int fdgs_debug_blend_stats(const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws, size_t ws_bytes, int32_t N,
                            int32_t K, int64_t pair_capacity, void *cuda_stream, unsigned long long *stats_dev);
 
+/* Cull decision of every primitive for this view, uint8[N]: 0 visible, 1 culled by the temporal marginal (L324),
+ * 2 behind the near plane, 3 empty tile rectangle, 4 non-finite.  Recomputed from the parameters (does not touch a
+ * workspace): parity of the cull reasons, and cfg5's "fraction culled by the marginal temporal weight". */
+int fdgs_debug_cull_status(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *cuda_stream,
+                           unsigned char *status_dev);
+
 /* Number of kernel launches the library has issued so far in this process (bench.py's gpu_launches). */
 int64_t fdgs_launch_count(void);
 

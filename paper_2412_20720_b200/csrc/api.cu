@@ -361,6 +361,15 @@ int fdgs_debug_blend_stats(const fdgs_view* v, const fdgs_config* c, void* ws_pt
   return FDGS_OK;
 }
 
+int fdgs_debug_cull_status(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* stream, unsigned char* status_dev) {
+  if (!sc || !v || !c || !status_dev || sc->N < 0 || v->width <= 0 || v->height <= 0 || !(v->period_T > 0)) return FDGS_ERR_INVALID;
+  ViewParams vp; CfgParams cp;
+  make_params(v, c, vp, cp);
+  launch_cull_status(*sc, vp, cp, status_dev, (cudaStream_t)stream);
+  FDGS_CUDA(cudaGetLastError(), "cull status launch");
+  return FDGS_OK;
+}
+
 const char* fdgs_strerror(int code) {
   switch (code) {
     case FDGS_OK: return "ok";

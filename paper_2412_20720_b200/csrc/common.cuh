@@ -159,6 +159,7 @@ void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, con
                       const float* final_T, const unsigned int* n_contrib, cudaStream_t st);
 void launch_preprocess_bwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, int l1_buf,
                            const fdgs_grads& g, cudaStream_t st);
+void launch_cull_status(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, unsigned char* dst, cudaStream_t st);
 void launch_l1_loss(const float* image, const float* target, long long count, float* dL, float* loss, cudaStream_t st);
 void launch_export_records(const Workspace& ws, int N, float* dst, cudaStream_t st);
 void launch_export_keys(const Workspace& ws, int l2_buf, unsigned long long* dst, cudaStream_t st);

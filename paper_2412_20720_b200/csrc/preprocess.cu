@@ -115,6 +115,30 @@ __global__ void __launch_bounds__(128) preprocess_fwd_kernel(const fdgs_scene sc
   dst[2] = make_float4(r.b, r.depth, r.radius, r.w);
 }
 
+// Parity / measurement hook: the cull decision of every primitive (GeomStatus; 3 = empty tile rectangle), recomputed
+// from the parameters with the same device functions as the forward.
+__global__ void cull_status_kernel(const fdgs_scene sc, const ViewParams vp, const CfgParams cp, unsigned char* __restrict__ dst) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= sc.N) return;
+  Geom g;
+  int st = geom_forward(ldg4(sc.mean, i), ldg4(sc.log_scale, i), ldg4(sc.quat_l, i), ldg4(sc.quat_r, i), __ldg(sc.opacity_logit + i), vp, cp, g);
+  if (st == G_VISIBLE) {
+    const float mid = 0.5f * (g.a2 + g.c2), hd = 0.5f * (g.a2 - g.c2);
+    const float radius = cp.cutoff_sigma * sqrtf(mid + sqrtf(fmaxf(0.f, fmaf(hd, hd, g.b2 * g.b2))));
+    const float inv = 1.0f / TILE;
+    const int tx0 = min(max((int)floorf((g.u - radius) * inv), 0), vp.tiles_x), ty0 = min(max((int)floorf((g.v - radius) * inv), 0), vp.tiles_y);
+    const int tx1 = min(max((int)ceilf((g.u + radius) * inv), 0), vp.tiles_x), ty1 = min(max((int)ceilf((g.v + radius) * inv), 0), vp.tiles_y);
+    if (!(isfinite(g.u) && isfinite(g.v) && isfinite(radius) && tx1 > tx0 && ty1 > ty0)) st = G_CULL_RECT;
+  }
+  dst[i] = (unsigned char)st;
+}
+
+void launch_cull_status(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, unsigned char* dst, cudaStream_t st) {
+  if (sc.N <= 0) return;
+  cull_status_kernel<<<(sc.N + 127) / 128, 128, 0, st>>>(sc, vp, cp, dst);
+  ++g_launches;
+}
+
 void launch_preprocess_fwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, cudaStream_t st) {
   if (sc.N <= 0) return;
   const int threads = 128, blocks = (sc.N + threads - 1) / threads;

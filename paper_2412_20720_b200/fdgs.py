@@ -22,7 +22,7 @@ OK, ERR_INVALID, ERR_WORKSPACE, ERR_CUDA, ERR_PAIR_OVERFLOW = 0, -1, -2, -3, -4
 EXPORTED_SYMBOLS = ["fdgs_default_config", "fdgs_workspace_bytes", "fdgs_preprocess", "fdgs_render_forward",
                     "fdgs_render_backward", "fdgs_l1_loss", "fdgs_step_host", "fdgs_debug_export",
                     "fdgs_launch_count", "fdgs_strerror", "fdgs_set_stage_timing", "fdgs_get_stage_ms",
-                    "fdgs_debug_blend_stats", "fdgs_step_batch"]
+                    "fdgs_debug_blend_stats", "fdgs_step_batch", "fdgs_debug_cull_status"]
 MAX_BATCH = 8
 
 
@@ -80,6 +80,7 @@ def load():
                                    vp, vp, vp, C.POINTER(CGrads), vp]
     lib.fdgs_step_batch.argtypes = [C.POINTER(CScene), C.POINTER(CView), i32, C.POINTER(CConfig), i64, C.POINTER(CViewBuffers), vp, vp,
                                     C.POINTER(CGrads), vp]
+    lib.fdgs_debug_cull_status.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, vp]
     lib.fdgs_debug_export.argtypes = [vp, sz, C.c_int, vp, sz, vp]
     lib.fdgs_set_stage_timing.argtypes = [C.c_int]
     lib.fdgs_get_stage_ms.argtypes = [C.POINTER(C.c_float)]
@@ -279,6 +280,15 @@ class Renderer:
         if rc:
             raise FdgsError(rc, "fdgs_debug_blend_stats")
         return [int(x) for x in out.cpu()]
+
+    def cull_status(self, cview: CView):
+        """uint8[N]: 0 visible, 1 temporal marginal, 2 near plane, 3 empty rectangle, 4 non-finite."""
+        import torch
+        out = torch.zeros(max(self.ds.N, 1), dtype=torch.uint8, device=self.ws.device)
+        rc = self.lib.fdgs_debug_cull_status(C.byref(self._cs), C.byref(cview), C.byref(self.cfg), _stream(), out.data_ptr())
+        if rc:
+            raise FdgsError(rc, "fdgs_debug_cull_status")
+        return out[:self.ds.N]
 
     # -- parity hooks -----------------------------------------------------------------------------
     def export(self, what: int):

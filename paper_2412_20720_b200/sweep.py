@@ -1,0 +1,124 @@
+"""Secondary measurements of BASELINE.json's configs 2, 4 and 5 (bench.py times the headline config 3).
+
+    python -m paper_2412_20720_b200.sweep [--frames 24] [--max-n 8000000] [--skip-train]
+
+cfg5: forward-only render throughput over Gaussian count x resolution at evenly spaced query times: FPS (one frame at a
+time), per-stage ms (preprocess / sort incl. compaction, duplication and ranges / blend) and the fraction culled by the
+marginal temporal weight.  cfg2 / cfg4: forward+backward steps/s of their batch through fdgs_step_batch.
+One JSON line per measurement on stdout.  Synthetic seeded scenes (scenes.py); no CPU fallback.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+
+import numpy as np
+
+
+def _timed(fn, iters, warm, flush):
+    import torch
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    tot = 0.0
+    for _ in range(iters):
+        flush.fill_(1)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        fn()
+        e1.record()
+        torch.cuda.synchronize()
+        tot += e0.elapsed_time(e1)
+    return tot / iters
+
+
+def sweep_cfg5(frames, max_n, flush):
+    import torch
+    from . import fdgs, scenes
+    for (w, h) in ((1352, 1014), (1920, 1080)):
+        for n in (100_000, 500_000, 1_000_000, 2_000_000, 4_000_000, 8_000_000):
+            if n > max_n:
+                continue
+            sc = scenes.sweep(N=n, width=w, height=h, n_frames=120)
+            ds = fdgs.DeviceScene.from_scene(sc)
+            cap = max(1 << 22, 16 * n)
+            r = fdgs.Renderer(ds, w, h, cap)
+            idx = np.linspace(0, 119, frames).round().astype(int)
+            cvs = [fdgs.make_view(sc.views[i]) for i in idx]
+            ms, culled, pairs, nvis = [], [], [], []
+            fdgs.set_stage_timing(True)
+            stage = {k: 0.0 for k in fdgs.STAGES[:6]}
+            for cv in cvs:
+                def frame():
+                    r.preprocess(cv)
+                    r.forward(cv)
+                ms.append(_timed(frame, 3, 2, flush))
+                for k, v in fdgs.stage_ms().items():
+                    if k in stage:
+                        stage[k] += v / len(cvs)
+                st = r.export(fdgs.EXPORT_STATUS)
+                if st["overflow"]:
+                    raise RuntimeError(f"pair capacity exceeded: {st}")
+                culled.append(float((r.cull_status(cv) == 1).sum().item()) / n)     # culled by the marginal temporal weight
+                pairs.append(st["num_pairs"]); nvis.append(st["num_visible"])
+            fdgs.set_stage_timing(False)
+            ms_frame = float(np.mean(ms))
+            print(json.dumps({"config": "cfg5_sweep", "N": n, "width": w, "height": h, "frames": len(cvs), "fps": 1e3 / ms_frame,
+                              "ms_per_frame": ms_frame, "ms_min": float(np.min(ms)), "ms_max": float(np.max(ms)),
+                              "stage_ms": {"preprocess": stage["preprocess"],
+                                           "sort": stage["compact+tile_grid"] + stage["sort_depth"] + stage["offsets+duplicate"] + stage["sort_tile"],
+                                           "blend": stage["blend_fwd"]},
+                              "culled_by_marginal_fraction": float(np.mean(culled)), "visible_mean": float(np.mean(nvis)),
+                              "pairs_mean": float(np.mean(pairs))}), flush=True)
+            del r, ds, sc
+            torch.cuda.empty_cache()
+
+
+def train_cfg(name, scene, cap, flush):
+    import torch
+    from . import fdgs, scenes
+    ds = fdgs.DeviceScene.from_scene(scene)
+    v0 = scene.views[0]
+    nv = len(scene.views)
+    bs = fdgs.BatchStep(ds, v0.width, v0.height, cap, nv)
+    cvs = [fdgs.make_view(v) for v in scene.views]
+    for i, rr in enumerate(bs.renderers):
+        rr.target_dev.copy_(torch.from_numpy(scenes.target_image(scene.seed, i, v0.width, v0.height)).cuda())
+    grads = ds.zero_grads()
+
+    def step():
+        for g in grads.values():
+            if g is not None:
+                g.zero_()
+        bs.step(cvs, grads)
+    ms = _timed(step, 5, 3, flush)
+    sts = [rr.export(fdgs.EXPORT_STATUS) for rr in bs.renderers]
+    if any(s["overflow"] for s in sts):
+        raise RuntimeError(f"pair capacity exceeded: {sts}")
+    print(json.dumps({"config": name, "N": scene.N, "width": v0.width, "height": v0.height, "views_per_step": nv,
+                      "steps_per_s": 1e3 / ms, "ms_per_step": ms, "pairs_per_view": [s["num_pairs"] for s in sts],
+                      "visible_per_view": [s["num_visible"] for s in sts], "loss": float(bs.loss.sum())}), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--frames", type=int, default=24)
+    ap.add_argument("--max-n", type=int, default=8_000_000)
+    ap.add_argument("--skip-train", action="store_true")
+    ap.add_argument("--skip-sweep", action="store_true")
+    args = ap.parse_args()
+    import torch
+    from . import build, scenes
+    if not torch.cuda.is_available():
+        raise RuntimeError("sweep needs a CUDA device: the product has no CPU fallback")
+    build.build()
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+    if not args.skip_train:
+        train_cfg("cfg2_object", scenes.single_object(), 1 << 22, flush)
+        train_cfg("cfg4_driving", scenes.driving(), 160 * 1024 * 1024, flush)
+    if not args.skip_sweep:
+        sweep_cfg5(args.frames, args.max_n, flush)
+
+
+if __name__ == "__main__":
+    main()

@@ -27,7 +27,8 @@ def gpu_run(scene, view, cfg_overrides=None, pair_capacity=None, dL=None, with_m
                rects=r.export(fdgs.EXPORT_RECTS).cpu().numpy(), ranges=r.export(fdgs.EXPORT_RANGES).cpu().numpy(),
                sorted_vals=r.export(fdgs.EXPORT_SORTED_VALS).cpu().numpy(),
                sorted_keys=r.export(fdgs.EXPORT_SORTED_KEYS).cpu().numpy(),
-               tiles_touched=r.export(fdgs.EXPORT_TILES_TOUCHED).cpu().numpy(), status=r.export(fdgs.EXPORT_STATUS))
+               tiles_touched=r.export(fdgs.EXPORT_TILES_TOUCHED).cpu().numpy(), status=r.export(fdgs.EXPORT_STATUS),
+               cull_status=r.cull_status(cv).cpu().numpy())
     if dL is not None:
         g = ds.zero_grads(with_mean2d=with_mean2d)
         r.backward(cv, torch.from_numpy(np.ascontiguousarray(dL, dtype=np.float32)).cuda(), g)
@@ -46,6 +47,9 @@ def compare_prims(gpu, P, report):
     bad = (vis_o != vis_g) & ~fragile
     report["cull_mismatch_fragile"] = int(((vis_o != vis_g) & fragile).sum())
     assert bad.sum() == 0, f"{bad.sum()} non-fragile primitives with different cull decisions"
+    # the REASON of the cull (temporal marginal / near plane / empty rectangle / non-finite) agrees as well
+    assert (gpu["cull_status"][~fragile] == P.status[~fragile]).all()
+    assert ((gpu["cull_status"] == 0) == vis_g).all()
     both = vis_o & vis_g
     rec = gpu["records"][both]
     rel = lambda a, b, absol=0.0: np.abs(a - b) / (np.abs(b) + absol)
