@@ -61,6 +61,8 @@ def _load():
     lib.fdgs_oracle_sh_basis.argtypes = [C.c_int, dp, dp]
     lib.fdgs_oracle_forward.argtypes = [C.c_void_p, dp, dp, ip, dp]
     lib.fdgs_oracle_backward.argtypes = [C.c_void_p, dp] + [dp] * 8
+    lib.fdgs_oracle_get_depth_map.argtypes = [C.c_void_p, dp]
+    lib.fdgs_oracle_backward_aux.argtypes = [C.c_void_p, dp, dp, dp] + [dp] * 9
     lib.fdgs_oracle_num_threads.restype = C.c_int
     _lib = lib
     return lib
@@ -181,14 +183,29 @@ class Oracle:
         _load().fdgs_oracle_forward(self._h, _d(img), _d(fT), nc.ctypes.data_as(C.POINTER(C.c_int32)), _d(mg))
         return img, fT, nc, mg
 
-    def backward(self, dL_dimage):
-        """Requires forward().  Returns a dict of gradient arrays (float64) incl. 'mean2d' and 'g9'."""
+    def depth_map(self):
+        """Requires forward().  Auxiliary channel: rendered depth sum_k z_k alpha_k T_k, [H,W]."""
+        out = np.zeros((self.height, self.width))
+        _load().fdgs_oracle_get_depth_map(self._h, _d(out))
+        return out
+
+    def backward(self, dL_dimage, dL_ddepth=None, dL_dopacity=None):
+        """Requires forward().  Returns a dict of gradient arrays (float64) incl. 'mean2d', 'g9' and 'gz'.
+        dL_ddepth / dL_dopacity [H,W]: upstream gradients of the auxiliary depth map and of O = 1 - final_T."""
         g = np.ascontiguousarray(np.asarray(dL_dimage, dtype=np.float64))
         assert g.shape == (3, self.height, self.width)
+        aux = []
+        for a in (dL_ddepth, dL_dopacity):
+            if a is not None:
+                a = np.ascontiguousarray(np.asarray(a, dtype=np.float64))
+                assert a.shape == (self.height, self.width)
+            aux.append(a)
         out = dict(mean=np.zeros((self.N, 4)), log_scale=np.zeros((self.N, 4)), quat_l=np.zeros((self.N, 4)),
                    quat_r=np.zeros((self.N, 4)), opacity_logit=np.zeros(self.N), sh=np.zeros((self.N, self.K, 3)),
-                   mean2d=np.zeros((self.N, 2)), g9=np.zeros((self.N, 9)))
-        _load().fdgs_oracle_backward(self._h, _d(g), _d(out["mean"]), _d(out["log_scale"]), _d(out["quat_l"]),
-                                     _d(out["quat_r"]), _d(out["opacity_logit"]), _d(out["sh"]), _d(out["mean2d"]),
-                                     _d(out["g9"]))
+                   mean2d=np.zeros((self.N, 2)), g9=np.zeros((self.N, 9)), gz=np.zeros(self.N))
+        null = C.POINTER(C.c_double)()
+        _load().fdgs_oracle_backward_aux(self._h, _d(g), _d(aux[0]) if aux[0] is not None else null,
+                                         _d(aux[1]) if aux[1] is not None else null, _d(out["mean"]), _d(out["log_scale"]),
+                                         _d(out["quat_l"]), _d(out["quat_r"]), _d(out["opacity_logit"]), _d(out["sh"]),
+                                         _d(out["mean2d"]), _d(out["g9"]), _d(out["gz"]))
         return out

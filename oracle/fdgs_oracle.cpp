@@ -85,9 +85,11 @@ struct Oracle {
   std::vector<int32_t> tile_ids;   // [D] primitive ids, per tile sorted by (depth32 bits, id)
   // forward products
   std::vector<double> image, final_T, margin;
+  std::vector<double> depth_map;   // auxiliary channel: rendered depth sum_k z_k alpha_k T_k (eq. 29, DESIGN S18)
   std::vector<int32_t> n_contrib;
   // per-splat gradients from the blend backward: g_u,g_v,g_A,g_B,g_C,g_o,g_r,g_g,g_b
   std::vector<double> g9;
+  std::vector<double> gz;          // per-splat dL/d(camera depth z_k) from the auxiliary depth channel
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -334,12 +336,13 @@ void forward(Oracle& O) {
   const int W = V.width, H = V.height;
   O.image.assign((size_t)3 * W * H, 0); O.final_T.assign((size_t)W * H, 1);
   O.margin.assign((size_t)W * H, 1e300); O.n_contrib.assign((size_t)W * H, 0);
+  O.depth_map.assign((size_t)W * H, 0);
 #pragma omp parallel for schedule(dynamic, 1)
   for (int tl = 0; tl < O.tiles_x * O.tiles_y; ++tl) {
     const int tx = tl % O.tiles_x, ty = tl / O.tiles_x;
     for (int py = ty * TILE; py < std::min(H, (ty + 1) * TILE); ++py)
       for (int px = tx * TILE; px < std::min(W, (tx + 1) * TILE); ++px) {
-        double T = 1, C[3] = {0, 0, 0}, marg = 1e300;
+        double T = 1, C[3] = {0, 0, 0}, Dz = 0, marg = 1e300;
         int last = 0;
         for (int64_t k = O.tile_off[tl]; k < O.tile_off[tl + 1]; ++k) {   // front to back (eq. 6)
           const Prim& P = O.prims[O.tile_ids[k]];
@@ -351,12 +354,13 @@ void forward(Oracle& O) {
           if (c.transmittance_min > 0) marg = std::min(marg, rel_margin(Tn, c.transmittance_min));
           if (Tn < c.transmittance_min) break;           // the terminating splat does not contribute (S14)
           for (int ch = 0; ch < 3; ++ch) C[ch] += P.rgb[ch] * alpha * T;
+          Dz += P.p[2] * alpha * T;                        // depth is composited like a colour channel, no background
           T = Tn;
           last = (int)(k - O.tile_off[tl]) + 1;
         }
         const size_t pix = (size_t)py * W + px;
         for (int ch = 0; ch < 3; ++ch) O.image[(size_t)ch * W * H + pix] = C[ch] + T * V.bg[ch];
-        O.final_T[pix] = T; O.n_contrib[pix] = last; O.margin[pix] = marg;
+        O.final_T[pix] = T; O.n_contrib[pix] = last; O.margin[pix] = marg; O.depth_map[pix] = Dz;
       }
   }
 }
@@ -369,10 +373,15 @@ inline void add(double& dst, double v) {
 // Reverse-order gradient of the blend (VJP of eq. 6 with the truncations of forward()).
 // For contributors k = 1..m, T_k = prod_{j<k}(1-alpha_j), out = sum c_k alpha_k T_k + T_{m+1} bg:
 //   dL/dc_k = alpha_k T_k g;   dL/dalpha_k = g . (T_k c_k - S_k / (1 - alpha_k)),  S_k = everything behind k.
-void backward_blend(Oracle& O, const double* dL_dimage) {
+// Auxiliary channels (eq. 25, L256 eq. 29): depth D = sum_k z_k alpha_k T_k and accumulated opacity
+// O_gs = sum_k alpha_k T_k = 1 - T_{m+1}.  With upstream gD = dL/dD and gO = dL/dO_gs (either may be NULL):
+//   dL/dz_k += gD alpha_k T_k;   dL/dalpha_k += gD (T_k z_k - Sz_k / (1 - alpha_k)) + gO T_{m+1} / (1 - alpha_k),
+// Sz_k = depth accumulated behind k (no background term).
+void backward_blend(Oracle& O, const double* dL_dimage, const double* dL_ddepth = nullptr, const double* dL_dopacity = nullptr) {
   const View& V = O.view; const Cfg& c = O.cfg;
   const int W = V.width, H = V.height;
   O.g9.assign((size_t)O.N * 9, 0);
+  O.gz.assign((size_t)O.N, 0);
   const int tiles = O.tiles_x * O.tiles_y;
   std::vector<double>& acc = O.g9;
 #pragma omp parallel
@@ -385,6 +394,8 @@ void backward_blend(Oracle& O, const double* dL_dimage) {
           const size_t pix = (size_t)py * W + px;
           const double g[3] = {dL_dimage[pix], dL_dimage[(size_t)W * H + pix], dL_dimage[(size_t)2 * W * H + pix]};
           double T = O.final_T[pix];
+          const double T_final = T, gD = dL_ddepth ? dL_ddepth[pix] : 0.0, gO = dL_dopacity ? dL_dopacity[pix] : 0.0;
+          double Sz = 0;
           double S[3] = {T * V.bg[0], T * V.bg[1], T * V.bg[2]};   // S_m = T_{m+1} bg
           for (int64_t k = O.tile_off[tl] + O.n_contrib[pix] - 1; k >= O.tile_off[tl]; --k) {
             const int id = O.tile_ids[k];
@@ -399,6 +410,9 @@ void backward_blend(Oracle& O, const double* dL_dimage) {
               dalpha += g[ch] * (T * P.rgb[ch] - S[ch] / (1 - alpha));
               S[ch] += P.rgb[ch] * alpha * T;                         // S_{k-1}
             }
+            add(O.gz[id], gD * alpha * T);
+            dalpha += gD * (T * P.p[2] - Sz / (1 - alpha)) + gO * T_final / (1 - alpha);
+            Sz += P.p[2] * alpha * T;
             if (ac) continue;                                         // alpha clamped at alpha_max: zero slope (S16)
             add(a9[5], G * dalpha);                                     // d alpha / d o = G
             if (pc) continue;                                         // power clamped at 0: zero slope (S10)
@@ -417,7 +431,7 @@ void backward_blend(Oracle& O, const double* dL_dimage) {
 // VJP of preprocess_one for a visible primitive (chain of Appendix D of SURVEY.md re-derived in DESIGN.md;
 // finite differences in tests/ are the authority).  Accumulates (+=) into the gradient arrays.
 void backward_one(const Oracle& O, int i, const double g9[9], double* d_mean, double* d_ls, double* d_ql,
-                  double* d_qr, double* d_logit, double* d_sh, double* d_mean2d) {
+                  double* d_qr, double* d_logit, double* d_sh, double* d_mean2d, const double g_z = 0.0) {
   const Prim& P = O.prims[i]; const View& V = O.view; const Cfg& c = O.cfg;
   if (P.status != VISIBLE) return;
   const double g_u = g9[0], g_v = g9[1], g_A = g9[2], g_B = g9[3], g_C = g9[4], g_o = g9[5];
@@ -472,6 +486,7 @@ void backward_one(const Oracle& O, int i, const double g9[9], double* d_mean, do
   dp[0] = g_u * V.fx / z;
   dp[1] = g_v * V.fy / z;
   dp[2] = -g_u * V.fx * x / (z * z) - g_v * V.fy * y / (z * z);
+  dp[2] += g_z;                                   // auxiliary depth channel: z_k = p_z directly
   dp[2] += dJ[0][0] * (-V.fx / (z * z)) + dJ[1][1] * (-V.fy / (z * z));
   if (!P.clampx) { dp[0] += dJ[0][2] * (-V.fx / (z * z)); dp[2] += dJ[0][2] * (2 * V.fx * x / (z * z * z)); }
   else           { dp[2] += dJ[0][2] * (V.fx * P.xr / (z * z)); }      // J02 = -fx * xr / z with xr constant
@@ -653,6 +668,26 @@ void fdgs_oracle_backward(void* h, const double* dL_dimage, double* d_mean, doub
 #pragma omp parallel for schedule(static)
   for (int i = 0; i < O.N; ++i)
     backward_one(O, i, &O.g9[(size_t)9 * i], d_mean, d_log_scale, d_quat_l, d_quat_r, d_logit, d_sh, d_mean2d);
+}
+
+// Auxiliary channels.  depth_map[H,W] of the last fdgs_oracle_forward.
+void fdgs_oracle_get_depth_map(void* h, double* depth_map) {
+  Oracle& O = *(Oracle*)h;
+  std::copy(O.depth_map.begin(), O.depth_map.end(), depth_map);
+}
+
+// fdgs_oracle_backward with upstream gradients of the auxiliary channels as well: dL_ddepth[H,W], dL_dopacity[H,W]
+// (either may be NULL).  gz[N] (may be NULL) receives the per-splat dL/dz.
+void fdgs_oracle_backward_aux(void* h, const double* dL_dimage, const double* dL_ddepth, const double* dL_dopacity,
+                              double* d_mean, double* d_log_scale, double* d_quat_l, double* d_quat_r, double* d_logit,
+                              double* d_sh, double* d_mean2d, double* g9, double* gz) {
+  Oracle& O = *(Oracle*)h;
+  backward_blend(O, dL_dimage, dL_ddepth, dL_dopacity);
+  if (g9) std::copy(O.g9.begin(), O.g9.end(), g9);
+  if (gz) std::copy(O.gz.begin(), O.gz.end(), gz);
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < O.N; ++i)
+    backward_one(O, i, &O.g9[(size_t)9 * i], d_mean, d_log_scale, d_quat_l, d_quat_r, d_logit, d_sh, d_mean2d, O.gz[i]);
 }
 
 int fdgs_oracle_num_threads(void) {

@@ -1,0 +1,100 @@
+"""Pins of the oracle's auxiliary channels: rendered depth D = sum_k z_k alpha_k T_k (PAPER.md:L256,
+eq. 29 "rendered depth") and accumulated opacity O_gs = 1 - T_final (L233, eq. 25), forward and backward."""
+import numpy as np
+import pytest
+
+import oracle
+from helpers import hand_scene, oracle_for, rel_l2
+from paper_2412_20720_b200 import scenes
+
+PARAMS = ("mean", "log_scale", "quat_l", "quat_r", "opacity_logit", "sh")
+
+
+def test_single_splat_depth_is_z_times_alpha_and_opacity_is_alpha():
+    # isotropic splat on the optical axis at camera depth 4 + 1 = 5 (camera at z = -4, splat at z = +1)
+    sc = hand_scene([(0, 0, 1.0, 0.5)], [[-1.0] * 4], logit=[0.3])
+    o = oracle_for(sc)
+    img, fT, nc, _ = o.forward()
+    P = o.prims()
+    D = o.depth_map()
+    alpha = 1.0 - fT                               # one splat: O = alpha
+    assert abs(P.p_cam[0, 2] - 5.0) < 1e-12
+    np.testing.assert_allclose(D, 5.0 * alpha, rtol=0, atol=1e-13)
+    assert D.max() > 1.0 and alpha.max() < 0.99
+
+
+def test_two_layer_depth_is_the_over_composite_of_depths():
+    # two concentric splats at depths 4.5 and 6: D = z1 a1 + z2 a2 (1 - a1), O = a1 + a2 (1 - a1)
+    sc = hand_scene([(0, 0, 0.5, 0.5), (0, 0, 2.0, 0.5)], [[-0.5] * 4, [-0.3] * 4], logit=[-0.5, 0.8])
+    o = oracle_for(sc, cfg=dict(oracle.PURE_CFG))
+    img, fT, nc, _ = o.forward()
+    D = o.depth_map()
+    singles = []
+    for i in range(2):
+        oi = oracle_for(sc.subset([i]), cfg=dict(oracle.PURE_CFG))
+        _, fTi, _, _ = oi.forward()
+        singles.append(1.0 - fTi)
+    a1, a2 = singles
+    np.testing.assert_allclose(D, 4.5 * a1 + 6.0 * a2 * (1 - a1), atol=1e-12)
+    np.testing.assert_allclose(1 - fT, a1 + a2 * (1 - a1), atol=1e-12)
+
+
+def test_depth_does_not_change_colour_path():
+    sc = scenes.tiny()
+    o = oracle_for(sc)
+    o.forward()
+    G = scenes.upstream_normal(0, 64, 64).astype(np.float64)
+    g0 = o.backward(G)
+    g1 = o.backward(G, dL_ddepth=np.zeros((64, 64)), dL_dopacity=np.zeros((64, 64)))
+    for k in PARAMS:
+        assert np.array_equal(g0[k], g1[k])
+    assert np.abs(g1["gz"]).max() == 0
+
+
+def _loss(sc, G, GD, GO, cfg):
+    o = oracle_for(sc, cfg=cfg)
+    img, fT, nc, mg = o.forward()
+    return float((img * G).sum() + (o.depth_map() * GD).sum() + ((1 - fT) * GO).sum()), o, nc, mg
+
+
+@pytest.mark.parametrize("mode", ["default", "pure"])
+def test_aux_backward_matches_central_differences(mode):
+    cfg = dict(oracle.DEFAULT_CFG) if mode == "default" else dict(oracle.PURE_CFG)
+    for seed in range(100, 120):
+        sc = scenes.fd_scene(seed, 6)
+        for k in PARAMS:
+            setattr(sc, k, getattr(sc, k).astype(np.float64))
+        G = 0.3 * scenes.upstream_normal(seed, 64, 64).astype(np.float64)
+        GD = scenes.normal(seed, 210, 64 * 64).reshape(64, 64)
+        GO = scenes.normal(seed, 211, 64 * 64).reshape(64, 64)
+        L0, o0, nc0, mg0 = _loss(sc, G, GD, GO, cfg)
+        p0 = o0.prims()
+        if not (p0.status == 0).all():
+            continue
+        if not cfg.get("full_support") and (mg0.min() < 1e-4 or p0.fragility.min() < 1e-4):
+            continue
+        grads = o0.backward(G, GD, GO)
+        lists0 = o0.tile_lists()
+        for name in PARAMS:
+            arr = getattr(sc, name)
+            fd = np.zeros_like(arr)
+            it = np.nditer(arr, flags=["multi_index"])
+            for x in it:
+                idx = it.multi_index
+                x0 = float(x)
+                h = 1e-6 * max(1.0, abs(x0))
+                vals = []
+                for sgn in (+1, -1):
+                    arr[idx] = x0 + sgn * h
+                    Lp, op, ncp, _ = _loss(sc, G, GD, GO, cfg)
+                    assert np.array_equal(ncp, nc0) and np.array_equal(op.tile_lists()[1], lists0[1])
+                    assert np.array_equal(op.prims().clamp_bits, p0.clamp_bits)
+                    vals.append(Lp)
+                arr[idx] = x0
+                fd[idx] = (vals[0] - vals[1]) / (2 * h)
+            assert rel_l2(grads[name], fd) < 1e-5, (name, rel_l2(grads[name], fd))
+        # a depth-only loss must reach the parameters only through geometry and opacity, never through colour
+        g_depth_only = o0.backward(np.zeros_like(G), GD, None)
+        assert np.abs(g_depth_only["sh"]).max() == 0 and np.abs(g_depth_only["mean"]).max() > 0
+        return
+    pytest.fail("no finite-difference scene far from every threshold found")
