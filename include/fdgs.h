@@ -114,6 +114,20 @@ int fdgs_render_backward(const fdgs_scene *scene, const fdgs_view *view_host, co
                          size_t ws_bytes, int64_t pair_capacity, void *cuda_stream, const float *dL_dimage,
                          const float *final_T, const uint32_t *n_contrib, const fdgs_grads *grads_host);
 
+/* Auxiliary channels through the same blend (eq. 25, L256 eq. 29; reading S18):
+ *   accumulated opacity O_gs = sum_k alpha_k T_k = 1 - final_T          (already an output of fdgs_render_forward);
+ *   rendered depth      D    = sum_k z_k alpha_k T_k, z_k = camera depth of the conditional mean, no background term.
+ * fdgs_render_forward_aux = fdgs_render_forward + depth_map [H,W].
+ * fdgs_render_backward_aux = fdgs_render_backward with two more upstream gradients, dL_ddepth [H,W] and dL_dopacity
+ * [H,W] (= dL/dO_gs); either may be NULL.  Exact derivative of the forward as stated, accumulated into grads. */
+int fdgs_render_forward_aux(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws,
+                            size_t ws_bytes, int64_t pair_capacity, void *cuda_stream, float *image, float *final_T,
+                            uint32_t *n_contrib, float *depth_map);
+int fdgs_render_backward_aux(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws,
+                             size_t ws_bytes, int64_t pair_capacity, void *cuda_stream, const float *dL_dimage,
+                             const float *dL_ddepth, const float *dL_dopacity, const float *final_T,
+                             const uint32_t *n_contrib, const fdgs_grads *grads_host);
+
 /* Harness-side loss ("rendering loss"): L = mean |image - target| over 3HW values.
  * Writes dL/dimage [3,H,W] and adds L to *loss (device float, caller zeroes it). */
 int fdgs_l1_loss(const float *image, const float *target, int64_t count, float *dL_dimage, float *loss,
@@ -166,6 +180,7 @@ int fdgs_step_batch(const fdgs_scene *scene, const fdgs_view *views_host, int32_
 #define FDGS_EXPORT_RANGES 7        /* uint32[tiles,2]: [first, last+1) into the sorted arrays               */
 #define FDGS_EXPORT_SPLAT_GRADS 8   /* float[N,9]: dL/d(u, v, A, B, C, o, r, g, b) from the last backward    */
 #define FDGS_EXPORT_DEPTH_ORDER 9   /* uint32[num_visible]: ids of the survivors sorted by (depth bits, id)   */
+#define FDGS_EXPORT_SPLAT_GRAD_DEPTH 10 /* float[N]: dL/d(camera depth) per splat from the last fdgs_render_backward_aux */
 int fdgs_debug_export(const void *ws, size_t ws_bytes, int what, void *dst, size_t dst_bytes, void *cuda_stream);
 
 /* Measurement hooks (bench.py).  fdgs_set_stage_timing(1) makes the three calls record CUDA events at

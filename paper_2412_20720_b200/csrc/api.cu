@@ -145,7 +145,7 @@ int fdgs_preprocess(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config*
 
 // A6-A9.  The depth order of the survivors (level 1) is kept in the workspace for the backward.
 static int forward_impl(const fdgs_scene* sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, int64_t cap,
-                        cudaStream_t st, float* image, float* final_T, uint32_t* n_contrib, int* l1_buf_out, int* l2_buf_out) {
+                        cudaStream_t st, float* image, float* final_T, uint32_t* n_contrib, float* depth_map, int* l1_buf_out, int* l2_buf_out) {
   // scan_ticket[1] and sort_ticket[0..7] are adjacent in the header: clear them together
   FDGS_CUDA(cudaMemsetAsync(&ws.hdr->scan_ticket[1], 0, 9 * sizeof(unsigned int), st), "memset(tickets)");
   FDGS_CUDA(cudaMemsetAsync(ws.scan_state[1], 0, 8 * ((size_t)(sc->N > 0 ? sc->N : 1) / 256 + 2), st), "memset(scan)");
@@ -159,7 +159,7 @@ static int forward_impl(const fdgs_scene* sc, const ViewParams& vp, const CfgPar
   const int tile_bits = ceil_log2((long long)vp.tiles_x * vp.tiles_y);
   const int l2 = launch_sort_pairs(ws, ws.l2_keys, ws.l2_vals, &ws.hdr->num_pairs, cap, tile_bits, SORT_ITEMS_L2, 4, true, sms, st);
   mark(EV_FWD3, st);
-  launch_blend_fwd(ws, l2, vp, cp, image, final_T, n_contrib, st);
+  launch_blend_fwd(ws, l2, vp, cp, image, final_T, n_contrib, depth_map, st);
   mark(EV_FWD4, st);
   FDGS_CUDA(cudaGetLastError(), "forward launches");
   *l1_buf_out = l1; *l2_buf_out = l2;
@@ -176,8 +176,8 @@ static void sort_bufs(const fdgs_scene* sc, const ViewParams& vp, int64_t cap, i
 
 extern "C" {
 
-int fdgs_render_forward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
-                        int64_t cap, void* stream, float* image, float* final_T, uint32_t* n_contrib) {
+static int forward_entry(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
+                         int64_t cap, void* stream, float* image, float* final_T, uint32_t* n_contrib, float* depth_map) {
   int rc = check_common(sc, v, c, ws_ptr);
   if (rc) return rc;
   if (!image || !final_T || !n_contrib || cap < 1 || cap >= (1LL << 30)) return FDGS_ERR_INVALID;
@@ -187,7 +187,18 @@ int fdgs_render_forward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_con
   ViewParams vp; CfgParams cp;
   make_params(v, c, vp, cp);
   int l1, l2;
-  return forward_impl(sc, vp, cp, ws, cap, (cudaStream_t)stream, image, final_T, n_contrib, &l1, &l2);
+  return forward_impl(sc, vp, cp, ws, cap, (cudaStream_t)stream, image, final_T, n_contrib, depth_map, &l1, &l2);
+}
+
+int fdgs_render_forward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
+                        int64_t cap, void* stream, float* image, float* final_T, uint32_t* n_contrib) {
+  return forward_entry(sc, v, c, ws_ptr, ws_bytes, cap, stream, image, final_T, n_contrib, nullptr);
+}
+
+int fdgs_render_forward_aux(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
+                            int64_t cap, void* stream, float* image, float* final_T, uint32_t* n_contrib, float* depth_map) {
+  if (!depth_map) return FDGS_ERR_INVALID;
+  return forward_entry(sc, v, c, ws_ptr, ws_bytes, cap, stream, image, final_T, n_contrib, depth_map);
 }
 
 }  // extern "C"
@@ -196,7 +207,7 @@ int fdgs_render_forward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_con
 // non-atomic gradient read-modify-writes of concurrent views while their blend kernels overlap.
 static int backward_impl(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes, int64_t cap,
                          cudaStream_t st, const float* dL_dimage, const float* final_T, const uint32_t* n_contrib,
-                         const fdgs_grads* g, cudaEvent_t before_b2) {
+                         const fdgs_grads* g, cudaEvent_t before_b2, const float* dL_ddepth = nullptr, const float* dL_dopacity = nullptr) {
   int rc = check_common(sc, v, c, ws_ptr);
   if (rc) return rc;
   if (!dL_dimage || !final_T || !n_contrib || !g || cap < 1 || cap >= (1LL << 30)) return FDGS_ERR_INVALID;
@@ -210,11 +221,13 @@ static int backward_impl(const fdgs_scene* sc, const fdgs_view* v, const fdgs_co
   int l1, l2;
   sort_bufs(sc, vp, cap, &l1, &l2);
   if (sc->N > 0) FDGS_CUDA(cudaMemsetAsync(ws.g9, 0, sizeof(float) * 9 * (size_t)sc->N, st), "memset(g9)");
+  const bool aux = dL_ddepth || dL_dopacity;
+  if (aux && sc->N > 0) FDGS_CUDA(cudaMemsetAsync(ws.gz, 0, sizeof(float) * (size_t)sc->N, st), "memset(gz)");
   mark(EV_BWD0, st);
-  launch_blend_bwd(ws, l2, vp, cp, dL_dimage, final_T, n_contrib, st);          // B1
+  launch_blend_bwd(ws, l2, vp, cp, dL_dimage, final_T, n_contrib, dL_ddepth, dL_dopacity, st);   // B1
   mark(EV_BWD1, st);
   if (before_b2) FDGS_CUDA(cudaStreamWaitEvent(st, before_b2, 0), "wait before B2");
-  launch_preprocess_bwd(*sc, vp, cp, ws, l1, *g, st);                           // B2
+  launch_preprocess_bwd(*sc, vp, cp, ws, l1, *g, aux, st);                      // B2
   mark(EV_BWD2, st);
   FDGS_CUDA(cudaGetLastError(), "backward launches");
   return FDGS_OK;
@@ -226,6 +239,12 @@ int fdgs_render_backward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_co
                          int64_t cap, void* stream, const float* dL_dimage, const float* final_T, const uint32_t* n_contrib,
                          const fdgs_grads* g) {
   return backward_impl(sc, v, c, ws_ptr, ws_bytes, cap, (cudaStream_t)stream, dL_dimage, final_T, n_contrib, g, nullptr);
+}
+
+int fdgs_render_backward_aux(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
+                             int64_t cap, void* stream, const float* dL_dimage, const float* dL_ddepth, const float* dL_dopacity,
+                             const float* final_T, const uint32_t* n_contrib, const fdgs_grads* g) {
+  return backward_impl(sc, v, c, ws_ptr, ws_bytes, cap, (cudaStream_t)stream, dL_dimage, final_T, n_contrib, g, nullptr, dL_ddepth, dL_dopacity);
 }
 
 int fdgs_l1_loss(const float* image, const float* target, int64_t count, float* dL_dimage, float* loss, void* stream) {
@@ -423,6 +442,7 @@ extern "C" int fdgs_debug_export(const void* ws_ptr, size_t ws_bytes, int what, 
     case FDGS_EXPORT_SORTED_VALS: src = ws.l2_vals[l2]; need = 4 * (size_t)D; break;
     case FDGS_EXPORT_RANGES: src = ws.ranges; need = 8 * (size_t)h.tiles; break;
     case FDGS_EXPORT_SPLAT_GRADS: src = ws.g9; need = 36 * (size_t)N; break;
+    case FDGS_EXPORT_SPLAT_GRAD_DEPTH: src = ws.gz; need = 4 * (size_t)N; break;
     default: return FDGS_ERR_INVALID;
   }
   if (src) {

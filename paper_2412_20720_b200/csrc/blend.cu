@@ -18,7 +18,7 @@ __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.
 __device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
 // Shared-memory form of a splat: three float4, read as broadcast LDS.128
-//   s0 = (-ca, -cb, -cc, k1 = ca*(u-ox) + cb*(v-oy))   s1 = (k2 = cc*(v-oy), lo = log2(o), r, g)   s2 = (b, u-ox, v-oy, -)
+//   s0 = (-ca, -cb, -cc, k1 = ca*(u-ox) + cb*(v-oy))   s1 = (k2 = cc*(v-oy), lo = log2(o), r, g)   s2 = (b, u-ox, v-oy, depth)
 __device__ __forceinline__ void stage_splat(const SplatRec* __restrict__ rec, const unsigned int id, const float ox, const float oy,
                                             float4* s0, float4* s1, float4* s2) {
   const float4* src = reinterpret_cast<const float4*>(rec + id);
@@ -26,7 +26,7 @@ __device__ __forceinline__ void stage_splat(const SplatRec* __restrict__ rec, co
   const float ul = q0.x - ox, vl = q0.y - oy;
   *s0 = make_float4(-q0.z, -q0.w, -q1.x, fmaf(q0.z, ul, q0.w * vl));
   *s1 = make_float4(q1.x * vl, q1.y, q1.z, q1.w);
-  *s2 = make_float4(q2.x, ul, vl, 0.f);
+  *s2 = make_float4(q2.x, ul, vl, q2.y);
 }
 
 // Conservative test "can this splat reach alpha >= alpha_min anywhere on an 8x4 pixel patch?": in the whitened
@@ -57,11 +57,14 @@ struct Strip {
 // A9.  STATS = true: same walk without the patch culling, counting the work instead of writing the image
 // (fdgs_debug_blend_stats): stats[0] (pixel, splat) pairs walked until the pixel terminates, [1] pairs that reach the
 // exp2, [2] pairs composited, [3] splats staged into shared memory (summed over tiles).
-template <int PX, bool STATS>
+// AUX = true additionally composites the camera depth of the splats like a fourth colour channel without background
+// (rendered depth, eq. 29) into depth_map[H,W].
+template <int PX, bool STATS, bool AUX>
 __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
                                                              const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
                                                              float* __restrict__ image, float* __restrict__ final_T,
-                                                             unsigned int* __restrict__ n_contrib, unsigned long long* stats) {
+                                                             unsigned int* __restrict__ n_contrib, unsigned long long* stats,
+                                                             float* __restrict__ depth_map) {
   constexpr int BATCH = 256 / PX;
   __shared__ struct { float4 s0[BATCH], s1[BATCH], s2[BATCH]; } sm;
   const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
@@ -69,14 +72,14 @@ __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __rest
   const Strip<PX> sp(warp, lane);
   const int px = tx * TILE + sp.lx;
   const float x = sp.lx + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
-  float y[PX], T[PX], Cr[PX], Cg[PX], Cb[PX];
+  float y[PX], T[PX], Cr[PX], Cg[PX], Cb[PX], Dz[PX];
   unsigned int last[PX];
   bool done[PX], inside[PX];
 #pragma unroll
   for (int k = 0; k < PX; ++k) {
     const int ly = sp.ly0 + 4 * k;
     inside[k] = px < vp.width && ty * TILE + ly < vp.height;
-    y[k] = ly + 0.5f; T[k] = 1.f; Cr[k] = Cg[k] = Cb[k] = 0.f; last[k] = 0; done[k] = !inside[k];
+    y[k] = ly + 0.5f; T[k] = 1.f; Cr[k] = Cg[k] = Cb[k] = Dz[k] = 0.f; last[k] = 0; done[k] = !inside[k];
   }
   const uint2 range = ranges[tile];
   const int n = (int)(range.y - range.x);
@@ -129,6 +132,7 @@ __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __rest
           if (Tn < c_tmin) { done[k] = true; continue; }   // the terminating splat is not composited
           const float wgt = alpha * T[k];
           Cr[k] = fmaf(b.z, wgt, Cr[k]); Cg[k] = fmaf(b.w, wgt, Cg[k]); Cb[k] = fmaf(sm.s2[j].x, wgt, Cb[k]);
+          if (AUX) Dz[k] = fmaf(sm.s2[j].w, wgt, Dz[k]);
           T[k] = Tn;
           last[k] = base + j + 1;
           if (STATS) ++st_comp;
@@ -156,6 +160,7 @@ __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __rest
     const size_t pix = (size_t)(ty * TILE + sp.ly0 + 4 * k) * vp.width + px;
     image[pix] = fmaf(T[k], vp.bg[0], Cr[k]); image[hw + pix] = fmaf(T[k], vp.bg[1], Cg[k]); image[2 * hw + pix] = fmaf(T[k], vp.bg[2], Cb[k]);
     final_T[pix] = T[k]; n_contrib[pix] = last[k];
+    if (AUX) depth_map[pix] = Dz[k];
   }
 }
 
@@ -337,20 +342,20 @@ constexpr int HROW = 36;   // float4 per buffered hit: 32 lanes + pad (144 words
 template <int HBUF>        // hits buffered per warp (4, 8 or 16; 8 measured best: 4 flushes too often, 16 costs occupancy)
 struct Bwd2Shared {
   float4 s0[128], s1[128], s2[128];
-  float acc[9 * 129];
+  float acc[10 * 129];     // nine sums of the colour path + (AUX) sum of wgt * dL/ddepth
   unsigned int id[128];
   int max_contrib;
   int hitj[4][HBUF];
   float4 hit[4][HBUF][HROW];
-  float4 pg[4][32][2];     // per warp, per lane: (gr0, gg0, gb0, gr1), (gg1, gb1, -, -)
+  float4 pg[4][32][2];     // per warp, per lane: (gr0, gg0, gb0, gr1), (gg1, gb1, gD0, gD1)
 };
 
-template <int HBUF>
+template <int HBUF, bool AUX>
 __device__ __forceinline__ void bwd2_flush(Bwd2Shared<HBUF>& sm, const int warp, const int lane, const int n, const float sx0, const float sy0) {
   constexpr int LPH = 32 / HBUF;             // lanes per buffered hit (4 or 8); each sums 64 / LPH pixels
   __syncwarp();
   const int h = lane / LPH, q = lane % LPH;
-  float S[9] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};   // Sx, Sy, Sxx, Sxy, Syy, cr, cg, cb, S1
+  float S[10] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};   // Sx, Sy, Sxx, Sxy, Syy, cr, cg, cb, S1, (AUX) Sz
   int j = 0;
   if (h < n) {
     j = sm.hitj[warp][h];
@@ -372,10 +377,11 @@ __device__ __forceinline__ void bwd2_flush(Bwd2Shared<HBUF>& sm, const int warp,
       S[5] = fmaf(d.y, g0.x, S[5]); S[6] = fmaf(d.y, g0.y, S[6]); S[7] = fmaf(d.y, g0.z, S[7]);
       S[5] = fmaf(d.w, g0.w, S[5]); S[6] = fmaf(d.w, g1.x, S[6]); S[7] = fmaf(d.w, g1.y, S[7]);
       S[8] += d.x; S[8] += d.z;
+      if (AUX) { S[9] = fmaf(d.y, g1.z, S[9]); S[9] = fmaf(d.w, g1.w, S[9]); }
     }
   }
 #pragma unroll
-  for (int k = 0; k < 9; ++k)
+  for (int k = 0; k < (AUX ? 10 : 9); ++k)
 #pragma unroll
     for (int o = 1; o < LPH; o <<= 1) S[k] += __shfl_xor_sync(0xffffffffu, S[k], o);
   if (h < n) {                               // every lane of the hit holds all nine sums: lane q adds rows q, q + LPH, ...
@@ -396,15 +402,21 @@ __device__ __forceinline__ void bwd2_flush(Bwd2Shared<HBUF>& sm, const int warp,
       atomicAdd(&sm.acc[q * 129 + j], r0);
     }
     if (q == 0) atomicAdd(&sm.acc[8 * 129 + j], S[8]);
+    if (AUX && q == 1) atomicAdd(&sm.acc[9 * 129 + j], S[9]);
   }
   __syncwarp();
 }
 
-template <int HBUF, int MINB>
+// AUX = true: upstream gradients of the auxiliary channels as well (either pointer may be NULL): dL/ddepth enters as a
+// fourth colour channel (g.c_k -> g.c_k + gD z_k, one more sum Sz = sum wgt gD -> gz[id] = dL/dz_k), dL/dopacity
+// (O = 1 - T_final) only shifts the start of the colour-behind recurrence: s_last = T_final (g.bg - gO).
+template <int HBUF, int MINB, bool AUX>
 __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
                                                          const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
                                                          const float* __restrict__ dL_dimage, const float* __restrict__ final_T,
-                                                         const unsigned int* __restrict__ n_contrib, float* __restrict__ g9) {
+                                                         const unsigned int* __restrict__ n_contrib, float* __restrict__ g9,
+                                                         const float* __restrict__ dL_ddepth, const float* __restrict__ dL_dopacity,
+                                                         float* __restrict__ gz) {
   constexpr int PX = 2, BATCH = 128, ACC_STRIDE = 129;
   __shared__ Bwd2Shared<HBUF> sm;
   const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
@@ -415,25 +427,27 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
   const float sx0 = sp.xm - 4.0f, sy0 = sp.ym0 - 2.0f;          // strip origin (tile-local)
   const uint2 range = ranges[tile];
   const size_t hw = (size_t)vp.width * vp.height;
-  float y[PX], T[PX], s[PX], gr[PX], gg[PX], gb[PX];
+  float y[PX], T[PX], s[PX], gr[PX], gg[PX], gb[PX], gD[PX];
   int mine[PX], wmax[PX];
   int lane_max = 0;
 #pragma unroll
   for (int k = 0; k < PX; ++k) {
     const int ly = sp.ly0 + 4 * k, py = ty * TILE + ly;
-    y[k] = ly + 0.5f; T[k] = 1.f; mine[k] = 0; gr[k] = gg[k] = gb[k] = 0.f;
+    y[k] = ly + 0.5f; T[k] = 1.f; mine[k] = 0; gr[k] = gg[k] = gb[k] = gD[k] = 0.f;
+    float gO = 0.f;
     if (px < vp.width && py < vp.height) {
       const size_t pix = (size_t)py * vp.width + px;
       T[k] = final_T[pix]; mine[k] = (int)n_contrib[pix]; gr[k] = dL_dimage[pix]; gg[k] = dL_dimage[hw + pix]; gb[k] = dL_dimage[2 * hw + pix];
+      if (AUX) { if (dL_ddepth) gD[k] = dL_ddepth[pix]; if (dL_dopacity) gO = dL_dopacity[pix]; }
     }
-    s[k] = T[k] * (gr[k] * vp.bg[0] + gg[k] * vp.bg[1] + gb[k] * vp.bg[2]);
+    s[k] = T[k] * (gr[k] * vp.bg[0] + gg[k] * vp.bg[1] + gb[k] * vp.bg[2] - gO);
     int w = mine[k];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) w = max(w, __shfl_xor_sync(0xffffffffu, w, o));
     wmax[k] = w; lane_max = max(lane_max, w);
   }
   sm.pg[warp][lane][0] = make_float4(gr[0], gg[0], gb[0], gr[1]);
-  sm.pg[warp][lane][1] = make_float4(gg[1], gb[1], 0.f, 0.f);
+  sm.pg[warp][lane][1] = make_float4(gg[1], gb[1], gD[0], gD[1]);
   if (threadIdx.x == 0) sm.max_contrib = 0;
   __syncthreads();
   if (lane == 0) atomicMax(&sm.max_contrib, lane_max);
@@ -451,7 +465,7 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
       stage_splat(rec, id, ox, oy, &sm.s0[threadIdx.x], &sm.s1[threadIdx.x], &sm.s2[threadIdx.x]);
     }
 #pragma unroll
-    for (int k = 0; k < 9; ++k) sm.acc[k * ACC_STRIDE + threadIdx.x] = 0.f;
+    for (int k = 0; k < (AUX ? 10 : 9); ++k) sm.acc[k * ACC_STRIDE + threadIdx.x] = 0.f;
     __syncthreads();
     if (lo_pos < lane_max) {
      int nbuf = 0;                                      // buffered hits (warp-uniform)
@@ -486,7 +500,7 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
           }
         }
         if (!__any_sync(0xffffffffu, alpha[0] > 0.f || alpha[1] > 0.f)) continue;
-        const float cb = sm.s2[j].x;
+        const float cb = sm.s2[j].x, cz = AUX ? sm.s2[j].w : 0.f;
         float dpow[PX], wgt[PX];
 #pragma unroll
         for (int k = 0; k < PX; ++k) {                 // branch-free: alpha == 0 leaves T and s unchanged and yields zeros
@@ -494,17 +508,18 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
           const float Tk = alpha[k] > 0.f ? T[k] * iom : T[k];           // exact identity when alpha == 0
           T[k] = Tk;
           wgt[k] = alpha[k] * Tk;
-          const float gc = fmaf(gr[k], b.z, fmaf(gg[k], b.w, gb[k] * cb));   // dL/dpixel . c_k
+          float gc = fmaf(gr[k], b.z, fmaf(gg[k], b.w, gb[k] * cb));         // dL/dpixel . c_k
+          if (AUX) gc = fmaf(gD[k], cz, gc);
           const float dalpha = fmaf(Tk, gc, -s[k] * iom);
           s[k] = fmaf(gc, wgt[k], s[k]);
           dpow[k] = araw[k] > c_amax ? 0.f : alpha[k] * dalpha;      // alpha clamp active: no gradient through the exponent
         }
         sm.hit[warp][nbuf][lane] = make_float4(dpow[0], wgt[0], dpow[1], wgt[1]);
         if (lane == 0) sm.hitj[warp][nbuf] = j;
-        if (++nbuf == HBUF) { bwd2_flush<HBUF>(sm, warp, lane, HBUF, sx0, sy0); nbuf = 0; }
+        if (++nbuf == HBUF) { bwd2_flush<HBUF, AUX>(sm, warp, lane, HBUF, sx0, sy0); nbuf = 0; }
       }
      }
-     if (nbuf) bwd2_flush<HBUF>(sm, warp, lane, nbuf, sx0, sy0);
+     if (nbuf) bwd2_flush<HBUF, AUX>(sm, warp, lane, nbuf, sx0, sy0);
     }
     __syncthreads();
     if ((int)threadIdx.x < m) {
@@ -522,6 +537,7 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
       float* dst = g9 + (size_t)9 * sm.id[j];
 #pragma unroll
       for (int k = 0; k < 9; ++k) if (out[k] != 0.f) atomicAdd(dst + k, out[k]);
+      if (AUX) { const float sz = sm.acc[9 * ACC_STRIDE + j]; if (sz != 0.f) atomicAdd(gz + sm.id[j], sz); }
     }
   }
 }
@@ -535,22 +551,34 @@ static int blend_px() {
 }
 
 void launch_blend_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
-                      unsigned int* n_contrib, cudaStream_t st) {
+                      unsigned int* n_contrib, float* depth_map, cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
-#define FDGS_FWD(PXV) blend_fwd_kernel<PXV, false><<<tiles, 256 / PXV, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr)
+  if (depth_map) {
+    blend_fwd_kernel<2, false, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr, depth_map);
+    ++g_launches;
+    return;
+  }
+#define FDGS_FWD(PXV) blend_fwd_kernel<PXV, false, false><<<tiles, 256 / PXV, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr, nullptr)
   switch (blend_px()) { case 1: FDGS_FWD(1); break; case 4: FDGS_FWD(4); break; default: FDGS_FWD(2); }
 #undef FDGS_FWD
   ++g_launches;
 }
 
 void launch_blend_stats(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, unsigned long long* stats, cudaStream_t st) {
-  blend_fwd_kernel<1, true><<<vp.tiles_x * vp.tiles_y, 256, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, nullptr, nullptr, nullptr, stats);
+  blend_fwd_kernel<1, true, false><<<vp.tiles_x * vp.tiles_y, 256, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, nullptr, nullptr, nullptr, stats, nullptr);
   ++g_launches;
 }
 
 void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* dL_dimage,
-                      const float* final_T, const unsigned int* n_contrib, cudaStream_t st) {
+                      const float* final_T, const unsigned int* n_contrib, const float* dL_ddepth, const float* dL_dopacity,
+                      cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
+  if (dL_ddepth || dL_dopacity) {
+    blend_bwd2_kernel<8, 6, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9,
+                                                         dL_ddepth, dL_dopacity, ws.gz);
+    ++g_launches;
+    return;
+  }
 #define FDGS_BWD(PXV) blend_bwd_kernel<PXV><<<tiles, 256 / PXV, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9)
   static const bool direct = getenv("FDGS_BLEND_DIRECT") != nullptr;   // experiments: the shuffle-reduction kernel at PX = 2
   switch (blend_px()) {
@@ -558,7 +586,7 @@ void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, con
     case 4: FDGS_BWD(4); break;
     default:
       if (direct) FDGS_BWD(2);
-      else blend_bwd2_kernel<8, 6><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9);
+      else blend_bwd2_kernel<8, 6, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9, nullptr, nullptr, nullptr);
   }
 #undef FDGS_BWD
   ++g_launches;

@@ -84,6 +84,7 @@ struct Workspace {
   float* g9;                         // [N,9] per-splat gradients of the blend backward
   float4* aux;                       // [N] survivors: view direction (x, y, z) and (t - mu_t) / T, written by preprocess
   float4* dcol;                      // [N] survivors: colour backward -> geometry backward: dL/d dir (x, y, z), dL/d Delta
+  float* gz;                         // [N] auxiliary depth channel: dL/d(camera depth) per splat
   size_t lookback_bytes, zero_bytes; // zero_bytes: prefix of the workspace cleared by fdgs_preprocess
   size_t bytes;
 };
@@ -119,6 +120,7 @@ inline Workspace carve(void* base, long long N, long long K, long long W, long l
   w.g9 = (float*)take(4 * 9 * Np);
   w.aux = (float4*)take(16 * Np);
   w.dcol = (float4*)take(16 * Np);
+  w.gz = (float*)take(4 * Np);
   (void)K;
   w.bytes = off;
   return w;
@@ -153,12 +155,13 @@ void launch_tile_grid(const Workspace& ws, const ViewParams& vp, long long cap, 
 void launch_offsets(const Workspace& ws, int l1_buf, int N, cudaStream_t st);
 void launch_duplicate(const Workspace& ws, int l1_buf, int N, const ViewParams& vp, cudaStream_t st);
 void launch_blend_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
-                      unsigned int* n_contrib, cudaStream_t st);
+                      unsigned int* n_contrib, float* depth_map /*NULL = no auxiliary channel*/, cudaStream_t st);
 void launch_blend_stats(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, unsigned long long* stats, cudaStream_t st);
 void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* dL_dimage,
-                      const float* final_T, const unsigned int* n_contrib, cudaStream_t st);
+                      const float* final_T, const unsigned int* n_contrib, const float* dL_ddepth, const float* dL_dopacity,
+                      cudaStream_t st);
 void launch_preprocess_bwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, int l1_buf,
-                           const fdgs_grads& g, cudaStream_t st);
+                           const fdgs_grads& g, bool with_gz, cudaStream_t st);
 void launch_cull_status(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, unsigned char* dst, cudaStream_t st);
 void launch_l1_loss(const float* image, const float* target, long long count, float* dL, float* loss, cudaStream_t st);
 void launch_export_records(const Workspace& ws, int N, float* dst, cudaStream_t st);

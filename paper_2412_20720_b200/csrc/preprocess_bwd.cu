@@ -157,7 +157,7 @@ __global__ void __launch_bounds__(32 * CB_WARPS) colour_bwd_kernel(const float* 
 // Sigma_2d = B B^T + dI, B = T N, N = M3 - c m4^T / b, c = M3 m4, b = m4.m4, M = R diag(s), R = L(q_l) R(q_r).
 __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, const ViewParams vp, const CfgParams cp,
                                                        const unsigned int* __restrict__ vis_list, const WsHeader* __restrict__ hdr,
-                                                       const float* __restrict__ g9, const float4* __restrict__ dcol, const fdgs_grads gr) {
+                                                       const float* __restrict__ g9, const float4* __restrict__ dcol, const float* __restrict__ gz, const fdgs_grads gr) {
   const unsigned int slot = blockIdx.x * blockDim.x + threadIdx.x;
   if (slot >= hdr->num_visible) return;
   const int i = vis_list[slot];
@@ -231,6 +231,7 @@ __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, cons
     dp[0] = g_u * vp.fx * iz;
     dp[1] = g_v * vp.fy * iz;
     dp[2] = -(g_u * vp.fx * x + g_v * vp.fy * y) * iz2 - (dJ00 * vp.fx + dJ11 * vp.fy) * iz2;
+    if (gz) dp[2] += gz[i];                       // auxiliary depth channel: z_k = p_z
     if (!g.clampx) { dp[0] -= dJ02 * vp.fx * iz2; dp[2] += dJ02 * 2.f * vp.fx * x * iz2 * iz; }
     else           { dp[2] += dJ02 * vp.fx * g.xr * iz2; }
     if (!g.clampy) { dp[1] -= dJ12 * vp.fy * iz2; dp[2] += dJ12 * 2.f * vp.fy * y * iz2 * iz; }
@@ -335,7 +336,7 @@ __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, cons
 }
 
 void launch_preprocess_bwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, int l1_buf,
-                           const fdgs_grads& gr, cudaStream_t st) {
+                           const fdgs_grads& gr, bool with_gz, cudaStream_t st) {
   if (sc.N <= 0) return;
   // the survivor count lives on the device: launch for all N slots, surplus warps / threads exit at once
   (void)l1_buf;
@@ -346,7 +347,7 @@ void launch_preprocess_bwd(const fdgs_scene& sc, const ViewParams& vp, const Cfg
     if (KD == 1) FDGS_LAUNCH(1); else if (KD == 4) FDGS_LAUNCH(4); else if (KD == 9) FDGS_LAUNCH(9); else FDGS_LAUNCH(16);
 #undef FDGS_LAUNCH
   }
-  geom_bwd_kernel<<<(sc.N + 127) / 128, 128, 0, st>>>(sc, vp, cp, ws.vis_ids, ws.hdr, ws.g9, ws.dcol, gr);
+  geom_bwd_kernel<<<(sc.N + 127) / 128, 128, 0, st>>>(sc, vp, cp, ws.vis_ids, ws.hdr, ws.g9, ws.dcol, with_gz ? ws.gz : nullptr, gr);
   g_launches += 2;
 }
 

@@ -17,12 +17,13 @@ _lib = None
 
 OK, ERR_INVALID, ERR_WORKSPACE, ERR_CUDA, ERR_PAIR_OVERFLOW = 0, -1, -2, -3, -4
 (EXPORT_STATUS, EXPORT_RECORDS, EXPORT_RECTS, EXPORT_TILES_TOUCHED, EXPORT_OFFSETS, EXPORT_SORTED_KEYS,
- EXPORT_SORTED_VALS, EXPORT_RANGES, EXPORT_SPLAT_GRADS, EXPORT_DEPTH_ORDER) = range(10)
+ EXPORT_SORTED_VALS, EXPORT_RANGES, EXPORT_SPLAT_GRADS, EXPORT_DEPTH_ORDER, EXPORT_SPLAT_GRAD_DEPTH) = range(11)
 
 EXPORTED_SYMBOLS = ["fdgs_default_config", "fdgs_workspace_bytes", "fdgs_preprocess", "fdgs_render_forward",
                     "fdgs_render_backward", "fdgs_l1_loss", "fdgs_step_host", "fdgs_debug_export",
                     "fdgs_launch_count", "fdgs_strerror", "fdgs_set_stage_timing", "fdgs_get_stage_ms",
-                    "fdgs_debug_blend_stats", "fdgs_step_batch", "fdgs_debug_cull_status"]
+                    "fdgs_debug_blend_stats", "fdgs_step_batch", "fdgs_debug_cull_status", "fdgs_render_forward_aux",
+                    "fdgs_render_backward_aux"]
 MAX_BATCH = 8
 
 
@@ -75,6 +76,9 @@ def load():
     lib.fdgs_render_forward.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, vp, vp, vp]
     lib.fdgs_render_backward.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, vp, vp,
                                          vp, C.POINTER(CGrads)]
+    lib.fdgs_render_forward_aux.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, vp, vp, vp, vp]
+    lib.fdgs_render_backward_aux.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, vp, vp, vp,
+                                             vp, vp, C.POINTER(CGrads)]
     lib.fdgs_l1_loss.argtypes = [vp, vp, i64, vp, vp, vp]
     lib.fdgs_step_host.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, vp, vp, vp, vp,
                                    vp, vp, vp, C.POINTER(CGrads), vp]
@@ -253,6 +257,26 @@ class Renderer:
         if rc:
             raise FdgsError(rc, "fdgs_render_backward")
 
+    def forward_aux(self, cview: CView):
+        """Forward with the auxiliary depth channel: returns (image, depth_map); opacity is 1 - self.final_T."""
+        import torch
+        if getattr(self, "depth_map", None) is None:
+            self.depth_map = torch.empty((self.height, self.width), dtype=torch.float32, device=self.ws.device)
+        rc = self.lib.fdgs_render_forward_aux(C.byref(self._cs), C.byref(cview), C.byref(self.cfg), self.ws.data_ptr(),
+                                              self.ws_bytes, self.cap, _stream(), self.image.data_ptr(), self.final_T.data_ptr(),
+                                              self.n_contrib.data_ptr(), self.depth_map.data_ptr())
+        if rc:
+            raise FdgsError(rc, "fdgs_render_forward_aux")
+        return self.image, self.depth_map
+
+    def backward_aux(self, cview: CView, dL_dimage, dL_ddepth, dL_dopacity, grads: dict):
+        cg = grads_struct(grads)
+        rc = self.lib.fdgs_render_backward_aux(C.byref(self._cs), C.byref(cview), C.byref(self.cfg), self.ws.data_ptr(),
+                                               self.ws_bytes, self.cap, _stream(), dL_dimage.data_ptr(), _ptr(dL_ddepth),
+                                               _ptr(dL_dopacity), self.final_T.data_ptr(), self.n_contrib.data_ptr(), C.byref(cg))
+        if rc:
+            raise FdgsError(rc, "fdgs_render_backward_aux")
+
     def l1_loss(self, target):
         """loss += mean|image - target|; writes self.dL_dimage."""
         rc = self.lib.fdgs_l1_loss(self.image.data_ptr(), target.data_ptr(), self.image.numel(), self.dL_dimage.data_ptr(),
@@ -308,7 +332,7 @@ class Renderer:
                   EXPORT_TILES_TOUCHED: ((N,), torch.int32), EXPORT_OFFSETS: ((nvis,), torch.int32),
                   EXPORT_SORTED_KEYS: ((D,), torch.int64), EXPORT_SORTED_VALS: ((D,), torch.int32),
                   EXPORT_RANGES: ((tiles, 2), torch.int32), EXPORT_SPLAT_GRADS: ((N, 9), torch.float32),
-                  EXPORT_DEPTH_ORDER: ((nvis,), torch.int32)}
+                  EXPORT_DEPTH_ORDER: ((nvis,), torch.int32), EXPORT_SPLAT_GRAD_DEPTH: ((N,), torch.float32)}
         shape, dt = shapes[what]
         out = torch.zeros(shape, dtype=dt, device=dev)
         if out.numel() == 0:

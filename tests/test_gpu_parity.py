@@ -142,3 +142,63 @@ def test_blend_kernel_variants_in_a_fresh_process(env):
                         "-k", "cfg2_reduced_and_ragged or cfg1_tiny"], env=dict(os.environ, **env), capture_output=True, text=True, timeout=600)
     assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
     assert "2 passed" in r.stdout
+
+
+def _aux_parity(scene, label, view_index=0):
+    """Auxiliary channels (depth map, accumulated opacity) against the oracle: forward map and all parameter gradients of
+    a loss that touches colour, depth and opacity."""
+    import gpu_helpers as gh
+    import torch
+    from paper_2412_20720_b200 import fdgs
+    view = scene.views[view_index]
+    o = oracle_for(scene, view_index)
+    P = o.prims()
+    img_o, fT_o, nc_o, margin = o.forward()
+    D_o = o.depth_map()
+    W, H = view.width, view.height
+    dL = scenes.upstream_normal(scene.seed, W, H).astype(np.float64) / (3 * W * H)
+    gD = scenes.normal(scene.seed, 210, W * H).reshape(H, W) / (W * H)
+    gO = scenes.normal(scene.seed, 211, W * H).reshape(H, W) / (W * H)
+    go = o.backward(dL, gD, gO)
+    ds = fdgs.DeviceScene.from_scene(scene)
+    r = fdgs.Renderer(ds, W, H, max(1 << 16, 64 * scene.N))
+    cv = fdgs.make_view(view)
+    r.preprocess(cv)
+    img, dm = r.forward_aux(cv)
+    g = ds.zero_grads(with_mean2d=True)
+    f32 = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    r.backward_aux(cv, f32(dL), f32(gD), f32(gO), g)
+    torch.cuda.synchronize()
+    fragile = P.fragility < gh.FRAG_TOL
+    off, ids = o.tile_lists()
+    gpu = dict(ranges=r.export(fdgs.EXPORT_RANGES).cpu().numpy(), sorted_vals=r.export(fdgs.EXPORT_SORTED_VALS).cpu().numpy(),
+               sorted_keys=r.export(fdgs.EXPORT_SORTED_KEYS).cpu().numpy())
+    rep = dict(label=label)
+    bad_tiles = gh.compare_tile_lists(gpu, P, off, ids, fragile, rep)
+    flag = gh.flagged_pixels(bad_tiles, margin, W, H)
+    scale = max(1.0, float(np.abs(D_o).max()))
+    rep["depth_max_abs_rel"] = float(np.abs(dm.cpu().numpy().astype(np.float64) - D_o)[~flag].max() / scale)
+    rep["image_max_abs"] = float(np.abs(img.cpu().numpy().astype(np.float64) - img_o).max(0)[~flag].max())
+    keep = ~fragile
+    rep["gz_rel_l2"] = gh.rel_l2(r.export(fdgs.EXPORT_SPLAT_GRAD_DEPTH).cpu().numpy()[keep], go["gz"][keep])
+    for k in PARAMS + ("mean2d",):
+        rep["grad_" + k] = gh.rel_l2(g[k].cpu().numpy().astype(np.float64)[keep], go[k][keep])
+    print("PARITY_AUX " + json.dumps(rep))
+    assert rep["depth_max_abs_rel"] <= IMG_TOL and rep["image_max_abs"] <= IMG_TOL
+    assert rep["gz_rel_l2"] <= GRAD_TOL
+    for k in PARAMS + ("mean2d",):
+        assert rep["grad_" + k] <= GRAD_TOL, k
+    # depth / opacity gradients alone (no colour gradient): colour coefficients receive nothing
+    g2 = ds.zero_grads()
+    r.backward_aux(cv, torch.zeros_like(r.image), f32(gD), None, g2)
+    torch.cuda.synchronize()
+    assert float(g2["sh"].abs().max()) == 0.0 and float(g2["mean"].abs().max()) > 0.0
+
+
+def test_aux_channels_cfg1():
+    _aux_parity(scenes.tiny(), "aux cfg1")
+
+
+def test_aux_channels_cfg2_ragged_and_cfg4_heavy_tails():
+    _aux_parity(scenes.single_object(N=20000, width=250, height=190), "aux cfg2 20k 250x190")
+    _aux_parity(scenes.driving(N=40000, width=480, height=320, n_views=1), "aux cfg4 40k 480x320")
