@@ -47,7 +47,7 @@ def test_depth_does_not_change_colour_path():
     g0 = o.backward(G)
     g1 = o.backward(G, dL_ddepth=np.zeros((64, 64)), dL_dopacity=np.zeros((64, 64)))
     for k in PARAMS:
-        assert np.array_equal(g0[k], g1[k])
+        np.testing.assert_allclose(g0[k], g1[k], rtol=1e-11, atol=1e-13)     # OpenMP atomics: summation order varies
     assert np.abs(g1["gz"]).max() == 0
 
 
