@@ -33,9 +33,17 @@ def _full_parity(scene, view_index=0, cfg=None, dL_mode="normal", check_grads=Tr
     off, ids = o.tile_lists()
     rep["num_pairs_oracle"] = int(off[-1])
     bad_tiles = gh.compare_tile_lists(gpu, P, off, ids, fragile, rep)
+    member_tiles = rep.pop("_member_tiles")
     flag = gh.flagged_pixels(bad_tiles, margin, view.width, view.height)
     err = np.abs(gpu["image"] - img_o).max(0)
-    rep["flagged_pixels"] = int(flag.sum())
+    # Tiles that differ ONLY by swaps of near-tie depths hold two equally valid orders (S13): their pixels leave the strict
+    # comparison, are bounded loosely and do not count against the budget of flagged pixels (dense scenes: cfg4 has
+    # ~5000 splats per tile, so almost every tile holds some pair of depths within 1e-5 relative).
+    tie_only = gh.flagged_pixels(bad_tiles & ~member_tiles, np.full_like(margin, np.inf), view.width, view.height)
+    budget_flag = gh.flagged_pixels(member_tiles, margin, view.width, view.height)
+    rep["tie_swap_pixels"] = int((tie_only & ~budget_flag).sum())
+    rep["image_max_abs_tie_swap"] = float(err[tie_only].max()) if tie_only.any() else 0.0
+    rep["flagged_pixels"] = int(budget_flag.sum())
     rep["image_max_abs"] = float(err[~flag].max()) if (~flag).any() else 0.0
     rep["image_max_abs_flagged"] = float(err[flag].max()) if flag.any() else 0.0
     rep["final_T_max_abs"] = float(np.abs(gpu["final_T"] - fT_o)[~flag].max()) if (~flag).any() else 0.0
@@ -63,6 +71,7 @@ def _full_parity(scene, view_index=0, cfg=None, dL_mode="normal", check_grads=Tr
     print("PARITY " + json.dumps(rep))
     assert rep["image_max_abs"] <= IMG_TOL
     assert rep["flagged_pixels"] < 0.05 * flag.size          # flagged items are counted and reported, and stay few
+    assert rep["image_max_abs_tie_swap"] <= 1e-2             # a swapped near-tie pair changes a pixel by ~alpha_a alpha_b |c_a - c_b| T
     assert rep["final_T_max_abs"] <= IMG_TOL and rep["n_contrib_equal_frac"] > 0.999
     if check_grads:
         for k in PARAMS + ("mean2d",):
@@ -123,6 +132,19 @@ def test_sh_degree_variants(L, n_time):
     _full_parity(sc, label=f"L={L} n_time={n_time}")
 
 
+def test_cfg4_full_one_view():
+    """Largest config: 3M Gaussians, 1920x1280, camera inside the cloud (48 M pairs, ~5000 splats per tile)."""
+    import gpu_helpers as gh
+    sc = scenes.driving(n_views=1)
+    orig = gh.gpu_run
+    try:
+        gh.gpu_run = lambda scene, view, **kw: orig(scene, view, **dict(kw, pair_capacity=96 * 1024 * 1024))
+        rep, gpu, o = _full_parity(sc, dL_mode="l1", label="cfg4 3M 1920x1280 view0")
+    finally:
+        gh.gpu_run = orig
+    assert rep["num_pairs_gpu"] > 40_000_000
+
+
 def test_cfg3_full_one_view():
     """BASELINE.json's headline size in the launch configuration bench.py times: 1M Gaussians, 1352x1014."""
     sc = scenes.multiview_video(n_views=1)
@@ -175,6 +197,7 @@ def _aux_parity(scene, label, view_index=0):
                sorted_keys=r.export(fdgs.EXPORT_SORTED_KEYS).cpu().numpy())
     rep = dict(label=label)
     bad_tiles = gh.compare_tile_lists(gpu, P, off, ids, fragile, rep)
+    rep.pop("_member_tiles")
     flag = gh.flagged_pixels(bad_tiles, margin, W, H)
     scale = max(1.0, float(np.abs(D_o).max()))
     rep["depth_max_abs_rel"] = float(np.abs(dm.cpu().numpy().astype(np.float64) - D_o)[~flag].max() / scale)
