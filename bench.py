@@ -231,11 +231,13 @@ def run_fdgs(args):
     # ---- end to end through the C ABI with host buffers ----------------------------------------------------
     ms_e2e, _ = timed(step_host, max(3, args.steps // 2), 3)
     # ---- forward-only FPS (one frame = preprocess + forward of one view) -----------------------------------
-    fps_ms = []
+    fps_ms, fps_all = [], []
     for cv in cviews:
-        m, _ = timed(lambda: forward_only(cv), 25, 5)
+        m, per = timed(lambda: forward_only(cv), 25, 20)      # 20 warm-up + 25 timed frames per view: 100 timed frames
         fps_ms.append(m)
+        fps_all += per
     ms_frame = sum(fps_ms) / len(fps_ms)
+    fps_all.sort()
     # ---- playback throughput: consecutive frames in flight on separate streams / workspaces (cfg5-style free-viewpoint
     # video): the scans and sorts of frame k+1 overlap the blend of frame k -------------------------------
     streams = [torch.cuda.Stream() for _ in range(n_views)]
@@ -290,6 +292,9 @@ def run_fdgs(args):
                 "traffic": BLEND_BWD_NCU_TRAFFIC_BYTES if dom == "blend_bwd" else None,
                 "peak_source": "derived: 148 SMs x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md unit counts and max clock)",
                 "algorithmic_lane_instr_per_launch": instr / n_views, "ms_per_launch": stage[dom] / n_views}
+    peaks = fdgs.measure_peaks()           # measured FMA / MUFU pipe peaks next to the derived ALU roof
+    roofline["peak_measured_fma_tlane_per_s"] = peaks["fma_tlane_per_s"]
+    roofline["peak_measured_mufu_ex2_t_per_s"] = peaks["mufu_ex2_t_per_s"]
     per_stage = stage_rooflines(stage, work, ds.N, ds.K, n_views)
     for name, ins in (("blend_fwd", instr_fwd), ("blend_bwd", instr_bwd)):
         a = ins / (stage[name] * 1e-3) / 1e12
@@ -311,6 +316,7 @@ def run_fdgs(args):
                       "multi_gpu": "replicas only",
                       "schedule": "fdgs_step_batch: the 4 views on 4 worker streams and workspaces, gradient accumulation chained"},
            "forward_fps": world * 1e3 / ms_frame, "ms_per_frame": ms_frame,
+           "ms_per_frame_median": fps_all[len(fps_all) // 2], "ms_per_frame_min": fps_all[0], "frames_timed": len(fps_all),
            "forward_fps_pipelined": world * 1e3 / ms_frame_pipelined, "ms_per_frame_pipelined": ms_frame_pipelined,
            "e2e": {"value": world * 1e3 / ms_e2e, "unit": "steps/s", "h2d_bytes_per_step": n_views * img_bytes, "d2h_bytes_per_step": n_views * 4,
                    "ms_per_step": ms_e2e},

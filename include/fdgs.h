@@ -200,6 +200,12 @@ int fdgs_debug_blend_stats(const fdgs_view *view_host, const fdgs_config *cfg_ho
 int fdgs_debug_cull_status(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *cuda_stream,
                            unsigned char *status_dev);
 
+/* Measured pipe peaks of this GPU (the blend kernels' roofline denominators): FP32 FMA issue rate
+ * in T lane-instructions/s (8 independent FFMA chains per thread, 8 CTAs of 256 threads per SM) and MUFU.EX2 rate in
+ * T/s.  scratch_dev: >= 4 * 8 * 256 * (number of SMs) bytes.  Synchronises; takes a few ms. */
+int fdgs_debug_measure_peaks(void *scratch_dev, size_t scratch_bytes, void *cuda_stream, float *fma_tlane_per_s_host,
+                             float *mufu_t_per_s_host);
+
 /* Number of kernel launches the library has issued so far in this process (bench.py's gpu_launches). */
 int64_t fdgs_launch_count(void);
 

@@ -86,6 +86,37 @@ __global__ void export_keys_kernel(const unsigned int* __restrict__ tile_keys, c
   if (i < D) dst[i] = ((unsigned long long)tile_keys[i] << 32) | __float_as_uint(rec[ids[i]].depth);
 }
 
+// ---- measured pipe peaks: the denominators of the blend kernels' roofline ------------------------
+// 8 independent FFMA chains per thread: 1 lane-instruction per lane and issue slot, nothing else in the loop
+__global__ void __launch_bounds__(256) peak_fma_kernel(float* out, const int iters, const float s) {
+  float a[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) a[k] = threadIdx.x * 1e-3f + k;
+  for (int i = 0; i < iters; ++i)
+#pragma unroll
+    for (int u = 0; u < 8; ++u)
+#pragma unroll
+      for (int k = 0; k < 8; ++k) a[k] = fmaf(a[k], s, 1e-3f);
+  float r = 0.f;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) r += a[k];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = r;
+}
+__global__ void __launch_bounds__(256) peak_mufu_kernel(float* out, const int iters) {
+  float a[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) a[k] = -(threadIdx.x * 1e-3f + k);
+  for (int i = 0; i < iters; ++i)
+#pragma unroll
+    for (int u = 0; u < 8; ++u)
+#pragma unroll
+      for (int k = 0; k < 8; ++k) asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(a[k]));
+  float r = 0.f;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) r += a[k];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = r;
+}
+
 }  // namespace fdgs
 
 using namespace fdgs;
@@ -386,6 +417,37 @@ int fdgs_debug_cull_status(const fdgs_scene* sc, const fdgs_view* v, const fdgs_
   make_params(v, c, vp, cp);
   launch_cull_status(*sc, vp, cp, status_dev, (cudaStream_t)stream);
   FDGS_CUDA(cudaGetLastError(), "cull status launch");
+  return FDGS_OK;
+}
+
+int fdgs_debug_measure_peaks(void* scratch_dev, size_t scratch_bytes, void* stream, float* fma_tlane_per_s_host, float* mufu_t_per_s_host) {
+  if (!scratch_dev || !fma_tlane_per_s_host || !mufu_t_per_s_host) return FDGS_ERR_INVALID;
+  const int blocks = 8 * num_sms(), threads = 256;
+  if (scratch_bytes < sizeof(float) * (size_t)blocks * threads) return FDGS_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaEvent_t e0, e1;
+  FDGS_CUDA(cudaEventCreate(&e0), "event create");
+  FDGS_CUDA(cudaEventCreate(&e1), "event create");
+  float best_fma = 0.f, best_mufu = 0.f;
+  for (int rep = 0; rep < 4; ++rep) {          // first repetition warms up; best of the rest
+    const int it_f = 4000, it_m = 1000;
+    float ms = 0.f;
+    cudaEventRecord(e0, st);
+    peak_fma_kernel<<<blocks, threads, 0, st>>>((float*)scratch_dev, it_f, 0.999f);
+    cudaEventRecord(e1, st);
+    FDGS_CUDA(cudaEventSynchronize(e1), "peak sync");
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (rep) best_fma = fmaxf(best_fma, (float)((double)blocks * threads * it_f * 64.0 / (ms * 1e-3) / 1e12));
+    cudaEventRecord(e0, st);
+    peak_mufu_kernel<<<blocks, threads, 0, st>>>((float*)scratch_dev, it_m);
+    cudaEventRecord(e1, st);
+    FDGS_CUDA(cudaEventSynchronize(e1), "peak sync");
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (rep) best_mufu = fmaxf(best_mufu, (float)((double)blocks * threads * it_m * 64.0 / (ms * 1e-3) / 1e12));
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  FDGS_CUDA(cudaGetLastError(), "peak kernels");
+  *fma_tlane_per_s_host = best_fma; *mufu_t_per_s_host = best_mufu;
   return FDGS_OK;
 }
 

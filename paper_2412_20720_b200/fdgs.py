@@ -23,7 +23,7 @@ EXPORTED_SYMBOLS = ["fdgs_default_config", "fdgs_workspace_bytes", "fdgs_preproc
                     "fdgs_render_backward", "fdgs_l1_loss", "fdgs_step_host", "fdgs_debug_export",
                     "fdgs_launch_count", "fdgs_strerror", "fdgs_set_stage_timing", "fdgs_get_stage_ms",
                     "fdgs_debug_blend_stats", "fdgs_step_batch", "fdgs_debug_cull_status", "fdgs_render_forward_aux",
-                    "fdgs_render_backward_aux"]
+                    "fdgs_render_backward_aux", "fdgs_debug_measure_peaks"]
 MAX_BATCH = 8
 
 
@@ -85,6 +85,7 @@ def load():
     lib.fdgs_step_batch.argtypes = [C.POINTER(CScene), C.POINTER(CView), i32, C.POINTER(CConfig), i64, C.POINTER(CViewBuffers), vp, vp,
                                     C.POINTER(CGrads), vp]
     lib.fdgs_debug_cull_status.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, vp]
+    lib.fdgs_debug_measure_peaks.argtypes = [vp, sz, vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
     lib.fdgs_debug_export.argtypes = [vp, sz, C.c_int, vp, sz, vp]
     lib.fdgs_set_stage_timing.argtypes = [C.c_int]
     lib.fdgs_get_stage_ms.argtypes = [C.POINTER(C.c_float)]
@@ -123,6 +124,17 @@ def stage_ms() -> dict:
     if rc:
         raise FdgsError(rc, "fdgs_get_stage_ms")
     return {k: float(buf[i]) for i, k in enumerate(STAGES)}
+
+
+def measure_peaks() -> dict:
+    """Measured FP32-FMA issue peak (T lane-instructions/s) and MUFU.EX2 peak (T/s) of the current device."""
+    import torch
+    scratch = torch.empty(4 * 8 * 256 * 256, dtype=torch.uint8, device="cuda")
+    a, b = C.c_float(0), C.c_float(0)
+    rc = load().fdgs_debug_measure_peaks(scratch.data_ptr(), scratch.numel(), _stream(), C.byref(a), C.byref(b))
+    if rc:
+        raise FdgsError(rc, "fdgs_debug_measure_peaks")
+    return {"fma_tlane_per_s": float(a.value), "mufu_ex2_t_per_s": float(b.value)}
 
 
 def default_config(**overrides) -> CConfig:
