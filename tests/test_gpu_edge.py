@@ -174,3 +174,43 @@ def test_step_batch_matches_view_by_view():
     assert gh.rel_l2(g2["sh"].cpu().numpy(), g_ref["sh"].cpu().numpy()) < 1e-5
     with pytest.raises(ValueError):
         fdgs.BatchStep(ds, 200, 150, 1 << 21, 9)
+
+
+def test_autograd_front_end_matches_the_c_abi_path():
+    """paper_2412_20720_b200.autograd.Rasterizer: loss.backward() == fdgs_render_backward(_aux) with the same upstream."""
+    import gpu_helpers as gh
+    import torch
+    from paper_2412_20720_b200 import autograd, fdgs
+    sc = scenes.multiview_video(N=8000, width=160, height=112, n_views=1)
+    view = sc.views[0]
+    ds = fdgs.DeviceScene.from_scene(sc)
+    params = {k: getattr(ds, k).clone().requires_grad_(True) for k in autograd.PARAM_KEYS}
+    rast = autograd.Rasterizer(sc.sh_degree, sc.n_time, 160, 112, 1 << 20)
+    tgt = torch.from_numpy(scenes.target_image(3, 0, 160, 112)).cuda()
+    # colour only
+    img = rast(params, view)
+    (img - tgt).abs().mean().backward()
+    r = fdgs.Renderer(ds, 160, 112, 1 << 20)
+    cv = fdgs.make_view(view)
+    g = ds.zero_grads()
+    r.preprocess(cv); r.forward(cv); r.loss.zero_(); r.l1_loss(tgt); r.backward(cv, r.dL_dimage, g)
+    torch.cuda.synchronize()
+    assert torch.equal(img.detach(), r.image)
+    for k in autograd.PARAM_KEYS:
+        assert gh.rel_l2(params[k].grad.cpu().numpy(), g[k].cpu().numpy()) < 1e-5, k
+        params[k].grad = None
+    # colour + depth + opacity
+    img, depth, opac = rast(params, view, aux=True)
+    loss = (img * img).sum() * 1e-4 + (depth * 0.01).sum() + (opac * opac).sum() * 1e-3
+    loss.backward()
+    g2 = ds.zero_grads()
+    r.preprocess(cv); r.forward_aux(cv)
+    r.backward_aux(cv, (2e-4 * r.image).contiguous(), torch.full_like(r.depth_map, 0.01), (2e-3 * (1 - r.final_T)).contiguous(), g2)
+    torch.cuda.synchronize()
+    for k in autograd.PARAM_KEYS:
+        assert gh.rel_l2(params[k].grad.cpu().numpy(), g2[k].cpu().numpy()) < 1e-5, k
+    # a stale graph is refused instead of silently using the wrong workspace state
+    a = rast(params, view)
+    rast(params, view)
+    with pytest.raises(RuntimeError, match="rendered again"):
+        a.sum().backward()
