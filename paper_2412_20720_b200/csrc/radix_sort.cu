@@ -14,7 +14,9 @@ constexpr int LB_WIN = 8;
 constexpr unsigned int LB_AGG = 1u << 30, LB_PRE = 2u << 30, LB_MASK = (1u << 30) - 1;
 
 template <int ITEMS>
-__global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const unsigned int* __restrict__ keys_in, const unsigned int* __restrict__ vals_in,
+// 3 CTAs per SM (<= 85 registers): measured best at 50 M pairs (812 us for two passes vs 916 us at 2 CTAs / 128 registers);
+// 4 or 5 CTAs spill.
+__global__ void __launch_bounds__(SORT_THREADS, 3) onesweep_kernel(const unsigned int* __restrict__ keys_in, const unsigned int* __restrict__ vals_in,
                                                                 unsigned int* __restrict__ keys_out, unsigned int* __restrict__ vals_out,
                                                                 const unsigned int* __restrict__ count_dev, unsigned int* ticket,
                                                                 const unsigned int* __restrict__ digit_base /*[RADIX]*/,
@@ -64,7 +66,6 @@ __global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const unsigned i
     // size to the warp's digit counter with one shared atomic that returns the count of earlier rounds.  The ITEMS
     // peer masks are independent of each other and the atomics of one warp retire in program order, so nothing in this
     // loop waits on the previous round.
-    unsigned int grp[ITEMS];
 #pragma unroll
     for (int r = 0; r < ITEMS; ++r) {
       const bool valid = warp_base + r * 32 + lane < n;
@@ -79,16 +80,11 @@ __global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const unsigned i
         const unsigned int bal = __ballot_sync(0xffffffffu, bit);
         peers &= bit ? bal : ~bal;
       }
-      grp[r] = peers;
-    }
-#pragma unroll
-    for (int r = 0; r < ITEMS; ++r) {
-      const bool valid = warp_base + r * 32 + lane < n;
-      const int leader = __ffs(grp[r]) - 1;
+      const int leader = __ffs(peers) - 1;
       unsigned int old = 0;
-      if (valid && lane == leader) old = atomicAdd(&warp_hist[warp][(key[r] >> shift) & (RADIX - 1)], (unsigned int)__popc(grp[r]));
+      if (valid && lane == leader) old = atomicAdd(&warp_hist[warp][digit], (unsigned int)__popc(peers));
       old = __shfl_sync(0xffffffffu, old, leader);
-      rank[r] = (unsigned short)(old + __popc(grp[r] & lt_mask));
+      rank[r] = (unsigned short)(old + __popc(peers & lt_mask));
     }
     __syncthreads();
     // ---- thread d owns digit d: exclusive offsets over warps, tile count, look-back, local digit base
