@@ -185,7 +185,7 @@ static int forward_impl(const fdgs_scene* sc, const ViewParams& vp, const CfgPar
   const int l1 = launch_sort_pairs(ws, ws.l1_keys, ws.l1_vals, &ws.hdr->num_visible, sc->N, 32, SORT_ITEMS_L1, 0, false, sms, st);
   mark(EV_FWD1, st);
   launch_offsets(ws, l1, sc->N, st);
-  launch_duplicate(ws, l1, sc->N, vp, st);
+  launch_duplicate(ws, l1, sc->N, cap, vp, st);
   mark(EV_FWD2, st);
   const int tile_bits = ceil_log2((long long)vp.tiles_x * vp.tiles_y);
   const int l2 = launch_sort_pairs(ws, ws.l2_keys, ws.l2_vals, &ws.hdr->num_pairs, cap, tile_bits, SORT_ITEMS_L2, 4, true, sms, st);

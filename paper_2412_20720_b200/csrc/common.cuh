@@ -57,6 +57,7 @@ constexpr int SORT_ITEMS_L2 = 16;   // tile-id sort of D pairs
 constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_ITEMS = 8;
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
+constexpr int DUP_CHUNK = 2048;         // output pairs per CTA of the pair emission
 constexpr int MAX_GRID_CELLS = 50000;   // (tiles_x+1)*(tiles_y+1) must fit the tile-grid kernel's shared memory
 
 // Host-side view of the carved-up workspace.
@@ -76,6 +77,7 @@ struct Workspace {
   unsigned int* l1_vals[2];          // [N] primitive ids of survivors; after the sort: depth order
   unsigned int* vis_ids;             // [N] primitive ids of survivors in ascending id order (kept for the backward)
   unsigned int* offsets;             // [N] exclusive prefix sum of tiles_touched in depth order
+  unsigned int* chunk_first;         // [cap / DUP_CHUNK + 2] survivor (depth order) that owns output position k * DUP_CHUNK
   unsigned int* l2_keys[2];          // [cap] tile ids
   unsigned int* l2_vals[2];          // [cap] primitive ids
   unsigned int* sort_hist;           // [8][RADIX] digit counts of the 4 depth passes (raw) and exclusive bases of the tile-id passes
@@ -110,6 +112,7 @@ inline Workspace carve(void* base, long long N, long long K, long long W, long l
   for (int i = 0; i < 2; ++i) w.l1_vals[i] = (unsigned int*)take(4 * Np);
   w.vis_ids = (unsigned int*)take(4 * Np);
   w.offsets = (unsigned int*)take(4 * Np);
+  w.chunk_first = (unsigned int*)take(4 * ((size_t)cap / DUP_CHUNK + 2));
   for (int i = 0; i < 2; ++i) w.l2_keys[i] = (unsigned int*)take(4 * (size_t)cap);
   for (int i = 0; i < 2; ++i) w.l2_vals[i] = (unsigned int*)take(4 * (size_t)cap);
   const long long t1 = (Np + SORT_THREADS * SORT_ITEMS_L1 - 1) / (SORT_THREADS * SORT_ITEMS_L1);
@@ -153,7 +156,7 @@ int launch_sort_pairs(const Workspace& ws, unsigned int* const keys[2], unsigned
 void launch_tile_grid(const Workspace& ws, const ViewParams& vp, long long cap, int l2_passes, cudaStream_t st);
 // exclusive prefix sum of tiles_touched in depth order -> offsets
 void launch_offsets(const Workspace& ws, int l1_buf, int N, cudaStream_t st);
-void launch_duplicate(const Workspace& ws, int l1_buf, int N, const ViewParams& vp, cudaStream_t st);
+void launch_duplicate(const Workspace& ws, int l1_buf, int N, long long cap, const ViewParams& vp, cudaStream_t st);
 void launch_blend_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
                       unsigned int* n_contrib, float* depth_map /*NULL = no auxiliary channel*/, cudaStream_t st);
 void launch_blend_stats(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, unsigned long long* stats, cudaStream_t st);

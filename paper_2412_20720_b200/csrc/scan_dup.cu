@@ -95,10 +95,12 @@ __global__ void __launch_bounds__(SCAN_THREADS) compact_kernel(const unsigned in
   for (int p = 0; p < 4; ++p) { const unsigned int v = hist[p][threadIdx.x]; if (v) atomicAdd(sort_hist + p * RADIX + threadIdx.x, v); }
 }
 
-// offsets[j] = exclusive prefix of tiles_touched[sorted_ids[j]], j < num_visible (depth order)
+// offsets[j] = exclusive prefix of tiles_touched[sorted_ids[j]], j < num_visible (depth order).  Also fills the table the pair
+// emission starts from: chunk_first[k] = the survivor whose pairs contain output position k * DUP_CHUNK.
 __global__ void __launch_bounds__(SCAN_THREADS) offsets_kernel(const unsigned int* __restrict__ tiles_touched,
                                                                const unsigned int* __restrict__ sorted_ids, WsHeader* hdr,
-                                                               unsigned long long* state, unsigned int* __restrict__ offsets) {
+                                                               unsigned long long* state, unsigned int* __restrict__ offsets,
+                                                               unsigned int* __restrict__ chunk_first) {
   __shared__ unsigned int warp_sums[33], s_tile, s_prefix;
   const unsigned int n = hdr->num_visible;
   if (threadIdx.x == 0) s_tile = atomicAdd(&hdr->scan_ticket[1], 1u);
@@ -112,9 +114,16 @@ __global__ void __launch_bounds__(SCAN_THREADS) offsets_kernel(const unsigned in
   unsigned int total;
   const unsigned int excl = block_exclusive_scan(sum, total, warp_sums);
   const unsigned int prefix = lookback_prefix(state, tile, total, &s_prefix);
+  if (hdr->overflow) return;                               // D exceeds the capacity: nothing is emitted
   unsigned int run = prefix + excl;
 #pragma unroll
-  for (int k = 0; k < SCAN_ITEMS; ++k) { if (base + k < n) offsets[base + k] = run; run += c[k]; }
+  for (int k = 0; k < SCAN_ITEMS; ++k) {
+    if (base + k < n) {
+      offsets[base + k] = run;
+      for (unsigned int q = (run + DUP_CHUNK - 1) / DUP_CHUNK; q * DUP_CHUNK < run + c[k]; ++q) chunk_first[q] = base + k;
+    }
+    run += c[k];
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -166,41 +175,35 @@ __global__ void __launch_bounds__(1024) tile_grid_kernel(const int* __restrict__
 }
 
 // ---------------------------------------------------------------------------------------------
-// A6: pair emission in depth order.  A warp owns 32 consecutive survivors and walks the flattened sequence of
-// their tiles 32 at a time, so heavy-tailed footprints (one splat covering thousands of tiles) stay balanced
-// inside the warp and every store is coalesced.
+// A6: pair emission in depth order, balanced by OUTPUT: a CTA owns DUP_CHUNK consecutive pairs whatever the footprints of
+// the survivors that produce them (a splat covering the whole screen is spread over many CTAs, thousands of one-tile
+// splats share one).  The survivors of the chunk [chunk_first[k], chunk_first[k+1]] are staged in shared memory (offset,
+// id, rectangle), every thread finds the owner of its pairs by binary search there, and all stores are coalesced.
 __global__ void __launch_bounds__(256) duplicate_kernel(const unsigned int* __restrict__ sorted_ids, const unsigned int* __restrict__ offsets,
                                                         const ushort4* __restrict__ rect, const WsHeader* __restrict__ hdr,
-                                                        const int tiles_x, unsigned int* __restrict__ keys, unsigned int* __restrict__ vals) {
-  const unsigned int n = hdr->num_visible;
-  if (hdr->overflow) return;
-  const int lane = threadIdx.x & 31;
-  const unsigned int warp_base = (blockIdx.x * blockDim.x + threadIdx.x) & ~31u;
-  if (warp_base >= n) return;
-  const unsigned int j = warp_base + lane;
-  unsigned int id = 0, off = 0, cnt = 0;
-  ushort4 rc = make_ushort4(0, 0, 0, 0);
-  if (j < n) { id = sorted_ids[j]; off = offsets[j]; rc = rect[id]; cnt = (unsigned int)(rc.z - rc.x) * (unsigned int)(rc.w - rc.y); }
-  unsigned int incl = cnt;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) { const unsigned int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
-  const unsigned int total = __shfl_sync(0xffffffffu, incl, 31);
-  const unsigned int out_base = __shfl_sync(0xffffffffu, off, 0);
-  const unsigned int excl = incl - cnt;
-  const unsigned int rc_lo = rc.x | ((unsigned int)rc.y << 16), width = rc.z - rc.x;
-  for (unsigned int b = 0; b < total; b += 32) {
-    const unsigned int e = b + lane;
-    int owner = 0;
-#pragma unroll
-    for (int s = 16; s > 0; s >>= 1) { const unsigned int v = __shfl_sync(0xffffffffu, incl, owner + s - 1); if (v <= e) owner += s; }
-    owner = min(owner, 31);
-    const unsigned int o_excl = __shfl_sync(0xffffffffu, excl, owner), o_lo = __shfl_sync(0xffffffffu, rc_lo, owner);
-    const unsigned int o_w = __shfl_sync(0xffffffffu, width, owner), o_id = __shfl_sync(0xffffffffu, id, owner);
-    if (e < total) {
-      const unsigned int local = e - o_excl, ty = (o_lo >> 16) + local / o_w, tx = (o_lo & 0xffffu) + local % o_w;
-      keys[out_base + e] = ty * tiles_x + tx;
-      vals[out_base + e] = o_id;
-    }
+                                                        const unsigned int* __restrict__ chunk_first, const int tiles_x,
+                                                        unsigned int* __restrict__ keys, unsigned int* __restrict__ vals) {
+  __shared__ unsigned int s_off[DUP_CHUNK + 1], s_id[DUP_CHUNK + 1];
+  __shared__ ushort4 s_rc[DUP_CHUNK + 1];
+  const unsigned int D = hdr->num_pairs, n = hdr->num_visible;
+  const unsigned int start = blockIdx.x * DUP_CHUNK;
+  if (start >= D) return;                                  // also covers overflow (num_pairs == 0)
+  const unsigned int end = min(start + DUP_CHUNK, D);
+  const unsigned int j0 = chunk_first[blockIdx.x];
+  const unsigned int j1 = end < D ? chunk_first[blockIdx.x + 1] : n - 1;     // last survivor with pairs in this chunk
+  const unsigned int m = j1 - j0 + 1;                      // <= DUP_CHUNK + 1: every survivor emits at least one pair
+  for (unsigned int s = threadIdx.x; s < m; s += blockDim.x) {
+    const unsigned int id = sorted_ids[j0 + s];
+    s_off[s] = offsets[j0 + s]; s_id[s] = id; s_rc[s] = rect[id];
+  }
+  __syncthreads();
+  for (unsigned int e = start + threadIdx.x; e < end; e += blockDim.x) {
+    unsigned int lo = 0, hi = m;                           // largest s with s_off[s] <= e
+    while (hi - lo > 1) { const unsigned int mid = (lo + hi) >> 1; if (s_off[mid] <= e) lo = mid; else hi = mid; }
+    const ushort4 rc = s_rc[lo];
+    const unsigned int local = e - s_off[lo], w = rc.z - rc.x;
+    keys[e] = (rc.y + local / w) * tiles_x + rc.x + local % w;
+    vals[e] = s_id[lo];
   }
 }
 
@@ -228,7 +231,7 @@ void launch_compact(const Workspace& ws, int N, cudaStream_t st) {
 void launch_offsets(const Workspace& ws, int l1_buf, int N, cudaStream_t st) {
   if (N <= 0) return;
   const int blocks = (N + SCAN_TILE - 1) / SCAN_TILE;
-  offsets_kernel<<<blocks, SCAN_THREADS, 0, st>>>(ws.tiles_touched, ws.l1_vals[l1_buf], ws.hdr, ws.scan_state[1], ws.offsets);
+  offsets_kernel<<<blocks, SCAN_THREADS, 0, st>>>(ws.tiles_touched, ws.l1_vals[l1_buf], ws.hdr, ws.scan_state[1], ws.offsets, ws.chunk_first);
   ++g_launches;
 }
 
@@ -240,10 +243,11 @@ void launch_tile_grid(const Workspace& ws, const ViewParams& vp, long long cap, 
   ++g_launches;
 }
 
-void launch_duplicate(const Workspace& ws, int l1_buf, int N, const ViewParams& vp, cudaStream_t st) {
+void launch_duplicate(const Workspace& ws, int l1_buf, int N, long long cap, const ViewParams& vp, cudaStream_t st) {
   if (N <= 0) return;
-  const int blocks = (N + 255) / 256;
-  duplicate_kernel<<<blocks, 256, 0, st>>>(ws.l1_vals[l1_buf], ws.offsets, ws.rect, ws.hdr, vp.tiles_x, ws.l2_keys[0], ws.l2_vals[0]);
+  // D lives on the device: one CTA per possible chunk of the capacity, surplus CTAs exit at once
+  const unsigned int blocks = (unsigned int)((cap + DUP_CHUNK - 1) / DUP_CHUNK);
+  duplicate_kernel<<<blocks, 256, 0, st>>>(ws.l1_vals[l1_buf], ws.offsets, ws.rect, ws.hdr, ws.chunk_first, vp.tiles_x, ws.l2_keys[0], ws.l2_vals[0]);
   ++g_launches;
 }
 
