@@ -4,6 +4,8 @@
 // Nothing but the 9 per-splat gradients of the blend backward, the view direction / time offset kept by the forward
 // preprocess (ws.aux) and the hand-over vector ws.dcol is read from the workspace; gradients are accumulated (+=)
 // into the caller's arrays.
+#include <cstdlib>
+
 #include "geom.cuh"
 
 namespace fdgs {
@@ -140,6 +142,79 @@ __global__ void __launch_bounds__(32 * CB_WARPS) colour_bwd_kernel(const float* 
           colour_element<KD>(t, e, __ldg(coef + e), d, ax, ay, az, ad);
           dcoef[e] = d;
         }
+      }
+    }
+#pragma unroll
+    for (int o = 1; o <= 2; o <<= 1) {
+      ax += __shfl_xor_sync(0xffffffffu, ax, o); ay += __shfl_xor_sync(0xffffffffu, ay, o);
+      az += __shfl_xor_sync(0xffffffffu, az, o); ad += __shfl_xor_sync(0xffffffffu, ad, o);
+    }
+    if (valid && l == 0) dcol[id] = make_float4(ax, ay, az, ad);
+  }
+}
+
+// K8a for sh_degree 3 (KD = 16, every benchmark configuration): no shared-memory table and no index arithmetic.  Lane l of
+// the 4 lanes of a survivor owns the SH orders k = 4l .. 4l+3 of every Fourier order n: 12 contiguous floats
+// (4 orders x 3 channels = three 128-bit loads) of the coefficient block and of its gradient block per n, with the
+// (k, channel) pattern of every register known at compile time; the four Y_k, their gradients and the masked dL/dc
+// live in registers.  A warp has 8 survivors in flight, 6 x 128-bit loads per lane and Fourier order.
+__global__ void __launch_bounds__(128) colour_bwd16_kernel(const float* __restrict__ sh, const int n_time, const float inv_T,
+                                                           const unsigned int* __restrict__ vis_list, const WsHeader* __restrict__ hdr,
+                                                           const float* __restrict__ g9, const SplatRec* __restrict__ rec,
+                                                           const float4* __restrict__ aux, float* __restrict__ dsh, float4* __restrict__ dcol) {
+  const int lane = threadIdx.x & 31;
+  const unsigned int n_vis = hdr->num_visible;
+  const unsigned int warp_slot = (blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32;
+  if (warp_slot >= n_vis) return;
+  const int rec_len = n_time * 48, grp = lane >> 2, l = lane & 3;
+  {  // first batch of 8 survivors: both blocks on their way from HBM (one lane per survivor asks)
+    const unsigned int slot = warp_slot + lane;
+    if (lane < 8 && slot < n_vis) { const size_t off = (size_t)vis_list[slot] * rec_len; prefetch_l2(sh + off, 4 * rec_len); prefetch_l2(dsh + off, 4 * rec_len); }
+  }
+#pragma unroll 1
+  for (int b = 0; b < 4; ++b) {
+    const unsigned int slot = warp_slot + 8 * b + grp;
+    const bool valid = slot < n_vis;
+    {  // next batch's blocks: requested one batch ahead (deeper would thrash L2)
+      const unsigned int nslot = warp_slot + 8 * (b + 1) + lane;
+      if (b < 3 && lane < 8 && nslot < n_vis) { const size_t off = (size_t)vis_list[nslot] * rec_len; prefetch_l2(sh + off, 4 * rec_len); prefetch_l2(dsh + off, 4 * rec_len); }
+    }
+    float ax = 0.f, ay = 0.f, az = 0.f, ad = 0.f;
+    int id = 0;
+    if (valid) {
+      id = vis_list[slot];
+      const float4 a = __ldg(aux + id);                       // view direction, (t - mu_t) / T
+      float Yf[16], Gf[48], Y[4], G[12];
+      sh_basis<16>(a.x, a.y, a.z, Yf);
+      sh_grad_table<16>(a.x, a.y, a.z, Gf);
+#define FDGS_PICK(L0) { _Pragma("unroll") for (int k = 0; k < 4; ++k) { Y[k] = Yf[4 * L0 + k]; G[3 * k] = Gf[12 * L0 + 3 * k]; G[3 * k + 1] = Gf[12 * L0 + 3 * k + 1]; G[3 * k + 2] = Gf[12 * L0 + 3 * k + 2]; } }
+      if (l == 0) FDGS_PICK(0) else if (l == 1) FDGS_PICK(1) else if (l == 2) FDGS_PICK(2) else FDGS_PICK(3)
+#undef FDGS_PICK
+      // the colour clamp at 0 was active iff the stored (clamped) colour is 0: those channels carry no gradient
+      const float* gp = g9 + (size_t)9 * id;
+      const float4 q1 = __ldg(reinterpret_cast<const float4*>(rec + id) + 1);
+      const float cbl = __ldg(reinterpret_cast<const float*>(rec + id) + 8);
+      const float gc[3] = {q1.z > 0.f ? gp[6] : 0.f, q1.w > 0.f ? gp[7] : 0.f, cbl > 0.f ? gp[8] : 0.f};
+      const float4* c4p = reinterpret_cast<const float4*>(sh + (size_t)id * rec_len) + 3 * l;
+      float4* d4p = reinterpret_cast<float4*>(dsh + (size_t)id * rec_len) + 3 * l;
+      for (int n = 0; n < n_time; ++n, c4p += 12, d4p += 12) {
+        const float4 c0 = __ldg(c4p), c1 = __ldg(c4p + 1), c2 = __ldg(c4p + 2);
+        float4 d0 = d4p[0], d1 = d4p[1], d2 = d4p[2];
+        const float cn = cospif(2.0f * (float)n * a.w);
+        const float wsn = -6.283185307179586f * (float)n * inv_T * sinpif(2.0f * (float)n * a.w);
+        const float cv[12] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w, c2.x, c2.y, c2.z, c2.w};
+        float dv[12] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w, d2.x, d2.y, d2.z, d2.w};
+        const float gcn[3] = {gc[0] * cn, gc[1] * cn, gc[2] * cn};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          float t = 0.f;                                      // sum over channels of coef * masked dL/dc
+#pragma unroll
+          for (int ch = 0; ch < 3; ++ch) { dv[3 * k + ch] = fmaf(gcn[ch], Y[k], dv[3 * k + ch]); t = fmaf(cv[3 * k + ch], gc[ch], t); }
+          ad = fmaf(t * wsn, Y[k], ad);
+          const float tc = t * cn;
+          ax = fmaf(tc, G[3 * k], ax); ay = fmaf(tc, G[3 * k + 1], ay); az = fmaf(tc, G[3 * k + 2], az);
+        }
+        d4p[0] = make_float4(dv[0], dv[1], dv[2], dv[3]); d4p[1] = make_float4(dv[4], dv[5], dv[6], dv[7]); d4p[2] = make_float4(dv[8], dv[9], dv[10], dv[11]);
       }
     }
 #pragma unroll
@@ -344,7 +419,9 @@ void launch_preprocess_bwd(const fdgs_scene& sc, const ViewParams& vp, const Cfg
   {
     const int threads = 32 * CB_WARPS, blocks = (sc.N + threads - 1) / threads;
 #define FDGS_LAUNCH(KDV) colour_bwd_kernel<KDV><<<blocks, threads, 0, st>>>(sc.sh, sc.n_time, vp.inv_T, ws.vis_ids, ws.hdr, ws.g9, ws.rec, ws.aux, gr.sh, ws.dcol)
-    if (KD == 1) FDGS_LAUNCH(1); else if (KD == 4) FDGS_LAUNCH(4); else if (KD == 9) FDGS_LAUNCH(9); else FDGS_LAUNCH(16);
+    if (KD == 1) FDGS_LAUNCH(1); else if (KD == 4) FDGS_LAUNCH(4); else if (KD == 9) FDGS_LAUNCH(9);
+    else if (getenv("FDGS_COLOUR_BWD_TABLE")) FDGS_LAUNCH(16);      // A/B runs: the generic table kernel at degree 3
+    else colour_bwd16_kernel<<<blocks, threads, 0, st>>>(sc.sh, sc.n_time, vp.inv_T, ws.vis_ids, ws.hdr, ws.g9, ws.rec, ws.aux, gr.sh, ws.dcol);
 #undef FDGS_LAUNCH
   }
   geom_bwd_kernel<<<(sc.N + 127) / 128, 128, 0, st>>>(sc, vp, cp, ws.vis_ids, ws.hdr, ws.g9, ws.dcol, with_gz ? ws.gz : nullptr, gr);
