@@ -62,7 +62,7 @@ def _load():
     lib.fdgs_oracle_forward.argtypes = [C.c_void_p, dp, dp, ip, dp]
     lib.fdgs_oracle_backward.argtypes = [C.c_void_p, dp] + [dp] * 8
     lib.fdgs_oracle_get_depth_map.argtypes = [C.c_void_p, dp]
-    lib.fdgs_oracle_backward_aux.argtypes = [C.c_void_p, dp, dp, dp] + [dp] * 9
+    lib.fdgs_oracle_backward_aux.argtypes = [C.c_void_p, dp, dp, dp] + [dp] * 10
     lib.fdgs_oracle_num_threads.restype = C.c_int
     _lib = lib
     return lib
@@ -189,9 +189,10 @@ class Oracle:
         _load().fdgs_oracle_get_depth_map(self._h, _d(out))
         return out
 
-    def backward(self, dL_dimage, dL_ddepth=None, dL_dopacity=None):
+    def backward(self, dL_dimage, dL_ddepth=None, dL_dopacity=None, densify=None):
         """Requires forward().  Returns a dict of gradient arrays (float64) incl. 'mean2d', 'g9' and 'gz'.
-        dL_ddepth / dL_dopacity [H,W]: upstream gradients of the auxiliary depth map and of O = 1 - final_T."""
+        dL_ddepth / dL_dopacity [H,W]: upstream gradients of the auxiliary depth map and of O = 1 - final_T.
+        densify: float64 [N,3] accumulated into (+=): |dL/d(u,v)|, |dL/dmu_t|, visibility count."""
         g = np.ascontiguousarray(np.asarray(dL_dimage, dtype=np.float64))
         assert g.shape == (3, self.height, self.width)
         aux = []
@@ -207,5 +208,6 @@ class Oracle:
         _load().fdgs_oracle_backward_aux(self._h, _d(g), _d(aux[0]) if aux[0] is not None else null,
                                          _d(aux[1]) if aux[1] is not None else null, _d(out["mean"]), _d(out["log_scale"]),
                                          _d(out["quat_l"]), _d(out["quat_r"]), _d(out["opacity_logit"]), _d(out["sh"]),
-                                         _d(out["mean2d"]), _d(out["g9"]), _d(out["gz"]))
+                                         _d(out["mean2d"]), _d(out["g9"]), _d(out["gz"]),
+                                         _d(densify) if densify is not None else null)
         return out

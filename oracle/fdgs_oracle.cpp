@@ -431,7 +431,8 @@ void backward_blend(Oracle& O, const double* dL_dimage, const double* dL_ddepth 
 // VJP of preprocess_one for a visible primitive (chain of Appendix D of SURVEY.md re-derived in DESIGN.md;
 // finite differences in tests/ are the authority).  Accumulates (+=) into the gradient arrays.
 void backward_one(const Oracle& O, int i, const double g9[9], double* d_mean, double* d_ls, double* d_ql,
-                  double* d_qr, double* d_logit, double* d_sh, double* d_mean2d, const double g_z = 0.0) {
+                  double* d_qr, double* d_logit, double* d_sh, double* d_mean2d, const double g_z = 0.0,
+                  double* densify3 = nullptr) {
   const Prim& P = O.prims[i]; const View& V = O.view; const Cfg& c = O.cfg;
   if (P.status != VISIBLE) return;
   const double g_u = g9[0], g_v = g9[1], g_A = g9[2], g_B = g9[3], g_C = g9[4], g_o = g9[5];
@@ -512,6 +513,9 @@ void backward_one(const Oracle& O, int i, const double g9[9], double* d_mean, do
   d_b += -muc_a * P.dt / (P.b * P.b) + aGa / (P.b * P.b);
   for (int r = 0; r < 3; ++r) d_mean[4 * i + r] += d_muc[r];
   d_mean[4 * i + 3] += -d_dt;                                             // Delta = t - mu_t
+  // density-control indicators of this view: magnitude of the screen-space position gradient, magnitude
+  // of the mu_t gradient, and the number of views the primitive was visible in
+  if (densify3) { densify3[3 * i] += std::sqrt(g_u * g_u + g_v * g_v); densify3[3 * i + 1] += std::fabs(d_dt); densify3[3 * i + 2] += 1.0; }
   // gradient wrt the full symmetric 4x4 Sigma, then Sigma = M M^T, M = R4 diag(s)
   double GS[4][4];
   for (int r = 0; r < 3; ++r) for (int q = 0; q < 3; ++q) GS[r][q] = Gc[r][q];
@@ -677,17 +681,18 @@ void fdgs_oracle_get_depth_map(void* h, double* depth_map) {
 }
 
 // fdgs_oracle_backward with upstream gradients of the auxiliary channels as well: dL_ddepth[H,W], dL_dopacity[H,W]
-// (either may be NULL).  gz[N] (may be NULL) receives the per-splat dL/dz.
+// (either may be NULL).  gz[N] (may be NULL) receives the per-splat dL/dz.  densify3[N,3] (may be NULL) is accumulated
+// into (+=): |dL/d(u,v)|, |dL/dmu_t|, visibility count of this view (density-control indicators).
 void fdgs_oracle_backward_aux(void* h, const double* dL_dimage, const double* dL_ddepth, const double* dL_dopacity,
                               double* d_mean, double* d_log_scale, double* d_quat_l, double* d_quat_r, double* d_logit,
-                              double* d_sh, double* d_mean2d, double* g9, double* gz) {
+                              double* d_sh, double* d_mean2d, double* g9, double* gz, double* densify3) {
   Oracle& O = *(Oracle*)h;
   backward_blend(O, dL_dimage, dL_ddepth, dL_dopacity);
   if (g9) std::copy(O.g9.begin(), O.g9.end(), g9);
   if (gz) std::copy(O.gz.begin(), O.gz.end(), gz);
 #pragma omp parallel for schedule(static)
   for (int i = 0; i < O.N; ++i)
-    backward_one(O, i, &O.g9[(size_t)9 * i], d_mean, d_log_scale, d_quat_l, d_quat_r, d_logit, d_sh, d_mean2d, O.gz[i]);
+    backward_one(O, i, &O.g9[(size_t)9 * i], d_mean, d_log_scale, d_quat_l, d_quat_r, d_logit, d_sh, d_mean2d, O.gz[i], densify3);
 }
 
 int fdgs_oracle_num_threads(void) {

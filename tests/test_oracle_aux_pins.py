@@ -98,3 +98,23 @@ def test_aux_backward_matches_central_differences(mode):
         assert np.abs(g_depth_only["sh"]).max() == 0 and np.abs(g_depth_only["mean"]).max() > 0
         return
     pytest.fail("no finite-difference scene far from every threshold found")
+
+
+def test_densification_indicators_are_norms_of_the_per_view_gradients():
+    """spatial position gradient magnitude plus the mu_t gradient as density-control indicators.  Pinned by
+    their definition from quantities that are themselves pinned by finite differences: per view |dL/d(u,v)| and |dL/dmu_t|,
+    summed over views, with the visibility count."""
+    sc = scenes.multiview_video(N=300, width=96, height=64, n_views=3)
+    acc = np.zeros((sc.N, 3))
+    expect = np.zeros((sc.N, 3))
+    for vi in range(3):
+        o = oracle_for(sc, vi)
+        o.forward()
+        G = scenes.upstream_normal(vi, 96, 64).astype(np.float64)
+        g = o.backward(G, densify=acc)
+        vis = o.prims().status == 0
+        expect[:, 0] += np.where(vis, np.linalg.norm(g["mean2d"], axis=1), 0.0)
+        expect[:, 1] += np.where(vis, np.abs(g["mean"][:, 3]), 0.0)
+        expect[:, 2] += vis
+    np.testing.assert_allclose(acc, expect, rtol=1e-12, atol=1e-15)
+    assert acc[:, 2].max() == 3 and acc[:, 2].min() == 0 and acc[:, 0].max() > 0 and acc[:, 1].max() > 0
