@@ -75,7 +75,10 @@ typedef struct {
  * into them: zero them once per optimisation step and the views of a batch sum (L324 "batch size 4"). */
 typedef struct {
   float *mean, *log_scale, *quat_l, *quat_r, *opacity_logit, *sh;
-  float *mean2d; /* [N,2] optional (NULL ok): dL/d(u,v), the densification signal (L197) */
+  float *mean2d;  /* [N,2] optional (NULL ok): dL/d(u,v) in pixels, summed over views (L197)                          */
+  float *densify; /* [N,3] optional (NULL ok): density-control indicators, accumulated once per backward of a view the
+                     primitive is visible in (L197 "gradients of mu_t as an additional density control indicator"):
+                     [0] += |dL/d(u,v)| of this view, [1] += |dL/dmu_t| of this view, [2] += 1                          */
 } fdgs_grads;
 
 /* Fills the defaults listed above.  Returns FDGS_ERR_INVALID if cfg is NULL. */

@@ -358,6 +358,10 @@ __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, cons
     float4* dst = reinterpret_cast<float4*>(gr.mean) + i;
     float4 m = *dst;
     m.x += d_muc[0]; m.y += d_muc[1]; m.z += d_muc[2]; m.w += -d_dt;
+    if (gr.densify) {   // density-control indicators of this view
+      float* dn = gr.densify + (size_t)3 * i;
+      dn[0] += sqrtf(g_u * g_u + g_v * g_v); dn[1] += fabsf(d_dt); dn[2] += 1.0f;
+    }
     *dst = m;
   }
   // ---- M = R4 diag(s) ------------------------------------------------------------------------

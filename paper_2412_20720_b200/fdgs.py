@@ -45,7 +45,7 @@ class CConfig(C.Structure):
 
 
 class CGrads(C.Structure):
-    _fields_ = [(k, C.c_void_p) for k in ("mean", "log_scale", "quat_l", "quat_r", "opacity_logit", "sh", "mean2d")]
+    _fields_ = [(k, C.c_void_p) for k in ("mean", "log_scale", "quat_l", "quat_r", "opacity_logit", "sh", "mean2d", "densify")]
 
 
 class CViewBuffers(C.Structure):
@@ -203,16 +203,17 @@ class DeviceScene:
         return CScene(self.N, self.sh_degree, self.n_time, _ptr(self.mean), _ptr(self.log_scale), _ptr(self.quat_l),
                       _ptr(self.quat_r), _ptr(self.opacity_logit), _ptr(self.sh))
 
-    def zero_grads(self, with_mean2d=False):
+    def zero_grads(self, with_mean2d=False, with_densify=False):
         import torch
         g = {k: torch.zeros_like(getattr(self, k)) for k in ("mean", "log_scale", "quat_l", "quat_r", "opacity_logit", "sh")}
         g["mean2d"] = torch.zeros((self.N, 2), device=self.mean.device) if with_mean2d else None
+        g["densify"] = torch.zeros((self.N, 3), device=self.mean.device) if with_densify else None
         return g
 
 
 def grads_struct(g: dict) -> CGrads:
     return CGrads(_ptr(g["mean"]), _ptr(g["log_scale"]), _ptr(g["quat_l"]), _ptr(g["quat_r"]), _ptr(g["opacity_logit"]),
-                  _ptr(g["sh"]), _ptr(g.get("mean2d")))
+                  _ptr(g["sh"]), _ptr(g.get("mean2d")), _ptr(g.get("densify")))
 
 
 def workspace_bytes(N, K, width, height, pair_capacity) -> int:

@@ -60,7 +60,7 @@ def test_struct_layouts_match_the_header():
     assert C.sizeof(fdgs.CScene) == 64           # 3 x int32 (+pad) + 6 pointers
     assert C.sizeof(fdgs.CView) == 64 + 16 + 8 + 8 + 12
     assert C.sizeof(fdgs.CConfig) == 32
-    assert C.sizeof(fdgs.CGrads) == 56
+    assert C.sizeof(fdgs.CGrads) == 64
     assert C.sizeof(fdgs.CViewBuffers) == 64
 
 
