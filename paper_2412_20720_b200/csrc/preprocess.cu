@@ -21,12 +21,17 @@ __device__ __forceinline__ void colour_forward(const float* __restrict__ coef, c
   for (int n = 0; n < n_time; ++n) {
     const float cn = cospif(2.0f * (float)n * dt_over_T);
     const float* cf = coef + (size_t)n * KD * 3;
-    if (KD % 4 == 0) {       // 3 x float4 = 4 coefficients x 3 channels; record stride 12K B keeps 16-B alignment
+    if constexpr (KD % 4 == 0) {       // 3 x float4 = 4 coefficients x 3 channels; record stride 12K B keeps 16-B alignment
+      // all loads of this Fourier order are issued before the first use (volatile asm keeps them together; left alone the
+      // compiler recycles four registers and serialises the block into three dependent round trips)
+      float4 f[3 * (KD / 4)];
+#pragma unroll
+      for (int q = 0; q < 3 * (KD / 4); ++q)
+        asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(f[q].x), "=f"(f[q].y), "=f"(f[q].z), "=f"(f[q].w)
+                     : "l"(reinterpret_cast<const float4*>(cf) + q));
 #pragma unroll
       for (int k4 = 0; k4 < KD / 4; ++k4) {
-        const float4 f0 = __ldg(reinterpret_cast<const float4*>(cf) + 3 * k4);
-        const float4 f1 = __ldg(reinterpret_cast<const float4*>(cf) + 3 * k4 + 1);
-        const float4 f2 = __ldg(reinterpret_cast<const float4*>(cf) + 3 * k4 + 2);
+        const float4 f0 = f[3 * k4], f1 = f[3 * k4 + 1], f2 = f[3 * k4 + 2];
         const float y0 = cn * Y[4 * k4], y1 = cn * Y[4 * k4 + 1], y2 = cn * Y[4 * k4 + 2], y3 = cn * Y[4 * k4 + 3];
         acc[0] = fmaf(f0.x, y0, acc[0]); acc[1] = fmaf(f0.y, y0, acc[1]); acc[2] = fmaf(f0.z, y0, acc[2]);
         acc[0] = fmaf(f0.w, y1, acc[0]); acc[1] = fmaf(f1.x, y1, acc[1]); acc[2] = fmaf(f1.y, y1, acc[2]);

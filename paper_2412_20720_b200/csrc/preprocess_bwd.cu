@@ -243,6 +243,14 @@ __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, cons
     const float4 mean = ldg4b(sc.mean, i), ls = ldg4b(sc.log_scale, i), qlr = ldg4b(sc.quat_l, i), qrr = ldg4b(sc.quat_r, i);
     if (geom_forward(mean, ls, qlr, qrr, __ldg(sc.opacity_logit + i), vp, cp, g) != G_VISIBLE) return;
   }
+  // the gradient rows this thread will read-modify-write: requested now, consumed at the end of the chain (the compiler
+  // would otherwise issue each load right before its use: five serial round trips on a 12-warps-per-SM kernel)
+  float4 acc_mean, acc_ls, acc_ql, acc_qr;
+  ld_f4(reinterpret_cast<const float4*>(gr.mean) + i, acc_mean);
+  ld_f4(reinterpret_cast<const float4*>(gr.log_scale) + i, acc_ls);
+  ld_f4(reinterpret_cast<const float4*>(gr.quat_l) + i, acc_ql);
+  ld_f4(reinterpret_cast<const float4*>(gr.quat_r) + i, acc_qr);
+  const float acc_logit = gr.opacity_logit[i];
   const float* gp = g9 + (size_t)9 * i;
   const float g_u = gp[0], g_v = gp[1], g_A = gp[2], g_B = gp[3], g_C = gp[4], g_o = gp[5];
   if (gr.mean2d) { gr.mean2d[2 * i] += g_u; gr.mean2d[2 * i + 1] += g_v; }
@@ -319,7 +327,7 @@ __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, cons
 
   // ---- o = sigmoid(logit) w,  w = exp(-Delta^2 / 2b) -----------------------------------------
   const float inv_b = 1.0f / g.b;
-  gr.opacity_logit[i] += g_o * g.w * g.sig * (1.f - g.sig);
+  gr.opacity_logit[i] = acc_logit + g_o * g.w * g.sig * (1.f - g.sig);
   {
     const float d_w = g_o * g.sig;
     d_dt += d_w * g.w * (-g.dt * inv_b);
@@ -358,7 +366,7 @@ __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, cons
   // ---- mean ---------------------------------------------------------------------------------
   {
     float4* dst = reinterpret_cast<float4*>(gr.mean) + i;
-    float4 m = *dst;
+    float4 m = acc_mean;
     m.x += d_muc[0]; m.y += d_muc[1]; m.z += d_muc[2]; m.w += -d_dt;
     if (gr.densify) {   // density-control indicators of this view
       float* dn = gr.densify + (size_t)3 * i;
@@ -378,7 +386,7 @@ __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, cons
       dls[k] = ds * g.s[k];
     }
     float4* dst = reinterpret_cast<float4*>(gr.log_scale) + i;
-    float4 m = *dst;
+    float4 m = acc_ls;
     m.x += dls[0]; m.y += dls[1]; m.z += dls[2]; m.w += dls[3];
     *dst = m;
   }
@@ -407,7 +415,7 @@ __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, cons
     for (int k = 0; k < 4; ++k) { dl = fmaf(g.ql[k], dql[k], dl); dr = fmaf(g.qr[k], dqr[k], dr); }
     float4* dstl = reinterpret_cast<float4*>(gr.quat_l) + i;
     float4* dstr = reinterpret_cast<float4*>(gr.quat_r) + i;
-    float4 ml = *dstl, mr = *dstr;
+    float4 ml = acc_ql, mr = acc_qr;
     ml.x += (dql[0] - g.ql[0] * dl) * g.inv_nl; ml.y += (dql[1] - g.ql[1] * dl) * g.inv_nl;
     ml.z += (dql[2] - g.ql[2] * dl) * g.inv_nl; ml.w += (dql[3] - g.ql[3] * dl) * g.inv_nl;
     mr.x += (dqr[0] - g.qr[0] * dr) * g.inv_nr; mr.y += (dqr[1] - g.qr[1] * dr) * g.inv_nr;
