@@ -26,8 +26,9 @@ WORKLOAD = "cfg3_video: N=1M, K=48 (L=3 x n_time=3), 1352x1014, fov 60, 4 jitter
 PAIR_CAPACITY = 16 * 1024 * 1024
 SM_COUNT, LANES_PER_SM, SM_MAX_HZ = 148, 128, 1.965e9
 ALU_PEAK_TLANE = SM_COUNT * LANES_PER_SM * SM_MAX_HZ / 1e12      # 37.2 T lane-instructions/s
-# DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/r1_blend_bwd2_ncu_full.md)
-BLEND_BWD_NCU_TRAFFIC_BYTES = 94.9e6
+# DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
+# (profiles/r1_all_kernels_ncu_full_final.md: 87.5 MB read + 5.1 MB written)
+BLEND_BWD_NCU_TRAFFIC_BYTES = 92.6e6
 
 
 def hbm_peak():

@@ -5,7 +5,10 @@
  *
  * Everything behind these entry points is hand-written CUDA for sm_100a (no CPU fallback, no
  * library kernels).  The library never allocates device memory, never throws across the ABI and
- * never synchronises the stream unless a `_host` out-pointer is given.
+ * never synchronises the stream unless a `_host` out-pointer is given.  fdgs_preprocess / fdgs_render_forward(_aux) /
+ * fdgs_l1_loss / fdgs_render_backward(_aux) issue only kernels and device memsets on the caller's stream, so the sequence
+ * can be captured into a CUDA graph.  The library keeps a little process-global state (launch counter, timing events,
+ * worker streams of fdgs_step_batch / fdgs_step_host): calls are not re-entrant across host threads.
  *
  * Conventions
  *   - Every pointer is a DEVICE pointer unless its name ends in `_host`.  fdgs_view and

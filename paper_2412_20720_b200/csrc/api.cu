@@ -62,6 +62,10 @@ static void make_params(const fdgs_view* v, const fdgs_config* c, ViewParams& vp
   cp.log2_alpha_min = c->alpha_min > 0.f ? log2f(c->alpha_min) * (1.0f + 1e-6f) - 1e-6f : -INFINITY;
 }
 
+__global__ void init_header_kernel(WsHeader* hdr, long long N, long long K, long long W, long long H, long long cap, long long tiles) {
+  hdr->N = N; hdr->K = K; hdr->W = W; hdr->H = H; hdr->pair_capacity = cap; hdr->tiles = tiles;
+}
+
 // ---- parity exports -----------------------------------------------------------------------------
 __global__ void export_records_kernel(const SplatRec* __restrict__ rec, const unsigned int* __restrict__ tiles_touched, const int N,
                                       float* __restrict__ dst) {
@@ -149,9 +153,10 @@ int fdgs_preprocess(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config*
   make_params(v, c, vp, cp);
   // header (tickets, counters), coverage difference grid and scan states start from zero
   FDGS_CUDA(cudaMemsetAsync(ws_ptr, 0, ws.zero_bytes, st), "memset(header)");
-  WsHeader h; memset(&h, 0, sizeof(h));
-  h.N = sc->N; h.K = K; h.W = v->width; h.H = v->height; h.pair_capacity = cap; h.tiles = (long long)vp.tiles_x * vp.tiles_y;
-  FDGS_CUDA(cudaMemcpyAsync(&ws.hdr->N, &h.N, 6 * sizeof(long long), cudaMemcpyHostToDevice, st), "memcpy(header)");
+  // layout mirror for fdgs_debug_export: written by a kernel from its by-value arguments (no host-memory copy on the
+  // stream, so the whole call sequence can be captured into a CUDA graph)
+  init_header_kernel<<<1, 1, 0, st>>>(ws.hdr, sc->N, K, v->width, v->height, cap, (long long)vp.tiles_x * vp.tiles_y);
+  ++g_launches;
   mark(EV_PRE0, st);
   launch_preprocess_fwd(*sc, vp, cp, ws, st);                       // A1-A4 (+ coverage grid)
   mark(EV_PRE1, st);

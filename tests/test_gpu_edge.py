@@ -248,3 +248,38 @@ def test_densification_indicators_match_the_oracle():
     bs.step([fdgs.make_view(v) for v in sc.views], g2)
     torch.cuda.synchronize()
     assert torch.equal(g2["densify"][:, 2], g["densify"][:, 2]) and float(g2["densify"][:, 1].max()) > 0
+
+
+def test_whole_step_replays_from_a_cuda_graph():
+    """The call sequence issues no host-memory copies and no synchronisation: preprocess + forward + loss + backward is
+    captured once into a CUDA graph and replayed with the same result."""
+    import gpu_helpers as gh
+    import torch
+    from paper_2412_20720_b200 import fdgs
+    sc = scenes.multiview_video(N=8000, width=160, height=112, n_views=1)
+    ds = fdgs.DeviceScene.from_scene(sc)
+    r = fdgs.Renderer(ds, 160, 112, 1 << 20)
+    cv = fdgs.make_view(sc.views[0])
+    tgt = torch.from_numpy(scenes.target_image(3, 0, 160, 112)).cuda()
+    g_ref = ds.zero_grads()
+    r.preprocess(cv); r.forward(cv); r.loss.zero_(); r.l1_loss(tgt); r.backward(cv, r.dL_dimage, g_ref)
+    torch.cuda.synchronize()
+    img_ref = r.image.clone()
+    g = ds.zero_grads()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            r.preprocess(cv); r.forward(cv); r.loss.zero_(); r.l1_loss(tgt); r.backward(cv, r.dL_dimage, g)
+    torch.cuda.current_stream().wait_stream(side)
+    for _ in range(3):
+        for v in g.values():
+            if v is not None:
+                v.zero_()
+        r.image.zero_()
+        graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(r.image, img_ref)
+    for k in ("mean", "log_scale", "quat_l", "quat_r", "opacity_logit", "sh"):
+        assert gh.rel_l2(g[k].cpu().numpy(), g_ref[k].cpu().numpy()) < 1e-5, k
