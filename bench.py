@@ -54,7 +54,8 @@ def stage_rooflines(stage, work, N, K, n_views):
     out = {}
     for k, b in byts.items():
         gbs = b / (stage[k] * 1e-3) / 1e9
-        out[k] = {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "algorithmic_bytes": b}
+        out[k] = {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "frac_of_8tbs_spec": gbs / 8000.0,
+                  "algorithmic_bytes": b}
     out["peak_source_hbm"] = src
     return out
 
