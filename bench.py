@@ -181,13 +181,11 @@ def run_fdgs(args):
             if g is not None:
                 g.zero_()
 
-    def step_device():       # fdgs_step_batch, targets resident in HBM, nothing read back
-        zero_grads()
-        bs.step(cviews, grads)
+    def step_device():       # fdgs_step_batch, targets resident in HBM, nothing read back; gradients zeroed inside the call
+        bs.step(cviews, grads, zero_grads=True)
 
     def step_host():         # fdgs_step_batch with pinned HOST targets copied in and the four losses copied back (synchronises)
-        zero_grads()
-        bs.step(cviews, grads, targets_host=targets_host, loss_host=loss_host)
+        bs.step(cviews, grads, targets_host=targets_host, loss_host=loss_host, zero_grads=True)
 
     def forward_only(cv):
         r.preprocess(cv)

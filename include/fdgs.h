@@ -161,8 +161,11 @@ int fdgs_step_host(const fdgs_scene *scene, const fdgs_view *view_host, const fd
  *                             == NULL: target_dev already holds the target.
  *   loss_dev [num_views] device floats: loss of each view (overwritten).
  *   loss_host != NULL: the losses are copied back and `cuda_stream` is synchronised; NULL: fully asynchronous.
+ *   flags: FDGS_STEP_ZERO_GRADS = the six parameter-gradient arrays (and mean2d if given; not densify, which is meant to
+ *          accumulate over steps) are zeroed inside the call, on a side stream, hidden under the forward passes.
  * 1 <= num_views <= FDGS_MAX_BATCH; workspaces must be distinct. */
 #define FDGS_MAX_BATCH 8
+#define FDGS_STEP_ZERO_GRADS 1
 typedef struct {
   void *ws; size_t ws_bytes;     /* workspace of this view (fdgs_workspace_bytes)                      */
   const float *target_host;      /* see above                                                          */
@@ -173,7 +176,7 @@ typedef struct {
 } fdgs_view_buffers;
 int fdgs_step_batch(const fdgs_scene *scene, const fdgs_view *views_host, int32_t num_views, const fdgs_config *cfg_host,
                     int64_t pair_capacity, const fdgs_view_buffers *bufs_host, void *cuda_stream, float *loss_dev,
-                    const fdgs_grads *grads_host, float *loss_host);
+                    const fdgs_grads *grads_host, float *loss_host, int32_t flags);
 
 /* Parity hooks: copy one intermediate of the last calls on `ws` to dst (device memory).  Synchronises. */
 #define FDGS_EXPORT_STATUS 0        /* int64[4]: D, num_visible, overflow flag, pair_capacity               */

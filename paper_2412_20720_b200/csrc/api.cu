@@ -333,12 +333,13 @@ int fdgs_step_host(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* 
 }
 
 // Worker streams of fdgs_step_batch (one per view of the batch), created on first use.
-static cudaStream_t g_worker[FDGS_MAX_BATCH];
-static cudaEvent_t g_batch_fork = nullptr, g_b2_done[FDGS_MAX_BATCH];
+static cudaStream_t g_worker[FDGS_MAX_BATCH], g_zero_stream = nullptr;
+static cudaEvent_t g_batch_fork = nullptr, g_b2_done[FDGS_MAX_BATCH], g_zero_done = nullptr;
 
 int fdgs_step_batch(const fdgs_scene* sc, const fdgs_view* views, int32_t num_views, const fdgs_config* c, int64_t cap,
-                    const fdgs_view_buffers* bufs, void* stream, float* loss_dev, const fdgs_grads* g, float* loss_host) {
+                    const fdgs_view_buffers* bufs, void* stream, float* loss_dev, const fdgs_grads* g, float* loss_host, int32_t flags) {
   if (!sc || !views || !c || !bufs || !loss_dev || !g || num_views < 1 || num_views > FDGS_MAX_BATCH) return FDGS_ERR_INVALID;
+  if (sc->N > 0 && (!g->mean || !g->log_scale || !g->quat_l || !g->quat_r || !g->opacity_logit || !g->sh)) return FDGS_ERR_INVALID;
   for (int i = 0; i < num_views; ++i) {
     const fdgs_view_buffers& b = bufs[i];
     if (!b.ws || !b.target_dev || !b.image || !b.final_T || !b.n_contrib || !b.dL_dimage) return FDGS_ERR_INVALID;
@@ -350,9 +351,24 @@ int fdgs_step_batch(const fdgs_scene* sc, const fdgs_view* views, int32_t num_vi
       FDGS_CUDA(cudaStreamCreateWithFlags(&g_worker[i], cudaStreamNonBlocking), "worker stream");
       FDGS_CUDA(cudaEventCreateWithFlags(&g_b2_done[i], cudaEventDisableTiming), "worker event");
     }
+    FDGS_CUDA(cudaStreamCreateWithFlags(&g_zero_stream, cudaStreamNonBlocking), "zero stream");
+    FDGS_CUDA(cudaEventCreateWithFlags(&g_zero_done, cudaEventDisableTiming), "zero event");
     FDGS_CUDA(cudaEventCreateWithFlags(&g_batch_fork, cudaEventDisableTiming), "fork event");
   }
   FDGS_CUDA(cudaEventRecord(g_batch_fork, st), "fork");
+  const bool zero = (flags & FDGS_STEP_ZERO_GRADS) && sc->N > 0;
+  if (zero) {   // the gradient arrays are first touched by the first view's backward preprocess: zeroing them hides under the forward passes
+    const size_t N = (size_t)sc->N, K = (size_t)sc->n_time * (sc->sh_degree + 1) * (sc->sh_degree + 1);
+    FDGS_CUDA(cudaStreamWaitEvent(g_zero_stream, g_batch_fork, 0), "fork wait");
+    FDGS_CUDA(cudaMemsetAsync(g->mean, 0, 16 * N, g_zero_stream), "zero grads");
+    FDGS_CUDA(cudaMemsetAsync(g->log_scale, 0, 16 * N, g_zero_stream), "zero grads");
+    FDGS_CUDA(cudaMemsetAsync(g->quat_l, 0, 16 * N, g_zero_stream), "zero grads");
+    FDGS_CUDA(cudaMemsetAsync(g->quat_r, 0, 16 * N, g_zero_stream), "zero grads");
+    FDGS_CUDA(cudaMemsetAsync(g->opacity_logit, 0, 4 * N, g_zero_stream), "zero grads");
+    FDGS_CUDA(cudaMemsetAsync(g->sh, 0, 12 * K * N, g_zero_stream), "zero grads");
+    if (g->mean2d) FDGS_CUDA(cudaMemsetAsync(g->mean2d, 0, 8 * N, g_zero_stream), "zero grads");
+    FDGS_CUDA(cudaEventRecord(g_zero_done, g_zero_stream), "zero done");
+  }
   for (int i = 0; i < num_views; ++i) {
     const fdgs_view_buffers& b = bufs[i];
     cudaStream_t w = g_worker[i];
@@ -367,7 +383,7 @@ int fdgs_step_batch(const fdgs_scene* sc, const fdgs_view* views, int32_t num_vi
     rc = fdgs_l1_loss(b.image, b.target_dev, (int64_t)count, b.dL_dimage, loss_dev + i, w);
     if (rc) return rc;
     // blend backward of this view overlaps everything of the others; the gradient accumulation (B2) is chained
-    rc = backward_impl(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, b.dL_dimage, b.final_T, b.n_contrib, g, i > 0 ? g_b2_done[i - 1] : nullptr);
+    rc = backward_impl(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, b.dL_dimage, b.final_T, b.n_contrib, g, i > 0 ? g_b2_done[i - 1] : (zero ? g_zero_done : nullptr));
     if (rc) return rc;
     FDGS_CUDA(cudaEventRecord(g_b2_done[i], w), "record B2");
   }

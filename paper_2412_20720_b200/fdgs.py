@@ -83,7 +83,7 @@ def load():
     lib.fdgs_step_host.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, vp, vp, vp, vp,
                                    vp, vp, vp, C.POINTER(CGrads), vp]
     lib.fdgs_step_batch.argtypes = [C.POINTER(CScene), C.POINTER(CView), i32, C.POINTER(CConfig), i64, C.POINTER(CViewBuffers), vp, vp,
-                                    C.POINTER(CGrads), vp]
+                                    C.POINTER(CGrads), vp, i32]
     lib.fdgs_debug_cull_status.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, vp]
     lib.fdgs_debug_measure_peaks.argtypes = [vp, sz, vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
     lib.fdgs_debug_export.argtypes = [vp, sz, C.c_int, vp, sz, vp]
@@ -371,10 +371,10 @@ class BatchStep:
         self.loss = torch.zeros(num_views, dtype=torch.float32, device=dscene.mean.device)
         self._cs = dscene.c_struct()
 
-    def step(self, cviews, grads: dict, targets_host=None, loss_host=None):
+    def step(self, cviews, grads: dict, targets_host=None, loss_host=None, zero_grads=False):
         """targets_host: list of pinned [3,H,W] host tensors (copied inside the call) or None if every renderer's
         target_dev already holds its target.  loss_host: pinned float tensor [num_views] (copied back, synchronises)
-        or None (asynchronous)."""
+        or None (asynchronous).  zero_grads: the library zeroes the gradient arrays itself (FDGS_STEP_ZERO_GRADS)."""
         n = self.num_views
         views = (CView * n)(*cviews)
         bufs = (CViewBuffers * n)()
@@ -384,6 +384,6 @@ class BatchStep:
                                    r.dL_dimage.data_ptr())
         cg = grads_struct(grads)
         rc = self.lib.fdgs_step_batch(C.byref(self._cs), views, n, C.byref(self.cfg), self.cap, bufs, _stream(), self.loss.data_ptr(),
-                                      C.byref(cg), _ptr(loss_host))
+                                      C.byref(cg), _ptr(loss_host), 1 if zero_grads else 0)
         if rc:
             raise FdgsError(rc, "fdgs_step_batch")

@@ -167,9 +167,9 @@ def test_step_batch_matches_view_by_view():
     for k in ("mean", "log_scale", "quat_l", "quat_r", "opacity_logit", "sh"):
         assert gh.rel_l2(g[k].cpu().numpy(), g_ref[k].cpu().numpy()) < 1e-5, k
     assert np.allclose(loss_host.numpy(), np.array(losses_ref), rtol=1e-5)
-    # device-resident targets, asynchronous
-    g2 = ds.zero_grads()
-    bs.step(cvs, g2)
+    # device-resident targets, asynchronous, gradients zeroed by the library (they start from garbage here)
+    g2 = {k: (torch.full_like(v, 7.0) if v is not None else None) for k, v in ds.zero_grads().items()}
+    bs.step(cvs, g2, zero_grads=True)
     torch.cuda.synchronize()
     assert gh.rel_l2(g2["sh"].cpu().numpy(), g_ref["sh"].cpu().numpy()) < 1e-5
     with pytest.raises(ValueError):
