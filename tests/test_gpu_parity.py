@@ -225,3 +225,14 @@ def test_aux_channels_cfg1():
 def test_aux_channels_cfg2_ragged_and_cfg4_heavy_tails():
     _aux_parity(scenes.single_object(N=20000, width=250, height=190), "aux cfg2 20k 250x190")
     _aux_parity(scenes.driving(N=40000, width=480, height=320, n_views=1), "aux cfg4 40k 480x320")
+
+
+def test_anisotropic_intrinsics_offcentre_principal_point_rotated_camera():
+    """fx != fy, principal point away from the image centre, rotated / translated camera, coloured background, period != 1."""
+    base = scenes.fd_scene(100, 8)
+    big = scenes.tiny()
+    v = base.views[0]
+    view = scenes.View(v.view, v.fx * 1.15, v.fy * 0.9, v.cx + 5.25, v.cy - 3.5, 80, 56, 0.47, 0.7, (0.3, 0.1, 0.6)).as_fp32()
+    sc = scenes.Scene("intr", big.sh_degree, big.n_time, big.mean, big.log_scale, big.quat_l, big.quat_r, big.opacity_logit,
+                      big.sh, [view], 11)
+    _full_parity(sc, label="fx!=fy, off-centre, rotated camera")
