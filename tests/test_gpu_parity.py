@@ -236,3 +236,35 @@ def test_anisotropic_intrinsics_offcentre_principal_point_rotated_camera():
     sc = scenes.Scene("intr", big.sh_degree, big.n_time, big.mean, big.log_scale, big.quat_l, big.quat_r, big.opacity_logit,
                       big.sh, [view], 11)
     _full_parity(sc, label="fx!=fy, off-centre, rotated camera")
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3, 4, 5, 6])
+def test_fuzz_shapes_and_degrees(seed):
+    """Seeded random small cases: ragged image sizes (1 tile to a few dozen), N from a handful to a few thousand, every SH
+    degree and 1-4 Fourier orders, thresholds on / off, random pose, time and background."""
+    u = scenes.uniform(seed, 500, 16)
+    W, H = 17 + int(u[0] * 140), 9 + int(u[1] * 100)
+    N = 3 + int(u[2] ** 2 * 3000)
+    L, n_time = int(u[3] * 4) % 4, 1 + int(u[4] * 4) % 4
+    K = n_time * (L + 1) ** 2
+    mean = np.stack([2 * scenes.uniform(seed, 1, N) - 1, 2 * scenes.uniform(seed, 2, N) - 1, 2 * scenes.uniform(seed, 3, N) - 1,
+                     scenes.uniform(seed, 4, N)], axis=1)
+    ls = np.stack([-2.6 + 0.5 * scenes.normal(seed, 10 + k, N) for k in range(3)] + [-1.2 + 0.5 * scenes.normal(seed, 13, N)], axis=1)
+    ql = np.stack([scenes.normal(seed, 20 + k, N) for k in range(4)], axis=1)
+    qr = np.stack([scenes.normal(seed, 24 + k, N) for k in range(4)], axis=1)
+    logit = scenes.normal(seed, 30, N)
+    sh = 0.08 * scenes.normal(seed, 40, N * K * 3).reshape(N, K, 3)
+    sh[:, 0, :] += 0.6
+    fx = 0.5 * W / np.tan(np.deg2rad(20 + 30 * u[5]))
+    V = np.eye(4)
+    ang, axis = 0.5 * (u[6] - 0.5), np.array([u[7] - 0.5, u[8] - 0.5, u[9] - 0.5]) + 1e-3
+    axis = axis / np.linalg.norm(axis)
+    Kx = np.array([[0, -axis[2], axis[1]], [axis[2], 0, -axis[0]], [-axis[1], axis[0], 0]])
+    V[:3, :3] = np.eye(3) + np.sin(ang) * Kx + (1 - np.cos(ang)) * (Kx @ Kx)
+    V[:3, 3] = [0.3 * (u[10] - 0.5), 0.3 * (u[11] - 0.5), 3.0 + 2.0 * u[12]]
+    view = scenes.View(V.astype(np.float32), fx, fx * (0.9 + 0.2 * u[13]), 0.5 * W + 3 * (u[14] - 0.5), 0.5 * H, W, H, float(u[15]),
+                       0.5 + float(u[0]), (float(u[1]), float(u[2]), float(u[3]))).as_fp32()
+    f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+    sc = scenes.Scene("fuzz", L, n_time, f32(mean), f32(ls), f32(ql), f32(qr), f32(logit), f32(sh), [view], 100 + seed)
+    cfg = dict(alpha_min=0.0, transmittance_min=0.0) if seed % 3 == 0 else (dict(marginal_min=0.0) if seed % 3 == 1 else None)
+    _full_parity(sc, cfg=cfg, label=f"fuzz seed {seed}: N={N} {W}x{H} L={L} n_time={n_time} cfg={cfg}")
