@@ -320,7 +320,7 @@ __global__ void __launch_bounds__(256 / PX) blend_bwd_kernel(const uint2* __rest
       float out[9];
       out[0] = -fmaf(A, Sx, B * Sy); out[1] = -fmaf(B, Sx, C * Sy);
       out[2] = -0.5f * Sxx; out[3] = -Sxy; out[4] = -0.5f * Syy;
-      out[5] = S1 * exp2f(-sm.s1[j].y);
+      out[5] = S1 != 0.f ? S1 * exp2f(-sm.s1[j].y) : 0.f;   // o may underflow to 0 (marginal filter off): then nothing composited, S1 == 0
       out[6] = sm.acc[5 * ACC_STRIDE + j]; out[7] = sm.acc[6 * ACC_STRIDE + j]; out[8] = sm.acc[7 * ACC_STRIDE + j];
       float* dst = g9 + (size_t)9 * sm.id[j];
 #pragma unroll
@@ -532,7 +532,7 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
       float out[9];
       out[0] = -fmaf(A, Sx, B * Sy); out[1] = -fmaf(B, Sx, C * Sy);
       out[2] = -0.5f * Sxx; out[3] = -Sxy; out[4] = -0.5f * Syy;
-      out[5] = S1 * exp2f(-sm.s1[j].y);
+      out[5] = S1 != 0.f ? S1 * exp2f(-sm.s1[j].y) : 0.f;   // o may underflow to 0 (marginal filter off): then nothing composited, S1 == 0
       out[6] = sm.acc[5 * ACC_STRIDE + j]; out[7] = sm.acc[6 * ACC_STRIDE + j]; out[8] = sm.acc[7 * ACC_STRIDE + j];
       float* dst = g9 + (size_t)9 * sm.id[j];
 #pragma unroll

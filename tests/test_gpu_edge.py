@@ -283,3 +283,18 @@ def test_whole_step_replays_from_a_cuda_graph():
     assert torch.equal(r.image, img_ref)
     for k in ("mean", "log_scale", "quat_l", "quat_r", "opacity_logit", "sh"):
         assert gh.rel_l2(g[k].cpu().numpy(), g_ref[k].cpu().numpy()) < 1e-5, k
+
+
+def test_marginal_filter_off_with_underflowing_weight_gives_finite_zero_gradients():
+    """marginal_min = 0 (urban variant): a primitive 60 sigma away in time has o = sigmoid * w = 0 in fp32; it
+    is listed, composites nothing, and its gradients are exactly zero (regression: dL/do = S1 / o used to be 0 * inf)."""
+    import gpu_helpers as gh
+    sc = _f32(hand_scene([(0.0, 0.0, 0.0, 0.5), (0.1, 0.0, 0.5, 30.5)], [[-1.5, -1.5, -1.5, -0.7]] * 2, logit=[0.2, 0.4], sh=np.full((2, 1, 3), 1.0)))
+    out = gh.gpu_run(sc, sc.views[0], cfg_overrides=dict(marginal_min=0.0), dL=np.ones((3, 64, 64)))
+    assert out["num_visible"] == 2
+    for k, g in out["grads"].items():
+        if g is not None:
+            assert np.isfinite(g).all(), k
+    assert np.abs(out["grads"]["mean"][1]).max() == 0 and np.abs(out["grads"]["sh"][1]).max() == 0
+    assert np.abs(out["grads"]["mean"][0]).max() > 0
+    assert np.isfinite(out["g9"]).all()
