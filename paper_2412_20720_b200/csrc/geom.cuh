@@ -22,7 +22,7 @@ struct Geom {
   float xr, yr; bool clampx, clampy;
   float T[2][3], Bm[2][4];
   float a2, b2, c2, det;   // Sigma_2d entries (with dilation) and determinant
-  float sig;               // sigmoid(logit)
+  float sig, sig_neg;      // sigmoid(logit), sigmoid(-logit) = 1 - sigmoid(logit) without the cancellation
 };
 
 enum GeomStatus { G_VISIBLE = 0, G_CULL_TIME = 1, G_CULL_NEAR = 2, G_CULL_RECT = 3, G_CULL_NONFINITE = 4 };
@@ -137,6 +137,7 @@ __device__ __forceinline__ int geom_forward(const float4 mean, const float4 ls, 
   g.det = fmaf(cp.dilation, cp.dilation + n0 + n1, minors);
   if (!(g.det > 0.f) || !isfinite(g.det)) return G_CULL_NONFINITE;
   g.sig = 1.0f / (1.0f + expf(-logit));
+  g.sig_neg = 1.0f / (1.0f + expf(logit));
   return G_VISIBLE;
 }
 

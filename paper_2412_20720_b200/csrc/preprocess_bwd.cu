@@ -327,7 +327,7 @@ __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, cons
 
   // ---- o = sigmoid(logit) w,  w = exp(-Delta^2 / 2b) -----------------------------------------
   const float inv_b = 1.0f / g.b;
-  gr.opacity_logit[i] = acc_logit + g_o * g.w * g.sig * (1.f - g.sig);
+  gr.opacity_logit[i] = acc_logit + g_o * g.w * g.sig * g.sig_neg;
   {
     const float d_w = g_o * g.sig;
     d_dt += d_w * g.w * (-g.dt * inv_b);

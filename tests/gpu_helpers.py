@@ -61,7 +61,11 @@ def compare_prims(gpu, P, report):
         assert rel(rec[:, 9], P.p_cam[both][:, 2]).max() < 1e-5
         report["w_max_rel"] = float(rel(rec[:, 11], P.w[both], 1e-6).max())
         assert report["w_max_rel"] < 1e-5
-        assert np.abs(rec[:, 6:9] - P.rgb[both]).max() < 2e-5
+        # colour = 0.5 + sum of K terms coef * cos * Y: the fp32 error scales with the magnitude of the terms, not of the sum
+        sh = gpu["dscene"].sh.cpu().numpy().astype(np.float64)[both]
+        scale = 1.0 + np.abs(sh).sum(axis=1)
+        report["rgb_max_scaled"] = float((np.abs(rec[:, 6:9] - P.rgb[both]) / scale).max())
+        assert report["rgb_max_scaled"] < 1e-5
         nrm = np.sqrt(P.conic[both][:, 0] * P.conic[both][:, 2])[:, None]        # conic error relative to sqrt(A C)
         cerr = (np.abs(rec[:, 2:5] - P.conic[both]) / nrm).max(1)
         # primitives within a factor 2 of the near plane (z < 0.4): J ~ 1/z^2 amplifies the fp32 rounding of the camera-space
