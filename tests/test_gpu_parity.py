@@ -185,6 +185,8 @@ def _aux_parity(scene, label, view_index=0):
     dL = scenes.upstream_normal(scene.seed, W, H).astype(np.float64) / (3 * W * H)
     gD = scenes.normal(scene.seed, 210, W * H).reshape(H, W) / (W * H)
     gO = scenes.normal(scene.seed, 211, W * H).reshape(H, W) / (W * H)
+    keep_px = margin >= gh.MARGIN_TOL           # threshold-fragile pixels leave the loss on both sides (see _full_parity)
+    dL, gD, gO = dL * keep_px[None], gD * keep_px, gO * keep_px
     go = o.backward(dL, gD, gO)
     ds = fdgs.DeviceScene.from_scene(scene)
     r = fdgs.Renderer(ds, W, H, max(1 << 16, 64 * scene.N))
@@ -219,7 +221,9 @@ def _aux_parity(scene, label, view_index=0):
     g2 = ds.zero_grads()
     r.backward_aux(cv, torch.zeros_like(r.image), f32(gD), None, g2)
     torch.cuda.synchronize()
-    assert float(g2["sh"].abs().max()) == 0.0 and float(g2["mean"].abs().max()) > 0.0
+    assert float(g2["sh"].abs().max()) == 0.0
+    if np.abs(go["gz"]).max() > 0:
+        assert float(g2["mean"].abs().max()) > 0.0
 
 
 def test_aux_channels_cfg1():
