@@ -167,7 +167,5 @@ void launch_preprocess_bwd(const fdgs_scene& sc, const ViewParams& vp, const Cfg
                            const fdgs_grads& g, bool with_gz, cudaStream_t st);
 void launch_cull_status(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, unsigned char* dst, cudaStream_t st);
 void launch_l1_loss(const float* image, const float* target, long long count, float* dL, float* loss, cudaStream_t st);
-void launch_export_records(const Workspace& ws, int N, float* dst, cudaStream_t st);
-void launch_export_keys(const Workspace& ws, int l2_buf, unsigned long long* dst, cudaStream_t st);
 
 }  // namespace fdgs
