@@ -169,29 +169,4 @@ __device__ __forceinline__ void sh_basis(const float x, const float y, const flo
   }
 }
 
-// gradient wrt (x,y,z) of f = sum_k a[k] Y_k (polynomial extension)
-template <int KD>
-__device__ __forceinline__ void sh_grad(const float x, const float y, const float z, const float* a, float g[3]) {
-  float gx = 0.f, gy = 0.f, gz = 0.f;
-  if (KD > 1) { gy += -SH_C1 * a[1]; gz += SH_C1 * a[2]; gx += -SH_C1 * a[3]; }
-  if (KD > 4) {
-    gx += a[4] * SH_C2 * y;  gy += a[4] * SH_C2 * x;
-    gy += -a[5] * SH_C2 * z; gz += -a[5] * SH_C2 * y;
-    gx += -2.f * SH_C20 * a[6] * x; gy += -2.f * SH_C20 * a[6] * y; gz += 4.f * SH_C20 * a[6] * z;
-    gx += -a[7] * SH_C2 * z; gz += -a[7] * SH_C2 * x;
-    gx += 2.f * SH_C22 * a[8] * x; gy += -2.f * SH_C22 * a[8] * y;
-    if (KD > 9) {
-      const float xx = x * x, yy = y * y, zz = z * z;
-      gx += -a[9] * SH_C3 * 6.f * x * y;          gy += -a[9] * SH_C3 * 3.f * (xx - yy);
-      gx += a[10] * SH_C4 * y * z;                gy += a[10] * SH_C4 * x * z;                 gz += a[10] * SH_C4 * x * y;
-      gx += a[11] * SH_C5 * 2.f * x * y;          gy += -a[11] * SH_C5 * (4.f * zz - xx - 3.f * yy); gz += -a[11] * SH_C5 * 8.f * y * z;
-      gx += -a[12] * SH_C6 * 6.f * x * z;         gy += -a[12] * SH_C6 * 6.f * y * z;          gz += a[12] * SH_C6 * (6.f * zz - 3.f * xx - 3.f * yy);
-      gx += -a[13] * SH_C5 * (4.f * zz - 3.f * xx - yy); gy += a[13] * SH_C5 * 2.f * x * y;   gz += -a[13] * SH_C5 * 8.f * x * z;
-      gx += a[14] * SH_C4 * x * z;                gy += -a[14] * SH_C4 * y * z;                gz += a[14] * SH_C42 * (xx - yy);
-      gx += -a[15] * SH_C3 * 3.f * (xx - yy);     gy += a[15] * SH_C3 * 6.f * x * y;
-    }
-  }
-  g[0] = gx; g[1] = gy; g[2] = gz;
-}
-
 }  // namespace fdgs
