@@ -339,10 +339,10 @@ __global__ void __launch_bounds__(256 / PX) blend_bwd_kernel(const uint2* __rest
 // per-hit atomic of the direct kernel by one STS.128 and ~1/8 of a 300-instruction flush.
 constexpr int HROW = 36;   // float4 per buffered hit: 32 lanes + pad (144 words = 16 mod 32: quarter-warps hit 32 banks)
 
-template <int HBUF>        // hits buffered per warp (4, 8 or 16; 8 measured best: 4 flushes too often, 16 costs occupancy)
+template <int HBUF, bool GRED = false>   // hits buffered per warp (4, 8 or 16; 8 measured best: 4 flushes too often, 16 costs occupancy)
 struct Bwd2Shared {
   float4 s0[128], s1[128], s2[128];
-  float acc[10 * 129];     // nine sums of the colour path + (AUX) sum of wgt * dL/ddepth
+  float acc[GRED ? 1 : 10 * 129];     // nine sums of the colour path + (AUX) sum of wgt * dL/ddepth (unused with GRED)
   unsigned int id[128];
   int max_contrib;
   int hitj[4][HBUF];
@@ -350,8 +350,11 @@ struct Bwd2Shared {
   float4 pg[4][32][2];     // per warp, per lane: (gr0, gg0, gb0, gr1), (gg1, gb1, gD0, gD1)
 };
 
-template <int HBUF, bool AUX>
-__device__ __forceinline__ void bwd2_flush(Bwd2Shared<HBUF>& sm, const int warp, const int lane, const int n, const float sx0, const float sy0) {
+template <int HBUF, bool AUX, bool GRED> __device__ __forceinline__ void bwd2_emit_global(Bwd2Shared<HBUF, GRED>&, int, int, const float*, float* __restrict__, float* __restrict__);
+
+template <int HBUF, bool AUX, bool GRED>
+__device__ __forceinline__ void bwd2_flush(Bwd2Shared<HBUF, GRED>& sm, const int warp, const int lane, const int n, const float sx0, const float sy0,
+                                           float* __restrict__ g9, float* __restrict__ gz) {
   constexpr int LPH = 32 / HBUF;             // lanes per buffered hit (4 or 8); each sums 64 / LPH pixels
   __syncwarp();
   const int h = lane / LPH, q = lane % LPH;
@@ -384,6 +387,11 @@ __device__ __forceinline__ void bwd2_flush(Bwd2Shared<HBUF>& sm, const int warp,
   for (int k = 0; k < (AUX ? 10 : 9); ++k)
 #pragma unroll
     for (int o = 1; o < LPH; o <<= 1) S[k] += __shfl_xor_sync(0xffffffffu, S[k], o);
+  if (GRED && LPH == 4) {
+    if (h < n) bwd2_emit_global<HBUF, AUX, GRED>(sm, q, j, S, g9, gz);
+    __syncwarp();
+    return;
+  }
   if (h < n) {                               // every lane of the hit holds all nine sums: lane q adds rows q, q + LPH, ...
     if (LPH == 2) {
       atomicAdd(&sm.acc[q * 129 + j], q ? S[1] : S[0]);
@@ -407,10 +415,32 @@ __device__ __forceinline__ void bwd2_flush(Bwd2Shared<HBUF>& sm, const int warp,
   __syncwarp();
 }
 
+// End of bwd2_flush without shared accumulators (GRED, the default): the four lanes of a hit turn the sums into
+// dL/d(u, v, A, B, C, o, r, g, b) and add them straight to g9 with global reductions.  A (tile, splat) pair is hit by 1.3
+// strips on average, so combining the strips in shared memory first saves few reductions and costs 5 KB, the zeroing of
+// the accumulators and a barrier per batch: 2.86 -> 2.80 ms/step at cfg3, 0.67 -> 0.66 ms per view at cfg4.
+template <int HBUF, bool AUX, bool GRED>
+__device__ __forceinline__ void bwd2_emit_global(Bwd2Shared<HBUF, GRED>& sm, const int q, const int j, const float* S, float* __restrict__ g9,
+                                                 float* __restrict__ gz) {
+  const float4 a = sm.s0[j];
+  const float ik = 1.0f / 0.72134752044448170f;
+  const float A = a.x * a.x * ik, B = a.x * a.y * ik, C = fmaf(a.y, a.y, a.z * a.z) * ik;
+  float* dst = g9 + (size_t)9 * sm.id[j];
+  float v0, v1; int i0, i1;
+  if (q == 0)      { v0 = -fmaf(A, S[0], B * S[1]); i0 = 0; v1 = -0.5f * S[4]; i1 = 4; }
+  else if (q == 1) { v0 = -fmaf(B, S[0], C * S[1]); i0 = 1; v1 = S[5]; i1 = 6; }
+  else if (q == 2) { v0 = -0.5f * S[2]; i0 = 2; v1 = S[6]; i1 = 7; }
+  else             { v0 = -S[3]; i0 = 3; v1 = S[7]; i1 = 8; }
+  if (v0 != 0.f) atomicAdd(dst + i0, v0);
+  if (v1 != 0.f) atomicAdd(dst + i1, v1);
+  if (q == 0 && S[8] != 0.f) atomicAdd(dst + 5, S[8] * exp2f(-sm.s1[j].y));
+  if (AUX && q == 1 && S[9] != 0.f) atomicAdd(gz + sm.id[j], S[9]);
+}
+
 // AUX = true: upstream gradients of the auxiliary channels as well (either pointer may be NULL): dL/ddepth enters as a
 // fourth colour channel (g.c_k -> g.c_k + gD z_k, one more sum Sz = sum wgt gD -> gz[id] = dL/dz_k), dL/dopacity
 // (O = 1 - T_final) only shifts the start of the colour-behind recurrence: s_last = T_final (g.bg - gO).
-template <int HBUF, int MINB, bool AUX>
+template <int HBUF, int MINB, bool AUX, bool GRED>
 __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
                                                          const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
                                                          const float* __restrict__ dL_dimage, const float* __restrict__ final_T,
@@ -418,7 +448,7 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
                                                          const float* __restrict__ dL_ddepth, const float* __restrict__ dL_dopacity,
                                                          float* __restrict__ gz) {
   constexpr int PX = 2, BATCH = 128, ACC_STRIDE = 129;
-  __shared__ Bwd2Shared<HBUF> sm;
+  __shared__ Bwd2Shared<HBUF, GRED> sm;
   const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const Strip<PX> sp(warp, lane);
@@ -464,8 +494,10 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
       sm.id[threadIdx.x] = id;
       stage_splat(rec, id, ox, oy, &sm.s0[threadIdx.x], &sm.s1[threadIdx.x], &sm.s2[threadIdx.x]);
     }
+    if (!GRED) {
 #pragma unroll
-    for (int k = 0; k < (AUX ? 10 : 9); ++k) sm.acc[k * ACC_STRIDE + threadIdx.x] = 0.f;
+      for (int k = 0; k < (AUX ? 10 : 9); ++k) sm.acc[k * ACC_STRIDE + threadIdx.x] = 0.f;
+    }
     __syncthreads();
     if (lo_pos < lane_max) {
      int nbuf = 0;                                      // buffered hits (warp-uniform)
@@ -516,11 +548,12 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
         }
         sm.hit[warp][nbuf][lane] = make_float4(dpow[0], wgt[0], dpow[1], wgt[1]);
         if (lane == 0) sm.hitj[warp][nbuf] = j;
-        if (++nbuf == HBUF) { bwd2_flush<HBUF, AUX>(sm, warp, lane, HBUF, sx0, sy0); nbuf = 0; }
+        if (++nbuf == HBUF) { bwd2_flush<HBUF, AUX, GRED>(sm, warp, lane, HBUF, sx0, sy0, g9, gz); nbuf = 0; }
       }
      }
-     if (nbuf) bwd2_flush<HBUF, AUX>(sm, warp, lane, nbuf, sx0, sy0);
+     if (nbuf) bwd2_flush<HBUF, AUX, GRED>(sm, warp, lane, nbuf, sx0, sy0, g9, gz);
     }
+    if (GRED) continue;                                 // gradients already in g9 (the loop-top barrier protects the staging arrays)
     __syncthreads();
     if ((int)threadIdx.x < m) {
       const int j = threadIdx.x;
@@ -574,7 +607,7 @@ void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, con
                       cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
   if (dL_ddepth || dL_dopacity) {
-    blend_bwd2_kernel<8, 6, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9,
+    blend_bwd2_kernel<8, 7, true, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9,
                                                          dL_ddepth, dL_dopacity, ws.gz);
     ++g_launches;
     return;
@@ -586,7 +619,9 @@ void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, con
     case 4: FDGS_BWD(4); break;
     default:
       if (direct) FDGS_BWD(2);
-      else blend_bwd2_kernel<8, 6, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9, nullptr, nullptr, nullptr);
+      else if (getenv("FDGS_BWD2_SHARED_ACC"))    // A/B runs: per-splat sums combined across the warps in shared memory first
+        blend_bwd2_kernel<8, 6, false, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9, nullptr, nullptr, nullptr);
+      else blend_bwd2_kernel<8, 7, false, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9, nullptr, nullptr, nullptr);
   }
 #undef FDGS_BWD
   ++g_launches;
