@@ -607,7 +607,7 @@ void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, con
                       cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
   if (dL_ddepth || dL_dopacity) {
-    blend_bwd2_kernel<8, 7, true, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9,
+    blend_bwd2_kernel<8, 6, true, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9,
                                                          dL_ddepth, dL_dopacity, ws.gz);
     ++g_launches;
     return;
