@@ -215,6 +215,69 @@ int fdgs_debug_cull_status(const fdgs_scene *scene, const fdgs_view *view_host, 
 int fdgs_debug_measure_peaks(void *scratch_dev, size_t scratch_bytes, void *cuda_stream, float *fma_tlane_per_s_host,
                              float *mufu_t_per_s_host);
 
+/* ------------------------------------------------------------------------------------------------------------------
+ * Training-side per-primitive terms next to the rasterizer (readings
+ * T1-T6).  All are single streaming kernels over the parameter arrays (HBM-bound), asynchronous on `cuda_stream`.
+ * ------------------------------------------------------------------------------------------------------------------ */
+
+/* Learnable mask, forward (eq. 21-23): M = Sigmoid(mask_logit), M_hat = 1{M > mask_eps};
+ * S_hat = M_hat S, alpha_hat = M_hat alpha.  A masked primitive (M_hat = 0) has alpha_hat = 0 and contributes nothing,
+ * so the mask is applied by handing the renderer a copy of the opacity logits:
+ *   opacity_logit_out[i] = M_hat_i ? opacity_logit[i] : -inf     (a non-finite parameter culls the primitive)
+ * Render with a fdgs_scene whose opacity_logit is opacity_logit_out; kept primitives are untouched (M_hat = 1).
+ * mask_logit, opacity_logit, opacity_logit_out: [N] device.  In-place (out == in) is allowed. */
+int fdgs_mask_apply(const float *mask_logit, float mask_eps, const float *opacity_logit, float *opacity_logit_out,
+                    int32_t N, void *cuda_stream);
+
+typedef struct {
+  float lambda_sparse; /* weight of L_sparse = 1/N sum_i |q_l^i - q_r^i|_1 on the NORMALISED quaternions (eq. 26; T1) */
+  float lambda_covt;   /* weight of L_covt   = 1/N sum_i exp(-Sigma_44^i)                                (eq. 27)   */
+  float lambda_mask;   /* weight of L_mask   = 1/N sum_i Sigmoid(m_i)                                    (eq. 24)   */
+  float mask_eps;      /* threshold eps of eq. 21                                                                         */
+} fdgs_reg_config;
+
+/* Fused forward + backward of the three per-primitive regularisers, and the straight-through gradient of the mask.
+ * For every primitive i, in this order:
+ *   1. if mask_logit != NULL: with the rendering gradients ALREADY accumulated in grads (all views of the step),
+ *        grad_mask_logit[i] += M_hat_i (sum_k grads->log_scale[i,k] + grads->opacity_logit[i] / (1 - alpha_i)) M_i (1 - M_i)
+ *                              + lambda_mask M_i (1 - M_i) / N           (eq. 21-24; alpha_i = Sigmoid(scene->opacity_logit[i]),
+ *                                                                        the UNMASKED logits)
+ *   2. grads->log_scale, grads->quat_l, grads->quat_r += gradient of lambda_sparse L_sparse + lambda_covt L_covt.
+ *   3. losses_dev (NULL ok) [3] += (L_sparse, L_covt, L_mask), unweighted, summed with atomics (order not fixed).
+ * scene: only N, log_scale, quat_l, quat_r, opacity_logit are read.  Non-finite parameters or a zero quaternion make
+ * the primitive contribute nothing.  grads->mean / sh / mean2d / densify are not touched. */
+int fdgs_regularizers(const fdgs_scene *scene, const float *mask_logit, const fdgs_reg_config *rc_host,
+                      const fdgs_grads *grads, float *grad_mask_logit, float *losses_dev, void *cuda_stream);
+
+/* One dense Adam update of one parameter array (Kingma & Ba, Algorithm 1; the optimiser of [23], L324; T6):
+ *   m = beta1 m + (1-beta1) g;  v = beta2 v + (1-beta2) g^2;
+ *   p -= lr (m / (1-beta1^step)) / (sqrt(v / (1-beta2^step)) + eps)
+ * param, grad, exp_avg, exp_avg_sq: [count] device fp32, 16-byte aligned; step >= 1.  zero_grad != 0 also clears grad
+ * (saves the separate memset of the next step). */
+typedef struct { float lr, beta1, beta2, eps; int32_t step; } fdgs_adam_config;
+int fdgs_adam_step(float *param, float *grad, float *exp_avg, float *exp_avg_sq, int64_t count,
+                   const fdgs_adam_config *cfg_host, int32_t zero_grad, void *cuda_stream);
+
+/* Compact model of section 4.2 / 8.3.1 (T4): positions in binary16, opacity logit as a
+ * `opacity_bits`-bit min-max code, log-scale / both quaternions / base colour (k = 0) / remaining coefficients as
+ * residual-VQ indices (one uint8 per stage) into codebooks whose entries have the shape of the parameter they replace.
+ * Decoded value = SUM over stages (in stage order) of the indexed entries.  Entries per codebook <= 256. */
+typedef struct {
+  int32_t N, sh_degree, n_time;
+  const uint16_t *mean_f16;     /* [N,4] IEEE binary16 bit patterns                                                   */
+  const uint8_t *opacity_code;  /* [N]   logit = opacity_lo + code (opacity_hi - opacity_lo) / (2^opacity_bits - 1)   */
+  float opacity_lo, opacity_hi;
+  int32_t opacity_bits;         /* 1..8                                                                               */
+  int32_t scale_stages, scale_entries; const uint8_t *scale_idx; /* [N,stages] */ const float *scale_cb; /* [stages,entries,4] */
+  int32_t rot_stages, rot_entries;     const uint8_t *rot_l_idx, *rot_r_idx;      const float *rot_cb;   /* shared, [..,4]     */
+  int32_t dc_stages, dc_entries;       const uint8_t *dc_idx;                     const float *dc_cb;    /* [stages,entries,3] */
+  int32_t rest_stages, rest_entries;   const uint8_t *rest_idx;                   const float *rest_cb;  /* [stages,entries,(K-1)*3]; unused if K = 1 */
+} fdgs_compact_scene;
+
+/* Expands a compact model into the fp32 arrays of `out` (caller-owned, shapes of fdgs_scene for the same N, sh_degree,
+ * n_time; the const qualifiers of fdgs_scene are cast away for writing).  Stage counts 1..16. */
+int fdgs_decode_compact(const fdgs_compact_scene *compact, const fdgs_scene *out, void *cuda_stream);
+
 /* Number of kernel launches the library has issued so far in this process (bench.py's gpu_launches). */
 int64_t fdgs_launch_count(void);
 

@@ -9,7 +9,7 @@ namespace fdgs {
 
 static char g_cuda_err[256] = "no CUDA error recorded";
 
-static int cuda_fail(cudaError_t e, const char* where) {
+int cuda_fail(cudaError_t e, const char* where) {
   snprintf(g_cuda_err, sizeof(g_cuda_err), "CUDA error in %s: %s", where, cudaGetErrorString(e));
   return FDGS_ERR_CUDA;
 }

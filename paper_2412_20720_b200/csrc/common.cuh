@@ -141,6 +141,8 @@ __device__ __forceinline__ void prefetch_l2(const void* p, const int bytes) {
 
 // Launch counter (fdgs_launch_count) — bumped by every launcher.
 extern long long g_launches;
+// Records the CUDA error text for fdgs_strerror and returns FDGS_ERR_CUDA (api.cu).
+int cuda_fail(cudaError_t e, const char* where);
 
 // Launchers (each file implements its own; all asynchronous on `st`).
 void launch_preprocess_fwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, cudaStream_t st);

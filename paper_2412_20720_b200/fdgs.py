@@ -23,7 +23,8 @@ EXPORTED_SYMBOLS = ["fdgs_default_config", "fdgs_workspace_bytes", "fdgs_preproc
                     "fdgs_render_backward", "fdgs_l1_loss", "fdgs_step_host", "fdgs_debug_export",
                     "fdgs_launch_count", "fdgs_strerror", "fdgs_set_stage_timing", "fdgs_get_stage_ms",
                     "fdgs_debug_blend_stats", "fdgs_step_batch", "fdgs_debug_cull_status", "fdgs_render_forward_aux",
-                    "fdgs_render_backward_aux", "fdgs_debug_measure_peaks"]
+                    "fdgs_render_backward_aux", "fdgs_debug_measure_peaks", "fdgs_mask_apply", "fdgs_regularizers",
+                    "fdgs_adam_step", "fdgs_decode_compact"]
 MAX_BATCH = 8
 
 
@@ -51,6 +52,24 @@ class CGrads(C.Structure):
 class CViewBuffers(C.Structure):
     _fields_ = [("ws", C.c_void_p), ("ws_bytes", C.c_size_t), ("target_host", C.c_void_p), ("target_dev", C.c_void_p),
                 ("image", C.c_void_p), ("final_T", C.c_void_p), ("n_contrib", C.c_void_p), ("dL_dimage", C.c_void_p)]
+
+
+class CRegConfig(C.Structure):
+    _fields_ = [(k, C.c_float) for k in ("lambda_sparse", "lambda_covt", "lambda_mask", "mask_eps")]
+
+
+class CAdamConfig(C.Structure):
+    _fields_ = [("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float), ("step", C.c_int32)]
+
+
+class CCompactScene(C.Structure):
+    _fields_ = [("N", C.c_int32), ("sh_degree", C.c_int32), ("n_time", C.c_int32), ("mean_f16", C.c_void_p),
+                ("opacity_code", C.c_void_p), ("opacity_lo", C.c_float), ("opacity_hi", C.c_float), ("opacity_bits", C.c_int32),
+                ("scale_stages", C.c_int32), ("scale_entries", C.c_int32), ("scale_idx", C.c_void_p), ("scale_cb", C.c_void_p),
+                ("rot_stages", C.c_int32), ("rot_entries", C.c_int32), ("rot_l_idx", C.c_void_p), ("rot_r_idx", C.c_void_p),
+                ("rot_cb", C.c_void_p),
+                ("dc_stages", C.c_int32), ("dc_entries", C.c_int32), ("dc_idx", C.c_void_p), ("dc_cb", C.c_void_p),
+                ("rest_stages", C.c_int32), ("rest_entries", C.c_int32), ("rest_idx", C.c_void_p), ("rest_cb", C.c_void_p)]
 
 
 class FdgsError(RuntimeError):
@@ -90,6 +109,10 @@ def load():
     lib.fdgs_set_stage_timing.argtypes = [C.c_int]
     lib.fdgs_get_stage_ms.argtypes = [C.POINTER(C.c_float)]
     lib.fdgs_debug_blend_stats.argtypes = [C.POINTER(CView), C.POINTER(CConfig), vp, sz, i32, i32, i64, vp, vp]
+    lib.fdgs_mask_apply.argtypes = [vp, C.c_float, vp, vp, i32, vp]
+    lib.fdgs_regularizers.argtypes = [C.POINTER(CScene), vp, C.POINTER(CRegConfig), C.POINTER(CGrads), vp, vp, vp]
+    lib.fdgs_adam_step.argtypes = [vp, vp, vp, vp, i64, C.POINTER(CAdamConfig), i32, vp]
+    lib.fdgs_decode_compact.argtypes = [C.POINTER(CCompactScene), C.POINTER(CScene), vp]
     lib.fdgs_launch_count.restype = i64
     lib.fdgs_strerror.restype = C.c_char_p
     lib.fdgs_strerror.argtypes = [C.c_int]

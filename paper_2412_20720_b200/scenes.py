@@ -269,3 +269,38 @@ def fd_scene(seed: int, N: int = 8) -> Scene:
     V[:3, 3] = np.array([0.1, -0.05, 4.0])
     view = View(_f32(V), fx, fy, cx, cy, 64, 64, 0.5, 1.0, (0.1, 0.2, 0.3)).as_fp32()
     return Scene("fd", 1, 2, _f32(mean), _f32(ls), _f32(ql), _f32(qr), _f32(logit), _f32(sh), [view], seed)
+
+
+def compact_model(seed: int = 6, N: int = 1_000_000, sh_degree: int = 3, n_time: int = 3, rvq=((6, 64), (6, 64), (6, 64), (8, 256))) -> dict:
+    """Seeded stand-in for a compact model: codebook sizes of section 8.3.1 (scale 6x64, both
+    quaternions share 6x64, base colour 6x64, rest 8x256), uniformly random indices, binary16 positions in cfg3's box,
+    8-bit opacity codes over the logit range [-4, 6].  Stage s of a codebook holds values ~ N(centre_s, (spread / 2^s)):
+    the first stage carries the parameter's scale, later stages shrinking residuals, as a fitted residual VQ would.
+    Holds no arithmetic of the method — only random tables and indices."""
+    K = n_time * (sh_degree + 1) ** 2
+    (s_st, s_en), (r_st, r_en), (d_st, d_en), (c_st, c_en) = rvq
+
+    def book(stream, stages, entries, dim, centre, spread):
+        cb = normal(seed, stream, stages * entries * dim).reshape(stages, entries, dim) * spread
+        cb = cb / (2.0 ** np.arange(stages))[:, None, None]
+        cb[0] += np.asarray(centre, dtype=np.float64)
+        return _f32(cb)
+
+    def indices(stream, stages, entries):
+        return np.ascontiguousarray(np.minimum((uniform(seed, stream, N * stages) * entries).astype(np.int64), entries - 1)
+                                    .reshape(N, stages).astype(np.uint8))
+
+    mean = np.stack([-3 + 6 * uniform(seed, 1, N), -2 + 4 * uniform(seed, 2, N), 2 + 6 * uniform(seed, 3, N),
+                     10 * uniform(seed, 4, N)], axis=1)
+    out = dict(mean_f16=np.ascontiguousarray(mean.astype(np.float16)),
+               opacity_code=np.minimum((uniform(seed, 5, N) * 256).astype(np.int64), 255).astype(np.uint8),
+               opacity_lo=-4.0, opacity_hi=6.0, opacity_bits=8,
+               scale_cb=book(100, s_st, s_en, 4, [-4.0, -4.0, -4.0, -0.5], 0.6), scale_idx=indices(101, s_st, s_en),
+               rot_cb=book(110, r_st, r_en, 4, [0.0, 0.0, 0.0, 0.0], 1.0), rot_l_idx=indices(111, r_st, r_en),
+               rot_r_idx=indices(112, r_st, r_en),
+               dc_cb=book(120, d_st, d_en, 3, [0.5, 0.5, 0.5], 0.2), dc_idx=indices(121, d_st, d_en),
+               rest_cb=None, rest_idx=None)
+    if K > 1:
+        out["rest_cb"] = book(130, c_st, c_en, (K - 1) * 3, np.zeros((K - 1) * 3), 0.05)
+        out["rest_idx"] = indices(131, c_st, c_en)
+    return out

@@ -1,6 +1,6 @@
 """Secondary measurements of BASELINE.json's configs 2, 4 and 5 (bench.py times the headline config 3).
 
-    python -m paper_2412_20720_b200.sweep [--frames 24] [--max-n 8000000] [--skip-train]
+    python -m paper_2412_20720_b200.sweep [--frames 24] [--max-n 8000000] [--skip-train] [--train-terms]
 
 cfg5: forward-only render throughput over Gaussian count x resolution at evenly spaced query times: FPS (one frame at a
 time), per-stage ms (preprocess / sort incl. compaction, duplication and ranges / blend) and the fraction culled by the
@@ -100,12 +100,41 @@ def train_cfg(name, scene, cap, flush):
                       "visible_per_view": [s["num_visible"] for s in sts], "loss": float(bs.loss.sum())}), flush=True)
 
 
+def train_terms(flush, n=1_000_000):
+    """SURVEY 8(f) f2-f4 kernels at cfg3's size (N = 1 M, K = 48): ms and achieved HBM GB/s on ALGORITHMIC bytes
+    (DESIGN.md section 10): regularisers 176 B/primitive, Adam 28 B/element (32 with zero_grad) over the 161 floats of a
+    primitive, decode 41 B read + 644 B written per primitive."""
+    import torch
+    from . import fdgs, scenes, train
+    sc = scenes.multiview_video(N=n, n_views=1)
+    ds = fdgs.DeviceScene.from_scene(sc)
+    g = ds.zero_grads()
+    m = torch.randn(n, device="cuda")
+    gm, losses = torch.zeros(n, device="cuda"), torch.zeros(3, device="cuda")
+    ms = _timed(lambda: train.regularizers(ds, g, 0.01, 0.01, 0.01, m, 0.01, gm, losses), 20, 5, flush)
+    out = {"config": "train_terms", "N": n, "K": ds.K,
+           "regularizers": {"ms": ms, "bytes": 176 * n, "GBps": 176 * n / ms / 1e6}}
+    ms = _timed(lambda: train.mask_apply(m, 0.01, ds.opacity_logit, gm), 20, 5, flush)
+    out["mask_apply"] = {"ms": ms, "bytes": 12 * n, "GBps": 12 * n / ms / 1e6}
+    opt = train.Adam(ds, {k: 1e-4 for k in train.PARAMS})
+    elems = sum(getattr(ds, k).numel() for k in train.PARAMS)
+    ms = _timed(lambda: opt.step(g, zero_grad=True), 20, 5, flush)
+    out["adam_all_arrays_zero_grad"] = {"ms": ms, "bytes": 32 * elems, "GBps": 32 * elems / ms / 1e6, "launches": 6}
+    cm = scenes.compact_model(N=n)
+    dev = {k: (torch.from_numpy(v).cuda() if isinstance(v, np.ndarray) else v) for k, v in cm.items()}
+    ms = _timed(lambda: train.decode_compact(dev, 3, 3, ds), 20, 5, flush)
+    out["decode_compact"] = {"ms": ms, "bytes": (41 + 644) * n, "GBps": (41 + 644) * n / ms / 1e6,
+                             "l2_gather_bytes": (8 * 564 + 6 * 12 + 3 * 6 * 16) * n}
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--frames", type=int, default=24)
     ap.add_argument("--max-n", type=int, default=8_000_000)
     ap.add_argument("--skip-train", action="store_true")
     ap.add_argument("--skip-sweep", action="store_true")
+    ap.add_argument("--train-terms", action="store_true", help="time the f2-f4 kernels (mask, regularisers, Adam, decode) only")
     args = ap.parse_args()
     import torch
     from . import build, scenes
@@ -113,6 +142,9 @@ def main():
         raise RuntimeError("sweep needs a CUDA device: the product has no CPU fallback")
     build.build()
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+    if args.train_terms:
+        train_terms(flush)
+        return
     if not args.skip_train:
         train_cfg("cfg2_object", scenes.single_object(), 1 << 22, flush)
         train_cfg("cfg4_driving", scenes.driving(), 160 * 1024 * 1024, flush)
