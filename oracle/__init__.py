@@ -63,6 +63,7 @@ def _load():
     lib.fdgs_oracle_backward.argtypes = [C.c_void_p, dp] + [dp] * 8
     lib.fdgs_oracle_get_depth_map.argtypes = [C.c_void_p, dp]
     lib.fdgs_oracle_backward_aux.argtypes = [C.c_void_p, dp, dp, dp] + [dp] * 10
+    lib.fdgs_oracle_set_colour_override.argtypes = [C.c_void_p, dp]
     lib.fdgs_oracle_num_threads.restype = C.c_int
     _lib = lib
     return lib
@@ -211,3 +212,60 @@ class Oracle:
                                          _d(out["mean2d"]), _d(out["g9"]), _d(out["gz"]),
                                          _d(densify) if densify is not None else null)
         return out
+
+    # ---- feature channels and rendered optical flow (L410) ------------------------------------------
+    def _override(self, feat, c0):
+        """Channels c0..c0+2 of feat[N,C] become the composited 'colour' of the visible primitives (zero padded)."""
+        F = np.zeros((self.N, 3))
+        n = min(3, feat.shape[1] - c0)
+        F[:, :n] = feat[:, c0:c0 + n]
+        _load().fdgs_oracle_set_colour_override(self._h, _d(np.ascontiguousarray(F)))
+        return n
+
+    def render_features(self, feat):
+        """feat[N,C] -> F[C,H,W] = sum_k f_k alpha_k T_k: eq. 6 with the colour replaced by the feature vector, three
+        channels per pass over the same tile lists.  Call preprocess() with bg = 0 first.  The override stays active."""
+        feat = np.ascontiguousarray(np.asarray(feat, dtype=np.float64))
+        out = np.zeros((feat.shape[1], self.height, self.width))
+        for c0 in range(0, feat.shape[1], 3):
+            n = self._override(feat, c0)
+            out[c0:c0 + n] = self.forward()[0][:n]
+        return out
+
+    def backward_features(self, feat, dL_dF):
+        """VJP of render_features: returns (grad_feat[N,C], dict of parameter gradients through alpha_k, T_k).
+        Per pass the blend backward yields dL/df in g9[:,6:9]; the geometry gradients of the passes add up."""
+        feat = np.ascontiguousarray(np.asarray(feat, dtype=np.float64))
+        dL_dF = np.asarray(dL_dF, dtype=np.float64)
+        gf = np.zeros_like(feat)
+        total = None
+        for c0 in range(0, feat.shape[1], 3):
+            n = self._override(feat, c0)
+            self.forward()
+            g3 = np.zeros((3, self.height, self.width))
+            g3[:n] = dL_dF[c0:c0 + n]
+            g = self.backward(g3)
+            gf[:, c0:c0 + n] = g["g9"][:, 6:6 + n]
+            if total is None:
+                total = {k: g[k].copy() for k in ("mean", "log_scale", "quat_l", "quat_r", "opacity_logit", "sh")}
+            else:
+                for k in total:
+                    total[k] += g[k]
+        return gf, total
+
+    def splat_flow(self, view, intr, dt_next):
+        """Per-splat 2D displacement between the frames at t and t + dt_next: the conditional mean
+        mu_xyz|t is linear in t (eq. 9), mu_c(t + d) = mu_c(t) + Sigma_1:3,4 / Sigma_44 d; both are projected with
+        eq. 3 and subtracted.  Zero for primitives not visible at t or behind the camera at t + dt_next."""
+        P = self.prims()
+        V = np.asarray(view, dtype=np.float64).reshape(4, 4)
+        fx, fy, cx, cy = intr
+        flow = np.zeros((self.N, 2))
+        for i in np.nonzero(P.status == STATUS_VISIBLE)[0]:
+            _, Sigma = self.rot_cov(int(i))
+            mu2 = P.mu_c[i] + Sigma[:3, 3] / Sigma[3, 3] * dt_next
+            p2 = V[:3, :3] @ mu2 + V[:3, 3]
+            if p2[2] <= 0:
+                continue
+            flow[i] = (fx * p2[0] / p2[2] + cx - P.uv[i, 0], fy * p2[1] / p2[2] + cy - P.uv[i, 1])
+        return flow

@@ -90,6 +90,7 @@ struct Oracle {
   // per-splat gradients from the blend backward: g_u,g_v,g_A,g_B,g_C,g_o,g_r,g_g,g_b
   std::vector<double> g9;
   std::vector<double> gz;          // per-splat dL/d(camera depth z_k) from the auxiliary depth channel
+  bool colour_override = false;    // feature channels: P.rgb holds free per-splat values, not eq. 20
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -438,8 +439,8 @@ void backward_one(const Oracle& O, int i, const double g9[9], double* d_mean, do
   const double g_u = g9[0], g_v = g9[1], g_A = g9[2], g_B = g9[3], g_C = g9[4], g_o = g9[5];
   if (d_mean2d) { d_mean2d[2 * i] += g_u; d_mean2d[2 * i + 1] += g_v; }
   double d_muc[3] = {0, 0, 0}, d_dt = 0, d_b = 0;
-  // (A4) colour
-  {
+  // (A4) colour — skipped when the composited channels are free per-splat features (their gradient is g9[6..8] itself)
+  if (!O.colour_override) {
     double Y[16], dY[16][3];
     sh_basis(O.L, P.dir, Y, dY);
     const double* coef = &O.sh[(size_t)i * O.K * 3];
@@ -586,6 +587,7 @@ int fdgs_oracle_preprocess(void* h, const double* view16, const double* intr, in
                            double period_T, const double* bg, const double* cfg9) {
   Oracle& O = *(Oracle*)h;
   if (width <= 0 || height <= 0) return -1;
+  O.colour_override = false;
   for (int r = 0; r < 3; ++r) { for (int q = 0; q < 3; ++q) O.view.Wm[r][q] = view16[4 * r + q]; O.view.tau[r] = view16[4 * r + 3]; }
   O.view.fx = intr[0]; O.view.fy = intr[1]; O.view.cx = intr[2]; O.view.cy = intr[3];
   O.view.width = width; O.view.height = height; O.view.t = t; O.view.period_T = period_T;
@@ -693,6 +695,19 @@ void fdgs_oracle_backward_aux(void* h, const double* dL_dimage, const double* dL
 #pragma omp parallel for schedule(static)
   for (int i = 0; i < O.N; ++i)
     backward_one(O, i, &O.g9[(size_t)9 * i], d_mean, d_log_scale, d_quat_l, d_quat_r, d_logit, d_sh, d_mean2d, O.gz[i], densify3);
+}
+
+// Feature channels ("rendered following the same process as in Section 3.2, with the color c replaced by
+// the ... feature vector"; L410: the projected displacement rendered "using equation (6)" as optical flow): replaces the
+// colour of every visible primitive by rgb[N,3] (three channels at a time; more channels = more passes).  The override
+// stays until the next fdgs_oracle_preprocess; while it is active the backward returns dL/d(feature) in g9[:,6:9] and
+// chains only the geometry (u, v, conic, opacity) to the parameters.
+void fdgs_oracle_set_colour_override(void* h, const double* rgb) {
+  Oracle& O = *(Oracle*)h;
+  O.colour_override = true;
+  for (int i = 0; i < O.N; ++i)
+    if (O.prims[i].status == VISIBLE)
+      for (int ch = 0; ch < 3; ++ch) O.prims[i].rgb[ch] = rgb[(size_t)3 * i + ch];
 }
 
 int fdgs_oracle_num_threads(void) {
