@@ -216,6 +216,38 @@ int fdgs_debug_measure_peaks(void *scratch_dev, size_t scratch_bytes, void *cuda
                              float *mufu_t_per_s_host);
 
 /* ------------------------------------------------------------------------------------------------------------------
+ * Feature channels and rendered optical flow.
+ * "The 2D feature F at a specific view could be rendered following the same process as in Section 3.2, with the color c
+ * replaced by the normalized feature vector f":  F[c](pixel) = sum_k feat[k,c] alpha_k T_k over the same
+ * per-tile depth-ordered lists, thresholds and termination as the colour image; no background term.
+ * Call after fdgs_preprocess + fdgs_render_forward on the same ws / view / config.  The C channels go through the
+ * 3-channel blend kernels three at a time (ceil(C/3) launches).  scratch: device buffer of
+ * fdgs_features_scratch_bytes(N, W, H) bytes, 16-byte aligned, caller-owned (record copies + one 3-plane image).
+ * ------------------------------------------------------------------------------------------------------------------ */
+int fdgs_features_scratch_bytes(int32_t N, int32_t W, int32_t H, size_t *bytes_host);
+
+/* feat [N,C] device fp32 (C >= 1); out [C,H,W]. */
+int fdgs_render_features_forward(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws,
+                                 size_t ws_bytes, int64_t pair_capacity, void *cuda_stream, const float *feat, int32_t C,
+                                 void *scratch, size_t scratch_bytes, float *out);
+
+/* VJP of the above.  dL_dout [C,H,W]; final_T / n_contrib from fdgs_render_forward of this view.
+ *   grad_feat [N,C] += dL/dfeat;   grads (NULL = features only) += the gradient through alpha_k and T_k to mean,
+ *   log_scale, quat_l, quat_r, opacity_logit (grads->sh receives zeros: the 4DSH coefficients do not enter). */
+int fdgs_render_features_backward(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws,
+                                  size_t ws_bytes, int64_t pair_capacity, void *cuda_stream, const float *feat, int32_t C,
+                                  void *scratch, size_t scratch_bytes, const float *dL_dout, const float *final_T,
+                                  const uint32_t *n_contrib, float *grad_feat, const fdgs_grads *grads);
+
+/* Per-splat optical flow: "we project its 3D displacement between consecutive two frames to the image
+ * plane and render it using equation (6)".  flow [N,2] (pixels) = pi(mu_xyz|t+dt_next) - pi(mu_xyz|t), with
+ * mu_xyz|t+d = mu_xyz|t + Sigma_1:3,4 / Sigma_44 d (eq. 9 is linear in t) and pi the pinhole projection of eq. 3; zero for
+ * primitives culled at t or behind the camera at t + dt_next.  Call after fdgs_preprocess; render the result with
+ * fdgs_render_features_forward(feat = flow, C = 2). */
+int fdgs_splat_flow(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws, size_t ws_bytes,
+                    int64_t pair_capacity, void *cuda_stream, float dt_next, float *flow);
+
+/* ------------------------------------------------------------------------------------------------------------------
  * Training-side per-primitive terms next to the rasterizer (readings
  * T1-T6).  All are single streaming kernels over the parameter arrays (HBM-bound), asynchronous on `cuda_stream`.
  * ------------------------------------------------------------------------------------------------------------------ */

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfdgs.so")
-SOURCES = ["api.cu", "preprocess.cu", "preprocess_bwd.cu", "scan_dup.cu", "radix_sort.cu", "blend.cu", "train.cu"]
+SOURCES = ["api.cu", "features.cu", "preprocess.cu", "preprocess_bwd.cu", "scan_dup.cu", "radix_sort.cu", "blend.cu", "train.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
               "--use_fast_math=false"]
 

@@ -395,6 +395,124 @@ int fdgs_step_batch(const fdgs_scene* sc, const fdgs_view* views, int32_t num_vi
   return FDGS_OK;
 }
 
+}  // extern "C"
+
+// ---- feature channels and optical flow (features.cu) ---------------------------------------------------------------
+struct FeatScratch { SplatRec* rec; float* img3; float* final_T; unsigned int* n_contrib; size_t bytes; };
+static FeatScratch carve_feat(void* base, long long N, long long W, long long H) {
+  FeatScratch f; size_t off = 0;
+  auto take = [&](size_t b) { void* p = base ? (char*)base + off : nullptr; off += align_up(b); return p; };
+  f.rec = (SplatRec*)take(sizeof(SplatRec) * (size_t)(N > 0 ? N : 1));
+  f.img3 = (float*)take(sizeof(float) * 3 * W * H);
+  f.final_T = (float*)take(sizeof(float) * W * H);
+  f.n_contrib = (unsigned int*)take(sizeof(unsigned int) * W * H);
+  f.bytes = off;
+  return f;
+}
+
+int fdgs_features_scratch_bytes(int32_t N, int32_t W, int32_t H, size_t* bytes_host) {
+  if (!bytes_host || N < 0 || W <= 0 || H <= 0) return FDGS_ERR_INVALID;
+  *bytes_host = carve_feat(nullptr, N, W, H).bytes;
+  return FDGS_OK;
+}
+
+static int features_common(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes, int64_t cap,
+                           const float* feat, int32_t C, void* scratch, size_t scratch_bytes, Workspace& ws, FeatScratch& fs,
+                           ViewParams& vp, CfgParams& cp, int* l1, int* l2) {
+  int rc = check_common(sc, v, c, ws_ptr);
+  if (rc) return rc;
+  if (C < 1 || cap < 1 || cap >= (1LL << 30) || !scratch || !aligned16(scratch) || (sc->N > 0 && !feat)) return FDGS_ERR_INVALID;
+  const int K = sc->n_time * (sc->sh_degree + 1) * (sc->sh_degree + 1);
+  ws = carve(ws_ptr, sc->N, K, v->width, v->height, cap);
+  if (ws.bytes > ws_bytes) return FDGS_ERR_WORKSPACE;
+  fs = carve_feat(scratch, sc->N, v->width, v->height);
+  if (fs.bytes > scratch_bytes) return FDGS_ERR_WORKSPACE;
+  make_params(v, c, vp, cp);
+  vp.bg[0] = vp.bg[1] = vp.bg[2] = 0.f;                 // features have no background term
+  sort_bufs(sc, vp, cap, l1, l2);
+  return FDGS_OK;
+}
+
+extern "C" {
+
+int fdgs_render_features_forward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
+                                 int64_t cap, void* stream, const float* feat, int32_t C, void* scratch, size_t scratch_bytes,
+                                 float* out) {
+  Workspace ws; FeatScratch fs; ViewParams vp; CfgParams cp; int l1, l2;
+  int rc = features_common(sc, v, c, ws_ptr, ws_bytes, cap, feat, C, scratch, scratch_bytes, ws, fs, vp, cp, &l1, &l2);
+  if (rc) return rc;
+  if (!out) return FDGS_ERR_INVALID;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t HW = (size_t)v->width * v->height;
+  Workspace wf = ws;
+  wf.rec = fs.rec;
+  for (int c0 = 0; c0 < C; c0 += 3) {
+    const int n = C - c0 < 3 ? C - c0 : 3;
+    if (sc->N > 0) launch_feature_records(ws, feat, C, c0, sc->N, fs.rec, st);
+    float* img = n == 3 ? out + c0 * HW : fs.img3;      // a ragged last group is rendered aside and its planes copied
+    launch_blend_fwd(wf, l2, vp, cp, img, fs.final_T, fs.n_contrib, nullptr, st);
+    if (n < 3) FDGS_CUDA(cudaMemcpyAsync(out + c0 * HW, fs.img3, sizeof(float) * n * HW, cudaMemcpyDeviceToDevice, st), "copy planes");
+  }
+  FDGS_CUDA(cudaGetLastError(), "feature forward launches");
+  return FDGS_OK;
+}
+
+int fdgs_render_features_backward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
+                                  int64_t cap, void* stream, const float* feat, int32_t C, void* scratch, size_t scratch_bytes,
+                                  const float* dL_dout, const float* final_T, const uint32_t* n_contrib, float* grad_feat,
+                                  const fdgs_grads* g) {
+  Workspace ws; FeatScratch fs; ViewParams vp; CfgParams cp; int l1, l2;
+  int rc = features_common(sc, v, c, ws_ptr, ws_bytes, cap, feat, C, scratch, scratch_bytes, ws, fs, vp, cp, &l1, &l2);
+  if (rc) return rc;
+  if (!dL_dout || !final_T || !n_contrib || (sc->N > 0 && !grad_feat)) return FDGS_ERR_INVALID;
+  if (g && sc->N > 0) {
+    if (!g->mean || !g->log_scale || !g->quat_l || !g->quat_r || !g->opacity_logit || !g->sh) return FDGS_ERR_INVALID;
+    if (!aligned16(g->mean) || !aligned16(g->log_scale) || !aligned16(g->quat_l) || !aligned16(g->quat_r)) return FDGS_ERR_INVALID;
+  }
+  if (sc->N == 0) return FDGS_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t HW = (size_t)v->width * v->height;
+  Workspace wf = ws;
+  wf.rec = fs.rec;
+  FDGS_CUDA(cudaMemsetAsync(ws.g9, 0, sizeof(float) * 9 * (size_t)sc->N, st), "memset(g9)");
+  for (int c0 = 0; c0 < C; c0 += 3) {
+    const int n = C - c0 < 3 ? C - c0 : 3;
+    launch_feature_records(ws, feat, C, c0, sc->N, fs.rec, st);
+    const float* dL = dL_dout + c0 * HW;
+    if (n < 3) {                                        // ragged last group: zero-padded copy of its planes
+      FDGS_CUDA(cudaMemsetAsync(fs.img3, 0, sizeof(float) * 3 * HW, st), "memset(dL pad)");
+      FDGS_CUDA(cudaMemcpyAsync(fs.img3, dL, sizeof(float) * n * HW, cudaMemcpyDeviceToDevice, st), "copy planes");
+      dL = fs.img3;
+    }
+    launch_blend_bwd(wf, l2, vp, cp, dL, final_T, n_contrib, nullptr, nullptr, st);   // geometry slots of g9 add up over the passes
+    launch_extract_feature_grads(ws, grad_feat, C, c0, sc->N, st);
+  }
+  // chain (u, v, conic, opacity) to the parameters once; the colour slots are zero, so the 4DSH coefficients get nothing
+  if (g) launch_preprocess_bwd(*sc, vp, cp, ws, l1, *g, false, st);
+  FDGS_CUDA(cudaGetLastError(), "feature backward launches");
+  return FDGS_OK;
+}
+
+int fdgs_splat_flow(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes, int64_t cap,
+                    void* stream, float dt_next, float* flow) {
+  int rc = check_common(sc, v, c, ws_ptr);
+  if (rc) return rc;
+  if (cap < 1 || cap >= (1LL << 30) || (sc->N > 0 && (!flow || (reinterpret_cast<uintptr_t>(flow) & 7u)))) return FDGS_ERR_INVALID;
+  const int K = sc->n_time * (sc->sh_degree + 1) * (sc->sh_degree + 1);
+  const Workspace ws = carve(ws_ptr, sc->N, K, v->width, v->height, cap);
+  if (ws.bytes > ws_bytes) return FDGS_ERR_WORKSPACE;
+  if (sc->N == 0) return FDGS_OK;
+  ViewParams vp; CfgParams cp;
+  make_params(v, c, vp, cp);
+  launch_splat_flow(*sc, vp, cp, ws, dt_next, flow, (cudaStream_t)stream);
+  FDGS_CUDA(cudaGetLastError(), "flow launch");
+  return FDGS_OK;
+}
+
+}  // extern "C"
+
+extern "C" {
+
 int64_t fdgs_launch_count(void) { return g_launches; }
 
 int fdgs_set_stage_timing(int enable) {

@@ -24,7 +24,8 @@ EXPORTED_SYMBOLS = ["fdgs_default_config", "fdgs_workspace_bytes", "fdgs_preproc
                     "fdgs_launch_count", "fdgs_strerror", "fdgs_set_stage_timing", "fdgs_get_stage_ms",
                     "fdgs_debug_blend_stats", "fdgs_step_batch", "fdgs_debug_cull_status", "fdgs_render_forward_aux",
                     "fdgs_render_backward_aux", "fdgs_debug_measure_peaks", "fdgs_mask_apply", "fdgs_regularizers",
-                    "fdgs_adam_step", "fdgs_decode_compact"]
+                    "fdgs_adam_step", "fdgs_decode_compact", "fdgs_features_scratch_bytes", "fdgs_render_features_forward",
+                    "fdgs_render_features_backward", "fdgs_splat_flow"]
 MAX_BATCH = 8
 
 
@@ -113,6 +114,12 @@ def load():
     lib.fdgs_regularizers.argtypes = [C.POINTER(CScene), vp, C.POINTER(CRegConfig), C.POINTER(CGrads), vp, vp, vp]
     lib.fdgs_adam_step.argtypes = [vp, vp, vp, vp, i64, C.POINTER(CAdamConfig), i32, vp]
     lib.fdgs_decode_compact.argtypes = [C.POINTER(CCompactScene), C.POINTER(CScene), vp]
+    lib.fdgs_features_scratch_bytes.argtypes = [i32, i32, i32, C.POINTER(sz)]
+    lib.fdgs_render_features_forward.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, vp, i32,
+                                                 vp, sz, vp]
+    lib.fdgs_render_features_backward.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, vp, i32,
+                                                  vp, sz, vp, vp, vp, vp, C.POINTER(CGrads)]
+    lib.fdgs_splat_flow.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, C.c_float, vp]
     lib.fdgs_launch_count.restype = i64
     lib.fdgs_strerror.restype = C.c_char_p
     lib.fdgs_strerror.argtypes = [C.c_int]
@@ -312,6 +319,52 @@ class Renderer:
                                                _ptr(dL_dopacity), self.final_T.data_ptr(), self.n_contrib.data_ptr(), C.byref(cg))
         if rc:
             raise FdgsError(rc, "fdgs_render_backward_aux")
+
+    # ---- feature channels / optical flow (include/fdgs.h "Feature channels") ----
+    def _feat_scratch(self):
+        import torch
+        if getattr(self, "_fscratch", None) is None:
+            n = C.c_size_t(0)
+            rc = self.lib.fdgs_features_scratch_bytes(self.ds.N, self.width, self.height, C.byref(n))
+            if rc:
+                raise FdgsError(rc, "fdgs_features_scratch_bytes")
+            self._fscratch = torch.empty(int(n.value), dtype=torch.uint8, device=self.ws.device)
+        return self._fscratch
+
+    def features_forward(self, cview: CView, feat, out=None):
+        """feat [N,C] float32 CUDA -> [C,H,W]; call after preprocess + forward of this view."""
+        import torch
+        Cn = int(feat.shape[1])
+        out = torch.empty((Cn, self.height, self.width), dtype=torch.float32, device=feat.device) if out is None else out
+        sc = self._feat_scratch()
+        rc = self.lib.fdgs_render_features_forward(C.byref(self._cs), C.byref(cview), C.byref(self.cfg), self.ws.data_ptr(),
+                                                   self.ws_bytes, self.cap, _stream(), feat.data_ptr(), Cn, sc.data_ptr(),
+                                                   sc.numel(), out.data_ptr())
+        if rc:
+            raise FdgsError(rc, "fdgs_render_features_forward")
+        return out
+
+    def features_backward(self, cview: CView, feat, dL_dout, grad_feat, grads: Optional[dict] = None):
+        Cn = int(feat.shape[1])
+        sc = self._feat_scratch()
+        cg = grads_struct(grads) if grads is not None else None
+        rc = self.lib.fdgs_render_features_backward(C.byref(self._cs), C.byref(cview), C.byref(self.cfg), self.ws.data_ptr(),
+                                                    self.ws_bytes, self.cap, _stream(), feat.data_ptr(), Cn, sc.data_ptr(),
+                                                    sc.numel(), dL_dout.data_ptr(), self.final_T.data_ptr(),
+                                                    self.n_contrib.data_ptr(), grad_feat.data_ptr(),
+                                                    C.byref(cg) if cg is not None else None)
+        if rc:
+            raise FdgsError(rc, "fdgs_render_features_backward")
+
+    def splat_flow(self, cview: CView, dt_next: float):
+        """Per-splat 2D displacement [N,2] between t and t + dt_next; call after preprocess."""
+        import torch
+        flow = torch.empty((self.ds.N, 2), dtype=torch.float32, device=self.ws.device)
+        rc = self.lib.fdgs_splat_flow(C.byref(self._cs), C.byref(cview), C.byref(self.cfg), self.ws.data_ptr(), self.ws_bytes,
+                                      self.cap, _stream(), float(dt_next), flow.data_ptr())
+        if rc:
+            raise FdgsError(rc, "fdgs_splat_flow")
+        return flow
 
     def l1_loss(self, target):
         """loss += mean|image - target|; writes self.dL_dimage."""
