@@ -444,15 +444,9 @@ int fdgs_render_features_forward(const fdgs_scene* sc, const fdgs_view* v, const
   if (!out) return FDGS_ERR_INVALID;
   cudaStream_t st = (cudaStream_t)stream;
   const size_t HW = (size_t)v->width * v->height;
-  Workspace wf = ws;
-  wf.rec = fs.rec;
-  for (int c0 = 0; c0 < C; c0 += 3) {
-    const int n = C - c0 < 3 ? C - c0 : 3;
-    if (sc->N > 0) launch_feature_records(ws, feat, C, c0, sc->N, fs.rec, st);
-    float* img = n == 3 ? out + c0 * HW : fs.img3;      // a ragged last group is rendered aside and its planes copied
-    launch_blend_fwd(wf, l2, vp, cp, img, fs.final_T, fs.n_contrib, nullptr, st);
-    if (n < 3) FDGS_CUDA(cudaMemcpyAsync(out + c0 * HW, fs.img3, sizeof(float) * n * HW, cudaMemcpyDeviceToDevice, st), "copy planes");
-  }
+  (void)HW;
+  // dedicated C-channel kernel: alpha evaluated once per 16 channels, features gathered by id next to the records
+  launch_blend_feat_fwd(ws, l2, vp, cp, feat, C, out, st);
   FDGS_CUDA(cudaGetLastError(), "feature forward launches");
   return FDGS_OK;
 }

@@ -164,6 +164,113 @@ __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __rest
   }
 }
 
+// Feature channels: the walk of blend_fwd_kernel<2> — same staging, same patch culling, the
+// SAME expression for alpha, so every skip / termination decision is bit-identical to the colour pass — compositing CH
+// per-splat feature values per pass instead of (r, g, b): alpha is evaluated once for CH channels.  feat[N,C] is gathered
+// by id into shared memory next to the splat records; channels c0 .. c0+CH-1 (zero beyond C); no background.
+template <int CH>
+__global__ void __launch_bounds__(128) blend_feat_fwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
+                                                             const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
+                                                             const float* __restrict__ feat, const int C, const int c0,
+                                                             float* __restrict__ out) {
+  constexpr int PX = 2, BATCH = 128;
+  __shared__ struct { float4 s0[BATCH], s1[BATCH], s2[BATCH]; float4 f[BATCH][CH / 4]; } sm;
+  const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const Strip<PX> sp(warp, lane);
+  const int px = tx * TILE + sp.lx;
+  const float x = sp.lx + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
+  float y[PX], T[PX], acc[PX][CH];
+  bool done[PX], inside[PX];
+#pragma unroll
+  for (int k = 0; k < PX; ++k) {
+    const int ly = sp.ly0 + 4 * k;
+    inside[k] = px < vp.width && ty * TILE + ly < vp.height;
+    y[k] = ly + 0.5f; T[k] = 1.f; done[k] = !inside[k];
+#pragma unroll
+    for (int c = 0; c < CH; ++c) acc[k][c] = 0.f;
+  }
+  const uint2 range = ranges[tile];
+  const int n = (int)(range.y - range.x);
+  const bool vec = (C & 3) == 0 && (c0 & 3) == 0 && c0 + CH <= C;       // 128-bit gathers when the row slice is aligned
+  float c_l2min = cp.log2_alpha_min, c_amax = cp.alpha_max, c_amin = cp.alpha_min, c_tmin = cp.transmittance_min;
+  asm volatile("" : "+f"(c_l2min), "+f"(c_amax), "+f"(c_amin), "+f"(c_tmin));
+  for (int base = 0; base < n; base += BATCH) {
+    if (__syncthreads_and(done[0] && done[1])) break;
+    const int m = min(BATCH, n - base);
+    if ((int)threadIdx.x < m) {
+      const unsigned int id = vals[range.x + base + threadIdx.x];
+      stage_splat(rec, id, ox, oy, &sm.s0[threadIdx.x], &sm.s1[threadIdx.x], &sm.s2[threadIdx.x]);
+      const float* src = feat + (size_t)id * C + c0;
+      if (vec) {
+#pragma unroll
+        for (int q = 0; q < CH / 4; ++q) sm.f[threadIdx.x][q] = __ldg(reinterpret_cast<const float4*>(src) + q);
+      } else {
+#pragma unroll
+        for (int q = 0; q < CH / 4; ++q) {
+          float4 v;
+          v.x = c0 + 4 * q + 0 < C ? __ldg(src + 4 * q + 0) : 0.f; v.y = c0 + 4 * q + 1 < C ? __ldg(src + 4 * q + 1) : 0.f;
+          v.z = c0 + 4 * q + 2 < C ? __ldg(src + 4 * q + 2) : 0.f; v.w = c0 + 4 * q + 3 < C ? __ldg(src + 4 * q + 3) : 0.f;
+          sm.f[threadIdx.x][q] = v;
+        }
+      }
+    }
+    __syncthreads();
+    unsigned int alive = 0;
+#pragma unroll
+    for (int k = 0; k < PX; ++k) if (!__all_sync(0xffffffffu, done[k])) alive |= 1u << k;
+    if (!alive) continue;
+    for (int jb = 0; jb < m; jb += 32) {
+      unsigned int hk[PX], any = 0;
+      float4 ta, tb;
+      if (jb + lane < m) { ta = sm.s0[jb + lane]; tb = sm.s1[jb + lane]; }
+#pragma unroll
+      for (int k = 0; k < PX; ++k) {
+        hk[k] = ((alive >> k) & 1u) ? __ballot_sync(0xffffffffu, jb + lane < m && patch_hit(ta, tb, sp.xm, sp.ym0 + 4.f * k, c_l2min)) : 0u;
+        any |= hk[k];
+      }
+      while (any) {
+        const int bit = __ffs(any) - 1;
+        any &= any - 1;
+        const int j = jb + bit;
+        const float4 a = sm.s0[j], b = sm.s1[j];
+        const float e1x = fmaf(a.x, x, a.w);
+#pragma unroll
+        for (int k = 0; k < PX; ++k) {
+          if (!((hk[k] >> bit) & 1u)) continue;
+          const float e1 = fmaf(a.y, y[k], e1x);
+          const float e2 = fmaf(a.z, y[k], b.x);
+          const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
+          if (done[k] || l2a < c_l2min) continue;
+          const float alpha = fminf(c_amax, ex2_approx(l2a));
+          if (alpha < c_amin) continue;
+          const float Tn = fmaf(-T[k], alpha, T[k]);
+          if (Tn < c_tmin) { done[k] = true; continue; }
+          const float wgt = alpha * T[k];
+#pragma unroll
+          for (int q = 0; q < CH / 4; ++q) {
+            const float4 f = sm.f[j][q];
+            acc[k][4 * q + 0] = fmaf(f.x, wgt, acc[k][4 * q + 0]); acc[k][4 * q + 1] = fmaf(f.y, wgt, acc[k][4 * q + 1]);
+            acc[k][4 * q + 2] = fmaf(f.z, wgt, acc[k][4 * q + 2]); acc[k][4 * q + 3] = fmaf(f.w, wgt, acc[k][4 * q + 3]);
+          }
+          T[k] = Tn;
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < PX; ++k) if (((alive >> k) & 1u) && __all_sync(0xffffffffu, done[k])) alive &= ~(1u << k);
+      if (!alive) break;
+    }
+  }
+  const size_t hw = (size_t)vp.width * vp.height;
+#pragma unroll
+  for (int k = 0; k < PX; ++k) {
+    if (!inside[k]) continue;
+    const size_t pix = (size_t)(ty * TILE + sp.ly0 + 4 * k) * vp.width + px;
+#pragma unroll
+    for (int c = 0; c < CH; ++c) if (c0 + c < C) out[(size_t)(c0 + c) * hw + pix] = acc[k][c];
+  }
+}
+
 // ---------------------------------------------------------------------------------------------
 // Sum of 8 values over the 32 lanes with 9 shuffles (halving exchange), result k lands on lane 4k.
 __device__ __forceinline__ float warp_reduce8(float v[8], const int lane) {
@@ -625,6 +732,18 @@ void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, con
   }
 #undef FDGS_BWD
   ++g_launches;
+}
+
+void launch_blend_feat_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* feat, int C,
+                           float* out, cudaStream_t st) {
+  const int tiles = vp.tiles_x * vp.tiles_y;
+  for (int c0 = 0; c0 < C;) {                    // 16 channels per pass, a tail of <= 4 in a 4-channel pass
+    static const bool no32 = getenv("FDGS_FEAT_NO32") != nullptr;     // A/B runs: two 16-channel passes instead of one of 32
+    if (C - c0 >= 32 && !no32) { blend_feat_fwd_kernel<32><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, feat, C, c0, out); c0 += 32; }
+    else if (C - c0 > 4) { blend_feat_fwd_kernel<16><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, feat, C, c0, out); c0 += 16; }
+    else { blend_feat_fwd_kernel<4><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, feat, C, c0, out); c0 += 4; }
+    ++g_launches;
+  }
 }
 
 }  // namespace fdgs

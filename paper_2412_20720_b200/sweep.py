@@ -128,6 +128,33 @@ def train_terms(flush, n=1_000_000):
     print(json.dumps(out), flush=True)
 
 
+def feature_terms(flush, n=1_000_000, C=32):
+    """Feature channels (D = 32) and optical flow at cfg3's size, view 0: ms per call next to the colour
+    forward / backward of the same view."""
+    import torch
+    from . import fdgs, scenes
+    sc = scenes.multiview_video(N=n, n_views=1)
+    ds = fdgs.DeviceScene.from_scene(sc)
+    v = sc.views[0]
+    r = fdgs.Renderer(ds, v.width, v.height, 1 << 24)
+    cv = fdgs.make_view(v)
+    r.preprocess(cv, sync=True)
+    r.forward(cv)
+    feat = torch.randn((n, C), device="cuda")
+    G = torch.randn((C, v.height, v.width), device="cuda")
+    gf, g = torch.zeros_like(feat), ds.zero_grads()
+    out = {"config": "feature_terms", "N": n, "C": C, "width": v.width, "height": v.height}
+    out["colour_forward_ms"] = _timed(lambda: r.forward(cv), 10, 3, flush)
+    out["colour_backward_ms"] = _timed(lambda: r.backward(cv, G[:3].contiguous(), g), 10, 3, flush)
+    out["features_forward_ms"] = _timed(lambda: r.features_forward(cv, feat), 10, 3, flush)
+    out["features_backward_ms"] = _timed(lambda: r.features_backward(cv, feat, G, gf, g), 10, 3, flush)
+    out["features_backward_feat_only_ms"] = _timed(lambda: r.features_backward(cv, feat, G, gf, None), 10, 3, flush)
+    out["splat_flow_ms"] = _timed(lambda: r.splat_flow(cv, 1.0 / 30.0), 10, 3, flush)
+    flow = r.splat_flow(cv, 1.0 / 30.0)
+    out["flow_map_forward_ms"] = _timed(lambda: r.features_forward(cv, flow), 10, 3, flush)
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--frames", type=int, default=24)
@@ -144,6 +171,7 @@ def main():
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
     if args.train_terms:
         train_terms(flush)
+        feature_terms(flush)
         return
     if not args.skip_train:
         train_cfg("cfg2_object", scenes.single_object(), 1 << 22, flush)
