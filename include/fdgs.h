@@ -220,9 +220,12 @@ int fdgs_debug_measure_peaks(void *scratch_dev, size_t scratch_bytes, void *cuda
  * "The 2D feature F at a specific view could be rendered following the same process as in Section 3.2, with the color c
  * replaced by the normalized feature vector f":  F[c](pixel) = sum_k feat[k,c] alpha_k T_k over the same
  * per-tile depth-ordered lists, thresholds and termination as the colour image; no background term.
- * Call after fdgs_preprocess + fdgs_render_forward on the same ws / view / config.  The C channels go through the
- * 3-channel blend kernels three at a time (ceil(C/3) launches).  scratch: device buffer of
- * fdgs_features_scratch_bytes(N, W, H) bytes, 16-byte aligned, caller-owned (record copies + one 3-plane image).
+ * Call after fdgs_preprocess + fdgs_render_forward on the same ws / view / config (tile lists and records are reused).
+ * Forward: a dedicated C-channel kernel, alpha evaluated once per 32 channels (ceil(C/32) launches), every skip and
+ * termination decision bit-identical to the colour pass.  Backward with grads == NULL (geometry frozen, the setting of
+ * L300): a dedicated front-to-back kernel, 32 channels per launch.  Backward with grads != NULL: the 3-channel backward
+ * blend kernel three channels at a time (ceil(C/3) launches) on a copy of the records in `scratch`.
+ * scratch: device buffer of fdgs_features_scratch_bytes(N, W, H) bytes, 16-byte aligned, caller-owned.
  * ------------------------------------------------------------------------------------------------------------------ */
 int fdgs_features_scratch_bytes(int32_t N, int32_t W, int32_t H, size_t *bytes_host);
 

@@ -34,6 +34,20 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+CMP_LIB = os.path.join(HERE, "libfdgs_cubcmp.so")
+
+
+def build_compare(force: bool = False) -> str:
+    """The CUB comparison sort (csrc/compare/): a separate library, used only by `sweep --sort-compare`."""
+    src = os.path.join(CSRC, "compare", "cub_sort_compare.cu")
+    if force or not os.path.exists(CMP_LIB) or os.path.getmtime(CMP_LIB) < os.path.getmtime(src):
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
+        subprocess.run([nvcc, *flags, "-shared", "-o", CMP_LIB, src], check=True)
+    return CMP_LIB
+
+
 if __name__ == "__main__":
     build(force="--force" in sys.argv, verbose="-v" in sys.argv)
+    build_compare(force="--force" in sys.argv)
     print(LIB)

@@ -468,6 +468,11 @@ int fdgs_render_features_backward(const fdgs_scene* sc, const fdgs_view* v, cons
   const size_t HW = (size_t)v->width * v->height;
   Workspace wf = ws;
   wf.rec = fs.rec;
+  if (!g) {   // geometry frozen: dL/dfeat only needs the weights alpha_k T_k — dedicated front-to-back kernel
+    launch_blend_feat_bwd(ws, l2, vp, cp, dL_dout, C, grad_feat, st);
+    FDGS_CUDA(cudaGetLastError(), "feature backward launches");
+    return FDGS_OK;
+  }
   FDGS_CUDA(cudaMemsetAsync(ws.g9, 0, sizeof(float) * 9 * (size_t)sc->N, st), "memset(g9)");
   for (int c0 = 0; c0 < C; c0 += 3) {
     const int n = C - c0 < 3 ? C - c0 : 3;

@@ -271,6 +271,134 @@ __global__ void __launch_bounds__(128) blend_feat_fwd_kernel(const uint2* __rest
   }
 }
 
+// dL/dfeat alone (geometry frozen — the setting of PAPER.md:L300 "for a pre-trained 4DGS, we introduce a feature vector"):
+//     dL/df_k[c] = sum_pixels alpha_k T_k dL/dF[c](pixel)
+// needs only the weights alpha_k T_k, so it is a FRONT-TO-BACK walk (the one of the forward kernels, same decisions) and
+// the reduction over pixels is a small dense product [hits x pixels] . [pixels x channels].  Transposed accumulation:
+// a warp parks the weights of its 64 pixels for 8 hit splats in shared memory, then turns round with LANE = CHANNEL:
+// lane c sums w[hit][pixel] * g[pixel][c] over the strip for the 8 hits (1 conflict-free LDS of g and 2 broadcast LDS.128
+// of w per 8 FFMA) and adds the result to grad_feat with one coalesced 128-byte reduction per hit.  32 channels per pass.
+__global__ void __launch_bounds__(128) blend_feat_bwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
+                                                             const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
+                                                             const float* __restrict__ dL_dout, const int C, const int c0,
+                                                             float* __restrict__ grad_feat) {
+  constexpr int PX = 2, BATCH = 128, HB = 8, GS = 33;
+  __shared__ struct {
+    float4 s0[BATCH], s1[BATCH], s2[BATCH];
+    unsigned int id[BATCH];
+    float g[256 * GS];               // dL/dF of the tile, [pixel][channel], stride 33: conflict-free both ways
+    float4 w[4][64][HB / 4];         // per warp: weights of its 64 pixels for HB parked hits
+    unsigned int hid[4][HB];
+  } sm;
+  const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const Strip<PX> sp(warp, lane);
+  const int px = tx * TILE + sp.lx;
+  const float x = sp.lx + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
+  const size_t hw = (size_t)vp.width * vp.height;
+  // stage dL/dF: thread t owns tile pixels t and t + 128
+  for (int p = threadIdx.x; p < 256; p += 128) {
+    const int gx = tx * TILE + (p & 15), gy = ty * TILE + (p >> 4);
+    const bool in = gx < vp.width && gy < vp.height;
+    const size_t pix = (size_t)gy * vp.width + gx;
+#pragma unroll 8
+    for (int c = 0; c < 32; ++c) sm.g[p * GS + c] = (in && c0 + c < C) ? __ldg(dL_dout + (size_t)(c0 + c) * hw + pix) : 0.f;
+  }
+  float y[PX], T[PX];
+  bool done[PX];
+  int tp[PX];                        // tile pixel index of the lane's two pixels
+#pragma unroll
+  for (int k = 0; k < PX; ++k) {
+    const int ly = sp.ly0 + 4 * k;
+    y[k] = ly + 0.5f; T[k] = 1.f;
+    done[k] = !(px < vp.width && ty * TILE + ly < vp.height);
+    tp[k] = ly * 16 + sp.lx;
+  }
+  const uint2 range = ranges[tile];
+  const int n = (int)(range.y - range.x);
+  float c_l2min = cp.log2_alpha_min, c_amax = cp.alpha_max, c_amin = cp.alpha_min, c_tmin = cp.transmittance_min;
+  asm volatile("" : "+f"(c_l2min), "+f"(c_amax), "+f"(c_amin), "+f"(c_tmin));
+  int nbuf = 0;
+  float* wl = reinterpret_cast<float*>(sm.w[warp]);         // [64][HB] floats
+  auto flush = [&](const int count) {
+    __syncwarp();
+    float acc[HB];
+#pragma unroll
+    for (int h = 0; h < HB; ++h) acc[h] = 0.f;
+    for (int q = 0; q < 64; ++q) {
+      const int tpq = ((q >> 5) * 4 + sp.ly0 - (lane >> 3) + ((q & 31) >> 3)) * 16 + (sp.lx - (lane & 7)) + (q & 7);
+      const float gq = sm.g[tpq * GS + lane];
+      const float4 w0 = sm.w[warp][q][0], w1 = sm.w[warp][q][1];
+      acc[0] = fmaf(w0.x, gq, acc[0]); acc[1] = fmaf(w0.y, gq, acc[1]); acc[2] = fmaf(w0.z, gq, acc[2]); acc[3] = fmaf(w0.w, gq, acc[3]);
+      acc[4] = fmaf(w1.x, gq, acc[4]); acc[5] = fmaf(w1.y, gq, acc[5]); acc[6] = fmaf(w1.z, gq, acc[6]); acc[7] = fmaf(w1.w, gq, acc[7]);
+    }
+    if (c0 + lane < C) {
+#pragma unroll
+      for (int h = 0; h < HB; ++h)
+        if (h < count && acc[h] != 0.f) atomicAdd(grad_feat + (size_t)sm.hid[warp][h] * C + c0 + lane, acc[h]);
+    }
+    __syncwarp();
+  };
+  for (int base = 0; base < n; base += BATCH) {
+    if (__syncthreads_and(done[0] && done[1])) break;
+    const int m = min(BATCH, n - base);
+    if ((int)threadIdx.x < m) {
+      const unsigned int id = vals[range.x + base + threadIdx.x];
+      sm.id[threadIdx.x] = id;
+      stage_splat(rec, id, ox, oy, &sm.s0[threadIdx.x], &sm.s1[threadIdx.x], &sm.s2[threadIdx.x]);
+    }
+    __syncthreads();
+    unsigned int alive = 0;
+#pragma unroll
+    for (int k = 0; k < PX; ++k) if (!__all_sync(0xffffffffu, done[k])) alive |= 1u << k;
+    if (alive) {
+      for (int jb = 0; jb < m; jb += 32) {
+        unsigned int hk[PX], any = 0;
+        float4 ta, tb;
+        if (jb + lane < m) { ta = sm.s0[jb + lane]; tb = sm.s1[jb + lane]; }
+#pragma unroll
+        for (int k = 0; k < PX; ++k) {
+          hk[k] = ((alive >> k) & 1u) ? __ballot_sync(0xffffffffu, jb + lane < m && patch_hit(ta, tb, sp.xm, sp.ym0 + 4.f * k, c_l2min)) : 0u;
+          any |= hk[k];
+        }
+        while (any) {
+          const int bit = __ffs(any) - 1;
+          any &= any - 1;
+          const int j = jb + bit;
+          const float4 a = sm.s0[j], b = sm.s1[j];
+          const float e1x = fmaf(a.x, x, a.w);
+          float wgt[PX];
+#pragma unroll
+          for (int k = 0; k < PX; ++k) {
+            wgt[k] = 0.f;
+            if (!((hk[k] >> bit) & 1u)) continue;
+            const float e1 = fmaf(a.y, y[k], e1x);
+            const float e2 = fmaf(a.z, y[k], b.x);
+            const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
+            if (done[k] || l2a < c_l2min) continue;
+            const float alpha = fminf(c_amax, ex2_approx(l2a));
+            if (alpha < c_amin) continue;
+            const float Tn = fmaf(-T[k], alpha, T[k]);
+            if (Tn < c_tmin) { done[k] = true; continue; }
+            wgt[k] = alpha * T[k];
+            T[k] = Tn;
+          }
+          if (!__any_sync(0xffffffffu, wgt[0] != 0.f || wgt[1] != 0.f)) continue;
+          wl[lane * HB + nbuf] = wgt[0];
+          wl[(32 + lane) * HB + nbuf] = wgt[1];
+          if (lane == 0) sm.hid[warp][nbuf] = sm.id[j];
+          if (++nbuf == HB) { flush(HB); nbuf = 0; }
+        }
+#pragma unroll
+        for (int k = 0; k < PX; ++k) if (((alive >> k) & 1u) && __all_sync(0xffffffffu, done[k])) alive &= ~(1u << k);
+        if (!alive) break;
+      }
+    }
+    // the hit buffers reference sm.id of this batch only through hid (copied), so the next batch may overwrite the staging
+  }
+  if (nbuf) flush(nbuf);
+}
+
 // ---------------------------------------------------------------------------------------------
 // Sum of 8 values over the 32 lanes with 9 shuffles (halving exchange), result k lands on lane 4k.
 __device__ __forceinline__ float warp_reduce8(float v[8], const int lane) {
@@ -732,6 +860,15 @@ void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, con
   }
 #undef FDGS_BWD
   ++g_launches;
+}
+
+void launch_blend_feat_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* dL_dout, int C,
+                           float* grad_feat, cudaStream_t st) {
+  const int tiles = vp.tiles_x * vp.tiles_y;
+  for (int c0 = 0; c0 < C; c0 += 32) {
+    blend_feat_bwd_kernel<<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dout, C, c0, grad_feat);
+    ++g_launches;
+  }
 }
 
 void launch_blend_feat_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* feat, int C,

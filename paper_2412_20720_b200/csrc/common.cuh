@@ -170,6 +170,8 @@ void launch_preprocess_bwd(const fdgs_scene& sc, const ViewParams& vp, const Cfg
 void launch_cull_status(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, unsigned char* dst, cudaStream_t st);
 void launch_blend_feat_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* feat, int C,
                            float* out, cudaStream_t st);
+void launch_blend_feat_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* dL_dout, int C,
+                           float* grad_feat, cudaStream_t st);
 void launch_feature_records(const Workspace& ws, const float* feat, int C, int c0, int N, SplatRec* dst, cudaStream_t st);
 void launch_extract_feature_grads(const Workspace& ws, float* grad_feat, int C, int c0, int N, cudaStream_t st);
 void launch_splat_flow(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, float dt_next, float* flow,

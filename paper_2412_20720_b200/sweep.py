@@ -15,8 +15,13 @@ import json
 import numpy as np
 
 
+ONCE = False      # --once: every operation runs twice (1 warm-up + 1 timed) so that a profiler capture covers all kernels
+
+
 def _timed(fn, iters, warm, flush):
     import torch
+    if ONCE:
+        iters, warm = 1, 1
     for _ in range(warm):
         fn()
     torch.cuda.synchronize()
@@ -128,6 +133,98 @@ def train_terms(flush, n=1_000_000):
     print(json.dumps(out), flush=True)
 
 
+def sort_compare(flush):
+    """north_star: "a hand-written device radix sort ... (CUB only as a comparison)".  For one view of cfg3 and of cfg4: the
+    library's whole binning stage (compaction + tile grid + depth sort + offsets + pair emission + tile sort, CUDA events
+    inside the library) next to cub::DeviceRadixSort::SortPairs over the same D pairs as literal 64-bit tile|depth keys
+    (32 + ceil(log2 tiles) significant bits) — the single sort of [23]'s rasterizer, which additionally needs the key
+    emission and a range-finding pass that are not timed here."""
+    import ctypes as C
+    import torch
+    from . import build, fdgs, scenes
+    cmp_lib = C.CDLL(build.build_compare())
+    cmp_lib.fdgs_cmp_cub_sort_pairs.argtypes = [C.c_void_p] * 4 + [C.c_int64, C.c_int, C.c_void_p, C.POINTER(C.c_size_t), C.c_void_p]
+    for name, sc, cap in (("cfg3_video", scenes.multiview_video(n_views=1), 1 << 24), ("cfg4_driving", scenes.driving(n_views=1), 160 << 20)):
+        ds = fdgs.DeviceScene.from_scene(sc)
+        v = sc.views[0]
+        r = fdgs.Renderer(ds, v.width, v.height, cap)
+        cv = fdgs.make_view(v)
+        fdgs.set_stage_timing(True)
+        ours = {k: 0.0 for k in fdgs.STAGES[1:5]}
+        reps = 1 if ONCE else 10
+        for _ in range(reps + 2):
+            flush.fill_(1)
+            r.preprocess(cv)
+            r.forward(cv)
+            torch.cuda.synchronize()
+            st = fdgs.stage_ms()
+            if _ >= 2:
+                for k in ours:
+                    ours[k] += st[k] / reps
+        fdgs.set_stage_timing(False)
+        status = r.export(fdgs.EXPORT_STATUS)
+        D = status["num_pairs"]
+        keys_sorted = r.export(fdgs.EXPORT_SORTED_KEYS)[:D].contiguous()
+        vals_sorted = r.export(fdgs.EXPORT_SORTED_VALS)[:D].contiguous()
+        perm = torch.randperm(D, device="cuda")
+        keys_in, vals_in = keys_sorted[perm].contiguous(), vals_sorted[perm].contiguous()
+        keys_out, vals_out = torch.empty_like(keys_in), torch.empty_like(vals_in)
+        tiles = ((v.width + 15) // 16) * ((v.height + 15) // 16)
+        end_bit = 32 + max(1, (tiles - 1).bit_length())
+        nbytes = C.c_size_t(0)
+        stream = torch.cuda.current_stream().cuda_stream
+        rc = cmp_lib.fdgs_cmp_cub_sort_pairs(None, None, None, None, D, end_bit, None, C.byref(nbytes), stream)
+        assert rc == 0, rc
+        temp = torch.empty(max(int(nbytes.value), 1), dtype=torch.uint8, device="cuda")
+
+        def cub():
+            rc = cmp_lib.fdgs_cmp_cub_sort_pairs(keys_in.data_ptr(), keys_out.data_ptr(), vals_in.data_ptr(), vals_out.data_ptr(), D,
+                                                 end_bit, temp.data_ptr(), C.byref(nbytes), stream)
+            assert rc == 0, rc
+        ms_cub = _timed(cub, 10, 3, flush)
+        torch.cuda.synchronize()
+        same = bool(torch.equal(keys_out.view(torch.int64), keys_sorted.view(torch.int64)))
+        print(json.dumps({"config": "sort_compare_" + name, "N": sc.N, "pairs": D, "visible": status["num_visible"], "key_bits": end_bit,
+                          "ours_ms": ours, "ours_total_ms": sum(ours.values()),
+                          "ours_sorts_only_ms": ours["sort_depth"] + ours["sort_tile"],
+                          "cub_sortpairs_64bit_ms": ms_cub, "cub_keys_equal_ours": same,
+                          "note": "ours_total includes compaction, tile ranges, offsets and pair emission; the CUB figure is the sort alone"}),
+              flush=True)
+        del r, ds, keys_in, vals_in, keys_out, vals_out, keys_sorted, vals_sorted, perm, temp
+        torch.cuda.empty_cache()
+
+
+def full_training_step(flush):
+    """cfg3 step with the optimiser inside the timed region: fdgs_step_batch (4 views) + fdgs_regularizers + dense Adam over
+    all six arrays (gradients cleared by the Adam pass)."""
+    import torch
+    from . import fdgs, scenes, train
+    sc = scenes.multiview_video()
+    ds = fdgs.DeviceScene.from_scene(sc)
+    v0 = sc.views[0]
+    bs = fdgs.BatchStep(ds, v0.width, v0.height, 1 << 24, len(sc.views))
+    cvs = [fdgs.make_view(v) for v in sc.views]
+    for i, rr in enumerate(bs.renderers):
+        rr.target_dev.copy_(torch.from_numpy(scenes.target_image(sc.seed, i, v0.width, v0.height)).cuda())
+    g = ds.zero_grads()
+    opt = train.Adam(ds, {k: 1e-6 for k in train.PARAMS})
+
+    def render_only():
+        for a in g.values():
+            if a is not None:
+                a.zero_()
+        bs.step(cvs, g)
+
+    def step():
+        bs.step(cvs, g)
+        train.regularizers(ds, g, lambda_sparse=1e-4, lambda_covt=1e-4)
+        opt.step(g, zero_grad=True)
+    ms0 = _timed(render_only, 10, 3, flush)
+    ms1 = _timed(step, 10, 3, flush)
+    print(json.dumps({"config": "cfg3_full_training_step", "N": sc.N, "views_per_step": len(sc.views),
+                      "render_fwd_bwd_ms": ms0, "with_regularizers_and_adam_ms": ms1, "steps_per_s_with_optimizer": 1e3 / ms1}), flush=True)
+
+
 def feature_terms(flush, n=1_000_000, C=32):
     """Feature channels (D = 32) and optical flow at cfg3's size, view 0: ms per call next to the colour
     forward / backward of the same view."""
@@ -161,17 +258,25 @@ def main():
     ap.add_argument("--max-n", type=int, default=8_000_000)
     ap.add_argument("--skip-train", action="store_true")
     ap.add_argument("--skip-sweep", action="store_true")
+    ap.add_argument("--once", action="store_true", help="one warm-up and one timed iteration per operation (for ncu captures)")
+    ap.add_argument("--sort-compare", action="store_true", help="binning stage vs cub::DeviceRadixSort on 64-bit keys (comparison only)")
     ap.add_argument("--train-terms", action="store_true", help="time the f2-f4 kernels (mask, regularisers, Adam, decode) only")
     args = ap.parse_args()
+    global ONCE
+    ONCE = args.once
     import torch
     from . import build, scenes
     if not torch.cuda.is_available():
         raise RuntimeError("sweep needs a CUDA device: the product has no CPU fallback")
     build.build()
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+    if args.sort_compare:
+        sort_compare(flush)
+        return
     if args.train_terms:
         train_terms(flush)
         feature_terms(flush)
+        full_training_step(flush)
         return
     if not args.skip_train:
         train_cfg("cfg2_object", scenes.single_object(), 1 << 22, flush)
