@@ -306,13 +306,11 @@ __global__ void __launch_bounds__(128) blend_feat_bwd_kernel(const uint2* __rest
   }
   float y[PX], T[PX];
   bool done[PX];
-  int tp[PX];                        // tile pixel index of the lane's two pixels
 #pragma unroll
   for (int k = 0; k < PX; ++k) {
     const int ly = sp.ly0 + 4 * k;
     y[k] = ly + 0.5f; T[k] = 1.f;
     done[k] = !(px < vp.width && ty * TILE + ly < vp.height);
-    tp[k] = ly * 16 + sp.lx;
   }
   const uint2 range = ranges[tile];
   const int n = (int)(range.y - range.x);
