@@ -169,7 +169,7 @@ __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __rest
 // per-splat feature values per pass instead of (r, g, b): alpha is evaluated once for CH channels.  feat[N,C] is gathered
 // by id into shared memory next to the splat records; channels c0 .. c0+CH-1 (zero beyond C); no background.
 template <int CH>
-__global__ void __launch_bounds__(128) blend_feat_fwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
+__global__ void __launch_bounds__(128, CH == 32 ? 4 : (CH == 4 ? 9 : 1)) blend_feat_fwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
                                                              const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
                                                              const float* __restrict__ feat, const int C, const int c0,
                                                              float* __restrict__ out) {
@@ -282,9 +282,9 @@ __global__ void __launch_bounds__(128) blend_feat_bwd_kernel(const uint2* __rest
                                                              const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
                                                              const float* __restrict__ dL_dout, const int C, const int c0,
                                                              float* __restrict__ grad_feat) {
-  constexpr int PX = 2, BATCH = 128, HB = 8, GS = 33;
+  constexpr int PX = 2, BATCH = 64, HB = 8, GS = 33;     // 44 KB of shared memory: 5 CTAs per SM
   __shared__ struct {
-    float4 s0[BATCH], s1[BATCH], s2[BATCH];
+    float4 s0[BATCH], s1[BATCH];
     unsigned int id[BATCH];
     float g[256 * GS];               // dL/dF of the tile, [pixel][channel], stride 33: conflict-free both ways
     float4 w[4][64][HB / 4];         // per warp: weights of its 64 pixels for HB parked hits
@@ -343,7 +343,8 @@ __global__ void __launch_bounds__(128) blend_feat_bwd_kernel(const uint2* __rest
     if ((int)threadIdx.x < m) {
       const unsigned int id = vals[range.x + base + threadIdx.x];
       sm.id[threadIdx.x] = id;
-      stage_splat(rec, id, ox, oy, &sm.s0[threadIdx.x], &sm.s1[threadIdx.x], &sm.s2[threadIdx.x]);
+      float4 unused;                  // colours are not needed here
+      stage_splat(rec, id, ox, oy, &sm.s0[threadIdx.x], &sm.s1[threadIdx.x], &unused);
     }
     __syncthreads();
     unsigned int alive = 0;
