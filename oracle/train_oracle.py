@@ -102,7 +102,9 @@ def regularizers(log_scale, quat_l, quat_r, mask_logit=None, lambda_sparse=1.0, 
     if mask_logit is not None:
         M = sigmoid(mask_logit)                         # eq. 24: L_mask = mean_i M_i,  M = Sigmoid(m) (L215)
         losses["mask"] = float(M.mean())
-        grads["mask_logit"] = lambda_mask * M * (1.0 - M) / N
+        # dM/dm = M (1 - M), evaluated as Sigmoid(m) Sigmoid(-m): the same quantity without the cancellation of 1 - M for
+        # saturated m (|m| > 37 rounds M to exactly 0 or 1 in float64)
+        grads["mask_logit"] = lambda_mask * M * sigmoid(-np.asarray(mask_logit, dtype=np.float64)) / N
     return losses, grads
 
 
@@ -132,7 +134,7 @@ def mask_backward(mask_logit, eps, opacity_logit, g_log_scale, g_opacity_logit):
     Mh = mask_hat(mask_logit, eps)
     one_minus = sigmoid(-np.asarray(opacity_logit, dtype=np.float64))      # 1 - alpha
     dL_dMhat = np.asarray(g_log_scale, dtype=np.float64).sum(axis=1) + np.asarray(g_opacity_logit, dtype=np.float64) / one_minus
-    return Mh * dL_dMhat * M * (1.0 - M)
+    return Mh * dL_dMhat * M * sigmoid(-np.asarray(mask_logit, dtype=np.float64))      # M (1 - M) without cancellation
 
 
 # ---------------------------------------------------------------------------------------------------------------

@@ -93,7 +93,7 @@ __global__ void __launch_bounds__(256) regularizers_kernel(const fdgs_scene sc, 
         S44 = fmaf(r4[k] * r4[k], s2[k], S44);
       }
       const float e = expf(-S44);
-      if (isfinite(e)) {
+      if (e > 0.f && isfinite(S44)) {     // e == 0 (Sigma_44 large or overflowed): loss and gradient vanish, 0 * inf must not appear
         l_covt = e;
         const float gS = -rc.lambda_covt * e * invN;
         float gr[4], gl[4];

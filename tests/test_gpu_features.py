@@ -82,6 +82,29 @@ def test_feature_maps_and_gradients_match_the_oracle(name, C):
     assert rel_l2(gf2.cpu().numpy(), ogf) < 1e-3
 
 
+@pytest.mark.parametrize("C", [1, 3, 4, 7, 16, 33, 36, 40, 67])
+def test_channel_counts_cover_every_pass_combination(C):
+    """32-, 16- and 4-channel forward instantiations, aligned and ragged row slices, one to three backward passes."""
+    sc = scenes.tiny()
+    view = _zero_bg(sc.views[0])
+    feat = scenes.normal(40 + C, 3, sc.N * C).reshape(sc.N, C).astype(np.float32)
+    G = scenes.normal(50 + C, 4, C * view.width * view.height).reshape(C, view.height, view.width).astype(np.float32)
+    ds, r, cv = _setup(sc, view)
+    ft = torch.from_numpy(feat).cuda()
+    F = r.features_forward(cv, ft)
+    gf = torch.zeros_like(ft)
+    r.features_backward(cv, ft, torch.from_numpy(G).cuda(), gf, None)
+    torch.cuda.synchronize()
+    o = run_pre(make_oracle(sc), view)
+    margin = o.forward()[3]
+    ok = margin > 1e-4
+    want = o.render_features(feat.astype(np.float64))
+    assert np.abs(F.cpu().numpy().astype(np.float64) - want)[:, ok].max() < 1e-4
+    if ok.all():                                                              # no threshold-fragile pixel in this scene
+        ogf, _ = o.backward_features(feat.astype(np.float64), G.astype(np.float64))
+        assert rel_l2(gf.cpu().numpy(), ogf) < 1e-3
+
+
 def test_constant_feature_is_one_minus_final_T_and_colour_path_is_untouched():
     sc = scenes.tiny()
     view = sc.views[0]

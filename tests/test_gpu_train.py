@@ -231,6 +231,53 @@ def test_training_loop_through_the_library_recovers_a_perturbed_scene():
         assert g[k].abs().max().item() == 0                                  # cleared by the optimiser for the next step
 
 
+def test_regularizers_and_adam_survive_extreme_parameters():
+    """Huge / tiny scales, saturated logits, denormal gradients, counts below one vector: finite results that match the oracle."""
+    N = 8
+    ls = np.array([[-40, -40, -40, -40], [30, 30, 30, 30], [0, 0, 0, 44.5], [-3, -2, -1, 0], [5, -5, 5, -5], [0, 0, 0, -20],
+                   [1, 1, 1, 1], [-1, -1, -1, 3]], dtype=np.float32)
+    r = np.random.default_rng(3)
+    ql = r.normal(size=(N, 4)).astype(np.float32)
+    qr = r.normal(size=(N, 4)).astype(np.float32)
+    ql[6] *= 1e-18
+    qr[7] *= 1e15
+    sc = scenes.Scene("x", 0, 1, np.zeros((N, 4), np.float32), ls, ql, qr, np.array([-60, 60, 0, 1, -1, 30, -30, 2], np.float32),
+                      np.zeros((N, 1, 3), np.float32), [], 0)
+    ds = fdgs.DeviceScene.from_scene(sc)
+    g = ds.zero_grads()
+    g["log_scale"] += 1e-3
+    g["opacity_logit"] += 1e-3
+    m = np.array([-50, 50, 0, 1, -1, 20, -20, 0.5], np.float32)
+    gm, losses = torch.zeros(N, device="cuda"), torch.zeros(3, device="cuda")
+    train.regularizers(ds, g, 0.5, 0.5, 0.5, _cuda(m), 0.3, gm, losses)
+    torch.cuda.synchronize()
+    L, G = T.regularizers(ls, ql, qr, m, 0.5, 0.5, 0.5)
+    want_m = G["mask_logit"] + T.mask_backward(m, 0.3, sc.opacity_logit, np.full((N, 4), 1e-3), np.full(N, 1e-3))
+    for k in ("log_scale", "quat_l", "quat_r"):
+        got = g[k].cpu().numpy().astype(np.float64) - (1e-3 if k == "log_scale" else 0.0)
+        assert np.isfinite(got).all()
+        assert np.abs(got - G[k]).max() <= 2e-5 * max(np.abs(G[k]).max(), 1e-30) + 1e-9, k      # fp32 against the largest entry
+    got_m = gm.cpu().numpy().astype(np.float64)
+    fin = np.isfinite(want_m)                                                # alpha = 1 in fp32 only: 1/(1-alpha) overflows there
+    assert np.isfinite(got_m).all() and np.abs(got_m[fin] - want_m[fin]).max() <= 1e-4 * np.abs(want_m[fin]).max()
+    np.testing.assert_allclose(losses.cpu().numpy(), [L["sparse"], L["covt"], L["mask"]], rtol=2e-5)
+    # Adam on 1, 3 and 5 elements (below / across one 128-bit vector), with a denormal and a huge gradient
+    for n in (1, 3, 5):
+        p0 = np.linspace(-1, 1, n).astype(np.float32)
+        gr = np.array([1e-40, 3e30, -2.0, 0.0, 7e-12][:n], dtype=np.float32)
+        p, mm, vv = _cuda(p0), torch.zeros(n, device="cuda"), torch.zeros(n, device="cuda")
+        train.adam_step(p, _cuda(gr), mm, vv, 1, float(np.float32(0.01)), float(np.float32(0.9)), float(np.float32(0.999)), float(np.float32(1e-15)))
+        torch.cuda.synchronize()
+        op, om, ov = T.adam_step(p0.astype(np.float64), gr.astype(np.float64), np.zeros(n), np.zeros(n), 1, float(np.float32(0.01)),
+                                 float(np.float32(0.9)), float(np.float32(0.999)), float(np.float32(1e-15)))
+        got = p.cpu().numpy().astype(np.float64)
+        big = np.abs(gr) > 1e19                                              # g^2 overflows fp32: v = inf, the update is 0 instead of lr
+        assert np.isfinite(got).all()
+        small = np.abs(gr) < 1e-30                                           # g^2 underflows fp32: m / (0 + eps) instead of sign(g) lr
+        sel = ~big & ~small
+        np.testing.assert_allclose(got[sel], op[sel], rtol=0, atol=3e-6)
+
+
 def test_train_entry_points_validate_arguments():
     lib = fdgs.load()
     assert lib.fdgs_mask_apply(None, 0.5, None, None, 10, None) == fdgs.ERR_INVALID
