@@ -1,6 +1,7 @@
 // api.cu — the C ABI of include/fdgs.h: argument validation, workspace carve-up, launch sequence.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 
 #include "common.cuh"
@@ -347,8 +348,16 @@ int fdgs_step_batch(const fdgs_scene* sc, const fdgs_view* views, int32_t num_vi
   }
   cudaStream_t st = (cudaStream_t)stream;
   if (!g_batch_fork) {
+    // FDGS_BATCH_PRIO (experiment): view i's stream gets a higher priority than view i+1's, so that the views drift apart
+    // and the HBM-bound stages of one overlap the issue-bound blend kernels of the next
+    int lo = 0, hi = 0;
+    cudaDeviceGetStreamPriorityRange(&lo, &hi);          // lo = least priority (numerically largest)
+    const char* pe = getenv("FDGS_BATCH_PRIO");
+    const int prio_mode = pe ? atoi(pe) : 0;
     for (int i = 0; i < FDGS_MAX_BATCH; ++i) {
-      FDGS_CUDA(cudaStreamCreateWithFlags(&g_worker[i], cudaStreamNonBlocking), "worker stream");
+      int pr = lo;
+      if (prio_mode == 1) { pr = hi + i; if (pr > lo) pr = lo; }
+      FDGS_CUDA(cudaStreamCreateWithPriority(&g_worker[i], cudaStreamNonBlocking, pr), "worker stream");
       FDGS_CUDA(cudaEventCreateWithFlags(&g_b2_done[i], cudaEventDisableTiming), "worker event");
     }
     FDGS_CUDA(cudaStreamCreateWithFlags(&g_zero_stream, cudaStreamNonBlocking), "zero stream");
