@@ -61,6 +61,8 @@ static void make_params(const fdgs_view* v, const fdgs_config* c, ViewParams& vp
   cp.transmittance_min = c->transmittance_min; cp.dilation = c->dilation; cp.cutoff_sigma = c->cutoff_sigma;
   cp.znear = c->znear; cp.guard = c->guard;
   cp.log2_alpha_min = c->alpha_min > 0.f ? log2f(c->alpha_min) * (1.0f + 1e-6f) - 1e-6f : -INFINITY;
+  cp.default_thresholds = c->alpha_min == FDGS_DEF_ALPHA_MIN && c->alpha_max == FDGS_DEF_ALPHA_MAX && c->transmittance_min == FDGS_DEF_T_MIN;
+  if (cp.default_thresholds) cp.log2_alpha_min = FDGS_DEF_L2MIN;   // every kernel, specialised or not, compares against the same value
 }
 
 __global__ void init_header_kernel(WsHeader* hdr, long long N, long long K, long long W, long long H, long long cap, long long tiles) {

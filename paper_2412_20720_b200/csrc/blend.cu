@@ -59,7 +59,8 @@ struct Strip {
 // exp2, [2] pairs composited, [3] splats staged into shared memory (summed over tiles).
 // AUX = true additionally composites the camera depth of the splats like a fourth colour channel without background
 // (rendered depth, eq. 29) into depth_map[H,W].
-template <int PX, bool STATS, bool AUX>
+// DEF = true: the thresholds of [23] as immediates (cp.default_thresholds; see common.cuh).
+template <int PX, bool STATS, bool AUX, bool DEF>
 __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
                                                              const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
                                                              float* __restrict__ image, float* __restrict__ final_T,
@@ -72,25 +73,27 @@ __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __rest
   const Strip<PX> sp(warp, lane);
   const int px = tx * TILE + sp.lx;
   const float x = sp.lx + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
-  float y[PX], T[PX], Cr[PX], Cg[PX], Cb[PX], Dz[PX];
+  const float c_l2min = DEF ? FDGS_DEF_L2MIN : cp.log2_alpha_min, c_amax = DEF ? FDGS_DEF_ALPHA_MAX : cp.alpha_max;
+  const float c_amin = DEF ? FDGS_DEF_ALPHA_MIN : cp.alpha_min, c_tmin = DEF ? FDGS_DEF_T_MIN : cp.transmittance_min;
+  // lmin[k]: the skip threshold of pixel k, +inf once the pixel has terminated (or lies outside the image) — the "done"
+  // state costs no flag and no extra test in the loop
+  float y[PX], T[PX], Cr[PX], Cg[PX], Cb[PX], Dz[PX], lmin[PX];
   unsigned int last[PX];
-  bool done[PX], inside[PX];
+  bool inside[PX];
+#define FDGS_DONE(k) (lmin[k] > 3.0e38f)
 #pragma unroll
   for (int k = 0; k < PX; ++k) {
     const int ly = sp.ly0 + 4 * k;
     inside[k] = px < vp.width && ty * TILE + ly < vp.height;
-    y[k] = ly + 0.5f; T[k] = 1.f; Cr[k] = Cg[k] = Cb[k] = Dz[k] = 0.f; last[k] = 0; done[k] = !inside[k];
+    y[k] = ly + 0.5f; T[k] = 1.f; Cr[k] = Cg[k] = Cb[k] = Dz[k] = 0.f; last[k] = 0; lmin[k] = inside[k] ? c_l2min : INFINITY;
   }
   const uint2 range = ranges[tile];
   const int n = (int)(range.y - range.x);
-  // thresholds pinned in registers (otherwise each use re-reads the constant bank: an issue slot per use in this loop)
-  float c_l2min = cp.log2_alpha_min, c_amax = cp.alpha_max, c_amin = cp.alpha_min, c_tmin = cp.transmittance_min;
-  asm volatile("" : "+f"(c_l2min), "+f"(c_amax), "+f"(c_amin), "+f"(c_tmin));
   unsigned int st_walk = 0, st_exp = 0, st_comp = 0, st_stage = 0;
   for (int base = 0; base < n; base += BATCH) {
     bool all_done = true;
 #pragma unroll
-    for (int k = 0; k < PX; ++k) all_done = all_done && done[k];
+    for (int k = 0; k < PX; ++k) all_done = all_done && FDGS_DONE(k);
     if (__syncthreads_and(all_done)) break;
     const int m = min(BATCH, n - base);
     if (STATS && threadIdx.x == 0) st_stage += m;
@@ -98,7 +101,7 @@ __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __rest
     __syncthreads();
     unsigned int alive = 0;                           // sub-patches with an unsaturated pixel (warp-uniform)
 #pragma unroll
-    for (int k = 0; k < PX; ++k) if (!__all_sync(0xffffffffu, done[k])) alive |= 1u << k;
+    for (int k = 0; k < PX; ++k) if (!__all_sync(0xffffffffu, FDGS_DONE(k))) alive |= 1u << k;
     if (!alive) continue;
     for (int jb = 0; jb < m; jb += 32) {
       // lane l tests splat jb+l against each live sub-patch; the ballots list the splats worth evaluating per pixel
@@ -123,13 +126,15 @@ __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __rest
           const float e1 = fmaf(a.y, y[k], e1x);
           const float e2 = fmaf(a.z, y[k], b.x);
           const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
-          if (STATS && !done[k]) ++st_walk;
-          if (done[k] || l2a < c_l2min) continue;              // alpha < alpha_min: skipped
+          if (STATS && !FDGS_DONE(k)) ++st_walk;
+          if (!(l2a >= lmin[k])) continue;                     // alpha < alpha_min (or pixel done): skipped
           const float alpha = fminf(c_amax, ex2_approx(l2a));
           if (STATS) ++st_exp;
           if (alpha < c_amin) continue;
           const float Tn = fmaf(-T[k], alpha, T[k]);
-          if (Tn < c_tmin) { done[k] = true; continue; }   // the terminating splat is not composited
+          const bool term = Tn < c_tmin;                       // the terminating splat is not composited
+          lmin[k] = term ? INFINITY : lmin[k];
+          if (term) continue;
           const float wgt = alpha * T[k];
           Cr[k] = fmaf(b.z, wgt, Cr[k]); Cg[k] = fmaf(b.w, wgt, Cg[k]); Cb[k] = fmaf(sm.s2[j].x, wgt, Cb[k]);
           if (AUX) Dz[k] = fmaf(sm.s2[j].w, wgt, Dz[k]);
@@ -139,10 +144,11 @@ __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __rest
         }
       }
 #pragma unroll
-      for (int k = 0; k < PX; ++k) if (((alive >> k) & 1u) && __all_sync(0xffffffffu, done[k])) alive &= ~(1u << k);
+      for (int k = 0; k < PX; ++k) if (((alive >> k) & 1u) && __all_sync(0xffffffffu, FDGS_DONE(k))) alive &= ~(1u << k);
       if (!alive) break;
     }
   }
+#undef FDGS_DONE
   if (STATS) {
     unsigned int v[4] = {st_walk, st_exp, st_comp, st_stage};
 #pragma unroll
@@ -241,7 +247,7 @@ __global__ void __launch_bounds__(128, CH == 32 ? 4 : (CH == 4 ? 9 : 1)) blend_f
           const float e1 = fmaf(a.y, y[k], e1x);
           const float e2 = fmaf(a.z, y[k], b.x);
           const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
-          if (done[k] || l2a < c_l2min) continue;
+          if (done[k] || !(l2a >= c_l2min)) continue;
           const float alpha = fminf(c_amax, ex2_approx(l2a));
           if (alpha < c_amin) continue;
           const float Tn = fmaf(-T[k], alpha, T[k]);
@@ -374,7 +380,7 @@ __global__ void __launch_bounds__(128) blend_feat_bwd_kernel(const uint2* __rest
             const float e1 = fmaf(a.y, y[k], e1x);
             const float e2 = fmaf(a.z, y[k], b.x);
             const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
-            if (done[k] || l2a < c_l2min) continue;
+            if (done[k] || !(l2a >= c_l2min)) continue;
             const float alpha = fminf(c_amax, ex2_approx(l2a));
             if (alpha < c_amin) continue;
             const float Tn = fmaf(-T[k], alpha, T[k]);
@@ -509,7 +515,7 @@ __global__ void __launch_bounds__(256 / PX) blend_bwd_kernel(const uint2* __rest
           const float e1 = fmaf(a.y, y[k], e1x);
           const float e2 = fmaf(a.z, y[k], b.x);
           const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
-          if ((lo_pos + j < mine[k]) && !(l2a < cp.log2_alpha_min)) {
+          if ((lo_pos + j < mine[k]) && l2a >= cp.log2_alpha_min) {
             araw[k] = ex2_approx(l2a); alpha[k] = fminf(cp.alpha_max, araw[k]); act[k] = !(alpha[k] < cp.alpha_min);
           }
           some = some || act[k];
@@ -674,7 +680,7 @@ __device__ __forceinline__ void bwd2_emit_global(Bwd2Shared<HBUF, GRED>& sm, con
 // AUX = true: upstream gradients of the auxiliary channels as well (either pointer may be NULL): dL/ddepth enters as a
 // fourth colour channel (g.c_k -> g.c_k + gD z_k, one more sum Sz = sum wgt gD -> gz[id] = dL/dz_k), dL/dopacity
 // (O = 1 - T_final) only shifts the start of the colour-behind recurrence: s_last = T_final (g.bg - gO).
-template <int HBUF, int MINB, bool AUX, bool GRED>
+template <int HBUF, int MINB, bool AUX, bool GRED, bool DEF>
 __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
                                                          const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
                                                          const float* __restrict__ dL_dimage, const float* __restrict__ final_T,
@@ -717,9 +723,9 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
   if (lane == 0) atomicMax(&sm.max_contrib, lane_max);
   __syncthreads();
   const int total = sm.max_contrib;
-  // thresholds pinned in registers (otherwise each use re-reads the constant bank: an issue slot per use in this loop)
-  float c_l2min = cp.log2_alpha_min, c_amax = cp.alpha_max, c_amin = cp.alpha_min;
-  asm volatile("" : "+f"(c_l2min), "+f"(c_amax), "+f"(c_amin));
+  // DEF: the thresholds of [23] as immediates (cp.default_thresholds; see common.cuh)
+  const float c_l2min = DEF ? FDGS_DEF_L2MIN : cp.log2_alpha_min, c_amax = DEF ? FDGS_DEF_ALPHA_MAX : cp.alpha_max;
+  const float c_amin = DEF ? FDGS_DEF_ALPHA_MIN : cp.alpha_min;
   for (int hi = total; hi > 0; hi -= BATCH) {           // batch covers list positions [lo_pos, hi)
     const int lo_pos = max(0, hi - BATCH), m = hi - lo_pos;
     __syncthreads();                                    // previous batch fully flushed
@@ -759,7 +765,7 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
           const float e1 = fmaf(a.y, y[k], e1x);
           const float e2 = fmaf(a.z, y[k], b.x);
           const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
-          if ((lo_pos + j < mine[k]) && !(l2a < c_l2min)) {
+          if ((lo_pos + j < mine[k]) && l2a >= c_l2min) {
             araw[k] = ex2_approx(l2a);
             const float al = fminf(c_amax, araw[k]);
             alpha[k] = al < c_amin ? 0.f : al;
@@ -817,22 +823,29 @@ static int blend_px() {
   return px;
 }
 
+// FDGS_BLEND_NO_DEF: A/B runs of the generic instantiations at the default thresholds.
+static bool no_def() { static const bool v = getenv("FDGS_BLEND_NO_DEF") != nullptr; return v; }
+
 void launch_blend_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
                       unsigned int* n_contrib, float* depth_map, cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
   if (depth_map) {
-    blend_fwd_kernel<2, false, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr, depth_map);
+    blend_fwd_kernel<2, false, true, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr, depth_map);
     ++g_launches;
     return;
   }
-#define FDGS_FWD(PXV) blend_fwd_kernel<PXV, false, false><<<tiles, 256 / PXV, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr, nullptr)
-  switch (blend_px()) { case 1: FDGS_FWD(1); break; case 4: FDGS_FWD(4); break; default: FDGS_FWD(2); }
+#define FDGS_FWD(PXV, DEFV) blend_fwd_kernel<PXV, false, false, DEFV><<<tiles, 256 / PXV, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr, nullptr)
+  switch (blend_px()) {
+    case 1: FDGS_FWD(1, false); break;
+    case 4: FDGS_FWD(4, false); break;
+    default: if (cp.default_thresholds && !no_def()) FDGS_FWD(2, true); else FDGS_FWD(2, false);
+  }
 #undef FDGS_FWD
   ++g_launches;
 }
 
 void launch_blend_stats(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, unsigned long long* stats, cudaStream_t st) {
-  blend_fwd_kernel<1, true, false><<<vp.tiles_x * vp.tiles_y, 256, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, nullptr, nullptr, nullptr, stats, nullptr);
+  blend_fwd_kernel<1, true, false, false><<<vp.tiles_x * vp.tiles_y, 256, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, nullptr, nullptr, nullptr, stats, nullptr);
   ++g_launches;
 }
 
@@ -841,7 +854,7 @@ void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, con
                       cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
   if (dL_ddepth || dL_dopacity) {
-    blend_bwd2_kernel<8, 6, true, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9,
+    blend_bwd2_kernel<8, 6, true, true, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9,
                                                          dL_ddepth, dL_dopacity, ws.gz);
     ++g_launches;
     return;
@@ -854,8 +867,10 @@ void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, con
     default:
       if (direct) FDGS_BWD(2);
       else if (getenv("FDGS_BWD2_SHARED_ACC"))    // A/B runs: per-splat sums combined across the warps in shared memory first
-        blend_bwd2_kernel<8, 6, false, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9, nullptr, nullptr, nullptr);
-      else blend_bwd2_kernel<8, 7, false, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9, nullptr, nullptr, nullptr);
+        blend_bwd2_kernel<8, 6, false, false, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9, nullptr, nullptr, nullptr);
+      else if (cp.default_thresholds && !no_def())
+        blend_bwd2_kernel<8, 7, false, true, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9, nullptr, nullptr, nullptr);
+      else blend_bwd2_kernel<8, 7, false, true, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9, nullptr, nullptr, nullptr);
   }
 #undef FDGS_BWD
   ++g_launches;

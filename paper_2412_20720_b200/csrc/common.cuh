@@ -36,7 +36,17 @@ struct ViewParams {   // by-value kernel parameter
 struct CfgParams {
   float marginal_min, alpha_min, alpha_max, transmittance_min, dilation, cutoff_sigma, znear, guard;
   float log2_alpha_min;   // log2(alpha_min) (-inf if alpha_min == 0)
+  int default_thresholds; // 1: alpha_min, alpha_max, transmittance_min are the values of [23] (S8) — the blend
+                          // kernels then run an instantiation with the four thresholds as immediates
 };
+
+// Thresholds of [23] ("adopted the settings of [23]"; S8).  A kernel argument used in the
+// blend loops costs a constant-bank load per use on sm_100a (LDCU / LDC in SASS: ptxas does not keep it in a register),
+// so the hot kernels have an instantiation with these as immediates.
+#define FDGS_DEF_ALPHA_MIN (1.0f / 255.0f)
+#define FDGS_DEF_ALPHA_MAX 0.99f
+#define FDGS_DEF_T_MIN 1e-4f
+#define FDGS_DEF_L2MIN (-0x1.ffa3ap+2f)   // log2f(1/255) * (1 + 1e-6) - 1e-6 in fp32 (= -7.994362)
 
 // Device-side header at the start of the workspace (zeroed by fdgs_preprocess).
 struct WsHeader {
