@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __rest
 // SAME expression for alpha, so every skip / termination decision is bit-identical to the colour pass — compositing CH
 // per-splat feature values per pass instead of (r, g, b): alpha is evaluated once for CH channels.  feat[N,C] is gathered
 // by id into shared memory next to the splat records; channels c0 .. c0+CH-1 (zero beyond C); no background.
-template <int CH>
+template <int CH, bool DEF>
 __global__ void __launch_bounds__(128, CH == 32 ? 4 : (CH == 4 ? 9 : 1)) blend_feat_fwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
                                                              const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
                                                              const float* __restrict__ feat, const int C, const int c0,
@@ -199,8 +199,8 @@ __global__ void __launch_bounds__(128, CH == 32 ? 4 : (CH == 4 ? 9 : 1)) blend_f
   const uint2 range = ranges[tile];
   const int n = (int)(range.y - range.x);
   const bool vec = (C & 3) == 0 && (c0 & 3) == 0 && c0 + CH <= C;       // 128-bit gathers when the row slice is aligned
-  float c_l2min = cp.log2_alpha_min, c_amax = cp.alpha_max, c_amin = cp.alpha_min, c_tmin = cp.transmittance_min;
-  asm volatile("" : "+f"(c_l2min), "+f"(c_amax), "+f"(c_amin), "+f"(c_tmin));
+  const float c_l2min = DEF ? FDGS_DEF_L2MIN : cp.log2_alpha_min, c_amax = DEF ? FDGS_DEF_ALPHA_MAX : cp.alpha_max;
+  const float c_amin = DEF ? FDGS_DEF_ALPHA_MIN : cp.alpha_min, c_tmin = DEF ? FDGS_DEF_T_MIN : cp.transmittance_min;
   for (int base = 0; base < n; base += BATCH) {
     if (__syncthreads_and(done[0] && done[1])) break;
     const int m = min(BATCH, n - base);
@@ -284,6 +284,7 @@ __global__ void __launch_bounds__(128, CH == 32 ? 4 : (CH == 4 ? 9 : 1)) blend_f
 // a warp parks the weights of its 64 pixels for 8 hit splats in shared memory, then turns round with LANE = CHANNEL:
 // lane c sums w[hit][pixel] * g[pixel][c] over the strip for the 8 hits (1 conflict-free LDS of g and 2 broadcast LDS.128
 // of w per 8 FFMA) and adds the result to grad_feat with one coalesced 128-byte reduction per hit.  32 channels per pass.
+template <bool DEF>
 __global__ void __launch_bounds__(128) blend_feat_bwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
                                                              const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
                                                              const float* __restrict__ dL_dout, const int C, const int c0,
@@ -320,8 +321,8 @@ __global__ void __launch_bounds__(128) blend_feat_bwd_kernel(const uint2* __rest
   }
   const uint2 range = ranges[tile];
   const int n = (int)(range.y - range.x);
-  float c_l2min = cp.log2_alpha_min, c_amax = cp.alpha_max, c_amin = cp.alpha_min, c_tmin = cp.transmittance_min;
-  asm volatile("" : "+f"(c_l2min), "+f"(c_amax), "+f"(c_amin), "+f"(c_tmin));
+  const float c_l2min = DEF ? FDGS_DEF_L2MIN : cp.log2_alpha_min, c_amax = DEF ? FDGS_DEF_ALPHA_MAX : cp.alpha_max;
+  const float c_amin = DEF ? FDGS_DEF_ALPHA_MIN : cp.alpha_min, c_tmin = DEF ? FDGS_DEF_T_MIN : cp.transmittance_min;
   int nbuf = 0;
   float* wl = reinterpret_cast<float*>(sm.w[warp]);         // [64][HB] floats
   auto flush = [&](const int count) {
@@ -605,6 +606,35 @@ __device__ __forceinline__ void bwd2_flush(Bwd2Shared<HBUF, GRED>& sm, const int
     const float4 c = sm.s2[j];
     const float ux = c.y - (sx0 + 0.5f) - (float)(q & 7), vy = c.z - (sy0 + 0.5f);
     const float4* row = sm.hit[warp][h];
+    if constexpr (LPH == 4) {
+      // The lane's pixels sit at fixed offsets from its first one — column 4 (i & 1), row (i >> 1), + 4 rows in sub-patch
+      // 1 — so the five moment sums about the splat centre (ux, vy) follow from a handful of offset-weighted sums of
+      // dpow (small integer weights, most of them 0) instead of 19 operations per pixel pair:
+      //   sum dpow (ux - a)^m (vy - b)^n = binomial expansion in the raw sums below.
+      float M0 = 0.f, T4 = 0.f, Z = 0.f, Z4 = 0.f, W1 = 0.f, W2 = 0.f, V = 0.f, X1 = 0.f;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int p = 4 * i + q;
+        const float4 d = row[p];               // dpow0, wgt0, dpow1, wgt1
+        const float4 g0 = sm.pg[warp][p][0], g1 = sm.pg[warp][p][1];
+        const float t = d.x + d.z, b0 = (float)(i >> 1);
+        M0 += t; Z += d.z;
+        if (i >> 1) { W1 = fmaf(b0, t, W1); W2 = fmaf(b0 * b0, t, W2); V = fmaf(b0, d.z, V); }
+        if (i & 1) { T4 += t; Z4 += d.z; if (i >> 1) X1 = fmaf(b0, t, X1); }
+        S[5] = fmaf(d.y, g0.x, S[5]); S[6] = fmaf(d.y, g0.y, S[6]); S[7] = fmaf(d.y, g0.z, S[7]);
+        S[5] = fmaf(d.w, g0.w, S[5]); S[6] = fmaf(d.w, g1.x, S[6]); S[7] = fmaf(d.w, g1.y, S[7]);
+        if (AUX) { S[9] = fmaf(d.y, g1.z, S[9]); S[9] = fmaf(d.w, g1.w, S[9]); }
+      }
+      const float Mx = 4.f * T4, Mxx = 16.f * T4;                       // sum a t, sum a^2 t            (a = 0 or 4)
+      const float My = fmaf(4.f, Z, W1);                                // sum (b0 t + 4 dpow1)
+      const float Myy = fmaf(16.f, Z, fmaf(8.f, V, W2));                // sum (b0^2 t + (8 b0 + 16) dpow1)
+      const float Mxy = 4.f * fmaf(4.f, Z4, X1);                        // sum a (b0 t + 4 dpow1)
+      S[0] = fmaf(ux, M0, -Mx); S[1] = fmaf(vy, M0, -My);
+      S[2] = fmaf(ux, fmaf(ux, M0, -2.f * Mx), Mxx);
+      S[3] = fmaf(ux, fmaf(vy, M0, -My), fmaf(-vy, Mx, Mxy));
+      S[4] = fmaf(vy, fmaf(vy, M0, -2.f * My), Myy);
+      S[8] = M0;
+    } else
 #pragma unroll
     for (int i = 0; i < 32 / LPH; ++i) {     // pixel slot p = LPH i + q: column (p % 8), row (p / 8) of both sub-patches
       const int p = LPH * i + q;
@@ -815,6 +845,9 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
   }
 }
 
+// FDGS_BLEND_NO_DEF: A/B runs of the generic instantiations at the default thresholds.
+static bool no_def() { static const bool v = getenv("FDGS_BLEND_NO_DEF") != nullptr; return v; }
+
 // Pixels per lane of the two blend kernels.  2 is the measured optimum on cfg3; FDGS_BLEND_PX
 // overrides it for experiments (1, 2 or 4).
 static int blend_px() {
@@ -823,14 +856,12 @@ static int blend_px() {
   return px;
 }
 
-// FDGS_BLEND_NO_DEF: A/B runs of the generic instantiations at the default thresholds.
-static bool no_def() { static const bool v = getenv("FDGS_BLEND_NO_DEF") != nullptr; return v; }
-
 void launch_blend_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
                       unsigned int* n_contrib, float* depth_map, cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
   if (depth_map) {
-    blend_fwd_kernel<2, false, true, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr, depth_map);
+    if (cp.default_thresholds && !no_def()) blend_fwd_kernel<2, false, true, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr, depth_map);
+    else blend_fwd_kernel<2, false, true, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr, depth_map);
     ++g_launches;
     return;
   }
@@ -854,8 +885,12 @@ void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, con
                       cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
   if (dL_ddepth || dL_dopacity) {
-    blend_bwd2_kernel<8, 6, true, true, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9,
-                                                         dL_ddepth, dL_dopacity, ws.gz);
+    if (cp.default_thresholds && !no_def())
+      blend_bwd2_kernel<8, 6, true, true, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9,
+                                                                       dL_ddepth, dL_dopacity, ws.gz);
+    else
+      blend_bwd2_kernel<8, 6, true, true, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9,
+                                                                        dL_ddepth, dL_dopacity, ws.gz);
     ++g_launches;
     return;
   }
@@ -880,7 +915,8 @@ void launch_blend_feat_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp
                            float* grad_feat, cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
   for (int c0 = 0; c0 < C; c0 += 32) {
-    blend_feat_bwd_kernel<<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dout, C, c0, grad_feat);
+    if (cp.default_thresholds && !no_def()) blend_feat_bwd_kernel<true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dout, C, c0, grad_feat);
+    else blend_feat_bwd_kernel<false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dout, C, c0, grad_feat);
     ++g_launches;
   }
 }
@@ -890,9 +926,13 @@ void launch_blend_feat_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp
   const int tiles = vp.tiles_x * vp.tiles_y;
   for (int c0 = 0; c0 < C;) {                    // 16 channels per pass, a tail of <= 4 in a 4-channel pass
     static const bool no32 = getenv("FDGS_FEAT_NO32") != nullptr;     // A/B runs: two 16-channel passes instead of one of 32
-    if (C - c0 >= 32 && !no32) { blend_feat_fwd_kernel<32><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, feat, C, c0, out); c0 += 32; }
-    else if (C - c0 > 4) { blend_feat_fwd_kernel<16><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, feat, C, c0, out); c0 += 16; }
-    else { blend_feat_fwd_kernel<4><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, feat, C, c0, out); c0 += 4; }
+    const bool def = cp.default_thresholds && !no_def();
+#define FDGS_FEAT(CHV) do { if (def) blend_feat_fwd_kernel<CHV, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, feat, C, c0, out); \
+                            else blend_feat_fwd_kernel<CHV, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, feat, C, c0, out); c0 += CHV; } while (0)
+    if (C - c0 >= 32 && !no32) FDGS_FEAT(32);
+    else if (C - c0 > 4) FDGS_FEAT(16);
+    else FDGS_FEAT(4);
+#undef FDGS_FEAT
     ++g_launches;
   }
 }
