@@ -133,7 +133,7 @@ __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __rest
           if (alpha < c_amin) continue;
           const float Tn = fmaf(-T[k], alpha, T[k]);
           const bool term = Tn < c_tmin;                       // the terminating splat is not composited
-          lmin[k] = term ? INFINITY : lmin[k];
+          asm("{\n\t.reg .pred p;\n\tsetp.lt.f32 p, %1, %2;\n\t@p mov.b32 %0, 0x7f800000;\n\t}" : "+f"(lmin[k]) : "f"(Tn), "f"(c_tmin));
           if (term) continue;
           const float wgt = alpha * T[k];
           Cr[k] = fmaf(b.z, wgt, Cr[k]); Cg[k] = fmaf(b.w, wgt, Cg[k]); Cb[k] = fmaf(sm.s2[j].x, wgt, Cb[k]);
