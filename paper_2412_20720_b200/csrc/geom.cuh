@@ -61,24 +61,28 @@ __device__ __forceinline__ int geom_forward(const float4 mean, const float4 ls, 
   // an entry of R that is small against its terms would otherwise carry ~1e-7 ABSOLUTE error, and the time
   // row of R is multiplied by a scale s_t that is typically 30x the spatial ones, so Sigma_44 and the marginal
   // weight would lose up to two digits for nearly time-orthogonal primitives.
+  // The time row of R (row 3) comes first: it alone gives Sigma_44 and hence the marginal cull, which removes three
+  // primitives out of four at cfg3 before the other twelve entries are formed.  One fp64 rsqrt: the product of the
+  // two normalisations scales the right factor.
+  double qld[4], qrd[4];
   {
-    double dl2 = 0.0, dr2 = 0.0, qld[4], qrd[4];
+    double dl2 = 0.0, dr2 = 0.0;
 #pragma unroll
     for (int k = 0; k < 4; ++k) { dl2 = fma((double)qlr[k], (double)qlr[k], dl2); dr2 = fma((double)qrr[k], (double)qrr[k], dr2); }
-    const double il = rsqrt(dl2), ir = rsqrt(dr2);
+    const double nrm = rsqrt(dl2 * dr2);
 #pragma unroll
-    for (int k = 0; k < 4; ++k) { qld[k] = qlr[k] * il; qrd[k] = qrr[k] * ir; }
-    const double a = qld[0], b = qld[1], c = qld[2], d = qld[3], p = qrd[0], q = qrd[1], r = qrd[2], t = qrd[3];
-    const double Ld[4][4] = {{a, -b, -c, -d}, {b, a, -d, c}, {c, d, a, -b}, {d, -c, b, a}};
-    const double Rd[4][4] = {{p, -q, -r, -t}, {q, p, t, -r}, {r, -t, p, q}, {t, r, -q, p}};
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        const double acc = fma(Ld[i][0], Rd[0][k], fma(Ld[i][1], Rd[1][k], fma(Ld[i][2], Rd[2][k], Ld[i][3] * Rd[3][k])));
-        g.R4[i][k] = (float)acc; g.M[i][k] = (float)acc * g.s[k];
-      }
+    for (int k = 0; k < 4; ++k) { qld[k] = qlr[k]; qrd[k] = qrr[k] * nrm; }
   }
+  const double Ld[4][4] = {{qld[0], -qld[1], -qld[2], -qld[3]}, {qld[1], qld[0], -qld[3], qld[2]},
+                           {qld[2], qld[3], qld[0], -qld[1]}, {qld[3], -qld[2], qld[1], qld[0]}};
+  const double Rd[4][4] = {{qrd[0], -qrd[1], -qrd[2], -qrd[3]}, {qrd[1], qrd[0], qrd[3], -qrd[2]},
+                           {qrd[2], -qrd[3], qrd[0], qrd[1]}, {qrd[3], qrd[2], -qrd[1], qrd[0]}};
+#define FDGS_R_ROW(i)                                                                                                         \
+  _Pragma("unroll") for (int k = 0; k < 4; ++k) {                                                                             \
+    const double acc = fma(Ld[i][0], Rd[0][k], fma(Ld[i][1], Rd[1][k], fma(Ld[i][2], Rd[2][k], Ld[i][3] * Rd[3][k])));      \
+    g.R4[i][k] = (float)acc; g.M[i][k] = (float)acc * g.s[k];                                                                 \
+  }
+  FDGS_R_ROW(3)
   // eq. 10: marginal weight, and the p(t) < marginal_min filter (L324)
   g.b = g.M[3][0] * g.M[3][0] + g.M[3][1] * g.M[3][1] + g.M[3][2] * g.M[3][2] + g.M[3][3] * g.M[3][3];
   g.dt = vp.t - mean.w;
@@ -87,6 +91,8 @@ __device__ __forceinline__ int geom_forward(const float4 mean, const float4 ls, 
   if (g.w < cp.marginal_min) return G_CULL_TIME;
   // the primitive is alive at t: start fetching what only survivors read (its colour block) under the arithmetic below
   if (prefetch) prefetch_l2(prefetch, prefetch_bytes);
+  FDGS_R_ROW(0) FDGS_R_ROW(1) FDGS_R_ROW(2)
+#undef FDGS_R_ROW
   // eq. 9 in factor form
   const float inv_b = 1.0f / g.b;
   const float mu3[3] = {mean.x, mean.y, mean.z};
