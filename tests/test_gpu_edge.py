@@ -298,3 +298,28 @@ def test_marginal_filter_off_with_underflowing_weight_gives_finite_zero_gradient
     assert np.abs(out["grads"]["mean"][1]).max() == 0 and np.abs(out["grads"]["sh"][1]).max() == 0
     assert np.abs(out["grads"]["mean"][0]).max() > 0
     assert np.isfinite(out["g9"]).all()
+
+
+def test_default_threshold_instantiations_agree_with_the_generic_kernels():
+    """The blend kernels run an instantiation with the thresholds of [23] as immediates when the configuration holds exactly
+    those values.  Moving alpha_max by one ulp selects the generic kernels (thresholds read from the
+    kernel arguments): image, transmittance, contributor counts and gradients must agree up to the effect of that ulp."""
+    import gpu_helpers as gh
+    sc = _f32(scenes.tiny(seed=7, N=2000))
+    v = sc.views[0]
+    rng = np.random.default_rng(11)
+    dL = rng.standard_normal((3, v.height, v.width))
+    a = gh.gpu_run(sc, v, dL=dL)
+    amax = float(np.nextafter(np.float32(0.99), np.float32(0.0)))
+    b = gh.gpu_run(sc, v, cfg_overrides=dict(alpha_max=amax), dL=dL)
+    assert a["num_pairs"] == b["num_pairs"] and a["num_pairs"] > 0
+    assert np.abs(a["image"] - b["image"]).max() <= 1e-6
+    assert np.abs(a["final_T"] - b["final_T"]).max() <= 1e-6
+    assert (a["n_contrib"] != b["n_contrib"]).mean() <= 1e-3
+    for k, g in a["grads"].items():
+        if g is None:
+            continue
+        den = np.linalg.norm(g)
+        assert den > 0 or np.linalg.norm(b["grads"][k]) == 0, k
+        if den > 0:
+            assert np.linalg.norm(g - b["grads"][k]) / den <= 1e-4, k
