@@ -61,12 +61,14 @@ struct Strip {
 // (rendered depth, eq. 29) into depth_map[H,W].
 // DEF = true: the thresholds of [23] as immediates (cp.default_thresholds; see common.cuh).
 template <int PX, bool STATS, bool AUX, bool DEF>
-__global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
+__global__ void __launch_bounds__(256 / PX, PX == 2 && !STATS ? 9 : 1) blend_fwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
                                                              const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
                                                              float* __restrict__ image, float* __restrict__ final_T,
                                                              unsigned int* __restrict__ n_contrib, unsigned long long* stats,
                                                              float* __restrict__ depth_map) {
-  constexpr int BATCH = 256 / PX;
+  // splats staged per batch: two per thread at PX = 2 — half the barriers (12 % of the warp samples sat at the loop-top
+  // barrier with 128) and twice the gathers in flight per thread
+  constexpr int NT = 256 / PX, BATCH = PX == 2 ? 2 * NT : NT;
   __shared__ struct { float4 s0[BATCH], s1[BATCH], s2[BATCH]; } sm;
   const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -97,7 +99,9 @@ __global__ void __launch_bounds__(256 / PX) blend_fwd_kernel(const uint2* __rest
     if (__syncthreads_and(all_done)) break;
     const int m = min(BATCH, n - base);
     if (STATS && threadIdx.x == 0) st_stage += m;
-    if ((int)threadIdx.x < m) stage_splat(rec, vals[range.x + base + threadIdx.x], ox, oy, &sm.s0[threadIdx.x], &sm.s1[threadIdx.x], &sm.s2[threadIdx.x]);
+#pragma unroll
+    for (int i = threadIdx.x; i < BATCH; i += NT)
+      if (i < m) stage_splat(rec, vals[range.x + base + i], ox, oy, &sm.s0[i], &sm.s1[i], &sm.s2[i]);
     __syncthreads();
     unsigned int alive = 0;                           // sub-patches with an unsaturated pixel (warp-uniform)
 #pragma unroll
