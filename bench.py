@@ -27,8 +27,8 @@ PAIR_CAPACITY = 16 * 1024 * 1024
 SM_COUNT, LANES_PER_SM, SM_MAX_HZ = 148, 128, 1.965e9
 ALU_PEAK_TLANE = SM_COUNT * LANES_PER_SM * SM_MAX_HZ / 1e12      # 37.2 T lane-instructions/s
 # DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
-# (profiles/r1_all_kernels_ncu_full_final.md: 88.5 MB read + 5.7 MB written)
-BLEND_BWD_NCU_TRAFFIC_BYTES = 94.2e6
+# (profiles/r1_all_kernels_ncu_full_final.md: 88.5 MB read + 6.1 MB written)
+BLEND_BWD_NCU_TRAFFIC_BYTES = 94.6e6
 
 
 def hbm_peak():
