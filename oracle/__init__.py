@@ -33,11 +33,19 @@ PURE_CFG = dict(marginal_min=0.0, alpha_min=0.0, alpha_max=1.0, transmittance_mi
 
 
 def build(force: bool = False) -> str:
-    """Compile the oracle with g++ (-O2 -fopenmp).  Returns the path of the shared library."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["g++", "-O2", "-fopenmp", "-shared", "-fPIC", "-std=c++17", "-ffp-contract=off", _SRC, "-o", _LIB]
+    """Compile the oracle with g++ (-O2 -fopenmp).  Returns the path of the shared library.
+    FDGS_ORACLE_SANITIZE=1 builds and loads an -fsanitize=address,undefined variant instead; run the
+    CPU suite under it with
+        FDGS_ORACLE_SANITIZE=1 LD_PRELOAD=$(g++ -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 \
+            python -m pytest tests -m "not gpu" -q"""
+    lib, extra = _LIB, []
+    if os.environ.get("FDGS_ORACLE_SANITIZE"):
+        lib = os.path.join(_HERE, "libfdgs_oracle_san.so")
+        extra = ["-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
+    if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(_SRC):
+        cmd = ["g++", "-O2", "-fopenmp", "-shared", "-fPIC", "-std=c++17", "-ffp-contract=off", *extra, _SRC, "-o", lib]
         subprocess.run(cmd, check=True)
-    return _LIB
+    return lib
 
 
 def _load():
@@ -59,6 +67,7 @@ def _load():
     lib.fdgs_oracle_get_prims.argtypes = [C.c_void_p, dp]
     lib.fdgs_oracle_get_rot_cov.argtypes = [C.c_void_p, C.c_int, dp, dp]
     lib.fdgs_oracle_sh_basis.argtypes = [C.c_int, dp, dp]
+    lib.fdgs_oracle_sh_basis_grad.argtypes = [C.c_int, dp, dp, dp]
     lib.fdgs_oracle_forward.argtypes = [C.c_void_p, dp, dp, ip, dp]
     lib.fdgs_oracle_backward.argtypes = [C.c_void_p, dp] + [dp] * 8
     lib.fdgs_oracle_get_depth_map.argtypes = [C.c_void_p, dp]
@@ -82,6 +91,15 @@ def sh_basis(sh_degree: int, direction) -> np.ndarray:
     Y = np.zeros((sh_degree + 1) ** 2, dtype=np.float64)
     _load().fdgs_oracle_sh_basis(int(sh_degree), _d(d), _d(Y))
     return Y
+
+
+def sh_basis_grad(sh_degree: int, direction):
+    """(Y[(L+1)^2], dY/d(x,y,z)[(L+1)^2,3]) of the polynomial extension, as the oracle's backward uses them."""
+    d = np.ascontiguousarray(direction, dtype=np.float64)
+    K = (sh_degree + 1) ** 2
+    Y, G = np.zeros(K, dtype=np.float64), np.zeros((K, 3), dtype=np.float64)
+    _load().fdgs_oracle_sh_basis_grad(int(sh_degree), _d(d), _d(Y), _d(G))
+    return Y, G
 
 
 @dataclass

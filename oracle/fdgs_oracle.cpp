@@ -652,6 +652,11 @@ void fdgs_oracle_get_rot_cov(void* h, int i, double* R16, double* Sigma16) {
 
 // real SH basis values Y[(L+1)^2] at unit direction dir3 — for the quadrature / library pins
 void fdgs_oracle_sh_basis(int sh_degree, const double* dir3, double* Y) { sh_basis(sh_degree, dir3, Y, nullptr); }
+// the same with the hand-written gradient rows grad[(L+1)^2][3] of the polynomial extension — exported so that a
+// `-m "not gpu"` test can pin them against central differences of the values (tests/test_oracle_pins.py)
+void fdgs_oracle_sh_basis_grad(int sh_degree, const double* dir3, double* Y, double* grad) {
+  sh_basis(sh_degree, dir3, Y, reinterpret_cast<double (*)[3]>(grad));
+}
 
 // image[3,H,W], final_T[H,W], n_contrib[H,W] int32 (1 + list position of the last contributor),
 // margin[H,W] (min relative margin of any alpha / transmittance test at that pixel)

@@ -252,8 +252,10 @@ def target_image(seed: int, view_index: int, width: int, height: int) -> np.ndar
     return _f32(uniform(seed, 300 + view_index, 3 * width * height).reshape(3, height, width))
 
 
-def fd_scene(seed: int, N: int = 8) -> Scene:
-    """Finite-difference scenes: <=8 large, translucent splats far from every threshold."""
+def fd_scene(seed: int, N: int = 8, sh_degree: int = 1, n_time: int = 2) -> Scene:
+    """Finite-difference scenes: <=8 large, translucent splats far from every threshold; K = n_time (L+1)^2
+    colour coefficients per channel (the defaults give the K = 8 scenes of round 1 unchanged)."""
+    K = n_time * (sh_degree + 1) ** 2
     mean = np.stack([uniform(seed, 1, N) - 0.5, uniform(seed, 2, N) - 0.5, uniform(seed, 3, N) - 0.5,
                      0.5 + 0.3 * (uniform(seed, 4, N) - 0.5)], axis=1)
     ls = np.stack([-1.5 + 0.2 * normal(seed, 10 + k, N) for k in range(3)] + [-0.5 + 0.2 * normal(seed, 13, N)], axis=1)
@@ -261,14 +263,14 @@ def fd_scene(seed: int, N: int = 8) -> Scene:
     ql = ql * (0.5 + uniform(seed, 28, N))[:, None]     # non-unit on purpose: normalisation is inside
     qr = qr * (0.5 + uniform(seed, 29, N))[:, None]
     logit = 0.5 * normal(seed, 30, N)
-    sh = 0.05 * normal(seed, 40, N * 8 * 3).reshape(N, 8, 3)
+    sh = 0.05 * normal(seed, 40, N * K * 3).reshape(N, K, 3)
     sh[:, 0, :] = 1.0 + 0.1 * normal(seed, 41, N * 3).reshape(N, 3)
     fx, fy, cx, cy = _pinhole(64, 64, 50.0)
     V = np.eye(4)
     V[:3, :3] = _axis_angle(np.array([0.3, 1.0, 0.2]), 0.2)
     V[:3, 3] = np.array([0.1, -0.05, 4.0])
     view = View(_f32(V), fx, fy, cx, cy, 64, 64, 0.5, 1.0, (0.1, 0.2, 0.3)).as_fp32()
-    return Scene("fd", 1, 2, _f32(mean), _f32(ls), _f32(ql), _f32(qr), _f32(logit), _f32(sh), [view], seed)
+    return Scene("fd", sh_degree, n_time, _f32(mean), _f32(ls), _f32(ql), _f32(qr), _f32(logit), _f32(sh), [view], seed)
 
 
 def compact_model(seed: int = 6, N: int = 1_000_000, sh_degree: int = 3, n_time: int = 3, rvq=((6, 64), (6, 64), (6, 64), (8, 256))) -> dict:

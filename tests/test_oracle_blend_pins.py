@@ -168,14 +168,16 @@ def _loss_and_state(sc, G, cfg):
     return float((img * G).sum()), o, nc, mg
 
 
-def _fd_check(seed, cfg, tol=1e-5):
-    sc = scenes.fd_scene(seed, 8)
+def _fd_check(seed, cfg, tol=1e-5, N=8, sh_degree=1, n_time=2, scene=None, need_clamp=0):
+    sc = scene if scene is not None else scenes.fd_scene(seed, N, sh_degree, n_time)
     for k in PARAMS:                       # promote to float64 so that +-h is representable
         setattr(sc, k, getattr(sc, k).astype(np.float64))
     G = scenes.upstream_normal(seed, 64, 64).astype(np.float64)
     L0, o0, nc0, mg0 = _loss_and_state(sc, G, cfg)
     p0 = o0.prims()
     assert (p0.status == 0).all()
+    if need_clamp:                         # the guard-band clamped branch of J must be the one differentiated
+        assert all((int(b) & need_clamp) for b in p0.clamp_bits), p0.clamp_bits
     if not cfg.get("full_support"):
         if mg0.min() < 1e-4 or p0.fragility.min() < 1e-4:
             return None                    # too close to a discontinuity: the caller resamples
@@ -205,14 +207,53 @@ def _fd_check(seed, cfg, tol=1e-5):
     return worst
 
 
+# (L, n_time): the round-1 pin (1, 2); degree 2 alone; and the colour order every benchmark configuration runs, degree 3 x
+# 3 Fourier orders (eq. 20, PAPER.md:L187 with Delta per L183) — the hand-derived gradient rows of Y_4..Y_15 and the n >= 2
+# branch of the Delta-derivative are only reached here
 @pytest.mark.parametrize("mode", ["default", "pure"])
-def test_backward_matches_central_differences(mode):
+@pytest.mark.parametrize("L,n_time,N", [(1, 2, 8), (2, 1, 6), (3, 3, 4)])
+def test_backward_matches_central_differences(mode, L, n_time, N):
     cfg = dict(oracle.DEFAULT_CFG) if mode == "default" else dict(oracle.PURE_CFG)
     for seed in range(100, 120):
-        res = _fd_check(seed, cfg)
+        res = _fd_check(seed, cfg, N=N, sh_degree=L, n_time=n_time)
         if res is not None:
+            assert res["sh"] < 1e-5 and res["mean"] < 1e-5
             return
     pytest.fail("no finite-difference scene far from every threshold found")
+
+
+def _clamp_scene(L=1, n_time=2):
+    """Two large splats whose centres project OUTSIDE the guard band (|x/z| resp. |y/z| > 1.3 W / (2 fx) = 0.606 for the
+    64x64, fov 50 camera at distance 4), so that J is evaluated at the clamped ratio
+    while their 3-sigma support still reaches into the image: splat 0 clamps in x (bit 8), splat 1 in y (bit 16)."""
+    K = n_time * (L + 1) ** 2
+    rng = np.random.default_rng(7)
+    sh = 0.05 * rng.standard_normal((2, K, 3))
+    sh[:, 0, :] = 1.0 + 0.1 * rng.standard_normal((2, 3))
+    ql = rng.standard_normal((2, 4)); qr = rng.standard_normal((2, 4))
+    # a mild space-time tilt only: q_r = (a, b, c, -d) + noise keeps the splat near its spatial position at t
+    qr = ql * np.array([1, 1, 1, -1]) + 0.1 * qr
+    return hand_scene([(3.4, 0.2, 0.0, 0.45), (-0.3, -3.3, 0.3, 0.55)], [np.log([0.8, 0.7, 0.75, 0.6]), np.log([0.7, 0.8, 0.75, 0.6])],
+                      quat_l=ql, quat_r=qr, logit=[0.4, -0.2], sh=sh, sh_degree=L, n_time=n_time, bg=(0.1, 0.2, 0.3))
+
+
+@pytest.mark.parametrize("mode", ["default", "pure"])
+def test_backward_with_the_guard_band_clamp_active(mode):
+    """The clamped-J branch of the forward and of backward_one ('x' = lim z => that entry is
+    -fx lim / z') against central differences; _fd_check asserts that the clamp bits are set and identical at +-h."""
+    cfg = dict(oracle.DEFAULT_CFG) if mode == "default" else dict(oracle.PURE_CFG)
+    sc = _clamp_scene()
+    o = oracle_for(sc, cfg=cfg)
+    bits = o.prims().clamp_bits.astype(int)
+    assert bits[0] & 8 and bits[1] & 16, bits
+    img = o.forward()[0]
+    assert img.max() > 0.3 and (np.abs(img - np.array([0.1, 0.2, 0.3])[:, None, None]).max(0) > 1e-3).mean() > 0.2   # the splats are on screen
+    res = _fd_check(0, cfg, scene=sc, need_clamp=24)
+    assert res is not None and max(res.values()) < 1e-5, res
+    # and the clamp matters: the unclamped Jacobian gives a different footprint (guard = 100 disables the clamp)
+    o2 = oracle_for(sc, cfg=dict(cfg, guard=100.0))
+    assert not (o2.prims().clamp_bits.astype(int) & 24).any()
+    assert np.abs(o2.prims().conic - o.prims().conic).max() > 1e-4
 
 
 def test_backward_invariants():

@@ -275,3 +275,30 @@ def test_isotropic_splat_on_axis_closed_form():
     ref = a[None] * col[:, None, None] + (1 - a)[None] * np.array([0.1, 0.2, 0.3])[:, None, None]
     np.testing.assert_allclose(img, ref, atol=1e-14)
     np.testing.assert_allclose(fT, 1 - a, atol=1e-15)
+
+
+def test_sh_gradient_rows_against_central_differences():
+    """The 48 hand-written entries dY_k/d(x,y,z), k < 16, of the polynomial extension (used by the backward of eq. 20 for
+    dL/d dir) against central differences of the VALUES, which are themselves pinned by scipy and quadrature above.
+    The Y_k are polynomials of degree <= 3, so a central difference with step h is exact up to h^2 * (third derivative):
+    1e-5 is a loose bound; a wrong sign, factor or index in any row fails it by O(1).  Points off the unit sphere as well
+    (the extension, not the restriction, is what the chain rule through dir = d / |d| needs)."""
+    rng = np.random.default_rng(3)
+    for trial in range(20):
+        d = rng.standard_normal(3)
+        if trial % 2 == 0:
+            d /= np.linalg.norm(d)
+        for L in (0, 1, 2, 3):
+            Y, G = oracle.sh_basis_grad(L, d)
+            np.testing.assert_allclose(Y, oracle.sh_basis(L, d), rtol=0, atol=0)
+            h = 1e-5
+            for c in range(3):
+                e = np.zeros(3); e[c] = h
+                fd = (oracle.sh_basis(L, d + e) - oracle.sh_basis(L, d - e)) / (2 * h)
+                np.testing.assert_allclose(G[:, c], fd, rtol=1e-7, atol=1e-7)
+    # Euler's theorem for homogeneous polynomials pins the rows a second, independent way: d . grad Y_k = l Y_k
+    d = rng.standard_normal(3)
+    Y, G = oracle.sh_basis_grad(3, d)
+    deg = np.array([l for l in range(4) for _ in range(2 * l + 1)], dtype=np.float64)
+    # Y_6 and the degree-3 rows are written with z^2-x^2-y^2 style terms: all homogeneous of degree l
+    np.testing.assert_allclose(G @ d, deg * Y, rtol=1e-12, atol=1e-12)
