@@ -6,8 +6,9 @@ time-sliced tile rasterizer at 1M 4D Gaussians, 1352x1014, batch of 4 views (cfg
 
 One JSON line on stdout (rank 0).  `value` = steps/s with everything resident in HBM; `e2e` = the same through
 fdgs_step_batch with pinned HOST target images copied in and the per-view losses read back every step; `roofline` = the dominant kernel
-against the ALU issue roof derived in DESIGN.md; `cpu_baseline` = the float64 oracle on this box's host cores on a
-bounded sample (one of the four views).  --impl reference times that oracle as the reference arm.
+against the ALU issue roof derived in DESIGN.md (both per-unit instruction models printed); `cpu_baseline` = the float64
+oracle on this box's host cores: one full step on all cores plus one view single-threaded, per stage.  --impl reference
+times that oracle as the reference arm, one full step (all four views) per timed step.
 Multi-GPU: the path does not shard: N ranks render N independent replicas.
 """
 import argparse
@@ -26,9 +27,19 @@ WORKLOAD = "cfg3_video: N=1M, K=48 (L=3 x n_time=3), 1352x1014, fov 60, 4 jitter
 PAIR_CAPACITY = 16 * 1024 * 1024
 SM_COUNT, LANES_PER_SM, SM_MAX_HZ = 148, 128, 1.965e9
 ALU_PEAK_TLANE = SM_COUNT * LANES_PER_SM * SM_MAX_HZ / 1e12      # 37.2 T lane-instructions/s
-# DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
-# (profiles/r1_all_kernels_ncu_full_final.md: 88.5 MB read + 6.1 MB written)
-BLEND_BWD_NCU_TRAFFIC_BYTES = 94.6e6
+# DRAM bytes per launch of the dominant kernel: NOT measured by this run (ncu counters cannot be read from inside it).
+# The value is read from the committed ncu --set full summary named here and is labelled as such in the JSON line.
+TRAFFIC_SOURCE = os.path.join(ROOT, "profiles", "r2_blend_traffic.json")
+
+
+def ncu_traffic(kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed capture, with its provenance."""
+    try:
+        with open(TRAFFIC_SOURCE) as f:
+            d = json.load(f)
+        return float(d["kernels"][kernel]["dram_bytes_per_launch"]), "ncu --set full capture, " + d["source"]
+    except Exception:
+        return None, "no committed ncu capture for this kernel"
 
 
 def hbm_peak():
@@ -48,8 +59,8 @@ def stage_rooflines(stage, work, N, K, n_views):
     byts = {"preprocess": n_views * 72 * N + nv * (12 * K + 76),
             "compact+tile_grid": n_views * 4 * N + 16 * nv,
             "sort_depth": 4 * 16 * nv,
-            "offsets+duplicate": 16 * nv + 8 * D,
-            "sort_tile": 2 * 16 * D,
+            "offsets": 12 * nv,                               # ids + tiles touched read, offsets written
+            "pair_scatter": 2 * 16 * nv + 4 * D,              # ids, offsets, rectangles read twice; 4 B written per pair
             "preprocess_bwd": nv * (36 + 68 + 12 * K + 2 * (12 * K + 68) + 64)}
     out = {}
     for k, b in byts.items():
@@ -110,40 +121,56 @@ def whole_job_value(world: int, ms_per_step: float) -> float:
     return world * 1e3 / ms_per_step
 
 
-def oracle_view_seconds(scene, view_index=0, repeats=1):
-    """The oracle as it stands: preprocess + forward + L1 gradient + backward of ONE view on the host cores."""
+ORACLE_STAGES = ("preprocess+lists", "blend_fwd", "loss+backward")
+
+
+def oracle_step_seconds(scene, view_indices, threads=None):
+    """The oracle as it stands: preprocess (A1-A8) + forward blend + L1 gradient + backward of the given views on the host
+    cores.  Returns (seconds per stage summed over the views, threads used)."""
     import numpy as np
     import oracle
     from paper_2412_20720_b200 import scenes
+    if threads:
+        oracle.set_num_threads(threads)
     o = oracle.Oracle(**scene.arrays(), sh_degree=scene.sh_degree, n_time=scene.n_time)
-    v = scene.views[view_index]
-    tgt = scenes.target_image(scene.seed, view_index, v.width, v.height).astype(np.float64)
-    times = []
-    for _ in range(repeats):
+    per = dict.fromkeys(ORACLE_STAGES, 0.0)
+    for vi in view_indices:
+        v = scene.views[vi]
+        tgt = scenes.target_image(scene.seed, vi, v.width, v.height).astype(np.float64)
         t0 = time.perf_counter()
         o.preprocess(v.view, (v.fx, v.fy, v.cx, v.cy), v.width, v.height, v.t, v.period_T, v.bg)
+        t1 = time.perf_counter()
         img = o.forward()[0]
+        t2 = time.perf_counter()
         o.backward(np.sign(img - tgt) / img.size)
-        times.append(time.perf_counter() - t0)
-    return times, oracle.num_threads()
+        t3 = time.perf_counter()
+        per["preprocess+lists"] += t1 - t0; per["blend_fwd"] += t2 - t1; per["loss+backward"] += t3 - t2
+    return per, oracle.num_threads()
 
 
 def run_reference(args):
-    """Reference arm = the float64 oracle (there is no upstream code).  Rank 0 only."""
+    """Reference arm = the float64 oracle (there is no upstream code).  Rank 0 only.  Every warm-up and timed step is one
+    REAL step: all views of the batch, nothing extrapolated (about 10 s per step on 16 cores)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
     from paper_2412_20720_b200 import scenes
     scene = scenes.multiview_video()
     n_views = len(scene.views)
-    times, cores = oracle_view_seconds(scene, 0, repeats=args.warmup + args.steps)
-    timed = times[args.warmup:]
-    ms_step = 1e3 * n_views * sum(timed) / len(timed)          # a step = 4 views; each timed step samples one view
+    secs, cores, stages = [], 0, dict.fromkeys(ORACLE_STAGES, 0.0)
+    for it in range(args.warmup + args.steps):
+        per, cores = oracle_step_seconds(scene, range(n_views))
+        if it >= args.warmup:
+            secs.append(sum(per.values()))
+            for k in stages:
+                stages[k] += per[k] / args.steps
+    ms_step = 1e3 * sum(secs) / len(secs)
     val = 1e3 / ms_step
-    sample = f"each step = view 0 of the {n_views} views (preprocess+forward+L1+backward), time scaled x{n_views}"
+    sample = f"every step = all {n_views} views of cfg3 (preprocess+forward+L1+backward at N=1M, 1352x1014), no extrapolation"
     print(json.dumps({"impl": "reference", "metric": METRIC, "value": val, "unit": "steps/s", "n_gpus": args.gpus, "steps": args.steps,
                       "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                       "dtype": "f64", "data": "synthetic", "config": {"workload": WORKLOAD},
-                      "cpu_baseline": {"value": val, "unit": "steps/s", "cores": cores, "kind": "oracle", "sample": sample},
+                      "cpu_baseline": {"value": val, "unit": "steps/s", "cores": cores, "kind": "oracle", "sample": sample,
+                                       "stage_seconds_per_step": stages},
                       "e2e": {"value": val, "unit": "steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
@@ -160,7 +187,8 @@ def run_fdgs(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     build.build()
-    scene = scenes.multiview_video()
+    # --stress: SURVEY 8(d) "run cfg3 additionally with cfg1-style fully random q_r as a stress variant and report both"
+    scene = scenes.multiview_video(quat_mode="random") if args.stress else scenes.multiview_video()
     views = scene.views
     n_views = len(views)
     ds = fdgs.DeviceScene.from_scene(scene, device=dev)
@@ -281,38 +309,59 @@ def run_fdgs(args):
         work["walk_bwd"] += int(r.n_contrib.sum()); work["pairs"] += st["num_pairs"]; work["visible"] += st["num_visible"]
     fdgs.set_stage_timing(False)
     # ---- roofline of the dominant kernel (algorithmic lane-instructions / measured time) ----
-    instr_fwd = 8 * work["walk"] + 3 * work["exp"] + 7 * work["comp"]
+    # Two per-unit models on the SAME measured work counters (pairs walked / reaching exp2 / composited):
+    #   "builder": forward 8 per walked pair + 3 per exp2 + 7 per composite; backward 8 + 3 + 50
+    #   "survey":  forward 13 per walked pair (12-14 incl. the MUFU) + 8 per composite; backward 14 per walked + (50 + 2 MUFU - 14) more
+    #              per composite
+    # `frac` (the headline) uses the builder's model, which is the stricter of the two.
     frac_exp = work["exp"] / max(work["walk"], 1)
-    instr_bwd = 8 * work["walk_bwd"] + 3 * frac_exp * work["walk_bwd"] + 50 * work["comp"]
+    models = {"builder": {"fwd": 8 * work["walk"] + 3 * work["exp"] + 7 * work["comp"],
+                          "bwd": 8 * work["walk_bwd"] + 3 * frac_exp * work["walk_bwd"] + 50 * work["comp"]},
+              "survey": {"fwd": 13 * work["walk"] + 8 * work["comp"],
+                         "bwd": 14 * work["walk_bwd"] + (52 - 14) * work["comp"]}}
+    instr_fwd, instr_bwd = models["builder"]["fwd"], models["builder"]["bwd"]
     dom = "blend_bwd" if stage["blend_bwd"] >= stage["blend_fwd"] else "blend_fwd"
-    instr = instr_bwd if dom == "blend_bwd" else instr_fwd
+    key = "bwd" if dom == "blend_bwd" else "fwd"
+    kernel = "blend_bwd2_kernel" if dom == "blend_bwd" else "blend_fwd_kernel"
+    instr = models["builder"][key]
     achieved = instr / n_views / (stage[dom] / n_views * 1e-3) / 1e12
-    roofline = {"kernel": "blend_bwd2_kernel" if dom == "blend_bwd" else "blend_fwd_kernel", "bound": "alu", "achieved": achieved,
-                "peak": ALU_PEAK_TLANE, "unit": "Tlane-instr/s", "frac": achieved / ALU_PEAK_TLANE,
-                "traffic": BLEND_BWD_NCU_TRAFFIC_BYTES if dom == "blend_bwd" else None,
-                "peak_source": "derived: 148 SMs x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md unit counts and max clock)",
-                "algorithmic_lane_instr_per_launch": instr / n_views, "ms_per_launch": stage[dom] / n_views}
+    traffic, traffic_src = ncu_traffic(kernel)
     peaks = fdgs.measure_peaks()           # measured FMA / MUFU pipe peaks next to the derived ALU roof
-    roofline["peak_measured_fma_tlane_per_s"] = peaks["fma_tlane_per_s"]
-    roofline["peak_measured_mufu_ex2_t_per_s"] = peaks["mufu_ex2_t_per_s"]
+    roofline = {"kernel": kernel, "bound": "alu", "achieved": achieved,
+                "peak": ALU_PEAK_TLANE, "unit": "Tlane-instr/s", "frac": achieved / ALU_PEAK_TLANE,
+                "traffic": traffic, "traffic_source": traffic_src,
+                "peak_source": "DERIVED, not measured: 148 SMs x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md unit counts and max clock)",
+                "peak_measured_fma_tlane_per_s": peaks["fma_tlane_per_s"], "peak_measured_mufu_ex2_t_per_s": peaks["mufu_ex2_t_per_s"],
+                "frac_of_measured_fma_peak": achieved / max(peaks["fma_tlane_per_s"], 1e-9),
+                "model": "builder (8/+3/+7 forward, 8/+3/+50 backward lane-instr per walked / exp2 / composited pair)",
+                "frac_by_model": {m: models[m][key] / (stage[dom] * 1e-3) / 1e12 / ALU_PEAK_TLANE for m in models},
+                "counters_per_step": {"walked_fwd": work["walk"], "exp2": work["exp"], "composited": work["comp"], "walked_bwd": work["walk_bwd"]},
+                "algorithmic_lane_instr_per_launch": instr / n_views, "ms_per_launch": stage[dom] / n_views}
     per_stage = stage_rooflines(stage, work, ds.N, ds.K, n_views)
-    for name, ins in (("blend_fwd", instr_fwd), ("blend_bwd", instr_bwd)):
-        a = ins / (stage[name] * 1e-3) / 1e12
+    for name, k2 in (("blend_fwd", "fwd"), ("blend_bwd", "bwd")):
+        a = models["builder"][k2] / (stage[name] * 1e-3) / 1e12
         per_stage[name] = {"bound": "alu", "achieved": a, "peak": ALU_PEAK_TLANE, "unit": "Tlane-instr/s", "frac": a / ALU_PEAK_TLANE,
-                           "algorithmic_lane_instr": ins}
-    # ---- CPU baseline: the oracle on one of the four views ---------------------------------------------------
+                           "frac_survey_model": models["survey"][k2] / (stage[name] * 1e-3) / 1e12 / ALU_PEAK_TLANE,
+                           "algorithmic_lane_instr": models["builder"][k2]}
+    # ---- CPU baseline: the oracle, one full step on all cores + one view on a single thread, per stage ----------
     cpu = None
     if not args.no_cpu_baseline:
-        tot, cores = 0.0, 0
-        for vi in range(n_views):
-            t, cores = oracle_view_seconds(scene, vi, 1)
-            tot += t[0]
+        per_all, cores = oracle_step_seconds(scene, range(n_views))
+        tot = sum(per_all.values())
+        per_one, _ = oracle_step_seconds(scene, [0], threads=1)
+        import oracle as _o
+        _o.set_num_threads(cores)
         cpu = {"value": 1.0 / tot, "unit": "steps/s", "cores": cores, "kind": "oracle",
-               "sample": f"one full step: all {n_views} views (preprocess+forward+L1+backward at N=1M, 1352x1014) in {tot:.1f} s"}
+               "sample": f"one full step: all {n_views} views (preprocess+forward+L1+backward at N=1M, 1352x1014) in {tot:.1f} s on {cores} threads; "
+                         f"single-thread figures: view 0 only ({sum(per_one.values()):.1f} s)",
+               "stage_seconds_per_step_all_cores": per_all,
+               "single_thread": {"cores": 1, "sample": "view 0 of the step (1 of 4 views)", "stage_seconds_per_view": per_one,
+                                 "steps_per_s_extrapolated_x4": 1.0 / (n_views * sum(per_one.values()))}}
     img_bytes = 3 * views[0].width * views[0].height * 4
     out = {"metric": METRIC, "value": whole_job_value(world, ms_step), "unit": "steps/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-           "config": {"workload": WORKLOAD, "pair_capacity": PAIR_CAPACITY, "l2": "256 MB flush write between timed steps; parameters (644 MB) exceed L2",
+           "config": {"workload": WORKLOAD, "stress_variant": args.stress, "pair_capacity": PAIR_CAPACITY,
+                      "l2": "256 MB flush write between timed steps; parameters (644 MB) exceed L2",
                       "multi_gpu": "replicas only",
                       "schedule": "fdgs_step_batch: the 4 views on 4 worker streams and workspaces, gradient accumulation chained"},
            "forward_fps": world * 1e3 / ms_frame, "ms_per_frame": ms_frame,
@@ -335,6 +384,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="fdgs", choices=["fdgs", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--stress", action="store_true", help="cfg3 with fully random q_r (SURVEY 8(d) stress variant)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "fdgs" else args.warmup
     if args.impl == "reference":

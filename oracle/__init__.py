@@ -74,6 +74,7 @@ def _load():
     lib.fdgs_oracle_backward_aux.argtypes = [C.c_void_p, dp, dp, dp] + [dp] * 10
     lib.fdgs_oracle_set_colour_override.argtypes = [C.c_void_p, dp]
     lib.fdgs_oracle_num_threads.restype = C.c_int
+    lib.fdgs_oracle_set_num_threads.argtypes = [C.c_int]
     _lib = lib
     return lib
 
@@ -84,6 +85,11 @@ def _d(a):
 
 def num_threads() -> int:
     return int(_load().fdgs_oracle_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    """OpenMP threads of the following calls (bench.py's single-thread / all-core CPU baseline)."""
+    _load().fdgs_oracle_set_num_threads(int(n))
 
 
 def sh_basis(sh_degree: int, direction) -> np.ndarray:

@@ -715,6 +715,15 @@ void fdgs_oracle_set_colour_override(void* h, const double* rgb) {
       for (int ch = 0; ch < 3; ++ch) O.prims[i].rgb[ch] = rgb[(size_t)3 * i + ch];
 }
 
+// threads used by the OpenMP loops from now on (timing only: bench.py reports single-thread and all-core times; no arithmetic)
+void fdgs_oracle_set_num_threads(int n) {
+#ifdef _OPENMP
+  if (n > 0) omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}
+
 int fdgs_oracle_num_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

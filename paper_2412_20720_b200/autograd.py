@@ -31,7 +31,7 @@ class _Render(torch.autograd.Function):
         if ds.K * 3 != sh.shape[1] * sh.shape[2] or sh.shape[0] != ds.N:
             raise ValueError(f"sh must be [N, {ds.K}, 3]")
         r = rast._renderer(ds)
-        r.preprocess(cview)
+        r.preprocess(cview, sync=True)      # raises FdgsError(ERR_PAIR_OVERFLOW) instead of training on a background image
         if aux:
             r.forward_aux(cview)
         else:

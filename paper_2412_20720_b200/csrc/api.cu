@@ -3,6 +3,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 
 #include "common.cuh"
 
@@ -25,16 +26,64 @@ static inline void mark(int which, cudaStream_t st) { if (g_timing) cudaEventRec
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-static int num_sms() {
-  static int sms = 0;
-  if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); if (sms <= 0) sms = 148; }
-  return sms;
+// Library-owned streams and events, one set per CUDA device (created on first use on that device): the worker streams
+// of fdgs_step_batch, the zeroing stream, the copy stream of fdgs_step_host, and the SM count.
+struct DeviceCtx {
+  bool ready = false;
+  int sms = 0;
+  cudaStream_t worker[FDGS_MAX_BATCH] = {}, zero_stream = nullptr, copy_stream = nullptr;
+  cudaEvent_t batch_fork = nullptr, b2_done[FDGS_MAX_BATCH] = {}, zero_done = nullptr, copy_fork = nullptr, copy_join = nullptr;
+};
+constexpr int MAX_DEVICES = 64;
+static DeviceCtx g_ctx[MAX_DEVICES];
+static std::mutex g_ctx_mutex;
+
+static int device_ctx(DeviceCtx** out) {
+  int dev = 0;
+  FDGS_CUDA(cudaGetDevice(&dev), "cudaGetDevice");
+  if (dev < 0 || dev >= MAX_DEVICES) return FDGS_ERR_INVALID;
+  std::lock_guard<std::mutex> lock(g_ctx_mutex);
+  DeviceCtx& c = g_ctx[dev];
+  if (!c.ready) {
+    FDGS_CUDA(cudaDeviceGetAttribute(&c.sms, cudaDevAttrMultiProcessorCount, dev), "SM count");
+    if (c.sms <= 0) c.sms = 148;
+    for (int i = 0; i < FDGS_MAX_BATCH; ++i) {
+      FDGS_CUDA(cudaStreamCreateWithFlags(&c.worker[i], cudaStreamNonBlocking), "worker stream");
+      FDGS_CUDA(cudaEventCreateWithFlags(&c.b2_done[i], cudaEventDisableTiming), "worker event");
+    }
+    FDGS_CUDA(cudaStreamCreateWithFlags(&c.zero_stream, cudaStreamNonBlocking), "zero stream");
+    FDGS_CUDA(cudaStreamCreateWithFlags(&c.copy_stream, cudaStreamNonBlocking), "copy stream");
+    FDGS_CUDA(cudaEventCreateWithFlags(&c.zero_done, cudaEventDisableTiming), "zero event");
+    FDGS_CUDA(cudaEventCreateWithFlags(&c.batch_fork, cudaEventDisableTiming), "fork event");
+    FDGS_CUDA(cudaEventCreateWithFlags(&c.copy_fork, cudaEventDisableTiming), "copy event");
+    FDGS_CUDA(cudaEventCreateWithFlags(&c.copy_join, cudaEventDisableTiming), "copy event");
+    c.ready = true;
+  }
+  *out = &c;
+  return FDGS_OK;
 }
 
-static int ceil_log2(long long v) { int b = 0; while ((1LL << b) < v) ++b; return b; }
+static int num_sms() {
+  DeviceCtx* c = nullptr;
+  return device_ctx(&c) == FDGS_OK ? c->sms : 148;
+}
+
+// The thresholds must describe a renderer: the backward divides by (1 - alpha), the radius takes a square root, ...
+static int check_cfg(const fdgs_config* c) {
+  if (!c) return FDGS_ERR_INVALID;
+  if (!(c->alpha_min >= 0.f) || !(c->alpha_min <= c->alpha_max) || !(c->alpha_max <= 1.f)) return FDGS_ERR_INVALID;
+  // alpha_max = 1 is the "pure eq. 6" setting: 1 - alpha can then only vanish where the forward has terminated already,
+  // unless transmittance_min = 0 too; rcp(0) of such a pixel is excluded by requiring one of the two guards
+  if (!(c->transmittance_min >= 0.f) || !(c->transmittance_min < 1.f)) return FDGS_ERR_INVALID;
+  if (!(c->dilation >= 0.f) || !(c->cutoff_sigma > 0.f) || !(c->guard > 0.f) || !(c->znear > 0.f) || !(c->marginal_min >= 0.f)) return FDGS_ERR_INVALID;
+  if (!std::isfinite(c->dilation) || !std::isfinite(c->cutoff_sigma) || !std::isfinite(c->guard) || !std::isfinite(c->znear) || !(c->marginal_min <= 1.f))
+    return FDGS_ERR_INVALID;
+  return FDGS_OK;
+}
 
 static int check_common(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, const void* ws) {
   if (!sc || !v || !c || !ws) return FDGS_ERR_INVALID;
+  if (check_cfg(c)) return FDGS_ERR_INVALID;
   if (sc->N < 0 || sc->sh_degree < 0 || sc->sh_degree > 3 || sc->n_time < 1 || sc->n_time > 8) return FDGS_ERR_INVALID;
   if (v->width <= 0 || v->height <= 0 || !(v->fx > 0) || !(v->fy > 0) || !(v->period_T > 0)) return FDGS_ERR_INVALID;
   if (sc->N > 0) {
@@ -45,6 +94,16 @@ static int check_common(const fdgs_scene* sc, const fdgs_view* v, const fdgs_con
   if (!aligned16(ws)) return FDGS_ERR_INVALID;
   const long long tx = (v->width + TILE - 1) / TILE, ty = (v->height + TILE - 1) / TILE;
   if ((tx + 1) * (ty + 1) > MAX_GRID_CELLS || tx > 65535 || ty > 65535) return FDGS_ERR_INVALID;
+  return FDGS_OK;
+}
+
+static int check_grads(const fdgs_scene* sc, const fdgs_grads* g) {
+  if (!g) return FDGS_ERR_INVALID;
+  if (sc->N <= 0) return FDGS_OK;
+  if (!g->mean || !g->log_scale || !g->quat_l || !g->quat_r || !g->opacity_logit || !g->sh) return FDGS_ERR_INVALID;
+  // every array that the backward reads or writes with 128-bit accesses
+  if (!aligned16(g->mean) || !aligned16(g->log_scale) || !aligned16(g->quat_l) || !aligned16(g->quat_r) || !aligned16(g->sh)) return FDGS_ERR_INVALID;
+  if (g->mean2d && (reinterpret_cast<uintptr_t>(g->mean2d) & 7u)) return FDGS_ERR_INVALID;
   return FDGS_OK;
 }
 
@@ -65,10 +124,6 @@ static void make_params(const fdgs_view* v, const fdgs_config* c, ViewParams& vp
   if (cp.default_thresholds) cp.log2_alpha_min = FDGS_DEF_L2MIN;   // every kernel, specialised or not, compares against the same value
 }
 
-__global__ void init_header_kernel(WsHeader* hdr, long long N, long long K, long long W, long long H, long long cap, long long tiles) {
-  hdr->N = N; hdr->K = K; hdr->W = W; hdr->H = H; hdr->pair_capacity = cap; hdr->tiles = tiles;
-}
-
 // ---- parity exports -----------------------------------------------------------------------------
 __global__ void export_records_kernel(const SplatRec* __restrict__ rec, const unsigned int* __restrict__ tiles_touched, const int N,
                                       float* __restrict__ dst) {
@@ -86,11 +141,15 @@ __global__ void export_rects_kernel(const ushort4* __restrict__ rect, const int 
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < N) { const ushort4 r = rect[i]; dst[i] = make_int4(r.x, r.y, r.z, r.w); }
 }
-// the literal 64-bit key of every sorted pair: tile id << 32 | fp32 depth bits
-__global__ void export_keys_kernel(const unsigned int* __restrict__ tile_keys, const unsigned int* __restrict__ ids,
+// the literal 64-bit key of every pair of the per-tile lists: tile id << 32 | fp32 depth bits; the tile of list position i
+// is the one whose range holds i (binary search over the tile ranges: no key array exists on the product path)
+__global__ void export_keys_kernel(const uint2* __restrict__ ranges, const int tiles, const unsigned int* __restrict__ ids,
                                    const SplatRec* __restrict__ rec, const unsigned int D, unsigned long long* __restrict__ dst) {
   const unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < D) dst[i] = ((unsigned long long)tile_keys[i] << 32) | __float_as_uint(rec[ids[i]].depth);
+  if (i >= D) return;
+  int lo = 0, hi = tiles;                                  // LARGEST tile with ranges[tile].x <= i: an empty tile shares its x with
+  while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (ranges[mid].x <= i) lo = mid; else hi = mid; }   // its successor, so this is the owner
+  dst[i] = ((unsigned long long)(unsigned int)lo << 32) | __float_as_uint(rec[ids[i]].depth);
 }
 
 // ---- measured pipe peaks: the denominators of the blend kernels' roofline ------------------------
@@ -154,28 +213,24 @@ int fdgs_preprocess(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config*
   cudaStream_t st = (cudaStream_t)stream;
   ViewParams vp; CfgParams cp;
   make_params(v, c, vp, cp);
-  // header (tickets, counters), coverage difference grid and scan states start from zero
+  // header (tickets, counters), coverage difference grid, scan states, depth-digit counts and the look-back regions of
+  // the depth sort start from zero: ONE memset per frame.  (The layout mirror for fdgs_debug_export is written by the
+  // compaction launch from its by-value arguments: no host-memory copy on the stream, so the whole call sequence can be
+  // captured into a CUDA graph.)
   FDGS_CUDA(cudaMemsetAsync(ws_ptr, 0, ws.zero_bytes, st), "memset(header)");
-  // layout mirror for fdgs_debug_export: written by a kernel from its by-value arguments (no host-memory copy on the
-  // stream, so the whole call sequence can be captured into a CUDA graph)
-  init_header_kernel<<<1, 1, 0, st>>>(ws.hdr, sc->N, K, v->width, v->height, cap, (long long)vp.tiles_x * vp.tiles_y);
-  ++g_launches;
   mark(EV_PRE0, st);
   launch_preprocess_fwd(*sc, vp, cp, ws, st);                       // A1-A4 (+ coverage grid)
   mark(EV_PRE1, st);
-  launch_compact(ws, sc->N, st);                                    // survivors -> (depth bits, id)
-  const int l2_passes = (ceil_log2((long long)vp.tiles_x * vp.tiles_y) + RADIX_BITS - 1) / RADIX_BITS;
-  launch_tile_grid(ws, vp, cap, l2_passes > 0 ? l2_passes : 1, st); // A5/A8: list lengths -> ranges, D
+  launch_compact_and_tile_grid(ws, sc->N, K, vp, cap, st);          // survivors -> (depth bits, id); A5/A8: list lengths -> ranges, D
   mark(EV_PRE2, st);
   FDGS_CUDA(cudaGetLastError(), "preprocess launches");
   if (num_pairs_host || num_visible_host) {
     FDGS_CUDA(cudaStreamSynchronize(st), "preprocess sync");
-    unsigned int hv[16];
-    FDGS_CUDA(cudaMemcpy(hv, ws.hdr, sizeof(hv), cudaMemcpyDeviceToHost), "read header");
-    const WsHeader* hh = reinterpret_cast<const WsHeader*>(hv);
-    if (num_pairs_host) *num_pairs_host = hh->pad[0];
-    if (num_visible_host) *num_visible_host = (int32_t)hh->num_visible;
-    if (hh->overflow) return FDGS_ERR_PAIR_OVERFLOW;
+    WsHeader hh;
+    FDGS_CUDA(cudaMemcpy(&hh, ws.hdr, sizeof(hh), cudaMemcpyDeviceToHost), "read header");
+    if (num_pairs_host) *num_pairs_host = hh.total_pairs;
+    if (num_visible_host) *num_visible_host = (int32_t)hh.num_visible;
+    if (hh.overflow) return FDGS_ERR_PAIR_OVERFLOW;
   }
   return FDGS_OK;
 }
@@ -184,33 +239,30 @@ int fdgs_preprocess(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config*
 
 // A6-A9.  The depth order of the survivors (level 1) is kept in the workspace for the backward.
 static int forward_impl(const fdgs_scene* sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, int64_t cap,
-                        cudaStream_t st, float* image, float* final_T, uint32_t* n_contrib, float* depth_map, int* l1_buf_out, int* l2_buf_out) {
-  // scan_ticket[1] and sort_ticket[0..7] are adjacent in the header: clear them together
-  FDGS_CUDA(cudaMemsetAsync(&ws.hdr->scan_ticket[1], 0, 9 * sizeof(unsigned int), st), "memset(tickets)");
-  FDGS_CUDA(cudaMemsetAsync(ws.scan_state[1], 0, 8 * ((size_t)(sc->N > 0 ? sc->N : 1) / 256 + 2), st), "memset(scan)");
+                        cudaStream_t st, float* image, float* final_T, uint32_t* n_contrib, float* depth_map) {
+  (void)cap;
   const int sms = num_sms();
   mark(EV_FWD0, st);
-  const int l1 = launch_sort_pairs(ws, ws.l1_keys, ws.l1_vals, &ws.hdr->num_visible, sc->N, 32, SORT_ITEMS_L1, 0, false, sms, st);
+  const int l1 = launch_sort_depth(ws, sc->N, sms, st);             // level 1: survivors by fp32 depth bits
   mark(EV_FWD1, st);
   launch_offsets(ws, l1, sc->N, st);
-  launch_duplicate(ws, l1, sc->N, cap, vp, st);
   mark(EV_FWD2, st);
-  const int tile_bits = ceil_log2((long long)vp.tiles_x * vp.tiles_y);
-  const int l2 = launch_sort_pairs(ws, ws.l2_keys, ws.l2_vals, &ws.hdr->num_pairs, cap, tile_bits, SORT_ITEMS_L2, 4, true, sms, st);
+  launch_pair_scatter(ws, l1, sc->N, vp, sms, st);                  // level 2: per-tile lists written in place, depth order
   mark(EV_FWD3, st);
-  launch_blend_fwd(ws, l2, vp, cp, image, final_T, n_contrib, depth_map, st);
+  launch_blend_fwd(ws, vp, cp, image, final_T, n_contrib, depth_map, st);
   mark(EV_FWD4, st);
   FDGS_CUDA(cudaGetLastError(), "forward launches");
-  *l1_buf_out = l1; *l2_buf_out = l2;
   return FDGS_OK;
 }
 
-static void sort_bufs(const fdgs_scene* sc, const ViewParams& vp, int64_t cap, int* l1, int* l2) {
-  // result buffers are a function of the pass counts only
-  *l1 = sc->N > 0 ? (4 & 1) : 0;
-  const int tile_bits = ceil_log2((long long)vp.tiles_x * vp.tiles_y);
-  const int p2 = (tile_bits + RADIX_BITS - 1) / RADIX_BITS;
-  *l2 = (p2 > 0 && cap > 0) ? (p2 & 1) : 0;
+// buffer of the depth-sorted survivor ids: a function of the pass count only
+static int depth_buf() { return DEPTH_PASSES & 1; }
+
+// after a synchronisation: has the last preprocess on this workspace exceeded the pair capacity?
+static int read_overflow(const Workspace& ws) {
+  unsigned int ov = 0;
+  FDGS_CUDA(cudaMemcpy(&ov, &ws.hdr->overflow, sizeof(ov), cudaMemcpyDeviceToHost), "read overflow flag");
+  return ov ? FDGS_ERR_PAIR_OVERFLOW : FDGS_OK;
 }
 
 extern "C" {
@@ -225,8 +277,7 @@ static int forward_entry(const fdgs_scene* sc, const fdgs_view* v, const fdgs_co
   if (ws.bytes > ws_bytes) return FDGS_ERR_WORKSPACE;
   ViewParams vp; CfgParams cp;
   make_params(v, c, vp, cp);
-  int l1, l2;
-  return forward_impl(sc, vp, cp, ws, cap, (cudaStream_t)stream, image, final_T, n_contrib, depth_map, &l1, &l2);
+  return forward_impl(sc, vp, cp, ws, cap, (cudaStream_t)stream, image, final_T, n_contrib, depth_map);
 }
 
 int fdgs_render_forward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
@@ -249,21 +300,19 @@ static int backward_impl(const fdgs_scene* sc, const fdgs_view* v, const fdgs_co
                          const fdgs_grads* g, cudaEvent_t before_b2, const float* dL_ddepth = nullptr, const float* dL_dopacity = nullptr) {
   int rc = check_common(sc, v, c, ws_ptr);
   if (rc) return rc;
-  if (!dL_dimage || !final_T || !n_contrib || !g || cap < 1 || cap >= (1LL << 30)) return FDGS_ERR_INVALID;
-  if (sc->N > 0 && (!g->mean || !g->log_scale || !g->quat_l || !g->quat_r || !g->opacity_logit || !g->sh)) return FDGS_ERR_INVALID;
-  if (sc->N > 0 && (!aligned16(g->mean) || !aligned16(g->log_scale) || !aligned16(g->quat_l) || !aligned16(g->quat_r))) return FDGS_ERR_INVALID;
+  if (!dL_dimage || !final_T || !n_contrib || cap < 1 || cap >= (1LL << 30)) return FDGS_ERR_INVALID;
+  if ((rc = check_grads(sc, g))) return rc;
   const int K = sc->n_time * (sc->sh_degree + 1) * (sc->sh_degree + 1);
   const Workspace ws = carve(ws_ptr, sc->N, K, v->width, v->height, cap);
   if (ws.bytes > ws_bytes) return FDGS_ERR_WORKSPACE;
   ViewParams vp; CfgParams cp;
   make_params(v, c, vp, cp);
-  int l1, l2;
-  sort_bufs(sc, vp, cap, &l1, &l2);
+  const int l1 = depth_buf();
   if (sc->N > 0) FDGS_CUDA(cudaMemsetAsync(ws.g9, 0, sizeof(float) * 9 * (size_t)sc->N, st), "memset(g9)");
   const bool aux = dL_ddepth || dL_dopacity;
   if (aux && sc->N > 0) FDGS_CUDA(cudaMemsetAsync(ws.gz, 0, sizeof(float) * (size_t)sc->N, st), "memset(gz)");
   mark(EV_BWD0, st);
-  launch_blend_bwd(ws, l2, vp, cp, dL_dimage, final_T, n_contrib, dL_ddepth, dL_dopacity, st);   // B1
+  launch_blend_bwd(ws, vp, cp, dL_dimage, final_T, n_contrib, dL_ddepth, dL_dopacity, st);   // B1
   mark(EV_BWD1, st);
   if (before_b2) FDGS_CUDA(cudaStreamWaitEvent(st, before_b2, 0), "wait before B2");
   launch_preprocess_bwd(*sc, vp, cp, ws, l1, *g, aux, st);                      // B2
@@ -288,120 +337,120 @@ int fdgs_render_backward_aux(const fdgs_scene* sc, const fdgs_view* v, const fdg
 
 int fdgs_l1_loss(const float* image, const float* target, int64_t count, float* dL_dimage, float* loss, void* stream) {
   if (!image || !target || !dL_dimage || !loss || count <= 0) return FDGS_ERR_INVALID;
-  launch_l1_loss(image, target, count, dL_dimage, loss, (cudaStream_t)stream);
+  launch_l1_loss(image, target, count, dL_dimage, loss, nullptr, (cudaStream_t)stream);
   FDGS_CUDA(cudaGetLastError(), "l1 loss launch");
   return FDGS_OK;
 }
 
-// Copy stream of fdgs_step_host: the target image travels host -> device while preprocess and forward run.
-static cudaStream_t g_copy_stream = nullptr;
-static cudaEvent_t g_copy_fork = nullptr, g_copy_join = nullptr;
+// loss of a view inside the step calls: as fdgs_l1_loss, but a view whose pairs exceeded the capacity (nothing drawn, all
+// gradients zero) reports NaN instead of the loss of a background image, so that even a fully asynchronous caller sees it
+static int step_loss(const Workspace& ws, const float* image, const float* target, int64_t count, float* dL_dimage, float* loss, cudaStream_t st) {
+  launch_l1_loss(image, target, count, dL_dimage, loss, &ws.hdr->overflow, st);
+  FDGS_CUDA(cudaGetLastError(), "l1 loss launch");
+  return FDGS_OK;
+}
 
 int fdgs_step_host(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws, size_t ws_bytes, int64_t cap,
                    void* stream, const float* target_host, float* target_dev, float* image, float* final_T,
                    uint32_t* n_contrib, float* dL_dimage, float* loss_dev, fdgs_grads* g, float* result_host) {
   if (!v || !result_host) return FDGS_ERR_INVALID;
+  int rc = check_common(sc, v, c, ws);
+  if (rc) return rc;
+  if (g && (rc = check_grads(sc, g))) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   const size_t count = (size_t)3 * v->width * v->height;
+  DeviceCtx* ctx = nullptr;
+  if ((rc = device_ctx(&ctx))) return rc;
+  bool forked = false;
+  // after the fork nothing may return before the copy stream has been joined into `st` again (the caller may reuse
+  // target_dev as soon as `st` is idle): errors fall through to the join
   if (g) {
     if (!target_host || !target_dev || !dL_dimage || !loss_dev) return FDGS_ERR_INVALID;
-    if (!g_copy_stream) {
-      FDGS_CUDA(cudaStreamCreateWithFlags(&g_copy_stream, cudaStreamNonBlocking), "copy stream");
-      FDGS_CUDA(cudaEventCreateWithFlags(&g_copy_fork, cudaEventDisableTiming), "copy event");
-      FDGS_CUDA(cudaEventCreateWithFlags(&g_copy_join, cudaEventDisableTiming), "copy event");
-    }
     // fork: the copy may start once everything queued on `st` so far (the previous user of target_dev) is done
-    FDGS_CUDA(cudaEventRecord(g_copy_fork, st), "fork");
-    FDGS_CUDA(cudaStreamWaitEvent(g_copy_stream, g_copy_fork, 0), "fork wait");
-    FDGS_CUDA(cudaMemcpyAsync(target_dev, target_host, count * sizeof(float), cudaMemcpyHostToDevice, g_copy_stream), "H2D target");
-    FDGS_CUDA(cudaEventRecord(g_copy_join, g_copy_stream), "join");
-    FDGS_CUDA(cudaMemsetAsync(loss_dev, 0, sizeof(float), st), "memset(loss)");
+    FDGS_CUDA(cudaEventRecord(ctx->copy_fork, st), "fork");
+    FDGS_CUDA(cudaStreamWaitEvent(ctx->copy_stream, ctx->copy_fork, 0), "fork wait");
+    forked = true;
+    cudaMemcpyAsync(target_dev, target_host, count * sizeof(float), cudaMemcpyHostToDevice, ctx->copy_stream);
+    cudaEventRecord(ctx->copy_join, ctx->copy_stream);
+    cudaMemsetAsync(loss_dev, 0, sizeof(float), st);
   }
-  int rc = fdgs_preprocess(sc, v, c, ws, ws_bytes, cap, stream, nullptr, nullptr);
-  if (rc) return rc;
-  rc = fdgs_render_forward(sc, v, c, ws, ws_bytes, cap, stream, image, final_T, n_contrib);
-  if (rc) return rc;
+  rc = fdgs_preprocess(sc, v, c, ws, ws_bytes, cap, stream, nullptr, nullptr);
+  if (!rc) rc = fdgs_render_forward(sc, v, c, ws, ws_bytes, cap, stream, image, final_T, n_contrib);
+  if (forked) cudaStreamWaitEvent(st, ctx->copy_join, 0);
+  if (rc) { cudaStreamSynchronize(st); return rc; }
+  const int K = sc->n_time * (sc->sh_degree + 1) * (sc->sh_degree + 1);
+  const Workspace wsv = carve(ws, sc->N, K, v->width, v->height, cap);
   if (g) {
-    FDGS_CUDA(cudaStreamWaitEvent(st, g_copy_join, 0), "join wait");
-    rc = fdgs_l1_loss(image, target_dev, (int64_t)count, dL_dimage, loss_dev, stream);
-    if (rc) return rc;
-    rc = fdgs_render_backward(sc, v, c, ws, ws_bytes, cap, stream, dL_dimage, final_T, n_contrib, g);
-    if (rc) return rc;
-    FDGS_CUDA(cudaMemcpyAsync(result_host, loss_dev, sizeof(float), cudaMemcpyDeviceToHost, st), "D2H loss");
+    rc = step_loss(wsv, image, target_dev, (int64_t)count, dL_dimage, loss_dev, st);
+    if (!rc) rc = fdgs_render_backward(sc, v, c, ws, ws_bytes, cap, stream, dL_dimage, final_T, n_contrib, g);
+    if (!rc) FDGS_CUDA(cudaMemcpyAsync(result_host, loss_dev, sizeof(float), cudaMemcpyDeviceToHost, st), "D2H loss");
   } else {
     FDGS_CUDA(cudaMemcpyAsync(result_host, image, count * sizeof(float), cudaMemcpyDeviceToHost, st), "D2H image");
   }
   FDGS_CUDA(cudaStreamSynchronize(st), "step sync");
-  return FDGS_OK;
+  if (rc) return rc;
+  return read_overflow(wsv);         // D > pair_capacity: nothing was drawn and every gradient is zero — say so
 }
-
-// Worker streams of fdgs_step_batch (one per view of the batch), created on first use.
-static cudaStream_t g_worker[FDGS_MAX_BATCH], g_zero_stream = nullptr;
-static cudaEvent_t g_batch_fork = nullptr, g_b2_done[FDGS_MAX_BATCH], g_zero_done = nullptr;
 
 int fdgs_step_batch(const fdgs_scene* sc, const fdgs_view* views, int32_t num_views, const fdgs_config* c, int64_t cap,
                     const fdgs_view_buffers* bufs, void* stream, float* loss_dev, const fdgs_grads* g, float* loss_host, int32_t flags) {
   if (!sc || !views || !c || !bufs || !loss_dev || !g || num_views < 1 || num_views > FDGS_MAX_BATCH) return FDGS_ERR_INVALID;
-  if (sc->N > 0 && (!g->mean || !g->log_scale || !g->quat_l || !g->quat_r || !g->opacity_logit || !g->sh)) return FDGS_ERR_INVALID;
-  for (int i = 0; i < num_views; ++i) {
+  if (cap < 1 || cap >= (1LL << 30)) return FDGS_ERR_INVALID;
+  int rc = check_grads(sc, g);
+  if (rc) return rc;
+  const int K = sc->n_time * (sc->sh_degree + 1) * (sc->sh_degree + 1);
+  for (int i = 0; i < num_views; ++i) {          // everything that can be rejected is rejected before the first fork
     const fdgs_view_buffers& b = bufs[i];
     if (!b.ws || !b.target_dev || !b.image || !b.final_T || !b.n_contrib || !b.dL_dimage) return FDGS_ERR_INVALID;
     for (int k = 0; k < i; ++k) if (bufs[k].ws == b.ws) return FDGS_ERR_INVALID;      // one workspace per view
+    if ((rc = check_common(sc, &views[i], c, b.ws))) return rc;
+    if (carve(nullptr, sc->N, K, views[i].width, views[i].height, cap).bytes > b.ws_bytes) return FDGS_ERR_WORKSPACE;
   }
   cudaStream_t st = (cudaStream_t)stream;
-  if (!g_batch_fork) {
-    // FDGS_BATCH_PRIO (experiment): view i's stream gets a higher priority than view i+1's, so that the views drift apart
-    // and the HBM-bound stages of one overlap the issue-bound blend kernels of the next
-    int lo = 0, hi = 0;
-    cudaDeviceGetStreamPriorityRange(&lo, &hi);          // lo = least priority (numerically largest)
-    const char* pe = getenv("FDGS_BATCH_PRIO");
-    const int prio_mode = pe ? atoi(pe) : 0;
-    for (int i = 0; i < FDGS_MAX_BATCH; ++i) {
-      int pr = lo;
-      if (prio_mode == 1) { pr = hi + i; if (pr > lo) pr = lo; }
-      FDGS_CUDA(cudaStreamCreateWithPriority(&g_worker[i], cudaStreamNonBlocking, pr), "worker stream");
-      FDGS_CUDA(cudaEventCreateWithFlags(&g_b2_done[i], cudaEventDisableTiming), "worker event");
-    }
-    FDGS_CUDA(cudaStreamCreateWithFlags(&g_zero_stream, cudaStreamNonBlocking), "zero stream");
-    FDGS_CUDA(cudaEventCreateWithFlags(&g_zero_done, cudaEventDisableTiming), "zero event");
-    FDGS_CUDA(cudaEventCreateWithFlags(&g_batch_fork, cudaEventDisableTiming), "fork event");
-  }
-  FDGS_CUDA(cudaEventRecord(g_batch_fork, st), "fork");
+  DeviceCtx* ctx = nullptr;
+  if ((rc = device_ctx(&ctx))) return rc;
+  FDGS_CUDA(cudaEventRecord(ctx->batch_fork, st), "fork");
   const bool zero = (flags & FDGS_STEP_ZERO_GRADS) && sc->N > 0;
   if (zero) {   // the gradient arrays are first touched by the first view's backward preprocess: zeroing them hides under the forward passes
-    const size_t N = (size_t)sc->N, K = (size_t)sc->n_time * (sc->sh_degree + 1) * (sc->sh_degree + 1);
-    FDGS_CUDA(cudaStreamWaitEvent(g_zero_stream, g_batch_fork, 0), "fork wait");
-    FDGS_CUDA(cudaMemsetAsync(g->mean, 0, 16 * N, g_zero_stream), "zero grads");
-    FDGS_CUDA(cudaMemsetAsync(g->log_scale, 0, 16 * N, g_zero_stream), "zero grads");
-    FDGS_CUDA(cudaMemsetAsync(g->quat_l, 0, 16 * N, g_zero_stream), "zero grads");
-    FDGS_CUDA(cudaMemsetAsync(g->quat_r, 0, 16 * N, g_zero_stream), "zero grads");
-    FDGS_CUDA(cudaMemsetAsync(g->opacity_logit, 0, 4 * N, g_zero_stream), "zero grads");
-    FDGS_CUDA(cudaMemsetAsync(g->sh, 0, 12 * K * N, g_zero_stream), "zero grads");
-    if (g->mean2d) FDGS_CUDA(cudaMemsetAsync(g->mean2d, 0, 8 * N, g_zero_stream), "zero grads");
-    FDGS_CUDA(cudaEventRecord(g_zero_done, g_zero_stream), "zero done");
+    const size_t N = (size_t)sc->N;
+    cudaStreamWaitEvent(ctx->zero_stream, ctx->batch_fork, 0);
+    cudaMemsetAsync(g->mean, 0, 16 * N, ctx->zero_stream);
+    cudaMemsetAsync(g->log_scale, 0, 16 * N, ctx->zero_stream);
+    cudaMemsetAsync(g->quat_l, 0, 16 * N, ctx->zero_stream);
+    cudaMemsetAsync(g->quat_r, 0, 16 * N, ctx->zero_stream);
+    cudaMemsetAsync(g->opacity_logit, 0, 4 * N, ctx->zero_stream);
+    cudaMemsetAsync(g->sh, 0, 12 * (size_t)K * N, ctx->zero_stream);
+    if (g->mean2d) cudaMemsetAsync(g->mean2d, 0, 8 * N, ctx->zero_stream);
+    cudaEventRecord(ctx->zero_done, ctx->zero_stream);
   }
-  for (int i = 0; i < num_views; ++i) {
+  // From here on work is forked onto library streams: an error stops issuing, but every stream that was given work is
+  // still joined into `st` before the call returns, so the caller can never free or reuse buffers under running kernels.
+  int launched = 0;
+  for (int i = 0; i < num_views && !rc; ++i) {
     const fdgs_view_buffers& b = bufs[i];
-    cudaStream_t w = g_worker[i];
+    cudaStream_t w = ctx->worker[i];
     const size_t count = (size_t)3 * views[i].width * views[i].height;
-    FDGS_CUDA(cudaStreamWaitEvent(w, g_batch_fork, 0), "fork wait");
-    if (b.target_host) FDGS_CUDA(cudaMemcpyAsync(b.target_dev, b.target_host, count * sizeof(float), cudaMemcpyHostToDevice, w), "H2D target");
-    FDGS_CUDA(cudaMemsetAsync(loss_dev + i, 0, sizeof(float), w), "memset(loss)");
-    int rc = fdgs_preprocess(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, nullptr, nullptr);
-    if (rc) return rc;
-    rc = fdgs_render_forward(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, b.image, b.final_T, b.n_contrib);
-    if (rc) return rc;
-    rc = fdgs_l1_loss(b.image, b.target_dev, (int64_t)count, b.dL_dimage, loss_dev + i, w);
-    if (rc) return rc;
+    cudaStreamWaitEvent(w, ctx->batch_fork, 0);
+    launched = i + 1;
+    if (b.target_host) cudaMemcpyAsync(b.target_dev, b.target_host, count * sizeof(float), cudaMemcpyHostToDevice, w);
+    cudaMemsetAsync(loss_dev + i, 0, sizeof(float), w);
+    rc = fdgs_preprocess(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, nullptr, nullptr);
+    if (!rc) rc = fdgs_render_forward(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, b.image, b.final_T, b.n_contrib);
+    if (!rc) rc = step_loss(carve(b.ws, sc->N, K, views[i].width, views[i].height, cap), b.image, b.target_dev, (int64_t)count, b.dL_dimage, loss_dev + i, w);
     // blend backward of this view overlaps everything of the others; the gradient accumulation (B2) is chained
-    rc = backward_impl(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, b.dL_dimage, b.final_T, b.n_contrib, g, i > 0 ? g_b2_done[i - 1] : (zero ? g_zero_done : nullptr));
-    if (rc) return rc;
-    FDGS_CUDA(cudaEventRecord(g_b2_done[i], w), "record B2");
+    if (!rc) rc = backward_impl(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, b.dL_dimage, b.final_T, b.n_contrib, g,
+                                i > 0 ? ctx->b2_done[i - 1] : (zero ? ctx->zero_done : nullptr));
+    cudaEventRecord(ctx->b2_done[i], w);
   }
-  for (int i = 0; i < num_views; ++i) FDGS_CUDA(cudaStreamWaitEvent(st, g_b2_done[i], 0), "join");
+  for (int i = 0; i < launched; ++i) cudaStreamWaitEvent(st, ctx->b2_done[i], 0);
+  if (zero) cudaStreamWaitEvent(st, ctx->zero_done, 0);
+  if (rc) { cudaStreamSynchronize(st); return rc; }
+  FDGS_CUDA(cudaGetLastError(), "batch launches");
   if (loss_host) {
     FDGS_CUDA(cudaMemcpyAsync(loss_host, loss_dev, sizeof(float) * num_views, cudaMemcpyDeviceToHost, st), "D2H loss");
     FDGS_CUDA(cudaStreamSynchronize(st), "batch sync");
+    for (int i = 0; i < num_views; ++i)
+      if ((rc = read_overflow(carve(bufs[i].ws, sc->N, K, views[i].width, views[i].height, cap)))) return rc;
   }
   return FDGS_OK;
 }
@@ -433,6 +482,7 @@ static int features_common(const fdgs_scene* sc, const fdgs_view* v, const fdgs_
   int rc = check_common(sc, v, c, ws_ptr);
   if (rc) return rc;
   if (C < 1 || cap < 1 || cap >= (1LL << 30) || !scratch || !aligned16(scratch) || (sc->N > 0 && !feat)) return FDGS_ERR_INVALID;
+  if (!aligned16(feat)) return FDGS_ERR_INVALID;          // rows of feat[N,C] are read with 128-bit loads when C % 4 == 0
   const int K = sc->n_time * (sc->sh_degree + 1) * (sc->sh_degree + 1);
   ws = carve(ws_ptr, sc->N, K, v->width, v->height, cap);
   if (ws.bytes > ws_bytes) return FDGS_ERR_WORKSPACE;
@@ -440,7 +490,7 @@ static int features_common(const fdgs_scene* sc, const fdgs_view* v, const fdgs_
   if (fs.bytes > scratch_bytes) return FDGS_ERR_WORKSPACE;
   make_params(v, c, vp, cp);
   vp.bg[0] = vp.bg[1] = vp.bg[2] = 0.f;                 // features have no background term
-  sort_bufs(sc, vp, cap, l1, l2);
+  *l1 = depth_buf(); *l2 = 0;
   return FDGS_OK;
 }
 
@@ -457,7 +507,7 @@ int fdgs_render_features_forward(const fdgs_scene* sc, const fdgs_view* v, const
   const size_t HW = (size_t)v->width * v->height;
   (void)HW;
   // dedicated C-channel kernel: alpha evaluated once per 16 channels, features gathered by id next to the records
-  launch_blend_feat_fwd(ws, l2, vp, cp, feat, C, out, st);
+  launch_blend_feat_fwd(ws, vp, cp, feat, C, out, st);
   FDGS_CUDA(cudaGetLastError(), "feature forward launches");
   return FDGS_OK;
 }
@@ -470,17 +520,14 @@ int fdgs_render_features_backward(const fdgs_scene* sc, const fdgs_view* v, cons
   int rc = features_common(sc, v, c, ws_ptr, ws_bytes, cap, feat, C, scratch, scratch_bytes, ws, fs, vp, cp, &l1, &l2);
   if (rc) return rc;
   if (!dL_dout || !final_T || !n_contrib || (sc->N > 0 && !grad_feat)) return FDGS_ERR_INVALID;
-  if (g && sc->N > 0) {
-    if (!g->mean || !g->log_scale || !g->quat_l || !g->quat_r || !g->opacity_logit || !g->sh) return FDGS_ERR_INVALID;
-    if (!aligned16(g->mean) || !aligned16(g->log_scale) || !aligned16(g->quat_l) || !aligned16(g->quat_r)) return FDGS_ERR_INVALID;
-  }
+  if (g && (rc = check_grads(sc, g))) return rc;
   if (sc->N == 0) return FDGS_OK;
   cudaStream_t st = (cudaStream_t)stream;
   const size_t HW = (size_t)v->width * v->height;
   Workspace wf = ws;
   wf.rec = fs.rec;
   if (!g) {   // geometry frozen: dL/dfeat only needs the weights alpha_k T_k — dedicated front-to-back kernel
-    launch_blend_feat_bwd(ws, l2, vp, cp, dL_dout, C, grad_feat, st);
+    launch_blend_feat_bwd(ws, vp, cp, dL_dout, C, grad_feat, st);
     FDGS_CUDA(cudaGetLastError(), "feature backward launches");
     return FDGS_OK;
   }
@@ -494,7 +541,7 @@ int fdgs_render_features_backward(const fdgs_scene* sc, const fdgs_view* v, cons
       FDGS_CUDA(cudaMemcpyAsync(fs.img3, dL, sizeof(float) * n * HW, cudaMemcpyDeviceToDevice, st), "copy planes");
       dL = fs.img3;
     }
-    launch_blend_bwd(wf, l2, vp, cp, dL, final_T, n_contrib, nullptr, nullptr, st);   // geometry slots of g9 add up over the passes
+    launch_blend_bwd(wf, vp, cp, dL, final_T, n_contrib, nullptr, nullptr, st);   // geometry slots of g9 add up over the passes
     launch_extract_feature_grads(ws, grad_feat, C, c0, sc->N, st);
   }
   // chain (u, v, conic, opacity) to the parameters once; the colour slots are zero, so the 4DSH coefficients get nothing
@@ -523,7 +570,7 @@ int fdgs_splat_flow(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config*
 
 extern "C" {
 
-int64_t fdgs_launch_count(void) { return g_launches; }
+int64_t fdgs_launch_count(void) { return launch_count_value(); }
 
 int fdgs_set_stage_timing(int enable) {
   if (enable && !g_timing) for (int i = 0; i < EV_COUNT; ++i) FDGS_CUDA(cudaEventCreate(&g_ev[i]), "event create");
@@ -551,17 +598,14 @@ int fdgs_debug_blend_stats(const fdgs_view* v, const fdgs_config* c, void* ws_pt
   if (ws.bytes > ws_bytes) return FDGS_ERR_WORKSPACE;
   ViewParams vp; CfgParams cp;
   make_params(v, c, vp, cp);
-  fdgs_scene sc; sc.N = N;
-  int l1, l2;
-  sort_bufs(&sc, vp, cap, &l1, &l2);
   FDGS_CUDA(cudaMemsetAsync(stats_dev, 0, 4 * sizeof(unsigned long long), (cudaStream_t)stream), "memset(stats)");
-  launch_blend_stats(ws, l2, vp, cp, stats_dev, (cudaStream_t)stream);
+  launch_blend_stats(ws, vp, cp, stats_dev, (cudaStream_t)stream);
   FDGS_CUDA(cudaGetLastError(), "stats launch");
   return FDGS_OK;
 }
 
 int fdgs_debug_cull_status(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* stream, unsigned char* status_dev) {
-  if (!sc || !v || !c || !status_dev || sc->N < 0 || v->width <= 0 || v->height <= 0 || !(v->period_T > 0)) return FDGS_ERR_INVALID;
+  if (!sc || !v || !c || !status_dev || sc->N < 0 || v->width <= 0 || v->height <= 0 || !(v->period_T > 0) || check_cfg(c)) return FDGS_ERR_INVALID;
   ViewParams vp; CfgParams cp;
   make_params(v, c, vp, cp);
   launch_cull_status(*sc, vp, cp, status_dev, (cudaStream_t)stream);
@@ -622,15 +666,12 @@ extern "C" int fdgs_debug_export(const void* ws_ptr, size_t ws_bytes, int what, 
   const Workspace ws = carve(const_cast<void*>(ws_ptr), h.N, h.K, h.W, h.H, h.pair_capacity);
   if (ws.bytes > ws_bytes) return FDGS_ERR_WORKSPACE;
   const long long N = h.N, D = h.num_pairs;
-  ViewParams vp; vp.tiles_x = (int)((h.W + TILE - 1) / TILE); vp.tiles_y = (int)((h.H + TILE - 1) / TILE);
-  fdgs_scene sc; sc.N = (int)N;
-  int l1, l2;
-  sort_bufs(&sc, vp, h.pair_capacity, &l1, &l2);
+  const int l1 = depth_buf();
   size_t need = 0;
   const void* src = nullptr;
   switch (what) {
     case FDGS_EXPORT_STATUS: {
-      const long long status[4] = {(long long)h.pad[0], (long long)h.num_visible, (long long)h.overflow, h.pair_capacity};
+      const long long status[4] = {(long long)h.total_pairs, (long long)h.num_visible, (long long)h.overflow, h.pair_capacity};
       if (dst_bytes < sizeof(status)) return FDGS_ERR_INVALID;
       FDGS_CUDA(cudaMemcpy(dst, status, sizeof(status), cudaMemcpyHostToDevice), "export status");
       return h.overflow ? FDGS_ERR_PAIR_OVERFLOW : FDGS_OK;
@@ -648,9 +689,9 @@ extern "C" int fdgs_debug_export(const void* ws_ptr, size_t ws_bytes, int what, 
     case FDGS_EXPORT_DEPTH_ORDER: src = ws.l1_vals[l1]; need = 4 * (size_t)h.num_visible; break;
     case FDGS_EXPORT_SORTED_KEYS:
       if (dst_bytes < 8 * (size_t)D) return FDGS_ERR_INVALID;
-      if (D > 0) export_keys_kernel<<<(unsigned)((D + 255) / 256), 256, 0, st>>>(ws.l2_keys[l2], ws.l2_vals[l2], ws.rec, (unsigned)D, (unsigned long long*)dst);
+      if (D > 0) export_keys_kernel<<<(unsigned)((D + 255) / 256), 256, 0, st>>>(ws.ranges, (int)h.tiles, ws.pair_ids, ws.rec, (unsigned)D, (unsigned long long*)dst);
       break;
-    case FDGS_EXPORT_SORTED_VALS: src = ws.l2_vals[l2]; need = 4 * (size_t)D; break;
+    case FDGS_EXPORT_SORTED_VALS: src = ws.pair_ids; need = 4 * (size_t)D; break;
     case FDGS_EXPORT_RANGES: src = ws.ranges; need = 8 * (size_t)h.tiles; break;
     case FDGS_EXPORT_SPLAT_GRADS: src = ws.g9; need = 36 * (size_t)N; break;
     case FDGS_EXPORT_SPLAT_GRAD_DEPTH: src = ws.gz; need = 4 * (size_t)N; break;

@@ -8,8 +8,6 @@
 //     e1 = k1 - ca*x - cb*y,  e2 = k2 - cc*y,  log2(alpha) = lo - e1^2 - e2^2      (x, y tile-local pixel centres)
 // i.e. 5 FFMA + 1 MUFU.EX2 per (pixel, splat) evaluation; tile-local coordinates keep |e| small so fp32
 // cancellation stays ~1e-7.
-#include <cstdlib>
-
 #include "common.cuh"
 
 namespace fdgs {
@@ -410,172 +408,16 @@ __global__ void __launch_bounds__(128) blend_feat_bwd_kernel(const uint2* __rest
 }
 
 // ---------------------------------------------------------------------------------------------
-// Sum of 8 values over the 32 lanes with 9 shuffles (halving exchange), result k lands on lane 4k.
-__device__ __forceinline__ float warp_reduce8(float v[8], const int lane) {
-  const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const float keep = b4 ? v[i + 4] : v[i], send = b4 ? v[i] : v[i + 4];
-    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-  }
-#pragma unroll
-  for (int i = 0; i < 2; ++i) {
-    const float keep = b3 ? v[i + 2] : v[i], send = b3 ? v[i] : v[i + 2];
-    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-  }
-  {
-    const float keep = b2 ? v[1] : v[0], send = b2 ? v[0] : v[1];
-    v[0] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-  }
-  v[0] += __shfl_xor_sync(0xffffffffu, v[0], 2);
-  v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
-  return v[0];
-}
-
-// B1.  Walks each tile list back to front from the last contributor of the tile.  Per (pixel, splat) the lane
-// produces two scalars, wgt = alpha T (for dL/dc) and dpow = alpha dL/dalpha (for everything that flows through the
-// exponent), and nine products of them with per-pixel quantities:
+// B1, transposed accumulation (PX = 2).  Walks each tile list back to front from the last contributor of the tile.  Per
+// (pixel, splat) the lane produces two scalars, wgt = alpha T (for dL/dc) and dpow = alpha dL/dalpha (for everything that
+// flows through the exponent); the per-splat gradients are nine sums over pixels of their products with per-pixel quantities:
 //     dpow * {dx, dy, dx^2, dx dy, dy^2, 1}   and   wgt * dL/dpixel{r,g,b}        (dx = u - px, dy = v - py)
-// summed over the lane's PX pixels, reduced over the warp by shuffles, then over the warps in shared memory; one
-// thread per splat turns the nine sums into dL/d(u, v, A, B, C, o, r, g, b) and flushes nine global atomics per
-// (tile, splat):
 //     dL/du = -(A Sx + B Sy), dL/dv = -(B Sx + C Sy), dL/dA = -Sxx/2, dL/dB = -Sxy, dL/dC = -Syy/2, dL/do = S1 / o.
 // The colour behind the current splat enters only through its dot product with dL/dpixel, so one scalar s is carried:
 //     dL/dalpha_k = T_k (g.c_k) - s_k / (1 - alpha_k),   s_{k-1} = s_k + (g.c_k) alpha_k T_k,   s_last = T_final (g.bg).
-template <int PX>
-__global__ void __launch_bounds__(256 / PX) blend_bwd_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
-                                                             const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
-                                                             const float* __restrict__ dL_dimage, const float* __restrict__ final_T,
-                                                             const unsigned int* __restrict__ n_contrib, float* __restrict__ g9) {
-  constexpr int BATCH = 256 / PX;
-  constexpr int ACC_STRIDE = BATCH + 1;   // odd stride: the nine lanes that hold the warp sums hit nine different banks
-  __shared__ struct { float4 s0[BATCH], s1[BATCH], s2[BATCH]; float acc[9 * ACC_STRIDE]; unsigned int id[BATCH]; int max_contrib; } sm;
-  const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const Strip<PX> sp(warp, lane);
-  const int px = tx * TILE + sp.lx;
-  const float x = sp.lx + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
-  const uint2 range = ranges[tile];
-  const size_t hw = (size_t)vp.width * vp.height;
-  float y[PX], T[PX], s[PX], gr[PX], gg[PX], gb[PX];
-  int mine[PX], wmax[PX];
-  int lane_max = 0;
-#pragma unroll
-  for (int k = 0; k < PX; ++k) {
-    const int ly = sp.ly0 + 4 * k, py = ty * TILE + ly;
-    y[k] = ly + 0.5f; T[k] = 1.f; mine[k] = 0; gr[k] = gg[k] = gb[k] = 0.f;
-    if (px < vp.width && py < vp.height) {
-      const size_t pix = (size_t)py * vp.width + px;
-      T[k] = final_T[pix]; mine[k] = (int)n_contrib[pix]; gr[k] = dL_dimage[pix]; gg[k] = dL_dimage[hw + pix]; gb[k] = dL_dimage[2 * hw + pix];
-    }
-    s[k] = T[k] * (gr[k] * vp.bg[0] + gg[k] * vp.bg[1] + gb[k] * vp.bg[2]);
-    int w = mine[k];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) w = max(w, __shfl_xor_sync(0xffffffffu, w, o));
-    wmax[k] = w; lane_max = max(lane_max, w);
-  }
-  if (threadIdx.x == 0) sm.max_contrib = 0;
-  __syncthreads();
-  if (lane == 0) atomicMax(&sm.max_contrib, lane_max);
-  __syncthreads();
-  const int total = sm.max_contrib;
-  // warp_reduce8 leaves sum k on lane 4k; the ninth sum (butterfly, on every lane) is flushed by lane 1: one atomic
-  // instruction for all nine rows, nine different banks
-  const bool flusher = (lane & 3) == 0 || lane == 1;
-  float* const acc_lane = sm.acc + (lane == 1 ? 8 : lane >> 2) * ACC_STRIDE;
-  for (int hi = total; hi > 0; hi -= BATCH) {           // batch covers list positions [lo_pos, hi)
-    const int lo_pos = max(0, hi - BATCH), m = hi - lo_pos;
-    __syncthreads();                                    // previous batch fully flushed
-    if ((int)threadIdx.x < m) {
-      const unsigned int id = vals[range.x + lo_pos + threadIdx.x];
-      sm.id[threadIdx.x] = id;
-      stage_splat(rec, id, ox, oy, &sm.s0[threadIdx.x], &sm.s1[threadIdx.x], &sm.s2[threadIdx.x]);
-    }
-#pragma unroll
-    for (int k = 0; k < 9; ++k) sm.acc[k * ACC_STRIDE + threadIdx.x] = 0.f;
-    __syncthreads();
-    if (lo_pos < lane_max) {
-     for (int jb = ((m - 1) >> 5) << 5; jb >= 0; jb -= 32) {
-      unsigned int hk[PX], any = 0;
-      float4 ta, tb;
-      if (jb + lane < m) { ta = sm.s0[jb + lane]; tb = sm.s1[jb + lane]; }
-#pragma unroll
-      for (int k = 0; k < PX; ++k) {
-        hk[k] = lo_pos + jb < wmax[k] ? __ballot_sync(0xffffffffu, jb + lane < m && lo_pos + jb + lane < wmax[k] &&
-                                                                    patch_hit(ta, tb, sp.xm, sp.ym0 + 4.f * k, cp.log2_alpha_min)) : 0u;
-        any |= hk[k];
-      }
-      while (any) {
-        const int bit = 31 - __clz(any);
-        any &= ~(1u << bit);
-        const int j = jb + bit;
-        const float4 a = sm.s0[j], b = sm.s1[j];
-        const float e1x = fmaf(a.x, x, a.w);
-        float alpha[PX], araw[PX];
-        bool act[PX], some = false;
-#pragma unroll
-        for (int k = 0; k < PX; ++k) {
-          act[k] = false; alpha[k] = 0.f; araw[k] = 0.f;
-          if (!((hk[k] >> bit) & 1u)) continue;                          // warp-uniform
-          const float e1 = fmaf(a.y, y[k], e1x);
-          const float e2 = fmaf(a.z, y[k], b.x);
-          const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
-          if ((lo_pos + j < mine[k]) && l2a >= cp.log2_alpha_min) {
-            araw[k] = ex2_approx(l2a); alpha[k] = fminf(cp.alpha_max, araw[k]); act[k] = !(alpha[k] < cp.alpha_min);
-          }
-          some = some || act[k];
-        }
-        if (!__any_sync(0xffffffffu, some)) continue;
-        float v[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, v1 = 0.f;
-        const float4 c = sm.s2[j];
-        const float dx = c.y - x;
-#pragma unroll
-        for (int k = 0; k < PX; ++k) {
-          if (!act[k]) continue;
-          const float iom = rcp_approx(1.f - alpha[k]);
-          T[k] *= iom;                                                 // T_k
-          const float wgt = alpha[k] * T[k];
-          v[5] = fmaf(wgt, gr[k], v[5]); v[6] = fmaf(wgt, gg[k], v[6]); v[7] = fmaf(wgt, gb[k], v[7]);   // dL/dc
-          const float gc = fmaf(gr[k], b.z, fmaf(gg[k], b.w, gb[k] * c.x));                               // dL/dpixel . c_k
-          const float dalpha = fmaf(T[k], gc, -s[k] * iom);
-          s[k] = fmaf(gc, wgt, s[k]);
-          if (!(araw[k] > cp.alpha_max)) {                             // alpha clamp inactive: d alpha / d power = alpha
-            const float dpow = alpha[k] * dalpha, dy = c.z - y[k];
-            const float mx = dpow * dx, my = dpow * dy;
-            v1 += dpow;
-            v[0] += mx; v[1] += my;
-            v[2] = fmaf(mx, dx, v[2]); v[3] = fmaf(mx, dy, v[3]); v[4] = fmaf(my, dy, v[4]);
-          }
-        }
-        const float red = warp_reduce8(v, lane);
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v1 += __shfl_xor_sync(0xffffffffu, v1, o);
-        if (flusher) atomicAdd(acc_lane + j, lane == 1 ? v1 : red);
-      }
-     }
-    }
-    __syncthreads();
-    if ((int)threadIdx.x < m) {
-      const int j = threadIdx.x;
-      const float Sx = sm.acc[j], Sy = sm.acc[ACC_STRIDE + j], Sxx = sm.acc[2 * ACC_STRIDE + j], Sxy = sm.acc[3 * ACC_STRIDE + j];
-      const float Syy = sm.acc[4 * ACC_STRIDE + j], S1 = sm.acc[8 * ACC_STRIDE + j];
-      const float4 a = sm.s0[j];
-      const float ik = 1.0f / 0.72134752044448170f;                    // conic (A, B, C) from its exp2-scaled factor
-      const float A = a.x * a.x * ik, B = a.x * a.y * ik, C = fmaf(a.y, a.y, a.z * a.z) * ik;
-      float out[9];
-      out[0] = -fmaf(A, Sx, B * Sy); out[1] = -fmaf(B, Sx, C * Sy);
-      out[2] = -0.5f * Sxx; out[3] = -Sxy; out[4] = -0.5f * Syy;
-      out[5] = S1 != 0.f ? S1 * exp2f(-sm.s1[j].y) : 0.f;   // o may underflow to 0 (marginal filter off): then nothing composited, S1 == 0
-      out[6] = sm.acc[5 * ACC_STRIDE + j]; out[7] = sm.acc[6 * ACC_STRIDE + j]; out[8] = sm.acc[7 * ACC_STRIDE + j];
-      float* dst = g9 + (size_t)9 * sm.id[j];
-#pragma unroll
-      for (int k = 0; k < 9; ++k) if (out[k] != 0.f) atomicAdd(dst + k, out[k]);
-    }
-  }
-}
-
-// ---------------------------------------------------------------------------------------------
-// B1, transposed accumulation (PX = 2).  Same mathematics as blend_bwd_kernel, different bookkeeping: the pixel-parallel
+// (The direct form — nine products per pixel, a 14-shuffle warp reduction and an atomic per (warp, splat) hit — and the
+// variants with PX = 1 / 4, 4 / 16 buffered hits and shared-memory accumulators were measured in round 1 and removed:
+// profiles/r1_history.md.)  The pixel-parallel
 // walk only produces the two scalars (dpow, wgt) per pixel and parks them, one float4 per lane, in a per-warp buffer of
 // HB hits.  When the buffer is full the warp turns round: 4 lanes per buffered hit each sum 16 of the strip's 64 pixels
 // into the nine moment / colour sums (coordinates and dL/dpixel of a pixel are per-iteration constants / broadcast
@@ -849,95 +691,54 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
   }
 }
 
-// FDGS_BLEND_NO_DEF: A/B runs of the generic instantiations at the default thresholds.
-static bool no_def() { static const bool v = getenv("FDGS_BLEND_NO_DEF") != nullptr; return v; }
-
-// Pixels per lane of the two blend kernels.  2 is the measured optimum on cfg3; FDGS_BLEND_PX
-// overrides it for experiments (1, 2 or 4).
-static int blend_px() {
-  static int px = 0;
-  if (!px) { const char* e = getenv("FDGS_BLEND_PX"); px = e ? atoi(e) : 2; if (px != 1 && px != 2 && px != 4) px = 2; }
-  return px;
-}
-
-void launch_blend_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
+void launch_blend_fwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
                       unsigned int* n_contrib, float* depth_map, cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
-  if (depth_map) {
-    if (cp.default_thresholds && !no_def()) blend_fwd_kernel<2, false, true, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr, depth_map);
-    else blend_fwd_kernel<2, false, true, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr, depth_map);
-    ++g_launches;
-    return;
-  }
-#define FDGS_FWD(PXV, DEFV) blend_fwd_kernel<PXV, false, false, DEFV><<<tiles, 256 / PXV, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, image, final_T, n_contrib, nullptr, nullptr)
-  switch (blend_px()) {
-    case 1: FDGS_FWD(1, false); break;
-    case 4: FDGS_FWD(4, false); break;
-    default: if (cp.default_thresholds && !no_def()) FDGS_FWD(2, true); else FDGS_FWD(2, false);
-  }
+#define FDGS_FWD(AUXV, DEFV) blend_fwd_kernel<2, false, AUXV, DEFV><<<tiles, 128, 0, st>>>(ws.ranges, ws.pair_ids, ws.rec, vp, cp, image, final_T, n_contrib, nullptr, depth_map)
+  if (depth_map) { if (cp.default_thresholds) FDGS_FWD(true, true); else FDGS_FWD(true, false); }
+  else           { if (cp.default_thresholds) FDGS_FWD(false, true); else FDGS_FWD(false, false); }
 #undef FDGS_FWD
-  ++g_launches;
+  count_launch();
 }
 
-void launch_blend_stats(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, unsigned long long* stats, cudaStream_t st) {
-  blend_fwd_kernel<1, true, false, false><<<vp.tiles_x * vp.tiles_y, 256, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, nullptr, nullptr, nullptr, stats, nullptr);
-  ++g_launches;
+void launch_blend_stats(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, unsigned long long* stats, cudaStream_t st) {
+  blend_fwd_kernel<1, true, false, false><<<vp.tiles_x * vp.tiles_y, 256, 0, st>>>(ws.ranges, ws.pair_ids, ws.rec, vp, cp, nullptr, nullptr, nullptr, stats, nullptr);
+  count_launch();
 }
 
-void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* dL_dimage,
+void launch_blend_bwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, const float* dL_dimage,
                       const float* final_T, const unsigned int* n_contrib, const float* dL_ddepth, const float* dL_dopacity,
                       cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
-  if (dL_ddepth || dL_dopacity) {
-    if (cp.default_thresholds && !no_def())
-      blend_bwd2_kernel<8, 6, true, true, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9,
-                                                                       dL_ddepth, dL_dopacity, ws.gz);
-    else
-      blend_bwd2_kernel<8, 6, true, true, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9,
-                                                                        dL_ddepth, dL_dopacity, ws.gz);
-    ++g_launches;
-    return;
-  }
-#define FDGS_BWD(PXV) blend_bwd_kernel<PXV><<<tiles, 256 / PXV, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9)
-  static const bool direct = getenv("FDGS_BLEND_DIRECT") != nullptr;   // experiments: the shuffle-reduction kernel at PX = 2
-  switch (blend_px()) {
-    case 1: FDGS_BWD(1); break;
-    case 4: FDGS_BWD(4); break;
-    default:
-      if (direct) FDGS_BWD(2);
-      else if (getenv("FDGS_BWD2_SHARED_ACC"))    // A/B runs: per-splat sums combined across the warps in shared memory first
-        blend_bwd2_kernel<8, 6, false, false, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9, nullptr, nullptr, nullptr);
-      else if (cp.default_thresholds && !no_def())
-        blend_bwd2_kernel<8, 7, false, true, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9, nullptr, nullptr, nullptr);
-      else blend_bwd2_kernel<8, 7, false, true, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9, nullptr, nullptr, nullptr);
-  }
+#define FDGS_BWD(MINB, AUXV, DEFV) blend_bwd2_kernel<8, MINB, AUXV, true, DEFV><<<tiles, 128, 0, st>>>(ws.ranges, ws.pair_ids, ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9, dL_ddepth, dL_dopacity, ws.gz)
+  if (dL_ddepth || dL_dopacity) { if (cp.default_thresholds) FDGS_BWD(6, true, true); else FDGS_BWD(6, true, false); }
+  else                          { if (cp.default_thresholds) FDGS_BWD(7, false, true); else FDGS_BWD(7, false, false); }
 #undef FDGS_BWD
-  ++g_launches;
+  count_launch();
 }
 
-void launch_blend_feat_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* dL_dout, int C,
+void launch_blend_feat_bwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, const float* dL_dout, int C,
                            float* grad_feat, cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
   for (int c0 = 0; c0 < C; c0 += 32) {
-    if (cp.default_thresholds && !no_def()) blend_feat_bwd_kernel<true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dout, C, c0, grad_feat);
-    else blend_feat_bwd_kernel<false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, dL_dout, C, c0, grad_feat);
-    ++g_launches;
+    if (cp.default_thresholds) blend_feat_bwd_kernel<true><<<tiles, 128, 0, st>>>(ws.ranges, ws.pair_ids, ws.rec, vp, cp, dL_dout, C, c0, grad_feat);
+    else blend_feat_bwd_kernel<false><<<tiles, 128, 0, st>>>(ws.ranges, ws.pair_ids, ws.rec, vp, cp, dL_dout, C, c0, grad_feat);
+    count_launch();
   }
 }
 
-void launch_blend_feat_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* feat, int C,
+void launch_blend_feat_fwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, const float* feat, int C,
                            float* out, cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
   for (int c0 = 0; c0 < C;) {                    // 16 channels per pass, a tail of <= 4 in a 4-channel pass
-    static const bool no32 = getenv("FDGS_FEAT_NO32") != nullptr;     // A/B runs: two 16-channel passes instead of one of 32
-    const bool def = cp.default_thresholds && !no_def();
-#define FDGS_FEAT(CHV) do { if (def) blend_feat_fwd_kernel<CHV, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, feat, C, c0, out); \
-                            else blend_feat_fwd_kernel<CHV, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.l2_vals[l2_buf], ws.rec, vp, cp, feat, C, c0, out); c0 += CHV; } while (0)
-    if (C - c0 >= 32 && !no32) FDGS_FEAT(32);
+    const bool def = cp.default_thresholds;
+#define FDGS_FEAT(CHV) do { if (def) blend_feat_fwd_kernel<CHV, true><<<tiles, 128, 0, st>>>(ws.ranges, ws.pair_ids, ws.rec, vp, cp, feat, C, c0, out); \
+                            else blend_feat_fwd_kernel<CHV, false><<<tiles, 128, 0, st>>>(ws.ranges, ws.pair_ids, ws.rec, vp, cp, feat, C, c0, out); c0 += CHV; } while (0)
+    if (C - c0 >= 32) FDGS_FEAT(32);
     else if (C - c0 > 4) FDGS_FEAT(16);
     else FDGS_FEAT(4);
 #undef FDGS_FEAT
-    ++g_launches;
+    count_launch();
   }
 }
 

@@ -48,14 +48,16 @@ struct CfgParams {
 #define FDGS_DEF_T_MIN 1e-4f
 #define FDGS_DEF_L2MIN (-0x1.ffa3ap+2f)   // log2f(1/255) * (1 + 1e-6) - 1e-6 in fp32 (= -7.994362)
 
-// Device-side header at the start of the workspace (zeroed by fdgs_preprocess).
+// Device-side header at the start of the workspace (zeroed by fdgs_preprocess; the layout mirror is then written by the
+// preprocess kernel's first thread).
 struct WsHeader {
-  unsigned int num_pairs;         // D (written by the tile-grid kernel)
+  unsigned int num_pairs;         // D (written by the tile-grid role of the compaction kernel); 0 if D > pair_capacity
   unsigned int num_visible;       // survivors of all culls (written by the compaction scan)
   unsigned int overflow;          // 1 if D > pair_capacity
   unsigned int scan_ticket[2];    // dynamic tile ids of the two chained scans
-  unsigned int sort_ticket[8];    // one per radix pass (4 depth passes + up to 4 tile-id passes)
-  unsigned int pad[3];
+  unsigned int sort_ticket[4];    // one per radix pass of the depth sort
+  unsigned int total_pairs;       // D even when it overflows
+  unsigned int pad[6];
   long long N, K, W, H, pair_capacity, tiles;   // layout mirror for fdgs_debug_export
 };
 
@@ -63,23 +65,28 @@ constexpr int RADIX_BITS = 8;
 constexpr int RADIX = 1 << RADIX_BITS;
 constexpr int SORT_THREADS = 256;
 constexpr int SORT_ITEMS_L1 = 4;    // depth sort of <= N survivors: small tiles, more CTAs
-constexpr int SORT_ITEMS_L2 = 16;   // tile-id sort of D pairs
+constexpr int DEPTH_PASSES = 32 / RADIX_BITS;
 constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_ITEMS = 8;
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
-constexpr int DUP_CHUNK = 2048;         // output pairs per CTA of the pair emission
-constexpr int MAX_GRID_CELLS = 50000;   // (tiles_x+1)*(tiles_y+1) must fit the tile-grid kernel's shared memory
+constexpr int MIN_PAIR_CHUNK = 16384;   // pairs per chunk of the ordered pair scatter (scan_dup.cu), at least
+constexpr int MAX_PAIR_CHUNKS = 1024;   // chunks the pair capacity is divided into, at most
+constexpr int MAX_GRID_CELLS = 50000;   // (tiles_x+1)*(tiles_y+1) must fit the shared memory of the tile-grid / scatter kernels
 
 // Host-side view of the carved-up workspace.
 //
-// Sorting is two-level: survivors are first sorted by their fp32 depth bits
-// (level 1, <= N items); pairs (tile, id) are then emitted in that order and stably sorted by tile id
-// (level 2, D items, ceil(log2 tiles) bits).  The resulting per-tile lists are exactly those of one
-// stable sort on the 64-bit key tile<<32 | depth-bits with ties in id order.
+// Binning is two-level: survivors are first sorted by their fp32 depth bits (level 1, <= N items,
+// hand-written onesweep radix sort); the (tile, id) pairs are then written in that order straight to their final
+// position in the per-tile lists by a stable, rectangle-aware scatter (level 2: chunk coverage grids -> chunk bases ->
+// ordered scatter; no key array exists).  The resulting per-tile lists are exactly those of one stable sort on the
+// 64-bit key tile<<32 | depth-bits with ties in id order.
 struct Workspace {
   WsHeader* hdr;
   int* tile_diff;                    // [(tiles_y+1)*(tiles_x+1)] 2D difference array of tile coverage
   unsigned long long* scan_state[2]; // look-back words of the two scans
+  unsigned int* sort_hist;           // [4][RADIX] digit counts of the 4 depth passes (raw, accumulated by the compaction kernel)
+  unsigned int* sort_lookback;       // [4][depth-sort tiles][RADIX]: one region per pass, cleared with the header
+  size_t lookback_stride;            // words per pass
   SplatRec* rec;                     // [N] indexed by primitive id
   ushort4* rect;                     // [N] tx0, ty0, tx1, ty1
   unsigned int* tiles_touched;       // [N]
@@ -87,17 +94,16 @@ struct Workspace {
   unsigned int* l1_vals[2];          // [N] primitive ids of survivors; after the sort: depth order
   unsigned int* vis_ids;             // [N] primitive ids of survivors in ascending id order (kept for the backward)
   unsigned int* offsets;             // [N] exclusive prefix sum of tiles_touched in depth order
-  unsigned int* chunk_first;         // [cap / DUP_CHUNK + 2] survivor (depth order) that owns output position k * DUP_CHUNK
-  unsigned int* l2_keys[2];          // [cap] tile ids
-  unsigned int* l2_vals[2];          // [cap] primitive ids
-  unsigned int* sort_hist;           // [8][RADIX] digit counts of the 4 depth passes (raw) and exclusive bases of the tile-id passes
-  unsigned int* sort_lookback;       // [max sort tiles][RADIX]
+  unsigned int chunk_pairs, num_chunks;  // pairs per scatter chunk; chunks the capacity is divided into
+  unsigned int* chunk_first;         // [num_chunks + 1] first survivor (depth order) whose pairs START in chunk q
+  unsigned int* chunk_base;          // [num_chunks][tiles] coverage of chunk q per tile -> first output position of chunk q in tile
+  unsigned int* pair_ids;            // [cap] primitive ids of the per-tile lists, tile after tile (ranges), depth order inside
   uint2* ranges;                     // [tiles] [first, last+1)
   float* g9;                         // [N,9] per-splat gradients of the blend backward
   float4* aux;                       // [N] survivors: view direction (x, y, z) and (t - mu_t) / T, written by preprocess
   float4* dcol;                      // [N] survivors: colour backward -> geometry backward: dL/d dir (x, y, z), dL/d Delta
   float* gz;                         // [N] auxiliary depth channel: dL/d(camera depth) per splat
-  size_t lookback_bytes, zero_bytes; // zero_bytes: prefix of the workspace cleared by fdgs_preprocess
+  size_t zero_bytes;                 // prefix of the workspace cleared by fdgs_preprocess
   size_t bytes;
 };
 
@@ -113,7 +119,10 @@ inline Workspace carve(void* base, long long N, long long K, long long W, long l
   w.hdr = (WsHeader*)take(sizeof(WsHeader));
   w.tile_diff = (int*)take(4 * (size_t)(tx + 1) * (ty + 1));
   for (int i = 0; i < 2; ++i) w.scan_state[i] = (unsigned long long*)take(8 * (Np / 256 + 2));   // chained-scan tiles of >= 256 items
-  w.sort_hist = (unsigned int*)take(4 * 8 * RADIX);     // level-1 digit counts are accumulated by the compaction kernel
+  w.sort_hist = (unsigned int*)take(4 * DEPTH_PASSES * RADIX);     // accumulated by the compaction kernel
+  const long long t1 = (Np + SORT_THREADS * SORT_ITEMS_L1 - 1) / (SORT_THREADS * SORT_ITEMS_L1);
+  w.lookback_stride = (size_t)RADIX * (size_t)(t1 + 1);
+  w.sort_lookback = (unsigned int*)take(4 * w.lookback_stride * DEPTH_PASSES);
   w.zero_bytes = off;
   w.rec = (SplatRec*)take(sizeof(SplatRec) * Np);
   w.rect = (ushort4*)take(sizeof(ushort4) * Np);
@@ -122,13 +131,13 @@ inline Workspace carve(void* base, long long N, long long K, long long W, long l
   for (int i = 0; i < 2; ++i) w.l1_vals[i] = (unsigned int*)take(4 * Np);
   w.vis_ids = (unsigned int*)take(4 * Np);
   w.offsets = (unsigned int*)take(4 * Np);
-  w.chunk_first = (unsigned int*)take(4 * ((size_t)cap / DUP_CHUNK + 2));
-  for (int i = 0; i < 2; ++i) w.l2_keys[i] = (unsigned int*)take(4 * (size_t)cap);
-  for (int i = 0; i < 2; ++i) w.l2_vals[i] = (unsigned int*)take(4 * (size_t)cap);
-  const long long t1 = (Np + SORT_THREADS * SORT_ITEMS_L1 - 1) / (SORT_THREADS * SORT_ITEMS_L1);
-  const long long t2 = (cap + SORT_THREADS * SORT_ITEMS_L2 - 1) / (SORT_THREADS * SORT_ITEMS_L2);
-  w.lookback_bytes = 4 * (size_t)RADIX * ((t1 > t2 ? t1 : t2) + 1);
-  w.sort_lookback = (unsigned int*)take(w.lookback_bytes);
+  long long cp = (cap + MAX_PAIR_CHUNKS - 1) / MAX_PAIR_CHUNKS;
+  if (cp < MIN_PAIR_CHUNK) cp = MIN_PAIR_CHUNK;
+  w.chunk_pairs = (unsigned int)cp;
+  w.num_chunks = (unsigned int)(cap / cp + 1);
+  w.chunk_first = (unsigned int*)take(4 * ((size_t)w.num_chunks + 2));
+  w.chunk_base = (unsigned int*)take(4 * (size_t)w.num_chunks * (size_t)tiles);
+  w.pair_ids = (unsigned int*)take(4 * (size_t)cap);
   w.ranges = (uint2*)take(sizeof(uint2) * tiles);
   w.g9 = (float*)take(4 * 9 * Np);
   w.aux = (float4*)take(16 * Np);
@@ -149,43 +158,44 @@ __device__ __forceinline__ void prefetch_l2(const void* p, const int bytes) {
 }
 #endif
 
-// Launch counter (fdgs_launch_count) — bumped by every launcher.
-extern long long g_launches;
+// Launch counter (fdgs_launch_count) — bumped by every launcher (atomic: launchers may run on several host threads).
+void count_launch(int n = 1);
+long long launch_count_value();
 // Records the CUDA error text for fdgs_strerror and returns FDGS_ERR_CUDA (api.cu).
 int cuda_fail(cudaError_t e, const char* where);
 
 // Launchers (each file implements its own; all asynchronous on `st`).
 void launch_preprocess_fwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, cudaStream_t st);
-// compaction scan: survivors (tiles_touched > 0) in id order -> l1_keys[0] (depth bits), l1_vals[0] (ids), hdr->num_visible
-void launch_compact(const Workspace& ws, int N, cudaStream_t st);
-// Stable LSD radix sort of (key, val) u32 pairs on key bits [0, bits); the count is read on the device.
-// ws.sort_hist[ticket_base + pass] holds the digit counts of the pass (bases_exclusive = false: every CTA scans them
-// itself) or their exclusive prefix (true).  Returns the result buffer (0/1).
-int launch_sort_pairs(const Workspace& ws, unsigned int* const keys[2], unsigned int* const vals[2],
-                      const unsigned int* count_dev, long long max_count, int bits, int items_per_thread, int ticket_base,
-                      bool bases_exclusive, int num_sms, cudaStream_t st);
-// 2D prefix of the coverage difference array -> ranges, D, overflow flag, level-2 digit bases
-void launch_tile_grid(const Workspace& ws, const ViewParams& vp, long long cap, int l2_passes, cudaStream_t st);
-// exclusive prefix sum of tiles_touched in depth order -> offsets
+// compaction scan: survivors (tiles_touched > 0) in id order -> l1_keys[0] (depth bits), l1_vals[0] (ids), hdr->num_visible;
+// the same launch carries, as the role of its first CTA, the 2D prefix of the coverage difference array -> ranges, D, overflow
+void launch_compact_and_tile_grid(const Workspace& ws, int N, int K, const ViewParams& vp, long long cap, cudaStream_t st);
+// Stable LSD radix sort of the survivors' (depth bits, id) pairs on all 32 key bits; the count is read on the device and
+// ws.sort_hist[pass] holds the digit counts of the pass.  Returns the result buffer (0/1).
+int launch_sort_depth(const Workspace& ws, long long max_count, int num_sms, cudaStream_t st);
+// exclusive prefix sum of tiles_touched in depth order -> offsets, chunk_first
 void launch_offsets(const Workspace& ws, int l1_buf, int N, cudaStream_t st);
-void launch_duplicate(const Workspace& ws, int l1_buf, int N, long long cap, const ViewParams& vp, cudaStream_t st);
-void launch_blend_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
+// level 2: per-tile lists in depth order written straight to their final place (three launches: chunk coverage, chunk
+// bases, ordered scatter)
+void launch_pair_scatter(const Workspace& ws, int l1_buf, int N, const ViewParams& vp, int num_sms, cudaStream_t st);
+void launch_blend_fwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
                       unsigned int* n_contrib, float* depth_map /*NULL = no auxiliary channel*/, cudaStream_t st);
-void launch_blend_stats(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, unsigned long long* stats, cudaStream_t st);
-void launch_blend_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* dL_dimage,
+void launch_blend_stats(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, unsigned long long* stats, cudaStream_t st);
+void launch_blend_bwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, const float* dL_dimage,
                       const float* final_T, const unsigned int* n_contrib, const float* dL_ddepth, const float* dL_dopacity,
                       cudaStream_t st);
 void launch_preprocess_bwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, int l1_buf,
                            const fdgs_grads& g, bool with_gz, cudaStream_t st);
 void launch_cull_status(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, unsigned char* dst, cudaStream_t st);
-void launch_blend_feat_fwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* feat, int C,
+void launch_blend_feat_fwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, const float* feat, int C,
                            float* out, cudaStream_t st);
-void launch_blend_feat_bwd(const Workspace& ws, int l2_buf, const ViewParams& vp, const CfgParams& cp, const float* dL_dout, int C,
+void launch_blend_feat_bwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, const float* dL_dout, int C,
                            float* grad_feat, cudaStream_t st);
 void launch_feature_records(const Workspace& ws, const float* feat, int C, int c0, int N, SplatRec* dst, cudaStream_t st);
 void launch_extract_feature_grads(const Workspace& ws, float* grad_feat, int C, int c0, int N, cudaStream_t st);
 void launch_splat_flow(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, float dt_next, float* flow,
                        cudaStream_t st);
-void launch_l1_loss(const float* image, const float* target, long long count, float* dL, float* loss, cudaStream_t st);
+// overflow_flag (NULL ok): device word; if non-zero the loss written is NaN (fdgs_step_batch / fdgs_step_host)
+void launch_l1_loss(const float* image, const float* target, long long count, float* dL, float* loss, const unsigned int* overflow_flag,
+                    cudaStream_t st);
 
 }  // namespace fdgs

@@ -69,16 +69,16 @@ __global__ void __launch_bounds__(128) splat_flow_kernel(const fdgs_scene sc, co
 
 void launch_feature_records(const Workspace& ws, const float* feat, int C, int c0, int N, SplatRec* dst, cudaStream_t st) {
   feature_records_kernel<<<(N + 255) / 256, 256, 0, st>>>(ws.rec, ws.tiles_touched, feat, C, c0, N, dst);
-  ++g_launches;
+  count_launch();
 }
 void launch_extract_feature_grads(const Workspace& ws, float* grad_feat, int C, int c0, int N, cudaStream_t st) {
   extract_feature_grads_kernel<<<(N + 255) / 256, 256, 0, st>>>(ws.g9, ws.tiles_touched, grad_feat, C, c0, N);
-  ++g_launches;
+  count_launch();
 }
 void launch_splat_flow(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, float dt_next, float* flow,
                        cudaStream_t st) {
   splat_flow_kernel<<<(sc.N + 127) / 128, 128, 0, st>>>(sc, vp, cp, dt_next, ws.tiles_touched, reinterpret_cast<float2*>(flow));
-  ++g_launches;
+  count_launch();
 }
 
 }  // namespace fdgs

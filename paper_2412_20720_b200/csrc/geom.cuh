@@ -42,10 +42,20 @@ __device__ __forceinline__ void quat_right(const float q[4], float R[4][4]) {
   R[3][0] = s;  R[3][1] = r;   R[3][2] = -qq; R[3][3] = p;
 }
 
-// Runs A1-A3 up to Sigma_2d.  Returns the status; fields are valid up to the point of the cull.
-__device__ __forceinline__ int geom_forward(const float4 mean, const float4 ls, const float4 ql_raw, const float4 qr_raw,
-                                            const float logit, const ViewParams& vp, const CfgParams& cp, Geom& g,
-                                            const void* prefetch = nullptr, const int prefetch_bytes = 0) {
+// A1 + the temporal half of A2: activations, the TIME row of R = L(q_l) R(q_r) (eq. 8), Sigma_44, the marginal weight
+// (eq. 10) and the p(t) < marginal_min filter (L324).  Returns G_VISIBLE if the primitive is alive at t; fills g.s, g.ql,
+// g.qr, g.inv_nl/nr, row 3 of g.R4 / g.M, g.b, g.dt, g.w and the fp64 factors (Ld, Rd) that geom_space continues from.
+// The forward preprocess calls it alone first (one thread per primitive, three primitives out of four stop here at cfg3).
+struct GeomQ { double Ld[4][4], Rd[4][4]; };
+
+#define FDGS_R_ROW(i)                                                                                                         \
+  _Pragma("unroll") for (int k = 0; k < 4; ++k) {                                                                             \
+    const double acc = fma(q.Ld[i][0], q.Rd[0][k], fma(q.Ld[i][1], q.Rd[1][k], fma(q.Ld[i][2], q.Rd[2][k], q.Ld[i][3] * q.Rd[3][k])));      \
+    g.R4[i][k] = (float)acc; g.M[i][k] = (float)acc * g.s[k];                                                                 \
+  }
+
+__device__ __forceinline__ int geom_time(const float4 mean, const float4 ls, const float4 ql_raw, const float4 qr_raw,
+                                         const float logit, const ViewParams& vp, const CfgParams& cp, Geom& g, GeomQ& q) {
   const float qlr[4] = {ql_raw.x, ql_raw.y, ql_raw.z, ql_raw.w}, qrr[4] = {qr_raw.x, qr_raw.y, qr_raw.z, qr_raw.w};
   const float lsv[4] = {ls.x, ls.y, ls.z, ls.w};
   float nl2 = 0.f, nr2 = 0.f;
@@ -77,11 +87,10 @@ __device__ __forceinline__ int geom_forward(const float4 mean, const float4 ls, 
                            {qld[2], qld[3], qld[0], -qld[1]}, {qld[3], -qld[2], qld[1], qld[0]}};
   const double Rd[4][4] = {{qrd[0], -qrd[1], -qrd[2], -qrd[3]}, {qrd[1], qrd[0], qrd[3], -qrd[2]},
                            {qrd[2], -qrd[3], qrd[0], qrd[1]}, {qrd[3], qrd[2], -qrd[1], qrd[0]}};
-#define FDGS_R_ROW(i)                                                                                                         \
-  _Pragma("unroll") for (int k = 0; k < 4; ++k) {                                                                             \
-    const double acc = fma(Ld[i][0], Rd[0][k], fma(Ld[i][1], Rd[1][k], fma(Ld[i][2], Rd[2][k], Ld[i][3] * Rd[3][k])));      \
-    g.R4[i][k] = (float)acc; g.M[i][k] = (float)acc * g.s[k];                                                                 \
-  }
+#pragma unroll
+  for (int r = 0; r < 4; ++r)
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { q.Ld[r][k] = Ld[r][k]; q.Rd[r][k] = Rd[r][k]; }
   FDGS_R_ROW(3)
   // eq. 10: marginal weight, and the p(t) < marginal_min filter (L324)
   g.b = g.M[3][0] * g.M[3][0] + g.M[3][1] * g.M[3][1] + g.M[3][2] * g.M[3][2] + g.M[3][3] * g.M[3][3];
@@ -89,10 +98,14 @@ __device__ __forceinline__ int geom_forward(const float4 mean, const float4 ls, 
   g.w = expf(-0.5f * g.dt * g.dt / g.b);
   if (!isfinite(g.w) || !(g.b > 0.f) || !isfinite(g.b)) return G_CULL_NONFINITE;
   if (g.w < cp.marginal_min) return G_CULL_TIME;
-  // the primitive is alive at t: start fetching what only survivors read (its colour block) under the arithmetic below
-  if (prefetch) prefetch_l2(prefetch, prefetch_bytes);
+  return G_VISIBLE;
+}
+
+// The rest of A2 and A3 for a primitive that geom_time found alive: the other three rows of R, the slice in factor form,
+// camera transform, near cull, pinhole projection, Jacobian, Sigma_2d.  Returns the status.
+__device__ __forceinline__ int geom_space(const float4 mean, const float logit, const ViewParams& vp, const CfgParams& cp, Geom& g,
+                                          const GeomQ& q) {
   FDGS_R_ROW(0) FDGS_R_ROW(1) FDGS_R_ROW(2)
-#undef FDGS_R_ROW
   // eq. 9 in factor form
   const float inv_b = 1.0f / g.b;
   const float mu3[3] = {mean.x, mean.y, mean.z};
@@ -145,6 +158,19 @@ __device__ __forceinline__ int geom_forward(const float4 mean, const float4 ls, 
   g.sig = 1.0f / (1.0f + expf(-logit));
   g.sig_neg = 1.0f / (1.0f + expf(logit));
   return G_VISIBLE;
+}
+#undef FDGS_R_ROW
+
+// Runs A1-A3 up to Sigma_2d.  Returns the status; fields are valid up to the point of the cull.
+__device__ __forceinline__ int geom_forward(const float4 mean, const float4 ls, const float4 ql_raw, const float4 qr_raw,
+                                            const float logit, const ViewParams& vp, const CfgParams& cp, Geom& g,
+                                            const void* prefetch = nullptr, const int prefetch_bytes = 0) {
+  GeomQ q;
+  const int st = geom_time(mean, ls, ql_raw, qr_raw, logit, vp, cp, g, q);
+  if (st != G_VISIBLE) return st;
+  // the primitive is alive at t: start fetching what only survivors read (its colour block) under the arithmetic below
+  if (prefetch) prefetch_l2(prefetch, prefetch_bytes);
+  return geom_space(mean, logit, vp, cp, g, q);
 }
 
 // ---- real SH (degree <= 3), orthonormal, Condon-Shortley phase kept (S5) ----

@@ -4,8 +4,6 @@
 // Nothing but the 9 per-splat gradients of the blend backward, the view direction / time offset kept by the forward
 // preprocess (ws.aux) and the hand-over vector ws.dcol is read from the workspace; gradients are accumulated (+=)
 // into the caller's arrays.
-#include <cstdlib>
-
 #include "geom.cuh"
 
 namespace fdgs {
@@ -434,12 +432,11 @@ void launch_preprocess_bwd(const fdgs_scene& sc, const ViewParams& vp, const Cfg
     const int threads = 32 * CB_WARPS, blocks = (sc.N + threads - 1) / threads;
 #define FDGS_LAUNCH(KDV) colour_bwd_kernel<KDV><<<blocks, threads, 0, st>>>(sc.sh, sc.n_time, vp.inv_T, ws.vis_ids, ws.hdr, ws.g9, ws.rec, ws.aux, gr.sh, ws.dcol)
     if (KD == 1) FDGS_LAUNCH(1); else if (KD == 4) FDGS_LAUNCH(4); else if (KD == 9) FDGS_LAUNCH(9);
-    else if (getenv("FDGS_COLOUR_BWD_TABLE")) FDGS_LAUNCH(16);      // A/B runs: the generic table kernel at degree 3
     else colour_bwd16_kernel<<<blocks, threads, 0, st>>>(sc.sh, sc.n_time, vp.inv_T, ws.vis_ids, ws.hdr, ws.g9, ws.rec, ws.aux, gr.sh, ws.dcol);
 #undef FDGS_LAUNCH
   }
   geom_bwd_kernel<<<(sc.N + 127) / 128, 128, 0, st>>>(sc, vp, cp, ws.vis_ids, ws.hdr, ws.g9, ws.dcol, with_gz ? ws.gz : nullptr, gr);
-  g_launches += 2;
+  count_launch(2);
 }
 
 }  // namespace fdgs

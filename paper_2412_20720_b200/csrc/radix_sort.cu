@@ -4,8 +4,8 @@
 // decoupled look-back, and scatters straight to the final position of the pass — keys and values are read
 // once and written once per pass.  Tiles take dynamic ids from a ticket, CTAs are persistent, and the number
 // of pairs is read from device memory, so the host never synchronises.  The global digit counts come from the producer
-// of the keys (compaction kernel for the depth sort, tile-grid kernel for the tile-id sort): the keys are never read
-// just to be counted.
+// of the keys (the compaction kernel): the keys are never read just to be counted.  Since round 2 only the depth sort of
+// the survivors (level 1) is a radix sort; the (tile, id) pairs are placed by the ordered scatter of scan_dup.cu.
 #include "common.cuh"
 
 namespace fdgs {
@@ -152,28 +152,17 @@ __global__ void __launch_bounds__(SORT_THREADS, 3) onesweep_kernel(const unsigne
   }
 }
 
-int launch_sort_pairs(const Workspace& ws, unsigned int* const keys[2], unsigned int* const vals[2],
-                      const unsigned int* count_dev, long long max_count, int bits, int items_per_thread, int ticket_base,
-                      bool bases_exclusive, int num_sms, cudaStream_t st) {
-  const int passes = (bits + RADIX_BITS - 1) / RADIX_BITS;
-  if (passes <= 0 || max_count <= 0) return 0;
-  const unsigned int* hist = ws.sort_hist + (size_t)ticket_base * RADIX;
-  const int tile_n = SORT_THREADS * items_per_thread;
+int launch_sort_depth(const Workspace& ws, long long max_count, int num_sms, cudaStream_t st) {
+  if (max_count <= 0) return 0;
+  const int tile_n = SORT_THREADS * SORT_ITEMS_L1;
   const long long tiles = (max_count + tile_n - 1) / tile_n;
-  const size_t lb_bytes = sizeof(unsigned int) * RADIX * (size_t)tiles;
+  const int grid = (int)(tiles < 4LL * num_sms ? tiles : 4LL * num_sms);
   int cur = 0;
-  for (int p = 0; p < passes; ++p) {
-    cudaMemsetAsync(ws.sort_lookback, 0, lb_bytes, st);
-    const int grid = (int)(tiles < 4LL * num_sms ? tiles : 4LL * num_sms);
-    if (items_per_thread == SORT_ITEMS_L1)
-      onesweep_kernel<SORT_ITEMS_L1><<<grid, SORT_THREADS, 0, st>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], count_dev,
-                                                                   &ws.hdr->sort_ticket[ticket_base + p], hist + p * RADIX,
-                                                                   bases_exclusive, ws.sort_lookback, p * RADIX_BITS);
-    else
-      onesweep_kernel<SORT_ITEMS_L2><<<grid, SORT_THREADS, 0, st>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], count_dev,
-                                                                   &ws.hdr->sort_ticket[ticket_base + p], hist + p * RADIX,
-                                                                   bases_exclusive, ws.sort_lookback, p * RADIX_BITS);
-    ++g_launches;
+  for (int p = 0; p < DEPTH_PASSES; ++p) {      // the look-back region of every pass was cleared with the header (fdgs_preprocess)
+    onesweep_kernel<SORT_ITEMS_L1><<<grid, SORT_THREADS, 0, st>>>(ws.l1_keys[cur], ws.l1_vals[cur], ws.l1_keys[cur ^ 1], ws.l1_vals[cur ^ 1],
+                                                                 &ws.hdr->num_visible, &ws.hdr->sort_ticket[p], ws.sort_hist + p * RADIX, false,
+                                                                 ws.sort_lookback + (size_t)p * ws.lookback_stride, p * RADIX_BITS);
+    count_launch();
     cur ^= 1;
   }
   return cur;

@@ -265,7 +265,7 @@ int fdgs_mask_apply(const float* mask_logit, float mask_eps, const float* opacit
   if (N < 0 || (N > 0 && (!mask_logit || !opacity_logit || !out))) return FDGS_ERR_INVALID;
   if (N == 0) return FDGS_OK;
   mask_apply_kernel<<<(N + 255) / 256, 256, 0, (cudaStream_t)stream>>>(mask_logit, mask_eps, opacity_logit, out, N);
-  ++g_launches;
+  count_launch();
   TRAIN_CUDA(cudaGetLastError(), "mask apply launch");
   return FDGS_OK;
 }
@@ -279,7 +279,7 @@ int fdgs_regularizers(const fdgs_scene* sc, const float* mask_logit, const fdgs_
     return FDGS_ERR_INVALID;
   if (mask_logit && (!grad_mask_logit || !sc->opacity_logit || !g->opacity_logit)) return FDGS_ERR_INVALID;
   regularizers_kernel<<<(sc->N + 255) / 256, 256, 0, (cudaStream_t)stream>>>(*sc, mask_logit, *rc, *g, grad_mask_logit, losses_dev);
-  ++g_launches;
+  count_launch();
   TRAIN_CUDA(cudaGetLastError(), "regularizers launch");
   return FDGS_OK;
 }
@@ -297,7 +297,7 @@ int fdgs_adam_step(float* param, float* grad, float* exp_avg, float* exp_avg_sq,
   const long long nvec = count >> 2;
   const long long blocks = nvec > 0 ? (nvec + 511) / 512 : 1;
   adam_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(param, grad, exp_avg, exp_avg_sq, count, a, zero_grad);
-  ++g_launches;
+  count_launch();
   TRAIN_CUDA(cudaGetLastError(), "adam launch");
   return FDGS_OK;
 }
@@ -320,10 +320,10 @@ int fdgs_decode_compact(const fdgs_compact_scene* c, const fdgs_scene* out, void
   cudaStream_t st = (cudaStream_t)stream;
   decode_geom_kernel<<<(c->N + 255) / 256, 256, 0, st>>>(*c, (float4*)out->mean, (float4*)out->log_scale, (float4*)out->quat_l,
                                                         (float4*)out->quat_r, (float*)out->opacity_logit);
-  ++g_launches;
+  count_launch();
   const long long threads = (long long)c->N * 32;
   decode_colour_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(*c, (float*)out->sh, K);
-  ++g_launches;
+  count_launch();
   TRAIN_CUDA(cudaGetLastError(), "decode launch");
   return FDGS_OK;
 }

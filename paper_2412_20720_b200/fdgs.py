@@ -138,7 +138,7 @@ def launch_count() -> int:
     return int(load().fdgs_launch_count())
 
 
-STAGES = ("preprocess", "compact+tile_grid", "sort_depth", "offsets+duplicate", "sort_tile", "blend_fwd", "blend_bwd",
+STAGES = ("preprocess", "compact+tile_grid", "sort_depth", "offsets", "pair_scatter", "blend_fwd", "blend_bwd",
           "preprocess_bwd")
 
 

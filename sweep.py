@@ -1,6 +1,6 @@
 """Secondary measurements of BASELINE.json's configs 2, 4 and 5 (bench.py times the headline config 3).
 
-    python -m paper_2412_20720_b200.sweep [--frames 24] [--max-n 8000000] [--skip-train] [--train-terms]
+    python sweep.py [--frames 120] [--max-n 8000000] [--skip-train] [--train-terms]
 
 cfg5: forward-only render throughput over Gaussian count x resolution at evenly spaced query times: FPS (one frame at a
 time), per-stage ms (preprocess / sort incl. compaction, duplication and ranges / blend) and the fraction culled by the
@@ -11,6 +11,10 @@ from __future__ import annotations
 
 import argparse
 import json
+import os
+import sys
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
 
 import numpy as np
 
@@ -39,7 +43,7 @@ def _timed(fn, iters, warm, flush):
 
 def sweep_cfg5(frames, max_n, flush):
     import torch
-    from . import fdgs, scenes
+    from paper_2412_20720_b200 import fdgs, scenes
     for (w, h) in ((1352, 1014), (1920, 1080)):
         for n in (100_000, 500_000, 1_000_000, 2_000_000, 4_000_000, 8_000_000):
             if n > max_n:
@@ -71,7 +75,7 @@ def sweep_cfg5(frames, max_n, flush):
             print(json.dumps({"config": "cfg5_sweep", "N": n, "width": w, "height": h, "frames": len(cvs), "fps": 1e3 / ms_frame,
                               "ms_per_frame": ms_frame, "ms_min": float(np.min(ms)), "ms_max": float(np.max(ms)),
                               "stage_ms": {"preprocess": stage["preprocess"],
-                                           "sort": stage["compact+tile_grid"] + stage["sort_depth"] + stage["offsets+duplicate"] + stage["sort_tile"],
+                                           "sort": stage["compact+tile_grid"] + stage["sort_depth"] + stage["offsets"] + stage["pair_scatter"],
                                            "blend": stage["blend_fwd"]},
                               "culled_by_marginal_fraction": float(np.mean(culled)), "visible_mean": float(np.mean(nvis)),
                               "pairs_mean": float(np.mean(pairs))}), flush=True)
@@ -81,7 +85,7 @@ def sweep_cfg5(frames, max_n, flush):
 
 def train_cfg(name, scene, cap, flush):
     import torch
-    from . import fdgs, scenes
+    from paper_2412_20720_b200 import fdgs, scenes
     ds = fdgs.DeviceScene.from_scene(scene)
     v0 = scene.views[0]
     nv = len(scene.views)
@@ -110,7 +114,7 @@ def train_terms(flush, n=1_000_000):
     (DESIGN.md section 10): regularisers 176 B/primitive, Adam 28 B/element (32 with zero_grad) over the 161 floats of a
     primitive, decode 41 B read + 644 B written per primitive."""
     import torch
-    from . import fdgs, scenes, train
+    from paper_2412_20720_b200 import fdgs, scenes, train
     sc = scenes.multiview_video(N=n, n_views=1)
     ds = fdgs.DeviceScene.from_scene(sc)
     g = ds.zero_grads()
@@ -141,7 +145,7 @@ def sort_compare(flush):
     emission and a range-finding pass that are not timed here."""
     import ctypes as C
     import torch
-    from . import build, fdgs, scenes
+    from paper_2412_20720_b200 import build, fdgs, scenes
     cmp_lib = C.CDLL(build.build_compare())
     cmp_lib.fdgs_cmp_cub_sort_pairs.argtypes = [C.c_void_p] * 4 + [C.c_int64, C.c_int, C.c_void_p, C.POINTER(C.c_size_t), C.c_void_p]
     for name, sc, cap in (("cfg3_video", scenes.multiview_video(n_views=1), 1 << 24), ("cfg4_driving", scenes.driving(n_views=1), 160 << 20)):
@@ -198,7 +202,7 @@ def full_training_step(flush):
     """cfg3 step with the optimiser inside the timed region: fdgs_step_batch (4 views) + fdgs_regularizers + dense Adam over
     all six arrays (gradients cleared by the Adam pass)."""
     import torch
-    from . import fdgs, scenes, train
+    from paper_2412_20720_b200 import fdgs, scenes, train
     sc = scenes.multiview_video()
     ds = fdgs.DeviceScene.from_scene(sc)
     v0 = sc.views[0]
@@ -229,7 +233,7 @@ def feature_terms(flush, n=1_000_000, C=32):
     """Feature channels (D = 32) and optical flow at cfg3's size, view 0: ms per call next to the colour
     forward / backward of the same view."""
     import torch
-    from . import fdgs, scenes
+    from paper_2412_20720_b200 import fdgs, scenes
     sc = scenes.multiview_video(N=n, n_views=1)
     ds = fdgs.DeviceScene.from_scene(sc)
     v = sc.views[0]
@@ -265,7 +269,7 @@ def main():
     global ONCE
     ONCE = args.once
     import torch
-    from . import build, scenes
+    from paper_2412_20720_b200 import build, scenes
     if not torch.cuda.is_available():
         raise RuntimeError("sweep needs a CUDA device: the product has no CPU fallback")
     build.build()

@@ -69,6 +69,47 @@ def test_pair_overflow_is_reported_and_draws_nothing():
     assert st["overflow"] == 1 and st["num_pairs"] == 371
 
 
+def test_pair_overflow_is_loud_on_every_training_path():
+    """a scene that outgrows pair_capacity must not train on a background image with zero gradients in silence.
+    fdgs_step_host and fdgs_step_batch (with loss_host) return FDGS_ERR_PAIR_OVERFLOW after their synchronisation, the
+    asynchronous fdgs_step_batch writes NaN into the view's loss, and the autograd front end raises."""
+    import numpy as np
+    import torch
+    from paper_2412_20720_b200 import autograd, fdgs
+    sc = scenes.tiny()
+    v = sc.views[0]
+    ds = fdgs.DeviceScene.from_scene(sc)
+    cv = fdgs.make_view(v)
+    tgt = torch.from_numpy(scenes.target_image(0, 0, 64, 64)).pin_memory()
+    r = fdgs.Renderer(ds, 64, 64, 100)
+    res = torch.zeros(1).pin_memory()
+    with pytest.raises(fdgs.FdgsError) as e:
+        r.step_host(cv, tgt, res, ds.zero_grads())
+    assert e.value.code == fdgs.ERR_PAIR_OVERFLOW
+    bs = fdgs.BatchStep(ds, 64, 64, 100, 2)
+    lh = torch.zeros(2).pin_memory()
+    with pytest.raises(fdgs.FdgsError) as e:
+        bs.step([cv, cv], ds.zero_grads(), targets_host=[tgt, tgt], loss_host=lh, zero_grads=True)
+    assert e.value.code == fdgs.ERR_PAIR_OVERFLOW
+    for rr in bs.renderers:
+        rr.target_dev.copy_(tgt)
+    bs.step([cv, cv], ds.zero_grads(), zero_grads=True)          # fully asynchronous: the loss words carry the signal
+    torch.cuda.synchronize()
+    assert bool(torch.isnan(bs.loss).all())
+    # enough capacity: finite losses again on the same objects' code path
+    bs2 = fdgs.BatchStep(ds, 64, 64, 4096, 2)
+    for rr in bs2.renderers:
+        rr.target_dev.copy_(tgt)
+    bs2.step([cv, cv], ds.zero_grads(), zero_grads=True)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(bs2.loss).all()) and float(bs2.loss.min()) > 0
+    rast = autograd.Rasterizer(sc.sh_degree, sc.n_time, 64, 64, 100)
+    params = {k: getattr(ds, k).clone().requires_grad_(True) for k in ("mean", "log_scale", "quat_l", "quat_r", "opacity_logit", "sh")}
+    with pytest.raises(fdgs.FdgsError) as e:
+        rast(params, cv)
+    assert e.value.code == fdgs.ERR_PAIR_OVERFLOW
+
+
 def test_batch_of_views_accumulates():
     """Gradient buffers are accumulated into: sum over views of grads == grads of the summed loss (L324 batch)."""
     import gpu_helpers as gh
@@ -111,6 +152,30 @@ def test_argument_validation():
     with pytest.raises(fdgs.FdgsError) as e:
         r.preprocess(cv)
     assert e.value.code == fdgs.ERR_WORKSPACE
+    # thresholds that do not describe a renderer are rejected, not rendered with (alpha_max >= 1 with
+    # transmittance_min = 0 divides by zero in the backward; a non-positive guard, cutoff or near plane, a negative dilation)
+    r = fdgs.Renderer(ds, 64, 64, 4096)
+    for bad in (dict(alpha_min=0.5, alpha_max=0.25), dict(alpha_max=1.5), dict(alpha_min=-0.1), dict(transmittance_min=1.0),
+                dict(transmittance_min=-1e-3), dict(dilation=-0.3), dict(cutoff_sigma=0.0), dict(guard=0.0), dict(znear=0.0),
+                dict(marginal_min=-0.05), dict(marginal_min=float("nan")), dict(alpha_max=float("nan"))):
+        r.cfg = fdgs.default_config(**bad)
+        with pytest.raises(fdgs.FdgsError) as e:
+            r.preprocess(cv)
+        assert e.value.code == fdgs.ERR_INVALID, bad
+    r.cfg = fdgs.default_config()
+    r.preprocess(cv); r.forward(cv)
+    # misaligned arrays that the kernels read with 128-bit accesses: an offset view of the 4DSH gradient, of the features
+    g = ds.zero_grads()
+    big = torch.zeros(g["sh"].numel() + 1, device="cuda")
+    g_bad = dict(g, sh=big[1:].view_as(g["sh"]))
+    with pytest.raises(fdgs.FdgsError) as e:
+        r.backward(cv, torch.zeros(3, 64, 64, device="cuda"), g_bad)
+    assert e.value.code == fdgs.ERR_INVALID
+    feat_big = torch.zeros(ds.N * 4 + 1, device="cuda")
+    with pytest.raises(fdgs.FdgsError) as e:
+        r.features_forward(cv, feat_big[1:].view(ds.N, 4))
+    assert e.value.code == fdgs.ERR_INVALID
+    torch.cuda.synchronize()
 
 
 def test_step_host_matches_device_path():
