@@ -59,8 +59,7 @@ def stage_rooflines(stage, work, N, K, n_views):
     byts = {"preprocess": n_views * 72 * N + nv * (12 * K + 76),
             "compact+tile_grid": n_views * 4 * N + 16 * nv,
             "sort_depth": 4 * 16 * nv,
-            "offsets": 12 * nv,                               # ids + tiles touched read, offsets written
-            "pair_scatter": 2 * 16 * nv + 4 * D,              # ids, offsets, rectangles read twice; 4 B written per pair
+            "tile_lists": 12 * nv + 4 * D,                    # ids and rectangles of the survivors read, 4 B written per pair
             "preprocess_bwd": nv * (36 + 68 + 12 * K + 2 * (12 * K + 68) + 64)}
     out = {}
     for k, b in byts.items():

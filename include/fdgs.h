@@ -7,8 +7,9 @@
  * library kernels).  The library never allocates device memory, never throws across the ABI and
  * never synchronises the stream unless a `_host` out-pointer is given.  fdgs_preprocess / fdgs_render_forward(_aux) /
  * fdgs_l1_loss / fdgs_render_backward(_aux) issue only kernels and device memsets on the caller's stream, so the sequence
- * can be captured into a CUDA graph.  The library keeps a little process-global state (launch counter, timing events,
- * worker streams of fdgs_step_batch / fdgs_step_host): calls are not re-entrant across host threads.
+ * can be captured into a CUDA graph.  The library keeps a little process-global state (atomic launch counter, timing
+ * events, and per CUDA device the worker streams of fdgs_step_batch / fdgs_step_host, created under a mutex): the step
+ * calls of ONE device are not re-entrant across host threads, everything else is.
  *
  * Conventions
  *   - Every pointer is a DEVICE pointer unless its name ends in `_host`.  fdgs_view and
@@ -103,12 +104,13 @@ int fdgs_preprocess(const fdgs_scene *scene, const fdgs_view *view_host, const f
                     int32_t *num_visible_host);
 
 /* Steps A6-A9: order the (tile, primitive) pairs as a stable sort on the key (tile id << 32 | fp32
- * depth bits) with ties in primitive-id order would (done two-level: survivors by depth, then pairs by
- * tile id — DESIGN.md), per-tile ranges, front-to-back alpha compositing of
+ * depth bits) with ties in primitive-id order would (done two-level: survivors sorted by depth, then every pair
+ * written straight to its place in its tile's list — DESIGN.md), per-tile ranges, front-to-back alpha compositing of
  * p_i(t) p_i(u,v|t) alpha_i c_i (eq. 6).  Outputs: image [3,H,W], final_T [H,W] (transmittance
  * left), n_contrib [H,W] (1 + position in the tile list of the last splat composited).
  * If D exceeded pair_capacity nothing is drawn (image = bg) and the overflow is reported by
- * fdgs_debug_export(FDGS_EXPORT_STATUS) or the next synchronising call. */
+ * fdgs_debug_export(FDGS_EXPORT_STATUS) or the next synchronising call.
+ * Each call consumes the tickets and look-back state that fdgs_preprocess prepared on `ws`: one forward per preprocess. */
 int fdgs_render_forward(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws,
                         size_t ws_bytes, int64_t pair_capacity, void *cuda_stream, float *image, float *final_T,
                         uint32_t *n_contrib);
@@ -144,7 +146,8 @@ int fdgs_l1_loss(const float *image, const float *target, int64_t count, float *
  * copies the loss (1 float) — or, when grads_host == NULL, the image — back to the host and
  * synchronises the stream.  target_host / result_host should be pinned.  The host -> device copy of the target runs
  * on a library-owned copy stream, forked from and joined to `cuda_stream` by events, so it overlaps preprocess and
- * forward; `target_dev` must not be touched by other streams during the call. */
+ * forward; `target_dev` must not be touched by other streams during the call.  Returns FDGS_ERR_PAIR_OVERFLOW if D
+ * exceeded pair_capacity (the result is then the loss / image of an empty rendering). */
 int fdgs_step_host(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws,
                    size_t ws_bytes, int64_t pair_capacity, void *cuda_stream, const float *target_host,
                    float *target_dev, float *image, float *final_T, uint32_t *n_contrib, float *dL_dimage,
@@ -159,8 +162,12 @@ int fdgs_step_host(const fdgs_scene *scene, const fdgs_view *view_host, const fd
  * the three functions view by view, up to fp32 summation order of the blend atomics.
  *   bufs_host[i].target_host  != NULL: [3,H,W] pinned host image, copied to target_dev inside the call;
  *                             == NULL: target_dev already holds the target.
- *   loss_dev [num_views] device floats: loss of each view (overwritten).
- *   loss_host != NULL: the losses are copied back and `cuda_stream` is synchronised; NULL: fully asynchronous.
+ *   loss_dev [num_views] device floats: loss of each view (overwritten); NaN for a view whose pairs exceeded
+ *                             pair_capacity (nothing drawn, zero gradients): the signal an asynchronous caller gets.
+ *   loss_host != NULL: the losses are copied back, `cuda_stream` is synchronised and FDGS_ERR_PAIR_OVERFLOW is returned if
+ *                             any view overflowed; NULL: fully asynchronous.
+ * If an argument is rejected or a launch fails after work has been forked onto the worker streams, they are joined into
+ * `cuda_stream` and it is synchronised before the error is returned: no kernel still runs on the caller's buffers.
  *   flags: FDGS_STEP_ZERO_GRADS = the six parameter-gradient arrays (and mean2d if given; not densify, which is meant to
  *          accumulate over steps) are zeroed inside the call, on a side stream, hidden under the forward passes.
  * 1 <= num_views <= FDGS_MAX_BATCH; workspaces must be distinct. */
@@ -183,7 +190,7 @@ int fdgs_step_batch(const fdgs_scene *scene, const fdgs_view *views_host, int32_
 #define FDGS_EXPORT_RECORDS 1       /* float[N,12]: u, v, conic A, B, C, opacity o, r, g, b, depth, radius, w */
 #define FDGS_EXPORT_RECTS 2         /* int32[N,4]: tx0, ty0, tx1, ty1 (all 0 for culled primitives)          */
 #define FDGS_EXPORT_TILES_TOUCHED 3 /* uint32[N]                                                             */
-#define FDGS_EXPORT_OFFSETS 4       /* uint32[num_visible] exclusive prefix sum of tiles_touched in depth order */
+/* 4 was FDGS_EXPORT_OFFSETS (round 1: prefix sum of tiles_touched in depth order); the pair emission it served is gone */
 #define FDGS_EXPORT_SORTED_KEYS 5   /* uint64[D]                                                             */
 #define FDGS_EXPORT_SORTED_VALS 6   /* uint32[D] primitive ids                                               */
 #define FDGS_EXPORT_RANGES 7        /* uint32[tiles,2]: [first, last+1) into the sorted arrays               */
@@ -194,8 +201,8 @@ int fdgs_debug_export(const void *ws, size_t ws_bytes, int what, void *dst, size
 
 /* Measurement hooks (bench.py).  fdgs_set_stage_timing(1) makes the three calls record CUDA events at
  * their stage boundaries; fdgs_get_stage_ms waits for them and fills ms_host[8]: preprocess kernel, compaction +
- * tile grid, depth sort, offsets + pair emission, tile sort, forward blend, backward blend, backward preprocess
- * (-1 for a stage that has not run).  fdgs_debug_blend_stats re-walks the tile lists of the last forward on `ws`
+ * tile grid, depth sort, tile lists (row scatter), forward blend, backward blend, backward preprocess, and -1 in the
+ * unused eighth slot (-1 as well for a stage that has not run).  fdgs_debug_blend_stats re-walks the tile lists of the last forward on `ws`
  * and writes uint64[4] to stats_dev: (pixel, splat) pairs walked, pairs reaching the exp2, pairs composited,
  * splats staged — the algorithmic work of the blend kernels. */
 int fdgs_set_stage_timing(int enable);

@@ -19,7 +19,7 @@ int cuda_fail(cudaError_t e, const char* where) {
 
 // Optional per-stage timing (fdgs_set_stage_timing): CUDA events recorded on the caller's stream at the stage
 // boundaries; off by default so that the product path carries no event records.
-enum { EV_PRE0, EV_PRE1, EV_PRE2, EV_FWD0, EV_FWD1, EV_FWD2, EV_FWD3, EV_FWD4, EV_BWD0, EV_BWD1, EV_BWD2, EV_COUNT };
+enum { EV_PRE0, EV_PRE1, EV_PRE2, EV_FWD0, EV_FWD1, EV_FWD2, EV_FWD3, EV_BWD0, EV_BWD1, EV_BWD2, EV_COUNT };
 static int g_timing = 0;
 static cudaEvent_t g_ev[EV_COUNT];
 static inline void mark(int which, cudaStream_t st) { if (g_timing) cudaEventRecord(g_ev[which], st); }
@@ -245,12 +245,10 @@ static int forward_impl(const fdgs_scene* sc, const ViewParams& vp, const CfgPar
   mark(EV_FWD0, st);
   const int l1 = launch_sort_depth(ws, sc->N, sms, st);             // level 1: survivors by fp32 depth bits
   mark(EV_FWD1, st);
-  launch_offsets(ws, l1, sc->N, st);
+  launch_row_scatter(ws, l1, sc->N, vp, sms, st);                       // level 2: per-tile lists written in place, depth order
   mark(EV_FWD2, st);
-  launch_pair_scatter(ws, l1, sc->N, vp, sms, st);                  // level 2: per-tile lists written in place, depth order
-  mark(EV_FWD3, st);
   launch_blend_fwd(ws, vp, cp, image, final_T, n_contrib, depth_map, st);
-  mark(EV_FWD4, st);
+  mark(EV_FWD3, st);
   FDGS_CUDA(cudaGetLastError(), "forward launches");
   return FDGS_OK;
 }
@@ -581,9 +579,10 @@ int fdgs_set_stage_timing(int enable) {
 
 int fdgs_get_stage_ms(float* ms_host) {
   if (!ms_host || !g_timing) return FDGS_ERR_INVALID;
-  const int pairs[8][2] = {{EV_PRE0, EV_PRE1}, {EV_PRE1, EV_PRE2}, {EV_FWD0, EV_FWD1}, {EV_FWD1, EV_FWD2},
-                           {EV_FWD2, EV_FWD3}, {EV_FWD3, EV_FWD4}, {EV_BWD0, EV_BWD1}, {EV_BWD1, EV_BWD2}};
-  for (int k = 0; k < 8; ++k) {
+  const int pairs[7][2] = {{EV_PRE0, EV_PRE1}, {EV_PRE1, EV_PRE2}, {EV_FWD0, EV_FWD1}, {EV_FWD1, EV_FWD2},
+                           {EV_FWD2, EV_FWD3}, {EV_BWD0, EV_BWD1}, {EV_BWD1, EV_BWD2}};
+  ms_host[7] = -1.f;
+  for (int k = 0; k < 7; ++k) {
     ms_host[k] = -1.f;
     if (cudaEventSynchronize(g_ev[pairs[k][1]]) == cudaSuccess) cudaEventElapsedTime(&ms_host[k], g_ev[pairs[k][0]], g_ev[pairs[k][1]]);
   }
@@ -685,7 +684,6 @@ extern "C" int fdgs_debug_export(const void* ws_ptr, size_t ws_bytes, int what, 
       if (N > 0) export_rects_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(ws.rect, (int)N, (int4*)dst);
       break;
     case FDGS_EXPORT_TILES_TOUCHED: src = ws.tiles_touched; need = 4 * (size_t)N; break;
-    case FDGS_EXPORT_OFFSETS: src = ws.offsets; need = 4 * (size_t)h.num_visible; break;
     case FDGS_EXPORT_DEPTH_ORDER: src = ws.l1_vals[l1]; need = 4 * (size_t)h.num_visible; break;
     case FDGS_EXPORT_SORTED_KEYS:
       if (dst_bytes < 8 * (size_t)D) return FDGS_ERR_INVALID;

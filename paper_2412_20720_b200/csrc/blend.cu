@@ -15,6 +15,47 @@ namespace fdgs {
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
+// ---- bulk asynchronous copies (TMA, non-tensor form) and their mbarriers: records are gathered global -> shared by the
+// copy engine while the warps composite the previous batch (SASS: UBLKCP, SYNCS) ----
+// FDGS_BLEND_ASYNC selects the staging of the forward blend at COMPILE time (measurement builds: FDGS_NVCC_EXTRA, build.py):
+//   0 (product): synchronous LDG -> convert -> STS, 256 splats per batch (blend_fwd_kernel<2>);
+//   1: cp.async.bulk + mbarrier, 2: cp.async (LDGSTS) — blend_fwd_async_kernel.  Both async pipelines were built,
+//   verified against the oracle and measured on B200 in round 2 and LOSE to the synchronous staging (1.436 / 1.339 vs
+//   1.248 ms per 4 views at cfg3; profiles/r2_blend_staging_ab.md), so they are not in libfdgs.so.
+#ifndef FDGS_BLEND_ASYNC
+#define FDGS_BLEND_ASYNC 0
+#endif
+__device__ __forceinline__ unsigned int smem_u32(const void* p) { return (unsigned int)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, const unsigned int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* bar, const unsigned int bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(unsigned long long* bar, const unsigned int parity) {
+  unsigned int ok;
+  asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+               : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, const unsigned int parity) { while (!mbar_try_wait(bar, parity)) {} }
+// one record (48 B, 16-byte aligned on both sides) global -> shared; completion is counted in bytes on `bar`
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, const unsigned int bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+
+// tile-local form of a record, in place: (q0, q1, q2) of SplatRec -> (s0, s1, s2) below
+__device__ __forceinline__ void convert_splat(float4* r, const float ox, const float oy) {
+  const float4 q0 = r[0], q1 = r[1], q2 = r[2];
+  const float ul = q0.x - ox, vl = q0.y - oy;
+  r[0] = make_float4(-q0.z, -q0.w, -q1.x, fmaf(q0.z, ul, q0.w * vl));
+  r[1] = make_float4(q1.x * vl, q1.y, q1.z, q1.w);
+  r[2] = make_float4(q2.x, ul, vl, q2.y);
+}
+
 // Shared-memory form of a splat: three float4, read as broadcast LDS.128
 //   s0 = (-ca, -cb, -cc, k1 = ca*(u-ox) + cb*(v-oy))   s1 = (k2 = cc*(v-oy), lo = log2(o), r, g)   s2 = (b, u-ox, v-oy, depth)
 __device__ __forceinline__ void stage_splat(const SplatRec* __restrict__ rec, const unsigned int id, const float ox, const float oy,
@@ -171,6 +212,167 @@ __global__ void __launch_bounds__(256 / PX, PX == 2 && !STATS ? 9 : 1) blend_fwd
     if (AUX) depth_map[pix] = Dz[k];
   }
 }
+
+#if FDGS_BLEND_ASYNC
+// A9 with bulk-asynchronous staging (north_star subsystem 5).  Same walk, same decisions, same arithmetic as
+// blend_fwd_kernel<2>; what changes is how a batch of splats reaches shared memory:
+//   - the 48-byte record of every listed splat is gathered by one `cp.async.bulk` (the copy engine: no register, no
+//     scoreboard slot, no LDG -> STS round trip in the warps) into a RAW slot owned by the issuing thread; completion is
+//     counted in bytes on one mbarrier, whose phase also needs all 128 threads to arrive, so that a phase can never
+//     complete before every thread has seen the previous one;
+//   - one batch ahead, the thread converts the record of its slot to tile-local form into the structure-of-arrays
+//     buffer of the NEXT batch (two such buffers alternate) and at once asks the copy engine for the record of the batch
+//     after that, into the same slot: the copy has a whole batch of compositing to land;
+//   - so there is ONE block barrier per batch — the `__syncthreads_and` that votes on early termination — instead of two,
+//     and no global-memory latency between barriers; the ids are loaded (coalesced) one more batch ahead into a register.
+// Before the CTA exits it waits for the copy it has issued last (shared memory of a finished CTA is reallocated).
+// MODE 1: cp.async.bulk + mbarrier as described.  MODE 2: the same pipeline with three 16-byte `cp.async` (LDGSTS) per
+// record instead of one bulk copy, completion by `cp.async.wait_group` of the issuing thread (no mbarrier): kept for the
+// A/B numbers in profiles/ (build with -DFDGS_BLEND_ASYNC=2).
+template <bool AUX, bool DEF, int MODE>
+__global__ void __launch_bounds__(128, 8) blend_fwd_async_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
+                                                                 const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
+                                                                 float* __restrict__ image, float* __restrict__ final_T,
+                                                                 unsigned int* __restrict__ n_contrib, float* __restrict__ depth_map) {
+  constexpr int PX = 2, BATCH = 128;
+  __shared__ __align__(16) float4 raw[BATCH][3];
+  __shared__ struct { float4 s0[BATCH], s1[BATCH], s2[BATCH]; } sm[2];
+  __shared__ __align__(8) unsigned long long full;
+  const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const Strip<PX> sp(warp, lane);
+  const int px = tx * TILE + sp.lx;
+  const float x = sp.lx + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
+  const float c_l2min = DEF ? FDGS_DEF_L2MIN : cp.log2_alpha_min, c_amax = DEF ? FDGS_DEF_ALPHA_MAX : cp.alpha_max;
+  const float c_amin = DEF ? FDGS_DEF_ALPHA_MIN : cp.alpha_min, c_tmin = DEF ? FDGS_DEF_T_MIN : cp.transmittance_min;
+  float y[PX], T[PX], Cr[PX], Cg[PX], Cb[PX], Dz[PX], lmin[PX];
+  unsigned int last[PX];
+  bool inside[PX];
+#define FDGS_DONE(k) (lmin[k] > 3.0e38f)
+#pragma unroll
+  for (int k = 0; k < PX; ++k) {
+    const int ly = sp.ly0 + 4 * k;
+    inside[k] = px < vp.width && ty * TILE + ly < vp.height;
+    y[k] = ly + 0.5f; T[k] = 1.f; Cr[k] = Cg[k] = Cb[k] = Dz[k] = 0.f; last[k] = 0; lmin[k] = inside[k] ? c_l2min : INFINITY;
+  }
+  const uint2 range = ranges[tile];
+  const int n = (int)(range.y - range.x), nb = (n + BATCH - 1) / BATCH;
+  if (MODE == 1) {
+    if (threadIdx.x == 0) { mbar_init(&full, 128); fence_mbar_init(); }
+    __syncthreads();
+  }
+  auto load_id = [&](const int k) -> unsigned int { const int i = k * BATCH + (int)threadIdx.x; return i < n ? vals[range.x + i] : 0u; };
+  // batch k: every thread arrives on the barrier's phase k; the threads that own a splat of the batch add its 48 bytes to
+  // the phase and ask the copy engine for them
+  auto issue = [&](const int k, const unsigned int id) {
+    if (MODE == 2) {
+      if (k * BATCH + (int)threadIdx.x < n) {
+        const float4* src = reinterpret_cast<const float4*>(rec + id);
+#pragma unroll
+        for (int q = 0; q < 3; ++q)
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(&raw[threadIdx.x][q])), "l"(src + q) : "memory");
+      }
+      asm volatile("cp.async.commit_group;" ::: "memory");
+    } else if (k * BATCH + (int)threadIdx.x < n) {
+      mbar_arrive_expect_tx(&full, 48u);
+      bulk_g2s(&raw[threadIdx.x][0], rec + id, 48u, &full);
+    } else {
+      asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&full)) : "memory");
+    }
+  };
+  // wait until batch k has landed; my record, converted to tile-local form, goes to the buffer of batch k
+  auto convert = [&](const int k) {
+    if (MODE == 2) asm volatile("cp.async.wait_group 0;" ::: "memory");      // my own three copies: nobody else reads my raw slot
+    else mbar_wait(&full, (unsigned int)k & 1u);
+    if (k * BATCH + (int)threadIdx.x < n) {
+      const float4 q0 = raw[threadIdx.x][0], q1 = raw[threadIdx.x][1], q2 = raw[threadIdx.x][2];
+      const float ul = q0.x - ox, vl = q0.y - oy;
+      sm[k & 1].s0[threadIdx.x] = make_float4(-q0.z, -q0.w, -q1.x, fmaf(q0.z, ul, q0.w * vl));
+      sm[k & 1].s1[threadIdx.x] = make_float4(q1.x * vl, q1.y, q1.z, q1.w);
+      sm[k & 1].s2[threadIdx.x] = make_float4(q2.x, ul, vl, q2.y);
+    }
+  };
+  unsigned int id_next = 0;
+  if (nb > 0) { issue(0, load_id(0)); convert(0); }
+  if (nb > 1) { if (MODE == 1) fence_proxy_async(); issue(1, load_id(1)); }
+  if (nb > 2) id_next = load_id(2);
+  int k = 0;
+  for (; k < nb; ++k) {
+    bool all_done = true;
+#pragma unroll
+    for (int q = 0; q < PX; ++q) all_done = all_done && FDGS_DONE(q);
+    // the one barrier of the batch: every warp has left batch k-1 (its buffer, which is the one of batch k+1, may be
+    // overwritten), the conversions of batch k are visible, and the vote on early termination
+    if (__syncthreads_and(all_done)) break;
+    if (k + 1 < nb) {
+      convert(k + 1);                                 // landed long ago: issued one iteration earlier
+      if (k + 2 < nb) {
+        if (MODE == 1) fence_proxy_async();           // my generic-proxy reads of the raw slot, before the copy engine rewrites it
+        issue(k + 2, id_next);
+        id_next = k + 3 < nb ? load_id(k + 3) : 0u;
+      }
+    }
+    const int base = k * BATCH, m = min(BATCH, n - base);
+    const auto& sb = sm[k & 1];
+    unsigned int alive = 0;                           // sub-patches with an unsaturated pixel (warp-uniform)
+#pragma unroll
+    for (int q = 0; q < PX; ++q) if (!__all_sync(0xffffffffu, FDGS_DONE(q))) alive |= 1u << q;
+    if (!alive) continue;
+    for (int jb = 0; jb < m; jb += 32) {
+      unsigned int hk[PX], any = 0;
+      float4 ta, tb;
+      if (jb + lane < m) { ta = sb.s0[jb + lane]; tb = sb.s1[jb + lane]; }
+#pragma unroll
+      for (int q = 0; q < PX; ++q) {
+        hk[q] = ((alive >> q) & 1u) ? __ballot_sync(0xffffffffu, jb + lane < m && patch_hit(ta, tb, sp.xm, sp.ym0 + 4.f * q, c_l2min)) : 0u;
+        any |= hk[q];
+      }
+      while (any) {
+        const int bit = __ffs(any) - 1;
+        any &= any - 1;
+        const int j = jb + bit;
+        const float4 a = sb.s0[j], b = sb.s1[j];
+        const float e1x = fmaf(a.x, x, a.w);
+#pragma unroll
+        for (int q = 0; q < PX; ++q) {
+          if (!((hk[q] >> bit) & 1u)) continue;                          // warp-uniform
+          const float e1 = fmaf(a.y, y[q], e1x);
+          const float e2 = fmaf(a.z, y[q], b.x);
+          const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
+          if (!(l2a >= lmin[q])) continue;                     // alpha < alpha_min (or pixel done): skipped
+          const float alpha = fminf(c_amax, ex2_approx(l2a));
+          if (alpha < c_amin) continue;
+          const float Tn = fmaf(-T[q], alpha, T[q]);
+          const bool term = Tn < c_tmin;                       // the terminating splat is not composited
+          asm("{\n\t.reg .pred p;\n\tsetp.lt.f32 p, %1, %2;\n\t@p mov.b32 %0, 0x7f800000;\n\t}" : "+f"(lmin[q]) : "f"(Tn), "f"(c_tmin));
+          if (term) continue;
+          const float wgt = alpha * T[q];
+          Cr[q] = fmaf(b.z, wgt, Cr[q]); Cg[q] = fmaf(b.w, wgt, Cg[q]); Cb[q] = fmaf(sb.s2[j].x, wgt, Cb[q]);
+          if (AUX) Dz[q] = fmaf(sb.s2[j].w, wgt, Dz[q]);
+          T[q] = Tn;
+          last[q] = base + j + 1;
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < PX; ++q) if (((alive >> q) & 1u) && __all_sync(0xffffffffu, FDGS_DONE(q))) alive &= ~(1u << q);
+      if (!alive) break;
+    }
+  }
+#undef FDGS_DONE
+  // early termination at the top of iteration k: batch k + 1 (if any) was issued one iteration earlier and has not been waited for
+  if (k + 1 < nb) { if (MODE == 2) asm volatile("cp.async.wait_group 0;" ::: "memory"); else mbar_wait(&full, (unsigned int)(k + 1) & 1u); }
+  const size_t hw = (size_t)vp.width * vp.height;
+#pragma unroll
+  for (int q = 0; q < PX; ++q) {
+    if (!inside[q]) continue;
+    const size_t pix = (size_t)(ty * TILE + sp.ly0 + 4 * q) * vp.width + px;
+    image[pix] = fmaf(T[q], vp.bg[0], Cr[q]); image[hw + pix] = fmaf(T[q], vp.bg[1], Cg[q]); image[2 * hw + pix] = fmaf(T[q], vp.bg[2], Cb[q]);
+    final_T[pix] = T[q]; n_contrib[pix] = last[q];
+    if (AUX) depth_map[pix] = Dz[q];
+  }
+}
+
+#endif  // FDGS_BLEND_ASYNC
 
 // Feature channels: the walk of blend_fwd_kernel<2> — same staging, same patch culling, the
 // SAME expression for alpha, so every skip / termination decision is bit-identical to the colour pass — compositing CH
@@ -694,7 +896,11 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
 void launch_blend_fwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
                       unsigned int* n_contrib, float* depth_map, cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
+#if FDGS_BLEND_ASYNC
+#define FDGS_FWD(AUXV, DEFV) blend_fwd_async_kernel<AUXV, DEFV, FDGS_BLEND_ASYNC><<<tiles, 128, 0, st>>>(ws.ranges, ws.pair_ids, ws.rec, vp, cp, image, final_T, n_contrib, depth_map)
+#else
 #define FDGS_FWD(AUXV, DEFV) blend_fwd_kernel<2, false, AUXV, DEFV><<<tiles, 128, 0, st>>>(ws.ranges, ws.pair_ids, ws.rec, vp, cp, image, final_T, n_contrib, nullptr, depth_map)
+#endif
   if (depth_map) { if (cp.default_thresholds) FDGS_FWD(true, true); else FDGS_FWD(true, false); }
   else           { if (cp.default_thresholds) FDGS_FWD(false, true); else FDGS_FWD(false, false); }
 #undef FDGS_FWD

@@ -69,16 +69,16 @@ constexpr int DEPTH_PASSES = 32 / RADIX_BITS;
 constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_ITEMS = 8;
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
-constexpr int MIN_PAIR_CHUNK = 16384;   // pairs per chunk of the ordered pair scatter (scan_dup.cu), at least
-constexpr int MAX_PAIR_CHUNKS = 1024;   // chunks the pair capacity is divided into, at most
+constexpr int RS_MIN_CHUNK = 2048, RS_MAX_CHUNK = 32768;   // survivors per chunk of the row scatter (scan_dup.cu)
+constexpr int RS_MAX_ITERS = RS_MAX_CHUNK / 32;
 constexpr int MAX_GRID_CELLS = 50000;   // (tiles_x+1)*(tiles_y+1) must fit the shared memory of the tile-grid / scatter kernels
 
 // Host-side view of the carved-up workspace.
 //
 // Binning is two-level: survivors are first sorted by their fp32 depth bits (level 1, <= N items,
 // hand-written onesweep radix sort); the (tile, id) pairs are then written in that order straight to their final
-// position in the per-tile lists by a stable, rectangle-aware scatter (level 2: chunk coverage grids -> chunk bases ->
-// ordered scatter; no key array exists).  The resulting per-tile lists are exactly those of one stable sort on the
+// position in the per-tile lists by a stable, rectangle-aware scatter (level 2, "row scatter": one CTA per chunk of
+// survivors and tile row; no key array exists).  The resulting per-tile lists are exactly those of one stable sort on the
 // 64-bit key tile<<32 | depth-bits with ties in id order.
 struct Workspace {
   WsHeader* hdr;
@@ -93,10 +93,10 @@ struct Workspace {
   unsigned int* l1_keys[2];          // [N] fp32 depth bits of survivors (double buffer)
   unsigned int* l1_vals[2];          // [N] primitive ids of survivors; after the sort: depth order
   unsigned int* vis_ids;             // [N] primitive ids of survivors in ascending id order (kept for the backward)
-  unsigned int* offsets;             // [N] exclusive prefix sum of tiles_touched in depth order
-  unsigned int chunk_pairs, num_chunks;  // pairs per scatter chunk; chunks the capacity is divided into
-  unsigned int* chunk_first;         // [num_chunks + 1] first survivor (depth order) whose pairs START in chunk q
-  unsigned int* chunk_base;          // [num_chunks][tiles] coverage of chunk q per tile -> first output position of chunk q in tile
+  unsigned int* sorted_ys;           // [N] tile rows   y0 | y1 << 16 of the survivors in depth order (written by the last depth-sort pass)
+  unsigned int* sorted_xs;           // [N] tile columns x0 | x1 << 16, same order
+  unsigned int rs_chunk, rs_chunks;  // survivors per chunk of the row scatter; chunks N is divided into
+  unsigned int* rs_state;            // [rs_chunks][tiles] look-back words of the row scatter (count of chunk c in tile T), cleared with the header
   unsigned int* pair_ids;            // [cap] primitive ids of the per-tile lists, tile after tile (ranges), depth order inside
   uint2* ranges;                     // [tiles] [first, last+1)
   float* g9;                         // [N,9] per-splat gradients of the blend backward
@@ -123,6 +123,12 @@ inline Workspace carve(void* base, long long N, long long K, long long W, long l
   const long long t1 = (Np + SORT_THREADS * SORT_ITEMS_L1 - 1) / (SORT_THREADS * SORT_ITEMS_L1);
   w.lookback_stride = (size_t)RADIX * (size_t)(t1 + 1);
   w.sort_lookback = (unsigned int*)take(4 * w.lookback_stride * DEPTH_PASSES);
+  long long ch = ((Np + 127) / 128 + 255) / 256 * 256;    // <= 128 chunks unless that makes them larger than RS_MAX_CHUNK
+  if (ch < RS_MIN_CHUNK) ch = RS_MIN_CHUNK;
+  if (ch > RS_MAX_CHUNK) ch = RS_MAX_CHUNK;
+  w.rs_chunk = (unsigned int)ch;
+  w.rs_chunks = (unsigned int)((Np + ch - 1) / ch);
+  w.rs_state = (unsigned int*)take(4 * (size_t)w.rs_chunks * (size_t)tiles);
   w.zero_bytes = off;
   w.rec = (SplatRec*)take(sizeof(SplatRec) * Np);
   w.rect = (ushort4*)take(sizeof(ushort4) * Np);
@@ -130,13 +136,8 @@ inline Workspace carve(void* base, long long N, long long K, long long W, long l
   for (int i = 0; i < 2; ++i) w.l1_keys[i] = (unsigned int*)take(4 * Np);
   for (int i = 0; i < 2; ++i) w.l1_vals[i] = (unsigned int*)take(4 * Np);
   w.vis_ids = (unsigned int*)take(4 * Np);
-  w.offsets = (unsigned int*)take(4 * Np);
-  long long cp = (cap + MAX_PAIR_CHUNKS - 1) / MAX_PAIR_CHUNKS;
-  if (cp < MIN_PAIR_CHUNK) cp = MIN_PAIR_CHUNK;
-  w.chunk_pairs = (unsigned int)cp;
-  w.num_chunks = (unsigned int)(cap / cp + 1);
-  w.chunk_first = (unsigned int*)take(4 * ((size_t)w.num_chunks + 2));
-  w.chunk_base = (unsigned int*)take(4 * (size_t)w.num_chunks * (size_t)tiles);
+  w.sorted_ys = (unsigned int*)take(4 * Np);
+  w.sorted_xs = (unsigned int*)take(4 * Np);
   w.pair_ids = (unsigned int*)take(4 * (size_t)cap);
   w.ranges = (uint2*)take(sizeof(uint2) * tiles);
   w.g9 = (float*)take(4 * 9 * Np);
@@ -170,13 +171,11 @@ void launch_preprocess_fwd(const fdgs_scene& sc, const ViewParams& vp, const Cfg
 // the same launch carries, as the role of its first CTA, the 2D prefix of the coverage difference array -> ranges, D, overflow
 void launch_compact_and_tile_grid(const Workspace& ws, int N, int K, const ViewParams& vp, long long cap, cudaStream_t st);
 // Stable LSD radix sort of the survivors' (depth bits, id) pairs on all 32 key bits; the count is read on the device and
-// ws.sort_hist[pass] holds the digit counts of the pass.  Returns the result buffer (0/1).
+// ws.sort_hist[pass] holds the digit counts of the pass.  The last pass also writes the tile rectangles of the survivors
+// in the final order (sorted_ys / sorted_xs).  Returns the result buffer (0/1).
 int launch_sort_depth(const Workspace& ws, long long max_count, int num_sms, cudaStream_t st);
-// exclusive prefix sum of tiles_touched in depth order -> offsets, chunk_first
-void launch_offsets(const Workspace& ws, int l1_buf, int N, cudaStream_t st);
-// level 2: per-tile lists in depth order written straight to their final place (three launches: chunk coverage, chunk
-// bases, ordered scatter)
-void launch_pair_scatter(const Workspace& ws, int l1_buf, int N, const ViewParams& vp, int num_sms, cudaStream_t st);
+// level 2: per-tile lists in depth order written straight to their final place (scan_dup.cu "row scatter")
+void launch_row_scatter(const Workspace& ws, int l1_buf, int N, const ViewParams& vp, int num_sms, cudaStream_t st);
 void launch_blend_fwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
                       unsigned int* n_contrib, float* depth_map /*NULL = no auxiliary channel*/, cudaStream_t st);
 void launch_blend_stats(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, unsigned long long* stats, cudaStream_t st);

@@ -13,14 +13,18 @@ namespace fdgs {
 constexpr int LB_WIN = 8;
 constexpr unsigned int LB_AGG = 1u << 30, LB_PRE = 2u << 30, LB_MASK = (1u << 30) - 1;
 
-template <int ITEMS>
+template <int ITEMS, bool LAST>
+// LAST: the final pass also gathers the tile rectangle of every survivor and writes it next to the id, in the sorted
+// order (ys = y0 | y1 << 16, xs = x0 | x1 << 16): the row scatter reads them coalesced.
 // 3 CTAs per SM (<= 85 registers): measured best at 50 M pairs (812 us for two passes vs 916 us at 2 CTAs / 128 registers);
 // 4 or 5 CTAs spill.
 __global__ void __launch_bounds__(SORT_THREADS, 3) onesweep_kernel(const unsigned int* __restrict__ keys_in, const unsigned int* __restrict__ vals_in,
                                                                 unsigned int* __restrict__ keys_out, unsigned int* __restrict__ vals_out,
                                                                 const unsigned int* __restrict__ count_dev, unsigned int* ticket,
                                                                 const unsigned int* __restrict__ digit_base /*[RADIX]*/,
-                                                                const bool bases_exclusive, volatile unsigned int* lookback, const int shift) {
+                                                                const bool bases_exclusive, volatile unsigned int* lookback, const int shift,
+                                                                const ushort4* __restrict__ rect, unsigned int* __restrict__ ys_out,
+                                                                unsigned int* __restrict__ xs_out) {
   constexpr int TILE_N = SORT_THREADS * ITEMS, WARPS = SORT_THREADS / 32;
   __shared__ unsigned int warp_hist[WARPS][RADIX];   // per-warp digit counts -> exclusive offsets over warps
   __shared__ unsigned int s_local[RADIX];            // first slot of each digit inside the sorted tile
@@ -145,7 +149,9 @@ __global__ void __launch_bounds__(SORT_THREADS, 3) onesweep_kernel(const unsigne
       if (slot < valid_n) {
         const unsigned int k = s_keys[slot];
         const unsigned int out = s_global[(k >> shift) & (RADIX - 1)] + slot;
-        keys_out[out] = k; vals_out[out] = s_vals[slot];
+        const unsigned int v = s_vals[slot];
+        keys_out[out] = k; vals_out[out] = v;
+        if (LAST) { const ushort4 rc = rect[v]; ys_out[out] = (unsigned int)rc.y | ((unsigned int)rc.w << 16); xs_out[out] = (unsigned int)rc.x | ((unsigned int)rc.z << 16); }
       }
     }
     __syncthreads();
@@ -159,9 +165,11 @@ int launch_sort_depth(const Workspace& ws, long long max_count, int num_sms, cud
   const int grid = (int)(tiles < 4LL * num_sms ? tiles : 4LL * num_sms);
   int cur = 0;
   for (int p = 0; p < DEPTH_PASSES; ++p) {      // the look-back region of every pass was cleared with the header (fdgs_preprocess)
-    onesweep_kernel<SORT_ITEMS_L1><<<grid, SORT_THREADS, 0, st>>>(ws.l1_keys[cur], ws.l1_vals[cur], ws.l1_keys[cur ^ 1], ws.l1_vals[cur ^ 1],
-                                                                 &ws.hdr->num_visible, &ws.hdr->sort_ticket[p], ws.sort_hist + p * RADIX, false,
-                                                                 ws.sort_lookback + (size_t)p * ws.lookback_stride, p * RADIX_BITS);
+#define FDGS_PASS(LASTV) onesweep_kernel<SORT_ITEMS_L1, LASTV><<<grid, SORT_THREADS, 0, st>>>(ws.l1_keys[cur], ws.l1_vals[cur], ws.l1_keys[cur ^ 1], ws.l1_vals[cur ^ 1], \
+                                                                 &ws.hdr->num_visible, &ws.hdr->sort_ticket[p], ws.sort_hist + p * RADIX, false,                    \
+                                                                 ws.sort_lookback + (size_t)p * ws.lookback_stride, p * RADIX_BITS, ws.rect, ws.sorted_ys, ws.sorted_xs)
+    if (p == DEPTH_PASSES - 1) FDGS_PASS(true); else FDGS_PASS(false);
+#undef FDGS_PASS
     count_launch();
     cur ^= 1;
   }

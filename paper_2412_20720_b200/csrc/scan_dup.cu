@@ -1,5 +1,5 @@
 // scan_dup.cu — A5/A6/A7b/A8 for sm_100a: compaction scan (+ depth digit counts) with the tile-grid prefix (ranges, D) as a
-// role of its first CTA, offsets scan, and the rectangle-aware ordered scatter that writes the per-tile lists.
+// role of its first CTA, and the row scatter that writes the per-tile lists in depth order without sorting the pairs.
 #include "common.cuh"
 
 namespace fdgs {
@@ -144,201 +144,183 @@ __global__ void __launch_bounds__(SCAN_THREADS) compact_kernel(const unsigned in
   for (int p = 0; p < 4; ++p) { const unsigned int v = hist[p][threadIdx.x]; if (v) atomicAdd(sort_hist + p * RADIX + threadIdx.x, v); }
 }
 
-// offsets[j] = exclusive prefix of tiles_touched[sorted_ids[j]], j < num_visible (depth order).  Also cuts the emission
-// order into chunks of ~chunk_pairs pairs made of WHOLE survivors: survivor j belongs to chunk offsets[j] / chunk_pairs, and
-// chunk_first[q] = the first survivor of chunk q or later (= num_visible past the last one), q <= num_chunks.
-__global__ void __launch_bounds__(SCAN_THREADS) offsets_kernel(const unsigned int* __restrict__ tiles_touched,
-                                                               const unsigned int* __restrict__ sorted_ids, WsHeader* hdr,
-                                                               unsigned long long* state, unsigned int* __restrict__ offsets,
-                                                               unsigned int* __restrict__ chunk_first, const unsigned int chunk_pairs,
-                                                               const unsigned int num_chunks) {
-  __shared__ unsigned int warp_sums[33], s_tile, s_prefix;
-  const unsigned int n = hdr->num_visible;
-  if (threadIdx.x == 0) s_tile = atomicAdd(&hdr->scan_ticket[1], 1u);
-  __syncthreads();
-  const unsigned int tile = s_tile;
-  if (n == 0) {                                             // nothing visible: every chunk is empty
-    if (tile == 0) for (unsigned int q = threadIdx.x; q <= num_chunks; q += blockDim.x) chunk_first[q] = 0;
-    return;
-  }
-  if ((unsigned long long)tile * SCAN_TILE >= n) return;   // tickets are dense: every tile below this one exists
-  const unsigned int base = tile * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
-  unsigned int c[SCAN_ITEMS], sum = 0;
-#pragma unroll
-  for (int k = 0; k < SCAN_ITEMS; ++k) { c[k] = base + k < n ? tiles_touched[sorted_ids[base + k]] : 0; sum += c[k]; }
-  unsigned int total;
-  const unsigned int excl = block_exclusive_scan(sum, total, warp_sums);
-  const unsigned int prefix = lookback_prefix(state, tile, total, &s_prefix);
-  if (hdr->overflow) return;                               // D exceeds the capacity: nothing is emitted
-  unsigned int run = prefix + excl;
-  // chunk of the previous survivor (-1 before the first one): every chunk id in (previous, mine] starts at me
-  long long prev_chunk = -1;
-  if (base > 0 && base < n) prev_chunk = (long long)((run - tiles_touched[sorted_ids[base - 1]]) / chunk_pairs);
-#pragma unroll
-  for (int k = 0; k < SCAN_ITEMS; ++k) {
-    if (base + k < n) {
-      offsets[base + k] = run;
-      const long long mine = run / chunk_pairs;
-      for (long long q = prev_chunk + 1; q <= mine; ++q) chunk_first[q] = base + k;
-      prev_chunk = mine;
-      if (base + k == n - 1) for (unsigned int q = (unsigned int)mine + 1; q <= num_chunks; ++q) chunk_first[q] = n;
-    }
-    run += c[k];
-  }
-}
-
 // ---------------------------------------------------------------------------------------------
-// A6/A7, level 2: the per-tile lists in depth order, written straight to their final place.
+// A6/A7, level 2: the per-tile lists in depth order, written straight to their final place ("row scatter").
 //
-// Survivors arrive sorted by depth (level 1); survivor j covers the tile rectangle rect[j].  The list of tile T is
-// {j : T in rect[j]} in ascending j, stored at [ranges[T].x, ranges[T].y) — a stable partition of the emission order
-// (j, tiles of rect[j]) by tile, i.e. what a stable sort of the (tile, id) pairs by tile id produces.  Because the ranges
-// are already known from the coverage grid and the covered sets are RECTANGLES, no sort is needed:
-//   1. chunk_cover_kernel: the emission order is cut into chunks of whole survivors (chunk_first); a CTA builds the
-//      coverage count of its chunk for every tile with a 2D difference array in shared memory (4 atomics per survivor +
-//      one 2D prefix, whatever the footprints);
-//   2. chunk_base_kernel: exclusive prefix over the chunks, per tile, started at ranges[T].x = the output position at
-//      which chunk q starts writing in tile T;
-//   3. pair_scatter_kernel: a CTA per chunk walks its survivors in order, 32 at a time.  Within such a group the
-//      rank of survivor s in tile T is the number of lower-numbered members that also cover T: every (member, tile)
-//      pair ORs its member bit into a per-tile mask in shared memory, the rank is a popcount of the lower bits, and the
-//      highest member advances the tile's cursor by the group's count.  O(1) work per pair, 4 bytes written per pair,
-//      no key array, no look-back, no histogram.
-// Replaces offsets + pair emission + a 2-pass radix sort of the D pairs (round 1: 146 us per view at cfg3).
-__global__ void __launch_bounds__(256) chunk_cover_kernel(const unsigned int* __restrict__ sorted_ids, const ushort4* __restrict__ rect,
-                                                          const WsHeader* __restrict__ hdr, const unsigned int* __restrict__ chunk_first,
-                                                          const unsigned int chunk_pairs, const int tiles_x, const int tiles_y,
-                                                          unsigned int* __restrict__ chunk_base) {
-  extern __shared__ int grid[];                 // (tiles_y+1) x (tiles_x+1)
-  const unsigned int D = hdr->num_pairs;
-  const unsigned int q = blockIdx.x;
-  if ((unsigned long long)q * chunk_pairs >= D) return;    // also covers overflow (num_pairs == 0)
-  const int sx = tiles_x + 1, rows = tiles_y + 1, cells = sx * rows;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-  for (int i = threadIdx.x; i < cells; i += blockDim.x) grid[i] = 0;
-  __syncthreads();
-  const unsigned int j0 = chunk_first[q], j1 = chunk_first[q + 1];
-  for (unsigned int j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
-    const ushort4 rc = rect[sorted_ids[j]];
-    atomicAdd(&grid[rc.y * sx + rc.x], 1); atomicAdd(&grid[rc.y * sx + rc.z], -1);
-    atomicAdd(&grid[rc.w * sx + rc.x], -1); atomicAdd(&grid[rc.w * sx + rc.z], 1);
-  }
-  __syncthreads();
-  for (int y = warp; y < rows; y += nwarps) {
-    int carry = 0;
-    for (int x0 = 0; x0 < sx; x0 += 32) {
-      const int x = x0 + lane;
-      int v = x < sx ? grid[y * sx + x] : 0;
+// Survivors arrive sorted by depth (level 1) together with their tile rectangles (ys = y0 | y1 << 16, xs = x0 | x1 << 16,
+// gathered by the last pass of the depth sort).  The list of tile T is {j : T in rect[j]} in ascending j, stored at
+// [ranges[T].x, ranges[T].y): a stable partition of the emission order by tile — what a stable sort of the (tile, id)
+// pairs by tile id produces.  The ranges are already known from the coverage grid, and the covered sets are rectangles,
+// i.e. x-intervals in every tile row, so no sort is needed.  One CTA owns (chunk c of RS-chunk consecutive survivors,
+// tile row y, block of RS_XB tile columns):
+//   1. filter: the CTA scans the chunk's y-ranges (4 bytes per survivor, coalesced) and keeps the survivors that cover
+//      its row — ballots, so the hits stay in depth order; their x-intervals go into a 1D difference array, whose prefix
+//      is the chunk's count for every tile of the row;
+//   2. the counts are published at once and the exclusive prefix over the earlier chunks of the same row is fetched by
+//      decoupled look-back (per tile column; chunk ids come from a ticket, so every predecessor is already running);
+//      ranges[T].x + that prefix = where this chunk starts writing in tile T;
+//   3. ranks inside the chunk: hit h (depth order) sets bit h in the bit mask of every tile it covers; the rank of a
+//      hit in a tile is the popcount of the lower bits — a prefix over the mask words plus one masked popcount.  Every
+//      (hit, tile) pair then stores its primitive id at its final position.  O(1) work per pair, 4 bytes written per
+//      pair; no key array, no sort, no per-pair search.
+// Replaces offsets scan + pair emission + 2-pass radix sort of the D pairs (round 1: 146 us per view at cfg3) and the
+// first round-2 design (per-chunk 2D coverage tables + ordered scatter in groups of 32 survivors: 150 us — its groups were
+// too small to amortise their barriers where the splats are small).
+constexpr int RS_THREADS = 256, RS_LC = 512, RS_WORDS = RS_LC / 32, RS_XB = 128;
+constexpr unsigned int RS_AGG = 1u << 30, RS_PRE = 2u << 30, RS_MASK = (1u << 30) - 1;
+
+__global__ void __launch_bounds__(RS_THREADS) row_scatter_kernel(WsHeader* hdr, const unsigned int* __restrict__ ys, const unsigned int* __restrict__ xs,
+                                                                 const unsigned int* __restrict__ ids, const uint2* __restrict__ ranges,
+                                                                 volatile unsigned int* lb_state, const int tiles_x, const int tiles_y,
+                                                                 const int xblocks, const unsigned int chunk, unsigned int* __restrict__ pair_ids) {
+  constexpr int UN = 8;                                // survivors per thread in flight: the scan is latency-bound otherwise
+  __shared__ unsigned int mask[RS_WORDS][RS_XB], pref[RS_WORDS][RS_XB];
+  __shared__ unsigned int list_j[RS_LC], list_x[RS_LC];
+  __shared__ unsigned int bal_s[RS_MAX_ITERS];
+  __shared__ unsigned short off[RS_MAX_ITERS + 2];     // exclusive prefix of the hit counts: <= RS_MAX_CHUNK = 32768
+  __shared__ int diff[RS_XB + 1];
+  __shared__ unsigned int cursor[RS_XB], s_ticket;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned int n = hdr->num_visible;
+  if (hdr->overflow) return;
+  const unsigned int per_chunk = (unsigned int)tiles_y * xblocks;
+  const int tiles = tiles_x * tiles_y;
+  // persistent CTAs: work items (chunk, row, column block) are taken from a ticket, chunk-major, until the survivors run out
+  while (true) {
+    __syncthreads();                                    // previous item finished with the shared arrays
+    if (threadIdx.x == 0) s_ticket = atomicAdd(&hdr->scan_ticket[1], 1u);
+    for (int i = threadIdx.x; i <= RS_XB; i += RS_THREADS) diff[i] = 0;
+    for (int i = threadIdx.x; i < RS_WORDS * RS_XB; i += RS_THREADS) (&mask[0][0])[i] = 0;
+    __syncthreads();
+    const unsigned int c = s_ticket / per_chunk, rr = s_ticket % per_chunk;
+    if ((unsigned long long)c * chunk >= n) return;     // tickets are dense: every chunk below this one exists
+    const int y = rr / xblocks, xbase = (rr % xblocks) * RS_XB, nx = min(RS_XB, tiles_x - xbase);
+    const unsigned int j0 = c * chunk, j1 = min(n, j0 + chunk);
+    const unsigned int iters = (j1 - j0 + 31) / 32, trips = (iters + RS_THREADS / 32 - 1) / (RS_THREADS / 32);
+    // Survivor j0 + 32 it + lane is lane `lane` of "iteration" it; thread (warp, lane) takes the iterations 8 i + warp.
+    // ---- 1. filter on the tile rows (and, with several column blocks, on the columns): one ballot per iteration ----
+    for (unsigned int i0 = 0; i0 < trips; i0 += UN) {
+      unsigned int yv[UN], xv[UN];
 #pragma unroll
-      for (int o = 1; o < 32; o <<= 1) { const int n = __shfl_up_sync(0xffffffffu, v, o); if (lane >= o) v += n; }
-      v += carry;
-      if (x < sx) grid[y * sx + x] = v;
-      carry = __shfl_sync(0xffffffffu, v, 31);
-    }
-  }
-  __syncthreads();
-  // column pass fused with the write-out: thread x walks down its column
-  unsigned int* out = chunk_base + (size_t)q * tiles_x * tiles_y;
-  for (int x = threadIdx.x; x < tiles_x; x += blockDim.x) {
-    int run = 0;
-    for (int y = 0; y < tiles_y; ++y) { run += grid[y * sx + x]; out[y * tiles_x + x] = (unsigned int)run; }
-  }
-}
-
-// exclusive prefix over the active chunks, per tile, in place; thread (g, t): chunk group g of CB_GROUPS, tile t of 32
-constexpr int CB_GROUPS = 8, CB_TILES = 32;
-__global__ void __launch_bounds__(CB_GROUPS * CB_TILES) chunk_base_kernel(const WsHeader* __restrict__ hdr, const uint2* __restrict__ ranges,
-                                                                            const unsigned int chunk_pairs, const int tiles,
-                                                                            unsigned int* __restrict__ chunk_base) {
-  __shared__ unsigned int part[CB_GROUPS][CB_TILES];
-  const unsigned int D = hdr->num_pairs;
-  if (D == 0) return;
-  const unsigned int nq = (D + chunk_pairs - 1) / chunk_pairs;         // active chunks
-  const int t = blockIdx.x * CB_TILES + (threadIdx.x & (CB_TILES - 1)), g = threadIdx.x / CB_TILES;
-  const unsigned int per = (nq + CB_GROUPS - 1) / CB_GROUPS, q0 = min(nq, g * per), q1 = min(nq, q0 + per);
-  unsigned int sum = 0;
-  if (t < tiles) for (unsigned int q = q0; q < q1; ++q) sum += chunk_base[(size_t)q * tiles + t];
-  part[g][threadIdx.x & (CB_TILES - 1)] = sum;
-  __syncthreads();
-  if (t >= tiles) return;
-  unsigned int run = ranges[t].x;
-  for (int gg = 0; gg < g; ++gg) run += part[gg][threadIdx.x & (CB_TILES - 1)];
-  for (unsigned int q = q0; q < q1; ++q) { const size_t i = (size_t)q * tiles + t; const unsigned int c = chunk_base[i]; chunk_base[i] = run; run += c; }
-}
-
-constexpr int SC_GROUP = 32;        // survivors ranked together (one bit each in the per-tile mask)
-constexpr int SC_STAGE = 1024;      // survivors staged in shared memory at a time
-template <bool CURSOR_SMEM>
-__global__ void __launch_bounds__(256) pair_scatter_kernel(const unsigned int* __restrict__ sorted_ids, const unsigned int* __restrict__ offsets,
-                                                           const ushort4* __restrict__ rect, const WsHeader* __restrict__ hdr,
-                                                           const unsigned int* __restrict__ chunk_first, const unsigned int chunk_pairs,
-                                                           const int tiles_x, const int tiles, unsigned int* __restrict__ chunk_base,
-                                                           unsigned int* __restrict__ pair_ids) {
-  extern __shared__ unsigned int sc_smem[];     // mask[tiles] (+ cursor[tiles] if CURSOR_SMEM)
-  __shared__ unsigned int s_off[SC_STAGE + 1], s_id[SC_STAGE];
-  __shared__ ushort4 s_rc[SC_STAGE];
-  const unsigned int D = hdr->num_pairs;
-  const unsigned int q = blockIdx.x;
-  if ((unsigned long long)q * chunk_pairs >= D) return;
-  unsigned int* mask = sc_smem;
-  unsigned int* cursor = CURSOR_SMEM ? sc_smem + tiles : chunk_base + (size_t)q * tiles;
-  for (int i = threadIdx.x; i < tiles; i += blockDim.x) { mask[i] = 0; if (CURSOR_SMEM) cursor[i] = chunk_base[(size_t)q * tiles + i]; }
-  const unsigned int j0 = chunk_first[q], j1 = chunk_first[q + 1];
-  for (unsigned int jb = j0; jb < j1; jb += SC_STAGE) {
-    const unsigned int m = min((unsigned int)SC_STAGE, j1 - jb);
-    __syncthreads();                                      // previous stage consumed; (first trip) mask / cursor initialised
-    for (unsigned int s = threadIdx.x; s < m; s += blockDim.x) {
-      const unsigned int id = sorted_ids[jb + s];
-      s_off[s] = offsets[jb + s]; s_id[s] = id; s_rc[s] = rect[id];
+      for (int u = 0; u < UN; ++u) {
+        const unsigned int j = j0 + (i0 + u) * RS_THREADS + threadIdx.x;
+        yv[u] = j < j1 ? ys[j] : 0u;                              // y0 = y1 = 0: covers no row
+        xv[u] = (xblocks > 1 && j < j1) ? xs[j] : 0xffff0000u;    // one column block: every x-interval intersects it
+      }
+#pragma unroll
+      for (int u = 0; u < UN; ++u) {
+        const unsigned int it = (i0 + u) * (RS_THREADS / 32) + warp;
+        const bool hit = (int)(yv[u] & 0xffffu) <= y && (int)(yv[u] >> 16) > y &&
+                         (int)(xv[u] & 0xffffu) < xbase + nx && (int)(xv[u] >> 16) > xbase;
+        const unsigned int bal = __ballot_sync(0xffffffffu, hit);
+        if (lane == 0 && it < iters) { bal_s[it] = bal; off[it] = (unsigned short)__popc(bal); }
+      }
     }
     __syncthreads();
-    if (threadIdx.x == 0) { const ushort4 rc = s_rc[m - 1]; s_off[m] = s_off[m - 1] + (unsigned int)(rc.z - rc.x) * (unsigned int)(rc.w - rc.y); }
+    if (warp == 0) {                          // exclusive prefix of the per-iteration hit counts
+      unsigned int carry = 0;
+      for (unsigned int i0 = 0; i0 < iters; i0 += 32) {
+        const unsigned int v = i0 + lane < iters ? off[i0 + lane] : 0;
+        unsigned int incl = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const unsigned int t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
+        if (i0 + lane < iters) off[i0 + lane] = (unsigned short)(carry + incl - v);
+        carry += __shfl_sync(0xffffffffu, incl, 31);
+      }
+      if (lane == 0) off[iters] = (unsigned short)carry;
+    }
     __syncthreads();
-    for (unsigned int g0 = 0; g0 < m; g0 += SC_GROUP) {   // groups of 32 survivors, in order
-      const unsigned int gm = min((unsigned int)SC_GROUP, m - g0);
-      const unsigned int e0 = s_off[g0], e1 = s_off[g0 + gm];
-      // a thread owns the pairs e0 + tid + 256 i; the first PC of them keep (tile, member) in registers across the phases
-      constexpr int PC = 4;
-      unsigned int ctile[PC], cbit[PC];
-      auto locate = [&](const unsigned int e, unsigned int& tile, unsigned int& bit) {
-        unsigned int lo = g0, hi = g0 + gm;                // largest s with s_off[s] <= e
-        while (hi - lo > 1) { const unsigned int mid = (lo + hi) >> 1; if (s_off[mid] <= e) lo = mid; else hi = mid; }
-        const ushort4 rc = s_rc[lo];
-        const unsigned int local = e - s_off[lo], w = rc.z - rc.x;
-        tile = (rc.y + local / w) * tiles_x + rc.x + local % w;
-        bit = lo - g0;
-      };
-      // phase 1: every pair of the group finds its member and tile, and sets its bit in the tile's mask
-#pragma unroll
-      for (int i = 0; i < PC; ++i) {
-        const unsigned int e = e0 + threadIdx.x + i * 256;
-        if (e < e1) { locate(e, ctile[i], cbit[i]); atomicOr(&mask[ctile[i]], 1u << cbit[i]); }
+    const unsigned int H = off[iters];
+    // ---- 2. rounds of up to RS_LC hits (depth order).  The first round also covers the difference array of ALL hits,
+    //         the publication of the counts and the look-back. ----
+    for (unsigned int r0 = 0; r0 < H || r0 == 0; r0 += RS_LC) {
+      if (r0 > 0) {
+        __syncthreads();                                // previous round consumed
+        for (int i = threadIdx.x; i < RS_WORDS * RS_XB; i += RS_THREADS) (&mask[0][0])[i] = 0;
+        __syncthreads();
       }
-      for (unsigned int e = e0 + threadIdx.x + PC * 256; e < e1; e += 256) { unsigned int t, b; locate(e, t, b); atomicOr(&mask[t], 1u << b); }
-      __syncthreads();
-      // phase 2: rank inside the group = members below me that cover the tile; the cursor is not touched yet
-#pragma unroll
-      for (int i = 0; i < PC; ++i) {
-        const unsigned int e = e0 + threadIdx.x + i * 256;
-        if (e < e1) pair_ids[cursor[ctile[i]] + __popc(mask[ctile[i]] & ((1u << cbit[i]) - 1u))] = s_id[g0 + cbit[i]];
-      }
-      for (unsigned int e = e0 + threadIdx.x + PC * 256; e < e1; e += 256) {
-        unsigned int t, b; locate(e, t, b);
-        pair_ids[cursor[t] + __popc(mask[t] & ((1u << b) - 1u))] = s_id[g0 + b];
+      // 2a. the hit list of the round, dense: thread it expands the ballot of iteration it
+      for (unsigned int it = threadIdx.x; it < iters; it += RS_THREADS) {
+        unsigned int bal = bal_s[it], h = off[it];
+        while (bal) {
+          const int bit = __ffs(bal) - 1;
+          bal &= bal - 1;
+          if (h >= r0 && h < r0 + RS_LC) list_j[h - r0] = j0 + it * 32 + bit;
+          ++h;
+        }
       }
       __syncthreads();
-      // phase 3: the highest member of a tile advances its cursor by the group's count and clears the mask
-#pragma unroll
-      for (int i = 0; i < PC; ++i) {
-        const unsigned int e = e0 + threadIdx.x + i * 256;
-        if (e < e1) { const unsigned int mk = mask[ctile[i]]; if ((mk >> cbit[i]) == 1u) { cursor[ctile[i]] += __popc(mk); mask[ctile[i]] = 0; } }
+      // 2b. one thread per hit: x-interval, bits into the masks of the tiles it covers (first round: every hit of the chunk
+      //     also enters the difference array, in strides of RS_LC)
+      const unsigned int m = H > r0 ? min((unsigned int)RS_LC, H - r0) : 0u;
+      for (unsigned int hl = threadIdx.x; hl < m; hl += RS_THREADS) {
+        const unsigned int xw = xs[list_j[hl]];
+        const unsigned int x0 = (unsigned int)max((int)(xw & 0xffffu) - xbase, 0), x1 = (unsigned int)min((int)(xw >> 16) - xbase, nx);
+        list_x[hl] = x0 | (x1 << 16);
+        if (r0 == 0) { atomicAdd(&diff[x0], 1); atomicAdd(&diff[x1], -1); }
+        const unsigned int bitv = 1u << (hl & 31);
+        for (unsigned int x = x0; x < x1; ++x) atomicOr(&mask[hl >> 5][x], bitv);
       }
-      for (unsigned int e = e0 + threadIdx.x + PC * 256; e < e1; e += 256) {
-        unsigned int t, b; locate(e, t, b);
-        const unsigned int mk = mask[t];
-        if ((mk >> b) == 1u) { cursor[t] += __popc(mk); mask[t] = 0; }
+      if (r0 == 0) {
+        if (H > RS_LC) {                      // rare: hits beyond the first round still count; walk the ballots for them
+          for (unsigned int it = threadIdx.x; it < iters; it += RS_THREADS) {
+            unsigned int bal = bal_s[it], h = off[it];
+            while (bal) {
+              const int bit = __ffs(bal) - 1;
+              bal &= bal - 1;
+              if (h >= RS_LC) {
+                const unsigned int xw = xs[j0 + it * 32 + bit];
+                atomicAdd(&diff[max((int)(xw & 0xffffu) - xbase, 0)], 1); atomicAdd(&diff[min((int)(xw >> 16) - xbase, nx)], -1);
+              }
+              ++h;
+            }
+          }
+        }
+        __syncthreads();
+        if (warp == 1) {                      // count of every tile column of the row = prefix of the difference array (RS_XB = 4 x 32)
+          int v[4], sum = 0;
+#pragma unroll
+          for (int k = 0; k < 4; ++k) { sum += diff[lane * 4 + k]; v[k] = sum; }
+          int incl = sum;
+#pragma unroll
+          for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
+#pragma unroll
+          for (int k = 0; k < 4; ++k) diff[lane * 4 + k] = incl - sum + v[k];
+        }
+        __syncthreads();
+        // publish the counts, look back over the earlier chunks of this row
+        if ((int)threadIdx.x < nx) {
+          const int t = y * tiles_x + xbase + threadIdx.x;
+          const unsigned int my_count = (unsigned int)diff[threadIdx.x];
+          volatile unsigned int* st = lb_state + t;
+          st[(size_t)c * tiles] = (c == 0 ? RS_PRE : RS_AGG) | my_count;
+          unsigned int excl = 0;
+          if (c > 0) {
+            for (long long cc = (long long)c - 1; cc >= 0; --cc) {
+              unsigned int v;
+              while (((v = st[(size_t)cc * tiles]) >> 30) == 0) __nanosleep(64);
+              excl += v & RS_MASK;
+              if ((v >> 30) == 2) break;
+            }
+            st[(size_t)c * tiles] = RS_PRE | (excl + my_count);
+          }
+          cursor[threadIdx.x] = ranges[t].x + excl;
+        }
+      }
+      __syncthreads();                                  // masks and list of this round complete (first round: cursor as well)
+      // 2c. ranks from the bit masks
+      if ((int)threadIdx.x < nx) {                      // per tile column: running count over the mask words
+        unsigned int run = cursor[threadIdx.x];
+#pragma unroll 8
+        for (int k = 0; k < RS_WORDS; ++k) { pref[k][threadIdx.x] = run; run += __popc(mask[k][threadIdx.x]); }
+        cursor[threadIdx.x] = run;
       }
       __syncthreads();
+      // 2d. ids to their final positions
+      for (unsigned int hl = threadIdx.x; hl < m; hl += RS_THREADS) {
+        const unsigned int id = ids[list_j[hl]], xw = list_x[hl], k = hl >> 5, below = (1u << (hl & 31)) - 1u;
+        for (unsigned int x = xw & 0xffffu; x < (xw >> 16); ++x) pair_ids[pref[k][x] + __popc(mask[k][x] & below)] = id;
+      }
     }
   }
 }
@@ -370,36 +352,15 @@ void launch_compact_and_tile_grid(const Workspace& ws, int N, int K, const ViewP
   count_launch();
 }
 
-void launch_offsets(const Workspace& ws, int l1_buf, int N, cudaStream_t st) {
+void launch_row_scatter(const Workspace& ws, int l1_buf, int N, const ViewParams& vp, int num_sms, cudaStream_t st) {
   if (N <= 0) return;
-  const int blocks = (N + SCAN_TILE - 1) / SCAN_TILE;
-  offsets_kernel<<<blocks, SCAN_THREADS, 0, st>>>(ws.tiles_touched, ws.l1_vals[l1_buf], ws.hdr, ws.scan_state[1], ws.offsets, ws.chunk_first,
-                                                  ws.chunk_pairs, ws.num_chunks);
+  const int xblocks = (vp.tiles_x + RS_XB - 1) / RS_XB;
+  // the survivor count lives on the device: persistent CTAs take (chunk, row, column block) items from a ticket
+  const unsigned long long items = (unsigned long long)ws.rs_chunks * (unsigned int)vp.tiles_y * xblocks;
+  const unsigned int blocks = (unsigned int)(items < 8ull * num_sms ? items : 8ull * num_sms);
+  row_scatter_kernel<<<blocks, RS_THREADS, 0, st>>>(ws.hdr, ws.sorted_ys, ws.sorted_xs, ws.l1_vals[l1_buf], ws.ranges, ws.rs_state, vp.tiles_x, vp.tiles_y,
+                                                    xblocks, ws.rs_chunk, ws.pair_ids);
   count_launch();
-}
-
-void launch_pair_scatter(const Workspace& ws, int l1_buf, int N, const ViewParams& vp, int num_sms, cudaStream_t st) {
-  if (N <= 0) return;
-  (void)num_sms;
-  const int tiles = vp.tiles_x * vp.tiles_y;
-  const size_t grid_smem = 4 * (size_t)(vp.tiles_x + 1) * (vp.tiles_y + 1);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(chunk_cover_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * MAX_GRID_CELLS);
-    cudaFuncSetAttribute(pair_scatter_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 8 * (MAX_GRID_CELLS / 2));
-    cudaFuncSetAttribute(pair_scatter_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * MAX_GRID_CELLS);
-    attr_set = true;
-  }
-  // D lives on the device: one CTA per possible chunk of the capacity, surplus CTAs exit at once
-  chunk_cover_kernel<<<ws.num_chunks, 256, grid_smem, st>>>(ws.l1_vals[l1_buf], ws.rect, ws.hdr, ws.chunk_first, ws.chunk_pairs, vp.tiles_x, vp.tiles_y, ws.chunk_base);
-  chunk_base_kernel<<<(tiles + CB_TILES - 1) / CB_TILES, CB_GROUPS * CB_TILES, 0, st>>>(ws.hdr, ws.ranges, ws.chunk_pairs, tiles, ws.chunk_base);
-  if (tiles <= MAX_GRID_CELLS / 2)
-    pair_scatter_kernel<true><<<ws.num_chunks, 256, 8 * (size_t)tiles, st>>>(ws.l1_vals[l1_buf], ws.offsets, ws.rect, ws.hdr, ws.chunk_first, ws.chunk_pairs,
-                                                                           vp.tiles_x, tiles, ws.chunk_base, ws.pair_ids);
-  else
-    pair_scatter_kernel<false><<<ws.num_chunks, 256, 4 * (size_t)tiles, st>>>(ws.l1_vals[l1_buf], ws.offsets, ws.rect, ws.hdr, ws.chunk_first, ws.chunk_pairs,
-                                                                            vp.tiles_x, tiles, ws.chunk_base, ws.pair_ids);
-  count_launch(3);
 }
 
 void launch_l1_loss(const float* image, const float* target, long long count, float* dL, float* loss, const unsigned int* overflow_flag,

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libfdgs.so")
 _lib = None
 
 OK, ERR_INVALID, ERR_WORKSPACE, ERR_CUDA, ERR_PAIR_OVERFLOW = 0, -1, -2, -3, -4
-(EXPORT_STATUS, EXPORT_RECORDS, EXPORT_RECTS, EXPORT_TILES_TOUCHED, EXPORT_OFFSETS, EXPORT_SORTED_KEYS,
+(EXPORT_STATUS, EXPORT_RECORDS, EXPORT_RECTS, EXPORT_TILES_TOUCHED, _EXPORT_UNUSED_4, EXPORT_SORTED_KEYS,
  EXPORT_SORTED_VALS, EXPORT_RANGES, EXPORT_SPLAT_GRADS, EXPORT_DEPTH_ORDER, EXPORT_SPLAT_GRAD_DEPTH) = range(11)
 
 EXPORTED_SYMBOLS = ["fdgs_default_config", "fdgs_workspace_bytes", "fdgs_preprocess", "fdgs_render_forward",
@@ -138,8 +138,7 @@ def launch_count() -> int:
     return int(load().fdgs_launch_count())
 
 
-STAGES = ("preprocess", "compact+tile_grid", "sort_depth", "offsets", "pair_scatter", "blend_fwd", "blend_bwd",
-          "preprocess_bwd")
+STAGES = ("preprocess", "compact+tile_grid", "sort_depth", "tile_lists", "blend_fwd", "blend_bwd", "preprocess_bwd")
 
 
 def set_stage_timing(on: bool):
@@ -418,7 +417,7 @@ class Renderer:
         if overflow:
             D = 0
         shapes = {EXPORT_RECORDS: ((N, 12), torch.float32), EXPORT_RECTS: ((N, 4), torch.int32),
-                  EXPORT_TILES_TOUCHED: ((N,), torch.int32), EXPORT_OFFSETS: ((nvis,), torch.int32),
+                  EXPORT_TILES_TOUCHED: ((N,), torch.int32),
                   EXPORT_SORTED_KEYS: ((D,), torch.int64), EXPORT_SORTED_VALS: ((D,), torch.int32),
                   EXPORT_RANGES: ((tiles, 2), torch.int32), EXPORT_SPLAT_GRADS: ((N, 9), torch.float32),
                   EXPORT_DEPTH_ORDER: ((nvis,), torch.int32), EXPORT_SPLAT_GRAD_DEPTH: ((N,), torch.float32)}

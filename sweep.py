@@ -56,7 +56,7 @@ def sweep_cfg5(frames, max_n, flush):
             cvs = [fdgs.make_view(sc.views[i]) for i in idx]
             ms, culled, pairs, nvis = [], [], [], []
             fdgs.set_stage_timing(True)
-            stage = {k: 0.0 for k in fdgs.STAGES[:6]}
+            stage = {k: 0.0 for k in fdgs.STAGES[:5]}
             for cv in cvs:
                 def frame():
                     r.preprocess(cv)
@@ -75,7 +75,7 @@ def sweep_cfg5(frames, max_n, flush):
             print(json.dumps({"config": "cfg5_sweep", "N": n, "width": w, "height": h, "frames": len(cvs), "fps": 1e3 / ms_frame,
                               "ms_per_frame": ms_frame, "ms_min": float(np.min(ms)), "ms_max": float(np.max(ms)),
                               "stage_ms": {"preprocess": stage["preprocess"],
-                                           "sort": stage["compact+tile_grid"] + stage["sort_depth"] + stage["offsets"] + stage["pair_scatter"],
+                                           "sort": stage["compact+tile_grid"] + stage["sort_depth"] + stage["tile_lists"],
                                            "blend": stage["blend_fwd"]},
                               "culled_by_marginal_fraction": float(np.mean(culled)), "visible_mean": float(np.mean(nvis)),
                               "pairs_mean": float(np.mean(pairs))}), flush=True)
@@ -154,7 +154,7 @@ def sort_compare(flush):
         r = fdgs.Renderer(ds, v.width, v.height, cap)
         cv = fdgs.make_view(v)
         fdgs.set_stage_timing(True)
-        ours = {k: 0.0 for k in fdgs.STAGES[1:5]}
+        ours = {k: 0.0 for k in fdgs.STAGES[1:4]}
         reps = 1 if ONCE else 10
         for _ in range(reps + 2):
             flush.fill_(1)
@@ -190,7 +190,7 @@ def sort_compare(flush):
         same = bool(torch.equal(keys_out.view(torch.int64), keys_sorted.view(torch.int64)))
         print(json.dumps({"config": "sort_compare_" + name, "N": sc.N, "pairs": D, "visible": status["num_visible"], "key_bits": end_bit,
                           "ours_ms": ours, "ours_total_ms": sum(ours.values()),
-                          "ours_sorts_only_ms": ours["sort_depth"] + ours["sort_tile"],
+                          "ours_sorts_only_ms": ours["sort_depth"] + ours["tile_lists"],
                           "cub_sortpairs_64bit_ms": ms_cub, "cub_keys_equal_ours": same,
                           "note": "ours_total includes compaction, tile ranges, offsets and pair emission; the CUB figure is the sort alone"}),
               flush=True)
