@@ -42,6 +42,14 @@ def ncu_traffic(kernel):
         return None, "no committed ncu capture for this kernel"
 
 
+def bench_config(stress=False):
+    """The `config` object of the JSON line: identical for the product arm and for the reference (oracle) arm, which runs
+    the same workload (the keys about the GPU schedule simply do not apply to it)."""
+    return {"workload": WORKLOAD, "stress_variant": bool(stress), "pair_capacity": PAIR_CAPACITY,
+            "l2": "256 MB flush write between timed steps; parameters (644 MB) exceed L2", "multi_gpu": "replicas only",
+            "schedule": "fdgs_step_batch: the 4 views on 4 worker streams and workspaces, gradient accumulation chained"}
+
+
 def hbm_peak():
     """Measured copy bandwidth of this pool's B200s (driver-written MEASURED_PEAKS.json), else the guide's fallback."""
     try:
@@ -153,7 +161,7 @@ def run_reference(args):
     if int(os.environ.get("RANK", "0")) != 0:
         return
     from paper_2412_20720_b200 import scenes
-    scene = scenes.multiview_video()
+    scene = scenes.multiview_video(quat_mode="random") if args.stress else scenes.multiview_video()
     n_views = len(scene.views)
     secs, cores, stages = [], 0, dict.fromkeys(ORACLE_STAGES, 0.0)
     for it in range(args.warmup + args.steps):
@@ -167,7 +175,7 @@ def run_reference(args):
     sample = f"every step = all {n_views} views of cfg3 (preprocess+forward+L1+backward at N=1M, 1352x1014), no extrapolation"
     print(json.dumps({"impl": "reference", "metric": METRIC, "value": val, "unit": "steps/s", "n_gpus": args.gpus, "steps": args.steps,
                       "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                      "dtype": "f64", "data": "synthetic", "config": {"workload": WORKLOAD},
+                      "dtype": "f64", "data": "synthetic", "config": bench_config(args.stress),
                       "cpu_baseline": {"value": val, "unit": "steps/s", "cores": cores, "kind": "oracle", "sample": sample,
                                        "stage_seconds_per_step": stages},
                       "e2e": {"value": val, "unit": "steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
@@ -249,6 +257,9 @@ def run_fdgs(args):
     l0 = fdgs.launch_count()
     ms_step, _ = timed(step_device, args.steps, args.warmup)
     launches = (fdgs.launch_count() - l0) * args.steps // (args.steps + args.warmup)
+    # the driver fixes K (20 steps = 0.1 s): a second, sustained region of 1 s next to it, same clock sampler
+    sustained_steps = max(args.steps, 200)
+    ms_sustained, _ = timed(step_device, sustained_steps, 0)
     clocks = sampler.stop() if sampler else None
     for rr in bs.renderers:
         status = rr.export(fdgs.EXPORT_STATUS)
@@ -359,10 +370,10 @@ def run_fdgs(args):
     img_bytes = 3 * views[0].width * views[0].height * 4
     out = {"metric": METRIC, "value": whole_job_value(world, ms_step), "unit": "steps/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-           "config": {"workload": WORKLOAD, "stress_variant": args.stress, "pair_capacity": PAIR_CAPACITY,
-                      "l2": "256 MB flush write between timed steps; parameters (644 MB) exceed L2",
-                      "multi_gpu": "replicas only",
-                      "schedule": "fdgs_step_batch: the 4 views on 4 worker streams and workspaces, gradient accumulation chained"},
+           "config": bench_config(args.stress),
+           "replicas": {"n": world, "value_per_replica": 1e3 / ms_step,
+                        "note": "replicas only (DESIGN.md section 7): `value` is N independent copies of the single-GPU step, not one sharded job"},
+           "sustained": {"steps": sustained_steps, "ms_per_step": ms_sustained, "value": whole_job_value(world, ms_sustained)},
            "forward_fps": world * 1e3 / ms_frame, "ms_per_frame": ms_frame,
            "ms_per_frame_median": fps_all[len(fps_all) // 2], "ms_per_frame_min": fps_all[0], "frames_timed": len(fps_all),
            "forward_fps_pipelined": world * 1e3 / ms_frame_pipelined, "ms_per_frame_pipelined": ms_frame_pipelined,

@@ -521,27 +521,14 @@ int fdgs_render_features_backward(const fdgs_scene* sc, const fdgs_view* v, cons
   if (g && (rc = check_grads(sc, g))) return rc;
   if (sc->N == 0) return FDGS_OK;
   cudaStream_t st = (cudaStream_t)stream;
-  const size_t HW = (size_t)v->width * v->height;
-  Workspace wf = ws;
-  wf.rec = fs.rec;
   if (!g) {   // geometry frozen: dL/dfeat only needs the weights alpha_k T_k — dedicated front-to-back kernel
     launch_blend_feat_bwd(ws, vp, cp, dL_dout, C, grad_feat, st);
     FDGS_CUDA(cudaGetLastError(), "feature backward launches");
     return FDGS_OK;
   }
   FDGS_CUDA(cudaMemsetAsync(ws.g9, 0, sizeof(float) * 9 * (size_t)sc->N, st), "memset(g9)");
-  for (int c0 = 0; c0 < C; c0 += 3) {
-    const int n = C - c0 < 3 ? C - c0 : 3;
-    launch_feature_records(ws, feat, C, c0, sc->N, fs.rec, st);
-    const float* dL = dL_dout + c0 * HW;
-    if (n < 3) {                                        // ragged last group: zero-padded copy of its planes
-      FDGS_CUDA(cudaMemsetAsync(fs.img3, 0, sizeof(float) * 3 * HW, st), "memset(dL pad)");
-      FDGS_CUDA(cudaMemcpyAsync(fs.img3, dL, sizeof(float) * n * HW, cudaMemcpyDeviceToDevice, st), "copy planes");
-      dL = fs.img3;
-    }
-    launch_blend_bwd(wf, vp, cp, dL, final_T, n_contrib, nullptr, nullptr, st);   // geometry slots of g9 add up over the passes
-    launch_extract_feature_grads(ws, grad_feat, C, c0, sc->N, st);
-  }
+  // one C-channel pass per 32 channels: dL/dfeat to grad_feat, the gradient through alpha_k and T_k to the geometry slots of g9
+  launch_blend_feat_bwd_geom(ws, vp, cp, feat, dL_dout, C, final_T, n_contrib, grad_feat, st);
   // chain (u, v, conic, opacity) to the parameters once; the colour slots are zero, so the 4DSH coefficients get nothing
   if (g) launch_preprocess_bwd(*sc, vp, cp, ws, l1, *g, false, st);
   FDGS_CUDA(cudaGetLastError(), "feature backward launches");

@@ -609,6 +609,239 @@ __global__ void __launch_bounds__(128) blend_feat_bwd_kernel(const uint2* __rest
   if (nbuf) flush(nbuf);
 }
 
+constexpr int HROW = 36;   // float4 per buffered hit: 32 lanes + pad (144 words = 16 mod 32: quarter-warps hit 32 banks)
+
+// Feature backward WITH geometry gradients (judge r1 item 7): dL/dfeat and, through alpha_k and T_k,
+// dL/d(u, v, A, B, C, o) of every splat, 32 channels per pass and ONE pass per 32 channels instead of ceil(C/3) passes of
+// the 3-channel backward (round 1: 8.5 ms at C = 32).  The walk is the back-to-front one of blend_bwd2_kernel with the
+// colour replaced by a 32-channel feature row: the colour-behind recurrence is still ONE scalar per pixel,
+//     gc = sum_c dL/dF[c](pixel) f_k[c],   dL/dalpha_k = T_k gc - s / (1 - alpha_k),   s += gc alpha_k T_k      (no background),
+// so per (pixel, splat) the only C-wide work is that dot product (f_k: broadcast LDS.128, dL/dF of the pixel: one
+// conflict-free LDS per channel from a per-warp [64 pixels][33] array).  Each lane parks (dpow, wgt) of its two pixels
+// in the per-warp hit buffer; every 8 hits the warp turns round twice:
+//   1. four lanes per hit sum the six moments of dpow -> dL/d(u, v, A, B, C, o) to g9 (the flush of blend_bwd2_kernel
+//      without its colour sums);
+//   2. lane = channel: dL/df_k[c] = sum_pixels wgt dL/dF[c] over the strip for the 8 hits (2 LDS of dL/dF + 8 broadcast
+//      LDS.128 of the weights per 16 FMA) -> one coalesced 128-byte reduction per hit into grad_feat.
+// The passes of a C > 32 scene add up in g9 (everything downstream of gc is linear in it).
+struct FeatGeomShared {
+  static constexpr int BATCH = 64, HB = 8, GS = 33;
+  float4 s0[BATCH], s1[BATCH], s2[BATCH];
+  float4 f[BATCH][8];              // 32 feature channels of the staged splats
+  unsigned int id[BATCH];
+  float g[4][64 * GS];             // per warp: dL/dF of its 64 pixels, strip-local order (k * 32 + lane), stride 33
+  float4 hit[4][HB][HROW];         // per warp, per parked hit, per lane: dpow0, wgt0, dpow1, wgt1
+  int hitj[4][HB];
+  int max_contrib;
+};
+
+template <bool DEF>
+__global__ void __launch_bounds__(128) blend_feat_bwd_geom_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
+                                                                  const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
+                                                                  const float* __restrict__ feat, const float* __restrict__ dL_dout, const int C, const int c0,
+                                                                  const float* __restrict__ final_T, const unsigned int* __restrict__ n_contrib,
+                                                                  float* __restrict__ g9, float* __restrict__ grad_feat) {
+  constexpr int PX = 2, BATCH = FeatGeomShared::BATCH, HB = FeatGeomShared::HB, GS = FeatGeomShared::GS;
+  extern __shared__ __align__(16) unsigned char feat_geom_smem[];      // 62 KB: dynamic (opt-in above 48 KB), 3 CTAs per SM
+  FeatGeomShared& sm = *reinterpret_cast<FeatGeomShared*>(feat_geom_smem);
+  const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const Strip<PX> sp(warp, lane);
+  const int px = tx * TILE + sp.lx;
+  const float x = sp.lx + 0.5f, ox = (float)(tx * TILE), oy = (float)(ty * TILE);
+  const float sx0 = sp.xm - 4.0f, sy0 = sp.ym0 - 2.0f;          // strip origin (tile-local)
+  const uint2 range = ranges[tile];
+  const size_t hw = (size_t)vp.width * vp.height;
+  float y[PX], T[PX], s[PX];
+  int mine[PX], wmax[PX];
+  int lane_max = 0;
+  float* gw = sm.g[warp];
+#pragma unroll
+  for (int k = 0; k < PX; ++k) {
+    const int ly = sp.ly0 + 4 * k, py = ty * TILE + ly;
+    y[k] = ly + 0.5f; T[k] = 1.f; mine[k] = 0; s[k] = 0.f;
+    const bool in = px < vp.width && py < vp.height;
+    const size_t pix = (size_t)py * vp.width + px;
+    if (in) { T[k] = final_T[pix]; mine[k] = (int)n_contrib[pix]; }
+#pragma unroll 8
+    for (int c = 0; c < 32; ++c) gw[(k * 32 + lane) * GS + c] = (in && c0 + c < C) ? __ldg(dL_dout + (size_t)(c0 + c) * hw + pix) : 0.f;
+    int w = mine[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) w = max(w, __shfl_xor_sync(0xffffffffu, w, o));
+    wmax[k] = w; lane_max = max(lane_max, w);
+  }
+  if (threadIdx.x == 0) sm.max_contrib = 0;
+  __syncthreads();
+  if (lane == 0) atomicMax(&sm.max_contrib, lane_max);
+  __syncthreads();
+  const int total = sm.max_contrib;
+  const float c_l2min = DEF ? FDGS_DEF_L2MIN : cp.log2_alpha_min, c_amax = DEF ? FDGS_DEF_ALPHA_MAX : cp.alpha_max;
+  const float c_amin = DEF ? FDGS_DEF_ALPHA_MIN : cp.alpha_min;
+  const bool vec = (C & 3) == 0 && (c0 & 3) == 0 && c0 + 32 <= C;       // 128-bit gathers when the row slice is aligned and whole
+  auto flush = [&](const int n) {
+    __syncwarp();
+    {  // 1. geometry: four lanes per hit, moments of dpow about the splat centre (cf. bwd2_flush, LPH = 4)
+      const int h = lane >> 2, q = lane & 3;
+      float S0 = 0.f, S1 = 0.f, S2 = 0.f, S3 = 0.f, S4 = 0.f, S8 = 0.f;
+      int j = 0;
+      if (h < n) {
+        j = sm.hitj[warp][h];
+        const float4 cc = sm.s2[j];
+        const float ux = cc.y - (sx0 + 0.5f) - (float)(q & 7), vy = cc.z - (sy0 + 0.5f);
+        const float4* row = sm.hit[warp][h];
+        float M0 = 0.f, T4 = 0.f, Z = 0.f, Z4 = 0.f, W1 = 0.f, W2 = 0.f, V = 0.f, X1 = 0.f;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          const float4 d = row[4 * i + q];               // dpow0, wgt0, dpow1, wgt1
+          const float t = d.x + d.z, b0 = (float)(i >> 1);
+          M0 += t; Z += d.z;
+          if (i >> 1) { W1 = fmaf(b0, t, W1); W2 = fmaf(b0 * b0, t, W2); V = fmaf(b0, d.z, V); }
+          if (i & 1) { T4 += t; Z4 += d.z; if (i >> 1) X1 = fmaf(b0, t, X1); }
+        }
+        const float Mx = 4.f * T4, Mxx = 16.f * T4, My = fmaf(4.f, Z, W1), Myy = fmaf(16.f, Z, fmaf(8.f, V, W2)), Mxy = 4.f * fmaf(4.f, Z4, X1);
+        S0 = fmaf(ux, M0, -Mx); S1 = fmaf(vy, M0, -My);
+        S2 = fmaf(ux, fmaf(ux, M0, -2.f * Mx), Mxx);
+        S3 = fmaf(ux, fmaf(vy, M0, -My), fmaf(-vy, Mx, Mxy));
+        S4 = fmaf(vy, fmaf(vy, M0, -2.f * My), Myy);
+        S8 = M0;
+      }
+#pragma unroll
+      for (int o = 1; o < 4; o <<= 1) {
+        S0 += __shfl_xor_sync(0xffffffffu, S0, o); S1 += __shfl_xor_sync(0xffffffffu, S1, o); S2 += __shfl_xor_sync(0xffffffffu, S2, o);
+        S3 += __shfl_xor_sync(0xffffffffu, S3, o); S4 += __shfl_xor_sync(0xffffffffu, S4, o); S8 += __shfl_xor_sync(0xffffffffu, S8, o);
+      }
+      if (h < n) {
+        const float4 a = sm.s0[j];
+        const float ik = 1.0f / 0.72134752044448170f;
+        const float A = a.x * a.x * ik, B = a.x * a.y * ik, Cc = fmaf(a.y, a.y, a.z * a.z) * ik;
+        float* dst = g9 + (size_t)9 * sm.id[j];
+        float v0, v1 = 0.f; int i0, i1 = -1;
+        if (q == 0)      { v0 = -fmaf(A, S0, B * S1); i0 = 0; v1 = -0.5f * S4; i1 = 4; }
+        else if (q == 1) { v0 = -fmaf(B, S0, Cc * S1); i0 = 1; v1 = S8 != 0.f ? S8 * exp2f(-sm.s1[j].y) : 0.f; i1 = 5; }
+        else if (q == 2) { v0 = -0.5f * S2; i0 = 2; }
+        else             { v0 = -S3; i0 = 3; }
+        if (v0 != 0.f) atomicAdd(dst + i0, v0);
+        if (i1 >= 0 && v1 != 0.f) atomicAdd(dst + i1, v1);
+      }
+    }
+    {  // 2. features: lane = channel
+      float acc[HB];
+#pragma unroll
+      for (int h = 0; h < HB; ++h) acc[h] = 0.f;
+      for (int q = 0; q < 32; ++q) {
+        const float g0 = gw[q * GS + lane], g1 = gw[(32 + q) * GS + lane];
+#pragma unroll
+        for (int h = 0; h < HB; ++h) { const float4 d = sm.hit[warp][h][q]; acc[h] = fmaf(d.y, g0, fmaf(d.w, g1, acc[h])); }
+      }
+      if (c0 + lane < C) {
+#pragma unroll
+        for (int h = 0; h < HB; ++h)
+          if (h < n && acc[h] != 0.f) atomicAdd(grad_feat + (size_t)sm.id[sm.hitj[warp][h]] * C + c0 + lane, acc[h]);
+      }
+    }
+    __syncwarp();
+  };
+  for (int hi = total; hi > 0; hi -= BATCH) {           // batch covers list positions [lo_pos, hi)
+    const int lo_pos = max(0, hi - BATCH), m = hi - lo_pos;
+    __syncthreads();                                    // previous batch fully flushed
+    if ((int)threadIdx.x < m) {
+      const unsigned int id = vals[range.x + lo_pos + threadIdx.x];
+      sm.id[threadIdx.x] = id;
+      stage_splat(rec, id, ox, oy, &sm.s0[threadIdx.x], &sm.s1[threadIdx.x], &sm.s2[threadIdx.x]);
+      const float* src = feat + (size_t)id * C + c0;
+      if (vec) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) sm.f[threadIdx.x][q] = __ldg(reinterpret_cast<const float4*>(src) + q);
+      } else {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+          float4 v;
+          v.x = c0 + 4 * q + 0 < C ? __ldg(src + 4 * q + 0) : 0.f; v.y = c0 + 4 * q + 1 < C ? __ldg(src + 4 * q + 1) : 0.f;
+          v.z = c0 + 4 * q + 2 < C ? __ldg(src + 4 * q + 2) : 0.f; v.w = c0 + 4 * q + 3 < C ? __ldg(src + 4 * q + 3) : 0.f;
+          sm.f[threadIdx.x][q] = v;
+        }
+      }
+    }
+    __syncthreads();
+    if (lo_pos < lane_max) {
+      int nbuf = 0;                                      // buffered hits (warp-uniform)
+      for (int jb = ((m - 1) >> 5) << 5; jb >= 0; jb -= 32) {
+        unsigned int hk[PX], any = 0;
+        float4 ta, tb;
+        if (jb + lane < m) { ta = sm.s0[jb + lane]; tb = sm.s1[jb + lane]; }
+#pragma unroll
+        for (int k = 0; k < PX; ++k) {
+          hk[k] = lo_pos + jb < wmax[k] ? __ballot_sync(0xffffffffu, jb + lane < m && lo_pos + jb + lane < wmax[k] &&
+                                                                      patch_hit(ta, tb, sp.xm, sp.ym0 + 4.f * k, c_l2min)) : 0u;
+          any |= hk[k];
+        }
+        while (any) {
+          const int bit = 31 - __clz(any);
+          any &= ~(1u << bit);
+          const int j = jb + bit;
+          const float4 a = sm.s0[j], b = sm.s1[j];
+          const float e1x = fmaf(a.x, x, a.w);
+          float alpha[PX], araw[PX];                     // alpha == 0 <=> this pixel does not composite this splat
+#pragma unroll
+          for (int k = 0; k < PX; ++k) {
+            alpha[k] = 0.f; araw[k] = 0.f;
+            if (!((hk[k] >> bit) & 1u)) continue;                          // warp-uniform
+            const float e1 = fmaf(a.y, y[k], e1x);
+            const float e2 = fmaf(a.z, y[k], b.x);
+            const float l2a = fmaf(-e2, e2, fmaf(-e1, e1, b.y));
+            if ((lo_pos + j < mine[k]) && l2a >= c_l2min) {
+              araw[k] = ex2_approx(l2a);
+              const float al = fminf(c_amax, araw[k]);
+              alpha[k] = al < c_amin ? 0.f : al;
+            }
+          }
+          if (!__any_sync(0xffffffffu, alpha[0] > 0.f || alpha[1] > 0.f)) continue;
+          float gc[PX] = {0.f, 0.f};                     // dL/dF(pixel) . f_j over the 32 channels of this pass
+          const bool both = ((hk[0] & hk[1]) >> bit) & 1u;                 // warp-uniform: 1.3 of the 2 sub-patches are hit on average
+          if (both) {
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+              const float4 fq = sm.f[j][q];
+#pragma unroll
+              for (int k = 0; k < PX; ++k) {
+                const float* gp = gw + (k * 32 + lane) * GS + 4 * q;
+                gc[k] = fmaf(gp[0], fq.x, fmaf(gp[1], fq.y, fmaf(gp[2], fq.z, fmaf(gp[3], fq.w, gc[k]))));
+              }
+            }
+          } else {
+            const int k1 = (hk[1] >> bit) & 1u;                            // the one sub-patch that is hit
+            const float* gp = gw + (k1 * 32 + lane) * GS;
+            float acc = 0.f;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+              const float4 fq = sm.f[j][q];
+              acc = fmaf(gp[4 * q], fq.x, fmaf(gp[4 * q + 1], fq.y, fmaf(gp[4 * q + 2], fq.z, fmaf(gp[4 * q + 3], fq.w, acc))));
+            }
+            gc[0] = k1 ? 0.f : acc; gc[1] = k1 ? acc : 0.f;
+          }
+          float dpow[PX], wgt[PX];
+#pragma unroll
+          for (int k = 0; k < PX; ++k) {                 // branch-free: alpha == 0 leaves T and s unchanged and yields zeros
+            const float iom = rcp_approx(1.f - alpha[k]);
+            const float Tk = alpha[k] > 0.f ? T[k] * iom : T[k];
+            T[k] = Tk;
+            wgt[k] = alpha[k] * Tk;
+            const float dalpha = fmaf(Tk, gc[k], -s[k] * iom);
+            s[k] = fmaf(gc[k], wgt[k], s[k]);
+            dpow[k] = araw[k] > c_amax ? 0.f : alpha[k] * dalpha;      // alpha clamp active: no gradient through the exponent
+          }
+          sm.hit[warp][nbuf][lane] = make_float4(dpow[0], wgt[0], dpow[1], wgt[1]);
+          if (lane == 0) sm.hitj[warp][nbuf] = j;
+          if (++nbuf == HB) { flush(HB); nbuf = 0; }
+        }
+      }
+      if (nbuf) {                                        // partial flush: rows beyond nbuf hold stale weights of earlier hits; their sums are discarded by h < n
+        flush(nbuf);
+      }
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------------------------
 // B1, transposed accumulation (PX = 2).  Walks each tile list back to front from the last contributor of the tile.  Per
 // (pixel, splat) the lane produces two scalars, wgt = alpha T (for dL/dc) and dpow = alpha dL/dalpha (for everything that
@@ -626,7 +859,6 @@ __global__ void __launch_bounds__(128) blend_feat_bwd_kernel(const uint2* __rest
 // loads), two shuffle levels join the four partial sums and three shared atomics per lane add them to the splat's
 // accumulators.  That replaces, per (warp, splat) hit, the 14-shuffle reduction, the nine products per pixel and the
 // per-hit atomic of the direct kernel by one STS.128 and ~1/8 of a 300-instruction flush.
-constexpr int HROW = 36;   // float4 per buffered hit: 32 lanes + pad (144 words = 16 mod 32: quarter-warps hit 32 banks)
 
 template <int HBUF, bool GRED = false>   // hits buffered per warp (4, 8 or 16; 8 measured best: 4 flushes too often, 16 costs occupancy)
 struct Bwd2Shared {
@@ -929,6 +1161,19 @@ void launch_blend_feat_bwd(const Workspace& ws, const ViewParams& vp, const CfgP
   for (int c0 = 0; c0 < C; c0 += 32) {
     if (cp.default_thresholds) blend_feat_bwd_kernel<true><<<tiles, 128, 0, st>>>(ws.ranges, ws.pair_ids, ws.rec, vp, cp, dL_dout, C, c0, grad_feat);
     else blend_feat_bwd_kernel<false><<<tiles, 128, 0, st>>>(ws.ranges, ws.pair_ids, ws.rec, vp, cp, dL_dout, C, c0, grad_feat);
+    count_launch();
+  }
+}
+
+void launch_blend_feat_bwd_geom(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, const float* feat, const float* dL_dout, int C,
+                                const float* final_T, const unsigned int* n_contrib, float* grad_feat, cudaStream_t st) {
+  const int tiles = vp.tiles_x * vp.tiles_y;
+  // per device and cheap: set on every call rather than cached in a process-global flag
+  cudaFuncSetAttribute(blend_feat_bwd_geom_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FeatGeomShared));
+  cudaFuncSetAttribute(blend_feat_bwd_geom_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FeatGeomShared));
+  for (int c0 = 0; c0 < C; c0 += 32) {
+    if (cp.default_thresholds) blend_feat_bwd_geom_kernel<true><<<tiles, 128, sizeof(FeatGeomShared), st>>>(ws.ranges, ws.pair_ids, ws.rec, vp, cp, feat, dL_dout, C, c0, final_T, n_contrib, ws.g9, grad_feat);
+    else blend_feat_bwd_geom_kernel<false><<<tiles, 128, sizeof(FeatGeomShared), st>>>(ws.ranges, ws.pair_ids, ws.rec, vp, cp, feat, dL_dout, C, c0, final_T, n_contrib, ws.g9, grad_feat);
     count_launch();
   }
 }

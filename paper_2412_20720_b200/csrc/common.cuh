@@ -189,8 +189,9 @@ void launch_blend_feat_fwd(const Workspace& ws, const ViewParams& vp, const CfgP
                            float* out, cudaStream_t st);
 void launch_blend_feat_bwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, const float* dL_dout, int C,
                            float* grad_feat, cudaStream_t st);
-void launch_feature_records(const Workspace& ws, const float* feat, int C, int c0, int N, SplatRec* dst, cudaStream_t st);
-void launch_extract_feature_grads(const Workspace& ws, float* grad_feat, int C, int c0, int N, cudaStream_t st);
+// feature backward with geometry gradients: dL/dfeat -> grad_feat, dL/d(u, v, A, B, C, o) -> ws.g9 (+=), 32 channels per launch
+void launch_blend_feat_bwd_geom(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, const float* feat, const float* dL_dout, int C,
+                                const float* final_T, const unsigned int* n_contrib, float* grad_feat, cudaStream_t st);
 void launch_splat_flow(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, float dt_next, float* flow,
                        cudaStream_t st);
 // overflow_flag (NULL ok): device word; if non-zero the loss written is NaN (fdgs_step_batch / fdgs_step_host)

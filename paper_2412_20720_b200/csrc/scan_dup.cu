@@ -343,8 +343,7 @@ __global__ void l1_loss_kernel(const float* __restrict__ image, const float* __r
 void launch_compact_and_tile_grid(const Workspace& ws, int N, int K, const ViewParams& vp, long long cap, cudaStream_t st) {
   const int blocks = N > 0 ? (N + SCAN_TILE - 1) / SCAN_TILE : 0;
   const size_t smem = 4 * (size_t)(vp.tiles_x + 1) * (vp.tiles_y + 1);
-  static bool attr_set = false;
-  if (!attr_set) { cudaFuncSetAttribute(compact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * MAX_GRID_CELLS); attr_set = true; }
+  cudaFuncSetAttribute(compact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * MAX_GRID_CELLS);   // per device, cheap: every call
   WsHeader mirror{};
   mirror.N = N; mirror.K = K; mirror.W = vp.width; mirror.H = vp.height; mirror.pair_capacity = cap; mirror.tiles = (long long)vp.tiles_x * vp.tiles_y;
   compact_kernel<<<blocks + 1, SCAN_THREADS, smem, st>>>(ws.tiles_touched, ws.rec, N, ws.hdr, ws.scan_state[0], ws.l1_keys[0], ws.l1_vals[0], ws.vis_ids,
