@@ -32,7 +32,7 @@ struct DeviceCtx {
   bool ready = false;
   int sms = 0;
   cudaStream_t worker[FDGS_MAX_BATCH] = {}, zero_stream = nullptr, copy_stream = nullptr;
-  cudaEvent_t batch_fork = nullptr, b2_done[FDGS_MAX_BATCH] = {}, zero_done = nullptr, copy_fork = nullptr, copy_join = nullptr;
+  cudaEvent_t batch_fork = nullptr, b2_done[FDGS_MAX_BATCH] = {}, copy_done[FDGS_MAX_BATCH] = {}, zero_done = nullptr, copy_fork = nullptr, copy_join = nullptr;
 };
 constexpr int MAX_DEVICES = 64;
 static DeviceCtx g_ctx[MAX_DEVICES];
@@ -50,6 +50,7 @@ static int device_ctx(DeviceCtx** out) {
     for (int i = 0; i < FDGS_MAX_BATCH; ++i) {
       FDGS_CUDA(cudaStreamCreateWithFlags(&c.worker[i], cudaStreamNonBlocking), "worker stream");
       FDGS_CUDA(cudaEventCreateWithFlags(&c.b2_done[i], cudaEventDisableTiming), "worker event");
+      FDGS_CUDA(cudaEventCreateWithFlags(&c.copy_done[i], cudaEventDisableTiming), "copy event");
     }
     FDGS_CUDA(cudaStreamCreateWithFlags(&c.zero_stream, cudaStreamNonBlocking), "zero stream");
     FDGS_CUDA(cudaStreamCreateWithFlags(&c.copy_stream, cudaStreamNonBlocking), "copy stream");
@@ -423,6 +424,15 @@ int fdgs_step_batch(const fdgs_scene* sc, const fdgs_view* views, int32_t num_vi
   }
   // From here on work is forked onto library streams: an error stops issuing, but every stream that was given work is
   // still joined into `st` before the call returns, so the caller can never free or reuse buffers under running kernels.
+  // host targets travel on the copy stream, view after view, while the views' preprocess and forward passes run: a view
+  // only waits for its own target right before its loss kernel
+  bool copies = false;
+  for (int i = 0; i < num_views; ++i) {
+    if (!bufs[i].target_host) continue;
+    if (!copies) { cudaStreamWaitEvent(ctx->copy_stream, ctx->batch_fork, 0); copies = true; }
+    cudaMemcpyAsync(bufs[i].target_dev, bufs[i].target_host, (size_t)3 * views[i].width * views[i].height * sizeof(float), cudaMemcpyHostToDevice, ctx->copy_stream);
+    cudaEventRecord(ctx->copy_done[i], ctx->copy_stream);
+  }
   int launched = 0;
   for (int i = 0; i < num_views && !rc; ++i) {
     const fdgs_view_buffers& b = bufs[i];
@@ -430,10 +440,10 @@ int fdgs_step_batch(const fdgs_scene* sc, const fdgs_view* views, int32_t num_vi
     const size_t count = (size_t)3 * views[i].width * views[i].height;
     cudaStreamWaitEvent(w, ctx->batch_fork, 0);
     launched = i + 1;
-    if (b.target_host) cudaMemcpyAsync(b.target_dev, b.target_host, count * sizeof(float), cudaMemcpyHostToDevice, w);
     cudaMemsetAsync(loss_dev + i, 0, sizeof(float), w);
     rc = fdgs_preprocess(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, nullptr, nullptr);
     if (!rc) rc = fdgs_render_forward(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, b.image, b.final_T, b.n_contrib);
+    if (b.target_host) cudaStreamWaitEvent(w, ctx->copy_done[i], 0);     // also on the error path: the copy is joined through this stream
     if (!rc) rc = step_loss(carve(b.ws, sc->N, K, views[i].width, views[i].height, cap), b.image, b.target_dev, (int64_t)count, b.dL_dimage, loss_dev + i, w);
     // blend backward of this view overlaps everything of the others; the gradient accumulation (B2) is chained
     if (!rc) rc = backward_impl(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, b.dL_dimage, b.final_T, b.n_contrib, g,
@@ -442,6 +452,7 @@ int fdgs_step_batch(const fdgs_scene* sc, const fdgs_view* views, int32_t num_vi
   }
   for (int i = 0; i < launched; ++i) cudaStreamWaitEvent(st, ctx->b2_done[i], 0);
   if (zero) cudaStreamWaitEvent(st, ctx->zero_done, 0);
+  if (copies) { cudaEventRecord(ctx->copy_join, ctx->copy_stream); cudaStreamWaitEvent(st, ctx->copy_join, 0); }
   if (rc) { cudaStreamSynchronize(st); return rc; }
   FDGS_CUDA(cudaGetLastError(), "batch launches");
   if (loss_host) {
