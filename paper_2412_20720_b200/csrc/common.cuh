@@ -67,7 +67,10 @@ constexpr int SORT_THREADS = 256;
 constexpr int SORT_ITEMS_L1 = 4;    // depth sort of <= N survivors: small tiles, more CTAs
 constexpr int DEPTH_PASSES = 32 / RADIX_BITS;
 constexpr int SCAN_THREADS = 256;
-constexpr int SCAN_ITEMS = 8;
+#ifndef FDGS_SCAN_ITEMS
+#define FDGS_SCAN_ITEMS 8
+#endif
+constexpr int SCAN_ITEMS = FDGS_SCAN_ITEMS;
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
 constexpr int RS_MIN_CHUNK = 2048, RS_MAX_CHUNK = 32768;   // survivors per chunk of the row scatter (scan_dup.cu)
 constexpr int RS_MAX_ITERS = RS_MAX_CHUNK / 32;

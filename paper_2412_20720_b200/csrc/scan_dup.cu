@@ -67,7 +67,13 @@ __device__ void tile_grid_role(const int* __restrict__ tile_diff, const int tile
                                WsHeader* hdr, const WsHeader mirror, uint2* __restrict__ ranges, int* grid, unsigned int* warp_sums) {
   const int sx = tiles_x + 1, rows = tiles_y + 1, cells = sx * rows, tiles = tiles_x * tiles_y;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-  for (int i = threadIdx.x; i < cells; i += blockDim.x) grid[i] = tile_diff[i];
+  for (int i0 = threadIdx.x; i0 < cells; i0 += 8 * blockDim.x) {      // eight independent loads per thread in flight
+    int v[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) v[k] = i0 + k * (int)blockDim.x < cells ? tile_diff[i0 + k * blockDim.x] : 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) if (i0 + k * (int)blockDim.x < cells) grid[i0 + k * blockDim.x] = v[k];
+  }
   __syncthreads();
   for (int y = warp; y < rows; y += nwarps) {             // inclusive scan along x, one warp per row
     int carry = 0;
@@ -82,19 +88,34 @@ __device__ void tile_grid_role(const int* __restrict__ tile_diff, const int tile
     }
   }
   __syncthreads();
-  for (int x = threadIdx.x; x < sx; x += blockDim.x) { int run = 0; for (int y = 0; y < rows; ++y) { run += grid[y * sx + x]; grid[y * sx + x] = run; } }
+  // columns by threads; eight loads in flight per step (a load never aliases the stores of the same step: another row)
+  for (int x = threadIdx.x; x < sx; x += blockDim.x) {
+    int run = 0;
+    for (int y0 = 0; y0 < rows; y0 += 8) {
+      int v[8];
+#pragma unroll
+      for (int k = 0; k < 8; ++k) v[k] = y0 + k < rows ? grid[(y0 + k) * sx + x] : 0;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) { run += v[k]; if (y0 + k < rows) grid[(y0 + k) * sx + x] = run; }
+    }
+  }
   __syncthreads();
-  // exclusive scan over tiles in row-major order; each thread owns a contiguous chunk
-  const int per = (tiles + blockDim.x - 1) / blockDim.x, t0 = threadIdx.x * per, t1 = min(t0 + per, tiles);
+  // exclusive scan over tiles in row-major order; each thread owns a contiguous chunk and walks it as (row, column)
+  const int per = (tiles + blockDim.x - 1) / blockDim.x, t0 = min((int)threadIdx.x * per, tiles), t1 = min(t0 + per, tiles);
+  const int ty0 = t0 / tiles_x, tx0 = t0 - ty0 * tiles_x;
   unsigned int sum = 0;
-  for (int t = t0; t < t1; ++t) sum += (unsigned int)grid[(t / tiles_x) * sx + (t % tiles_x)];
+  for (int t = t0, ty = ty0, tx = tx0; t < t1; ++t) {
+    sum += (unsigned int)grid[ty * sx + tx];
+    if (++tx == tiles_x) { tx = 0; ++ty; }
+  }
   unsigned int total;
   unsigned int run = block_exclusive_scan(sum, total, warp_sums);
   const bool overflow = total > cap;
-  for (int t = t0; t < t1; ++t) {
-    const unsigned int c = (unsigned int)grid[(t / tiles_x) * sx + (t % tiles_x)];
+  for (int t = t0, ty = ty0, tx = tx0; t < t1; ++t) {
+    const unsigned int c = (unsigned int)grid[ty * sx + tx];
     ranges[t] = overflow ? make_uint2(0, 0) : make_uint2(run, run + c);
     run += c;
+    if (++tx == tiles_x) { tx = 0; ++ty; }
   }
   if (threadIdx.x == 0) {
     hdr->num_pairs = overflow ? 0u : total; hdr->overflow = overflow ? 1u : 0u; hdr->total_pairs = total;
@@ -115,14 +136,17 @@ __global__ void __launch_bounds__(SCAN_THREADS) compact_kernel(const unsigned in
                                                                const WsHeader mirror, uint2* __restrict__ ranges) {
   extern __shared__ int grid[];                 // (tiles_y+1) x (tiles_x+1), used by CTA 0 only
   __shared__ unsigned int warp_sums[33], s_tile, s_prefix, hist[4][RADIX];
-  if (blockIdx.x == 0) { tile_grid_role(tile_diff, tiles_x, tiles_y, cap, hdr, mirror, ranges, grid, warp_sums); return; }
+  if (blockIdx.x == 0) {
+    tile_grid_role(tile_diff, tiles_x, tiles_y, cap, hdr, mirror, ranges, grid, warp_sums);
+    return;
+  }
   if (threadIdx.x == 0) s_tile = atomicAdd(&hdr->scan_ticket[0], 1u);
 #pragma unroll
   for (int p = 0; p < 4; ++p) hist[p][threadIdx.x] = 0;     // SCAN_THREADS == RADIX
   __syncthreads();
   const unsigned int tile = s_tile;
   const long long base = (long long)tile * SCAN_TILE + (long long)threadIdx.x * SCAN_ITEMS;
-  unsigned int flags = 0, cnt = 0;
+  unsigned int flags = 0, cnt = 0;   // SCAN_ITEMS <= 32 bits
 #pragma unroll
   for (int k = 0; k < SCAN_ITEMS; ++k)
     if (base + k < N && tiles_touched[base + k] > 0) { flags |= 1u << k; ++cnt; }
@@ -135,8 +159,19 @@ __global__ void __launch_bounds__(SCAN_THREADS) compact_kernel(const unsigned in
     if (flags & (1u << k)) {
       const unsigned int key = __float_as_uint(rec[base + k].depth);
       keys[pos] = key; vals[pos] = (unsigned int)(base + k); vis_ids[pos] = (unsigned int)(base + k); ++pos;
+      // digit counts of the four depth passes.  The two low digits of an fp32 depth are spread over all 256 bins; the two
+      // high ones (exponent and top mantissa bits) take a handful of values in a whole scene, so a plain shared atomic would
+      // serialise the CTA on one or two addresses (38 % of this kernel's stall samples): the lanes that are here together
+      // are grouped by digit first and one of each group adds the group's size
+      atomicAdd(&hist[0][key & (RADIX - 1)], 1u);
+      atomicAdd(&hist[1][(key >> RADIX_BITS) & (RADIX - 1)], 1u);
+      const unsigned int am = __activemask();
 #pragma unroll
-      for (int p = 0; p < 4; ++p) atomicAdd(&hist[p][(key >> (RADIX_BITS * p)) & (RADIX - 1)], 1u);
+      for (int p = 2; p < 4; ++p) {
+        const unsigned int d = (key >> (RADIX_BITS * p)) & (RADIX - 1);
+        const unsigned int peers = __match_any_sync(am, d);
+        if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&hist[p][d], (unsigned int)__popc(peers));
+      }
     }
   if (tile == gridDim.x - 2 && threadIdx.x == 0) hdr->num_visible = prefix + total;    // gridDim.x - 1 compaction tiles
   __syncthreads();

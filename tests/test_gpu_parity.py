@@ -124,6 +124,21 @@ def test_cfg4_reduced_heavy_tails():
     _full_parity(sc, dL_mode="l1", label="cfg4 40k 480x320")
 
 
+def test_wide_image_two_column_blocks_and_several_rounds_of_the_row_scatter():
+    """Row scatter edge cases: 2200 px = 138 tile columns, i.e. TWO column blocks of 128 per tile row, and a driving-style
+    scene whose large splats put far more than 512 hits of a chunk into one tile row (several mask rounds per work item);
+    N small enough for the minimum chunk (2048 survivors)."""
+    sc = scenes.driving(N=30000, width=2200, height=80, n_views=1)
+    rep, gpu, o = _full_parity(sc, dL_mode="l1", label="cfg4-style 30k 2200x80 (138 tile columns)")
+    off, _ = o.tile_lists()
+    assert len(off) - 1 == 138 * 5 and rep["num_pairs_gpu"] > 40_000
+    P = o.prims()
+    rect = P.rect[P.status == 0]
+    per_row = [int(((rect[:, 1] <= y) & (rect[:, 3] > y)).sum()) for y in range(5)]
+    assert max(per_row) > 512              # one (chunk, row) work item holds more than one round of hits
+    assert int((rect[:, 2] > 128).sum()) > 0 and int((rect[:, 0] < 128).sum()) > 0      # both column blocks are used
+
+
 @pytest.mark.parametrize("L,n_time", [(0, 1), (2, 1), (1, 3), (3, 2)])
 def test_sh_degree_variants(L, n_time):
     base = scenes.tiny()
