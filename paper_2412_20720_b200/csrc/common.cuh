@@ -64,7 +64,10 @@ struct WsHeader {
 constexpr int RADIX_BITS = 8;
 constexpr int RADIX = 1 << RADIX_BITS;
 constexpr int SORT_THREADS = 256;
-constexpr int SORT_ITEMS_L1 = 4;    // depth sort of <= N survivors: small tiles, more CTAs
+#ifndef FDGS_SORT_ITEMS
+#define FDGS_SORT_ITEMS 8
+#endif
+constexpr int SORT_ITEMS_L1 = FDGS_SORT_ITEMS;   // 2048-key tiles: 0.206 ms per 4 views at cfg3 (4: 0.212, 16: 0.259)    // depth sort of <= N survivors: small tiles, more CTAs
 constexpr int DEPTH_PASSES = 32 / RADIX_BITS;
 constexpr int SCAN_THREADS = 256;
 #ifndef FDGS_SCAN_ITEMS
