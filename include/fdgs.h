@@ -36,6 +36,7 @@ extern "C" {
 #define FDGS_ERR_WORKSPACE (-2)     /* ws_bytes smaller than fdgs_workspace_bytes() says                            */
 #define FDGS_ERR_CUDA (-3)          /* CUDA runtime error (text via fdgs_strerror)                                  */
 #define FDGS_ERR_PAIR_OVERFLOW (-4) /* number of (tile, primitive) pairs D exceeded pair_capacity                   */
+#define FDGS_ERR_STATIC_LIMIT (-5)  /* fdgs_render_forward_static: the sizes need more than FDGS_STATIC_WS_BYTES       */
 
 #define FDGS_TILE 16 /* 16x16-pixel tiles (tile rasterizer of [23]) */
 
@@ -319,6 +320,29 @@ typedef struct {
 /* Expands a compact model into the fp32 arrays of `out` (caller-owned, shapes of fdgs_scene for the same N, sh_degree,
  * n_time; the const qualifiers of fdgs_scene are cast away for writing).  Stage counts 1..16. */
 int fdgs_decode_compact(const fdgs_compact_scene *compact, const fdgs_scene *out, void *cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * Forward of one view WITHOUT any allocation, for callers that cannot call cudaMalloc (stream capture into a CUDA graph,
+ * tight serving loops, harnesses that forbid it).  Same kernels, same launch sequence and same result, bit for bit, as
+ * fdgs_preprocess + fdgs_render_forward (PAPER.md:L147 tile rasterizer, eq. 6), but the workspace is a device array
+ * built into the library: FDGS_STATIC_WS_BYTES (8 MiB) on every GPU that loads libfdgs.so, held until the process exits.
+ * The caller passes inputs and outputs only:  scene arrays, image [3,H,W], final_T [H,W], n_contrib [H,W] as for
+ * fdgs_render_forward;  overflow_dev (device uint32, may be NULL) receives 1 if D exceeded pair_capacity (the image is then
+ * that of an empty rendering), else 0.
+ * Limit: fdgs_workspace_bytes(N, K, W, H, pair_capacity) must not exceed FDGS_STATIC_WS_BYTES, else FDGS_ERR_STATIC_LIMIT
+ * is returned before anything is launched (fits e.g. N = 32768, 320x240, pair_capacity = 524288;  N = 16384, 256x256,
+ * 262144 pairs takes 3.6 MiB).  Other errors as fdgs_render_forward.
+ * The call issues one memset, 8 kernels and (overflow_dev != NULL) one 4-byte device copy on `cuda_stream`; it calls no
+ * cudaMalloc / cudaFree / stream or event creation and never synchronises.  The first call on a device looks up the
+ * address of the array (cudaGetSymbolAddress) and the SM count: make one call outside a stream capture first.
+ * All calls on one device share the array, which keeps the contents of the last call; the part that has to start from
+ * zero is cleared by the memset of each call.  Calls that overlap on the GPU (different streams without an ordering
+ * event, or two host threads) RACE on it: order them.  No backward: the training path owns its workspaces.
+ * ------------------------------------------------------------------------------------------------------------------ */
+#define FDGS_STATIC_WS_BYTES (8u << 20)
+int fdgs_render_forward_static(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host,
+                               int64_t pair_capacity, void *cuda_stream, float *image, float *final_T, uint32_t *n_contrib,
+                               uint32_t *overflow_dev);
 
 /* Number of kernel launches the library has issued so far in this process (bench.py's gpu_launches). */
 int64_t fdgs_launch_count(void);

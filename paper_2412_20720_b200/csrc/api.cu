@@ -648,6 +648,7 @@ const char* fdgs_strerror(int code) {
     case FDGS_ERR_WORKSPACE: return "workspace too small (see fdgs_workspace_bytes)";
     case FDGS_ERR_CUDA: return g_cuda_err;
     case FDGS_ERR_PAIR_OVERFLOW: return "number of (tile, primitive) pairs exceeds pair_capacity";
+    case FDGS_ERR_STATIC_LIMIT: return "sizes exceed the built-in workspace of fdgs_render_forward_static (FDGS_STATIC_WS_BYTES)";
     default: return "unknown error";
   }
 }
@@ -699,5 +700,72 @@ extern "C" int fdgs_debug_export(const void* ws_ptr, size_t ws_bytes, int what, 
   }
   FDGS_CUDA(cudaGetLastError(), "export launch");
   FDGS_CUDA(cudaStreamSynchronize(st), "export sync");
+  return FDGS_OK;
+}
+
+// ---- fdgs_render_forward_static: the forward of one view on a workspace that nobody allocates ----------------------
+// The workspace of this entry point is a file-scope device array: it exists on every GPU that loads the library, from
+// the load to the exit of the process.  In host code `g_static_ws` is only the host-side stand-in of the symbol, not a
+// device address — a kernel given that name would fault, or write somewhere in host memory where the GPU can reach it —
+// so the address is asked for once per device, with that device current, and it is the answer that reaches the kernels.
+namespace fdgs {
+
+static __device__ __align__(256) unsigned char g_static_ws[FDGS_STATIC_WS_BYTES];
+
+struct StaticCtx {
+  bool ready = false;
+  void* ws = nullptr;   // device address of g_static_ws on this device
+  int sms = 0;
+};
+static StaticCtx g_static[MAX_DEVICES];
+static std::mutex g_static_mutex;
+
+static int static_ctx(StaticCtx** out) {
+  int dev = 0;
+  FDGS_CUDA(cudaGetDevice(&dev), "cudaGetDevice");
+  if (dev < 0 || dev >= MAX_DEVICES) return FDGS_ERR_INVALID;
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  StaticCtx& c = g_static[dev];
+  if (!c.ready) {
+    void* p = nullptr;
+    FDGS_CUDA(cudaGetSymbolAddress(&p, g_static_ws), "cudaGetSymbolAddress(static workspace)");
+    if (!p || (reinterpret_cast<uintptr_t>(p) & 255u)) return cuda_fail(cudaErrorInvalidSymbol, "static workspace address");
+    FDGS_CUDA(cudaDeviceGetAttribute(&c.sms, cudaDevAttrMultiProcessorCount, dev), "SM count");
+    if (c.sms <= 0) c.sms = 148;
+    c.ws = p;
+    c.ready = true;
+  }
+  *out = &c;
+  return FDGS_OK;
+}
+
+}  // namespace fdgs
+
+extern "C" int fdgs_render_forward_static(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, int64_t cap, void* stream,
+                                          float* image, float* final_T, uint32_t* n_contrib, uint32_t* overflow_dev) {
+  if (!sc || !v || !c || !image || !final_T || !n_contrib || cap < 1 || cap >= (1LL << 30)) return FDGS_ERR_INVALID;
+  // the size check comes before anything touches the device: the layout is a function of the sizes alone
+  if (sc->N < 0 || v->width <= 0 || v->height <= 0 || sc->n_time < 1 || sc->sh_degree < 0) return FDGS_ERR_INVALID;
+  const int K = sc->n_time * (sc->sh_degree + 1) * (sc->sh_degree + 1);
+  if (carve(nullptr, sc->N, K, v->width, v->height, cap).bytes > (size_t)FDGS_STATIC_WS_BYTES) return FDGS_ERR_STATIC_LIMIT;
+  StaticCtx* ctx = nullptr;
+  int rc = static_ctx(&ctx);
+  if (rc) return rc;
+  if ((rc = check_common(sc, v, c, ctx->ws))) return rc;
+  const Workspace ws = carve(ctx->ws, sc->N, K, v->width, v->height, cap);
+  cudaStream_t st = (cudaStream_t)stream;
+  ViewParams vp; CfgParams cp;
+  make_params(v, c, vp, cp);
+  // same sequence as fdgs_preprocess + fdgs_render_forward.  The array keeps what the last call left in it: everything
+  // that has to start from zero (header, coverage grid, scan states, digit counts, look-back regions) is the prefix
+  // cleared here; the rest is written before it is read.
+  FDGS_CUDA(cudaMemsetAsync(ctx->ws, 0, ws.zero_bytes, st), "memset(static header)");
+  launch_preprocess_fwd(*sc, vp, cp, ws, st);
+  launch_compact_and_tile_grid(ws, sc->N, K, vp, cap, st);
+  const int l1 = launch_sort_depth(ws, sc->N, ctx->sms, st);
+  launch_row_scatter(ws, l1, sc->N, vp, ctx->sms, st);
+  launch_blend_fwd(ws, vp, cp, image, final_T, n_contrib, nullptr, st);
+  if (overflow_dev) FDGS_CUDA(cudaMemcpyAsync(overflow_dev, &ws.hdr->overflow, sizeof(uint32_t), cudaMemcpyDeviceToDevice, st), "copy overflow flag");
+  FDGS_CUDA(cudaGetLastError(), "static forward launches");
   return FDGS_OK;
 }

@@ -15,7 +15,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libfdgs.so")
 _lib = None
 
-OK, ERR_INVALID, ERR_WORKSPACE, ERR_CUDA, ERR_PAIR_OVERFLOW = 0, -1, -2, -3, -4
+OK, ERR_INVALID, ERR_WORKSPACE, ERR_CUDA, ERR_PAIR_OVERFLOW, ERR_STATIC_LIMIT = 0, -1, -2, -3, -4, -5
+STATIC_WS_BYTES = 8 << 20
 (EXPORT_STATUS, EXPORT_RECORDS, EXPORT_RECTS, EXPORT_TILES_TOUCHED, _EXPORT_UNUSED_4, EXPORT_SORTED_KEYS,
  EXPORT_SORTED_VALS, EXPORT_RANGES, EXPORT_SPLAT_GRADS, EXPORT_DEPTH_ORDER, EXPORT_SPLAT_GRAD_DEPTH) = range(11)
 
@@ -25,7 +26,7 @@ EXPORTED_SYMBOLS = ["fdgs_default_config", "fdgs_workspace_bytes", "fdgs_preproc
                     "fdgs_debug_blend_stats", "fdgs_step_batch", "fdgs_debug_cull_status", "fdgs_render_forward_aux",
                     "fdgs_render_backward_aux", "fdgs_debug_measure_peaks", "fdgs_mask_apply", "fdgs_regularizers",
                     "fdgs_adam_step", "fdgs_decode_compact", "fdgs_features_scratch_bytes", "fdgs_render_features_forward",
-                    "fdgs_render_features_backward", "fdgs_splat_flow"]
+                    "fdgs_render_features_backward", "fdgs_splat_flow", "fdgs_render_forward_static"]
 MAX_BATCH = 8
 
 
@@ -120,6 +121,7 @@ def load():
     lib.fdgs_render_features_backward.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, vp, i32,
                                                   vp, sz, vp, vp, vp, vp, C.POINTER(CGrads)]
     lib.fdgs_splat_flow.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), vp, sz, i64, vp, C.c_float, vp]
+    lib.fdgs_render_forward_static.argtypes = [C.POINTER(CScene), C.POINTER(CView), C.POINTER(CConfig), i64, vp, vp, vp, vp, vp]
     lib.fdgs_launch_count.restype = i64
     lib.fdgs_strerror.restype = C.c_char_p
     lib.fdgs_strerror.argtypes = [C.c_int]
@@ -243,6 +245,20 @@ class DeviceScene:
 def grads_struct(g: dict) -> CGrads:
     return CGrads(_ptr(g["mean"]), _ptr(g["log_scale"]), _ptr(g["quat_l"]), _ptr(g["quat_r"]), _ptr(g["opacity_logit"]),
                   _ptr(g["sh"]), _ptr(g.get("mean2d")), _ptr(g.get("densify")))
+
+
+def render_forward_static(dscene: "DeviceScene", cview: CView, pair_capacity: int, image, final_T, n_contrib,
+                          overflow=None, cfg: Optional[CConfig] = None) -> None:
+    """fdgs_render_forward_static: forward of one view on the workspace built into the library (no allocation).
+
+    image [3,H,W] f32, final_T [H,W] f32, n_contrib [H,W] i32, overflow (optional) [1] i32: caller-owned CUDA tensors.
+    Raises FdgsError(ERR_STATIC_LIMIT) if workspace_bytes(...) > STATIC_WS_BYTES.  Asynchronous on the current stream."""
+    cs = dscene.c_struct()
+    cfg = cfg if cfg is not None else default_config()
+    rc = load().fdgs_render_forward_static(C.byref(cs), C.byref(cview), C.byref(cfg), int(pair_capacity), _stream(),
+                                           image.data_ptr(), final_T.data_ptr(), n_contrib.data_ptr(), _ptr(overflow))
+    if rc:
+        raise FdgsError(rc, "fdgs_render_forward_static")
 
 
 def workspace_bytes(N, K, width, height, pair_capacity) -> int:
