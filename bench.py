@@ -47,7 +47,7 @@ def bench_config(stress=False):
     the same workload (the keys about the GPU schedule simply do not apply to it)."""
     return {"workload": WORKLOAD, "stress_variant": bool(stress), "pair_capacity": PAIR_CAPACITY,
             "l2": "256 MB flush write between timed steps; parameters (644 MB) exceed L2", "multi_gpu": "replicas only",
-            "schedule": "fdgs_step_batch: the 4 views on 4 worker streams and workspaces, gradient accumulation chained"}
+            "schedule": "fdgs_step_batch: the 4 views on 4 worker streams and workspaces; backward preprocess of the batch after the last blend (one colour pass over the union of the views' survivors, geometry view after view)"}
 
 
 def hbm_peak():

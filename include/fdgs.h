@@ -158,9 +158,12 @@ int fdgs_step_host(const fdgs_scene *scene, const fdgs_view *view_host, const fd
  * preprocess + forward + L1 loss against its target + backward, gradients of all views accumulated into `grads_host`
  * (+=; the caller zeroes them).  The views run on library-owned worker streams forked from and joined to `cuda_stream`
  * by events, each on its OWN workspace and buffers, so the latency-bound stages of one view (scans, sorts) overlap the
- * blend kernels of the others; only the gradient accumulation into the shared arrays (second half of the backward) is
- * chained view after view, because it is a non-atomic read-modify-write.  The accumulated result is the same as calling
- * the three functions view by view, up to fp32 summation order of the blend atomics.
+ * blend kernels of the others.  The second half of the backward (B2, the accumulation into the shared gradient arrays, a
+ * non-atomic read-modify-write) follows when the blend backward of every view is done: with sh_degree 3, n_time <= 4 and
+ * num_views <= 4 its colour part is ONE pass over the primitives for all views — the coefficient block of a primitive seen
+ * by several views of the batch is read once and its gradient block read and written once (written only, under
+ * FDGS_STEP_ZERO_GRADS) — followed by the geometry part view after view; otherwise B2 runs per view, chained.  The
+ * accumulated result is the same as calling the three functions view by view, up to fp32 summation order.
  *   bufs_host[i].target_host  != NULL: [3,H,W] pinned host image, copied to target_dev inside the call;
  *                             == NULL: target_dev already holds the target.
  *   loss_dev [num_views] device floats: loss of each view (overwritten); NaN for a view whose pairs exceeded

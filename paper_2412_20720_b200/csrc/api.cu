@@ -296,7 +296,8 @@ int fdgs_render_forward_aux(const fdgs_scene* sc, const fdgs_view* v, const fdgs
 // non-atomic gradient read-modify-writes of concurrent views while their blend kernels overlap.
 static int backward_impl(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes, int64_t cap,
                          cudaStream_t st, const float* dL_dimage, const float* final_T, const uint32_t* n_contrib,
-                         const fdgs_grads* g, cudaEvent_t before_b2, const float* dL_ddepth = nullptr, const float* dL_dopacity = nullptr) {
+                         const fdgs_grads* g, cudaEvent_t before_b2, const float* dL_ddepth = nullptr, const float* dL_dopacity = nullptr,
+                         bool b1_only = false) {
   int rc = check_common(sc, v, c, ws_ptr);
   if (rc) return rc;
   if (!dL_dimage || !final_T || !n_contrib || cap < 1 || cap >= (1LL << 30)) return FDGS_ERR_INVALID;
@@ -313,6 +314,7 @@ static int backward_impl(const fdgs_scene* sc, const fdgs_view* v, const fdgs_co
   mark(EV_BWD0, st);
   launch_blend_bwd(ws, vp, cp, dL_dimage, final_T, n_contrib, dL_ddepth, dL_dopacity, st);   // B1
   mark(EV_BWD1, st);
+  if (b1_only) { FDGS_CUDA(cudaGetLastError(), "backward launches"); return FDGS_OK; }     // fdgs_step_batch: B2 of all views follows in one pass
   if (before_b2) FDGS_CUDA(cudaStreamWaitEvent(st, before_b2, 0), "wait before B2");
   launch_preprocess_bwd(*sc, vp, cp, ws, l1, *g, aux, st);                      // B2
   mark(EV_BWD2, st);
@@ -433,6 +435,8 @@ int fdgs_step_batch(const fdgs_scene* sc, const fdgs_view* views, int32_t num_vi
     cudaMemcpyAsync(bufs[i].target_dev, bufs[i].target_host, (size_t)3 * views[i].width * views[i].height * sizeof(float), cudaMemcpyHostToDevice, ctx->copy_stream);
     cudaEventRecord(ctx->copy_done[i], ctx->copy_stream);
   }
+  // sh_degree 3 with up to 4 Fourier orders and up to 4 views (every benchmark configuration): one colour pass for the whole batch
+  const bool batched_b2 = sc->sh_degree == 3 && sc->n_time <= 4 && num_views > 1 && num_views <= 4;
   int launched = 0;
   for (int i = 0; i < num_views && !rc; ++i) {
     const fdgs_view_buffers& b = bufs[i];
@@ -445,10 +449,28 @@ int fdgs_step_batch(const fdgs_scene* sc, const fdgs_view* views, int32_t num_vi
     if (!rc) rc = fdgs_render_forward(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, b.image, b.final_T, b.n_contrib);
     if (b.target_host) cudaStreamWaitEvent(w, ctx->copy_done[i], 0);     // also on the error path: the copy is joined through this stream
     if (!rc) rc = step_loss(carve(b.ws, sc->N, K, views[i].width, views[i].height, cap), b.image, b.target_dev, (int64_t)count, b.dL_dimage, loss_dev + i, w);
-    // blend backward of this view overlaps everything of the others; the gradient accumulation (B2) is chained
+    // blend backward of this view overlaps everything of the others.  B2: with the batched colour pass every view stops
+    // after B1 and the backward preprocess of all views follows below; otherwise B2 runs here, chained view after view
     if (!rc) rc = backward_impl(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, b.dL_dimage, b.final_T, b.n_contrib, g,
-                                i > 0 ? ctx->b2_done[i - 1] : (zero ? ctx->zero_done : nullptr));
+                                batched_b2 ? nullptr : (i > 0 ? ctx->b2_done[i - 1] : (zero ? ctx->zero_done : nullptr)), nullptr, nullptr, batched_b2);
     cudaEventRecord(ctx->b2_done[i], w);
+  }
+  if (batched_b2 && !rc && launched == num_views) {
+    // One pass over the primitives does the colour part (A4) for every view that sees them: coefficient and gradient
+    // blocks of a primitive shared by several views move once.  Then the geometry part view by view (each reads its own
+    // dcol and read-modify-writes the caller's arrays, so they stay in order on one stream).
+    cudaStream_t w0 = ctx->worker[0];
+    for (int i = 1; i < num_views; ++i) cudaStreamWaitEvent(w0, ctx->b2_done[i], 0);
+    if (zero) cudaStreamWaitEvent(w0, ctx->zero_done, 0);
+    Workspace wss[FDGS_MAX_BATCH]; float inv_T[FDGS_MAX_BATCH];
+    for (int i = 0; i < num_views; ++i) { wss[i] = carve(bufs[i].ws, sc->N, K, views[i].width, views[i].height, cap); inv_T[i] = 1.0f / views[i].period_T; }
+    launch_colour_bwd_batch(*sc, num_views, wss, inv_T, *g, zero, w0);
+    for (int i = 0; i < num_views; ++i) {
+      ViewParams vp; CfgParams cp;
+      make_params(&views[i], c, vp, cp);
+      launch_geom_bwd(*sc, vp, cp, wss[i], *g, w0);
+    }
+    cudaEventRecord(ctx->b2_done[0], w0);
   }
   for (int i = 0; i < launched; ++i) cudaStreamWaitEvent(st, ctx->b2_done[i], 0);
   if (zero) cudaStreamWaitEvent(st, ctx->zero_done, 0);

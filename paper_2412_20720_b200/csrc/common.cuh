@@ -190,6 +190,12 @@ void launch_blend_bwd(const Workspace& ws, const ViewParams& vp, const CfgParams
                       cudaStream_t st);
 void launch_preprocess_bwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, int l1_buf,
                            const fdgs_grads& g, bool with_gz, cudaStream_t st);
+// batched step: colour part of the backward preprocess of all V views in one pass (false: not available for this scene),
+// and the geometry part of one view
+// grads_are_zero: g.sh was cleared for this step, so the pass writes its sums instead of adding to what it would have to read
+bool launch_colour_bwd_batch(const fdgs_scene& sc, int V, const Workspace* ws, const float* inv_T, const fdgs_grads& g, bool grads_are_zero,
+                             cudaStream_t st);
+void launch_geom_bwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, const fdgs_grads& g, cudaStream_t st);
 void launch_cull_status(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, unsigned char* dst, cudaStream_t st);
 void launch_blend_feat_fwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, const float* feat, int C,
                            float* out, cudaStream_t st);

@@ -226,6 +226,150 @@ __global__ void __launch_bounds__(128) colour_bwd16_kernel(const float* __restri
   }
 }
 
+// K8a for a BATCH of up to 4 views (fdgs_step_batch, sh_degree 3): the colour backward of all V views of a step in one pass
+// over the primitives.  A primitive that survives in several views of the batch (54 % of the (view, survivor) pairs of cfg3
+// fall on primitives seen by another view too) has its 12K-byte coefficient block read once and its gradient block
+// read-modified-written once, instead of once per view: both stay in registers (NT Fourier orders x 12 floats each per lane)
+// while the views that see the primitive are walked.  A warp owns 32 consecutive primitives, finds the members of the
+// union by ballot and serves 8 of them per round:
+//   phase 1  lane (member g, view l): loads that view's direction / time offset (aux), clamp flags (stored colour > 0) and
+//            dL/dc (g9) of the member and writes one table row to shared memory: Y[16], dY/d(x,y,z)[48], masked dL/dc,
+//            cos / -omega sin of the Fourier orders — every (member, view) pair costs one lane, all loads of a round are
+//            independent;
+//   phase 2  the 4 lanes of a member (SH orders 4l .. 4l+3, as in colour_bwd16_kernel) walk the views that see it, reading
+//            their quarter of the row; dL/d(dir, dt) of each (member, view) goes to that view's dcol.
+struct BatchColourArgs {
+  int V;
+  float inv_T[4];
+  const unsigned int* tiles_touched[4];
+  const float4* aux[4];
+  const SplatRec* rec[4];
+  const float* g9[4];
+  float4* dcol[4];
+};
+constexpr int CU_ROW = 76;      // floats per table row: Y 16 | G 48 | gc 3, pad | cos 4 | -omega sin 4
+
+#define FDGS_SEL4(arr, i) ((i) == 0 ? (arr)[0] : (i) == 1 ? (arr)[1] : (i) == 2 ? (arr)[2] : (arr)[3])
+
+// ZERO: the caller's gradient array was cleared for this step (FDGS_STEP_ZERO_GRADS): nothing to read, the sums are written.
+template <int NT, bool ZERO>
+__global__ void __launch_bounds__(128) colour_bwd16_union_kernel(const float* __restrict__ sh, const int N, const BatchColourArgs A,
+                                                                 float* __restrict__ dsh) {
+  __shared__ __align__(16) float tab[4][32][CU_ROW];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, grp = lane >> 2, l = lane & 3;
+  const int warp_base = (blockIdx.x * (blockDim.x >> 5) + warp) * 32;
+  if (warp_base >= N) return;
+  unsigned int seen = 0;                                        // bit v: this lane's primitive survives in view v
+  if (warp_base + lane < N) {
+#pragma unroll
+    for (int v = 0; v < 4; ++v) if (v < A.V) seen |= (__ldg(A.tiles_touched[v] + warp_base + lane) > 0u ? 1u : 0u) << v;
+  }
+  unsigned int members = __ballot_sync(0xffffffffu, seen != 0u);
+  constexpr int rec_len = NT * 48;
+#pragma unroll 1
+  while (members) {                                             // warp-uniform: 8 members of the union per round
+    const unsigned int src = __fns(members, 0, grp + 1);        // lane of the grp-th member, 0xffffffff if there is none
+    const bool valid = src != 0xffffffffu;
+    const unsigned int seen_src = __shfl_sync(0xffffffffu, seen, valid ? src : 0);
+    const unsigned int vm = valid ? seen_src : 0u;        // views that see this member
+    const int id = warp_base + (valid ? (int)src : 0);
+    float4 c[NT][3], d[NT][3];
+    float4* d4p = reinterpret_cast<float4*>(dsh + (size_t)id * rec_len) + 3 * l;
+    if (valid) {
+      const float4* c4p = reinterpret_cast<const float4*>(sh + (size_t)id * rec_len) + 3 * l;
+#pragma unroll
+      for (int n = 0; n < NT; ++n) { ld_nc_f4(c4p + 12 * n, c[n][0]); ld_nc_f4(c4p + 12 * n + 1, c[n][1]); ld_nc_f4(c4p + 12 * n + 2, c[n][2]); }
+      if (!ZERO) {
+#pragma unroll
+        for (int n = 0; n < NT; ++n) { ld_f4(d4p + 12 * n, d[n][0]); ld_f4(d4p + 12 * n + 1, d[n][1]); ld_f4(d4p + 12 * n + 2, d[n][2]); }
+      }
+    }
+    if (ZERO) {
+#pragma unroll
+      for (int n = 0; n < NT; ++n) d[n][0] = d[n][1] = d[n][2] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    // ---- phase 1: lane (grp, l) = (member, view l)
+    float* row = tab[warp][lane];
+    if ((vm >> l) & 1u) {
+      const float4 a = __ldg(FDGS_SEL4(A.aux, l) + id);
+      const SplatRec* rp = FDGS_SEL4(A.rec, l) + id;
+      const float* gp = FDGS_SEL4(A.g9, l) + (size_t)9 * id;
+      const float4 q1 = __ldg(reinterpret_cast<const float4*>(rp) + 1);
+      const float cbl = __ldg(reinterpret_cast<const float*>(rp) + 8);
+      const float g6 = __ldg(gp + 6), g7 = __ldg(gp + 7), g8 = __ldg(gp + 8);
+      const float inv_T = FDGS_SEL4(A.inv_T, l);
+      float Yf[16], Gf[48];
+      sh_basis<16>(a.x, a.y, a.z, Yf);
+      sh_grad_table<16>(a.x, a.y, a.z, Gf);
+      float4* r4 = reinterpret_cast<float4*>(row);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) r4[k] = make_float4(Yf[4 * k], Yf[4 * k + 1], Yf[4 * k + 2], Yf[4 * k + 3]);
+#pragma unroll
+      for (int k = 0; k < 12; ++k) r4[4 + k] = make_float4(Gf[4 * k], Gf[4 * k + 1], Gf[4 * k + 2], Gf[4 * k + 3]);
+      // the colour clamp at 0 was active iff the stored (clamped) colour is 0: those channels carry no gradient
+      r4[16] = make_float4(q1.z > 0.f ? g6 : 0.f, q1.w > 0.f ? g7 : 0.f, cbl > 0.f ? g8 : 0.f, 0.f);
+      float cn[4] = {0.f, 0.f, 0.f, 0.f}, wsn[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+      for (int n = 0; n < NT; ++n) {
+        cn[n] = cospif(2.0f * (float)n * a.w);
+        wsn[n] = -6.283185307179586f * (float)n * inv_T * sinpif(2.0f * (float)n * a.w);
+      }
+      r4[17] = make_float4(cn[0], cn[1], cn[2], cn[3]);
+      r4[18] = make_float4(wsn[0], wsn[1], wsn[2], wsn[3]);
+    }
+    __syncwarp();
+    // ---- phase 2: the 4 lanes of a member walk the views that see it
+    unsigned int rem = vm;
+    float4 mine = make_float4(0.f, 0.f, 0.f, 0.f);              // lane l keeps dL/d(dir, dt) of view l
+#pragma unroll 1
+    while (__any_sync(0xffffffffu, rem != 0u)) {
+      const bool act = rem != 0u;
+      const int v = act ? __ffs(rem) - 1 : 0;
+      rem &= rem - 1;
+      float ax = 0.f, ay = 0.f, az = 0.f, ad = 0.f;
+      if (act) {
+        const float4* r4 = reinterpret_cast<const float4*>(tab[warp][4 * grp + v]);
+        const float4 y4 = r4[l], ga = r4[4 + 3 * l], gb = r4[5 + 3 * l], gcv = r4[6 + 3 * l], g4 = r4[16], cn4 = r4[17], ws4 = r4[18];
+        const float Y[4] = {y4.x, y4.y, y4.z, y4.w};
+        const float G[12] = {ga.x, ga.y, ga.z, ga.w, gb.x, gb.y, gb.z, gb.w, gcv.x, gcv.y, gcv.z, gcv.w};
+        const float gc[3] = {g4.x, g4.y, g4.z};
+        const float cns[4] = {cn4.x, cn4.y, cn4.z, cn4.w}, wss[4] = {ws4.x, ws4.y, ws4.z, ws4.w};
+#pragma unroll
+        for (int n = 0; n < NT; ++n) {
+          const float cn = cns[n], wsn = wss[n];
+          const float cv[12] = {c[n][0].x, c[n][0].y, c[n][0].z, c[n][0].w, c[n][1].x, c[n][1].y, c[n][1].z, c[n][1].w, c[n][2].x, c[n][2].y, c[n][2].z, c[n][2].w};
+          float* dv = reinterpret_cast<float*>(&d[n][0]);
+          const float gcn[3] = {gc[0] * cn, gc[1] * cn, gc[2] * cn};
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            float t = 0.f;                                      // sum over channels of coef * masked dL/dc
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) { dv[3 * k + ch] = fmaf(gcn[ch], Y[k], dv[3 * k + ch]); t = fmaf(cv[3 * k + ch], gc[ch], t); }
+            ad = fmaf(t * wsn, Y[k], ad);
+            const float tc = t * cn;
+            ax = fmaf(tc, G[3 * k], ax); ay = fmaf(tc, G[3 * k + 1], ay); az = fmaf(tc, G[3 * k + 2], az);
+          }
+        }
+      }
+#pragma unroll
+      for (int o = 1; o <= 2; o <<= 1) {
+        ax += __shfl_xor_sync(0xffffffffu, ax, o); ay += __shfl_xor_sync(0xffffffffu, ay, o);
+        az += __shfl_xor_sync(0xffffffffu, az, o); ad += __shfl_xor_sync(0xffffffffu, ad, o);
+      }
+      if (act && v == l) mine = make_float4(ax, ay, az, ad);
+    }
+    if ((vm >> l) & 1u) FDGS_SEL4(A.dcol, l)[id] = mine;
+    if (valid) {
+#pragma unroll
+      for (int n = 0; n < NT; ++n) { d4p[12 * n] = d[n][0]; d4p[12 * n + 1] = d[n][1]; d4p[12 * n + 2] = d[n][2]; }
+    }
+    __syncwarp();                                               // the table is rewritten in the next round
+#pragma unroll
+    for (int k = 0; k < 8; ++k) members &= members - 1;          // drop the 8 members served (x & (x - 1) of 0 is 0)
+  }
+}
+#undef FDGS_SEL4
+
 // K8b (B2, geometry part): VJP of A3, A2, A1 for every survivor.  Recomputes the forward chain from the raw parameters
 // and accumulates (+=) into the caller's gradient arrays.  One thread owns one primitive, so the read-modify-write
 // needs no atomics.  The chain is differentiated in the same factor form the forward uses (geom.cuh):
@@ -437,6 +581,38 @@ void launch_preprocess_bwd(const fdgs_scene& sc, const ViewParams& vp, const Cfg
   }
   geom_bwd_kernel<<<(sc.N + 127) / 128, 128, 0, st>>>(sc, vp, cp, ws.vis_ids, ws.hdr, ws.g9, ws.dcol, with_gz ? ws.gz : nullptr, gr);
   count_launch(2);
+}
+
+// geometry part alone (the batched step runs it per view after the batched colour pass)
+void launch_geom_bwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, const fdgs_grads& gr, cudaStream_t st) {
+  if (sc.N <= 0) return;
+  geom_bwd_kernel<<<(sc.N + 127) / 128, 128, 0, st>>>(sc, vp, cp, ws.vis_ids, ws.hdr, ws.g9, ws.dcol, nullptr, gr);
+  count_launch();
+}
+
+// colour part of all V views of a batch in one pass (see colour_bwd16_union_kernel); false = not available for this
+// scene (sh_degree != 3 or more than 4 Fourier orders): the caller then runs the per-view kernels
+bool launch_colour_bwd_batch(const fdgs_scene& sc, int V, const Workspace* ws, const float* inv_T, const fdgs_grads& gr, bool grads_are_zero,
+                             cudaStream_t st) {
+  if (sc.sh_degree != 3 || sc.n_time > 4 || V < 1 || V > 4) return false;
+  if (sc.N <= 0) return true;
+  BatchColourArgs A{};
+  A.V = V;
+  for (int v = 0; v < V; ++v) {
+    A.inv_T[v] = inv_T[v]; A.tiles_touched[v] = ws[v].tiles_touched; A.aux[v] = ws[v].aux; A.rec[v] = ws[v].rec; A.g9[v] = ws[v].g9; A.dcol[v] = ws[v].dcol;
+  }
+  const int blocks = (sc.N + 127) / 128;
+#define FDGS_CU(NTV) do { if (grads_are_zero) colour_bwd16_union_kernel<NTV, true><<<blocks, 128, 0, st>>>(sc.sh, sc.N, A, gr.sh); \
+                         else colour_bwd16_union_kernel<NTV, false><<<blocks, 128, 0, st>>>(sc.sh, sc.N, A, gr.sh); } while (0)
+  switch (sc.n_time) {
+    case 1: FDGS_CU(1); break;
+    case 2: FDGS_CU(2); break;
+    case 3: FDGS_CU(3); break;
+    default: FDGS_CU(4); break;
+  }
+#undef FDGS_CU
+  count_launch();
+  return true;
 }
 
 }  // namespace fdgs

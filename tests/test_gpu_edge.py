@@ -241,6 +241,50 @@ def test_step_batch_matches_view_by_view():
         fdgs.BatchStep(ds, 200, 150, 1 << 21, 9)
 
 
+@pytest.mark.parametrize("n_views,sh_degree,n_time", [(2, 3, 1), (3, 3, 2), (4, 3, 3), (4, 3, 4),      # one colour pass for the batch
+                                                       (5, 3, 3), (3, 2, 3), (2, 3, 5)])                # per-view chain
+def test_step_batch_backward_preprocess_variants(n_views, sh_degree, n_time):
+    """The backward preprocess of fdgs_step_batch — one colour pass over the union of the views' survivors where the scene
+    allows it (sh_degree 3, <= 4 Fourier orders, <= 4 views), the per-view chain otherwise — adds to the caller's arrays
+    exactly what the view-by-view calls add, with and without FDGS_STEP_ZERO_GRADS."""
+    import gpu_helpers as gh
+    import torch
+    from paper_2412_20720_b200 import fdgs
+    W, H, N = 136, 104, 6000
+    base = scenes.multiview_video(N=N, width=W, height=H, n_views=n_views)
+    K = n_time * (sh_degree + 1) ** 2
+    sh = np.ascontiguousarray(np.resize(base.sh.reshape(N, -1), (N, 3 * K)).reshape(N, K, 3))
+    sc = scenes.Scene("variant", sh_degree, n_time, base.mean, base.log_scale, base.quat_l, base.quat_r, base.opacity_logit, sh,
+                      base.views, base.seed)
+    ds = fdgs.DeviceScene.from_scene(sc)
+    cvs = [fdgs.make_view(v) for v in sc.views]
+    tg = [torch.from_numpy(scenes.target_image(sc.seed, i, W, H)).cuda() for i in range(n_views)]
+    keys = ("mean", "log_scale", "quat_l", "quat_r", "opacity_logit", "sh")
+    r = fdgs.Renderer(ds, W, H, 1 << 20)
+    g_ref = ds.zero_grads()
+    seen = 0
+    for cv, t in zip(cvs, tg):
+        r.loss.zero_()
+        D, nvis = r.preprocess(cv, sync=True); r.forward(cv); r.l1_loss(t); r.backward(cv, r.dL_dimage, g_ref)
+        seen += nvis
+    torch.cuda.synchronize()
+    assert seen > 1000
+    ref = {k: g_ref[k].cpu().numpy().astype(np.float64) for k in keys}
+    bs = fdgs.BatchStep(ds, W, H, 1 << 20, n_views)
+    for rr, t in zip(bs.renderers, tg):
+        rr.target_dev.copy_(t)
+    g = ds.zero_grads()
+    for rep in (1, 2):                                           # the second call adds to what the first one left
+        bs.step(cvs, g)
+        torch.cuda.synchronize()
+        for k in keys:
+            assert gh.rel_l2(g[k].cpu().numpy(), rep * ref[k]) < 1e-5, (k, rep)
+    bs.step(cvs, g, zero_grads=True)                             # cleared by the library, then written
+    torch.cuda.synchronize()
+    for k in keys:
+        assert gh.rel_l2(g[k].cpu().numpy(), ref[k]) < 1e-5, k
+
+
 def test_autograd_front_end_matches_the_c_abi_path():
     """paper_2412_20720_b200.autograd.Rasterizer: loss.backward() == fdgs_render_backward(_aux) with the same upstream."""
     import gpu_helpers as gh
