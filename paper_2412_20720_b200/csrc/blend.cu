@@ -862,9 +862,10 @@ __global__ void __launch_bounds__(128) blend_feat_bwd_geom_kernel(const uint2* _
 
 template <int HBUF, bool GRED = false>   // hits buffered per warp (4, 8 or 16; 8 measured best: 4 flushes too often, 16 costs occupancy)
 struct Bwd2Shared {
-  float4 s0[128], s1[128], s2[128];
+  // slots 128 .. 128 + 4 HBUF - 1: per warp, the staged form of the hits it carries over a batch boundary (slot = hit index)
+  float4 s0[128 + 4 * HBUF], s1[128 + 4 * HBUF], s2[128 + 4 * HBUF];
   float acc[GRED ? 1 : 10 * 129];     // nine sums of the colour path + (AUX) sum of wgt * dL/ddepth (unused with GRED)
-  unsigned int id[128];
+  unsigned int id[128 + 4 * HBUF];
   int max_contrib;
   int hitj[4][HBUF];
   float4 hit[4][HBUF][HROW];
@@ -1036,9 +1037,10 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
   // DEF: the thresholds of [23] as immediates (cp.default_thresholds; see common.cuh)
   const float c_l2min = DEF ? FDGS_DEF_L2MIN : cp.log2_alpha_min, c_amax = DEF ? FDGS_DEF_ALPHA_MAX : cp.alpha_max;
   const float c_amin = DEF ? FDGS_DEF_ALPHA_MIN : cp.alpha_min;
+  int nbuf = 0;                                         // buffered hits of this warp (warp-uniform)
   for (int hi = total; hi > 0; hi -= BATCH) {           // batch covers list positions [lo_pos, hi)
     const int lo_pos = max(0, hi - BATCH), m = hi - lo_pos;
-    __syncthreads();                                    // previous batch fully flushed
+    __syncthreads();                                    // previous batch fully walked (hits it left are in the carry slots)
     if ((int)threadIdx.x < m) {
       const unsigned int id = vals[range.x + lo_pos + threadIdx.x];
       sm.id[threadIdx.x] = id;
@@ -1050,7 +1052,6 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
     }
     __syncthreads();
     if (lo_pos < lane_max) {
-     int nbuf = 0;                                      // buffered hits (warp-uniform)
      for (int jb = ((m - 1) >> 5) << 5; jb >= 0; jb -= 32) {
       unsigned int hk[PX], any = 0;
       float4 ta, tb;
@@ -1101,7 +1102,16 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
         if (++nbuf == HBUF) { bwd2_flush<HBUF, AUX, GRED>(sm, warp, lane, HBUF, sx0, sy0, g9, gz); nbuf = 0; }
       }
      }
-     if (nbuf) bwd2_flush<HBUF, AUX, GRED>(sm, warp, lane, nbuf, sx0, sy0, g9, gz);
+     if (GRED && nbuf) {
+       // a partly filled buffer is not flushed at the batch boundary (a flush costs the same for 1 hit as for 8, and 19 %
+       // of the flushes were such): the staged form of its hits moves to the warp's carry slots, which the next batch's
+       // staging does not touch, and the buffer goes on filling
+       if (lane < nbuf) {
+         const int j = sm.hitj[warp][lane], dst = BATCH + warp * HBUF + lane;
+         if (j < BATCH) { sm.s0[dst] = sm.s0[j]; sm.s1[dst] = sm.s1[j]; sm.s2[dst] = sm.s2[j]; sm.id[dst] = sm.id[j]; sm.hitj[warp][lane] = dst; }
+       }
+       __syncwarp();
+     } else if (nbuf) { bwd2_flush<HBUF, AUX, GRED>(sm, warp, lane, nbuf, sx0, sy0, g9, gz); nbuf = 0; }
     }
     if (GRED) continue;                                 // gradients already in g9 (the loop-top barrier protects the staging arrays)
     __syncthreads();
@@ -1123,6 +1133,7 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
       if (AUX) { const float sz = sm.acc[9 * ACC_STRIDE + j]; if (sz != 0.f) atomicAdd(gz + sm.id[j], sz); }
     }
   }
+  if (GRED && nbuf) bwd2_flush<HBUF, AUX, GRED>(sm, warp, lane, nbuf, sx0, sy0, g9, gz);     // what the last batch left
 }
 
 void launch_blend_fwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
