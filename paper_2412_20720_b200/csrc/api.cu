@@ -32,7 +32,7 @@ struct DeviceCtx {
   bool ready = false;
   int sms = 0;
   cudaStream_t worker[FDGS_MAX_BATCH] = {}, zero_stream = nullptr, copy_stream = nullptr;
-  cudaEvent_t batch_fork = nullptr, b2_done[FDGS_MAX_BATCH] = {}, copy_done[FDGS_MAX_BATCH] = {}, zero_done = nullptr, copy_fork = nullptr, copy_join = nullptr;
+  cudaEvent_t batch_fork = nullptr, b2_done[FDGS_MAX_BATCH] = {}, copy_done[FDGS_MAX_BATCH] = {}, zero_done = nullptr, copy_fork = nullptr, copy_join = nullptr, colour_done = nullptr;
 };
 constexpr int MAX_DEVICES = 64;
 static DeviceCtx g_ctx[MAX_DEVICES];
@@ -58,6 +58,7 @@ static int device_ctx(DeviceCtx** out) {
     FDGS_CUDA(cudaEventCreateWithFlags(&c.batch_fork, cudaEventDisableTiming), "fork event");
     FDGS_CUDA(cudaEventCreateWithFlags(&c.copy_fork, cudaEventDisableTiming), "copy event");
     FDGS_CUDA(cudaEventCreateWithFlags(&c.copy_join, cudaEventDisableTiming), "copy event");
+    FDGS_CUDA(cudaEventCreateWithFlags(&c.colour_done, cudaEventDisableTiming), "colour event");
     c.ready = true;
   }
   *out = &c;
@@ -465,12 +466,14 @@ int fdgs_step_batch(const fdgs_scene* sc, const fdgs_view* views, int32_t num_vi
     Workspace wss[FDGS_MAX_BATCH]; float inv_T[FDGS_MAX_BATCH];
     for (int i = 0; i < num_views; ++i) { wss[i] = carve(bufs[i].ws, sc->N, K, views[i].width, views[i].height, cap); inv_T[i] = 1.0f / views[i].period_T; }
     launch_colour_bwd_batch(*sc, num_views, wss, inv_T, *g, zero, w0);
-    for (int i = 0; i < num_views; ++i) {
+    cudaEventRecord(ctx->colour_done, w0);
+    for (int i = 0; i < num_views; ++i) {      // geometry part: the views side by side on their own streams, sums by reductions
       ViewParams vp; CfgParams cp;
       make_params(&views[i], c, vp, cp);
-      launch_geom_bwd(*sc, vp, cp, wss[i], *g, w0);
+      if (i > 0) cudaStreamWaitEvent(ctx->worker[i], ctx->colour_done, 0);
+      launch_geom_bwd(*sc, vp, cp, wss[i], *g, ctx->worker[i]);
+      cudaEventRecord(ctx->b2_done[i], ctx->worker[i]);
     }
-    cudaEventRecord(ctx->b2_done[0], w0);
   }
   for (int i = 0; i < launched; ++i) cudaStreamWaitEvent(st, ctx->b2_done[i], 0);
   if (zero) cudaStreamWaitEvent(st, ctx->zero_done, 0);

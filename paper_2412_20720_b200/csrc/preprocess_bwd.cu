@@ -374,6 +374,12 @@ __global__ void __launch_bounds__(128) colour_bwd16_union_kernel(const float* __
 // and accumulates (+=) into the caller's gradient arrays.  One thread owns one primitive, so the read-modify-write
 // needs no atomics.  The chain is differentiated in the same factor form the forward uses (geom.cuh):
 // Sigma_2d = B B^T + dI, B = T N, N = M3 - c m4^T / b, c = M3 m4, b = m4.m4, M = R diag(s), R = L(q_l) R(q_r).
+// ATOMIC (the batched step): the views of a batch run this kernel side by side, so the sums go to the caller's arrays as
+// vector reductions (red.global.add.v4.f32) instead of a read-modify-write by the owning thread, and nothing is read back.
+__device__ __forceinline__ void red_add_f4(float4* p, const float4 v) {
+  asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+template <bool ATOMIC>
 __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, const ViewParams vp, const CfgParams cp,
                                                        const unsigned int* __restrict__ vis_list, const WsHeader* __restrict__ hdr,
                                                        const float* __restrict__ g9, const float4* __restrict__ dcol, const float* __restrict__ gz, const fdgs_grads gr) {
@@ -387,15 +393,21 @@ __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, cons
   }
   // the gradient rows this thread will read-modify-write: requested now, consumed at the end of the chain (the compiler
   // would otherwise issue each load right before its use: five serial round trips on a 12-warps-per-SM kernel)
-  float4 acc_mean, acc_ls, acc_ql, acc_qr;
-  ld_f4(reinterpret_cast<const float4*>(gr.mean) + i, acc_mean);
-  ld_f4(reinterpret_cast<const float4*>(gr.log_scale) + i, acc_ls);
-  ld_f4(reinterpret_cast<const float4*>(gr.quat_l) + i, acc_ql);
-  ld_f4(reinterpret_cast<const float4*>(gr.quat_r) + i, acc_qr);
-  const float acc_logit = gr.opacity_logit[i];
+  float4 acc_mean = make_float4(0.f, 0.f, 0.f, 0.f), acc_ls = acc_mean, acc_ql = acc_mean, acc_qr = acc_mean;
+  float acc_logit = 0.f;
+  if (!ATOMIC) {
+    ld_f4(reinterpret_cast<const float4*>(gr.mean) + i, acc_mean);
+    ld_f4(reinterpret_cast<const float4*>(gr.log_scale) + i, acc_ls);
+    ld_f4(reinterpret_cast<const float4*>(gr.quat_l) + i, acc_ql);
+    ld_f4(reinterpret_cast<const float4*>(gr.quat_r) + i, acc_qr);
+    acc_logit = gr.opacity_logit[i];
+  }
   const float* gp = g9 + (size_t)9 * i;
   const float g_u = gp[0], g_v = gp[1], g_A = gp[2], g_B = gp[3], g_C = gp[4], g_o = gp[5];
-  if (gr.mean2d) { gr.mean2d[2 * i] += g_u; gr.mean2d[2 * i + 1] += g_v; }
+  if (gr.mean2d) {
+    if (ATOMIC) { atomicAdd(gr.mean2d + 2 * i, g_u); atomicAdd(gr.mean2d + 2 * i + 1, g_v); }
+    else { gr.mean2d[2 * i] += g_u; gr.mean2d[2 * i + 1] += g_v; }
+  }
   float dir[3], inv_rho;
   {
     const float dx = g.muc[0] - vp.cam[0], dy = g.muc[1] - vp.cam[1], dz = g.muc[2] - vp.cam[2];
@@ -469,7 +481,8 @@ __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, cons
 
   // ---- o = sigmoid(logit) w,  w = exp(-Delta^2 / 2b) -----------------------------------------
   const float inv_b = 1.0f / g.b;
-  gr.opacity_logit[i] = acc_logit + g_o * g.w * g.sig * g.sig_neg;
+  if (ATOMIC) atomicAdd(gr.opacity_logit + i, g_o * g.w * g.sig * g.sig_neg);
+  else gr.opacity_logit[i] = acc_logit + g_o * g.w * g.sig * g.sig_neg;
   {
     const float d_w = g_o * g.sig;
     d_dt += d_w * g.w * (-g.dt * inv_b);
@@ -512,9 +525,10 @@ __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, cons
     m.x += d_muc[0]; m.y += d_muc[1]; m.z += d_muc[2]; m.w += -d_dt;
     if (gr.densify) {   // density-control indicators of this view
       float* dn = gr.densify + (size_t)3 * i;
-      dn[0] += sqrtf(g_u * g_u + g_v * g_v); dn[1] += fabsf(d_dt); dn[2] += 1.0f;
+      if (ATOMIC) { atomicAdd(dn, sqrtf(g_u * g_u + g_v * g_v)); atomicAdd(dn + 1, fabsf(d_dt)); atomicAdd(dn + 2, 1.0f); }
+      else { dn[0] += sqrtf(g_u * g_u + g_v * g_v); dn[1] += fabsf(d_dt); dn[2] += 1.0f; }
     }
-    *dst = m;
+    if (ATOMIC) red_add_f4(dst, m); else *dst = m;
   }
   // ---- M = R4 diag(s) ------------------------------------------------------------------------
   float dR4[4][4];
@@ -530,7 +544,7 @@ __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, cons
     float4* dst = reinterpret_cast<float4*>(gr.log_scale) + i;
     float4 m = acc_ls;
     m.x += dls[0]; m.y += dls[1]; m.z += dls[2]; m.w += dls[3];
-    *dst = m;
+    if (ATOMIC) red_add_f4(dst, m); else *dst = m;
   }
   // ---- R4 = L(q_l) R(q_r), quaternion entries, normalisation -----------------------------------
   {
@@ -562,7 +576,7 @@ __global__ void __launch_bounds__(128) geom_bwd_kernel(const fdgs_scene sc, cons
     ml.z += (dql[2] - g.ql[2] * dl) * g.inv_nl; ml.w += (dql[3] - g.ql[3] * dl) * g.inv_nl;
     mr.x += (dqr[0] - g.qr[0] * dr) * g.inv_nr; mr.y += (dqr[1] - g.qr[1] * dr) * g.inv_nr;
     mr.z += (dqr[2] - g.qr[2] * dr) * g.inv_nr; mr.w += (dqr[3] - g.qr[3] * dr) * g.inv_nr;
-    *dstl = ml; *dstr = mr;
+    if (ATOMIC) { red_add_f4(dstl, ml); red_add_f4(dstr, mr); } else { *dstl = ml; *dstr = mr; }
   }
 }
 
@@ -579,14 +593,14 @@ void launch_preprocess_bwd(const fdgs_scene& sc, const ViewParams& vp, const Cfg
     else colour_bwd16_kernel<<<blocks, threads, 0, st>>>(sc.sh, sc.n_time, vp.inv_T, ws.vis_ids, ws.hdr, ws.g9, ws.rec, ws.aux, gr.sh, ws.dcol);
 #undef FDGS_LAUNCH
   }
-  geom_bwd_kernel<<<(sc.N + 127) / 128, 128, 0, st>>>(sc, vp, cp, ws.vis_ids, ws.hdr, ws.g9, ws.dcol, with_gz ? ws.gz : nullptr, gr);
+  geom_bwd_kernel<false><<<(sc.N + 127) / 128, 128, 0, st>>>(sc, vp, cp, ws.vis_ids, ws.hdr, ws.g9, ws.dcol, with_gz ? ws.gz : nullptr, gr);
   count_launch(2);
 }
 
-// geometry part alone (the batched step runs it per view after the batched colour pass)
+// geometry part alone (the batched step runs it after the batched colour pass, the views side by side: sums by reductions)
 void launch_geom_bwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, const fdgs_grads& gr, cudaStream_t st) {
   if (sc.N <= 0) return;
-  geom_bwd_kernel<<<(sc.N + 127) / 128, 128, 0, st>>>(sc, vp, cp, ws.vis_ids, ws.hdr, ws.g9, ws.dcol, nullptr, gr);
+  geom_bwd_kernel<true><<<(sc.N + 127) / 128, 128, 0, st>>>(sc, vp, cp, ws.vis_ids, ws.hdr, ws.g9, ws.dcol, nullptr, gr);
   count_launch();
 }
 
