@@ -64,13 +64,18 @@ def stage_rooflines(stage, work, N, K, n_views):
     the memory-bound stages, algorithmic lane-instructions vs the ALU issue peak for the two blend kernels."""
     peak, src = hbm_peak()
     nv, D = work["visible"], work["pairs"]          # summed over the views of the step
-    byts = {"preprocess": n_views * 72 * N + nv * (12 * K + 76),
+    # the public fdgs_preprocess / fdgs_render_forward pair (timed here stage by stage) evaluates the colour of a degree-3
+    # scene in a kernel of its own on a side stream, under the depth sort and the row scatter: two rows
+    byts = {"preprocess": n_views * 72 * N + nv * 76,               # geometry rows of every primitive; record, hand-over, rectangle of the survivors
+            "colour_side_stream": nv * (12 * K + 4 + 16 + 12),      # coefficient rows of the survivors; id and hand-over read, three colour slots written
             "compact+tile_grid": n_views * 4 * N + 16 * nv,
             "sort_depth": 4 * 16 * nv,
             "tile_lists": 12 * nv + 4 * D,                    # ids and rectangles of the survivors read, 4 B written per pair
             "preprocess_bwd": nv * (36 + 68 + 12 * K + 2 * (12 * K + 68) + 64)}
     out = {}
     for k, b in byts.items():
+        if not stage.get(k, 0.0) > 0.0:
+            continue
         gbs = b / (stage[k] * 1e-3) / 1e9
         out[k] = {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "frac_of_8tbs_spec": gbs / 8000.0,
                   "algorithmic_bytes": b}

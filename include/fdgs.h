@@ -98,6 +98,9 @@ int fdgs_workspace_bytes(int32_t N, int32_t K, int32_t W, int32_t H, int64_t pai
  * (eq. 7-8); time slice mu_xyz|t, Sigma_xyz|t and marginal weight (eq. 9-10)
  * with the p(t) < marginal_min filter (L324); EWA projection to a 2D conic (eq. 3-4);
  * 4DSH colour (eq. 20); tiles touched and their exclusive prefix sum.
+ * Scenes of sh_degree 3: the colour slots of the per-primitive records are filled in by the fdgs_render_forward(_aux) that
+ * follows (on a library-owned side stream, next to its depth sort and tile lists: only the blend reads the colours), so
+ * FDGS_EXPORT_RECORDS shows final colours after that call, not after this one.
  * If num_pairs_host / num_visible_host are non-NULL the stream is synchronised and D / the number
  * of surviving primitives are returned (and FDGS_ERR_PAIR_OVERFLOW if D > pair_capacity). */
 int fdgs_preprocess(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws,
@@ -111,7 +114,9 @@ int fdgs_preprocess(const fdgs_scene *scene, const fdgs_view *view_host, const f
  * left), n_contrib [H,W] (1 + position in the tile list of the last splat composited).
  * If D exceeded pair_capacity nothing is drawn (image = bg) and the overflow is reported by
  * fdgs_debug_export(FDGS_EXPORT_STATUS) or the next synchronising call.
- * Each call consumes the tickets and look-back state that fdgs_preprocess prepared on `ws`: one forward per preprocess. */
+ * Each call consumes the tickets and look-back state that fdgs_preprocess prepared on `ws`: one forward per preprocess.
+ * For sh_degree 3 the call forks the colour evaluation (A4) onto a library-owned stream and joins it back into
+ * `cuda_stream` before the blend; fork and join both happen inside the call, so it can be captured into a CUDA graph. */
 int fdgs_render_forward(const fdgs_scene *scene, const fdgs_view *view_host, const fdgs_config *cfg_host, void *ws,
                         size_t ws_bytes, int64_t pair_capacity, void *cuda_stream, float *image, float *final_T,
                         uint32_t *n_contrib);
@@ -205,8 +210,9 @@ int fdgs_debug_export(const void *ws, size_t ws_bytes, int what, void *dst, size
 
 /* Measurement hooks (bench.py).  fdgs_set_stage_timing(1) makes the three calls record CUDA events at
  * their stage boundaries; fdgs_get_stage_ms waits for them and fills ms_host[8]: preprocess kernel, compaction +
- * tile grid, depth sort, tile lists (row scatter), forward blend, backward blend, backward preprocess, and -1 in the
- * unused eighth slot (-1 as well for a stage that has not run).  fdgs_debug_blend_stats re-walks the tile lists of the last forward on `ws`
+ * tile grid, depth sort, tile lists (row scatter), forward blend, backward blend, backward preprocess, and the colour
+ * kernel that fdgs_render_forward runs on its side stream UNDER the depth sort and the row scatter (its time is not part
+ * of the frame's critical path) (-1 for a stage that has not run).  fdgs_debug_blend_stats re-walks the tile lists of the last forward on `ws`
  * and writes uint64[4] to stats_dev: (pixel, splat) pairs walked, pairs reaching the exp2, pairs composited,
  * splats staged — the algorithmic work of the blend kernels. */
 int fdgs_set_stage_timing(int enable);

@@ -3,6 +3,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <atomic>
 #include <mutex>
 
 #include "common.cuh"
@@ -19,7 +20,7 @@ int cuda_fail(cudaError_t e, const char* where) {
 
 // Optional per-stage timing (fdgs_set_stage_timing): CUDA events recorded on the caller's stream at the stage
 // boundaries; off by default so that the product path carries no event records.
-enum { EV_PRE0, EV_PRE1, EV_PRE2, EV_FWD0, EV_FWD1, EV_FWD2, EV_FWD3, EV_BWD0, EV_BWD1, EV_BWD2, EV_COUNT };
+enum { EV_PRE0, EV_PRE1, EV_PRE2, EV_FWD0, EV_FWD1, EV_FWD2, EV_FWD3, EV_BWD0, EV_BWD1, EV_BWD2, EV_COL0, EV_COL1, EV_COUNT };
 static int g_timing = 0;
 static cudaEvent_t g_ev[EV_COUNT];
 static inline void mark(int which, cudaStream_t st) { if (g_timing) cudaEventRecord(g_ev[which], st); }
@@ -28,9 +29,15 @@ static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 
 
 // Library-owned streams and events, one set per CUDA device (created on first use on that device): the worker streams
 // of fdgs_step_batch, the zeroing stream, the copy stream of fdgs_step_host, and the SM count.
+constexpr int SIDE_STREAMS = 8;
 struct DeviceCtx {
   bool ready = false;
   int sms = 0;
+  // side streams of fdgs_render_forward (colour of the survivors next to the depth sort and the row scatter): a call takes
+  // the next slot, so concurrent frames on different caller streams do not queue behind each other
+  cudaStream_t side[SIDE_STREAMS] = {};
+  cudaEvent_t side_fork[SIDE_STREAMS] = {}, side_join[SIDE_STREAMS] = {};
+  std::atomic<unsigned int> side_next{0};
   cudaStream_t worker[FDGS_MAX_BATCH] = {}, zero_stream = nullptr, copy_stream = nullptr;
   cudaEvent_t batch_fork = nullptr, b2_done[FDGS_MAX_BATCH] = {}, copy_done[FDGS_MAX_BATCH] = {}, zero_done = nullptr, copy_fork = nullptr, copy_join = nullptr, colour_done = nullptr;
 };
@@ -51,6 +58,11 @@ static int device_ctx(DeviceCtx** out) {
       FDGS_CUDA(cudaStreamCreateWithFlags(&c.worker[i], cudaStreamNonBlocking), "worker stream");
       FDGS_CUDA(cudaEventCreateWithFlags(&c.b2_done[i], cudaEventDisableTiming), "worker event");
       FDGS_CUDA(cudaEventCreateWithFlags(&c.copy_done[i], cudaEventDisableTiming), "copy event");
+    }
+    for (int i = 0; i < SIDE_STREAMS; ++i) {
+      FDGS_CUDA(cudaStreamCreateWithFlags(&c.side[i], cudaStreamNonBlocking), "side stream");
+      FDGS_CUDA(cudaEventCreateWithFlags(&c.side_fork[i], cudaEventDisableTiming), "side event");
+      FDGS_CUDA(cudaEventCreateWithFlags(&c.side_join[i], cudaEventDisableTiming), "side event");
     }
     FDGS_CUDA(cudaStreamCreateWithFlags(&c.zero_stream, cudaStreamNonBlocking), "zero stream");
     FDGS_CUDA(cudaStreamCreateWithFlags(&c.copy_stream, cudaStreamNonBlocking), "copy stream");
@@ -204,8 +216,11 @@ int fdgs_workspace_bytes(int32_t N, int32_t K, int32_t W, int32_t H, int64_t pai
   return FDGS_OK;
 }
 
-int fdgs_preprocess(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
-                    int64_t cap, void* stream, int64_t* num_pairs_host, int32_t* num_visible_host) {
+// split_colour: the preprocess kernel of a degree-3 scene stops after the geometry and the forward that follows evaluates
+// the colours on a side stream under the binning (the public pair fdgs_preprocess / fdgs_render_forward: shortest frame);
+// false: colour inside the preprocess kernel (fdgs_step_batch, whose views already overlap each other: least total work)
+static int preprocess_impl(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
+                           int64_t cap, void* stream, int64_t* num_pairs_host, int32_t* num_visible_host, bool split_colour) {
   int rc = check_common(sc, v, c, ws_ptr);
   if (rc) return rc;
   if (cap < 1 || cap >= (1LL << 30)) return FDGS_ERR_INVALID;
@@ -221,7 +236,7 @@ int fdgs_preprocess(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config*
   // captured into a CUDA graph.)
   FDGS_CUDA(cudaMemsetAsync(ws_ptr, 0, ws.zero_bytes, st), "memset(header)");
   mark(EV_PRE0, st);
-  launch_preprocess_fwd(*sc, vp, cp, ws, st);                       // A1-A4 (+ coverage grid)
+  launch_preprocess_fwd(*sc, vp, cp, ws, st, split_colour);         // A1-A4 (+ coverage grid)
   mark(EV_PRE1, st);
   launch_compact_and_tile_grid(ws, sc->N, K, vp, cap, st);          // survivors -> (depth bits, id); A5/A8: list lengths -> ranges, D
   mark(EV_PRE2, st);
@@ -237,18 +252,41 @@ int fdgs_preprocess(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config*
   return FDGS_OK;
 }
 
+int fdgs_preprocess(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
+                    int64_t cap, void* stream, int64_t* num_pairs_host, int32_t* num_visible_host) {
+  return preprocess_impl(sc, v, c, ws_ptr, ws_bytes, cap, stream, num_pairs_host, num_visible_host, true);
+}
+
 }  // extern "C"
 
 // A6-A9.  The depth order of the survivors (level 1) is kept in the workspace for the backward.
 static int forward_impl(const fdgs_scene* sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, int64_t cap,
-                        cudaStream_t st, float* image, float* final_T, uint32_t* n_contrib, float* depth_map) {
+                        cudaStream_t st, float* image, float* final_T, uint32_t* n_contrib, float* depth_map, bool split_colour) {
   (void)cap;
-  const int sms = num_sms();
+  DeviceCtx* ctx = nullptr;
+  int rc = device_ctx(&ctx);
+  if (rc) return rc;
+  const int sms = ctx->sms;
   mark(EV_FWD0, st);
+  // A4 of a degree-3 scene runs on a side stream while the survivors are sorted and scattered: only the blend needs the
+  // colours, and the binning launches are latency-bound chains of a few hundred CTAs (fork here, join before the blend;
+  // both inside this call, so the sequence stays capturable into a CUDA graph)
+  cudaEvent_t join = nullptr;
+  if (split_colour && sc->N > 0 && sc->sh_degree == 3) {
+    const unsigned int slot = ctx->side_next.fetch_add(1u, std::memory_order_relaxed) % SIDE_STREAMS;
+    FDGS_CUDA(cudaEventRecord(ctx->side_fork[slot], st), "fork(colour)");
+    FDGS_CUDA(cudaStreamWaitEvent(ctx->side[slot], ctx->side_fork[slot], 0), "fork(colour) wait");
+    mark(EV_COL0, ctx->side[slot]);
+    launch_colour_fwd(*sc, ws, sms, ctx->side[slot]);
+    mark(EV_COL1, ctx->side[slot]);
+    FDGS_CUDA(cudaEventRecord(ctx->side_join[slot], ctx->side[slot]), "join(colour)");
+    join = ctx->side_join[slot];
+  }
   const int l1 = launch_sort_depth(ws, sc->N, sms, st);             // level 1: survivors by fp32 depth bits
   mark(EV_FWD1, st);
   launch_row_scatter(ws, l1, sc->N, vp, sms, st);                       // level 2: per-tile lists written in place, depth order
   mark(EV_FWD2, st);
+  if (join) FDGS_CUDA(cudaStreamWaitEvent(st, join, 0), "join(colour) wait");
   launch_blend_fwd(ws, vp, cp, image, final_T, n_contrib, depth_map, st);
   mark(EV_FWD3, st);
   FDGS_CUDA(cudaGetLastError(), "forward launches");
@@ -268,7 +306,8 @@ static int read_overflow(const Workspace& ws) {
 extern "C" {
 
 static int forward_entry(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
-                         int64_t cap, void* stream, float* image, float* final_T, uint32_t* n_contrib, float* depth_map) {
+                         int64_t cap, void* stream, float* image, float* final_T, uint32_t* n_contrib, float* depth_map,
+                         bool split_colour = true) {
   int rc = check_common(sc, v, c, ws_ptr);
   if (rc) return rc;
   if (!image || !final_T || !n_contrib || cap < 1 || cap >= (1LL << 30)) return FDGS_ERR_INVALID;
@@ -277,7 +316,7 @@ static int forward_entry(const fdgs_scene* sc, const fdgs_view* v, const fdgs_co
   if (ws.bytes > ws_bytes) return FDGS_ERR_WORKSPACE;
   ViewParams vp; CfgParams cp;
   make_params(v, c, vp, cp);
-  return forward_impl(sc, vp, cp, ws, cap, (cudaStream_t)stream, image, final_T, n_contrib, depth_map);
+  return forward_impl(sc, vp, cp, ws, cap, (cudaStream_t)stream, image, final_T, n_contrib, depth_map, split_colour);
 }
 
 int fdgs_render_forward(const fdgs_scene* sc, const fdgs_view* v, const fdgs_config* c, void* ws_ptr, size_t ws_bytes,
@@ -446,8 +485,9 @@ int fdgs_step_batch(const fdgs_scene* sc, const fdgs_view* views, int32_t num_vi
     cudaStreamWaitEvent(w, ctx->batch_fork, 0);
     launched = i + 1;
     cudaMemsetAsync(loss_dev + i, 0, sizeof(float), w);
-    rc = fdgs_preprocess(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, nullptr, nullptr);
-    if (!rc) rc = fdgs_render_forward(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, b.image, b.final_T, b.n_contrib);
+    // colour inside the preprocess kernel: the views' front ends already run side by side, a side stream per view only adds work
+    rc = preprocess_impl(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, nullptr, nullptr, false);
+    if (!rc) rc = forward_entry(sc, &views[i], c, b.ws, b.ws_bytes, cap, w, b.image, b.final_T, b.n_contrib, nullptr, false);
     if (b.target_host) cudaStreamWaitEvent(w, ctx->copy_done[i], 0);     // also on the error path: the copy is joined through this stream
     if (!rc) rc = step_loss(carve(b.ws, sc->N, K, views[i].width, views[i].height, cap), b.image, b.target_dev, (int64_t)count, b.dL_dimage, loss_dev + i, w);
     // blend backward of this view overlaps everything of the others.  B2: with the batched colour pass every view stops
@@ -602,10 +642,9 @@ int fdgs_set_stage_timing(int enable) {
 
 int fdgs_get_stage_ms(float* ms_host) {
   if (!ms_host || !g_timing) return FDGS_ERR_INVALID;
-  const int pairs[7][2] = {{EV_PRE0, EV_PRE1}, {EV_PRE1, EV_PRE2}, {EV_FWD0, EV_FWD1}, {EV_FWD1, EV_FWD2},
-                           {EV_FWD2, EV_FWD3}, {EV_BWD0, EV_BWD1}, {EV_BWD1, EV_BWD2}};
-  ms_host[7] = -1.f;
-  for (int k = 0; k < 7; ++k) {
+  const int pairs[8][2] = {{EV_PRE0, EV_PRE1}, {EV_PRE1, EV_PRE2}, {EV_FWD0, EV_FWD1}, {EV_FWD1, EV_FWD2},
+                           {EV_FWD2, EV_FWD3}, {EV_BWD0, EV_BWD1}, {EV_BWD1, EV_BWD2}, {EV_COL0, EV_COL1}};
+  for (int k = 0; k < 8; ++k) {
     ms_host[k] = -1.f;
     if (cudaEventSynchronize(g_ev[pairs[k][1]]) == cudaSuccess) cudaEventElapsedTime(&ms_host[k], g_ev[pairs[k][0]], g_ev[pairs[k][1]]);
   }
@@ -785,7 +824,7 @@ extern "C" int fdgs_render_forward_static(const fdgs_scene* sc, const fdgs_view*
   // that has to start from zero (header, coverage grid, scan states, digit counts, look-back regions) is the prefix
   // cleared here; the rest is written before it is read.
   FDGS_CUDA(cudaMemsetAsync(ctx->ws, 0, ws.zero_bytes, st), "memset(static header)");
-  launch_preprocess_fwd(*sc, vp, cp, ws, st);
+  launch_preprocess_fwd(*sc, vp, cp, ws, st, false);       // colour inside the kernel: this entry point creates nothing, not even a side stream
   launch_compact_and_tile_grid(ws, sc->N, K, vp, cap, st);
   const int l1 = launch_sort_depth(ws, sc->N, ctx->sms, st);
   launch_row_scatter(ws, l1, sc->N, vp, ctx->sms, st);

@@ -172,7 +172,12 @@ long long launch_count_value();
 int cuda_fail(cudaError_t e, const char* where);
 
 // Launchers (each file implements its own; all asynchronous on `st`).
-void launch_preprocess_fwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, cudaStream_t st);
+// split_colour (degree-3 scenes only): stop after the geometry (A1-A3) and leave the colour slots of the records to
+// launch_colour_fwd, which fdgs_render_forward runs on a side stream under the binning launches
+void launch_preprocess_fwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, cudaStream_t st, bool split_colour);
+// A4 of a degree-3 scene: colour of the visible survivors into the records (after the compaction; only the blend reads it).
+// false: nothing to do (the preprocess kernel of the other degrees evaluates the colour itself).
+bool launch_colour_fwd(const fdgs_scene& sc, const Workspace& ws, int num_sms, cudaStream_t st);
 // compaction scan: survivors (tiles_touched > 0) in id order -> l1_keys[0] (depth bits), l1_vals[0] (ids), hdr->num_visible;
 // the same launch carries, as the role of its first CTA, the 2D prefix of the coverage difference array -> ranges, D, overflow
 void launch_compact_and_tile_grid(const Workspace& ws, int N, int K, const ViewParams& vp, long long cap, cudaStream_t st);

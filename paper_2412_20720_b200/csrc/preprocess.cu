@@ -152,13 +152,19 @@ __device__ __forceinline__ unsigned int tile_rect(const Geom& g, const ViewParam
 //      sectors (no L2 line prefetch, which over-fetched the mostly culled neighbours: 287 MB read per view for 216 needed
 //      in round 1), two shuffle levels join the partial colours, and lanes 0-3 store the 48-byte record and the 16-byte
 //      hand-over of the colour backward.
+// SPLIT = true (product since late round 2): the kernel stops after phase 2 — the phase-2 thread stores the geometric part
+// of the record (colour slots zero) and the colour hand-over (direction, Delta / T) itself, and the colour of the visible
+// survivors is evaluated by colour_fwd16_kernel below, which fdgs_render_forward runs on a side stream next to the depth
+// sort and the row scatter, i.e. off the critical path of a frame: those are latency-bound launches of a few hundred
+// CTAs that leave the memory system idle, and only the blend reads the colour.
 constexpr int PF_THREADS = 128;
+template <bool SPLIT>
 __global__ void __launch_bounds__(PF_THREADS) preprocess_fwd16_kernel(const fdgs_scene sc, const ViewParams vp, const CfgParams cp,
                                                                       SplatRec* __restrict__ rec, ushort4* __restrict__ rect,
                                                                       unsigned int* __restrict__ tiles_touched,
                                                                       int* __restrict__ tile_diff, float4* __restrict__ aux) {
   __shared__ unsigned short s_alive[PF_THREADS];
-  __shared__ float4 s_hand[PF_THREADS][4];      // per visible survivor: q0 | (cc, lo, depth, radius) | (w, dir x, y, z) | (dt/T, id, -, -)
+  __shared__ float4 s_hand[SPLIT ? 1 : PF_THREADS][4];      // per visible survivor: q0 | (cc, lo, depth, radius) | (w, dir x, y, z) | (dt/T, id, -, -)
   __shared__ int s_wcount[PF_THREADS / 32], s_wcount2[PF_THREADS / 32];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned int lt_mask = (1u << lane) - 1u;
@@ -208,8 +214,16 @@ __global__ void __launch_bounds__(PF_THREADS) preprocess_fwd16_kernel(const fdgs
       h1 = make_float4(sqrtf(kk / g.c2), log2f(g.sig) - kk * g.dt * g.dt / g.b, g.p[2], radius);   // cc = sqrt(k / c2); lo = log2(sigmoid w)
       h2 = make_float4(g.w, dir[0], dir[1], dir[2]);
       h3 = make_float4(g.dt * vp.inv_T, __int_as_float(id), 0.f, 0.f);
+      if (SPLIT) {
+        float4* dst = reinterpret_cast<float4*>(rec + id);
+        dst[0] = h0;                                            // u, v, ca, cb
+        dst[1] = make_float4(h1.x, h1.y, 0.f, 0.f);             // cc, lo, (r, g: colour role)
+        dst[2] = make_float4(0.f, h1.z, h1.w, h2.x);            // (b), depth, radius, w
+        aux[id] = make_float4(h2.y, h2.z, h2.w, h3.x);          // direction and Delta / T: read by the colour role and the colour backward
+      }
     }
   }
+  if (SPLIT) return;
   const unsigned int bal2 = __ballot_sync(0xffffffffu, visible);
   if (lane == 0) s_wcount2[warp] = __popc(bal2);
   __syncthreads();
@@ -272,6 +286,97 @@ __global__ void __launch_bounds__(PF_THREADS) preprocess_fwd16_kernel(const fdgs
   }
 }
 
+// A4 for the visible survivors of a degree-3 scene (eq. 20), after preprocess_fwd16_kernel<true> and the compaction: four
+// lanes per survivor (dense: the survivors come from the compacted id list), lane l owns the SH orders 4l .. 4l+3 of every
+// Fourier order — 48 contiguous bytes per order, three 128-bit loads — two shuffle levels join the partial sums, and the
+// three colour slots of the record are filled in.  The survivor count lives on the device: grid-stride over groups of 8.
+constexpr int CF_THREADS = 256;
+__global__ void __launch_bounds__(CF_THREADS) colour_fwd16_kernel(const float* __restrict__ sh, const int n_time, const float4* __restrict__ aux,
+                                                                  const unsigned int* __restrict__ vis_ids, const WsHeader* __restrict__ hdr,
+                                                                  SplatRec* __restrict__ rec) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, l = lane & 3;
+  const unsigned int n = hdr->num_visible;
+  const int rec_len = n_time * 48;
+  constexpr unsigned int PER_CTA = CF_THREADS / 4;
+  const unsigned int stride = gridDim.x * PER_CTA;
+  // the id and the hand-over of the NEXT group are requested before the coefficient loads of the current one: a trip is one
+  // memory round trip instead of three dependent ones (id -> direction -> coefficients)
+  unsigned int base = blockIdx.x * PER_CTA + warp * 8;
+  unsigned int id_n = 0;
+  float4 a_n = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (base + (lane >> 2) < n) { id_n = vis_ids[base + (lane >> 2)]; a_n = __ldg(aux + id_n); }
+  for (; base < n; base += stride) {     // warp-uniform trip count
+    const bool have = base + (lane >> 2) < n;
+    const unsigned int id = id_n;
+    const float4 a = a_n;
+    const float4* c4p = reinterpret_cast<const float4*>(sh + (size_t)id * rec_len) + 3 * l;
+    float4 f[9];
+    if (have) {
+#pragma unroll
+      for (int m = 0; m < 3; ++m)
+        if (m < n_time) {
+#pragma unroll
+          for (int qq = 0; qq < 3; ++qq)
+            asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(f[3 * m + qq].x), "=f"(f[3 * m + qq].y), "=f"(f[3 * m + qq].z), "=f"(f[3 * m + qq].w)
+                         : "l"(c4p + 12 * m + qq));
+        }
+    }
+    const unsigned int sv_n = base + stride + (lane >> 2);
+    if (sv_n < n) { id_n = vis_ids[sv_n]; a_n = __ldg(aux + id_n); }
+    float acc[3] = {0.f, 0.f, 0.f};
+    if (have) {
+      float Yf[16], Y[4];
+      sh_basis<16>(a.x, a.y, a.z, Yf);
+#define FDGS_PICK(L0) { _Pragma("unroll") for (int k = 0; k < 4; ++k) Y[k] = Yf[4 * L0 + k]; }
+      if (l == 0) FDGS_PICK(0) else if (l == 1) FDGS_PICK(1) else if (l == 2) FDGS_PICK(2) else FDGS_PICK(3)
+#undef FDGS_PICK
+      for (int n0 = 0; n0 < n_time; n0 += 3) {          // three Fourier orders (nine 128-bit loads per lane) at a time
+        if (n0 > 0) {
+#pragma unroll
+          for (int m = 0; m < 3; ++m)
+            if (n0 + m < n_time) {
+#pragma unroll
+              for (int qq = 0; qq < 3; ++qq)
+                asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(f[3 * m + qq].x), "=f"(f[3 * m + qq].y), "=f"(f[3 * m + qq].z), "=f"(f[3 * m + qq].w)
+                             : "l"(c4p + 12 * (n0 + m) + qq));
+            }
+        }
+#pragma unroll
+        for (int m = 0; m < 3; ++m)
+          if (n0 + m < n_time) {
+            const float cn = cospif(2.0f * (float)(n0 + m) * a.w);
+            const float4 f0 = f[3 * m], f1 = f[3 * m + 1], f2 = f[3 * m + 2];
+            const float y0 = cn * Y[0], y1 = cn * Y[1], y2 = cn * Y[2], y3 = cn * Y[3];
+            acc[0] = fmaf(f0.x, y0, acc[0]); acc[1] = fmaf(f0.y, y0, acc[1]); acc[2] = fmaf(f0.z, y0, acc[2]);
+            acc[0] = fmaf(f0.w, y1, acc[0]); acc[1] = fmaf(f1.x, y1, acc[1]); acc[2] = fmaf(f1.y, y1, acc[2]);
+            acc[0] = fmaf(f1.z, y2, acc[0]); acc[1] = fmaf(f1.w, y2, acc[1]); acc[2] = fmaf(f2.x, y2, acc[2]);
+            acc[0] = fmaf(f2.y, y3, acc[0]); acc[1] = fmaf(f2.z, y3, acc[1]); acc[2] = fmaf(f2.w, y3, acc[2]);
+          }
+      }
+    }
+#pragma unroll
+    for (int o = 1; o <= 2; o <<= 1) {
+      acc[0] += __shfl_xor_sync(0xffffffffu, acc[0], o); acc[1] += __shfl_xor_sync(0xffffffffu, acc[1], o); acc[2] += __shfl_xor_sync(0xffffffffu, acc[2], o);
+    }
+    if (have) {
+      float* dst = reinterpret_cast<float*>(rec + id);            // q1 = (cc, lo, r, g), q2 = (b, depth, radius, w)
+      if (l == 1) *reinterpret_cast<float2*>(dst + 6) = make_float2(fmaxf(acc[0] + 0.5f, 0.f), fmaxf(acc[1] + 0.5f, 0.f));
+      else if (l == 2) dst[8] = fmaxf(acc[2] + 0.5f, 0.f);
+    }
+  }
+}
+
+bool launch_colour_fwd(const fdgs_scene& sc, const Workspace& ws, int num_sms, cudaStream_t st) {
+  if (sc.N <= 0 || sc.sh_degree != 3) return false;      // the other degrees evaluate the colour inside preprocess_fwd_kernel<KD>
+  const long long groups = ((long long)sc.N + CF_THREADS / 4 - 1) / (CF_THREADS / 4);
+    // two CTAs per SM: the kernel shares the GPU with the depth sort, whose passes are chains of ~126 CTAs that slow down when
+  // they have to queue for an SM (measured at cfg3, frame ms: 1 per SM 0.503, 2: 0.493, 3: 0.501, 4: 0.506, 16: 0.507)
+  const int grid = (int)(groups < 2LL * num_sms ? groups : 2LL * num_sms);
+  colour_fwd16_kernel<<<grid, CF_THREADS, 0, st>>>(sc.sh, sc.n_time, ws.aux, ws.vis_ids, ws.hdr, ws.rec);
+  count_launch();
+  return true;
+}
+
 // Parity / measurement hook: the cull decision of every primitive (GeomStatus; 3 = empty tile rectangle), recomputed
 // from the parameters with the same device functions as the forward.
 __global__ void cull_status_kernel(const fdgs_scene sc, const ViewParams vp, const CfgParams cp, unsigned char* __restrict__ dst) {
@@ -296,13 +401,14 @@ void launch_cull_status(const fdgs_scene& sc, const ViewParams& vp, const CfgPar
   count_launch();
 }
 
-void launch_preprocess_fwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, cudaStream_t st) {
+void launch_preprocess_fwd(const fdgs_scene& sc, const ViewParams& vp, const CfgParams& cp, const Workspace& ws, cudaStream_t st, bool split_colour) {
   if (sc.N <= 0) return;
   const int threads = 128, blocks = (sc.N + threads - 1) / threads;
   const int KD = (sc.sh_degree + 1) * (sc.sh_degree + 1);
 #define FDGS_LAUNCH(KDV) preprocess_fwd_kernel<KDV><<<blocks, threads, 0, st>>>(sc, vp, cp, ws.rec, ws.rect, ws.tiles_touched, ws.tile_diff, ws.aux)
   if (KD == 1) FDGS_LAUNCH(1); else if (KD == 4) FDGS_LAUNCH(4); else if (KD == 9) FDGS_LAUNCH(9);
-  else preprocess_fwd16_kernel<<<blocks, PF_THREADS, 0, st>>>(sc, vp, cp, ws.rec, ws.rect, ws.tiles_touched, ws.tile_diff, ws.aux);
+  else if (split_colour) preprocess_fwd16_kernel<true><<<blocks, PF_THREADS, 0, st>>>(sc, vp, cp, ws.rec, ws.rect, ws.tiles_touched, ws.tile_diff, ws.aux);
+  else preprocess_fwd16_kernel<false><<<blocks, PF_THREADS, 0, st>>>(sc, vp, cp, ws.rec, ws.rect, ws.tiles_touched, ws.tile_diff, ws.aux);
 #undef FDGS_LAUNCH
   count_launch();
 }

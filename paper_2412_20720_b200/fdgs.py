@@ -140,7 +140,8 @@ def launch_count() -> int:
     return int(load().fdgs_launch_count())
 
 
-STAGES = ("preprocess", "compact+tile_grid", "sort_depth", "tile_lists", "blend_fwd", "blend_bwd", "preprocess_bwd")
+# "colour_side_stream": the colour kernel that fdgs_render_forward runs next to the depth sort and the row scatter (degree 3)
+STAGES = ("preprocess", "compact+tile_grid", "sort_depth", "tile_lists", "blend_fwd", "blend_bwd", "preprocess_bwd", "colour_side_stream")
 
 
 def set_stage_timing(on: bool):
