@@ -238,7 +238,7 @@ static int preprocess_impl(const fdgs_scene* sc, const fdgs_view* v, const fdgs_
   mark(EV_PRE0, st);
   launch_preprocess_fwd(*sc, vp, cp, ws, st, split_colour);         // A1-A4 (+ coverage grid)
   mark(EV_PRE1, st);
-  launch_compact_and_tile_grid(ws, sc->N, K, vp, cap, st);          // survivors -> (depth bits, id); A5/A8: list lengths -> ranges, D
+  launch_compact_and_tile_grid(ws, sc->N, K, vp, cp, cap, st);          // survivors -> (depth bits, id); A5/A8: list lengths -> ranges, D
   mark(EV_PRE2, st);
   FDGS_CUDA(cudaGetLastError(), "preprocess launches");
   if (num_pairs_host || num_visible_host) {
@@ -282,9 +282,9 @@ static int forward_impl(const fdgs_scene* sc, const ViewParams& vp, const CfgPar
     FDGS_CUDA(cudaEventRecord(ctx->side_join[slot], ctx->side[slot]), "join(colour)");
     join = ctx->side_join[slot];
   }
-  const int l1 = launch_sort_depth(ws, sc->N, sms, st);             // level 1: survivors by fp32 depth bits
+  launch_sort_depth(ws, sc->N, sms, st);                            // level 1: survivors by fp32 depth bits
   mark(EV_FWD1, st);
-  launch_row_scatter(ws, l1, sc->N, vp, sms, st);                       // level 2: per-tile lists written in place, depth order
+  launch_row_scatter(ws, sc->N, vp, sms, st);                       // level 2: per-tile lists written in place, depth order
   mark(EV_FWD2, st);
   if (join) FDGS_CUDA(cudaStreamWaitEvent(st, join, 0), "join(colour) wait");
   launch_blend_fwd(ws, vp, cp, image, final_T, n_contrib, depth_map, st);
@@ -293,8 +293,7 @@ static int forward_impl(const fdgs_scene* sc, const ViewParams& vp, const CfgPar
   return FDGS_OK;
 }
 
-// buffer of the depth-sorted survivor ids: a function of the pass count only
-static int depth_buf() { return DEPTH_PASSES & 1; }
+static int depth_buf() { return 0; }      // kept for the signature of launch_preprocess_bwd (unused there)
 
 // after a synchronisation: has the last preprocess on this workspace exceeded the pair capacity?
 static int read_overflow(const Workspace& ws) {
@@ -747,7 +746,7 @@ extern "C" int fdgs_debug_export(const void* ws_ptr, size_t ws_bytes, int what, 
       if (N > 0) export_rects_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(ws.rect, (int)N, (int4*)dst);
       break;
     case FDGS_EXPORT_TILES_TOUCHED: src = ws.tiles_touched; need = 4 * (size_t)N; break;
-    case FDGS_EXPORT_DEPTH_ORDER: src = ws.l1_vals[l1]; need = 4 * (size_t)h.num_visible; break;
+    case FDGS_EXPORT_DEPTH_ORDER: src = ws.sorted_ids; need = 4 * (size_t)h.num_visible; break;
     case FDGS_EXPORT_SORTED_KEYS:
       if (dst_bytes < 8 * (size_t)D) return FDGS_ERR_INVALID;
       if (D > 0) export_keys_kernel<<<(unsigned)((D + 255) / 256), 256, 0, st>>>(ws.ranges, (int)h.tiles, ws.pair_ids, ws.rec, (unsigned)D, (unsigned long long*)dst);
@@ -825,9 +824,9 @@ extern "C" int fdgs_render_forward_static(const fdgs_scene* sc, const fdgs_view*
   // cleared here; the rest is written before it is read.
   FDGS_CUDA(cudaMemsetAsync(ctx->ws, 0, ws.zero_bytes, st), "memset(static header)");
   launch_preprocess_fwd(*sc, vp, cp, ws, st, false);       // colour inside the kernel: this entry point creates nothing, not even a side stream
-  launch_compact_and_tile_grid(ws, sc->N, K, vp, cap, st);
-  const int l1 = launch_sort_depth(ws, sc->N, ctx->sms, st);
-  launch_row_scatter(ws, l1, sc->N, vp, ctx->sms, st);
+  launch_compact_and_tile_grid(ws, sc->N, K, vp, cp, cap, st);
+  launch_sort_depth(ws, sc->N, ctx->sms, st);
+  launch_row_scatter(ws, sc->N, vp, ctx->sms, st);
   launch_blend_fwd(ws, vp, cp, image, final_T, n_contrib, nullptr, st);
   if (overflow_dev) FDGS_CUDA(cudaMemcpyAsync(overflow_dev, &ws.hdr->overflow, sizeof(uint32_t), cudaMemcpyDeviceToDevice, st), "copy overflow flag");
   FDGS_CUDA(cudaGetLastError(), "static forward launches");

@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <string.h>
 
 #include "../../include/fdgs.h"
 
@@ -61,19 +62,24 @@ struct WsHeader {
   long long N, K, W, H, pair_capacity, tiles;   // layout mirror for fdgs_debug_export
 };
 
-constexpr int RADIX_BITS = 8;
+// Depth sort: LSD radix sort of key' = fp32 bits of the camera depth - fp32 bits of znear (every survivor has
+// z > znear, so key' > 0 and the order is that of the depth bits).  9-bit digits: three passes cover key' < 2^27, i.e. depths
+// up to 2^16 znear (13 km at znear = 0.2); a fourth pass over the remaining five bits is launched as well but returns at
+// once unless a survivor has such a depth (the digit counts of all four passes come from the compaction kernel).
+constexpr int RADIX_BITS = 9;
 constexpr int RADIX = 1 << RADIX_BITS;
 constexpr int SORT_THREADS = 256;
 #ifndef FDGS_SORT_ITEMS
 #define FDGS_SORT_ITEMS 8
 #endif
 constexpr int SORT_ITEMS_L1 = FDGS_SORT_ITEMS;   // 2048-key tiles: 0.206 ms per 4 views at cfg3 (4: 0.212, 16: 0.259)    // depth sort of <= N survivors: small tiles, more CTAs
-constexpr int DEPTH_PASSES = 32 / RADIX_BITS;
+constexpr int DEPTH_PASSES = 4;                  // 3 x 9 bits + the optional pass over bits 27..31
 constexpr int SCAN_THREADS = 256;
 #ifndef FDGS_SCAN_ITEMS
 #define FDGS_SCAN_ITEMS 8
 #endif
 constexpr int SCAN_ITEMS = FDGS_SCAN_ITEMS;
+static_assert(RADIX == 2 * SCAN_THREADS && RADIX == 2 * SORT_THREADS, "a thread of the compaction / sort kernels owns two digits");
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
 constexpr int RS_MIN_CHUNK = 2048, RS_MAX_CHUNK = 32768;   // survivors per chunk of the row scatter (scan_dup.cu)
 constexpr int RS_MAX_ITERS = RS_MAX_CHUNK / 32;
@@ -96,11 +102,12 @@ struct Workspace {
   SplatRec* rec;                     // [N] indexed by primitive id
   ushort4* rect;                     // [N] tx0, ty0, tx1, ty1
   unsigned int* tiles_touched;       // [N]
-  unsigned int* l1_keys[2];          // [N] fp32 depth bits of survivors (double buffer)
-  unsigned int* l1_vals[2];          // [N] primitive ids of survivors; after the sort: depth order
+  unsigned int* l1_keys[2];          // [N] depth keys of the survivors (fp32 depth bits - fp32 bits of znear; double buffer)
+  unsigned int* l1_vals[2];          // [N] primitive ids of the survivors (double buffer of the sort)
   unsigned int* vis_ids;             // [N] primitive ids of survivors in ascending id order (kept for the backward)
   unsigned int* sorted_ys;           // [N] tile rows   y0 | y1 << 16 of the survivors in depth order (written by the last depth-sort pass)
   unsigned int* sorted_xs;           // [N] tile columns x0 | x1 << 16, same order
+  unsigned int* sorted_ids;          // [N] primitive ids of the survivors in depth order (same pass: the pass count is decided on the device)
   unsigned int rs_chunk, rs_chunks;  // survivors per chunk of the row scatter; chunks N is divided into
   unsigned int* rs_state;            // [rs_chunks][tiles] look-back words of the row scatter (count of chunk c in tile T), cleared with the header
   unsigned int* pair_ids;            // [cap] primitive ids of the per-tile lists, tile after tile (ranges), depth order inside
@@ -114,6 +121,9 @@ struct Workspace {
 };
 
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+// what the compaction kernel subtracts from the fp32 depth bits of a survivor (see RADIX_BITS above)
+inline unsigned int depth_key_base(const CfgParams& cp) { unsigned int u; memcpy(&u, &cp.znear, sizeof(u)); return u; }
 
 inline Workspace carve(void* base, long long N, long long K, long long W, long long H, long long cap) {
   Workspace w;
@@ -144,6 +154,7 @@ inline Workspace carve(void* base, long long N, long long K, long long W, long l
   w.vis_ids = (unsigned int*)take(4 * Np);
   w.sorted_ys = (unsigned int*)take(4 * Np);
   w.sorted_xs = (unsigned int*)take(4 * Np);
+  w.sorted_ids = (unsigned int*)take(4 * Np);
   w.pair_ids = (unsigned int*)take(4 * (size_t)cap);
   w.ranges = (uint2*)take(sizeof(uint2) * tiles);
   w.g9 = (float*)take(4 * 9 * Np);
@@ -180,13 +191,14 @@ void launch_preprocess_fwd(const fdgs_scene& sc, const ViewParams& vp, const Cfg
 bool launch_colour_fwd(const fdgs_scene& sc, const Workspace& ws, int num_sms, cudaStream_t st);
 // compaction scan: survivors (tiles_touched > 0) in id order -> l1_keys[0] (depth bits), l1_vals[0] (ids), hdr->num_visible;
 // the same launch carries, as the role of its first CTA, the 2D prefix of the coverage difference array -> ranges, D, overflow
-void launch_compact_and_tile_grid(const Workspace& ws, int N, int K, const ViewParams& vp, long long cap, cudaStream_t st);
-// Stable LSD radix sort of the survivors' (depth bits, id) pairs on all 32 key bits; the count is read on the device and
-// ws.sort_hist[pass] holds the digit counts of the pass.  The last pass also writes the tile rectangles of the survivors
-// in the final order (sorted_ys / sorted_xs).  Returns the result buffer (0/1).
-int launch_sort_depth(const Workspace& ws, long long max_count, int num_sms, cudaStream_t st);
+void launch_compact_and_tile_grid(const Workspace& ws, int N, int K, const ViewParams& vp, const CfgParams& cp, long long cap, cudaStream_t st);
+// Stable LSD radix sort of the survivors' (depth key, id) pairs on all key bits (three 9-bit passes, a fourth if a key
+// needs it); the count is read on the device and ws.sort_hist[pass] holds the digit counts of the pass.  The last pass
+// that runs also writes the ids and the tile rectangles of the survivors in the final order (sorted_ids / sorted_ys /
+// sorted_xs).
+void launch_sort_depth(const Workspace& ws, long long max_count, int num_sms, cudaStream_t st);
 // level 2: per-tile lists in depth order written straight to their final place (scan_dup.cu "row scatter")
-void launch_row_scatter(const Workspace& ws, int l1_buf, int N, const ViewParams& vp, int num_sms, cudaStream_t st);
+void launch_row_scatter(const Workspace& ws, int N, const ViewParams& vp, int num_sms, cudaStream_t st);
 void launch_blend_fwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
                       unsigned int* n_contrib, float* depth_map /*NULL = no auxiliary channel*/, cudaStream_t st);
 void launch_blend_stats(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, unsigned long long* stats, cudaStream_t st);

@@ -133,7 +133,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) compact_kernel(const unsigned in
                                                                unsigned int* __restrict__ vals, unsigned int* __restrict__ vis_ids,
                                                                unsigned int* __restrict__ sort_hist, const int* __restrict__ tile_diff,
                                                                const int tiles_x, const int tiles_y, const unsigned int cap,
-                                                               const WsHeader mirror, uint2* __restrict__ ranges) {
+                                                               const WsHeader mirror, uint2* __restrict__ ranges, const unsigned int key_base) {
   extern __shared__ int grid[];                 // (tiles_y+1) x (tiles_x+1), used by CTA 0 only
   __shared__ unsigned int warp_sums[33], s_tile, s_prefix, hist[4][RADIX];
   if (blockIdx.x == 0) {
@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) compact_kernel(const unsigned in
   }
   if (threadIdx.x == 0) s_tile = atomicAdd(&hdr->scan_ticket[0], 1u);
 #pragma unroll
-  for (int p = 0; p < 4; ++p) hist[p][threadIdx.x] = 0;     // SCAN_THREADS == RADIX
+  for (int p = 0; p < 4; ++p) { hist[p][threadIdx.x] = 0; hist[p][threadIdx.x + SCAN_THREADS] = 0; }     // RADIX == 2 SCAN_THREADS
   __syncthreads();
   const unsigned int tile = s_tile;
   const long long base = (long long)tile * SCAN_TILE + (long long)threadIdx.x * SCAN_ITEMS;
@@ -157,9 +157,9 @@ __global__ void __launch_bounds__(SCAN_THREADS) compact_kernel(const unsigned in
 #pragma unroll
   for (int k = 0; k < SCAN_ITEMS; ++k)
     if (flags & (1u << k)) {
-      const unsigned int key = __float_as_uint(rec[base + k].depth);
+      const unsigned int key = __float_as_uint(rec[base + k].depth) - key_base;      // z > znear: the difference keeps the order of the bits
       keys[pos] = key; vals[pos] = (unsigned int)(base + k); vis_ids[pos] = (unsigned int)(base + k); ++pos;
-      // digit counts of the four depth passes.  The two low digits of an fp32 depth are spread over all 256 bins; the two
+      // digit counts of the four depth passes.  The two low digits of an fp32 depth are spread over all 512 bins; the two
       // high ones (exponent and top mantissa bits) take a handful of values in a whole scene, so a plain shared atomic would
       // serialise the CTA on one or two addresses (38 % of this kernel's stall samples): the lanes that are here together
       // are grouped by digit first and one of each group adds the group's size
@@ -176,7 +176,12 @@ __global__ void __launch_bounds__(SCAN_THREADS) compact_kernel(const unsigned in
   if (tile == gridDim.x - 2 && threadIdx.x == 0) hdr->num_visible = prefix + total;    // gridDim.x - 1 compaction tiles
   __syncthreads();
 #pragma unroll
-  for (int p = 0; p < 4; ++p) { const unsigned int v = hist[p][threadIdx.x]; if (v) atomicAdd(sort_hist + p * RADIX + threadIdx.x, v); }
+  for (int p = 0; p < 4; ++p)
+#pragma unroll
+    for (int h = 0; h < RADIX / SCAN_THREADS; ++h) {
+      const unsigned int v = hist[p][threadIdx.x + h * SCAN_THREADS];
+      if (v) atomicAdd(sort_hist + p * RADIX + threadIdx.x + h * SCAN_THREADS, v);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -375,24 +380,25 @@ __global__ void l1_loss_kernel(const float* __restrict__ image, const float* __r
   if ((threadIdx.x & 31) == 0) atomicAdd(loss, acc * inv);
 }
 
-void launch_compact_and_tile_grid(const Workspace& ws, int N, int K, const ViewParams& vp, long long cap, cudaStream_t st) {
+void launch_compact_and_tile_grid(const Workspace& ws, int N, int K, const ViewParams& vp, const CfgParams& cp, long long cap, cudaStream_t st) {
   const int blocks = N > 0 ? (N + SCAN_TILE - 1) / SCAN_TILE : 0;
   const size_t smem = 4 * (size_t)(vp.tiles_x + 1) * (vp.tiles_y + 1);
   cudaFuncSetAttribute(compact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * MAX_GRID_CELLS);   // per device, cheap: every call
   WsHeader mirror{};
   mirror.N = N; mirror.K = K; mirror.W = vp.width; mirror.H = vp.height; mirror.pair_capacity = cap; mirror.tiles = (long long)vp.tiles_x * vp.tiles_y;
   compact_kernel<<<blocks + 1, SCAN_THREADS, smem, st>>>(ws.tiles_touched, ws.rec, N, ws.hdr, ws.scan_state[0], ws.l1_keys[0], ws.l1_vals[0], ws.vis_ids,
-                                                        ws.sort_hist, ws.tile_diff, vp.tiles_x, vp.tiles_y, (unsigned int)cap, mirror, ws.ranges);
+                                                        ws.sort_hist, ws.tile_diff, vp.tiles_x, vp.tiles_y, (unsigned int)cap, mirror, ws.ranges,
+                                                        depth_key_base(cp));
   count_launch();
 }
 
-void launch_row_scatter(const Workspace& ws, int l1_buf, int N, const ViewParams& vp, int num_sms, cudaStream_t st) {
+void launch_row_scatter(const Workspace& ws, int N, const ViewParams& vp, int num_sms, cudaStream_t st) {
   if (N <= 0) return;
   const int xblocks = (vp.tiles_x + RS_XB - 1) / RS_XB;
   // the survivor count lives on the device: persistent CTAs take (chunk, row, column block) items from a ticket
   const unsigned long long items = (unsigned long long)ws.rs_chunks * (unsigned int)vp.tiles_y * xblocks;
   const unsigned int blocks = (unsigned int)(items < 8ull * num_sms ? items : 8ull * num_sms);
-  row_scatter_kernel<<<blocks, RS_THREADS, 0, st>>>(ws.hdr, ws.sorted_ys, ws.sorted_xs, ws.l1_vals[l1_buf], ws.ranges, ws.rs_state, vp.tiles_x, vp.tiles_y,
+  row_scatter_kernel<<<blocks, RS_THREADS, 0, st>>>(ws.hdr, ws.sorted_ys, ws.sorted_xs, ws.sorted_ids, ws.ranges, ws.rs_state, vp.tiles_x, vp.tiles_y,
                                                     xblocks, ws.rs_chunk, ws.pair_ids);
   count_launch();
 }

@@ -49,6 +49,40 @@ def test_single_tile_and_depth_ties():
     assert np.abs(out["image"] - o.forward()[0]).max() < 1e-5
 
 
+@pytest.mark.parametrize("far", [40.0, 60000.0])
+def test_depth_sort_pass_count_follows_the_depth_range(far):
+    """The depth sort runs three 9-bit passes over (fp32 depth bits - bits of znear) and a fourth only if a key has
+    bits above the 27th, i.e. a survivor deeper than 2^16 znear: splats from 0.3 to 40 units in front of the camera
+    take three passes, splats out to 60 000 units (18 octaves) all four.  Either way the per-tile order is that of the
+    oracle's sort on the full depth bits."""
+    import gpu_helpers as gh
+    rng = np.random.default_rng(11)
+    n = 600
+    z = np.exp(rng.uniform(np.log(0.3), np.log(far), n))                # log-uniform depth in front of the camera
+    xy = rng.uniform(-0.25, 0.25, (n, 2)) * z[:, None]                  # inside the 50 degree frustum at every depth
+    mean = np.column_stack([xy, z - 4.0, np.full(n, 0.5)])              # hand_scene puts the camera at z = -4
+    ls = np.column_stack([np.log(0.02 * z)] * 3 + [np.zeros(n)])        # footprints of a few pixels at every depth
+    sc = _f32(hand_scene(mean, ls, logit=rng.normal(0, 1, n), sh=rng.uniform(0, 2, (n, 1, 3)), width=96, height=80))
+    out = gh.gpu_run(sc, sc.views[0])
+    from paper_2412_20720_b200 import fdgs
+    o = oracle_for(sc)
+    P = o.prims()
+    off, ids = o.tile_lists()
+    assert out["num_visible"] > 0.9 * n
+    zs = P.p_cam[P.status == 0, 2]
+    assert (zs.max() > 0.2 * 2 ** 16) == (far > 1e4)                    # the case really is on the side of the limit it claims
+    order = out["renderer"].export(fdgs.EXPORT_DEPTH_ORDER).cpu().numpy()
+    d32 = out["records"][order, 9]
+    assert (np.diff(d32) >= 0).all()                                    # survivors in non-decreasing fp32 depth
+    same = d32[1:] == d32[:-1]
+    assert (order[1:][same] > order[:-1][same]).all()                   # ties in id order
+    rep = {}
+    frag = P.fragility < gh.FRAG_TOL
+    bad = gh.compare_tile_lists(out, P, off, ids, frag, rep)
+    assert bad.sum() <= 2, rep
+    assert np.abs(out["image"] - o.forward()[0]).max() < 1e-4
+
+
 def test_pair_overflow_is_reported_and_draws_nothing():
     import gpu_helpers as gh
     from paper_2412_20720_b200 import fdgs
