@@ -860,11 +860,10 @@ __global__ void __launch_bounds__(128) blend_feat_bwd_geom_kernel(const uint2* _
 // accumulators.  That replaces, per (warp, splat) hit, the 14-shuffle reduction, the nine products per pixel and the
 // per-hit atomic of the direct kernel by one STS.128 and ~1/8 of a 300-instruction flush.
 
-template <int HBUF, bool GRED = false>   // hits buffered per warp (4, 8 or 16; 8 measured best: 4 flushes too often, 16 costs occupancy)
+constexpr int HBUF = 8;   // hits buffered per warp (8 measured best: 4 flushes too often, 16 costs occupancy — profiles/r1_history.md)
 struct Bwd2Shared {
   // slots 128 .. 128 + 4 HBUF - 1: per warp, the staged form of the hits it carries over a batch boundary (slot = hit index)
   float4 s0[128 + 4 * HBUF], s1[128 + 4 * HBUF], s2[128 + 4 * HBUF];
-  float acc[GRED ? 1 : 10 * 129];     // nine sums of the colour path + (AUX) sum of wgt * dL/ddepth (unused with GRED)
   unsigned int id[128 + 4 * HBUF];
   int max_contrib;
   int hitj[4][HBUF];
@@ -872,12 +871,15 @@ struct Bwd2Shared {
   float4 pg[4][32][2];     // per warp, per lane: (gr0, gg0, gb0, gr1), (gg1, gb1, gD0, gD1)
 };
 
-template <int HBUF, bool AUX, bool GRED> __device__ __forceinline__ void bwd2_emit_global(Bwd2Shared<HBUF, GRED>&, int, int, const float*, float* __restrict__, float* __restrict__);
-
-template <int HBUF, bool AUX, bool GRED>
-__device__ __forceinline__ void bwd2_flush(Bwd2Shared<HBUF, GRED>& sm, const int warp, const int lane, const int n, const float sx0, const float sy0,
+// The warp turns round: four lanes per buffered hit, each sums 16 of the strip's 64 pixels; the four lanes then turn the
+// sums into dL/d(u, v, A, B, C, o, r, g, b) and add them straight to g9 with global reductions.  (A (tile, splat) pair is
+// hit by 1.3 strips on average, so combining the strips in shared memory first saved few reductions and cost 5 KB, the
+// zeroing of the accumulators and a barrier per batch: 2.86 -> 2.80 ms/step at cfg3 when it was removed.)
+template <bool AUX>
+__device__ __forceinline__ void bwd2_flush(Bwd2Shared& sm, const int warp, const int lane, const int n, const float sx0, const float sy0,
                                            float* __restrict__ g9, float* __restrict__ gz) {
-  constexpr int LPH = 32 / HBUF;             // lanes per buffered hit (4 or 8); each sums 64 / LPH pixels
+  constexpr int LPH = 32 / HBUF;             // lanes per buffered hit
+  static_assert(LPH == 4, "the raw-moment expansion below is written for four lanes per hit");
   __syncwarp();
   const int h = lane / LPH, q = lane % LPH;
   float S[10] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};   // Sx, Sy, Sxx, Sxy, Syy, cr, cg, cb, S1, (AUX) Sz
@@ -887,119 +889,71 @@ __device__ __forceinline__ void bwd2_flush(Bwd2Shared<HBUF, GRED>& sm, const int
     const float4 c = sm.s2[j];
     const float ux = c.y - (sx0 + 0.5f) - (float)(q & 7), vy = c.z - (sy0 + 0.5f);
     const float4* row = sm.hit[warp][h];
-    if constexpr (LPH == 4) {
-      // The lane's pixels sit at fixed offsets from its first one — column 4 (i & 1), row (i >> 1), + 4 rows in sub-patch
-      // 1 — so the five moment sums about the splat centre (ux, vy) follow from a handful of offset-weighted sums of
-      // dpow (small integer weights, most of them 0) instead of 19 operations per pixel pair:
-      //   sum dpow (ux - a)^m (vy - b)^n = binomial expansion in the raw sums below.
-      float M0 = 0.f, T4 = 0.f, Z = 0.f, Z4 = 0.f, W1 = 0.f, W2 = 0.f, V = 0.f, X1 = 0.f;
+    // The lane's pixels sit at fixed offsets from its first one — column 4 (i & 1), row (i >> 1), + 4 rows in sub-patch
+    // 1 — so the five moment sums about the splat centre (ux, vy) follow from a handful of offset-weighted sums of
+    // dpow (small integer weights, most of them 0) instead of 19 operations per pixel pair:
+    //   sum dpow (ux - a)^m (vy - b)^n = binomial expansion in the raw sums below.
+    float M0 = 0.f, T4 = 0.f, Z = 0.f, Z4 = 0.f, W1 = 0.f, W2 = 0.f, V = 0.f, X1 = 0.f;
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const int p = 4 * i + q;
-        const float4 d = row[p];               // dpow0, wgt0, dpow1, wgt1
-        const float4 g0 = sm.pg[warp][p][0], g1 = sm.pg[warp][p][1];
-        const float t = d.x + d.z, b0 = (float)(i >> 1);
-        M0 += t; Z += d.z;
-        if (i >> 1) { W1 = fmaf(b0, t, W1); W2 = fmaf(b0 * b0, t, W2); V = fmaf(b0, d.z, V); }
-        if (i & 1) { T4 += t; Z4 += d.z; if (i >> 1) X1 = fmaf(b0, t, X1); }
-        S[5] = fmaf(d.y, g0.x, S[5]); S[6] = fmaf(d.y, g0.y, S[6]); S[7] = fmaf(d.y, g0.z, S[7]);
-        S[5] = fmaf(d.w, g0.w, S[5]); S[6] = fmaf(d.w, g1.x, S[6]); S[7] = fmaf(d.w, g1.y, S[7]);
-        if (AUX) { S[9] = fmaf(d.y, g1.z, S[9]); S[9] = fmaf(d.w, g1.w, S[9]); }
-      }
-      const float Mx = 4.f * T4, Mxx = 16.f * T4;                       // sum a t, sum a^2 t            (a = 0 or 4)
-      const float My = fmaf(4.f, Z, W1);                                // sum (b0 t + 4 dpow1)
-      const float Myy = fmaf(16.f, Z, fmaf(8.f, V, W2));                // sum (b0^2 t + (8 b0 + 16) dpow1)
-      const float Mxy = 4.f * fmaf(4.f, Z4, X1);                        // sum a (b0 t + 4 dpow1)
-      S[0] = fmaf(ux, M0, -Mx); S[1] = fmaf(vy, M0, -My);
-      S[2] = fmaf(ux, fmaf(ux, M0, -2.f * Mx), Mxx);
-      S[3] = fmaf(ux, fmaf(vy, M0, -My), fmaf(-vy, Mx, Mxy));
-      S[4] = fmaf(vy, fmaf(vy, M0, -2.f * My), Myy);
-      S[8] = M0;
-    } else
-#pragma unroll
-    for (int i = 0; i < 32 / LPH; ++i) {     // pixel slot p = LPH i + q: column (p % 8), row (p / 8) of both sub-patches
-      const int p = LPH * i + q;
+    for (int i = 0; i < 8; ++i) {
+      const int p = 4 * i + q;
       const float4 d = row[p];               // dpow0, wgt0, dpow1, wgt1
-      const float4 g0 = sm.pg[warp][p][0], g1 = sm.pg[warp][p][1];
-      const float dx = ux - (float)((LPH * i) & 7);
-      const float dy0 = vy - (float)((LPH * i) >> 3), dy1 = dy0 - 4.0f;
-      const float mx0 = d.x * dx, my0 = d.x * dy0, mx1 = d.z * dx, my1 = d.z * dy1;
-      S[0] += mx0; S[0] += mx1; S[1] += my0; S[1] += my1;
-      S[2] = fmaf(mx0, dx, S[2]); S[2] = fmaf(mx1, dx, S[2]);
-      S[3] = fmaf(mx0, dy0, S[3]); S[3] = fmaf(mx1, dy1, S[3]);
-      S[4] = fmaf(my0, dy0, S[4]); S[4] = fmaf(my1, dy1, S[4]);
+      const float4 g0 = sm.pg[warp][p][0];
+      float4 g1;                             // without the auxiliary channels only (gg1, gb1) is needed: a 64-bit load is half the wavefronts
+      if (AUX) g1 = sm.pg[warp][p][1];
+      else { const float2 h = *reinterpret_cast<const float2*>(&sm.pg[warp][p][1]); g1 = make_float4(h.x, h.y, 0.f, 0.f); }
+      const float t = d.x + d.z, b0 = (float)(i >> 1);
+      M0 += t; Z += d.z;
+      if (i >> 1) { W1 = fmaf(b0, t, W1); W2 = fmaf(b0 * b0, t, W2); V = fmaf(b0, d.z, V); }
+      if (i & 1) { T4 += t; Z4 += d.z; if (i >> 1) X1 = fmaf(b0, t, X1); }
       S[5] = fmaf(d.y, g0.x, S[5]); S[6] = fmaf(d.y, g0.y, S[6]); S[7] = fmaf(d.y, g0.z, S[7]);
       S[5] = fmaf(d.w, g0.w, S[5]); S[6] = fmaf(d.w, g1.x, S[6]); S[7] = fmaf(d.w, g1.y, S[7]);
-      S[8] += d.x; S[8] += d.z;
       if (AUX) { S[9] = fmaf(d.y, g1.z, S[9]); S[9] = fmaf(d.w, g1.w, S[9]); }
     }
+    const float Mx = 4.f * T4, Mxx = 16.f * T4;                       // sum a t, sum a^2 t            (a = 0 or 4)
+    const float My = fmaf(4.f, Z, W1);                                // sum (b0 t + 4 dpow1)
+    const float Myy = fmaf(16.f, Z, fmaf(8.f, V, W2));                // sum (b0^2 t + (8 b0 + 16) dpow1)
+    const float Mxy = 4.f * fmaf(4.f, Z4, X1);                        // sum a (b0 t + 4 dpow1)
+    S[0] = fmaf(ux, M0, -Mx); S[1] = fmaf(vy, M0, -My);
+    S[2] = fmaf(ux, fmaf(ux, M0, -2.f * Mx), Mxx);
+    S[3] = fmaf(ux, fmaf(vy, M0, -My), fmaf(-vy, Mx, Mxy));
+    S[4] = fmaf(vy, fmaf(vy, M0, -2.f * My), Myy);
+    S[8] = M0;
   }
 #pragma unroll
   for (int k = 0; k < (AUX ? 10 : 9); ++k)
 #pragma unroll
     for (int o = 1; o < LPH; o <<= 1) S[k] += __shfl_xor_sync(0xffffffffu, S[k], o);
-  if (GRED && LPH == 4) {
-    if (h < n) bwd2_emit_global<HBUF, AUX, GRED>(sm, q, j, S, g9, gz);
-    __syncwarp();
-    return;
-  }
-  if (h < n) {                               // every lane of the hit holds all nine sums: lane q adds rows q, q + LPH, ...
-    if (LPH == 2) {
-      atomicAdd(&sm.acc[q * 129 + j], q ? S[1] : S[0]);
-      atomicAdd(&sm.acc[(q + 2) * 129 + j], q ? S[3] : S[2]);
-      atomicAdd(&sm.acc[(q + 4) * 129 + j], q ? S[5] : S[4]);
-      atomicAdd(&sm.acc[(q + 6) * 129 + j], q ? S[7] : S[6]);
-    } else if (LPH == 4) {
-      const float r0 = q == 0 ? S[0] : q == 1 ? S[1] : q == 2 ? S[2] : S[3];
-      const float r1 = q == 0 ? S[4] : q == 1 ? S[5] : q == 2 ? S[6] : S[7];
-      atomicAdd(&sm.acc[q * 129 + j], r0);
-      atomicAdd(&sm.acc[(q + 4) * 129 + j], r1);
-    } else {
-      float r0 = S[0];
-#pragma unroll
-      for (int k = 1; k < 8; ++k) r0 = q == k ? S[k] : r0;
-      atomicAdd(&sm.acc[q * 129 + j], r0);
-    }
-    if (q == 0) atomicAdd(&sm.acc[8 * 129 + j], S[8]);
-    if (AUX && q == 1) atomicAdd(&sm.acc[9 * 129 + j], S[9]);
+  if (h < n) {
+    const float4 a = sm.s0[j];
+    const float ik = 1.0f / 0.72134752044448170f;
+    const float A = a.x * a.x * ik, B = a.x * a.y * ik, C = fmaf(a.y, a.y, a.z * a.z) * ik;
+    float* dst = g9 + (size_t)9 * sm.id[j];
+    float v0, v1; int i0, i1;
+    if (q == 0)      { v0 = -fmaf(A, S[0], B * S[1]); i0 = 0; v1 = -0.5f * S[4]; i1 = 4; }
+    else if (q == 1) { v0 = -fmaf(B, S[0], C * S[1]); i0 = 1; v1 = S[5]; i1 = 6; }
+    else if (q == 2) { v0 = -0.5f * S[2]; i0 = 2; v1 = S[6]; i1 = 7; }
+    else             { v0 = -S[3]; i0 = 3; v1 = S[7]; i1 = 8; }
+    if (v0 != 0.f) atomicAdd(dst + i0, v0);
+    if (v1 != 0.f) atomicAdd(dst + i1, v1);
+    if (q == 0 && S[8] != 0.f) atomicAdd(dst + 5, S[8] * exp2f(-sm.s1[j].y));   // o may underflow to 0 (marginal filter off): then nothing composited, S1 == 0
+    if (AUX && q == 1 && S[9] != 0.f) atomicAdd(gz + sm.id[j], S[9]);
   }
   __syncwarp();
-}
-
-// End of bwd2_flush without shared accumulators (GRED, the default): the four lanes of a hit turn the sums into
-// dL/d(u, v, A, B, C, o, r, g, b) and add them straight to g9 with global reductions.  A (tile, splat) pair is hit by 1.3
-// strips on average, so combining the strips in shared memory first saves few reductions and costs 5 KB, the zeroing of
-// the accumulators and a barrier per batch: 2.86 -> 2.80 ms/step at cfg3, 0.67 -> 0.66 ms per view at cfg4.
-template <int HBUF, bool AUX, bool GRED>
-__device__ __forceinline__ void bwd2_emit_global(Bwd2Shared<HBUF, GRED>& sm, const int q, const int j, const float* S, float* __restrict__ g9,
-                                                 float* __restrict__ gz) {
-  const float4 a = sm.s0[j];
-  const float ik = 1.0f / 0.72134752044448170f;
-  const float A = a.x * a.x * ik, B = a.x * a.y * ik, C = fmaf(a.y, a.y, a.z * a.z) * ik;
-  float* dst = g9 + (size_t)9 * sm.id[j];
-  float v0, v1; int i0, i1;
-  if (q == 0)      { v0 = -fmaf(A, S[0], B * S[1]); i0 = 0; v1 = -0.5f * S[4]; i1 = 4; }
-  else if (q == 1) { v0 = -fmaf(B, S[0], C * S[1]); i0 = 1; v1 = S[5]; i1 = 6; }
-  else if (q == 2) { v0 = -0.5f * S[2]; i0 = 2; v1 = S[6]; i1 = 7; }
-  else             { v0 = -S[3]; i0 = 3; v1 = S[7]; i1 = 8; }
-  if (v0 != 0.f) atomicAdd(dst + i0, v0);
-  if (v1 != 0.f) atomicAdd(dst + i1, v1);
-  if (q == 0 && S[8] != 0.f) atomicAdd(dst + 5, S[8] * exp2f(-sm.s1[j].y));
-  if (AUX && q == 1 && S[9] != 0.f) atomicAdd(gz + sm.id[j], S[9]);
 }
 
 // AUX = true: upstream gradients of the auxiliary channels as well (either pointer may be NULL): dL/ddepth enters as a
 // fourth colour channel (g.c_k -> g.c_k + gD z_k, one more sum Sz = sum wgt gD -> gz[id] = dL/dz_k), dL/dopacity
 // (O = 1 - T_final) only shifts the start of the colour-behind recurrence: s_last = T_final (g.bg - gO).
-template <int HBUF, int MINB, bool AUX, bool GRED, bool DEF>
+template <int MINB, bool AUX, bool DEF>
 __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __restrict__ ranges, const unsigned int* __restrict__ vals,
                                                          const SplatRec* __restrict__ rec, const ViewParams vp, const CfgParams cp,
                                                          const float* __restrict__ dL_dimage, const float* __restrict__ final_T,
                                                          const unsigned int* __restrict__ n_contrib, float* __restrict__ g9,
                                                          const float* __restrict__ dL_ddepth, const float* __restrict__ dL_dopacity,
                                                          float* __restrict__ gz) {
-  constexpr int PX = 2, BATCH = 128, ACC_STRIDE = 129;
-  __shared__ Bwd2Shared<HBUF, GRED> sm;
+  constexpr int PX = 2, BATCH = 128;
+  __shared__ Bwd2Shared sm;
   const int tile = blockIdx.x, tx = tile % vp.tiles_x, ty = tile / vp.tiles_x;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const Strip<PX> sp(warp, lane);
@@ -1045,10 +999,6 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
       const unsigned int id = vals[range.x + lo_pos + threadIdx.x];
       sm.id[threadIdx.x] = id;
       stage_splat(rec, id, ox, oy, &sm.s0[threadIdx.x], &sm.s1[threadIdx.x], &sm.s2[threadIdx.x]);
-    }
-    if (!GRED) {
-#pragma unroll
-      for (int k = 0; k < (AUX ? 10 : 9); ++k) sm.acc[k * ACC_STRIDE + threadIdx.x] = 0.f;
     }
     __syncthreads();
     if (lo_pos < lane_max) {
@@ -1099,10 +1049,10 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
         }
         sm.hit[warp][nbuf][lane] = make_float4(dpow[0], wgt[0], dpow[1], wgt[1]);
         if (lane == 0) sm.hitj[warp][nbuf] = j;
-        if (++nbuf == HBUF) { bwd2_flush<HBUF, AUX, GRED>(sm, warp, lane, HBUF, sx0, sy0, g9, gz); nbuf = 0; }
+        if (++nbuf == HBUF) { bwd2_flush<AUX>(sm, warp, lane, HBUF, sx0, sy0, g9, gz); nbuf = 0; }
       }
      }
-     if (GRED && nbuf) {
+     if (nbuf) {
        // a partly filled buffer is not flushed at the batch boundary (a flush costs the same for 1 hit as for 8, and 19 %
        // of the flushes were such): the staged form of its hits moves to the warp's carry slots, which the next batch's
        // staging does not touch, and the buffer goes on filling
@@ -1111,29 +1061,10 @@ __global__ void __launch_bounds__(128, MINB) blend_bwd2_kernel(const uint2* __re
          if (j < BATCH) { sm.s0[dst] = sm.s0[j]; sm.s1[dst] = sm.s1[j]; sm.s2[dst] = sm.s2[j]; sm.id[dst] = sm.id[j]; sm.hitj[warp][lane] = dst; }
        }
        __syncwarp();
-     } else if (nbuf) { bwd2_flush<HBUF, AUX, GRED>(sm, warp, lane, nbuf, sx0, sy0, g9, gz); nbuf = 0; }
+     }
     }
-    if (GRED) continue;                                 // gradients already in g9 (the loop-top barrier protects the staging arrays)
-    __syncthreads();
-    if ((int)threadIdx.x < m) {
-      const int j = threadIdx.x;
-      const float Sx = sm.acc[j], Sy = sm.acc[ACC_STRIDE + j], Sxx = sm.acc[2 * ACC_STRIDE + j], Sxy = sm.acc[3 * ACC_STRIDE + j];
-      const float Syy = sm.acc[4 * ACC_STRIDE + j], S1 = sm.acc[8 * ACC_STRIDE + j];
-      const float4 a = sm.s0[j];
-      const float ik = 1.0f / 0.72134752044448170f;                    // conic (A, B, C) from its exp2-scaled factor
-      const float A = a.x * a.x * ik, B = a.x * a.y * ik, C = fmaf(a.y, a.y, a.z * a.z) * ik;
-      float out[9];
-      out[0] = -fmaf(A, Sx, B * Sy); out[1] = -fmaf(B, Sx, C * Sy);
-      out[2] = -0.5f * Sxx; out[3] = -Sxy; out[4] = -0.5f * Syy;
-      out[5] = S1 != 0.f ? S1 * exp2f(-sm.s1[j].y) : 0.f;   // o may underflow to 0 (marginal filter off): then nothing composited, S1 == 0
-      out[6] = sm.acc[5 * ACC_STRIDE + j]; out[7] = sm.acc[6 * ACC_STRIDE + j]; out[8] = sm.acc[7 * ACC_STRIDE + j];
-      float* dst = g9 + (size_t)9 * sm.id[j];
-#pragma unroll
-      for (int k = 0; k < 9; ++k) if (out[k] != 0.f) atomicAdd(dst + k, out[k]);
-      if (AUX) { const float sz = sm.acc[9 * ACC_STRIDE + j]; if (sz != 0.f) atomicAdd(gz + sm.id[j], sz); }
-    }
-  }
-  if (GRED && nbuf) bwd2_flush<HBUF, AUX, GRED>(sm, warp, lane, nbuf, sx0, sy0, g9, gz);     // what the last batch left
+  }                                                     // gradients are already in g9 (the loop-top barrier protects the staging arrays)
+  if (nbuf) bwd2_flush<AUX>(sm, warp, lane, nbuf, sx0, sy0, g9, gz);     // what the last batch left
 }
 
 void launch_blend_fwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,
@@ -1159,7 +1090,7 @@ void launch_blend_bwd(const Workspace& ws, const ViewParams& vp, const CfgParams
                       const float* final_T, const unsigned int* n_contrib, const float* dL_ddepth, const float* dL_dopacity,
                       cudaStream_t st) {
   const int tiles = vp.tiles_x * vp.tiles_y;
-#define FDGS_BWD(MINB, AUXV, DEFV) blend_bwd2_kernel<8, MINB, AUXV, true, DEFV><<<tiles, 128, 0, st>>>(ws.ranges, ws.pair_ids, ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9, dL_ddepth, dL_dopacity, ws.gz)
+#define FDGS_BWD(MINB, AUXV, DEFV) blend_bwd2_kernel<MINB, AUXV, DEFV><<<tiles, 128, 0, st>>>(ws.ranges, ws.pair_ids, ws.rec, vp, cp, dL_dimage, final_T, n_contrib, ws.g9, dL_ddepth, dL_dopacity, ws.gz)
   if (dL_ddepth || dL_dopacity) { if (cp.default_thresholds) FDGS_BWD(6, true, true); else FDGS_BWD(6, true, false); }
   else                          { if (cp.default_thresholds) FDGS_BWD(7, false, true); else FDGS_BWD(7, false, false); }
 #undef FDGS_BWD
