@@ -209,7 +209,10 @@ __global__ void __launch_bounds__(SCAN_THREADS) compact_kernel(const unsigned in
 constexpr int RS_THREADS = 256, RS_LC = 512, RS_WORDS = RS_LC / 32, RS_XB = 128;
 constexpr unsigned int RS_AGG = 1u << 30, RS_PRE = 2u << 30, RS_MASK = (1u << 30) - 1;
 
-__global__ void __launch_bounds__(RS_THREADS) row_scatter_kernel(WsHeader* hdr, const unsigned int* __restrict__ ys, const unsigned int* __restrict__ xs,
+// 6 CTAs per SM (40 registers): alone the kernel is 4 % faster at the 8 CTAs per SM the compiler picks by itself (32 registers),
+// but it never runs alone in a step or in playback — with 6 the other views' front ends find room next to it: step
+// 4.503 -> 4.475 ms, four frames in flight 2268 -> 2372 FPS, single frame 0.490 -> 0.493 ms (profiles/r2_front_end_history.md)
+__global__ void __launch_bounds__(RS_THREADS, 6) row_scatter_kernel(WsHeader* hdr, const unsigned int* __restrict__ ys, const unsigned int* __restrict__ xs,
                                                                  const unsigned int* __restrict__ ids, const uint2* __restrict__ ranges,
                                                                  volatile unsigned int* lb_state, const int tiles_x, const int tiles_y,
                                                                  const int xblocks, const unsigned int chunk, unsigned int* __restrict__ pair_ids) {
