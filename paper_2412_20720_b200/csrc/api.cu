@@ -284,7 +284,8 @@ static int forward_impl(const fdgs_scene* sc, const ViewParams& vp, const CfgPar
   }
   launch_sort_depth(ws, sc->N, sms, st);                            // level 1: survivors by fp32 depth bits
   mark(EV_FWD1, st);
-  launch_row_scatter(ws, sc->N, vp, sms, st);                       // level 2: per-tile lists written in place, depth order
+  launch_row_ballots(ws, sc->N, vp, sms, st);                       // level 2: which survivors cover which tile row ...
+  launch_row_scatter(ws, sc->N, vp, sms, st);                       // ... and the per-tile lists written in place, depth order
   mark(EV_FWD2, st);
   if (join) FDGS_CUDA(cudaStreamWaitEvent(st, join, 0), "join(colour) wait");
   launch_blend_fwd(ws, vp, cp, image, final_T, n_contrib, depth_map, st);
@@ -826,6 +827,7 @@ extern "C" int fdgs_render_forward_static(const fdgs_scene* sc, const fdgs_view*
   launch_preprocess_fwd(*sc, vp, cp, ws, st, false);       // colour inside the kernel: this entry point creates nothing, not even a side stream
   launch_compact_and_tile_grid(ws, sc->N, K, vp, cp, cap, st);
   launch_sort_depth(ws, sc->N, ctx->sms, st);
+  launch_row_ballots(ws, sc->N, vp, ctx->sms, st);
   launch_row_scatter(ws, sc->N, vp, ctx->sms, st);
   launch_blend_fwd(ws, vp, cp, image, final_T, n_contrib, nullptr, st);
   if (overflow_dev) FDGS_CUDA(cudaMemcpyAsync(overflow_dev, &ws.hdr->overflow, sizeof(uint32_t), cudaMemcpyDeviceToDevice, st), "copy overflow flag");

@@ -108,6 +108,8 @@ struct Workspace {
   unsigned int* sorted_ys;           // [N] tile rows   y0 | y1 << 16 of the survivors in depth order (written by the last depth-sort pass)
   unsigned int* sorted_xs;           // [N] tile columns x0 | x1 << 16, same order
   unsigned int* sorted_ids;          // [N] primitive ids of the survivors in depth order (same pass: the pass count is decided on the device)
+  unsigned int* row_ballots;         // [tiles_y][rb_stride] bit i of word (y, it): survivor 32 it + i (depth order) covers tile row y
+  size_t rb_stride;                  // words per tile row (>= ceil(N / 32))
   unsigned int rs_chunk, rs_chunks;  // survivors per chunk of the row scatter; chunks N is divided into
   unsigned int* rs_state;            // [rs_chunks][tiles] look-back words of the row scatter (count of chunk c in tile T), cleared with the header
   unsigned int* pair_ids;            // [cap] primitive ids of the per-tile lists, tile after tile (ranges), depth order inside
@@ -155,6 +157,8 @@ inline Workspace carve(void* base, long long N, long long K, long long W, long l
   w.sorted_ys = (unsigned int*)take(4 * Np);
   w.sorted_xs = (unsigned int*)take(4 * Np);
   w.sorted_ids = (unsigned int*)take(4 * Np);
+  w.rb_stride = (size_t)((Np + 31) / 32 + 31) / 32 * 32;
+  w.row_ballots = (unsigned int*)take(4 * w.rb_stride * (size_t)ty);
   w.pair_ids = (unsigned int*)take(4 * (size_t)cap);
   w.ranges = (uint2*)take(sizeof(uint2) * tiles);
   w.g9 = (float*)take(4 * 9 * Np);
@@ -197,6 +201,8 @@ void launch_compact_and_tile_grid(const Workspace& ws, int N, int K, const ViewP
 // that runs also writes the ids and the tile rectangles of the survivors in the final order (sorted_ids / sorted_ys /
 // sorted_xs).
 void launch_sort_depth(const Workspace& ws, long long max_count, int num_sms, cudaStream_t st);
+// level 2, first half: which survivors (depth order) cover which tile row, one ballot word per (row, 32 survivors)
+void launch_row_ballots(const Workspace& ws, int N, const ViewParams& vp, int num_sms, cudaStream_t st);
 // level 2: per-tile lists in depth order written straight to their final place (scan_dup.cu "row scatter")
 void launch_row_scatter(const Workspace& ws, int N, const ViewParams& vp, int num_sms, cudaStream_t st);
 void launch_blend_fwd(const Workspace& ws, const ViewParams& vp, const CfgParams& cp, float* image, float* final_T,

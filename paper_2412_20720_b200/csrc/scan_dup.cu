@@ -193,9 +193,9 @@ __global__ void __launch_bounds__(SCAN_THREADS) compact_kernel(const unsigned in
 // pairs by tile id produces.  The ranges are already known from the coverage grid, and the covered sets are rectangles,
 // i.e. x-intervals in every tile row, so no sort is needed.  One CTA owns (chunk c of RS-chunk consecutive survivors,
 // tile row y, block of RS_XB tile columns):
-//   1. filter: the CTA scans the chunk's y-ranges (4 bytes per survivor, coalesced) and keeps the survivors that cover
-//      its row — ballots, so the hits stay in depth order; their x-intervals go into a 1D difference array, whose prefix
-//      is the chunk's count for every tile of the row;
+//   1. filter: which survivors of the chunk cover the row is read from the ballot words of row_ballot_kernel (one word
+//      per 32 survivors, computed once for all rows); the hits stay in depth order; their x-intervals go into a 1D
+//      difference array, whose prefix is the chunk's count for every tile of the row;
 //   2. the counts are published at once and the exclusive prefix over the earlier chunks of the same row is fetched by
 //      decoupled look-back (per tile column; chunk ids come from a ticket, so every predecessor is already running);
 //      ranges[T].x + that prefix = where this chunk starts writing in tile T;
@@ -209,14 +209,40 @@ __global__ void __launch_bounds__(SCAN_THREADS) compact_kernel(const unsigned in
 constexpr int RS_THREADS = 256, RS_LC = 512, RS_WORDS = RS_LC / 32, RS_XB = 128;
 constexpr unsigned int RS_AGG = 1u << 30, RS_PRE = 2u << 30, RS_MASK = (1u << 30) - 1;
 
+// Row filter of the row scatter, once for all rows: a warp takes 32 consecutive survivors (depth order), loads their row
+// ranges once and votes row by row; lane y % 32 keeps the ballot of row y and stores it at (row, iteration).  The scatter
+// items (chunk, row) then read their ballots — one word per 32 survivors — instead of every item scanning the whole
+// chunk: rows x survivors tests (a third of the scatter's instructions at cfg3, most of them at 8 M Gaussians) become
+// survivors / 32 loads plus ~3 instructions per (row, 32 survivors).
+__global__ void __launch_bounds__(256) row_ballot_kernel(const WsHeader* __restrict__ hdr, const unsigned int* __restrict__ ys, const int tiles_y,
+                                                         const size_t stride, unsigned int* __restrict__ bal) {
+  const unsigned int n = hdr->num_visible;
+  if (hdr->overflow) return;
+  const unsigned int iters = (n + 31) / 32, lane = threadIdx.x & 31;
+  const unsigned int gw = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), nw = gridDim.x * (blockDim.x >> 5);
+  for (unsigned int it = gw; it < iters; it += nw) {
+    const unsigned int j = it * 32 + lane;
+    const unsigned int yv = j < n ? ys[j] : 0u;                          // y0 = y1 = 0: covers no row
+    const int y0 = (int)(yv & 0xffffu), y1 = (int)(yv >> 16);
+    for (int yb = 0; yb < tiles_y; yb += 32) {
+      unsigned int mine = 0;
+#pragma unroll
+      for (int k = 0; k < 32; ++k) {
+        const unsigned int b = __ballot_sync(0xffffffffu, y0 <= yb + k && y1 > yb + k);
+        if ((int)lane == k) mine = b;
+      }
+      if (yb + (int)lane < tiles_y) bal[(size_t)(yb + lane) * stride + it] = mine;
+    }
+  }
+}
+
 // 6 CTAs per SM (40 registers): alone the kernel is 4 % faster at the 8 CTAs per SM the compiler picks by itself (32 registers),
 // but it never runs alone in a step or in playback — with 6 the other views' front ends find room next to it: step
 // 4.503 -> 4.475 ms, four frames in flight 2268 -> 2372 FPS, single frame 0.490 -> 0.493 ms (profiles/r2_front_end_history.md)
-__global__ void __launch_bounds__(RS_THREADS, 6) row_scatter_kernel(WsHeader* hdr, const unsigned int* __restrict__ ys, const unsigned int* __restrict__ xs,
+__global__ void __launch_bounds__(RS_THREADS, 6) row_scatter_kernel(WsHeader* hdr, const unsigned int* __restrict__ bal, const size_t bal_stride, const unsigned int* __restrict__ xs,
                                                                  const unsigned int* __restrict__ ids, const uint2* __restrict__ ranges,
                                                                  volatile unsigned int* lb_state, const int tiles_x, const int tiles_y,
                                                                  const int xblocks, const unsigned int chunk, unsigned int* __restrict__ pair_ids) {
-  constexpr int UN = 8;                                // survivors per thread in flight: the scan is latency-bound otherwise
   __shared__ unsigned int mask[RS_WORDS][RS_XB], pref[RS_WORDS][RS_XB];
   __shared__ unsigned int list_j[RS_LC], list_x[RS_LC];
   __shared__ unsigned int bal_s[RS_MAX_ITERS];
@@ -239,25 +265,13 @@ __global__ void __launch_bounds__(RS_THREADS, 6) row_scatter_kernel(WsHeader* hd
     if ((unsigned long long)c * chunk >= n) return;     // tickets are dense: every chunk below this one exists
     const int y = rr / xblocks, xbase = (rr % xblocks) * RS_XB, nx = min(RS_XB, tiles_x - xbase);
     const unsigned int j0 = c * chunk, j1 = min(n, j0 + chunk);
-    const unsigned int iters = (j1 - j0 + 31) / 32, trips = (iters + RS_THREADS / 32 - 1) / (RS_THREADS / 32);
-    // Survivor j0 + 32 it + lane is lane `lane` of "iteration" it; thread (warp, lane) takes the iterations 8 i + warp.
-    // ---- 1. filter on the tile rows (and, with several column blocks, on the columns): one ballot per iteration ----
-    for (unsigned int i0 = 0; i0 < trips; i0 += UN) {
-      unsigned int yv[UN], xv[UN];
-#pragma unroll
-      for (int u = 0; u < UN; ++u) {
-        const unsigned int j = j0 + (i0 + u) * RS_THREADS + threadIdx.x;
-        yv[u] = j < j1 ? ys[j] : 0u;                              // y0 = y1 = 0: covers no row
-        xv[u] = (xblocks > 1 && j < j1) ? xs[j] : 0xffff0000u;    // one column block: every x-interval intersects it
-      }
-#pragma unroll
-      for (int u = 0; u < UN; ++u) {
-        const unsigned int it = (i0 + u) * (RS_THREADS / 32) + warp;
-        const bool hit = (int)(yv[u] & 0xffffu) <= y && (int)(yv[u] >> 16) > y &&
-                         (int)(xv[u] & 0xffffu) < xbase + nx && (int)(xv[u] >> 16) > xbase;
-        const unsigned int bal = __ballot_sync(0xffffffffu, hit);
-        if (lane == 0 && it < iters) { bal_s[it] = bal; off[it] = (unsigned short)__popc(bal); }
-      }
+    const unsigned int iters = (j1 - j0 + 31) / 32;
+    // ---- 1. the survivors of the chunk that cover this row: ballot words of row_ballot_kernel, one per 32 survivors
+    //         (survivor j0 + 32 it + i is bit i of word it).  With several column blocks the hits of the other blocks stay
+    //         in the list with an empty x-interval. ----
+    for (unsigned int it = threadIdx.x; it < iters; it += RS_THREADS) {
+      const unsigned int b = bal[(size_t)y * bal_stride + (j0 >> 5) + it];
+      bal_s[it] = b; off[it] = (unsigned short)__popc(b);
     }
     __syncthreads();
     if (warp == 0) {                          // exclusive prefix of the per-iteration hit counts
@@ -298,7 +312,8 @@ __global__ void __launch_bounds__(RS_THREADS, 6) row_scatter_kernel(WsHeader* hd
       const unsigned int m = H > r0 ? min((unsigned int)RS_LC, H - r0) : 0u;
       for (unsigned int hl = threadIdx.x; hl < m; hl += RS_THREADS) {
         const unsigned int xw = xs[list_j[hl]];
-        const unsigned int x0 = (unsigned int)max((int)(xw & 0xffffu) - xbase, 0), x1 = (unsigned int)min((int)(xw >> 16) - xbase, nx);
+        const int xa = min(max((int)(xw & 0xffffu) - xbase, 0), nx);           // clamped to the column block; a hit that lies in another
+        const unsigned int x0 = (unsigned int)xa, x1 = (unsigned int)max(min((int)(xw >> 16) - xbase, nx), xa);   // block keeps an empty interval
         list_x[hl] = x0 | (x1 << 16);
         if (r0 == 0) { atomicAdd(&diff[x0], 1); atomicAdd(&diff[x1], -1); }
         const unsigned int bitv = 1u << (hl & 31);
@@ -313,7 +328,8 @@ __global__ void __launch_bounds__(RS_THREADS, 6) row_scatter_kernel(WsHeader* hd
               bal &= bal - 1;
               if (h >= RS_LC) {
                 const unsigned int xw = xs[j0 + it * 32 + bit];
-                atomicAdd(&diff[max((int)(xw & 0xffffu) - xbase, 0)], 1); atomicAdd(&diff[min((int)(xw >> 16) - xbase, nx)], -1);
+                const int xa = min(max((int)(xw & 0xffffu) - xbase, 0), nx);
+                atomicAdd(&diff[xa], 1); atomicAdd(&diff[max(min((int)(xw >> 16) - xbase, nx), xa)], -1);
               }
               ++h;
             }
@@ -395,13 +411,21 @@ void launch_compact_and_tile_grid(const Workspace& ws, int N, int K, const ViewP
   count_launch();
 }
 
+void launch_row_ballots(const Workspace& ws, int N, const ViewParams& vp, int num_sms, cudaStream_t st) {
+  if (N <= 0) return;
+  const long long warps = ((long long)N + 31) / 32, ctas = (warps + 7) / 8;       // the survivor count lives on the device: grid-stride over its iterations
+  const int blocks = (int)(ctas < 8LL * num_sms ? ctas : 8LL * num_sms);
+  row_ballot_kernel<<<blocks, 256, 0, st>>>(ws.hdr, ws.sorted_ys, vp.tiles_y, ws.rb_stride, ws.row_ballots);
+  count_launch();
+}
+
 void launch_row_scatter(const Workspace& ws, int N, const ViewParams& vp, int num_sms, cudaStream_t st) {
   if (N <= 0) return;
   const int xblocks = (vp.tiles_x + RS_XB - 1) / RS_XB;
   // the survivor count lives on the device: persistent CTAs take (chunk, row, column block) items from a ticket
   const unsigned long long items = (unsigned long long)ws.rs_chunks * (unsigned int)vp.tiles_y * xblocks;
   const unsigned int blocks = (unsigned int)(items < 8ull * num_sms ? items : 8ull * num_sms);
-  row_scatter_kernel<<<blocks, RS_THREADS, 0, st>>>(ws.hdr, ws.sorted_ys, ws.sorted_xs, ws.sorted_ids, ws.ranges, ws.rs_state, vp.tiles_x, vp.tiles_y,
+  row_scatter_kernel<<<blocks, RS_THREADS, 0, st>>>(ws.hdr, ws.row_ballots, ws.rb_stride, ws.sorted_xs, ws.sorted_ids, ws.ranges, ws.rs_state, vp.tiles_x, vp.tiles_y,
                                                     xblocks, ws.rs_chunk, ws.pair_ids);
   count_launch();
 }
