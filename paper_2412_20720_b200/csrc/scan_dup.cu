@@ -1,9 +1,6 @@
 // scan_dup.cu — A5/A6/A7b/A8 for sm_100a: compaction scan (+ depth digit counts) with the tile-grid prefix (ranges, D) as a
 // role of its first CTA, and the row scatter that writes the per-tile lists in depth order without sorting the pairs.
 #include "common.cuh"
-#ifndef FDGS_RS_COLWALK
-#define FDGS_RS_COLWALK 1
-#endif
 
 namespace fdgs {
 
@@ -248,9 +245,7 @@ __global__ void __launch_bounds__(RS_THREADS, 6) row_scatter_kernel(WsHeader* hd
                                                                  const int xblocks, const unsigned int chunk, unsigned int* __restrict__ pair_ids) {
   __shared__ unsigned int mask[RS_WORDS][RS_XB], pref[RS_WORDS][RS_XB];
   __shared__ unsigned int list_j[RS_LC], list_x[RS_LC];
-#if FDGS_RS_COLWALK
-  __shared__ unsigned int list_id[RS_LC];
-#endif
+
   __shared__ unsigned int bal_s[RS_MAX_ITERS];
   __shared__ unsigned short off[RS_MAX_ITERS + 2];     // exclusive prefix of the hit counts: <= RS_MAX_CHUNK = 32768
   __shared__ int diff[RS_XB + 1];
@@ -318,9 +313,6 @@ __global__ void __launch_bounds__(RS_THREADS, 6) row_scatter_kernel(WsHeader* hd
       const unsigned int m = H > r0 ? min((unsigned int)RS_LC, H - r0) : 0u;
       for (unsigned int hl = threadIdx.x; hl < m; hl += RS_THREADS) {
         const unsigned int xw = xs[list_j[hl]];
-#if FDGS_RS_COLWALK
-        list_id[hl] = ids[list_j[hl]];
-#endif
         const int xa = min(max((int)(xw & 0xffffu) - xbase, 0), nx);           // clamped to the column block; a hit that lies in another
         const unsigned int x0 = (unsigned int)xa, x1 = (unsigned int)max(min((int)(xw >> 16) - xbase, nx), xa);   // block keeps an empty interval
         list_x[hl] = x0 | (x1 << 16);
@@ -385,31 +377,10 @@ __global__ void __launch_bounds__(RS_THREADS, 6) row_scatter_kernel(WsHeader* hd
       }
       __syncthreads();
       // 2d. ids to their final positions
-#if FDGS_RS_COLWALK
-      // by tile column: thread (x, part) walks the set bits of its share of the column's mask words in order — the position of a
-      // hit in the tile's list is then a running counter (no per-pair popcount, and neighbouring columns hold similar numbers
-      // of hits, where the hits of a warp cover intervals of very different lengths)
-      {
-        const int parts = RS_THREADS / nx > RS_WORDS ? RS_WORDS : RS_THREADS / nx;      // >= 2: nx <= RS_XB = RS_THREADS / 2
-        const int x = threadIdx.x % nx, part = threadIdx.x / nx;
-        if (part < parts) {
-          const int k0 = part * RS_WORDS / parts, k1 = (part + 1) * RS_WORDS / parts;
-          for (int k = k0; k < k1; ++k) {
-            unsigned int mk = mask[k][x], pos = pref[k][x];
-            while (mk) {
-              const int bit = __ffs(mk) - 1;
-              mk &= mk - 1;
-              pair_ids[pos++] = list_id[32 * k + bit];
-            }
-          }
-        }
-      }
-#else
       for (unsigned int hl = threadIdx.x; hl < m; hl += RS_THREADS) {
         const unsigned int id = ids[list_j[hl]], xw = list_x[hl], k = hl >> 5, below = (1u << (hl & 31)) - 1u;
         for (unsigned int x = xw & 0xffffu; x < (xw >> 16); ++x) pair_ids[pref[k][x] + __popc(mask[k][x] & below)] = id;
       }
-#endif
     }
   }
 }
