@@ -245,7 +245,6 @@ __global__ void __launch_bounds__(RS_THREADS, 6) row_scatter_kernel(WsHeader* hd
                                                                  const int xblocks, const unsigned int chunk, unsigned int* __restrict__ pair_ids) {
   __shared__ unsigned int mask[RS_WORDS][RS_XB], pref[RS_WORDS][RS_XB];
   __shared__ unsigned int list_j[RS_LC], list_x[RS_LC];
-
   __shared__ unsigned int bal_s[RS_MAX_ITERS];
   __shared__ unsigned short off[RS_MAX_ITERS + 2];     // exclusive prefix of the hit counts: <= RS_MAX_CHUNK = 32768
   __shared__ int diff[RS_XB + 1];
